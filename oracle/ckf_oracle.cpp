@@ -1,0 +1,927 @@
+// ckf_oracle.cpp — TEST INFRASTRUCTURE, NOT THE PRODUCT.
+//
+// A plain, slow, double-precision CPU implementation of combinatorial-Kalman-filter (CKF) track
+// finding, written from the paper (arxiv 2505.22822, §2) and the
+// textbook mathematics of the works it cites (refs [7],[8],[12]-[18]), following the
+// step-by-step rules of SURVEY.md §8(c) (U, G, F, P1-P6, J1-J5, N1-N6, V1-V5, R9-R11, T) in that
+// order and notation.  One seed at a time, std::vector + loops, dense 8x8 / 6x6 algebra, no blocking,
+// no SIMD, no code shared with the CUDA path (paper_2505_22822_b200/csrc/).  Only tests/,
+// __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference legs may load it.
+//
+// Build: g++ -O2 -std=c++17 -ffp-contract=off -fPIC -shared -pthread (oracle/build.py).
+//
+// Pins (tests/test_oracle_pins.py): analytic helix (P2-P5), finite-difference Jacobian (J1-J5),
+// closed-form scalar gain + information-form identity (V1-V3), Highland values (V5), multilinear field
+// (F), brute-force module sequence (N2-N5), brute-force CKF enumeration on a toy (R9-R11).
+// Parity unpinned (convention only, fixed by DESIGN.md): the order in which the per-seed cap R10 cuts,
+// hole-only-when-nothing-passes (A5), outward-only navigation (A7), inclusive in-bounds edges (A10),
+// min_measurements = 3 (A14).
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <algorithm>
+#include <thread>
+#include <vector>
+
+namespace {
+
+constexpr double KAPPA = 2.99792458e-4;  // GeV / (T mm)   (U)
+constexpr double PI = 3.14159265358979323846;
+
+// ---------------------------------------------------------------------------------- inputs (POD)
+struct OGeometry {
+  int32_t n_layers;
+  const double* layer_r;
+  const double* layer_half_z;
+  const int32_t* n_phi;
+  const int32_t* n_z;
+  const int32_t* module_offset;  // [n_layers+1]
+  int32_t n_modules;
+  const double* center;  // [M][3]
+  const double* axis_u;  // [M][3]
+  const double* axis_v;  // [M][3]
+  const double* half_u;
+  const double* half_v;
+  const double* x_over_x0;
+};
+
+struct OField {
+  int32_t kind;  // 0 uniform, 1 grid
+  double uniform_b[3];
+  int32_t n[3];
+  double origin[3];
+  double spacing[3];
+  const float* grid;  // [n0][n1][n2][3]
+};
+
+struct OConfig {
+  double chi2_max;
+  int32_t max_branches_per_surface;
+  int32_t max_candidates_per_seed;
+  int32_t max_holes;
+  int32_t min_measurements;
+  double rk_tolerance_mm;
+  double surface_tolerance_mm;
+  double h_max_mm;
+  double particle_mass_gev;
+  int32_t max_rk_steps_per_surface;
+  int32_t max_levels;
+};
+
+enum StopReason { STOP_NONE = 0, STOP_EXIT = 1, STOP_HOLES = 2, STOP_NOT_OUTGOING = 3, STOP_STEP_LIMIT = 4,
+                  STOP_NUMERIC = 5, STOP_LEVEL_LIMIT = 6 };
+
+struct Counters {
+  long long visits = 0, rk_trials = 0, rk_accepted = 0, gate_tests = 0, updates = 0, tips = 0;
+};
+
+// ---------------------------------------------------------------------------------- small algebra
+inline void cross(const double a[3], const double b[3], double o[3]) {
+  o[0] = a[1] * b[2] - a[2] * b[1];
+  o[1] = a[2] * b[0] - a[0] * b[2];
+  o[2] = a[0] * b[1] - a[1] * b[0];
+}
+inline double dot(const double a[3], const double b[3]) { return a[0] * b[0] + a[1] * b[1] + a[2] * b[2]; }
+
+// M(B) v := v x B  as a 3x3 matrix acting on v  (J2)
+inline void cross_matrix(const double B[3], double M[3][3]) {
+  M[0][0] = 0.0;   M[0][1] = B[2];  M[0][2] = -B[1];
+  M[1][0] = -B[2]; M[1][1] = 0.0;   M[1][2] = B[0];
+  M[2][0] = B[1];  M[2][1] = -B[0]; M[2][2] = 0.0;
+}
+inline void mat3_mul(const double A[3][3], const double B[3][3], double O[3][3]) {
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) {
+      double s = 0.0;
+      for (int k = 0; k < 3; ++k) s += A[i][k] * B[k][j];
+      O[i][j] = s;
+    }
+}
+
+// ---------------------------------------------------------------------------------- F: field
+// Trilinear read of the float32 grid; lerp along x, then y, then z, each as a + f (b - a).
+void field_at(const OField& f, const double r[3], double B[3]) {
+  if (f.kind == 0) {
+    B[0] = f.uniform_b[0]; B[1] = f.uniform_b[1]; B[2] = f.uniform_b[2];
+    return;
+  }
+  int idx[3];
+  double fr[3];
+  for (int a = 0; a < 3; ++a) {
+    double g = (r[a] - f.origin[a]) / f.spacing[a];
+    double fl = std::floor(g);
+    int i = (int)fl;
+    if (i < 0) i = 0;
+    if (i > f.n[a] - 2) i = f.n[a] - 2;
+    idx[a] = i;
+    fr[a] = g - (double)i;
+  }
+  const long long s0 = (long long)f.n[1] * f.n[2] * 3, s1 = (long long)f.n[2] * 3, s2 = 3;
+  const float* p = f.grid + idx[0] * s0 + idx[1] * s1 + idx[2] * s2;
+  for (int c = 0; c < 3; ++c) {
+    double v000 = p[c], v100 = p[s0 + c], v010 = p[s1 + c], v110 = p[s0 + s1 + c];
+    double v001 = p[s2 + c], v101 = p[s0 + s2 + c], v011 = p[s1 + s2 + c], v111 = p[s0 + s1 + s2 + c];
+    double x00 = v000 + fr[0] * (v100 - v000);
+    double x10 = v010 + fr[0] * (v110 - v010);
+    double x01 = v001 + fr[0] * (v101 - v001);
+    double x11 = v011 + fr[0] * (v111 - v011);
+    double y0 = x00 + fr[1] * (x10 - x00);
+    double y1 = x01 + fr[1] * (x11 - x01);
+    B[c] = y0 + fr[2] * (y1 - y0);
+  }
+}
+
+// ---------------------------------------------------------------------------------- free state + transport Jacobian
+// Free vector y = (r[0..2], t, d[0..2], q/p)  (U);  D = d y / d y_departure (8x8, J3)
+struct FreeState {
+  double r[3], t, d[3], qop;
+  double D[8][8];
+  double h_ctrl;   // P3/P4: step-size proposal carried between steps
+  int n_steps;     // attempted RKN4 steps since the tip left its module (P6)
+};
+
+void set_identity8(double D[8][8]) {
+  for (int i = 0; i < 8; ++i)
+    for (int j = 0; j < 8; ++j) D[i][j] = (i == j) ? 1.0 : 0.0;
+}
+
+// D <- Dstep * D
+void apply_step_jacobian(double D[8][8], const double Ds[8][8]) {
+  double O[8][8];
+  for (int i = 0; i < 8; ++i)
+    for (int j = 0; j < 8; ++j) {
+      double s = 0.0;
+      for (int k = 0; k < 8; ++k) s += Ds[i][k] * D[k][j];
+      O[i][j] = s;
+    }
+  std::memcpy(D, O, sizeof(O));
+}
+
+inline double inv_beta(double qop, double mass) { return std::sqrt(1.0 + mass * mass * qop * qop); }
+inline double dinvbeta_dqop(double qop, double mass) {
+  return mass * mass * qop / std::sqrt(1.0 + mass * mass * qop * qop);
+}
+
+// P2 + P3 + J2: one RKN4 trial of signed length h.  Returns the error estimate eps; on request applies it.
+struct Trial {
+  double k1[3], k2[3], k3[3], k4[3], B1[3], B2[3], B4[3];
+  double eps;
+};
+
+void rk_trial(const OField& fld, const FreeState& y, double h, Trial& T) {
+  const double lam = KAPPA * y.qop;
+  double tmp[3], dd[3], rm[3], re[3];
+  field_at(fld, y.r, T.B1);
+  cross(y.d, T.B1, tmp);
+  for (int i = 0; i < 3; ++i) T.k1[i] = lam * tmp[i];
+  for (int i = 0; i < 3; ++i) rm[i] = y.r[i] + 0.5 * h * y.d[i] + h * h / 8.0 * T.k1[i];
+  field_at(fld, rm, T.B2);
+  for (int i = 0; i < 3; ++i) dd[i] = y.d[i] + 0.5 * h * T.k1[i];
+  cross(dd, T.B2, tmp);
+  for (int i = 0; i < 3; ++i) T.k2[i] = lam * tmp[i];
+  for (int i = 0; i < 3; ++i) dd[i] = y.d[i] + 0.5 * h * T.k2[i];
+  cross(dd, T.B2, tmp);
+  for (int i = 0; i < 3; ++i) T.k3[i] = lam * tmp[i];
+  for (int i = 0; i < 3; ++i) re[i] = y.r[i] + h * y.d[i] + h * h / 2.0 * T.k3[i];
+  field_at(fld, re, T.B4);
+  for (int i = 0; i < 3; ++i) dd[i] = y.d[i] + h * T.k3[i];
+  cross(dd, T.B4, tmp);
+  for (int i = 0; i < 3; ++i) T.k4[i] = lam * tmp[i];
+  double e2 = 0.0;
+  for (int i = 0; i < 3; ++i) {
+    double e = T.k1[i] - T.k2[i] - T.k3[i] + T.k4[i];
+    e2 += e * e;
+  }
+  T.eps = h * h * std::sqrt(e2);
+}
+
+void rk_accept(FreeState& y, double h, const Trial& T, double mass) {
+  const double lam = KAPPA * y.qop;
+  // ---- J2: step Jacobian, field gradient neglected, h fixed
+  double M1[3][3], M2[3][3], M4[3][3], A1[3][3], A2[3][3], A3[3][3], A4[3][3], W[3][3], X[3][3];
+  double a1[3], a2[3], a3[3], a4[3], dd[3], t1[3], t2[3];
+  cross_matrix(T.B1, M1);
+  cross_matrix(T.B2, M2);
+  cross_matrix(T.B4, M4);
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) A1[i][j] = lam * M1[i][j];
+  cross(y.d, T.B1, a1);
+  // A2 = lam M(B2) (I + h/2 A1);  a2 = (d + h/2 k1) x B2 + lam (h/2 a1) x B2
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) W[i][j] = (i == j ? 1.0 : 0.0) + 0.5 * h * A1[i][j];
+  mat3_mul(M2, W, X);
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) A2[i][j] = lam * X[i][j];
+  for (int i = 0; i < 3; ++i) dd[i] = y.d[i] + 0.5 * h * T.k1[i];
+  cross(dd, T.B2, t1);
+  for (int i = 0; i < 3; ++i) dd[i] = 0.5 * h * a1[i];
+  cross(dd, T.B2, t2);
+  for (int i = 0; i < 3; ++i) a2[i] = t1[i] + lam * t2[i];
+  // A3 from k2 (same B2)
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) W[i][j] = (i == j ? 1.0 : 0.0) + 0.5 * h * A2[i][j];
+  mat3_mul(M2, W, X);
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) A3[i][j] = lam * X[i][j];
+  for (int i = 0; i < 3; ++i) dd[i] = y.d[i] + 0.5 * h * T.k2[i];
+  cross(dd, T.B2, t1);
+  for (int i = 0; i < 3; ++i) dd[i] = 0.5 * h * a2[i];
+  cross(dd, T.B2, t2);
+  for (int i = 0; i < 3; ++i) a3[i] = t1[i] + lam * t2[i];
+  // A4 from k3 with h and B4
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) W[i][j] = (i == j ? 1.0 : 0.0) + h * A3[i][j];
+  mat3_mul(M4, W, X);
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) A4[i][j] = lam * X[i][j];
+  for (int i = 0; i < 3; ++i) dd[i] = y.d[i] + h * T.k3[i];
+  cross(dd, T.B4, t1);
+  for (int i = 0; i < 3; ++i) dd[i] = h * a3[i];
+  cross(dd, T.B4, t2);
+  for (int i = 0; i < 3; ++i) a4[i] = t1[i] + lam * t2[i];
+
+  double Ds[8][8];
+  set_identity8(Ds);
+  for (int i = 0; i < 3; ++i) {
+    for (int j = 0; j < 3; ++j) {
+      Ds[i][4 + j] = (i == j ? h : 0.0) + h * h / 6.0 * (A1[i][j] + A2[i][j] + A3[i][j]);
+      Ds[4 + i][4 + j] = (i == j ? 1.0 : 0.0) + h / 6.0 * (A1[i][j] + 2.0 * A2[i][j] + 2.0 * A3[i][j] + A4[i][j]);
+    }
+    Ds[i][7] = KAPPA * (h * h / 6.0 * (a1[i] + a2[i] + a3[i]));
+    Ds[4 + i][7] = KAPPA * (h / 6.0 * (a1[i] + 2.0 * a2[i] + 2.0 * a3[i] + a4[i]));
+  }
+  Ds[3][7] = h * dinvbeta_dqop(y.qop, mass);
+  apply_step_jacobian(y.D, Ds);
+
+  // ---- P2: the state
+  double dn[3], nrm2 = 0.0;
+  for (int i = 0; i < 3; ++i) {
+    y.r[i] = y.r[i] + h * y.d[i] + h * h / 6.0 * (T.k1[i] + T.k2[i] + T.k3[i]);
+    dn[i] = y.d[i] + h / 6.0 * (T.k1[i] + 2.0 * T.k2[i] + 2.0 * T.k3[i] + T.k4[i]);
+    nrm2 += dn[i] * dn[i];
+  }
+  const double nrm = std::sqrt(nrm2);
+  for (int i = 0; i < 3; ++i) y.d[i] = dn[i] / nrm;
+  y.t += h * inv_beta(y.qop, mass);
+}
+
+// P5: field-free closing step of length s
+void straight_close(FreeState& y, double s, double mass) {
+  double Ds[8][8];
+  set_identity8(Ds);
+  for (int i = 0; i < 3; ++i) Ds[i][4 + i] = s;
+  Ds[3][7] = s * dinvbeta_dqop(y.qop, mass);
+  apply_step_jacobian(y.D, Ds);
+  for (int i = 0; i < 3; ++i) y.r[i] += s * y.d[i];
+  y.t += s * inv_beta(y.qop, mass);
+}
+
+struct Target {
+  int kind;      // 0 plane (c, n), 1 cylinder radius R around z
+  double c[3], n[3], R;
+};
+
+// P4: signed straight-line distance to the target along d.  Returns false if unreachable (P6).
+bool target_distance(const Target& tg, const FreeState& y, double& s, int& why) {
+  if (tg.kind == 0) {
+    double dn = dot(y.d, tg.n);
+    if (!(std::fabs(dn) > 1e-12)) { why = STOP_NUMERIC; return false; }
+    double rel[3] = {tg.c[0] - y.r[0], tg.c[1] - y.r[1], tg.c[2] - y.r[2]};
+    s = dot(rel, tg.n) / dn;
+    return true;
+  }
+  const double a = y.d[0] * y.d[0] + y.d[1] * y.d[1];
+  const double b = y.r[0] * y.d[0] + y.r[1] * y.d[1];
+  const double cc = y.r[0] * y.r[0] + y.r[1] * y.r[1] - tg.R * tg.R;
+  const double disc = b * b - a * cc;
+  if (!(b > 0.0) || !(disc >= 0.0)) { why = STOP_NOT_OUTGOING; return false; }
+  s = -cc / (b + std::sqrt(disc));
+  return true;
+}
+
+// P3-P6: step until the target is reached.  Returns STOP_NONE on success.
+int propagate_to(const OField& fld, const OConfig& cfg, const Target& tg, FreeState& y, Counters& cnt) {
+  const double mass = cfg.particle_mass_gev;
+  for (;;) {
+    double s;
+    int why = STOP_NUMERIC;
+    if (!target_distance(tg, y, s, why)) return why;
+    if (!std::isfinite(s)) return STOP_NUMERIC;
+    if (std::fabs(s) <= cfg.surface_tolerance_mm) {
+      straight_close(y, s, mass);
+      return STOP_NONE;
+    }
+    const double hlim = std::min(y.h_ctrl, cfg.h_max_mm);
+    double h = (std::fabs(s) <= hlim) ? s : (s > 0.0 ? hlim : -hlim);
+    for (;;) {
+      if (++y.n_steps > cfg.max_rk_steps_per_surface) return STOP_STEP_LIMIT;
+      Trial T;
+      rk_trial(fld, y, h, T);
+      ++cnt.rk_trials;
+      if (!std::isfinite(T.eps)) return STOP_NUMERIC;
+      double f;
+      if (T.eps == 0.0) f = 4.0;
+      else {
+        f = 0.9 * std::sqrt(std::sqrt(cfg.rk_tolerance_mm / T.eps));
+        if (f < 0.25) f = 0.25;
+        if (f > 4.0) f = 4.0;
+      }
+      if (T.eps <= cfg.rk_tolerance_mm) {
+        rk_accept(y, h, T, mass);
+        y.h_ctrl = std::fabs(h) * f;
+        ++cnt.rk_accepted;
+        break;
+      }
+      h = h * f;
+    }
+  }
+}
+
+// ---------------------------------------------------------------------------------- bound <-> free
+struct Module {
+  int id, layer, iphi, iz;
+  double c[3], u[3], v[3], n[3], half_u, half_v, x_over_x0;
+};
+
+Module get_module(const OGeometry& g, int id) {
+  Module m;
+  m.id = id;
+  int l = 0;
+  while (l + 1 < g.n_layers && id >= g.module_offset[l + 1]) ++l;
+  m.layer = l;
+  int loc = id - g.module_offset[l];
+  m.iphi = loc / g.n_z[l];
+  m.iz = loc % g.n_z[l];
+  for (int i = 0; i < 3; ++i) {
+    m.c[i] = g.center[3 * id + i];
+    m.u[i] = g.axis_u[3 * id + i];
+    m.v[i] = g.axis_v[3 * id + i];
+  }
+  cross(m.u, m.v, m.n);
+  m.half_u = g.half_u[id];
+  m.half_v = g.half_v[id];
+  m.x_over_x0 = g.x_over_x0[id];
+  return m;
+}
+
+// bound x = (l0, l1, phi, theta, q/p, t)
+void bound_to_free(const Module& m, const double x[6], FreeState& y, double B2F[8][6]) {
+  const double sp = std::sin(x[2]), cp = std::cos(x[2]), st = std::sin(x[3]), ct = std::cos(x[3]);
+  for (int i = 0; i < 3; ++i) y.r[i] = m.c[i] + x[0] * m.u[i] + x[1] * m.v[i];
+  y.t = x[5];
+  y.d[0] = st * cp; y.d[1] = st * sp; y.d[2] = ct;
+  y.qop = x[4];
+  // J1
+  for (int i = 0; i < 8; ++i)
+    for (int j = 0; j < 6; ++j) B2F[i][j] = 0.0;
+  for (int i = 0; i < 3; ++i) { B2F[i][0] = m.u[i]; B2F[i][1] = m.v[i]; }
+  B2F[3][5] = 1.0;
+  B2F[4][2] = -st * sp; B2F[5][2] = st * cp;  B2F[6][2] = 0.0;
+  B2F[4][3] = ct * cp;  B2F[5][3] = ct * sp;  B2F[6][3] = -st;
+  B2F[7][4] = 1.0;
+}
+
+// J4 + J5: arrival on plane of module m; outputs bound x', J (6x6) given B2F of the departure
+void arrive(const OField& fld, const OConfig& cfg, const Module& m, const FreeState& y, const double B2F[8][6],
+            double xo[6], double J[6][6]) {
+  const double mass = cfg.particle_mass_gev;
+  const double lam = KAPPA * y.qop;
+  double B[3], dxB[3];
+  field_at(fld, y.r, B);
+  cross(y.d, B, dxB);
+  // y' = (d, 1/beta, lam d x B, 0)
+  double yp[8] = {y.d[0], y.d[1], y.d[2], inv_beta(y.qop, mass), lam * dxB[0], lam * dxB[1], lam * dxB[2], 0.0};
+  const double nd = dot(m.n, y.d);
+  // P = I - y' w^T / (n.d),  w = (n, 0, 0, 0, 0, 0)
+  double P[8][8];
+  set_identity8(P);
+  for (int i = 0; i < 8; ++i)
+    for (int j = 0; j < 3; ++j) P[i][j] -= yp[i] * m.n[j] / nd;
+  // bound parameters on arrival (J5)
+  double rel[3] = {y.r[0] - m.c[0], y.r[1] - m.c[1], y.r[2] - m.c[2]};
+  const double phi = std::atan2(y.d[1], y.d[0]);
+  const double theta = std::atan2(std::hypot(y.d[0], y.d[1]), y.d[2]);
+  xo[0] = dot(rel, m.u); xo[1] = dot(rel, m.v); xo[2] = phi; xo[3] = theta; xo[4] = y.qop; xo[5] = y.t;
+  const double sp = std::sin(phi), cp = std::cos(phi), st = std::sin(theta), ct = std::cos(theta);
+  double F2B[6][8];
+  for (int i = 0; i < 6; ++i)
+    for (int j = 0; j < 8; ++j) F2B[i][j] = 0.0;
+  for (int j = 0; j < 3; ++j) { F2B[0][j] = m.u[j]; F2B[1][j] = m.v[j]; }
+  F2B[2][4] = -sp / st; F2B[2][5] = cp / st; F2B[2][6] = 0.0;
+  F2B[3][4] = ct * cp;  F2B[3][5] = ct * sp; F2B[3][6] = -st;
+  F2B[4][7] = 1.0;
+  F2B[5][3] = 1.0;
+  // J = F2B P D B2F
+  double PD[8][8], PDB[8][6];
+  for (int i = 0; i < 8; ++i)
+    for (int j = 0; j < 8; ++j) {
+      double s = 0.0;
+      for (int k = 0; k < 8; ++k) s += P[i][k] * y.D[k][j];
+      PD[i][j] = s;
+    }
+  for (int i = 0; i < 8; ++i)
+    for (int j = 0; j < 6; ++j) {
+      double s = 0.0;
+      for (int k = 0; k < 8; ++k) s += PD[i][k] * B2F[k][j];
+      PDB[i][j] = s;
+    }
+  for (int i = 0; i < 6; ++i)
+    for (int j = 0; j < 6; ++j) {
+      double s = 0.0;
+      for (int k = 0; k < 8; ++k) s += F2B[i][k] * PDB[k][j];
+      J[i][j] = s;
+    }
+}
+
+void transport_cov(const double J[6][6], const double C[6][6], double Co[6][6]) {
+  double JC[6][6], T[6][6];
+  for (int i = 0; i < 6; ++i)
+    for (int j = 0; j < 6; ++j) {
+      double s = 0.0;
+      for (int k = 0; k < 6; ++k) s += J[i][k] * C[k][j];
+      JC[i][j] = s;
+    }
+  for (int i = 0; i < 6; ++i)
+    for (int j = 0; j < 6; ++j) {
+      double s = 0.0;
+      for (int k = 0; k < 6; ++k) s += JC[i][k] * J[j][k];
+      T[i][j] = s;
+    }
+  for (int i = 0; i < 6; ++i)
+    for (int j = 0; j < 6; ++j) Co[i][j] = 0.5 * (T[i][j] + T[j][i]);
+}
+
+// ---------------------------------------------------------------------------------- V5: Highland
+double highland_theta0(double p, double x_eff, double mass) {
+  const double beta = p / std::sqrt(p * p + mass * mass);
+  return 0.0136 / (beta * p) * std::sqrt(x_eff) * (1.0 + 0.038 * std::log(x_eff / (beta * beta)));
+}
+
+void add_material(const OConfig& cfg, const Module& m, const double x[6], double C[6][6]) {
+  if (!(m.x_over_x0 > 0.0)) return;
+  const double st = std::sin(x[3]), ct = std::cos(x[3]);
+  const double d[3] = {st * std::cos(x[2]), st * std::sin(x[2]), ct};
+  const double cosi = std::fabs(dot(d, m.n));
+  const double p = 1.0 / std::fabs(x[4]);
+  const double th0 = highland_theta0(p, m.x_over_x0 / cosi, cfg.particle_mass_gev);
+  C[3][3] += th0 * th0;
+  C[2][2] += th0 * th0 / (st * st);
+}
+
+// ---------------------------------------------------------------------------------- N: navigation
+// straight-line test of one module from the point (r, d): N2 / N4
+bool line_hits_module(const Module& k, const double r[3], const double d[3], double s_min, double& s_out) {
+  const double dn = dot(d, k.n);
+  if (dn <= 1e-6) return false;
+  double rel[3] = {k.c[0] - r[0], k.c[1] - r[1], k.c[2] - r[2]};
+  const double s = dot(rel, k.n) / dn;
+  double q[3] = {r[0] + s * d[0] - k.c[0], r[1] + s * d[1] - k.c[1], r[2] + s * d[2] - k.c[2]};
+  if (!(std::fabs(dot(q, k.u)) <= k.half_u)) return false;
+  if (!(std::fabs(dot(q, k.v)) <= k.half_v)) return false;
+  if (!(s > s_min)) return false;
+  s_out = s;
+  return true;
+}
+
+// nearest in-bounds module among the 3x3 neighbourhood of (iphi, iz) on `layer`, excluding `exclude`
+int pick_in_neighbourhood(const OGeometry& g, int layer, int iphi, int iz, int exclude, const double r[3],
+                          const double d[3], double s_min) {
+  int best = -1;
+  double best_s = 0.0;
+  const int nphi = g.n_phi[layer], nz = g.n_z[layer];
+  for (int di = -1; di <= 1; ++di)
+    for (int dj = -1; dj <= 1; ++dj) {
+      const int jj = iz + dj;
+      if (jj < 0 || jj >= nz) continue;
+      const int ii = ((iphi + di) % nphi + nphi) % nphi;
+      const int id = g.module_offset[layer] + ii * nz + jj;
+      if (id == exclude) continue;
+      Module k = get_module(g, id);
+      double s;
+      if (!line_hits_module(k, r, d, s_min, s)) continue;
+      if (best < 0 || s < best_s || (s == best_s && id < best)) { best = id; best_s = s; }
+    }
+  return best;
+}
+
+// One surface-to-surface move (N1-N5 + P + J): from bound (x, C) on module `from` to the next module.
+// Material (V5) is added to C on leaving.  Returns STOP_NONE and (target, xp, Cp), or the stop reason.
+int move_to_next_module(const OGeometry& g, const OField& fld, const OConfig& cfg, int from, const double x[6],
+                        const double Cin[6][6], int& target, double xp[6], double Cp[6][6], double Jout[6][6],
+                        Counters& cnt) {
+  for (int i = 0; i < 6; ++i)
+    if (!std::isfinite(x[i])) return STOP_NUMERIC;
+  if (!(x[3] > 0.0 && x[3] < PI)) return STOP_NUMERIC;
+  const Module m = get_module(g, from);
+  double C[6][6];
+  std::memcpy(C, Cin, sizeof(C));
+  add_material(cfg, m, x, C);
+  FreeState y;
+  double B2F[8][6];
+  bound_to_free(m, x, y, B2F);
+  set_identity8(y.D);
+  y.h_ctrl = cfg.h_max_mm;
+  y.n_steps = 0;
+  // N2: overlap neighbour on the same layer
+  int tgt = pick_in_neighbourhood(g, m.layer, m.iphi, m.iz, m.id, y.r, y.d, 1e-3);
+  if (tgt < 0) {
+    // N3: next layer's cylinder, then N4 module choice at the portal
+    int lp = m.layer + 1;
+    for (;;) {
+      if (lp >= g.n_layers) return STOP_EXIT;
+      Target cyl;
+      cyl.kind = 1;
+      cyl.R = g.layer_r[lp];
+      int st = propagate_to(fld, cfg, cyl, y, cnt);
+      if (st != STOP_NONE) return st;
+      if (std::fabs(y.r[2]) > g.layer_half_z[lp]) { ++lp; continue; }
+      const int nphi = g.n_phi[lp], nz = g.n_z[lp];
+      const double len = 2.0 * g.half_v[g.module_offset[lp]];
+      const double phix = std::atan2(y.r[1], y.r[0]);
+      int i = (int)std::nearbyint(phix * nphi / (2.0 * PI));
+      i = ((i % nphi) + nphi) % nphi;
+      int j = (int)std::floor((y.r[2] + g.layer_half_z[lp]) / len);
+      if (j < 0) j = 0;
+      if (j > nz - 1) j = nz - 1;
+      tgt = pick_in_neighbourhood(g, lp, i, j, -1, y.r, y.d, -1e-3);
+      if (tgt >= 0) break;
+      ++lp;  // a crack is not a hole
+    }
+  }
+  // N5: to the target's plane
+  const Module k = get_module(g, tgt);
+  Target pl;
+  pl.kind = 0;
+  for (int i = 0; i < 3; ++i) { pl.c[i] = k.c[i]; pl.n[i] = k.n[i]; }
+  int st = propagate_to(fld, cfg, pl, y, cnt);
+  if (st != STOP_NONE) return st;
+  double J[6][6];
+  arrive(fld, cfg, k, y, B2F, xp, J);
+  transport_cov(J, C, Cp);
+  for (int i = 0; i < 6; ++i) {
+    if (!std::isfinite(xp[i])) return STOP_NUMERIC;
+    for (int j = 0; j < 6; ++j) {
+      if (Jout) Jout[i][j] = J[i][j];
+      if (!std::isfinite(Cp[i][j])) return STOP_NUMERIC;
+    }
+  }
+  target = tgt;
+  return STOP_NONE;
+}
+
+// ---------------------------------------------------------------------------------- V: visit
+// V1: chi2 of measurement (loc, var) against predicted (x, C)
+double predicted_chi2(const double x[6], const double C[6][6], const double loc[2], const double var[2]) {
+  const double r0 = loc[0] - x[0], r1 = loc[1] - x[1];
+  const double S00 = C[0][0] + var[0], S01 = C[0][1], S11 = C[1][1] + var[1];
+  const double det = S00 * S11 - S01 * S01;
+  return (r0 * r0 * S11 - 2.0 * r0 * r1 * S01 + r1 * r1 * S00) / det;
+}
+
+// V3: gain-form update, upper triangle mirrored, phi wrapped to (-pi, pi]
+void kalman_update(const double x[6], const double C[6][6], const double loc[2], const double var[2], double xo[6],
+                   double Co[6][6]) {
+  const double r0 = loc[0] - x[0], r1 = loc[1] - x[1];
+  const double S00 = C[0][0] + var[0], S01 = C[0][1], S11 = C[1][1] + var[1];
+  const double det = S00 * S11 - S01 * S01;
+  const double I00 = S11 / det, I01 = -S01 / det, I11 = S00 / det;
+  double K[6][2];
+  for (int i = 0; i < 6; ++i) {
+    K[i][0] = C[i][0] * I00 + C[i][1] * I01;
+    K[i][1] = C[i][0] * I01 + C[i][1] * I11;
+  }
+  for (int i = 0; i < 6; ++i) xo[i] = x[i] + K[i][0] * r0 + K[i][1] * r1;
+  for (int i = 0; i < 6; ++i)
+    for (int j = i; j < 6; ++j) {
+      const double v = C[i][j] - (K[i][0] * C[0][j] + K[i][1] * C[1][j]);
+      Co[i][j] = v;
+      Co[j][i] = v;
+    }
+  while (xo[2] > PI) xo[2] -= 2.0 * PI;
+  while (xo[2] <= -PI) xo[2] += 2.0 * PI;
+}
+
+// ---------------------------------------------------------------------------------- R: CKF control
+struct Link {
+  int parent;   // index into the seed's link vector, -1 = root
+  int meas;     // measurement index, -1 = hole
+  double chi2;
+};
+
+struct Tip {
+  double x[6], C[6][6];
+  int module;
+  int link;        // last link (-1 before level 0)
+  int n_meas, n_holes;
+  double chi2_sum;
+  // snapshot at the last measurement (V3)
+  double xs[6], Cs[6][6];
+  int module_s;
+};
+
+struct Track {
+  int seed, n_holes, last_module, stop_reason;
+  double x[6], C[6][6], chi2_sum;
+  std::vector<int> meas;
+  std::vector<double> chi2;
+};
+
+struct Sel { double chi2; int idx; };
+
+void run_seed(const OGeometry& g, const OField& fld, const OConfig& cfg, const int32_t* moff, const double* loc,
+              const double* var, int seed, int seed_module, const double* sx, const double* sC,
+              std::vector<Track>& out, Counters& cnt) {
+  std::vector<Link> links;
+  std::vector<Tip> tips(1);
+  {
+    Tip& t = tips[0];
+    for (int i = 0; i < 6; ++i) {
+      t.x[i] = sx[i];
+      for (int j = 0; j < 6; ++j) t.C[i][j] = sC[6 * i + j];
+    }
+    t.module = seed_module; t.link = -1; t.n_meas = 0; t.n_holes = 0; t.chi2_sum = 0.0; t.module_s = -1;
+    std::memset(t.xs, 0, sizeof(t.xs)); std::memset(t.Cs, 0, sizeof(t.Cs));
+  }
+  int finished = 0;
+  auto emit = [&](const Tip& t, int reason) {
+    ++finished;
+    if (t.n_meas < cfg.min_measurements) return;
+    Track tr;
+    tr.seed = seed; tr.n_holes = t.n_holes; tr.last_module = t.module_s; tr.stop_reason = reason;
+    std::memcpy(tr.x, t.xs, sizeof(tr.x)); std::memcpy(tr.C, t.Cs, sizeof(tr.C));
+    tr.chi2_sum = t.chi2_sum;
+    for (int l = t.link; l >= 0; l = links[l].parent)
+      if (links[l].meas >= 0) { tr.meas.push_back(links[l].meas); tr.chi2.push_back(links[l].chi2); }
+    std::reverse(tr.meas.begin(), tr.meas.end());
+    std::reverse(tr.chi2.begin(), tr.chi2.end());
+    out.push_back(std::move(tr));
+  };
+
+  for (int level = 0; !tips.empty(); ++level) {
+    if (level >= cfg.max_levels) {
+      for (const Tip& t : tips) emit(t, STOP_LEVEL_LIMIT);
+      break;
+    }
+    const int n = (int)tips.size();
+    cnt.tips += n;
+    // ---- step A: move every tip to its next module (level 0: N6, the seed's own module, J = I)
+    std::vector<int> stop(n, STOP_NONE), target(n, -1);
+    std::vector<Tip> pred(tips);
+    for (int i = 0; i < n; ++i) {
+      if (level == 0) {
+        const Tip& t = tips[i];
+        bool ok = (t.x[3] > 0.0 && t.x[3] < PI);
+        for (int a = 0; a < 6; ++a) ok = ok && std::isfinite(t.x[a]);
+        if (!ok) stop[i] = STOP_NUMERIC;
+        target[i] = t.module;
+        continue;
+      }
+      int tg = -1;
+      stop[i] = move_to_next_module(g, fld, cfg, tips[i].module, tips[i].x, tips[i].C, tg, pred[i].x, pred[i].C,
+                                    nullptr, cnt);
+      target[i] = tg;
+    }
+    // ---- step B: gate (V1, V2) -> wanted children
+    std::vector<std::vector<Sel>> sel(n);
+    std::vector<int> want(n, 0);
+    for (int i = 0; i < n; ++i) {
+      if (stop[i] != STOP_NONE) continue;
+      ++cnt.visits;
+      const int m = target[i];
+      std::vector<Sel> pass;
+      for (int k = moff[m]; k < moff[m + 1]; ++k) {
+        ++cnt.gate_tests;
+        const double c2 = predicted_chi2(pred[i].x, pred[i].C, loc + 2 * k, var + 2 * k);
+        if (c2 < cfg.chi2_max) pass.push_back({c2, k});
+      }
+      std::stable_sort(pass.begin(), pass.end(), [](const Sel& a, const Sel& b) {
+        return a.chi2 < b.chi2 || (a.chi2 == b.chi2 && a.idx < b.idx);
+      });
+      if ((int)pass.size() > cfg.max_branches_per_surface) pass.resize(cfg.max_branches_per_surface);
+      if (pass.empty()) {
+        // V4: hole
+        if (tips[i].n_holes + 1 > cfg.max_holes) { stop[i] = STOP_HOLES; pred[i].n_holes = tips[i].n_holes + 1; }
+        else want[i] = 1;
+      } else {
+        want[i] = (int)pass.size();
+      }
+      sel[i] = std::move(pass);
+    }
+    // ---- step C: per-seed cap (R10), greedy in tip order
+    const int Rm = cfg.max_candidates_per_seed - (finished + n);
+    long long P = 0;
+    std::vector<int> keep(n, 0);
+    for (int i = 0; i < n; ++i) {
+      if (want[i] < 1) continue;
+      const int e = want[i] - 1;
+      const long long room = std::max<long long>(0, (long long)Rm - P);
+      keep[i] = 1 + (int)std::min<long long>(e, room);
+      P += e;
+    }
+    // ---- step D: finished tips emit (tip order), children are made (V3, V4)
+    std::vector<Tip> next;
+    for (int i = 0; i < n; ++i) {
+      if (stop[i] != STOP_NONE) {
+        Tip t = tips[i];
+        if (stop[i] == STOP_HOLES) t.n_holes = pred[i].n_holes;
+        emit(t, stop[i]);
+        continue;
+      }
+      const int m = target[i];
+      if (sel[i].empty()) {
+        Tip c = pred[i];
+        c.module = m;
+        links.push_back({tips[i].link, -1, 0.0});
+        c.link = (int)links.size() - 1;
+        c.n_holes = tips[i].n_holes + 1;
+        next.push_back(c);
+        continue;
+      }
+      for (int j = 0; j < keep[i]; ++j) {
+        Tip c = pred[i];
+        const int k = sel[i][j].idx;
+        kalman_update(pred[i].x, pred[i].C, loc + 2 * k, var + 2 * k, c.x, c.C);
+        ++cnt.updates;
+        c.module = m;
+        links.push_back({tips[i].link, k, sel[i][j].chi2});
+        c.link = (int)links.size() - 1;
+        c.n_meas = tips[i].n_meas + 1;
+        c.chi2_sum = tips[i].chi2_sum + sel[i][j].chi2;
+        std::memcpy(c.xs, c.x, sizeof(c.x));
+        std::memcpy(c.Cs, c.C, sizeof(c.C));
+        c.module_s = m;
+        next.push_back(c);
+      }
+    }
+    tips.swap(next);
+  }
+}
+
+struct Result {
+  std::vector<Track> tracks;
+  Counters cnt;
+};
+
+}  // namespace
+
+// ====================================================================================== C interface
+extern "C" {
+
+struct oracle_result;
+
+// Runs the CKF over all seeds (static contiguous chunks over n_threads).  All pointers are HOST, double.
+void* oracle_ckf_find(const OGeometry* g, const OField* f, const OConfig* cfg, int32_t n_meas,
+                      const int32_t* module_offsets, const double* loc, const double* var, int32_t n_seeds,
+                      const int32_t* seed_module, const double* seed_params, const double* seed_cov,
+                      int32_t n_threads) {
+  (void)n_meas;
+  if (n_threads < 1) n_threads = 1;
+  if (n_threads > n_seeds) n_threads = std::max(1, n_seeds);
+  std::vector<std::vector<Track>> parts(n_threads);
+  std::vector<Counters> cnts(n_threads);
+  auto work = [&](int t) {
+    const long long lo = (long long)n_seeds * t / n_threads, hi = (long long)n_seeds * (t + 1) / n_threads;
+    for (long long s = lo; s < hi; ++s)
+      run_seed(*g, *f, *cfg, module_offsets, loc, var, (int)s, seed_module[s], seed_params + 6 * s,
+               seed_cov + 36 * s, parts[t], cnts[t]);
+  };
+  if (n_threads == 1) work(0);
+  else {
+    std::vector<std::thread> th;
+    for (int t = 0; t < n_threads; ++t) th.emplace_back(work, t);
+    for (auto& x : th) x.join();
+  }
+  Result* R = new Result();
+  for (int t = 0; t < n_threads; ++t) {
+    for (auto& tr : parts[t]) R->tracks.push_back(std::move(tr));
+    R->cnt.visits += cnts[t].visits; R->cnt.rk_trials += cnts[t].rk_trials;
+    R->cnt.rk_accepted += cnts[t].rk_accepted; R->cnt.gate_tests += cnts[t].gate_tests;
+    R->cnt.updates += cnts[t].updates; R->cnt.tips += cnts[t].tips;
+  }
+  return R;
+}
+
+int32_t oracle_result_n_tracks(const void* r) { return (int32_t)((const Result*)r)->tracks.size(); }
+int64_t oracle_result_n_entries(const void* r) {
+  int64_t n = 0;
+  for (const auto& t : ((const Result*)r)->tracks) n += (int64_t)t.meas.size();
+  return n;
+}
+void oracle_result_counters(const void* r, int64_t out[6]) {
+  const Counters& c = ((const Result*)r)->cnt;
+  out[0] = c.visits; out[1] = c.rk_trials; out[2] = c.rk_accepted; out[3] = c.gate_tests; out[4] = c.updates;
+  out[5] = c.tips;
+}
+void oracle_result_copy(const void* r, int32_t* track_offsets, int32_t* meas_idx, double* entry_chi2, int32_t* seed_id,
+                        int32_t* n_holes, int32_t* last_module, int32_t* stop_reason, double* params, double* cov,
+                        double* chi2_sum) {
+  const Result* R = (const Result*)r;
+  int32_t off = 0;
+  for (size_t t = 0; t < R->tracks.size(); ++t) {
+    const Track& tr = R->tracks[t];
+    track_offsets[t] = off;
+    for (size_t k = 0; k < tr.meas.size(); ++k) { meas_idx[off + k] = tr.meas[k]; entry_chi2[off + k] = tr.chi2[k]; }
+    off += (int32_t)tr.meas.size();
+    seed_id[t] = tr.seed; n_holes[t] = tr.n_holes; last_module[t] = tr.last_module; stop_reason[t] = tr.stop_reason;
+    for (int i = 0; i < 6; ++i) {
+      params[6 * t + i] = tr.x[i];
+      for (int j = 0; j < 6; ++j) cov[36 * t + 6 * i + j] = tr.C[i][j];
+    }
+    chi2_sum[t] = tr.chi2_sum;
+  }
+  track_offsets[R->tracks.size()] = off;
+}
+void oracle_result_free(void* r) { delete (Result*)r; }
+
+// ---- pieces exposed for the pins (tests/test_oracle_pins.py)
+void oracle_field_at(const OField* f, const double r[3], double B[3]) { field_at(*f, r, B); }
+
+// Free-state propagation to a plane (kind 0: c, n) or cylinder (kind 1: R).  y = (r, t, d, q/p) in/out;
+// D (8x8 row-major) out.  Returns stop reason (0 = arrived); n_steps out.
+int32_t oracle_propagate_free(const OField* f, const OConfig* cfg, int32_t kind, const double c[3], const double n[3],
+                              double R, double y[8], double D[64], int32_t* n_steps) {
+  FreeState s;
+  for (int i = 0; i < 3; ++i) { s.r[i] = y[i]; s.d[i] = y[4 + i]; }
+  s.t = y[3]; s.qop = y[7];
+  set_identity8(s.D);
+  s.h_ctrl = cfg->h_max_mm; s.n_steps = 0;
+  Target tg;
+  tg.kind = kind; tg.R = R;
+  for (int i = 0; i < 3; ++i) { tg.c[i] = c ? c[i] : 0.0; tg.n[i] = n ? n[i] : 0.0; }
+  Counters cnt;
+  int st = propagate_to(*f, *cfg, tg, s, cnt);
+  for (int i = 0; i < 3; ++i) { y[i] = s.r[i]; y[4 + i] = s.d[i]; }
+  y[3] = s.t; y[7] = s.qop;
+  if (D) std::memcpy(D, s.D, sizeof(s.D));
+  if (n_steps) *n_steps = s.n_steps;
+  return st;
+}
+
+// One full surface-to-surface move from module `from` (N1-N5, P, J, V5 material on leaving).
+int32_t oracle_move(const OGeometry* g, const OField* f, const OConfig* cfg, int32_t from, const double x[6],
+                    const double C[36], int32_t* target, double xp[6], double Cp[36], double J[36]) {
+  double Ci[6][6], Co[6][6], Jo[6][6];
+  std::memcpy(Ci, C, sizeof(Ci));
+  Counters cnt;
+  int tg = -1;
+  int st = move_to_next_module(*g, *f, *cfg, from, x, Ci, tg, xp, Co, Jo, cnt);
+  *target = tg;
+  if (st == STOP_NONE) {
+    std::memcpy(Cp, Co, sizeof(Co));
+    if (J) std::memcpy(J, Jo, sizeof(Jo));
+  }
+  return st;
+}
+
+// Bound -> bound transport between two given modules, no navigation, no material (for the FD pin of J1-J5).
+int32_t oracle_bound_to_bound(const OGeometry* g, const OField* f, const OConfig* cfg, int32_t from, int32_t to,
+                              const double x[6], double xp[6], double J[36]) {
+  const Module m = get_module(*g, from), k = get_module(*g, to);
+  FreeState y;
+  double B2F[8][6];
+  bound_to_free(m, x, y, B2F);
+  set_identity8(y.D);
+  y.h_ctrl = cfg->h_max_mm; y.n_steps = 0;
+  Target pl;
+  pl.kind = 0;
+  for (int i = 0; i < 3; ++i) { pl.c[i] = k.c[i]; pl.n[i] = k.n[i]; }
+  Counters cnt;
+  int st = propagate_to(*f, *cfg, pl, y, cnt);
+  if (st != STOP_NONE) return st;
+  double Jo[6][6];
+  arrive(*f, *cfg, k, y, B2F, xp, Jo);
+  if (J) std::memcpy(J, Jo, sizeof(Jo));
+  return 0;
+}
+
+void oracle_transport_cov(const double J[36], const double C[36], double Co[36]) {
+  double Jm[6][6], Cm[6][6], O[6][6];
+  std::memcpy(Jm, J, sizeof(Jm)); std::memcpy(Cm, C, sizeof(Cm));
+  transport_cov(Jm, Cm, O);
+  std::memcpy(Co, O, sizeof(O));
+}
+
+double oracle_predicted_chi2(const double x[6], const double C[36], const double loc[2], const double var[2]) {
+  double Cm[6][6];
+  std::memcpy(Cm, C, sizeof(Cm));
+  return predicted_chi2(x, Cm, loc, var);
+}
+
+void oracle_kalman_update(const double x[6], const double C[36], const double loc[2], const double var[2],
+                          double xo[6], double Co[36]) {
+  double Cm[6][6], O[6][6];
+  std::memcpy(Cm, C, sizeof(Cm));
+  kalman_update(x, Cm, loc, var, xo, O);
+  std::memcpy(Co, O, sizeof(O));
+}
+
+double oracle_highland_theta0(double p, double x_eff, double mass) { return highland_theta0(p, x_eff, mass); }
+
+void oracle_add_material(const OGeometry* g, const OConfig* cfg, int32_t module, const double x[6], double C[36]) {
+  double Cm[6][6];
+  std::memcpy(Cm, C, sizeof(Cm));
+  add_material(*cfg, get_module(*g, module), x, Cm);
+  std::memcpy(C, Cm, sizeof(Cm));
+}
+
+}  // extern "C"
