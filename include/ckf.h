@@ -1,0 +1,193 @@
+/* ckf.h — C ABI of the B200-native combinatorial-Kalman-filter (CKF) track-finding library.
+ *
+ * What the entry points compute is the operation of arxiv 2505.22822 §2: "track parameters
+ * and their covariances are propagated based on the fourth order Runge-Kutta-Nystrom method and the Kalman
+ * Filter is applied to measurements on intersected sensor modules to calculate a chi2 value [...]  If the
+ * chi2 is small enough, the measurement is attached to the track to make a new branch for the propagation
+ * to the next sensor module."  Seeds in, track patterns out; geometry and magnetic
+ * field cross to the device once, measurements/seeds/results per event.  The concrete rules
+ * (units, stepping, navigation, gate, branching, caps) are DESIGN.md §3, following SURVEY.md §8(c).
+ *
+ * Conventions
+ *   - Units: mm, GeV, tesla, c = 1 (time in mm).  Bound parameters (loc0, loc1, phi, theta, q/p, t).
+ *   - All structs are POD and passed by const pointer; no C++ types or exceptions cross the ABI.
+ *   - Return value: 0 (CKF_OK) on success, negative CKF_E_* otherwise; ckf_last_error() gives text.
+ *   - ckf_find is ASYNCHRONOUS on `cuda_stream` and never allocates: every workspace is reserved in
+ *     ckf_create from the max_* capacities (PAPER.md:84, :102 blame in-pipeline allocation for the lack of
+ *     stream scaling).  Capacity overflow is never silent: it sets a bit in *status.
+ *   - There is no CPU fallback: without a CUDA device ckf_create fails with CKF_E_CUDA.
+ */
+#ifndef CKF_H_
+#define CKF_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+#define CKF_ABI_VERSION 1
+
+/* return codes */
+#define CKF_OK 0
+#define CKF_E_ARG (-1)     /* null pointer, bad size, unsupported value              */
+#define CKF_E_CUDA (-2)    /* a CUDA runtime call failed (text in ckf_last_error)    */
+#define CKF_E_CAPACITY (-3) /* n_seeds / n_measurements exceed the handle's capacity  */
+
+/* bits of *ckf_tracks.status (device int32, written by ckf_find) */
+#define CKF_STATUS_TRACK_OVERFLOW 1  /* more candidates than max_tracks: the first max_tracks are kept       */
+#define CKF_STATUS_ENTRY_OVERFLOW 2  /* meas_idx capacity max_track_entries exceeded: later tracks dropped   */
+#define CKF_STATUS_LINK_OVERFLOW 4   /* candidate-link buffer (max_links) exhausted: some branches were cut  */
+
+/* stop reasons reported per candidate */
+#define CKF_STOP_EXIT 1         /* left the detector (past the last layer / beyond half-z everywhere) */
+#define CKF_STOP_HOLES 2        /* more than max_holes surfaces without a compatible measurement      */
+#define CKF_STOP_NOT_OUTGOING 3 /* not radially outgoing when a cylinder portal was targeted          */
+#define CKF_STOP_STEP_LIMIT 4   /* more than max_rk_steps_per_surface RKN4 trials on one move         */
+#define CKF_STOP_NUMERIC 5      /* non-finite value or theta outside (0, pi)                          */
+#define CKF_STOP_LEVEL_LIMIT 6  /* max_levels surfaces visited                                        */
+
+typedef struct ckf_handle ckf_handle; /* opaque; owns device geometry, field, workspaces */
+
+/* Detector: per-layer phi/z grid of planar modules (north_star "geometry store").  HOST pointers, copied
+ * during ckf_create.  Module id = module_offset[l] + i_phi * n_z[l] + i_z; the module's local frame is
+ * (axis_u, axis_v), its normal axis_u x axis_v; loc0 runs along axis_u, loc1 along axis_v.  Within a layer
+ * all modules share half_v (the z pitch used by the navigator is 2*half_v of the layer's first module) and
+ * n_phi >= 3. */
+typedef struct {
+  int32_t n_layers;
+  const double* layer_r;        /* [n_layers] mm, increasing                         */
+  const double* layer_half_z;   /* [n_layers] mm                                     */
+  const int32_t* n_phi;         /* [n_layers]                                        */
+  const int32_t* n_z;           /* [n_layers]                                        */
+  const int32_t* module_offset; /* [n_layers + 1]                                    */
+  int32_t n_modules;
+  const double* center;         /* [n_modules][3] mm                                 */
+  const double* axis_u;         /* [n_modules][3] unit                               */
+  const double* axis_v;         /* [n_modules][3] unit                               */
+  const double* half_u;         /* [n_modules] mm                                    */
+  const double* half_v;         /* [n_modules] mm                                    */
+  const double* x_over_x0;      /* [n_modules]; 0 = no material                      */
+} ckf_geometry;
+
+/* Magnetic field (north_star "magnetic-field store").  HOST pointers, copied during ckf_create.
+ * kind 1: value(ix,iy,iz) sits at origin + i*spacing; read by trilinear interpolation (x, then y, then z);
+ * outside the grid the edge cell extrapolates linearly. */
+typedef struct {
+  int32_t kind;        /* 0 uniform, 1 grid                            */
+  double uniform_b[3]; /* tesla                                        */
+  int32_t n[3];
+  double origin[3];
+  double spacing[3];
+  const float* grid;   /* [n0][n1][n2][3] tesla, float32 always        */
+} ckf_field;
+
+typedef struct {
+  int32_t precision;   /* 32 or 64: element type T of every `void*` array below and of the covariance algebra.
+                          The trajectory (position, direction, bound parameter vector) is float64 in both. */
+  double chi2_max;     /* gate: chi2 < chi2_max (strict), 2 dof                                           */
+  int32_t max_branches_per_surface; /* k best (chi2, index) passers become branches; 1..32                */
+  int32_t max_candidates_per_seed;  /* cap on leaves per seed (R10); >= 1                       */
+  int32_t max_holes;                /* a branch stops when its hole count exceeds this                   */
+  int32_t min_measurements;         /* a stopped branch is emitted iff it holds at least this many       */
+  double rk_tolerance_mm;           /* RKN4 local error bound per step                                   */
+  double surface_tolerance_mm;      /* landing: a straight closing step once |distance| <= this          */
+  double h_max_mm;                  /* largest step                                                      */
+  double particle_mass_gev;         /* muon hypothesis                                      */
+  int32_t max_rk_steps_per_surface;
+  int32_t max_levels;               /* <= 64                                                             */
+  /* capacities: every workspace and the bounds of the output arrays */
+  int32_t max_seeds;
+  int32_t max_measurements;
+  int32_t max_tracks;               /* capacity of the per-track output arrays                           */
+  int32_t max_track_entries;        /* capacity of meas_idx / entry_chi2                                 */
+  int32_t max_links;                /* candidate-link buffer entries; 0 = 48 * max_seeds                 */
+  int32_t n_streams;                /* independent workspaces; concurrent ckf_find calls up to this many */
+} ckf_config;
+
+/* Measurements of one event: CSR by module id (north_star).  DEVICE pointers, caller-owned, read-only.
+ * A measurement's index is its position in loc/var and is what ckf_tracks.meas_idx reports. */
+typedef struct {
+  int32_t n;
+  const int32_t* module_offsets; /* [n_modules + 1]; module m owns [off[m], off[m+1])  */
+  const void* loc;               /* T[n][2] local position (loc0, loc1) mm             */
+  const void* var;               /* T[n][2] variances mm^2                             */
+} ckf_measurements;
+
+/* Seeds: bound parameters + covariance on a module.  DEVICE pointers, caller-owned, read-only. */
+typedef struct {
+  int32_t n;
+  const int32_t* module_id; /* [n]                                               */
+  const void* params;       /* T[n][6]  loc0 loc1 phi theta q/p t                */
+  const void* cov;          /* T[n][36] row-major, symmetric                     */
+} ckf_seeds;
+
+/* Track candidates.  DEVICE pointers, caller-owned, caller-sized from max_tracks / max_track_entries.
+ * Order: by seed id; within a seed by the level at which the branch stopped, then by branch order
+ * (children of an earlier parent first, within a parent by (chi2, index) rank).  Deterministic.
+ * Not de-duplicated (ambiguity resolution is a later stage). */
+typedef struct {
+  int32_t* n_tracks;       /* [1] number of candidates written (<= max_tracks)                       */
+  int32_t* status;         /* [1] CKF_STATUS_* bits                                                  */
+  int32_t* track_offsets;  /* [max_tracks + 1] CSR into meas_idx / entry_chi2                        */
+  int32_t* meas_idx;       /* [max_track_entries] measurement indices in visit order, holes omitted  */
+  int32_t* seed_id;        /* [max_tracks]                                                           */
+  int32_t* n_holes;        /* [max_tracks]                                                           */
+  int32_t* last_module;    /* [max_tracks] module of the last measurement                            */
+  int32_t* stop_reason;    /* [max_tracks] CKF_STOP_*                                                */
+  void* params;            /* T[max_tracks][6]  filtered parameters at the last measurement */
+  void* cov;               /* T[max_tracks][36] their covariance, row-major                          */
+  void* chi2_sum;          /* T[max_tracks]                                                          */
+  void* entry_chi2;        /* T[max_track_entries] predicted chi2 of each attached measurement       */
+} ckf_tracks;
+
+/* Work counters of the last ckf_find on a workspace (for roofline accounting). */
+typedef struct {
+  int64_t tips;         /* branch tips processed (sum over levels)             */
+  int64_t visits;       /* surface visits (gate evaluations of a whole module)  */
+  int64_t rk_trials;    /* RKN4 trial steps                                     */
+  int64_t rk_accepted;  /* accepted RKN4 steps                                  */
+  int64_t gate_tests;   /* chi2 evaluations                                     */
+  int64_t updates;      /* Kalman updates                                       */
+  int64_t links;        /* candidate links appended                             */
+  int64_t iterations;   /* sum over thread blocks of level-loop passes          */
+} ckf_counters;
+
+/* Uploads geometry and field (once, at the first event) and reserves all workspaces.
+ * All pointers inside geometry/field are HOST.  *out receives the handle.  Fails with CKF_E_CUDA when no
+ * CUDA device of compute capability 10.x is present. */
+int ckf_create(const ckf_geometry* geometry, const ckf_field* field, const ckf_config* config, ckf_handle** out);
+
+/* Runs CKF track finding for one event on `cuda_stream` (a cudaStream_t; NULL = default stream).
+ * Asynchronous; all pointers in measurements/seeds/out are DEVICE pointers that must stay valid until the
+ * stream reaches the end of the call's work.  Up to n_streams calls may be in flight on different streams;
+ * further streams are ordered after the call that last used the recycled workspace. */
+int ckf_find(ckf_handle* handle, const ckf_measurements* measurements, const ckf_seeds* seeds, ckf_tracks* out,
+             void* cuda_stream);
+
+/* Same work with HOST buffers: copies measurements and seeds host->device, runs ckf_find, copies the
+ * candidates device->host, all on `cuda_stream` (PAPER.md:51 transfer policy; BASELINE config 4).  Buffers
+ * should be pinned for the copies to be asynchronous.  Device staging buffers belong to the handle.
+ * Output arrays are filled up to *n_tracks / track_offsets[*n_tracks] after the stream is synchronised. */
+int ckf_find_host(ckf_handle* handle, const ckf_measurements* measurements, const ckf_seeds* seeds, ckf_tracks* out,
+                  void* cuda_stream);
+
+/* Copies the work counters of the most recent ckf_find issued on `cuda_stream` (synchronises that stream). */
+int ckf_get_counters(ckf_handle* handle, void* cuda_stream, ckf_counters* out);
+
+/* Launch configuration chosen at ckf_create: thread blocks, threads per block, dynamic shared bytes,
+ * registers per thread of the level-loop kernel (any pointer may be NULL). */
+int ckf_get_launch_info(const ckf_handle* handle, int32_t* blocks, int32_t* threads, int32_t* smem_bytes,
+                        int32_t* regs);
+
+int ckf_destroy(ckf_handle* handle);
+
+/* Text of the last error on this handle (or of the last failed ckf_create when handle is NULL). */
+const char* ckf_last_error(const ckf_handle* handle);
+
+int ckf_abi_version(void);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* CKF_H_ */

@@ -1,0 +1,280 @@
+"""Thin Python binding of the C ABI in include/ckf.h — argument marshalling only.
+
+Every step of the CKF runs in the CUDA kernels of libckf.so; PyTorch provides device memory and streams.
+There is no CPU fallback: if libckf.so is missing or no CUDA device is present, calls raise.
+"""
+from __future__ import annotations
+
+import ctypes as C
+import os
+from dataclasses import dataclass
+from typing import Optional
+
+import numpy as np
+
+_dp = C.POINTER(C.c_double)
+_ip = C.POINTER(C.c_int32)
+_fp = C.POINTER(C.c_float)
+_vp = C.c_void_p
+
+HERE = os.path.dirname(os.path.abspath(__file__))
+LIB_PATH = os.path.join(HERE, "libckf.so")
+
+EXPORTS = ("ckf_create", "ckf_find", "ckf_find_host", "ckf_get_counters", "ckf_get_launch_info", "ckf_destroy",
+           "ckf_last_error", "ckf_abi_version")
+
+
+class ckf_geometry(C.Structure):
+    _fields_ = [("n_layers", C.c_int32), ("layer_r", _dp), ("layer_half_z", _dp), ("n_phi", _ip), ("n_z", _ip),
+                ("module_offset", _ip), ("n_modules", C.c_int32), ("center", _dp), ("axis_u", _dp), ("axis_v", _dp),
+                ("half_u", _dp), ("half_v", _dp), ("x_over_x0", _dp)]
+
+
+class ckf_field(C.Structure):
+    _fields_ = [("kind", C.c_int32), ("uniform_b", C.c_double * 3), ("n", C.c_int32 * 3), ("origin", C.c_double * 3),
+                ("spacing", C.c_double * 3), ("grid", _fp)]
+
+
+class ckf_config(C.Structure):
+    _fields_ = [("precision", C.c_int32), ("chi2_max", C.c_double), ("max_branches_per_surface", C.c_int32),
+                ("max_candidates_per_seed", C.c_int32), ("max_holes", C.c_int32), ("min_measurements", C.c_int32),
+                ("rk_tolerance_mm", C.c_double), ("surface_tolerance_mm", C.c_double), ("h_max_mm", C.c_double),
+                ("particle_mass_gev", C.c_double), ("max_rk_steps_per_surface", C.c_int32), ("max_levels", C.c_int32),
+                ("max_seeds", C.c_int32), ("max_measurements", C.c_int32), ("max_tracks", C.c_int32),
+                ("max_track_entries", C.c_int32), ("max_links", C.c_int32), ("n_streams", C.c_int32)]
+
+
+class ckf_measurements(C.Structure):
+    _fields_ = [("n", C.c_int32), ("module_offsets", _vp), ("loc", _vp), ("var", _vp)]
+
+
+class ckf_seeds(C.Structure):
+    _fields_ = [("n", C.c_int32), ("module_id", _vp), ("params", _vp), ("cov", _vp)]
+
+
+class ckf_tracks(C.Structure):
+    _fields_ = [("n_tracks", _vp), ("status", _vp), ("track_offsets", _vp), ("meas_idx", _vp), ("seed_id", _vp),
+                ("n_holes", _vp), ("last_module", _vp), ("stop_reason", _vp), ("params", _vp), ("cov", _vp),
+                ("chi2_sum", _vp), ("entry_chi2", _vp)]
+
+
+class ckf_counters(C.Structure):
+    _fields_ = [("tips", C.c_int64), ("visits", C.c_int64), ("rk_trials", C.c_int64), ("rk_accepted", C.c_int64),
+                ("gate_tests", C.c_int64), ("updates", C.c_int64), ("links", C.c_int64), ("iterations", C.c_int64)]
+
+
+_lib = None
+
+
+def load_library():
+    """Loads libckf.so (built in-tree by `_build.py`).  Raises if it is missing: no fallback."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise RuntimeError(f"{LIB_PATH} is missing: run `python -m paper_2505_22822_b200._build` "
+                               "(there is no CPU fallback)")
+        L = C.CDLL(LIB_PATH)
+        L.ckf_create.restype = C.c_int
+        L.ckf_create.argtypes = [C.POINTER(ckf_geometry), C.POINTER(ckf_field), C.POINTER(ckf_config), C.POINTER(_vp)]
+        for name in ("ckf_find", "ckf_find_host"):
+            fn = getattr(L, name)
+            fn.restype = C.c_int
+            fn.argtypes = [_vp, C.POINTER(ckf_measurements), C.POINTER(ckf_seeds), C.POINTER(ckf_tracks), _vp]
+        L.ckf_get_counters.restype = C.c_int
+        L.ckf_get_counters.argtypes = [_vp, _vp, C.POINTER(ckf_counters)]
+        L.ckf_get_launch_info.restype = C.c_int
+        L.ckf_get_launch_info.argtypes = [_vp, _ip, _ip, _ip, _ip]
+        L.ckf_destroy.restype = C.c_int
+        L.ckf_destroy.argtypes = [_vp]
+        L.ckf_last_error.restype = C.c_char_p
+        L.ckf_last_error.argtypes = [_vp]
+        L.ckf_abi_version.restype = C.c_int
+        _lib = L
+    return _lib
+
+
+def _d(a):
+    return np.ascontiguousarray(a, dtype=np.float64)
+
+
+def _i(a):
+    return np.ascontiguousarray(a, dtype=np.int32)
+
+
+def make_geometry(det, keep: list) -> ckf_geometry:
+    g = ckf_geometry()
+    g.n_layers = int(det.n_layers)
+    g.n_modules = int(det.n_modules)
+    for name, conv, pt in (("layer_r", _d, _dp), ("layer_half_z", _d, _dp), ("n_phi", _i, _ip), ("n_z", _i, _ip),
+                           ("module_offset", _i, _ip), ("center", _d, _dp), ("axis_u", _d, _dp), ("axis_v", _d, _dp),
+                           ("half_u", _d, _dp), ("half_v", _d, _dp), ("x_over_x0", _d, _dp)):
+        arr = conv(getattr(det, name))
+        keep.append(arr)
+        setattr(g, name, arr.ctypes.data_as(pt))
+    return g
+
+
+def make_field(fld, keep: list) -> ckf_field:
+    f = ckf_field()
+    f.kind = int(fld.kind)
+    for a in range(3):
+        f.uniform_b[a] = float(fld.uniform_b[a])
+        f.n[a] = int(fld.n[a])
+        f.origin[a] = float(fld.origin[a])
+        f.spacing[a] = float(fld.spacing[a])
+    if fld.grid is not None:
+        grid = np.ascontiguousarray(fld.grid, dtype=np.float32)
+        keep.append(grid)
+        f.grid = grid.ctypes.data_as(_fp)
+    return f
+
+
+def make_config(ckf, precision: int, max_seeds: int, max_measurements: int, max_tracks: int, max_track_entries: int,
+                max_links: int = 0, n_streams: int = 1) -> ckf_config:
+    c = ckf_config()
+    c.precision = int(precision)
+    for name in ("chi2_max", "max_branches_per_surface", "max_candidates_per_seed", "max_holes", "min_measurements",
+                 "rk_tolerance_mm", "surface_tolerance_mm", "h_max_mm", "particle_mass_gev",
+                 "max_rk_steps_per_surface", "max_levels"):
+        setattr(c, name, getattr(ckf, name))
+    c.max_seeds, c.max_measurements = int(max_seeds), int(max_measurements)
+    c.max_tracks, c.max_track_entries = int(max_tracks), int(max_track_entries)
+    c.max_links, c.n_streams = int(max_links), int(n_streams)
+    return c
+
+
+@dataclass
+class TrackArrays:
+    """Host copy of `ckf_tracks` (numpy)."""
+    n_tracks: int
+    status: int
+    track_offsets: np.ndarray
+    meas_idx: np.ndarray
+    entry_chi2: np.ndarray
+    seed_id: np.ndarray
+    n_holes: np.ndarray
+    last_module: np.ndarray
+    stop_reason: np.ndarray
+    params: np.ndarray
+    cov: np.ndarray
+    chi2_sum: np.ndarray
+
+    def meas_list(self, t: int):
+        return self.meas_idx[self.track_offsets[t]:self.track_offsets[t + 1]]
+
+
+class CKF:
+    """ckf_create / ckf_find / ckf_find_host / ckf_destroy with torch tensors as device memory."""
+
+    def __init__(self, det, fld, ckf, precision: int, max_seeds: int, max_measurements: int,
+                 max_tracks: Optional[int] = None, max_track_entries: Optional[int] = None, max_links: int = 0,
+                 n_streams: int = 1):
+        import torch
+        if not torch.cuda.is_available():
+            raise RuntimeError("no CUDA device: paper_2505_22822_b200 has no CPU fallback")
+        self.torch = torch
+        self.lib = load_library()
+        self.precision = int(precision)
+        self.tdtype = torch.float32 if precision == 32 else torch.float64
+        self.ndtype = np.float32 if precision == 32 else np.float64
+        self.n_modules = int(det.n_modules)
+        self.max_tracks = int(max_tracks if max_tracks is not None else 8 * max_seeds)
+        self.max_track_entries = int(max_track_entries if max_track_entries is not None else 16 * self.max_tracks)
+        keep = []
+        g = make_geometry(det, keep)
+        f = make_field(fld, keep)
+        self.config = make_config(ckf, precision, max_seeds, max_measurements, self.max_tracks, self.max_track_entries,
+                                  max_links, n_streams)
+        h = _vp()
+        rc = self.lib.ckf_create(C.byref(g), C.byref(f), C.byref(self.config), C.byref(h))
+        if rc != 0:
+            raise RuntimeError("ckf_create failed (%d): %s" % (rc, self.lib.ckf_last_error(None).decode()))
+        self.handle = h
+
+    # ------------------------------------------------------------------ device-resident path
+    def alloc_tracks(self, device="cuda"):
+        t = self.torch
+        i32 = dict(dtype=t.int32, device=device)
+        T = dict(dtype=self.tdtype, device=device)
+        nt, ne = self.max_tracks, self.max_track_entries
+        return dict(n_tracks=t.zeros(1, **i32), status=t.zeros(1, **i32), track_offsets=t.zeros(nt + 1, **i32),
+                    meas_idx=t.zeros(ne, **i32), seed_id=t.zeros(nt, **i32), n_holes=t.zeros(nt, **i32),
+                    last_module=t.zeros(nt, **i32), stop_reason=t.zeros(nt, **i32), params=t.zeros(nt, 6, **T),
+                    cov=t.zeros(nt, 36, **T), chi2_sum=t.zeros(nt, **T), entry_chi2=t.zeros(ne, **T))
+
+    def upload_event(self, ev, device="cuda"):
+        t = self.torch
+        return dict(
+            module_offsets=t.from_numpy(np.ascontiguousarray(ev.module_offsets, np.int32)).to(device),
+            loc=t.from_numpy(np.ascontiguousarray(ev.loc, self.ndtype)).to(device),
+            var=t.from_numpy(np.ascontiguousarray(ev.var, self.ndtype)).to(device),
+            seed_module=t.from_numpy(np.ascontiguousarray(ev.seed_module, np.int32)).to(device),
+            seed_params=t.from_numpy(np.ascontiguousarray(ev.seed_params, self.ndtype)).to(device),
+            seed_cov=t.from_numpy(np.ascontiguousarray(ev.seed_cov, self.ndtype)).to(device))
+
+    def _structs(self, d, out, ptr):
+        m = ckf_measurements(int(d["loc"].shape[0]), ptr(d["module_offsets"]), ptr(d["loc"]), ptr(d["var"]))
+        s = ckf_seeds(int(d["seed_module"].shape[0]), ptr(d["seed_module"]), ptr(d["seed_params"]), ptr(d["seed_cov"]))
+        o = ckf_tracks(*[ptr(out[k]) for k in ("n_tracks", "status", "track_offsets", "meas_idx", "seed_id", "n_holes",
+                                               "last_module", "stop_reason", "params", "cov", "chi2_sum",
+                                               "entry_chi2")])
+        return m, s, o
+
+    def find(self, dev_event: dict, out: dict, stream=None):
+        """Asynchronous ckf_find on device tensors; `stream` is a torch.cuda.Stream (default: current)."""
+        st = stream if stream is not None else self.torch.cuda.current_stream()
+        m, s, o = self._structs(dev_event, out, lambda x: x.data_ptr())
+        rc = self.lib.ckf_find(self.handle, C.byref(m), C.byref(s), C.byref(o), _vp(st.cuda_stream))
+        if rc != 0:
+            raise RuntimeError("ckf_find failed (%d): %s" % (rc, self.lib.ckf_last_error(self.handle).decode()))
+
+    def find_host(self, host_event: dict, host_out: dict, stream=None):
+        """ckf_find_host on (pinned) host tensors: H2D, find, D2H inside; synchronous on return."""
+        st = stream if stream is not None else self.torch.cuda.current_stream()
+        m, s, o = self._structs(host_event, host_out, lambda x: x.data_ptr())
+        rc = self.lib.ckf_find_host(self.handle, C.byref(m), C.byref(s), C.byref(o), _vp(st.cuda_stream))
+        if rc != 0:
+            raise RuntimeError("ckf_find_host failed (%d): %s" % (rc, self.lib.ckf_last_error(self.handle).decode()))
+
+    def pinned_event(self, ev):
+        d = self.upload_event(ev, device="cpu")
+        return {k: v.pin_memory() for k, v in d.items()}
+
+    def pinned_tracks(self):
+        d = self.alloc_tracks(device="cpu")
+        return {k: v.pin_memory() for k, v in d.items()}
+
+    def download(self, out: dict) -> TrackArrays:
+        cpu = {k: v.cpu().numpy() for k, v in out.items()} if out["n_tracks"].is_cuda else \
+            {k: v.numpy() for k, v in out.items()}
+        nt = int(cpu["n_tracks"][0])
+        ne = int(cpu["track_offsets"][nt]) if nt > 0 else 0
+        return TrackArrays(nt, int(cpu["status"][0]), cpu["track_offsets"][:nt + 1].copy(), cpu["meas_idx"][:ne].copy(),
+                           cpu["entry_chi2"][:ne].astype(np.float64), cpu["seed_id"][:nt].copy(),
+                           cpu["n_holes"][:nt].copy(), cpu["last_module"][:nt].copy(), cpu["stop_reason"][:nt].copy(),
+                           cpu["params"][:nt].astype(np.float64), cpu["cov"][:nt].astype(np.float64),
+                           cpu["chi2_sum"][:nt].astype(np.float64))
+
+    def counters(self, stream=None) -> dict:
+        st = stream if stream is not None else self.torch.cuda.current_stream()
+        c = ckf_counters()
+        rc = self.lib.ckf_get_counters(self.handle, _vp(st.cuda_stream), C.byref(c))
+        if rc != 0:
+            raise RuntimeError("ckf_get_counters failed: %s" % self.lib.ckf_last_error(self.handle).decode())
+        return {k: int(getattr(c, k)) for k, _ in ckf_counters._fields_}
+
+    def launch_info(self) -> dict:
+        v = [C.c_int32(0) for _ in range(4)]
+        self.lib.ckf_get_launch_info(self.handle, *[C.byref(x) for x in v])
+        return dict(blocks=v[0].value, threads=v[1].value, smem_bytes=v[2].value, regs=v[3].value)
+
+    def close(self):
+        if getattr(self, "handle", None):
+            self.lib.ckf_destroy(self.handle)
+            self.handle = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass

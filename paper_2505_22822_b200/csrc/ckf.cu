@@ -1,0 +1,390 @@
+// ckf.cu — C ABI of the B200-native CKF track-finding library (include/ckf.h): host side.
+//
+// ckf_create uploads the geometry store (a1) and field store (a2) once and reserves every
+// workspace; ckf_find enqueues five launches on the caller's stream and never allocates.
+// There is no CPU path in this library: all arithmetic of the method runs in the kernels of
+// ckf_level_loop.cuh / ckf_emit.cuh.
+#include <cuda_runtime.h>
+
+#include <cstdarg>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <string>
+#include <vector>
+
+#include "../../include/ckf.h"
+#include "ckf_emit.cuh"
+#include "ckf_host_geom.h"
+#include "ckf_level_loop.cuh"
+
+using namespace ckf;
+
+namespace {
+
+thread_local std::string g_create_error;
+
+struct Workspace {
+  // link buffer
+  double* lk_x = nullptr;
+  void* lk_C = nullptr;
+  int32_t *lk_module = nullptr, *lk_parent = nullptr, *lk_meas = nullptr, *lk_counts = nullptr, *lk_lastmeas = nullptr;
+  void *lk_chi2 = nullptr, *lk_chi2sum = nullptr;
+  int32_t *sd = nullptr;       // 3 * max_seeds + 2 * (max_seeds + 1)
+  int32_t* leaf = nullptr;     // 3 * max_seeds * cap
+  int2* queue = nullptr;
+  int32_t* globals = nullptr;  // cursor, link_count, first_bad, total[2]
+  unsigned long long* counters = nullptr;
+  // staging for ckf_find_host
+  int32_t* h_moff = nullptr; void *h_loc = nullptr, *h_var = nullptr;
+  int32_t* h_smod = nullptr; void *h_sx = nullptr, *h_sC = nullptr;
+  int32_t *o_nt = nullptr, *o_off = nullptr, *o_meas = nullptr, *o_seed = nullptr, *o_nh = nullptr, *o_lm = nullptr,
+          *o_stop = nullptr;
+  void *o_par = nullptr, *o_cov = nullptr, *o_c2 = nullptr, *o_ec2 = nullptr;
+  int32_t* pinned_nt = nullptr;  // host pinned [2]
+  cudaEvent_t done = nullptr;
+  void* stream_tag = nullptr;
+  bool used = false;
+};
+
+}  // namespace
+
+struct ckf_handle {
+  ckf_config cfg;
+  int device = 0, sm_count = 0;
+  int n_modules = 0, n_layers = 0;
+  ModuleRec* d_mod = nullptr;
+  LayerRec* d_layer = nullptr;
+  float4* d_grid = nullptr;
+  FieldDev fld;
+  CfgDev kcfg;
+  int grid = 0, smem = 0, regs = 0, qcap = 0, tsize = 4;
+  std::vector<Workspace> ws;
+  int next_ws = 0;
+  std::mutex mu;
+  std::string err;
+  std::vector<void*> allocs;
+};
+
+namespace {
+
+int fail(ckf_handle* h, int code, const char* fmt, ...) {
+  char buf[512];
+  va_list ap;
+  va_start(ap, fmt);
+  vsnprintf(buf, sizeof(buf), fmt, ap);
+  va_end(ap);
+  if (h) h->err = buf;
+  else g_create_error = buf;
+  return code;
+}
+
+#define CK(call)                                                                                        \
+  do {                                                                                                  \
+    cudaError_t e_ = (call);                                                                            \
+    if (e_ != cudaSuccess) return fail(h, CKF_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_)); \
+  } while (0)
+
+template <typename P>
+cudaError_t dalloc(ckf_handle* h, P** p, size_t bytes) {
+  void* q = nullptr;
+  cudaError_t e = cudaMalloc(&q, bytes ? bytes : 16);
+  if (e == cudaSuccess) { h->allocs.push_back(q); *p = (P*)q; }
+  return e;
+}
+
+template <typename T>
+void fill_params(ckf_handle* h, Workspace& w, KParams<T>& p) {
+  const ckf_config& c = h->cfg;
+  p.geo.mod = h->d_mod; p.geo.layer = h->d_layer; p.geo.n_layers = h->n_layers; p.geo.n_modules = h->n_modules;
+  p.fld = h->fld;
+  p.cfg = h->kcfg;
+  p.max_links = c.max_links;
+  p.lk_x = w.lk_x; p.lk_C = (T*)w.lk_C; p.lk_module = w.lk_module; p.lk_parent = w.lk_parent; p.lk_meas = w.lk_meas;
+  p.lk_chi2 = (T*)w.lk_chi2; p.lk_chi2sum = (T*)w.lk_chi2sum; p.lk_counts = w.lk_counts; p.lk_lastmeas = w.lk_lastmeas;
+  const size_t S = (size_t)c.max_seeds;
+  p.sd_extra = w.sd; p.sd_nemit = w.sd + S; p.sd_nentries = w.sd + 2 * S;
+  p.sd_track_base = w.sd + 3 * S; p.sd_entry_base = w.sd + 3 * S + (S + 1);
+  const size_t LC = S * (size_t)c.max_candidates_per_seed;
+  p.leaf_link = w.leaf; p.leaf_meta = w.leaf + LC; p.leaf_entry = w.leaf + 2 * LC;
+  p.queue = w.queue; p.qcap = h->qcap;
+  p.g_seed_cursor = w.globals; p.g_link_count = w.globals + 1; p.g_first_bad = w.globals + 2; p.g_total = w.globals + 3;
+  p.counters = w.counters;
+  p.max_tracks = c.max_tracks; p.max_entries = c.max_track_entries;
+}
+
+template <typename T>
+int launch_find(ckf_handle* h, Workspace& w, const ckf_measurements* m, const ckf_seeds* s, ckf_tracks* o,
+                cudaStream_t st) {
+  KParams<T> p;
+  fill_params<T>(h, w, p);
+  p.n_meas = m->n; p.n_seeds = s->n;
+  p.moff = m->module_offsets;
+  p.loc = (const typename Vec2<T>::type*)m->loc;
+  p.var = (const typename Vec2<T>::type*)m->var;
+  p.seed_module = s->module_id; p.seed_x = (const T*)s->params; p.seed_C = (const T*)s->cov;
+  p.o_ntracks = o->n_tracks; p.o_status = o->status; p.o_offsets = o->track_offsets; p.o_meas = o->meas_idx;
+  p.o_seed = o->seed_id; p.o_nholes = o->n_holes; p.o_lastmod = o->last_module; p.o_stop = o->stop_reason;
+  p.o_params = (T*)o->params; p.o_cov = (T*)o->cov; p.o_chi2sum = (T*)o->chi2_sum; p.o_entrychi2 = (T*)o->entry_chi2;
+  const int nb = (std::max(s->n, (int)CNT_N) + 255) / 256;
+  ckf_init_event<T><<<nb, 256, 0, st>>>(p);
+  ckf_level_loop<T, (sizeof(T) == 4 ? 2 : 1)><<<h->grid, NT, h->smem, st>>>(p);
+  ckf_scan_seeds<T><<<1, 1024, 0, st>>>(p);
+  ckf_emit_tracks<T><<<h->sm_count * 4, 256, 0, st>>>(p);
+  ckf_finalize<T><<<1, 1, 0, st>>>(p);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(h, CKF_E_CUDA, "kernel launch failed: %s", cudaGetErrorString(e));
+  return CKF_OK;
+}
+
+// Picks (or recycles) the workspace for this stream; orders the stream after the workspace's last user.
+Workspace* acquire_ws(ckf_handle* h, cudaStream_t st) {
+  std::lock_guard<std::mutex> lk(h->mu);
+  Workspace* w = nullptr;
+  for (auto& x : h->ws)
+    if (x.used && x.stream_tag == (void*)st) { w = &x; break; }
+  if (!w)
+    for (auto& x : h->ws)
+      if (!x.used) { w = &x; break; }
+  if (!w) { w = &h->ws[h->next_ws]; h->next_ws = (h->next_ws + 1) % (int)h->ws.size(); }
+  if (w->used && w->stream_tag != (void*)st) cudaStreamWaitEvent(st, w->done, 0);
+  w->used = true;
+  w->stream_tag = (void*)st;
+  return w;
+}
+
+}  // namespace
+
+extern "C" {
+
+int ckf_abi_version(void) { return CKF_ABI_VERSION; }
+
+const char* ckf_last_error(const ckf_handle* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+
+int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, ckf_handle** out) {
+  ckf_handle* h = nullptr;
+  if (!g || !f || !c || !out) return fail(h, CKF_E_ARG, "null argument");
+  *out = nullptr;
+  if (c->precision != 32 && c->precision != 64) return fail(h, CKF_E_ARG, "precision must be 32 or 64");
+  if (c->max_branches_per_surface < 1 || c->max_branches_per_surface > CAND)
+    return fail(h, CKF_E_ARG, "max_branches_per_surface must be in 1..%d", CAND);
+  if (c->max_candidates_per_seed < 1 || c->max_candidates_per_seed > NT)
+    return fail(h, CKF_E_ARG, "max_candidates_per_seed must be in 1..%d", NT);
+  if (c->max_levels < 1 || c->max_levels > 64) return fail(h, CKF_E_ARG, "max_levels must be in 1..64");
+  if (c->min_measurements < 1) return fail(h, CKF_E_ARG, "min_measurements must be >= 1");
+  if (c->max_seeds < 1 || c->max_measurements < 0 || c->max_tracks < 1 || c->max_track_entries < 1 || c->n_streams < 1)
+    return fail(h, CKF_E_ARG, "capacities must be positive");
+  if (g->n_layers < 1 || g->n_modules < 1) return fail(h, CKF_E_ARG, "empty geometry");
+  if (f->kind != 0 && f->kind != 1) return fail(h, CKF_E_ARG, "field kind must be 0 or 1");
+  if (f->kind == 1 && (!f->grid || f->n[0] < 2 || f->n[1] < 2 || f->n[2] < 2))
+    return fail(h, CKF_E_ARG, "field grid needs >= 2 nodes per axis");
+  for (int l = 0; l < g->n_layers; ++l)
+    if (g->n_phi[l] < 3 || g->n_z[l] < 1) return fail(h, CKF_E_ARG, "layer %d: n_phi >= 3 and n_z >= 1 required", l);
+
+  int ndev = 0;
+  if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1)
+    return fail(h, CKF_E_CUDA, "no CUDA device: this library has no CPU fallback");
+  h = new ckf_handle();
+  h->cfg = *c;
+  if (h->cfg.max_links <= 0) h->cfg.max_links = (int32_t)std::min<long long>(48LL * c->max_seeds, 0x7ffffff0LL);
+  h->tsize = c->precision == 32 ? 4 : 8;
+  auto bail = [&](int code) { std::string e = h->err; ckf_destroy(h); g_create_error = e; return code; };
+  cudaDeviceProp prop;
+  if (cudaGetDevice(&h->device) != cudaSuccess || cudaGetDeviceProperties(&prop, h->device) != cudaSuccess) {
+    fail(h, CKF_E_CUDA, "cudaGetDeviceProperties failed");
+    return bail(CKF_E_CUDA);
+  }
+  h->sm_count = prop.multiProcessorCount;
+  h->n_modules = g->n_modules;
+  h->n_layers = g->n_layers;
+
+  // ---- a1 geometry store
+  std::vector<ModuleRec> mods;
+  std::vector<LayerRec> layers;
+  build_geometry_records(*g, mods, layers);
+#define CKB(call)                                                                            \
+  do {                                                                                       \
+    cudaError_t e_ = (call);                                                                 \
+    if (e_ != cudaSuccess) {                                                                 \
+      fail(h, CKF_E_CUDA, "%s failed: %s", #call, cudaGetErrorString(e_));                   \
+      return bail(CKF_E_CUDA);                                                               \
+    }                                                                                        \
+  } while (0)
+  CKB(dalloc(h, &h->d_mod, mods.size() * sizeof(ModuleRec)));
+  CKB(dalloc(h, &h->d_layer, layers.size() * sizeof(LayerRec)));
+  CKB(cudaMemcpy(h->d_mod, mods.data(), mods.size() * sizeof(ModuleRec), cudaMemcpyHostToDevice));
+  CKB(cudaMemcpy(h->d_layer, layers.data(), layers.size() * sizeof(LayerRec), cudaMemcpyHostToDevice));
+  // ---- a2 field store
+  std::memset(&h->fld, 0, sizeof(h->fld));
+  h->fld.kind = f->kind;
+  for (int a = 0; a < 3; ++a) {
+    h->fld.ub[a] = f->uniform_b[a];
+    h->fld.n[a] = f->n[a];
+    h->fld.org[a] = f->origin[a];
+    h->fld.inv[a] = f->kind == 1 ? 1.0 / f->spacing[a] : 0.0;
+  }
+  if (f->kind == 1) {
+    const size_t np = (size_t)f->n[0] * f->n[1] * f->n[2];
+    std::vector<float4> pad(np);
+    for (size_t i = 0; i < np; ++i) pad[i] = make_float4(f->grid[3 * i], f->grid[3 * i + 1], f->grid[3 * i + 2], 0.f);
+    CKB(dalloc(h, &h->d_grid, np * sizeof(float4)));
+    CKB(cudaMemcpy(h->d_grid, pad.data(), np * sizeof(float4), cudaMemcpyHostToDevice));
+    h->fld.grid = h->d_grid;
+  }
+  // ---- config
+  h->kcfg.chi2_max = c->chi2_max; h->kcfg.rk_tol = c->rk_tolerance_mm; h->kcfg.surf_tol = c->surface_tolerance_mm;
+  h->kcfg.h_max = c->h_max_mm; h->kcfg.mass = c->particle_mass_gev; h->kcfg.max_branches = c->max_branches_per_surface;
+  h->kcfg.max_cands = c->max_candidates_per_seed; h->kcfg.max_holes = c->max_holes; h->kcfg.min_meas = c->min_measurements;
+  h->kcfg.max_rk_steps = c->max_rk_steps_per_surface; h->kcfg.max_levels = c->max_levels;
+  // ---- launch configuration of the level loop: one wave of resident blocks
+  int per_sm = 0;
+  cudaFuncAttributes fa;
+  if (c->precision == 32) {
+    h->smem = (int)Smem<float>::bytes(c->max_branches_per_surface);
+    CKB(cudaFuncSetAttribute(ckf_level_loop<float, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem));
+    CKB(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ckf_level_loop<float, 2>, NT, h->smem));
+    CKB(cudaFuncGetAttributes(&fa, ckf_level_loop<float, 2>));
+  } else {
+    h->smem = (int)Smem<double>::bytes(c->max_branches_per_surface);
+    CKB(cudaFuncSetAttribute(ckf_level_loop<double, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem));
+    CKB(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ckf_level_loop<double, 1>, NT, h->smem));
+    CKB(cudaFuncGetAttributes(&fa, ckf_level_loop<double, 1>));
+  }
+  if (per_sm < 1) { fail(h, CKF_E_CUDA, "level-loop kernel does not fit on an SM (smem %d B)", h->smem); return bail(CKF_E_CUDA); }
+  h->regs = fa.numRegs;
+  h->grid = per_sm * h->sm_count;
+  h->qcap = NT * c->max_candidates_per_seed;
+  // ---- workspaces
+  const size_t L = (size_t)h->cfg.max_links, S = (size_t)c->max_seeds, ts = (size_t)h->tsize;
+  h->ws.resize(c->n_streams);
+  for (auto& w : h->ws) {
+    CKB(dalloc(h, &w.lk_x, 6 * L * sizeof(double)));
+    CKB(dalloc(h, (char**)&w.lk_C, 21 * L * ts));
+    CKB(dalloc(h, &w.lk_module, L * 4)); CKB(dalloc(h, &w.lk_parent, L * 4)); CKB(dalloc(h, &w.lk_meas, L * 4));
+    CKB(dalloc(h, &w.lk_counts, L * 4)); CKB(dalloc(h, &w.lk_lastmeas, L * 4));
+    CKB(dalloc(h, (char**)&w.lk_chi2, L * ts)); CKB(dalloc(h, (char**)&w.lk_chi2sum, L * ts));
+    CKB(dalloc(h, &w.sd, (3 * S + 2 * (S + 1)) * 4));
+    CKB(dalloc(h, &w.leaf, 3 * S * (size_t)c->max_candidates_per_seed * 4));
+    CKB(dalloc(h, &w.queue, (size_t)h->grid * 2 * h->qcap * sizeof(int2)));
+    CKB(dalloc(h, &w.globals, 16 * 4));
+    CKB(dalloc(h, &w.counters, CNT_N * 8));
+    CKB(cudaEventCreateWithFlags(&w.done, cudaEventDisableTiming));
+    // staging for ckf_find_host
+    const size_t M = (size_t)c->max_measurements, NTK = (size_t)c->max_tracks, NE = (size_t)c->max_track_entries;
+    CKB(dalloc(h, &w.h_moff, ((size_t)g->n_modules + 1) * 4));
+    CKB(dalloc(h, (char**)&w.h_loc, 2 * M * ts)); CKB(dalloc(h, (char**)&w.h_var, 2 * M * ts));
+    CKB(dalloc(h, &w.h_smod, S * 4)); CKB(dalloc(h, (char**)&w.h_sx, 6 * S * ts)); CKB(dalloc(h, (char**)&w.h_sC, 36 * S * ts));
+    CKB(dalloc(h, &w.o_nt, 2 * 4)); CKB(dalloc(h, &w.o_off, (NTK + 1) * 4)); CKB(dalloc(h, &w.o_meas, NE * 4));
+    CKB(dalloc(h, &w.o_seed, NTK * 4)); CKB(dalloc(h, &w.o_nh, NTK * 4)); CKB(dalloc(h, &w.o_lm, NTK * 4));
+    CKB(dalloc(h, &w.o_stop, NTK * 4));
+    CKB(dalloc(h, (char**)&w.o_par, 6 * NTK * ts)); CKB(dalloc(h, (char**)&w.o_cov, 36 * NTK * ts));
+    CKB(dalloc(h, (char**)&w.o_c2, NTK * ts)); CKB(dalloc(h, (char**)&w.o_ec2, NE * ts));
+    CKB(cudaMallocHost((void**)&w.pinned_nt, 2 * 4));
+  }
+#undef CKB
+  *out = h;
+  return CKF_OK;
+}
+
+int ckf_find(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, ckf_tracks* o, void* stream) {
+  if (!h) return CKF_E_ARG;
+  if (!m || !s || !o) return fail(h, CKF_E_ARG, "null argument");
+  if (m->n < 0 || s->n < 0) return fail(h, CKF_E_ARG, "negative size");
+  if (s->n > h->cfg.max_seeds || m->n > h->cfg.max_measurements)
+    return fail(h, CKF_E_CAPACITY, "n_seeds %d / n_measurements %d exceed capacity %d / %d", s->n, m->n,
+                h->cfg.max_seeds, h->cfg.max_measurements);
+  if (!m->module_offsets || (m->n > 0 && (!m->loc || !m->var)) || (s->n > 0 && (!s->module_id || !s->params || !s->cov)))
+    return fail(h, CKF_E_ARG, "null input array");
+  if (!o->n_tracks || !o->status || !o->track_offsets || !o->meas_idx || !o->seed_id || !o->n_holes || !o->last_module ||
+      !o->stop_reason || !o->params || !o->cov || !o->chi2_sum || !o->entry_chi2)
+    return fail(h, CKF_E_ARG, "null output array");
+  cudaStream_t st = (cudaStream_t)stream;
+  Workspace* w = acquire_ws(h, st);
+  int rc = h->cfg.precision == 32 ? launch_find<float>(h, *w, m, s, o, st) : launch_find<double>(h, *w, m, s, o, st);
+  cudaEventRecord(w->done, st);
+  return rc;
+}
+
+int ckf_find_host(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, ckf_tracks* o, void* stream) {
+  if (!h) return CKF_E_ARG;
+  if (!m || !s || !o) return fail(h, CKF_E_ARG, "null argument");
+  if (m->n < 0 || s->n < 0 || s->n > h->cfg.max_seeds || m->n > h->cfg.max_measurements)
+    return fail(h, CKF_E_CAPACITY, "n_seeds %d / n_measurements %d exceed capacity", s->n, m->n);
+  cudaStream_t st = (cudaStream_t)stream;
+  Workspace* w = acquire_ws(h, st);
+  const size_t ts = (size_t)h->tsize;
+  CK(cudaMemcpyAsync(w->h_moff, m->module_offsets, ((size_t)h->n_modules + 1) * 4, cudaMemcpyHostToDevice, st));
+  CK(cudaMemcpyAsync(w->h_loc, m->loc, 2 * (size_t)m->n * ts, cudaMemcpyHostToDevice, st));
+  CK(cudaMemcpyAsync(w->h_var, m->var, 2 * (size_t)m->n * ts, cudaMemcpyHostToDevice, st));
+  CK(cudaMemcpyAsync(w->h_smod, s->module_id, (size_t)s->n * 4, cudaMemcpyHostToDevice, st));
+  CK(cudaMemcpyAsync(w->h_sx, s->params, 6 * (size_t)s->n * ts, cudaMemcpyHostToDevice, st));
+  CK(cudaMemcpyAsync(w->h_sC, s->cov, 36 * (size_t)s->n * ts, cudaMemcpyHostToDevice, st));
+  ckf_measurements dm = {m->n, w->h_moff, w->h_loc, w->h_var};
+  ckf_seeds ds = {s->n, w->h_smod, w->h_sx, w->h_sC};
+  ckf_tracks dt = {w->o_nt, w->o_nt + 1, w->o_off, w->o_meas, w->o_seed, w->o_nh, w->o_lm, w->o_stop,
+                   w->o_par, w->o_cov, w->o_c2, w->o_ec2};
+  int rc = h->cfg.precision == 32 ? launch_find<float>(h, *w, &dm, &ds, &dt, st) : launch_find<double>(h, *w, &dm, &ds, &dt, st);
+  if (rc != CKF_OK) return rc;
+  CK(cudaMemcpyAsync(w->pinned_nt, w->o_nt, 8, cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  const size_t nt = (size_t)w->pinned_nt[0];
+  *o->n_tracks = w->pinned_nt[0];
+  *o->status = w->pinned_nt[1];
+  CK(cudaMemcpyAsync(o->track_offsets, w->o_off, (nt + 1) * 4, cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(o->seed_id, w->o_seed, nt * 4, cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(o->n_holes, w->o_nh, nt * 4, cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(o->last_module, w->o_lm, nt * 4, cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(o->stop_reason, w->o_stop, nt * 4, cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(o->params, w->o_par, 6 * nt * ts, cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(o->cov, w->o_cov, 36 * nt * ts, cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(o->chi2_sum, w->o_c2, nt * ts, cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));  // track_offsets[nt] is needed for the entry count
+  const size_t ne = nt ? (size_t)o->track_offsets[nt] : 0;
+  CK(cudaMemcpyAsync(o->meas_idx, w->o_meas, ne * 4, cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(o->entry_chi2, w->o_ec2, ne * ts, cudaMemcpyDeviceToHost, st));
+  CK(cudaStreamSynchronize(st));
+  cudaEventRecord(w->done, st);
+  return CKF_OK;
+}
+
+int ckf_get_counters(ckf_handle* h, void* stream, ckf_counters* out) {
+  if (!h || !out) return CKF_E_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  Workspace* w = nullptr;
+  {
+    std::lock_guard<std::mutex> lk(h->mu);
+    for (auto& x : h->ws)
+      if (x.used && x.stream_tag == (void*)st) { w = &x; break; }
+  }
+  if (!w) return fail(h, CKF_E_ARG, "no ckf_find was issued on this stream");
+  unsigned long long c[CNT_N];
+  CK(cudaStreamSynchronize(st));
+  CK(cudaMemcpy(c, w->counters, sizeof(c), cudaMemcpyDeviceToHost));
+  out->tips = (int64_t)c[CNT_TIPS]; out->visits = (int64_t)c[CNT_VISITS]; out->rk_trials = (int64_t)c[CNT_TRIALS];
+  out->rk_accepted = (int64_t)c[CNT_ACCEPTED]; out->gate_tests = (int64_t)c[CNT_GATE];
+  out->updates = (int64_t)c[CNT_UPDATES]; out->links = (int64_t)c[CNT_LINKS]; out->iterations = (int64_t)c[CNT_ITER];
+  return CKF_OK;
+}
+
+int ckf_get_launch_info(const ckf_handle* h, int32_t* blocks, int32_t* threads, int32_t* smem, int32_t* regs) {
+  if (!h) return CKF_E_ARG;
+  if (blocks) *blocks = h->grid;
+  if (threads) *threads = NT;
+  if (smem) *smem = h->smem;
+  if (regs) *regs = h->regs;
+  return CKF_OK;
+}
+
+int ckf_destroy(ckf_handle* h) {
+  if (!h) return CKF_E_ARG;
+  cudaDeviceSynchronize();
+  for (auto& w : h->ws) {
+    if (w.done) cudaEventDestroy(w.done);
+    if (w.pinned_nt) cudaFreeHost(w.pinned_nt);
+  }
+  for (void* p : h->allocs) cudaFree(p);
+  delete h;
+  return CKF_OK;
+}
+
+}  // extern "C"

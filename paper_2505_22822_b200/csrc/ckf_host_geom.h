@@ -1,0 +1,43 @@
+// ckf_host_geom.h — host-side packing of ckf_geometry into the device geometry store (a1).
+#pragma once
+#include <vector>
+
+#include "../../include/ckf.h"
+#include "ckf_math.cuh"
+
+namespace ckf {
+
+inline void build_geometry_records(const ckf_geometry& g, std::vector<ModuleRec>& mods, std::vector<LayerRec>& layers) {
+  layers.resize(g.n_layers);
+  for (int l = 0; l < g.n_layers; ++l) {
+    LayerRec& L = layers[l];
+    L.r = g.layer_r[l];
+    L.half_z = g.layer_half_z[l];
+    L.n_phi = g.n_phi[l];
+    L.n_z = g.n_z[l];
+    L.offset = g.module_offset[l];
+    L.len_z = 2.0 * g.half_v[g.module_offset[l]];
+    L.pad = 0;
+  }
+  mods.resize(g.n_modules);
+  int l = 0;
+  for (int id = 0; id < g.n_modules; ++id) {
+    while (l + 1 < g.n_layers && id >= g.module_offset[l + 1]) ++l;
+    ModuleRec& m = mods[id];
+    for (int i = 0; i < 3; ++i) {
+      m.c[i] = g.center[3 * id + i];
+      m.u[i] = g.axis_u[3 * id + i];
+      m.v[i] = g.axis_v[3 * id + i];
+    }
+    m.n[0] = m.u[1] * m.v[2] - m.u[2] * m.v[1];
+    m.n[1] = m.u[2] * m.v[0] - m.u[0] * m.v[2];
+    m.n[2] = m.u[0] * m.v[1] - m.u[1] * m.v[0];
+    m.half_u = g.half_u[id];
+    m.half_v = g.half_v[id];
+    m.xx0 = g.x_over_x0[id];
+    m.layer = l;
+    m.iphi = (id - g.module_offset[l]) / g.n_z[l];
+  }
+}
+
+}  // namespace ckf

@@ -1,0 +1,68 @@
+"""Comparison of CUDA-path candidates with the oracle's (metric definitions: Table 1 caption —
+patterns match iff all measurements are identical; parameters by maximum relative difference; A15)."""
+import numpy as np
+
+FLOOR = np.array([1.0, 1.0, 1.0, 1.0, 0.0, 1.0])   # mm, mm, rad, rad, (none for q/p), mm
+
+
+def param_rel_diff(a, b):
+    """A15: |a-b| / max(|a|, |b|, floor); angles compared after wrapping the difference."""
+    d = a - b
+    d[..., 2] = (d[..., 2] + np.pi) % (2 * np.pi) - np.pi
+    den = np.maximum(np.maximum(np.abs(a), np.abs(b)), FLOOR)
+    return np.abs(d) / den
+
+
+def assert_bit_exact_lists(gpu, ora):
+    assert gpu.n_tracks == ora.n_tracks, (gpu.n_tracks, ora.n_tracks)
+    assert np.array_equal(gpu.seed_id, ora.seed_id)
+    assert np.array_equal(gpu.track_offsets, ora.track_offsets)
+    assert np.array_equal(gpu.meas_idx, ora.meas_idx)
+    assert np.array_equal(gpu.n_holes, ora.n_holes)
+    assert np.array_equal(gpu.stop_reason, ora.stop_reason)
+    assert np.array_equal(gpu.last_module, ora.last_module)
+
+
+def max_param_diffs(gpu, ora):
+    rel = param_rel_diff(gpu.params.copy(), ora.params.copy())
+    chi2 = np.abs(gpu.chi2_sum - ora.chi2_sum)
+    scale = np.sqrt(np.abs(ora.cov[:, [0, 7, 14, 21, 28, 35]]))
+    sc = (scale[:, :, None] * scale[:, None, :]).reshape(-1, 36)
+    cov = np.abs(gpu.cov - ora.cov) / np.maximum(sc, 1e-300)
+    return float(rel.max(initial=0.0)), float(chi2.max(initial=0.0)), float(cov.max(initial=0.0))
+
+
+def by_seed(tr):
+    """seed -> {tuple(meas list): track index}"""
+    out = {}
+    for t in range(tr.n_tracks):
+        out.setdefault(int(tr.seed_id[t]), {})[tuple(int(i) for i in tr.meas_list(t))] = t
+    return out
+
+
+def compare_fp32(gpu, ora, n_seeds):
+    """Returns dict: frac_identical seeds, mismatching seed ids, max param rel diff / chi2 abs diff on matched tracks."""
+    g, o = by_seed(gpu), by_seed(ora)
+    bad = []
+    gi, oi = [], []
+    for s in range(n_seeds):
+        gs, os_ = g.get(s, {}), o.get(s, {})
+        if set(gs) != set(os_):
+            bad.append(s)
+        for k in set(gs) & set(os_):
+            gi.append(gs[k])
+            oi.append(os_[k])
+    gi, oi = np.array(gi, int), np.array(oi, int)
+    rel = param_rel_diff(gpu.params[gi].copy(), ora.params[oi].copy()) if gi.size else np.zeros((0, 6))
+    chi2 = np.abs(gpu.chi2_sum[gi] - ora.chi2_sum[oi]) if gi.size else np.zeros(0)
+    # per-entry chi2 on matched tracks
+    emax = 0.0
+    for a, b in zip(gi[:20000], oi[:20000]):
+        ea = gpu.entry_chi2[gpu.track_offsets[a]:gpu.track_offsets[a + 1]]
+        eb = ora.entry_chi2[ora.track_offsets[b]:ora.track_offsets[b + 1]]
+        if ea.size:
+            emax = max(emax, float(np.max(np.abs(ea - eb))))
+    return dict(frac_identical=1.0 - len(bad) / max(1, n_seeds), bad_seeds=bad, n_matched=int(gi.size),
+                max_param_rel=float(rel.max(initial=0.0)), max_chi2_sum_abs=float(chi2.max(initial=0.0)),
+                max_entry_chi2_abs=emax,
+                table1=[float(np.mean(rel.max(axis=1) <= tol)) if gi.size else 1.0 for tol in (1e-4, 1e-3, 1e-2, 5e-2)])

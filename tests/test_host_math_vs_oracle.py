@@ -1,0 +1,71 @@
+"""GPU-less check of the CUDA path's per-tip arithmetic (csrc/ckf_math.cuh, ckf_nav.cuh compiled for the host by
+tests/hostcheck) against the oracle: every surface-to-surface move and every update along config 0 / config 2
+tracks.  The kernels inline exactly these functions; the -m gpu tests then check the orchestration."""
+import numpy as np
+import pytest
+
+import oracle
+import synth
+from tests.hostcheck import HostMath
+
+
+def _rel(a, b, floor):
+    return np.abs(a - b) / np.maximum(np.maximum(np.abs(a), np.abs(b)), floor)
+
+
+@pytest.mark.parametrize("config,precision,tol_x,tol_c", [(0, 64, 1e-10, 1e-9), (2, 64, 1e-10, 1e-9),
+                                                          (2, 32, 1e-9, 2e-5)])
+def test_moves_and_updates_match_oracle(config, precision, tol_x, tol_c):
+    det, fld, cfg = synth.config_bundle(config)
+    ev = synth.make_event(config, det=det, n_particles=60, n_fake_seeds=0)
+    st = oracle.Setup(det, fld, cfg.ckf)
+    hm = HostMath(det, fld, cfg.ckf)
+    floor_x = np.array([1.0, 1.0, 1.0, 1.0, 0.0, 1.0])
+    n_moves = n_upd = 0
+    for s in range(ev.n_seeds):
+        x = ev.seed_params[s].astype(np.float64)
+        Cm = ev.seed_cov[s].reshape(6, 6).astype(np.float64)
+        m = int(ev.seed_module[s])
+        truth = np.nonzero(ev.meas_particle == ev.seed_particle[s])[0]
+        for level in range(20):
+            if level > 0:
+                co, tgo, xo, Co, _ = oracle.move(st, m, x, Cm)
+                ch, tgh, xh, Ch, _ = hm.move(precision, m, x, Cm)
+                assert co == ch
+                if co != 0:
+                    break
+                assert tgo == tgh
+                fl = floor_x.copy()
+                fl[4] = abs(xo[4])
+                assert np.max(_rel(xo, xh, fl)) < tol_x
+                scale = np.sqrt(np.outer(np.diag(Co), np.diag(Co)))
+                assert np.max(np.abs(Co - Ch) / scale) < tol_c
+                n_moves += 1
+                x, Cm, m = xo, Co, tgo
+            # update with this particle's hit on the module, if any
+            hits = [i for i in truth if ev.meas_module[i] == m]
+            if hits:
+                i = hits[0]
+                loc, var = ev.loc[i].astype(np.float64), ev.var[i].astype(np.float64)
+                xu, Cu = oracle.kalman_update(x, Cm, loc, var)
+                c2 = oracle.predicted_chi2(x, Cm, loc, var)
+                xh, Ch, c2h = hm.update(precision, x, Cm, loc, var)
+                assert abs(c2 - c2h) < (1e-9 if precision == 64 else 1e-4) * max(1.0, c2)
+                fl = floor_x.copy()
+                fl[4] = abs(xu[4])
+                assert np.max(_rel(xu, xh, fl)) < (1e-12 if precision == 64 else 1e-7)
+                scale = np.sqrt(np.outer(np.diag(Cu), np.diag(Cu)))
+                assert np.max(np.abs(Cu - Ch) / scale) < (1e-9 if precision == 64 else 2e-5)
+                n_upd += 1
+                x, Cm = xu, Cu
+    assert n_moves > 400 and n_upd > 400
+
+
+def test_field_read_matches_oracle():
+    det, fld, cfg = synth.config_bundle(2)
+    st = oracle.Setup(det, fld, cfg.ckf)
+    hm = HostMath(det, fld, cfg.ckf)
+    rng = np.random.default_rng(2)
+    for _ in range(300):
+        r = rng.uniform(-1090, 1090, 3)
+        assert np.max(np.abs(oracle.field_at(st, r) - hm.field(r))) < 1e-12
