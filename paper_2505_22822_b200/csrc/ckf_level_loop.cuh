@@ -23,8 +23,7 @@ __device__ __forceinline__ int gate_tip(const KParams<T>& p, const Smem<T>& s, i
     if (k < end) {
       const auto lc = __ldg(p.loc + k);
       const auto vr = __ldg(p.var + k);
-      c2 = predicted_chi2<T>(l0, l1, C00, C01, C11, lc.x, lc.y, vr.x, vr.y);
-      pass = c2 < chi2_max;
+      pass = gate_chi2<T>(l0, l1, C00, C01, C11, lc.x, lc.y, vr.x, vr.y, chi2_max, c2);
     }
     const unsigned mask = __ballot_sync(0xffffffffu, pass);
     if (pass) {
@@ -55,8 +54,9 @@ __device__ __forceinline__ int gate_tip(const KParams<T>& p, const Smem<T>& s, i
       for (int k = beg + lane; k < end; k += 32) {
         const auto lc = __ldg(p.loc + k);
         const auto vr = __ldg(p.var + k);
-        const T c2 = predicted_chi2<T>(l0, l1, C00, C01, C11, lc.x, lc.y, vr.x, vr.y);
-        if (c2 < chi2_max && key_less<T>(last_c, last_i, c2, k) && (bi == 0x7fffffff || key_less<T>(c2, k, bc, bi))) {
+        T c2 = T(0);
+        const bool ok = gate_chi2<T>(l0, l1, C00, C01, C11, lc.x, lc.y, vr.x, vr.y, chi2_max, c2);
+        if (ok && key_less<T>(last_c, last_i, c2, k) && (bi == 0x7fffffff || key_less<T>(c2, k, bc, bi))) {
           bc = c2; bi = k;
         }
       }

@@ -182,25 +182,45 @@ CKF_HD T predicted_chi2(double l0, double l1, T C00, T C01, T C11, T m0, T m1, T
   return (r0 * r0 * S11 - T(2) * r0 * r1 * C01 + r1 * r1 * S00) / det;
 }
 
-// V3: gain-form update.  x float64 in/out, C packed upper triangle in/out.
+// V1 + V2 gate of one measurement.  T = float: a float32 pre-filter with a generous margin rejects the bulk
+// of the slice; the few survivors are re-evaluated in float64 so that the decision and the reported chi2 do
+// not carry float32 cancellation error.  T = double: one evaluation.
+template <typename T>
+CKF_HD bool gate_chi2(double l0, double l1, T C00, T C01, T C11, T m0, T m1, T v0, T v1, T chi2_max, T& chi2) {
+  const T c = predicted_chi2<T>(l0, l1, C00, C01, C11, m0, m1, v0, v1);
+  if (sizeof(T) == 8) {
+    chi2 = c;
+    return c < chi2_max;
+  }
+  if (!(c < chi2_max * T(1.01) + T(0.01))) return false;
+  const double cd = predicted_chi2<double>(l0, l1, (double)C00, (double)C01, (double)C11, (double)m0, (double)m1,
+                                           (double)v0, (double)v1);
+  chi2 = (T)cd;
+  return cd < (double)chi2_max;
+}
+
+// V3: gain-form update.  x float64 in/out, C packed upper triangle in/out (stored as T).  The arithmetic is
+// float64 in both modes: C' = C - K H C cancels two to three digits when a precise hit meets a loose
+// prediction, and the update is < 2 % of the work, so it is not worth a float32 error budget.
 template <typename T>
 CKF_HD void kalman_update(const double x[6], const T C[21], T m0, T m1, T v0, T v1, double xo[6], T Co[21]) {
-  const T r0 = (T)((double)m0 - x[0]), r1 = (T)((double)m1 - x[1]);
-  const T S00 = C[tri(0, 0)] + v0, S01 = C[tri(0, 1)], S11 = C[tri(1, 1)] + v1;
-  const T det = S00 * S11 - S01 * S01;
-  const T I00 = S11 / det, I01 = -S01 / det, I11 = S00 / det;
-  T K0[6], K1[6];
+  const double r0 = (double)m0 - x[0], r1 = (double)m1 - x[1];
+  const double S00 = (double)C[tri(0, 0)] + (double)v0, S01 = (double)C[tri(0, 1)], S11 = (double)C[tri(1, 1)] + (double)v1;
+  const double det = S00 * S11 - S01 * S01;
+  const double I00 = S11 / det, I01 = -S01 / det, I11 = S00 / det;
+  double K0[6], K1[6];
 #pragma unroll
   for (int i = 0; i < 6; ++i) {
-    K0[i] = C[tri(i, 0)] * I00 + C[tri(i, 1)] * I01;
-    K1[i] = C[tri(i, 0)] * I01 + C[tri(i, 1)] * I11;
+    K0[i] = (double)C[tri(i, 0)] * I00 + (double)C[tri(i, 1)] * I01;
+    K1[i] = (double)C[tri(i, 0)] * I01 + (double)C[tri(i, 1)] * I11;
   }
 #pragma unroll
-  for (int i = 0; i < 6; ++i) xo[i] = x[i] + (double)(K0[i] * r0 + K1[i] * r1);
+  for (int i = 0; i < 6; ++i) xo[i] = x[i] + (K0[i] * r0 + K1[i] * r1);
 #pragma unroll
   for (int i = 0; i < 6; ++i)
 #pragma unroll
-    for (int j = i; j < 6; ++j) Co[tri(i, j)] = C[tri(i, j)] - (K0[i] * C[tri(0, j)] + K1[i] * C[tri(1, j)]);
+    for (int j = i; j < 6; ++j)
+      Co[tri(i, j)] = (T)((double)C[tri(i, j)] - (K0[i] * (double)C[tri(0, j)] + K1[i] * (double)C[tri(1, j)]));
   while (xo[2] > PI_D) xo[2] -= 2.0 * PI_D;
   while (xo[2] <= -PI_D) xo[2] += 2.0 * PI_D;
 }

@@ -48,8 +48,9 @@ void update_t(const double* x, const double* C36, const double* loc, const doubl
   T C[21], Co[21];
   for (int i = 0; i < 6; ++i)
     for (int j = i; j < 6; ++j) C[tri(i, j)] = (T)C36[6 * i + j];
-  *chi2 = (double)predicted_chi2<T>(x[0], x[1], C[tri(0, 0)], C[tri(0, 1)], C[tri(1, 1)], (T)loc[0], (T)loc[1], (T)var[0],
-                                    (T)var[1]);
+  T c2 = T(0);
+  gate_chi2<T>(x[0], x[1], C[tri(0, 0)], C[tri(0, 1)], C[tri(1, 1)], (T)loc[0], (T)loc[1], (T)var[0], (T)var[1], T(1e30), c2);
+  *chi2 = (double)c2;
   kalman_update<T>(x, C, (T)loc[0], (T)loc[1], (T)var[0], (T)var[1], xo, Co);
   for (int i = 0; i < 6; ++i)
     for (int j = 0; j < 6; ++j) Co36[6 * i + j] = (double)Co[tri(i, j)];
