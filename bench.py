@@ -272,7 +272,7 @@ def main():
             "e2e": {"value": e2e_value, "unit": "seeds/s", "h2d_bytes_per_step": int(bi), "d2h_bytes_per_step": int(bo),
                     "streams": E2E_STREAMS, "events": n_e2e, "events_per_s": e2e_value / ev_last.n_seeds,
                     "how": "ckf_find_host, pinned host buffers, 4 host threads x 4 CUDA streams, wall clock"},
-            "gpu_launches": 5 * args.steps,
+            "gpu_launches": 6 * args.steps,
             "clocks": clocks,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                          "traffic": None, "kernel": "ckf_level_loop", "flop_per_launch": flop,

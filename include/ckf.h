@@ -26,7 +26,7 @@
 extern "C" {
 #endif
 
-#define CKF_ABI_VERSION 1
+#define CKF_ABI_VERSION 2
 
 /* return codes */
 #define CKF_OK 0
@@ -87,7 +87,7 @@ typedef struct {
                           The trajectory (position, direction, bound parameter vector) is float64 in both. */
   double chi2_max;     /* gate: chi2 < chi2_max (strict), 2 dof                                           */
   int32_t max_branches_per_surface; /* k best (chi2, index) passers become branches; 1..32                */
-  int32_t max_candidates_per_seed;  /* cap on leaves per seed (R10); >= 1                       */
+  int32_t max_candidates_per_seed;  /* cap on leaves per seed (R10); 1..256                     */
   int32_t max_holes;                /* a branch stops when its hole count exceeds this                   */
   int32_t min_measurements;         /* a stopped branch is emitted iff it holds at least this many       */
   double rk_tolerance_mm;           /* RKN4 local error bound per step                                   */
@@ -147,10 +147,12 @@ typedef struct {
   int64_t visits;       /* surface visits (gate evaluations of a whole module)  */
   int64_t rk_trials;    /* RKN4 trial steps                                     */
   int64_t rk_accepted;  /* accepted RKN4 steps                                  */
-  int64_t gate_tests;   /* chi2 evaluations                                     */
+  int64_t gate_tests;   /* chi2 evaluations the method defines: sum of visited slice lengths */
   int64_t updates;      /* Kalman updates                                       */
   int64_t links;        /* candidate links appended                             */
-  int64_t iterations;   /* sum over thread blocks of level-loop passes          */
+  int64_t iterations;   /* sum over warps of 32-tip chunks processed            */
+  int64_t gate_tests_executed; /* chi2 evaluations actually run: entries inside the loc0 windows
+                                  (the rest of each slice is excluded by chi2 >= r0^2/S00) */
 } ckf_counters;
 
 /* Uploads geometry and field (once, at the first event) and reserves all workspaces.

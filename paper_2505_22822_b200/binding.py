@@ -60,7 +60,8 @@ class ckf_tracks(C.Structure):
 
 class ckf_counters(C.Structure):
     _fields_ = [("tips", C.c_int64), ("visits", C.c_int64), ("rk_trials", C.c_int64), ("rk_accepted", C.c_int64),
-                ("gate_tests", C.c_int64), ("updates", C.c_int64), ("links", C.c_int64), ("iterations", C.c_int64)]
+                ("gate_tests", C.c_int64), ("updates", C.c_int64), ("links", C.c_int64), ("iterations", C.c_int64),
+                ("gate_tests_executed", C.c_int64)]
 
 
 _lib = None

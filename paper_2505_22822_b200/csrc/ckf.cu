@@ -1,7 +1,7 @@
 // ckf.cu — C ABI of the B200-native CKF track-finding library (include/ckf.h): host side.
 //
 // ckf_create uploads the geometry store (a1) and field store (a2) once and reserves every
-// workspace; ckf_find enqueues five launches on the caller's stream and never allocates.
+// workspace; ckf_find enqueues six launches on the caller's stream and never allocates.
 // There is no CPU path in this library: all arithmetic of the method runs in the kernels of
 // ckf_level_loop.cuh / ckf_emit.cuh.
 #include <cuda_runtime.h>
@@ -17,6 +17,7 @@
 #include "ckf_emit.cuh"
 #include "ckf_host_geom.h"
 #include "ckf_level_loop.cuh"
+#include "ckf_sort.cuh"
 
 using namespace ckf;
 
@@ -33,6 +34,9 @@ struct Workspace {
   int32_t *sd = nullptr;       // 3 * max_seeds + 2 * (max_seeds + 1)
   int32_t* leaf = nullptr;     // 3 * max_seeds * cap
   int2* queue = nullptr;
+  double* pred_x = nullptr; void* pred_C = nullptr; int32_t* pred_ts = nullptr;  // P1 -> P2-P4 predictions
+  void *s_loc = nullptr, *s_var = nullptr, *s_v0max = nullptr;  // gate index (ckf_sort_slices)
+  int32_t* s_idx = nullptr;
   int32_t* globals = nullptr;  // cursor, link_count, first_bad, total[2]
   unsigned long long* counters = nullptr;
   // staging for ckf_find_host
@@ -93,6 +97,14 @@ cudaError_t dalloc(ckf_handle* h, P** p, size_t bytes) {
   return e;
 }
 
+// Resident blocks per SM the level loop is compiled for: 4 x 128 threads at <= 128 registers (float),
+// 2 x 128 threads at <= 255 registers (double: the covariance algebra doubles its register footprint).
+#ifndef CKF_MINB
+#define CKF_MINB 4
+#endif
+template <typename T> struct MinBlocks { static constexpr int value = CKF_MINB; };
+template <> struct MinBlocks<double> { static constexpr int value = 2; };
+
 template <typename T>
 void fill_params(ckf_handle* h, Workspace& w, KParams<T>& p) {
   const ckf_config& c = h->cfg;
@@ -108,6 +120,9 @@ void fill_params(ckf_handle* h, Workspace& w, KParams<T>& p) {
   const size_t LC = S * (size_t)c.max_candidates_per_seed;
   p.leaf_link = w.leaf; p.leaf_meta = w.leaf + LC; p.leaf_entry = w.leaf + 2 * LC;
   p.queue = w.queue; p.qcap = h->qcap;
+  p.pred_x = w.pred_x; p.pred_C = (T*)w.pred_C; p.pred_ts = w.pred_ts;
+  p.s_loc = (typename Vec2<T>::type*)w.s_loc; p.s_var = (typename Vec2<T>::type*)w.s_var; p.s_idx = w.s_idx;
+  p.s_v0max = (T*)w.s_v0max;
   p.g_seed_cursor = w.globals; p.g_link_count = w.globals + 1; p.g_first_bad = w.globals + 2; p.g_total = w.globals + 3;
   p.counters = w.counters;
   p.max_tracks = c.max_tracks; p.max_entries = c.max_track_entries;
@@ -128,7 +143,8 @@ int launch_find(ckf_handle* h, Workspace& w, const ckf_measurements* m, const ck
   p.o_params = (T*)o->params; p.o_cov = (T*)o->cov; p.o_chi2sum = (T*)o->chi2_sum; p.o_entrychi2 = (T*)o->entry_chi2;
   const int nb = (std::max(s->n, (int)CNT_N) + 255) / 256;
   ckf_init_event<T><<<nb, 256, 0, st>>>(p);
-  ckf_level_loop<T, (sizeof(T) == 4 ? 2 : 1)><<<h->grid, NT, h->smem, st>>>(p);
+  ckf_sort_slices<T><<<h->sm_count * 8, SORT_NT, 0, st>>>(p);
+  ckf_level_loop<T, MinBlocks<T>::value><<<h->grid, NT, h->smem, st>>>(p);
   ckf_scan_seeds<T><<<1, 1024, 0, st>>>(p);
   ckf_emit_tracks<T><<<h->sm_count * 4, 256, 0, st>>>(p);
   ckf_finalize<T><<<1, 1, 0, st>>>(p);
@@ -166,10 +182,10 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
   if (!g || !f || !c || !out) return fail(h, CKF_E_ARG, "null argument");
   *out = nullptr;
   if (c->precision != 32 && c->precision != 64) return fail(h, CKF_E_ARG, "precision must be 32 or 64");
-  if (c->max_branches_per_surface < 1 || c->max_branches_per_surface > CAND)
-    return fail(h, CKF_E_ARG, "max_branches_per_surface must be in 1..%d", CAND);
-  if (c->max_candidates_per_seed < 1 || c->max_candidates_per_seed > NT)
-    return fail(h, CKF_E_ARG, "max_candidates_per_seed must be in 1..%d", NT);
+  if (c->max_branches_per_surface < 1 || c->max_branches_per_surface > 32)
+    return fail(h, CKF_E_ARG, "max_branches_per_surface must be in 1..32");
+  if (c->max_candidates_per_seed < 1 || c->max_candidates_per_seed > 256)
+    return fail(h, CKF_E_ARG, "max_candidates_per_seed must be in 1..256");
   if (c->max_levels < 1 || c->max_levels > 64) return fail(h, CKF_E_ARG, "max_levels must be in 1..64");
   if (c->min_measurements < 1) return fail(h, CKF_E_ARG, "min_measurements must be >= 1");
   if (c->max_seeds < 1 || c->max_measurements < 0 || c->max_tracks < 1 || c->max_track_entries < 1 || c->n_streams < 1)
@@ -236,24 +252,24 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
   h->kcfg.h_max = c->h_max_mm; h->kcfg.mass = c->particle_mass_gev; h->kcfg.max_branches = c->max_branches_per_surface;
   h->kcfg.max_cands = c->max_candidates_per_seed; h->kcfg.max_holes = c->max_holes; h->kcfg.min_meas = c->min_measurements;
   h->kcfg.max_rk_steps = c->max_rk_steps_per_surface; h->kcfg.max_levels = c->max_levels;
-  // ---- launch configuration of the level loop: one wave of resident blocks
+  // ---- launch configuration of the level loop: one wave of resident blocks, WPB autonomous warps each
   int per_sm = 0;
   cudaFuncAttributes fa;
   if (c->precision == 32) {
-    h->smem = (int)Smem<float>::bytes(c->max_branches_per_surface);
-    CKB(cudaFuncSetAttribute(ckf_level_loop<float, 2>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem));
-    CKB(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ckf_level_loop<float, 2>, NT, h->smem));
-    CKB(cudaFuncGetAttributes(&fa, ckf_level_loop<float, 2>));
+    h->smem = (int)(WPB * WSmem<float>::bytes(c->max_branches_per_surface));
+    CKB(cudaFuncSetAttribute(ckf_level_loop<float, MinBlocks<float>::value>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem));
+    CKB(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ckf_level_loop<float, MinBlocks<float>::value>, NT, h->smem));
+    CKB(cudaFuncGetAttributes(&fa, ckf_level_loop<float, MinBlocks<float>::value>));
   } else {
-    h->smem = (int)Smem<double>::bytes(c->max_branches_per_surface);
-    CKB(cudaFuncSetAttribute(ckf_level_loop<double, 1>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem));
-    CKB(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ckf_level_loop<double, 1>, NT, h->smem));
-    CKB(cudaFuncGetAttributes(&fa, ckf_level_loop<double, 1>));
+    h->smem = (int)(WPB * WSmem<double>::bytes(c->max_branches_per_surface));
+    CKB(cudaFuncSetAttribute(ckf_level_loop<double, MinBlocks<double>::value>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem));
+    CKB(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ckf_level_loop<double, MinBlocks<double>::value>, NT, h->smem));
+    CKB(cudaFuncGetAttributes(&fa, ckf_level_loop<double, MinBlocks<double>::value>));
   }
   if (per_sm < 1) { fail(h, CKF_E_CUDA, "level-loop kernel does not fit on an SM (smem %d B)", h->smem); return bail(CKF_E_CUDA); }
   h->regs = fa.numRegs;
   h->grid = per_sm * h->sm_count;
-  h->qcap = NT * c->max_candidates_per_seed;
+  h->qcap = MAX_LIVE_SEEDS * c->max_candidates_per_seed;
   // ---- workspaces
   const size_t L = (size_t)h->cfg.max_links, S = (size_t)c->max_seeds, ts = (size_t)h->tsize;
   h->ws.resize(c->n_streams);
@@ -265,7 +281,14 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     CKB(dalloc(h, (char**)&w.lk_chi2, L * ts)); CKB(dalloc(h, (char**)&w.lk_chi2sum, L * ts));
     CKB(dalloc(h, &w.sd, (3 * S + 2 * (S + 1)) * 4));
     CKB(dalloc(h, &w.leaf, 3 * S * (size_t)c->max_candidates_per_seed * 4));
-    CKB(dalloc(h, &w.queue, (size_t)h->grid * 2 * h->qcap * sizeof(int2)));
+    CKB(dalloc(h, &w.queue, (size_t)h->grid * WPB * 2 * h->qcap * sizeof(int2)));
+    CKB(dalloc(h, &w.pred_x, (size_t)h->grid * WPB * 6 * SUBW * sizeof(double)));
+    CKB(dalloc(h, (char**)&w.pred_C, (size_t)h->grid * WPB * 21 * SUBW * ts));
+    CKB(dalloc(h, &w.pred_ts, (size_t)h->grid * WPB * 2 * SUBW * 4));
+    CKB(dalloc(h, (char**)&w.s_loc, 2 * (size_t)c->max_measurements * ts));
+    CKB(dalloc(h, (char**)&w.s_var, 2 * (size_t)c->max_measurements * ts));
+    CKB(dalloc(h, &w.s_idx, (size_t)c->max_measurements * 4));
+    CKB(dalloc(h, (char**)&w.s_v0max, (size_t)g->n_modules * ts));
     CKB(dalloc(h, &w.globals, 16 * 4));
     CKB(dalloc(h, &w.counters, CNT_N * 8));
     CKB(cudaEventCreateWithFlags(&w.done, cudaEventDisableTiming));
@@ -363,6 +386,7 @@ int ckf_get_counters(ckf_handle* h, void* stream, ckf_counters* out) {
   out->tips = (int64_t)c[CNT_TIPS]; out->visits = (int64_t)c[CNT_VISITS]; out->rk_trials = (int64_t)c[CNT_TRIALS];
   out->rk_accepted = (int64_t)c[CNT_ACCEPTED]; out->gate_tests = (int64_t)c[CNT_GATE];
   out->updates = (int64_t)c[CNT_UPDATES]; out->links = (int64_t)c[CNT_LINKS]; out->iterations = (int64_t)c[CNT_ITER];
+  out->gate_tests_executed = (int64_t)c[CNT_GATE_EXEC];
   return CKF_OK;
 }
 

@@ -20,6 +20,10 @@
 #define CKF_HD inline
 #endif
 
+#ifndef CKF_JAC_ROLLED
+#define CKF_JAC_ROLLED 0
+#endif
+
 namespace ckf {
 
 constexpr double KAPPA = 2.99792458e-4;  // GeV / (T mm)
@@ -149,69 +153,96 @@ CKF_HD void jac_identity(Jac<T>& J) {
 CKF_HD double inv_beta(double qop, double mass) { return sqrt(1.0 + mass * mass * qop * qop); }
 CKF_HD double dinvbeta_dqop(double qop, double mass) { return mass * mass * qop / sqrt(1.0 + mass * mass * qop * qop); }
 
-// One RKN4 trial (P2): the four stage cross products cr_i (k_i = lam * cr_i), the three field values and the
-// error estimate eps = h^2 |k1 - k2 - k3 + k4| (P3).
+// One RKN4 trial (P2, P3).  What survives the trial is only what an accepted step needs, in the type it needs
+// it in (keeps the live register set of the hot loop small): the three field values and the four
+// q/p-derivative vectors kappa * cr_i as T for the Jacobian columns, the two stage sums
+// s1 = k1 + k2 + k3, s2 = k1 + 2 k2 + 2 k3 + k4 (k_i = lam * cr_i) for the state, and the error estimate
+// eps = h^2 |k1 - k2 - k3 + k4|.
+template <typename T>
 struct Trial {
-  double cr1[3], cr2[3], cr3[3], cr4[3];
-  double B1[3], B2[3], B4[3];
+  T B1[3], B2[3], B4[3];
+  T q1[3], q2[3], q3[3], q4[3];
+  double s1[3], s2[3];
   double eps;
 };
 
-CKF_HD void rk_trial(const FieldDev& fld, const Traj& y, double lam, double h, Trial& t) {
-  double w[3], p[3];
-  field_at(fld, y.r, t.B1);
-  cross3(y.d, t.B1, t.cr1);
-  const double h2 = 0.5 * h, h8 = h * h * 0.125;
+template <typename T>
+CKF_HD void rk_trial(const FieldDev& fld, const Traj& y, double lam, double h, Trial<T>& t) {
+  // The three field reads share ONE inlined copy of field_at (a rolled stage loop): the trial is the hot
+  // loop of the whole path and must stay small enough for the SM's instruction cache.
+  const double h2 = 0.5 * h, h8 = h * h * 0.125, hh2 = h * h * 0.5;
+  double cr1[3], cr2[3], cr3[3], cr4[3];
+#pragma unroll 1
+  for (int st = 0; st < 3; ++st) {
+    double p[3], B[3], w[3];
+    if (st == 0) {
 #pragma unroll
-  for (int i = 0; i < 3; ++i) p[i] = y.r[i] + h2 * y.d[i] + h8 * (lam * t.cr1[i]);
-  field_at(fld, p, t.B2);
+      for (int i = 0; i < 3; ++i) p[i] = y.r[i];
+    } else if (st == 1) {
 #pragma unroll
-  for (int i = 0; i < 3; ++i) w[i] = y.d[i] + h2 * (lam * t.cr1[i]);
-  cross3(w, t.B2, t.cr2);
+      for (int i = 0; i < 3; ++i) p[i] = y.r[i] + h2 * y.d[i] + h8 * (lam * cr1[i]);
+    } else {
 #pragma unroll
-  for (int i = 0; i < 3; ++i) w[i] = y.d[i] + h2 * (lam * t.cr2[i]);
-  cross3(w, t.B2, t.cr3);
-  const double hh2 = h * h * 0.5;
+      for (int i = 0; i < 3; ++i) p[i] = y.r[i] + h * y.d[i] + hh2 * (lam * cr3[i]);
+    }
+    field_at(fld, p, B);
+    if (st == 0) {
 #pragma unroll
-  for (int i = 0; i < 3; ++i) p[i] = y.r[i] + h * y.d[i] + hh2 * (lam * t.cr3[i]);
-  field_at(fld, p, t.B4);
+      for (int i = 0; i < 3; ++i) t.B1[i] = (T)B[i];
+      cross3(y.d, B, cr1);
+    } else if (st == 1) {
 #pragma unroll
-  for (int i = 0; i < 3; ++i) w[i] = y.d[i] + h * (lam * t.cr3[i]);
-  cross3(w, t.B4, t.cr4);
+      for (int i = 0; i < 3; ++i) { t.B2[i] = (T)B[i]; w[i] = y.d[i] + h2 * (lam * cr1[i]); }
+      cross3(w, B, cr2);
+#pragma unroll
+      for (int i = 0; i < 3; ++i) w[i] = y.d[i] + h2 * (lam * cr2[i]);
+      cross3(w, B, cr3);
+    } else {
+#pragma unroll
+      for (int i = 0; i < 3; ++i) { t.B4[i] = (T)B[i]; w[i] = y.d[i] + h * (lam * cr3[i]); }
+      cross3(w, B, cr4);
+    }
+  }
   double e2 = 0.0;
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
-    const double e = lam * t.cr1[i] - lam * t.cr2[i] - lam * t.cr3[i] + lam * t.cr4[i];
+    const double k1 = lam * cr1[i], k2 = lam * cr2[i], k3 = lam * cr3[i], k4 = lam * cr4[i];
+    const double e = k1 - k2 - k3 + k4;
     e2 += e * e;
+    t.s1[i] = k1 + k2 + k3;
+    t.s2[i] = k1 + 2.0 * k2 + 2.0 * k3 + k4;
+    t.q1[i] = (T)(KAPPA * cr1[i]); t.q2[i] = (T)(KAPPA * cr2[i]);
+    t.q3[i] = (T)(KAPPA * cr3[i]); t.q4[i] = (T)(KAPPA * cr4[i]);
   }
   t.eps = h * h * sqrt(e2);
 }
 
 // J2 applied to one column (dr, dd) of the running Jacobian: the linearised RKN4 step with h fixed and the
-// field gradient neglected.  WITH_Q adds the explicit q/p dependence kappa * cr_i (the q-column).
-template <typename T, bool WITH_Q>
-CKF_HD void jac_column(T lam, T h, const T B1[3], const T B2[3], const T B4[3], const T q1[3], const T q2[3],
-                       const T q3[3], const T q4[3], T dr[3], T dd[3]) {
+// field gradient neglected.  qf = 1 adds the explicit q/p dependence kappa * cr_i (the q-column), qf = 0 does
+// not (adding qf * q = +0 leaves the d-columns' values unchanged).
+template <typename T>
+CKF_HD void jac_column_q(T lam, T h, T qf, const T B1[3], const T B2[3], const T B4[3], const T q1[3], const T q2[3],
+                         const T q3[3], const T q4[3], T dr[3], T dd[3]) {
   T k1[3], k2[3], k3[3], k4[3], w[3];
   const T h2 = T(0.5) * h;
   cross3(dd, B1, k1);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) k1[i] = WITH_Q ? lam * k1[i] + q1[i] : lam * k1[i];
+  for (int i = 0; i < 3; ++i) k1[i] = lam * k1[i] + qf * q1[i];
 #pragma unroll
   for (int i = 0; i < 3; ++i) w[i] = dd[i] + h2 * k1[i];
   cross3(w, B2, k2);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) k2[i] = WITH_Q ? lam * k2[i] + q2[i] : lam * k2[i];
+  for (int i = 0; i < 3; ++i) k2[i] = lam * k2[i] + qf * q2[i];
 #pragma unroll
   for (int i = 0; i < 3; ++i) w[i] = dd[i] + h2 * k2[i];
   cross3(w, B2, k3);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) k3[i] = WITH_Q ? lam * k3[i] + q3[i] : lam * k3[i];
+  for (int i = 0; i < 3; ++i) k3[i] = lam * k3[i] + qf * q3[i];
 #pragma unroll
   for (int i = 0; i < 3; ++i) w[i] = dd[i] + h * k3[i];
   cross3(w, B4, k4);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) k4[i] = WITH_Q ? lam * k4[i] + q4[i] : lam * k4[i];
+  for (int i = 0; i < 3; ++i) k4[i] = lam * k4[i] + qf * q4[i];
   const T h6 = h * T(1.0 / 6.0), hh6 = h * h * T(1.0 / 6.0);
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
@@ -220,36 +251,44 @@ CKF_HD void jac_column(T lam, T h, const T B1[3], const T B2[3], const T B4[3], 
   }
 }
 
-// Accept a trial: D <- D_step D column by column (J2, J3), then the state (P2).
+// Accept a trial: D <- D_step D column by column (J2, J3), then the state (P2).  The four columns go through
+// ONE copy of the column code: a rolled loop that rotates the columns through fixed registers.
 template <typename T>
-CKF_HD void rk_accept(Traj& y, Jac<T>& J, double lam, double h, const Trial& t, double mass) {
+CKF_HD void rk_accept(Traj& y, Jac<T>& J, double h, const Trial<T>& t, double mass) {
   {
-    T B1[3], B2[3], B4[3], q1[3], q2[3], q3[3], q4[3];
+    const T lamT = (T)(KAPPA * y.qop), hT = (T)h;
+#if CKF_JAC_ROLLED
+    // rotation: after 4 rounds every column is back in its place
+#pragma unroll 1
+    for (int c = 0; c < 4; ++c) {
+      T dr[3] = {J.Rd[0][0], J.Rd[1][0], J.Rd[2][0]};
+      T dd[3] = {J.Dd[0][0], J.Dd[1][0], J.Dd[2][0]};
+      jac_column_q<T>(lamT, hT, c == 3 ? T(1) : T(0), t.B1, t.B2, t.B4, t.q1, t.q2, t.q3, t.q4, dr, dd);
 #pragma unroll
-    for (int i = 0; i < 3; ++i) {
-      B1[i] = (T)t.B1[i]; B2[i] = (T)t.B2[i]; B4[i] = (T)t.B4[i];
-      q1[i] = (T)(KAPPA * t.cr1[i]); q2[i] = (T)(KAPPA * t.cr2[i]);
-      q3[i] = (T)(KAPPA * t.cr3[i]); q4[i] = (T)(KAPPA * t.cr4[i]);
+      for (int i = 0; i < 3; ++i) {
+        J.Rd[i][0] = J.Rd[i][1]; J.Rd[i][1] = J.Rd[i][2]; J.Rd[i][2] = J.rq[i]; J.rq[i] = dr[i];
+        J.Dd[i][0] = J.Dd[i][1]; J.Dd[i][1] = J.Dd[i][2]; J.Dd[i][2] = J.dq[i]; J.dq[i] = dd[i];
+      }
     }
-    const T lamT = (T)lam, hT = (T)h;
+#else
 #pragma unroll
     for (int j = 0; j < 3; ++j) {
       T dr[3] = {J.Rd[0][j], J.Rd[1][j], J.Rd[2][j]};
       T dd[3] = {J.Dd[0][j], J.Dd[1][j], J.Dd[2][j]};
-      jac_column<T, false>(lamT, hT, B1, B2, B4, q1, q2, q3, q4, dr, dd);
+      jac_column_q<T>(lamT, hT, T(0), t.B1, t.B2, t.B4, t.q1, t.q2, t.q3, t.q4, dr, dd);
 #pragma unroll
       for (int i = 0; i < 3; ++i) { J.Rd[i][j] = dr[i]; J.Dd[i][j] = dd[i]; }
     }
-    jac_column<T, true>(lamT, hT, B1, B2, B4, q1, q2, q3, q4, J.rq, J.dq);
+    jac_column_q<T>(lamT, hT, T(1), t.B1, t.B2, t.B4, t.q1, t.q2, t.q3, t.q4, J.rq, J.dq);
+#endif
     J.tq += (T)(h * dinvbeta_dqop(y.qop, mass));
   }
   const double h6 = h / 6.0, hh6 = h * h / 6.0;
   double dn[3], n2 = 0.0;
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
-    const double k1 = lam * t.cr1[i], k2 = lam * t.cr2[i], k3 = lam * t.cr3[i], k4 = lam * t.cr4[i];
-    y.r[i] = y.r[i] + h * y.d[i] + hh6 * (k1 + k2 + k3);
-    dn[i] = y.d[i] + h6 * (k1 + 2.0 * k2 + 2.0 * k3 + k4);
+    y.r[i] = y.r[i] + h * y.d[i] + hh6 * t.s1[i];
+    dn[i] = y.d[i] + h6 * t.s2[i];
     n2 += dn[i] * dn[i];
   }
   const double nrm = sqrt(n2);
@@ -273,72 +312,11 @@ CKF_HD void straight_close(Traj& y, Jac<T>& J, double s, double mass) {
   y.t += s * inv_beta(y.qop, mass);
 }
 
-// ------------------------------------------------------------------------------------------ P4: targets
-struct Target {
-  int kind;  // 0 plane (c, n), 1 cylinder R
-  double c[3], n[3], R;
-};
-
-CKF_HD bool target_distance(const Target& tg, const Traj& y, double& s, int& why) {
-  if (tg.kind == 0) {
-    const double dn = dot3(y.d, tg.n);
-    if (!(fabs(dn) > 1e-12)) { why = STOP_NUMERIC; return false; }
-    const double rel[3] = {tg.c[0] - y.r[0], tg.c[1] - y.r[1], tg.c[2] - y.r[2]};
-    s = dot3(rel, tg.n) / dn;
-    return true;
-  }
-  const double a = y.d[0] * y.d[0] + y.d[1] * y.d[1];
-  const double b = y.r[0] * y.d[0] + y.r[1] * y.d[1];
-  const double cc = y.r[0] * y.r[0] + y.r[1] * y.r[1] - tg.R * tg.R;
-  const double disc = b * b - a * cc;
-  if (!(b > 0.0) || !(disc >= 0.0)) { why = STOP_NOT_OUTGOING; return false; }
-  s = -cc / (b + sqrt(disc));
-  return true;
-}
-
+// ------------------------------------------------------------------------------------------ step control
 struct StepCtl {
   double h_ctrl;
   int n_steps;
   int n_trials, n_accepted;  // work counters
 };
-
-// P3-P6: adaptive stepping until the target is reached.
-template <typename T>
-CKF_HD int propagate_to(const FieldDev& fld, const CfgDev& cfg, const Target& tg, Traj& y, Jac<T>& J, StepCtl& sc) {
-  const double lam = KAPPA * y.qop;
-  for (;;) {
-    double s;
-    int why = STOP_NUMERIC;
-    if (!target_distance(tg, y, s, why)) return why;
-    if (!isfinite(s)) return STOP_NUMERIC;
-    if (fabs(s) <= cfg.surf_tol) {
-      straight_close(y, J, s, cfg.mass);
-      return STOP_NONE;
-    }
-    const double hlim = fmin(sc.h_ctrl, cfg.h_max);
-    double h = (fabs(s) <= hlim) ? s : (s > 0.0 ? hlim : -hlim);
-    for (;;) {
-      if (++sc.n_steps > cfg.max_rk_steps) return STOP_STEP_LIMIT;
-      Trial t;
-      rk_trial(fld, y, lam, h, t);
-      ++sc.n_trials;
-      if (!isfinite(t.eps)) return STOP_NUMERIC;
-      double f;
-      if (t.eps == 0.0) f = 4.0;
-      else {
-        f = 0.9 * sqrt(sqrt(cfg.rk_tol / t.eps));
-        f = f < 0.25 ? 0.25 : f;
-        f = f > 4.0 ? 4.0 : f;
-      }
-      if (t.eps <= cfg.rk_tol) {
-        rk_accept(y, J, lam, h, t, cfg.mass);
-        sc.h_ctrl = fabs(h) * f;
-        ++sc.n_accepted;
-        break;
-      }
-      h = h * f;
-    }
-  }
-}
 
 }  // namespace ckf

@@ -28,7 +28,8 @@ CKF_HD bool line_hits_module(const ModuleRec& k, const double r[3], const double
   return true;
 }
 
-// Nearest in-bounds module of the 3x3 neighbourhood (phi wraps, z clamps) of (iphi, iz) on `layer`.
+// Nearest in-bounds module of the 3x3 neighbourhood (phi wraps, z clamps) of (iphi, iz) on `layer`: the
+// sequential form (host harness).  The kernel evaluates the same nine tests cooperatively, see pick_warp.
 CKF_HD int pick_in_neighbourhood(const GeoDev& g, int layer, int iphi, int iz, int exclude, const double r[3],
                                  const double d[3], double s_min) {
   const LayerRec L = g.layer[layer];
@@ -226,100 +227,203 @@ CKF_HD void kalman_update(const double x[6], const T C[21], T m0, T m1, T v0, T 
 }
 
 // ------------------------------------------------------------------------------------------ one move (step A)
-// From bound x on module `from` to the next module: N2-N5 with P and J.  Outputs the target module, the
-// predicted bound parameters, the 5x5 Jacobian block and the Highland variances to add to C[phi][phi],
-// C[theta][theta] before transport (V5, applied on leaving).  Work counters in sc.
+// From bound x on module `from` to the next module: N2-N5 with P and J, as a per-tip state machine whose
+// transitions are small functions.  The kernel (ckf_level_loop.cuh) keeps one Move per lane and calls the
+// transitions at warp-wide service points: lanes fetch new tips, pick modules, run RKN4 trials and do the
+// arrival algebra together, so every heavy piece of code runs converged.  The host test harness drives the
+// very same transitions one tip at a time (move_to_next_module below) against the oracle.
+//
+//   START --pick--> PLANE | CYL | FIN(EXIT)         N2 overlap neighbour, else next layer's cylinder
+//   CYL   --step--> CYL (one RKN4 trial) | LANDED    P3-P5 toward the portal cylinder of layer lp
+//   LANDED--pick--> PLANE | CYL | FIN(EXIT)         N3/N4 module choice at the portal; a crack is not a hole
+//   PLANE --step--> PLANE (one trial) | FIN          N5 toward the target module's plane
+//   FIN   --arrive-> predicted bound parameters + 5x5 Jacobian block (J4, J5)
+enum MovePhase : int { PH_IDLE = 0, PH_START = 1, PH_CYL = 2, PH_LANDED = 3, PH_PLANE = 4, PH_FIN = 5 };
+
+template <typename T>
+struct Move {
+  Traj y;
+  Jac<T> D;
+  T dep_d[3];           // direction on departure (J1)
+  T q_phi, q_theta;     // Highland variances to add before transport (V5)
+  double tc[3], tn[3];  // target plane (PH_PLANE)
+  double R;             // target cylinder radius (PH_CYL)
+  double h, h_ctrl;
+  int phase, stop, from, tgt, lp, n_steps;
+  bool retry;
+};
+
+// Validation + departure state.  Leaves the move in PH_START, or PH_FIN with stop = NUMERIC.
+template <typename T>
+CKF_HD void move_init(Move<T>& m, const GeoDev& g, const CfgDev& cfg, int from, const double x[6]) {
+  m.from = from; m.tgt = -1; m.lp = 0; m.n_steps = 0; m.retry = false; m.stop = STOP_NONE;
+  m.h = 0.0; m.h_ctrl = cfg.h_max; m.R = 0.0;
+  m.q_theta = T(0); m.q_phi = T(0);
+  m.y.qop = 0.0;
+  bool ok = true;
+#pragma unroll
+  for (int i = 0; i < 6; ++i) ok = ok && isfinite(x[i]);
+  ok = ok && (x[3] > 0.0 && x[3] < PI_D);
+  if (!ok) { m.stop = STOP_NUMERIC; m.phase = PH_FIN; return; }
+  const ModuleRec& k = g.mod[from];
+  double sp, cp, st, ct;
+  sincos(x[2], &sp, &cp);
+  sincos(x[3], &st, &ct);
+  m.y.d[0] = st * cp; m.y.d[1] = st * sp; m.y.d[2] = ct;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    m.y.r[i] = k.c[i] + x[0] * k.u[i] + x[1] * k.v[i];
+    m.dep_d[i] = (T)m.y.d[i];
+  }
+  m.y.t = x[5];
+  m.y.qop = x[4];
+  if (k.xx0 > 0.0) {
+    const double th2 = highland_theta0_sq(k.xx0, fabs(dot3(m.y.d, k.n)), m.y.qop, cfg.mass);
+    m.q_theta = (T)th2;
+    m.q_phi = (T)(th2 / (st * st));
+  }
+  jac_identity(m.D);
+  m.phase = PH_START;
+}
+
+// The 3x3 neighbourhood a move in PH_START / PH_LANDED wants tested.  Returns false when no module can be
+// picked (portal point beyond the layer's half length).
+struct PickRequest {
+  int layer, iphi, iz, exclude;
+  double s_min;
+};
+template <typename T>
+CKF_HD bool move_pick_request(const Move<T>& m, const GeoDev& g, PickRequest& q) {
+  if (m.phase == PH_START) {
+    const ModuleRec& k = g.mod[m.from];
+    q.layer = k.layer; q.iphi = k.iphi;
+    q.iz = m.from - g.layer[k.layer].offset - k.iphi * g.layer[k.layer].n_z;
+    q.exclude = m.from; q.s_min = 1e-3;
+    return true;
+  }
+  const LayerRec L = g.layer[m.lp];
+  q.layer = m.lp; q.exclude = -1; q.s_min = -1e-3; q.iphi = 0; q.iz = 0;
+  if (fabs(m.y.r[2]) > L.half_z) return false;
+  const double phix = atan2(m.y.r[1], m.y.r[0]);
+  const int i = (int)nearbyint(phix * L.n_phi / (2.0 * PI_D));
+  q.iphi = ((i % L.n_phi) + L.n_phi) % L.n_phi;
+  const int j = (int)floor((m.y.r[2] + L.half_z) / L.len_z);
+  q.iz = j < 0 ? 0 : (j > L.n_z - 1 ? L.n_z - 1 : j);
+  return true;
+}
+
+// Result of the pick (module id or -1) -> next phase.
+template <typename T>
+CKF_HD void move_pick_apply(Move<T>& m, const GeoDev& g, int tgt) {
+  if (tgt >= 0) {
+    const ModuleRec& k = g.mod[tgt];
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { m.tc[i] = k.c[i]; m.tn[i] = k.n[i]; }
+    m.tgt = tgt;
+    m.phase = PH_PLANE;
+    return;
+  }
+  m.lp = (m.phase == PH_START) ? g.mod[m.from].layer + 1 : m.lp + 1;
+  if (m.lp >= g.n_layers) { m.stop = STOP_EXIT; m.phase = PH_FIN; return; }
+  m.R = g.layer[m.lp].r;
+  m.phase = PH_CYL;
+}
+
+// One step of a move in PH_CYL / PH_PLANE: targeting + landing (P4, P5), else one RKN4 trial (P2, P3).
+template <typename T>
+CKF_HD void move_step(Move<T>& m, const FieldDev& fld, const CfgDev& cfg, int& n_trials, int& n_accepted) {
+  if (!m.retry) {
+    double s;
+    if (m.phase == PH_PLANE) {
+      const double dn = dot3(m.y.d, m.tn);
+      if (!(fabs(dn) > 1e-12)) { m.stop = STOP_NUMERIC; m.phase = PH_FIN; return; }
+      const double rel[3] = {m.tc[0] - m.y.r[0], m.tc[1] - m.y.r[1], m.tc[2] - m.y.r[2]};
+      s = dot3(rel, m.tn) / dn;
+    } else {
+      const double a = m.y.d[0] * m.y.d[0] + m.y.d[1] * m.y.d[1];
+      const double b = m.y.r[0] * m.y.d[0] + m.y.r[1] * m.y.d[1];
+      const double cc = m.y.r[0] * m.y.r[0] + m.y.r[1] * m.y.r[1] - m.R * m.R;
+      const double disc = b * b - a * cc;
+      if (!(b > 0.0) || !(disc >= 0.0)) { m.stop = STOP_NOT_OUTGOING; m.phase = PH_FIN; return; }
+      s = -cc / (b + sqrt(disc));
+    }
+    if (!isfinite(s)) { m.stop = STOP_NUMERIC; m.phase = PH_FIN; return; }
+    if (fabs(s) <= cfg.surf_tol) {
+      straight_close(m.y, m.D, s, cfg.mass);  // P5
+      m.phase = (m.phase == PH_PLANE) ? PH_FIN : PH_LANDED;
+      return;
+    }
+    const double hlim = fmin(m.h_ctrl, cfg.h_max);  // P4
+    m.h = (fabs(s) <= hlim) ? s : (s > 0.0 ? hlim : -hlim);
+  }
+  m.retry = false;
+  if (++m.n_steps > cfg.max_rk_steps) { m.stop = STOP_STEP_LIMIT; m.phase = PH_FIN; return; }
+  Trial<T> t;
+  rk_trial<T>(fld, m.y, KAPPA * m.y.qop, m.h, t);
+  ++n_trials;
+  if (!isfinite(t.eps)) { m.stop = STOP_NUMERIC; m.phase = PH_FIN; return; }
+  double f;
+  if (t.eps == 0.0) f = 4.0;
+  else {
+    f = 0.9 * sqrt(sqrt(cfg.rk_tol / t.eps));
+    f = f < 0.25 ? 0.25 : f;
+    f = f > 4.0 ? 4.0 : f;
+  }
+  if (t.eps <= cfg.rk_tol) {
+    rk_accept<T>(m.y, m.D, m.h, t, cfg.mass);
+    m.h_ctrl = fabs(m.h) * f;
+    ++n_accepted;
+  } else {
+    m.h = m.h * f;
+    m.retry = true;
+  }
+}
+
+// Arrival (J4, J5) of a move in PH_FIN with stop == NONE: predicted bound parameters and the 5x5 Jacobian
+// block.  Returns the final stop reason (NUMERIC if a predicted parameter is not finite).
+template <typename T>
+CKF_HD int move_arrive(const Move<T>& m, const GeoDev& g, const FieldDev& fld, const CfgDev& cfg, double xp[6],
+                       T J[5][5]) {
+  const ModuleRec& k = g.mod[m.tgt];
+  const ModuleRec& m0 = g.mod[m.from];
+  double B[3];
+  field_at(fld, m.y.r, B);
+  arrival_jacobian(m.D, m0.u, m0.v, m.dep_d, k, m.y, B, cfg.mass, J);
+  const double rel[3] = {m.y.r[0] - k.c[0], m.y.r[1] - k.c[1], m.y.r[2] - k.c[2]};
+  xp[0] = dot3(rel, k.u);
+  xp[1] = dot3(rel, k.v);
+  xp[2] = atan2(m.y.d[1], m.y.d[0]);
+  xp[3] = atan2(sqrt(m.y.d[0] * m.y.d[0] + m.y.d[1] * m.y.d[1]), m.y.d[2]);
+  xp[4] = m.y.qop;
+  xp[5] = m.y.t;
+  bool fin = true;
+#pragma unroll
+  for (int i = 0; i < 6; ++i) fin = fin && isfinite(xp[i]);
+  return fin ? STOP_NONE : STOP_NUMERIC;
+}
+
+// One tip at a time (host test harness): the transitions above in their natural order.
 template <typename T>
 CKF_HD int move_to_next_module(const GeoDev& g, const FieldDev& fld, const CfgDev& cfg, int from, const double x[6],
                                int& target, double xp[6], T J[5][5], T& q_phi, T& q_theta, StepCtl& sc) {
-#pragma unroll
-  for (int i = 0; i < 6; ++i)
-    if (!isfinite(x[i])) return STOP_NUMERIC;
-  if (!(x[3] > 0.0 && x[3] < PI_D)) return STOP_NUMERIC;
-  Traj y;
-  Jac<T> D;
-  T dep_d[3];
-  double dep_u[3], dep_v[3];
-  int layer, iphi, iz;
-  {
-    const ModuleRec& m = g.mod[from];
-    double sp, cp, st, ct;
-    sincos(x[2], &sp, &cp);
-    sincos(x[3], &st, &ct);
-    y.d[0] = st * cp; y.d[1] = st * sp; y.d[2] = ct;
-#pragma unroll
-    for (int i = 0; i < 3; ++i) {
-      y.r[i] = m.c[i] + x[0] * m.u[i] + x[1] * m.v[i];
-      dep_u[i] = m.u[i];
-      dep_v[i] = m.v[i];
-      dep_d[i] = (T)y.d[i];
-    }
-    y.t = x[5];
-    y.qop = x[4];
-    layer = m.layer;
-    iphi = m.iphi;
-    iz = from - g.layer[layer].offset - iphi * g.layer[layer].n_z;
-    if (m.xx0 > 0.0) {
-      const double th2 = highland_theta0_sq(m.xx0, fabs(dot3(y.d, m.n)), y.qop, cfg.mass);
-      q_theta = (T)th2;
-      q_phi = (T)(th2 / (st * st));
+  Move<T> m;
+  move_init(m, g, cfg, from, x);
+  while (m.phase != PH_FIN) {
+    if (m.phase == PH_START || m.phase == PH_LANDED) {
+      PickRequest q;
+      const bool ok = move_pick_request(m, g, q);
+      const int tgt = ok ? pick_in_neighbourhood(g, q.layer, q.iphi, q.iz, q.exclude, m.y.r, m.y.d, q.s_min) : -1;
+      move_pick_apply(m, g, tgt);
     } else {
-      q_theta = T(0);
-      q_phi = T(0);
+      move_step(m, fld, cfg, sc.n_trials, sc.n_accepted);
     }
   }
-  jac_identity(D);
-  sc.h_ctrl = cfg.h_max;
-  sc.n_steps = 0;
-  // N2: overlap neighbour on the same layer
-  int tgt = pick_in_neighbourhood(g, layer, iphi, iz, from, y.r, y.d, 1e-3);
-  if (tgt < 0) {
-    // N3 + N4: next layer's cylinder, module choice at the portal; a crack is not a hole
-    int lp = layer + 1;
-    for (;;) {
-      if (lp >= g.n_layers) return STOP_EXIT;
-      const LayerRec L = g.layer[lp];
-      Target cyl;
-      cyl.kind = 1;
-      cyl.R = L.r;
-      const int st = propagate_to(fld, cfg, cyl, y, D, sc);
-      if (st != STOP_NONE) return st;
-      if (fabs(y.r[2]) > L.half_z) { ++lp; continue; }
-      const double phix = atan2(y.r[1], y.r[0]);
-      int i = (int)nearbyint(phix * L.n_phi / (2.0 * PI_D));
-      i = ((i % L.n_phi) + L.n_phi) % L.n_phi;
-      int j = (int)floor((y.r[2] + L.half_z) / L.len_z);
-      j = j < 0 ? 0 : (j > L.n_z - 1 ? L.n_z - 1 : j);
-      tgt = pick_in_neighbourhood(g, lp, i, j, -1, y.r, y.d, -1e-3);
-      if (tgt >= 0) break;
-      ++lp;
-    }
-  }
-  // N5: to the target's plane, then J4 / J5
-  const ModuleRec& k = g.mod[tgt];
-  {
-    Target pl;
-    pl.kind = 0;
-#pragma unroll
-    for (int i = 0; i < 3; ++i) { pl.c[i] = k.c[i]; pl.n[i] = k.n[i]; }
-    const int st = propagate_to(fld, cfg, pl, y, D, sc);
-    if (st != STOP_NONE) return st;
-  }
-  double B[3];
-  field_at(fld, y.r, B);
-  arrival_jacobian(D, dep_u, dep_v, dep_d, k, y, B, cfg.mass, J);
-  const double rel[3] = {y.r[0] - k.c[0], y.r[1] - k.c[1], y.r[2] - k.c[2]};
-  xp[0] = dot3(rel, k.u);
-  xp[1] = dot3(rel, k.v);
-  xp[2] = atan2(y.d[1], y.d[0]);
-  xp[3] = atan2(sqrt(y.d[0] * y.d[0] + y.d[1] * y.d[1]), y.d[2]);
-  xp[4] = y.qop;
-  xp[5] = y.t;
-#pragma unroll
-  for (int i = 0; i < 6; ++i)
-    if (!isfinite(xp[i])) return STOP_NUMERIC;
-  target = tgt;
-  return STOP_NONE;
+  q_phi = m.q_phi;
+  q_theta = m.q_theta;
+  if (m.stop != STOP_NONE) return m.stop;
+  const int st = move_arrive(m, g, fld, cfg, xp, J);
+  if (st == STOP_NONE) target = m.tgt;
+  return st;
 }
 
 }  // namespace ckf

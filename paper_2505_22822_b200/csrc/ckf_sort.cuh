@@ -1,0 +1,104 @@
+// ckf_sort.cuh — per-event gate index (a7): every module's CSR slice re-ordered by loc0.
+//
+// chi2 = r^T S^-1 r >= r0^2 / S00 for a positive-definite 2x2 S, so a measurement can only pass the gate
+// chi2 < chi2_max if |loc0 - l0| < sqrt(chi2_max (C00 + var0)).  With the slice sorted by loc0 and the
+// slice's largest var0 known, the gate of a tip is a binary search for that window plus chi2 on the few
+// entries inside it, instead of chi2 on the whole slice (inner-layer modules of configs[3] hold ~500
+// measurements, a tip's window ~1-30).  The passer set, hence every result, is unchanged.
+#pragma once
+#include <climits>
+#include "ckf_kernels.cuh"
+
+namespace ckf {
+
+// One block per module (grid-stride).  Slices longer than SORT_CAP, or holding a variance that is not a
+// positive finite number, are copied through unsorted and flagged (s_v0max < 0): their tips gate the whole slice.
+template <typename T>
+__global__ void __launch_bounds__(SORT_NT) ckf_sort_slices(const KParams<T> p) {
+  __shared__ T s_key[SORT_CAP];
+  __shared__ int32_t s_id[SORT_CAP];
+  __shared__ T s_red[SORT_NT / 32];
+  __shared__ int s_bad;
+  const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
+  for (int m = blockIdx.x; m < p.geo.n_modules; m += gridDim.x) {
+    const int beg = __ldg(p.moff + m), end = __ldg(p.moff + m + 1), n = end - beg;
+    if (n <= 0) {
+      if (tid == 0) p.s_v0max[m] = T(0);
+      continue;
+    }
+    if (tid == 0) s_bad = 0;
+    __syncthreads();
+    // largest var0 and validity of the slice's variances
+    T vmax = T(0);
+    bool bad = false;
+    for (int i = tid; i < n; i += SORT_NT) {
+      const auto vr = p.var[beg + i];
+      bad = bad || !(vr.x > T(0)) || !(vr.y > T(0)) || !isfinite(vr.x) || !isfinite(vr.y);
+      vmax = vr.x > vmax ? vr.x : vmax;
+    }
+#pragma unroll
+    for (int o = 16; o > 0; o >>= 1) {
+      const T ov = __shfl_xor_sync(0xffffffffu, vmax, o);
+      vmax = ov > vmax ? ov : vmax;
+    }
+    if (lane == 0) s_red[warp] = vmax;
+    if (bad) s_bad = 1;
+    __syncthreads();
+    const bool unsorted = (s_bad != 0) || n > SORT_CAP;
+    if (unsorted) {
+      for (int i = tid; i < n; i += SORT_NT) {
+        p.s_loc[beg + i] = p.loc[beg + i];
+        p.s_var[beg + i] = p.var[beg + i];
+        p.s_idx[beg + i] = beg + i;
+      }
+      if (tid == 0) p.s_v0max[m] = T(-1);
+      __syncthreads();
+      continue;
+    }
+    int P = 1;
+    while (P < n) P <<= 1;
+    for (int i = tid; i < P; i += SORT_NT) {
+      T key = (T)INFINITY;
+      int id = INT_MAX;
+      if (i < n) {
+        key = p.loc[beg + i].x;
+        if (!(key == key)) key = (T)INFINITY;  // NaN sorts last; it can never pass the gate
+        id = beg + i;
+      }
+      s_key[i] = key;
+      s_id[i] = id;
+    }
+    __syncthreads();
+    // bitonic sort, ascending by (loc0, index)
+    for (int k = 2; k <= P; k <<= 1) {
+      for (int j = k >> 1; j > 0; j >>= 1) {
+        for (int i = tid; i < P; i += SORT_NT) {
+          const int ixj = i ^ j;
+          if (ixj > i) {
+            const T ka = s_key[i], kb = s_key[ixj];
+            const int ia = s_id[i], ib = s_id[ixj];
+            const bool up = (i & k) == 0;
+            const bool a_gt_b = key_less<T>(kb, ib, ka, ia);
+            if (a_gt_b == up) { s_key[i] = kb; s_key[ixj] = ka; s_id[i] = ib; s_id[ixj] = ia; }
+          }
+        }
+        __syncthreads();
+      }
+    }
+    for (int i = tid; i < n; i += SORT_NT) {
+      const int id = s_id[i];
+      p.s_loc[beg + i] = p.loc[id];
+      p.s_var[beg + i] = p.var[id];
+      p.s_idx[beg + i] = id;
+    }
+    if (tid == 0) {
+      T v = s_red[0];
+#pragma unroll
+      for (int w = 1; w < SORT_NT / 32; ++w) v = s_red[w] > v ? s_red[w] : v;
+      p.s_v0max[m] = v;
+    }
+    __syncthreads();
+  }
+}
+
+}  // namespace ckf
