@@ -37,7 +37,7 @@ extern "C" {
 /* bits of *ckf_tracks.status (device int32, written by ckf_find) */
 #define CKF_STATUS_TRACK_OVERFLOW 1  /* more candidates than max_tracks: the first max_tracks are kept       */
 #define CKF_STATUS_ENTRY_OVERFLOW 2  /* meas_idx capacity max_track_entries exceeded: later tracks dropped   */
-#define CKF_STATUS_LINK_OVERFLOW 4   /* candidate-link buffer (max_links) exhausted: some branches were cut  */
+#define CKF_STATUS_LINK_OVERFLOW 4   /* max_links or max_tips_per_level exhausted: some branches were cut    */
 
 /* stop reasons reported per candidate */
 #define CKF_STOP_EXIT 1         /* left the detector (past the last layer / beyond half-z everywhere) */
@@ -102,6 +102,7 @@ typedef struct {
   int32_t max_tracks;               /* capacity of the per-track output arrays                           */
   int32_t max_track_entries;        /* capacity of meas_idx / entry_chi2                                 */
   int32_t max_links;                /* candidate-link buffer entries; 0 = 48 * max_seeds                 */
+  int32_t max_tips_per_level;       /* live branch tips of one level, whole event; 0 = 8 * max_seeds     */
   int32_t n_streams;                /* independent workspaces; concurrent ckf_find calls up to this many */
 } ckf_config;
 
@@ -150,7 +151,7 @@ typedef struct {
   int64_t gate_tests;   /* chi2 evaluations the method defines: sum of visited slice lengths */
   int64_t updates;      /* Kalman updates                                       */
   int64_t links;        /* candidate links appended                             */
-  int64_t iterations;   /* sum over warps of 32-tip chunks processed            */
+  int64_t iterations;   /* levels that held at least one tip                    */
   int64_t gate_tests_executed; /* chi2 evaluations actually run: entries inside the loc0 windows
                                   (the rest of each slice is excluded by chi2 >= r0^2/S00) */
 } ckf_counters;
@@ -177,8 +178,8 @@ int ckf_find_host(ckf_handle* handle, const ckf_measurements* measurements, cons
 /* Copies the work counters of the most recent ckf_find issued on `cuda_stream` (synchronises that stream). */
 int ckf_get_counters(ckf_handle* handle, void* cuda_stream, ckf_counters* out);
 
-/* Launch configuration chosen at ckf_create: thread blocks, threads per block, dynamic shared bytes,
- * registers per thread of the level-loop kernel (any pointer may be NULL). */
+/* Launch configuration chosen at ckf_create for the hot kernel (ckf_step: navigation + RKN4): thread blocks,
+ * threads per block, shared bytes, registers per thread (any pointer may be NULL). */
 int ckf_get_launch_info(const ckf_handle* handle, int32_t* blocks, int32_t* threads, int32_t* smem_bytes,
                         int32_t* regs);
 

@@ -41,7 +41,8 @@ class ckf_config(C.Structure):
                 ("rk_tolerance_mm", C.c_double), ("surface_tolerance_mm", C.c_double), ("h_max_mm", C.c_double),
                 ("particle_mass_gev", C.c_double), ("max_rk_steps_per_surface", C.c_int32), ("max_levels", C.c_int32),
                 ("max_seeds", C.c_int32), ("max_measurements", C.c_int32), ("max_tracks", C.c_int32),
-                ("max_track_entries", C.c_int32), ("max_links", C.c_int32), ("n_streams", C.c_int32)]
+                ("max_track_entries", C.c_int32), ("max_links", C.c_int32), ("max_tips_per_level", C.c_int32),
+                ("n_streams", C.c_int32)]
 
 
 class ckf_measurements(C.Structure):
@@ -131,7 +132,7 @@ def make_field(fld, keep: list) -> ckf_field:
 
 
 def make_config(ckf, precision: int, max_seeds: int, max_measurements: int, max_tracks: int, max_track_entries: int,
-                max_links: int = 0, n_streams: int = 1) -> ckf_config:
+                max_links: int = 0, n_streams: int = 1, max_tips_per_level: int = 0) -> ckf_config:
     c = ckf_config()
     c.precision = int(precision)
     for name in ("chi2_max", "max_branches_per_surface", "max_candidates_per_seed", "max_holes", "min_measurements",
@@ -141,6 +142,7 @@ def make_config(ckf, precision: int, max_seeds: int, max_measurements: int, max_
     c.max_seeds, c.max_measurements = int(max_seeds), int(max_measurements)
     c.max_tracks, c.max_track_entries = int(max_tracks), int(max_track_entries)
     c.max_links, c.n_streams = int(max_links), int(n_streams)
+    c.max_tips_per_level = int(max_tips_per_level)
     return c
 
 
@@ -169,7 +171,7 @@ class CKF:
 
     def __init__(self, det, fld, ckf, precision: int, max_seeds: int, max_measurements: int,
                  max_tracks: Optional[int] = None, max_track_entries: Optional[int] = None, max_links: int = 0,
-                 n_streams: int = 1):
+                 n_streams: int = 1, max_tips_per_level: int = 0):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: paper_2505_22822_b200 has no CPU fallback")
@@ -185,7 +187,7 @@ class CKF:
         g = make_geometry(det, keep)
         f = make_field(fld, keep)
         self.config = make_config(ckf, precision, max_seeds, max_measurements, self.max_tracks, self.max_track_entries,
-                                  max_links, n_streams)
+                                  max_links, n_streams, max_tips_per_level)
         h = _vp()
         rc = self.lib.ckf_create(C.byref(g), C.byref(f), C.byref(self.config), C.byref(h))
         if rc != 0:

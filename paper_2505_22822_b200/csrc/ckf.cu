@@ -1,9 +1,9 @@
 // ckf.cu — C ABI of the B200-native CKF track-finding library (include/ckf.h): host side.
 //
 // ckf_create uploads the geometry store (a1) and field store (a2) once and reserves every
-// workspace; ckf_find enqueues six launches on the caller's stream and never allocates.
+// workspace; ckf_find enqueues its launches (five small kernels per level) on the caller's stream and never allocates.
 // There is no CPU path in this library: all arithmetic of the method runs in the kernels of
-// ckf_level_loop.cuh / ckf_emit.cuh.
+// ckf_step.cuh / ckf_visit.cuh / ckf_branch.cuh / ckf_sort.cuh / ckf_emit.cuh.
 #include <cuda_runtime.h>
 
 #include <cstdarg>
@@ -16,8 +16,10 @@
 #include "../../include/ckf.h"
 #include "ckf_emit.cuh"
 #include "ckf_host_geom.h"
-#include "ckf_level_loop.cuh"
+#include "ckf_branch.cuh"
 #include "ckf_sort.cuh"
+#include "ckf_step.cuh"
+#include "ckf_visit.cuh"
 
 using namespace ckf;
 
@@ -33,11 +35,15 @@ struct Workspace {
   void *lk_chi2 = nullptr, *lk_chi2sum = nullptr;
   int32_t *sd = nullptr;       // 3 * max_seeds + 2 * (max_seeds + 1)
   int32_t* leaf = nullptr;     // 3 * max_seeds * cap
-  int2* queue = nullptr;
-  double* pred_x = nullptr; void* pred_C = nullptr; int32_t* pred_ts = nullptr;  // P1 -> P2-P4 predictions
+  // level state (tips, move state, predictions, selections, scan)
+  int32_t *tip_link = nullptr, *tip_seed = nullptr;
+  double *mv_y = nullptr, *pd_x = nullptr;
+  void *mv_D = nullptr, *mv_dep = nullptr, *pd_C = nullptr, *sel_chi2 = nullptr;
+  int32_t *mv_from = nullptr, *mv_tgt = nullptr, *mv_stop = nullptr, *sel_idx = nullptr;
+  int32_t *t_nsel = nullptr, *t_want = nullptr, *t_counts = nullptr, *t_keep = nullptr, *t_kex = nullptr, *blk_sum = nullptr;
   void *s_loc = nullptr, *s_var = nullptr, *s_v0max = nullptr;  // gate index (ckf_sort_slices)
   int32_t* s_idx = nullptr;
-  int32_t* globals = nullptr;  // cursor, link_count, first_bad, total[2]
+  int32_t* globals = nullptr;  // GlobalId
   unsigned long long* counters = nullptr;
   // staging for ckf_find_host
   int32_t* h_moff = nullptr; void *h_loc = nullptr, *h_var = nullptr;
@@ -59,10 +65,10 @@ struct ckf_handle {
   int n_modules = 0, n_layers = 0;
   ModuleRec* d_mod = nullptr;
   LayerRec* d_layer = nullptr;
-  float4* d_grid = nullptr;
+  double* d_grid = nullptr;
   FieldDev fld;
   CfgDev kcfg;
-  int grid = 0, smem = 0, regs = 0, qcap = 0, tsize = 4;
+  int step_grid = 0, step_regs = 0, visit_grid = 0, visit_smem = 0, tcap = 0, tsize = 4;
   std::vector<Workspace> ws;
   int next_ws = 0;
   std::mutex mu;
@@ -97,13 +103,16 @@ cudaError_t dalloc(ckf_handle* h, P** p, size_t bytes) {
   return e;
 }
 
-// Resident blocks per SM the level loop is compiled for: 4 x 128 threads at <= 128 registers (float),
+// Resident blocks per SM ckf_step / ckf_visit are compiled for: 3 x 128 threads at <= 168 registers (float step:
+// measured faster than 4 x 128 at 128 registers with 300 B of spills), 4 x 128 at <= 128 registers (float visit),
 // 2 x 128 threads at <= 255 registers (double: the covariance algebra doubles its register footprint).
 #ifndef CKF_MINB
-#define CKF_MINB 4
+#define CKF_MINB 3
 #endif
 template <typename T> struct MinBlocks { static constexpr int value = CKF_MINB; };
 template <> struct MinBlocks<double> { static constexpr int value = 2; };
+template <typename T> struct VisitBlocks { static constexpr int value = 4; };
+template <> struct VisitBlocks<double> { static constexpr int value = 2; };
 
 template <typename T>
 void fill_params(ckf_handle* h, Workspace& w, KParams<T>& p) {
@@ -119,11 +128,16 @@ void fill_params(ckf_handle* h, Workspace& w, KParams<T>& p) {
   p.sd_track_base = w.sd + 3 * S; p.sd_entry_base = w.sd + 3 * S + (S + 1);
   const size_t LC = S * (size_t)c.max_candidates_per_seed;
   p.leaf_link = w.leaf; p.leaf_meta = w.leaf + LC; p.leaf_entry = w.leaf + 2 * LC;
-  p.queue = w.queue; p.qcap = h->qcap;
-  p.pred_x = w.pred_x; p.pred_C = (T*)w.pred_C; p.pred_ts = w.pred_ts;
+  p.tcap = h->tcap;
+  p.tip_link = w.tip_link; p.tip_seed = w.tip_seed;
+  p.mv_y = w.mv_y; p.mv_D = (T*)w.mv_D; p.mv_dep = (T*)w.mv_dep; p.mv_from = w.mv_from; p.mv_tgt = w.mv_tgt;
+  p.mv_stop = w.mv_stop;
+  p.pd_x = w.pd_x; p.pd_C = (T*)w.pd_C; p.sel_chi2 = (T*)w.sel_chi2; p.sel_idx = w.sel_idx;
+  p.t_nsel = w.t_nsel; p.t_want = w.t_want; p.t_counts = w.t_counts; p.t_keep = w.t_keep; p.t_kex = w.t_kex;
+  p.blk_sum = w.blk_sum;
   p.s_loc = (typename Vec2<T>::type*)w.s_loc; p.s_var = (typename Vec2<T>::type*)w.s_var; p.s_idx = w.s_idx;
   p.s_v0max = (T*)w.s_v0max;
-  p.g_seed_cursor = w.globals; p.g_link_count = w.globals + 1; p.g_first_bad = w.globals + 2; p.g_total = w.globals + 3;
+  p.g = w.globals;
   p.counters = w.counters;
   p.max_tracks = c.max_tracks; p.max_entries = c.max_track_entries;
 }
@@ -144,7 +158,16 @@ int launch_find(ckf_handle* h, Workspace& w, const ckf_measurements* m, const ck
   const int nb = (std::max(s->n, (int)CNT_N) + 255) / 256;
   ckf_init_event<T><<<nb, 256, 0, st>>>(p);
   ckf_sort_slices<T><<<h->sm_count * 8, SORT_NT, 0, st>>>(p);
-  ckf_level_loop<T, MinBlocks<T>::value><<<h->grid, NT, h->smem, st>>>(p);
+  // level loop: tips of level l were made by level l - 1; a tip at max_levels only stops (LEVEL_LIMIT) and emits.
+  // Kernels of an empty level return at once, so the loop needs no host read of the level's size.
+  const int scan_blocks = h->tcap / SCAN_NT + 1, wide = h->sm_count * 8;
+  for (int level = 0; level <= h->cfg.max_levels; ++level) {
+    if (level > 0) ckf_step<T, MinBlocks<T>::value><<<h->step_grid, STEP_NT, 0, st>>>(p, level);
+    ckf_visit<T, VisitBlocks<T>::value><<<h->visit_grid, VISIT_NT, h->visit_smem, st>>>(p, level);
+    ckf_cap<T><<<wide, SCAN_NT, 0, st>>>(p, level);
+    ckf_scan<T><<<scan_blocks, SCAN_NT, 0, st>>>(p, level);
+    ckf_update<T><<<wide, SCAN_NT, 0, st>>>(p, level);
+  }
   ckf_scan_seeds<T><<<1, 1024, 0, st>>>(p);
   ckf_emit_tracks<T><<<h->sm_count * 4, 256, 0, st>>>(p);
   ckf_finalize<T><<<1, 1, 0, st>>>(p);
@@ -238,13 +261,17 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     h->fld.n[a] = f->n[a];
     h->fld.org[a] = f->origin[a];
     h->fld.inv[a] = f->kind == 1 ? 1.0 / f->spacing[a] : 0.0;
+    h->fld.nm2[a] = (double)(f->n[a] - 2);
   }
   if (f->kind == 1) {
     const size_t np = (size_t)f->n[0] * f->n[1] * f->n[2];
-    std::vector<float4> pad(np);
-    for (size_t i = 0; i < np; ++i) pad[i] = make_float4(f->grid[3 * i], f->grid[3 * i + 1], f->grid[3 * i + 2], 0.f);
-    CKB(dalloc(h, &h->d_grid, np * sizeof(float4)));
-    CKB(cudaMemcpy(h->d_grid, pad.data(), np * sizeof(float4), cudaMemcpyHostToDevice));
+    std::vector<double> pad(4 * np);
+    for (size_t i = 0; i < np; ++i) {
+      pad[4 * i] = (double)f->grid[3 * i]; pad[4 * i + 1] = (double)f->grid[3 * i + 1];
+      pad[4 * i + 2] = (double)f->grid[3 * i + 2]; pad[4 * i + 3] = 0.0;
+    }
+    CKB(dalloc(h, &h->d_grid, 4 * np * sizeof(double)));
+    CKB(cudaMemcpy(h->d_grid, pad.data(), 4 * np * sizeof(double), cudaMemcpyHostToDevice));
     h->fld.grid = h->d_grid;
   }
   // ---- config
@@ -252,24 +279,32 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
   h->kcfg.h_max = c->h_max_mm; h->kcfg.mass = c->particle_mass_gev; h->kcfg.max_branches = c->max_branches_per_surface;
   h->kcfg.max_cands = c->max_candidates_per_seed; h->kcfg.max_holes = c->max_holes; h->kcfg.min_meas = c->min_measurements;
   h->kcfg.max_rk_steps = c->max_rk_steps_per_surface; h->kcfg.max_levels = c->max_levels;
-  // ---- launch configuration of the level loop: one wave of resident blocks, WPB autonomous warps each
-  int per_sm = 0;
-  cudaFuncAttributes fa;
-  if (c->precision == 32) {
-    h->smem = (int)(WPB * WSmem<float>::bytes(c->max_branches_per_surface));
-    CKB(cudaFuncSetAttribute(ckf_level_loop<float, MinBlocks<float>::value>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem));
-    CKB(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ckf_level_loop<float, MinBlocks<float>::value>, NT, h->smem));
-    CKB(cudaFuncGetAttributes(&fa, ckf_level_loop<float, MinBlocks<float>::value>));
-  } else {
-    h->smem = (int)(WPB * WSmem<double>::bytes(c->max_branches_per_surface));
-    CKB(cudaFuncSetAttribute(ckf_level_loop<double, MinBlocks<double>::value>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->smem));
-    CKB(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ckf_level_loop<double, MinBlocks<double>::value>, NT, h->smem));
-    CKB(cudaFuncGetAttributes(&fa, ckf_level_loop<double, MinBlocks<double>::value>));
+  // ---- launch configuration: ckf_step is persistent (one wave of resident blocks), ckf_visit grid-strides
+  {
+    int per_sm = 0, vper_sm = 0;
+    cudaFuncAttributes fa;
+    if (c->precision == 32) {
+      h->visit_smem = (int)((VISIT_NT / 32) * VSmem<float>::bytes(c->max_branches_per_surface));
+      CKB(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ckf_step<float, MinBlocks<float>::value>, STEP_NT, 0));
+      CKB(cudaFuncGetAttributes(&fa, ckf_step<float, MinBlocks<float>::value>));
+      CKB(cudaFuncSetAttribute(ckf_visit<float, VisitBlocks<float>::value>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->visit_smem));
+      CKB(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&vper_sm, ckf_visit<float, VisitBlocks<float>::value>, VISIT_NT, h->visit_smem));
+    } else {
+      h->visit_smem = (int)((VISIT_NT / 32) * VSmem<double>::bytes(c->max_branches_per_surface));
+      CKB(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ckf_step<double, MinBlocks<double>::value>, STEP_NT, 0));
+      CKB(cudaFuncGetAttributes(&fa, ckf_step<double, MinBlocks<double>::value>));
+      CKB(cudaFuncSetAttribute(ckf_visit<double, VisitBlocks<double>::value>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->visit_smem));
+      CKB(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&vper_sm, ckf_visit<double, VisitBlocks<double>::value>, VISIT_NT, h->visit_smem));
+    }
+    if (per_sm < 1 || vper_sm < 1) { fail(h, CKF_E_CUDA, "kernels do not fit on an SM (visit smem %d B)", h->visit_smem); return bail(CKF_E_CUDA); }
+    h->step_regs = fa.numRegs;
+    h->step_grid = per_sm * h->sm_count;
+    h->visit_grid = vper_sm * h->sm_count;
   }
-  if (per_sm < 1) { fail(h, CKF_E_CUDA, "level-loop kernel does not fit on an SM (smem %d B)", h->smem); return bail(CKF_E_CUDA); }
-  h->regs = fa.numRegs;
-  h->grid = per_sm * h->sm_count;
-  h->qcap = MAX_LIVE_SEEDS * c->max_candidates_per_seed;
+  if (h->cfg.max_tips_per_level <= 0)
+    h->cfg.max_tips_per_level = (int32_t)std::min<long long>(std::max<long long>(8LL * c->max_seeds, 1024), 0x7ffffff0LL);
+  if (h->cfg.max_tips_per_level < c->max_seeds) h->cfg.max_tips_per_level = c->max_seeds;
+  h->tcap = h->cfg.max_tips_per_level;
   // ---- workspaces
   const size_t L = (size_t)h->cfg.max_links, S = (size_t)c->max_seeds, ts = (size_t)h->tsize;
   h->ws.resize(c->n_streams);
@@ -281,10 +316,16 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     CKB(dalloc(h, (char**)&w.lk_chi2, L * ts)); CKB(dalloc(h, (char**)&w.lk_chi2sum, L * ts));
     CKB(dalloc(h, &w.sd, (3 * S + 2 * (S + 1)) * 4));
     CKB(dalloc(h, &w.leaf, 3 * S * (size_t)c->max_candidates_per_seed * 4));
-    CKB(dalloc(h, &w.queue, (size_t)h->grid * WPB * 2 * h->qcap * sizeof(int2)));
-    CKB(dalloc(h, &w.pred_x, (size_t)h->grid * WPB * 6 * SUBW * sizeof(double)));
-    CKB(dalloc(h, (char**)&w.pred_C, (size_t)h->grid * WPB * 21 * SUBW * ts));
-    CKB(dalloc(h, &w.pred_ts, (size_t)h->grid * WPB * 2 * SUBW * 4));
+    const size_t TC = (size_t)h->tcap, KB = (size_t)c->max_branches_per_surface;
+    CKB(dalloc(h, &w.tip_link, 2 * TC * 4)); CKB(dalloc(h, &w.tip_seed, 2 * TC * 4));
+    CKB(dalloc(h, &w.mv_y, 8 * TC * sizeof(double))); CKB(dalloc(h, &w.pd_x, 6 * TC * sizeof(double)));
+    CKB(dalloc(h, (char**)&w.mv_D, 25 * TC * ts)); CKB(dalloc(h, (char**)&w.mv_dep, 5 * TC * ts));
+    CKB(dalloc(h, (char**)&w.pd_C, 21 * TC * ts)); CKB(dalloc(h, (char**)&w.sel_chi2, KB * TC * ts));
+    CKB(dalloc(h, &w.sel_idx, KB * TC * 4));
+    CKB(dalloc(h, &w.mv_from, TC * 4)); CKB(dalloc(h, &w.mv_tgt, TC * 4)); CKB(dalloc(h, &w.mv_stop, TC * 4));
+    CKB(dalloc(h, &w.t_nsel, TC * 4)); CKB(dalloc(h, &w.t_want, TC * 4)); CKB(dalloc(h, &w.t_counts, TC * 4));
+    CKB(dalloc(h, &w.t_keep, TC * 4)); CKB(dalloc(h, &w.t_kex, TC * 4));
+    CKB(dalloc(h, &w.blk_sum, (TC / SCAN_NT + 2) * 4));
     CKB(dalloc(h, (char**)&w.s_loc, 2 * (size_t)c->max_measurements * ts));
     CKB(dalloc(h, (char**)&w.s_var, 2 * (size_t)c->max_measurements * ts));
     CKB(dalloc(h, &w.s_idx, (size_t)c->max_measurements * 4));
@@ -392,10 +433,10 @@ int ckf_get_counters(ckf_handle* h, void* stream, ckf_counters* out) {
 
 int ckf_get_launch_info(const ckf_handle* h, int32_t* blocks, int32_t* threads, int32_t* smem, int32_t* regs) {
   if (!h) return CKF_E_ARG;
-  if (blocks) *blocks = h->grid;
-  if (threads) *threads = NT;
-  if (smem) *smem = h->smem;
-  if (regs) *regs = h->regs;
+  if (blocks) *blocks = h->step_grid;
+  if (threads) *threads = STEP_NT;
+  if (smem) *smem = (int32_t)((STEP_NT / 32) * PickSmem::bytes());
+  if (regs) *regs = h->step_regs;
   return CKF_OK;
 }
 

@@ -5,14 +5,21 @@
 
 namespace ckf {
 
-// Resets every per-event device counter (no allocation, no memset calls in ckf_find).
+// Resets every per-event device counter and lays down level 0: one tip per seed, standing on no link.
+// (No allocation, no memset calls in ckf_find.)
 template <typename T>
 __global__ void ckf_init_event(const KParams<T> p) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
-  if (i < p.n_seeds) { p.sd_extra[i] = 0; p.sd_nemit[i] = 0; p.sd_nentries[i] = 0; }
+  if (i < p.n_seeds) {
+    p.sd_extra[i] = 0; p.sd_nemit[i] = 0; p.sd_nentries[i] = 0;
+    if (i < p.tcap) { p.tip_link[i] = -1; p.tip_seed[i] = i; p.mv_stop[i] = STOP_NONE; }
+  }
   if (i == 0) {
-    *p.g_seed_cursor = 0; *p.g_link_count = 0; *p.g_first_bad = INT_MAX; p.g_total[0] = 0; p.g_total[1] = 0;
-    *p.o_status = 0; *p.o_ntracks = 0;
+    for (int k = 0; k < G_N; ++k) p.g[k] = 0;
+    p.g[G_FIRST_BAD] = INT_MAX;
+    p.g[G_NTIPS0] = p.n_seeds < p.tcap ? p.n_seeds : p.tcap;
+    *p.o_status = p.n_seeds > p.tcap ? 4 : 0;
+    *p.o_ntracks = 0;
   }
   if (i < CNT_N) p.counters[i] = 0ull;
 }
@@ -44,14 +51,14 @@ __global__ void __launch_bounds__(1024) ckf_scan_seeds(const KParams<T> p) {
   }
   if (tid == 1023) {
     p.sd_track_base[S] = s_a[1023]; p.sd_entry_base[S] = s_b[1023];
-    p.g_total[0] = s_a[1023]; p.g_total[1] = s_b[1023];
+    p.g[G_TOTAL_TRACKS] = s_a[1023]; p.g[G_TOTAL_ENTRIES] = s_b[1023];
   }
 }
 
 // Thread per candidate: backtrace the links into the index list, copy the state at the last measurement.
 template <typename T>
 __global__ void __launch_bounds__(256) ckf_emit_tracks(const KParams<T> p) {
-  const int total = p.g_total[0];
+  const int total = p.g[G_TOTAL_TRACKS];
   const int cap = p.cfg.max_cands;
   for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < total; t += gridDim.x * blockDim.x) {
     // seed = last s with track_base[s] <= t
@@ -66,7 +73,7 @@ __global__ void __launch_bounds__(256) ckf_emit_tracks(const KParams<T> p) {
     const int off = p.sd_entry_base[seed] + p.leaf_entry[li];
     const int nm = p.lk_counts[leaf] & 0xffff;
     if (t >= p.max_tracks || off + nm > p.max_entries) {
-      atomicMin(p.g_first_bad, t);
+      atomicMin(p.g + G_FIRST_BAD, t);
       atomicOr(p.o_status, t >= p.max_tracks ? 1 : 2);
       continue;
     }
@@ -94,7 +101,7 @@ __global__ void __launch_bounds__(256) ckf_emit_tracks(const KParams<T> p) {
 
 template <typename T>
 __global__ void ckf_finalize(const KParams<T> p) {
-  const int total = p.g_total[0], bad = *p.g_first_bad;
+  const int total = p.g[G_TOTAL_TRACKS], bad = p.g[G_FIRST_BAD];
   const int n = total < bad ? total : bad;
   *p.o_ntracks = n;
   if (n == 0) p.o_offsets[0] = 0;

@@ -1,31 +1,35 @@
-// ckf_kernels.cuh — the CKF level loop as ONE persistent kernel per event whose worker is the WARP, plus the
-// slice-sort and emission kernels.
+// ckf_kernels.cuh — shared declarations of the CKF kernels (a3-a11).
 //
-// Design: seeds never interact (the only cross-branch rule, the per-seed cap R10, is per
-// seed), so a warp owns whole seeds from pull to emission and runs the entire level loop
-//   propagate (lane per tip, lockstep RKN4) -> gate (lanes over the flattened (tip, measurement) pairs of the
-//   loc0 windows) -> cap + warp prefix sums -> update + link append (lane per child) -> emission records
-// with __syncwarp only: no block barrier (a slow RKN4 loop delays 31 neighbours, not 255), no host round trip
-// for "n_active == 0", no per-level launches, no device-wide scan.  Warps pull seeds from a global cursor
-// whenever their last chunk of tips has free lanes (continuous batching).  Results are placed by seed id and
-// in-seed order, so the output is deterministic no matter which warp took which seed.
+// Design: the level loop is LEVEL-SYNCHRONOUS over the whole event and PHASE-SEPARATED into
+// small kernels, five per level:
+//   ckf_step    persistent lanes pull tips of the level from a global cursor and run the navigation +
+//               adaptive RKN4 state machine (ckf_nav.cuh) until the tip stands on its next module
+//   ckf_visit   arrival Jacobian + covariance transport (lane per tip), then the chi2 gate over the loc0
+//               windows of the sorted slices (flattened (tip, measurement) pairs) and the k best
+//   ckf_cap     per-seed cap R10 and emission records (one thread walks a seed's tips in order)
+//   ckf_scan    exclusive scan of the kept children -> child offsets, link allocation, next level's size
+//   ckf_update  thread per child: Kalman update or hole, link append, departure state of the next level
+// Why not one persistent kernel: measured on B200 (profiles/r01b), the monolithic level loop is ~100 KB of
+// SASS; with the warps of an SM in different phases the SM instruction cache misses 31 % of its requests and
+// the GPC-level instruction cache saturates (77 % of peak), which bounds the kernel regardless of occupancy.
+// Each kernel here keeps its hot loop within the SM's instruction cache and gets its own register budget.
+// Everything is placed by prefix sums in tip order (seed, then lineage), so the output is deterministic.
 #pragma once
 #include <cuda_runtime.h>
 #include "ckf_nav.cuh"
 
 namespace ckf {
 
-constexpr int WPB = 4;            // warps per block of the level loop (blocks exist only to carve shared memory)
-constexpr int NT = 32 * WPB;      // threads per block
 constexpr int CAND = 16;          // per-tip passer buffer of the gate fast path
-constexpr int MAX_LIVE_SEEDS = 48;  // seeds a warp may hold at once (bounds its tip queue)
-constexpr int SUBW = 128;          // tips of a warp's wave propagated together (persistent lanes); multiple of 32
-#ifndef CKF_SERVICE_MIN
-#define CKF_SERVICE_MIN 12
-#endif
-constexpr int SERVICE_MIN = CKF_SERVICE_MIN;    // lanes that must be waiting before a P1 service point is run early
+constexpr int STEP_NT = 128;      // threads per block of ckf_step
+constexpr int VISIT_NT = 128;     // threads per block of ckf_visit (4 warps, 32 tips each)
+constexpr int SCAN_NT = 256;      // threads per block of ckf_cap / ckf_scan / ckf_update; tile of the scan
 constexpr int SORT_NT = 128;      // threads per block of the slice sort
 constexpr int SORT_CAP = 2048;    // largest module slice sorted in shared memory; larger ones stay unsorted
+#ifndef CKF_SERVICE_MIN
+#define CKF_SERVICE_MIN 16
+#endif
+constexpr int SERVICE_MIN = CKF_SERVICE_MIN;  // lanes that must wait before a ckf_step service point runs early
 
 template <typename T> struct Vec2;
 template <> struct Vec2<float> { using type = float2; };
@@ -33,6 +37,10 @@ template <> struct Vec2<double> { using type = double2; };
 
 enum CounterId { CNT_TIPS = 0, CNT_VISITS, CNT_TRIALS, CNT_ACCEPTED, CNT_GATE, CNT_UPDATES, CNT_LINKS, CNT_ITER,
                  CNT_GATE_EXEC, CNT_N };
+
+// per-event device globals (int32 each)
+enum GlobalId { G_LINK_COUNT = 0, G_FIRST_BAD, G_TOTAL_TRACKS, G_TOTAL_ENTRIES, G_NTIPS0, G_NTIPS1, G_STEP_CURSOR,
+                G_SCAN_TICKET, G_LBASE, G_N };
 
 template <typename T>
 struct KParams {
@@ -52,7 +60,7 @@ struct KParams {
   typename Vec2<T>::type* s_var;   // [n_meas]
   int32_t* s_idx;                  // [n_meas] position in the caller's arrays (what meas_idx reports)
   T* s_v0max;                      // [n_modules] largest var0 of the slice; < 0 = slice left unsorted
-  // candidate-link buffer (a10): SoA, one entry per child ever made
+  // candidate-link buffer (a10): SoA, one entry per child ever made; a level's links are contiguous
   int32_t max_links;
   double* lk_x;        // [6][max_links]   bound parameters after the visit
   T* lk_C;             // [21][max_links]  packed covariance after the visit
@@ -72,18 +80,30 @@ struct KParams {
   int32_t* leaf_entry;   // entry offset inside the seed
   int32_t* sd_track_base;  // [n_seeds + 1] (emission scan)
   int32_t* sd_entry_base;  // [n_seeds + 1]
-  // per warp tip queues, double buffered: int2 (link or -(seed+1), seed)
-  int2* queue;
-  int32_t qcap;
-  // per warp predictions of one sub-wave (P1 -> P2-P4)
-  double* pred_x;    // [n_warps][6][SUBW]
-  T* pred_C;         // [n_warps][21][SUBW]
-  int32_t* pred_ts;  // [n_warps][2][SUBW] target, stop
+  // ---- tips of a level, ordered by seed then lineage; arrays [..][tcap], tip index fastest
+  int32_t tcap;
+  int32_t* tip_link;   // [2][tcap] (ping-pong by level parity) link the tip stands on, -1 = fresh seed
+  int32_t* tip_seed;   // [2][tcap]
+  // departure / arrival state of the move (ckf_update -> ckf_step -> ckf_visit)
+  double* mv_y;        // [8][tcap] r, d, t, q/p
+  T* mv_D;             // [25][tcap] transport Jacobian (ckf_step -> ckf_visit)
+  T* mv_dep;           // [5][tcap] direction on departure, Highland q_phi, q_theta
+  int32_t* mv_from;    // [tcap] module the tip stands on
+  int32_t* mv_tgt;     // [tcap] module reached
+  int32_t* mv_stop;    // [tcap] stop reason so far
+  // prediction + selection (ckf_visit -> ckf_cap, ckf_update)
+  double* pd_x;        // [6][tcap]
+  T* pd_C;             // [21][tcap]
+  T* sel_chi2;         // [K][tcap]
+  int32_t* sel_idx;    // [K][tcap]
+  int32_t* t_nsel;     // [tcap]
+  int32_t* t_want;     // [tcap]
+  int32_t* t_counts;   // [tcap] n_meas | n_holes << 16 of the tip (fatal hole included)
+  int32_t* t_keep;     // [tcap] children kept after R10
+  int32_t* t_kex;      // [tcap] exclusive prefix of t_keep inside the tip's scan tile
+  int32_t* blk_sum;    // [tcap / SCAN_NT + 1] kept children per scan tile, then exclusive offsets
   // globals
-  int32_t* g_seed_cursor;
-  int32_t* g_link_count;
-  int32_t* g_first_bad;
-  int32_t* g_total;  // [2] total tracks, total entries
+  int32_t* g;          // [G_N]
   unsigned long long* counters;
   // output
   int32_t max_tracks, max_entries;
@@ -101,66 +121,16 @@ __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
   }
   return v;
 }
-__device__ __forceinline__ int warp_incl_max(int v, int lane) {
-#pragma unroll
-  for (int o = 1; o < 32; o <<= 1) {
-    const int n = __shfl_up_sync(0xffffffffu, v, o);
-    if (lane >= o) v = max(v, n);
-  }
-  return v;
-}
 
 template <typename T>
 __device__ __forceinline__ bool key_less(T c1, int i1, T c2, int i2) {
   return c1 < c2 || (c1 == c2 && i1 < i2);
 }
 
-// Shared memory of ONE warp of the level loop (sizes depend on max_branches K).  Arrays are [..][32] with the
-// tip (lane) index fastest, so lane-per-tip accesses are conflict-free.
-template <typename T>
-struct WSmem {
-  double* px;       // [6][32] predicted bound parameters
-  T* pC;            // [21][32] predicted packed covariance
-  T* selchi2;       // [K][32]
-  int32_t* selidx;  // [K][32]
-  T* candchi2;      // [CAND][32]
-  int32_t* candidx; // [CAND][32]
-  T* chi2sum;       // [32]
-  int32_t *link, *seed, *target, *counts, *lastmeas, *nsel, *lo, *cnt;  // [32] each
-  int32_t *off, *Kex;  // [33]
-  __host__ __device__ static size_t bytes(int K) {
-    size_t b = 0;
-    b += sizeof(double) * 6 * 32;
-    b += sizeof(T) * 21 * 32;
-    b += (sizeof(T) + 4) * (size_t)K * 32;
-    b += (sizeof(T) + 4) * (size_t)CAND * 32;
-    b += sizeof(T) * 32;
-    b += 4 * 8 * 32;
-    b += 4 * 2 * 33;
-    const size_t p1 = 8 * 9 * 32 + 8 * 6 * 32 + 4 * 9 * 32 + 4 * 5 * 32;  // P1Smem::bytes(), aliased
-    b = b > p1 ? b : p1;
-    return (b + 15) & ~(size_t)15;
-  }
-  __device__ void carve(unsigned char* raw, int K) {
-    unsigned char* p = raw;
-    px = (double*)p; p += sizeof(double) * 6 * 32;
-    pC = (T*)p; p += sizeof(T) * 21 * 32;
-    selchi2 = (T*)p; p += sizeof(T) * (size_t)K * 32;
-    candchi2 = (T*)p; p += sizeof(T) * (size_t)CAND * 32;
-    chi2sum = (T*)p; p += sizeof(T) * 32;
-    selidx = (int32_t*)p; p += 4 * (size_t)K * 32;
-    candidx = (int32_t*)p; p += 4 * (size_t)CAND * 32;
-    link = (int32_t*)p; p += 4 * 32;
-    seed = (int32_t*)p; p += 4 * 32;
-    target = (int32_t*)p; p += 4 * 32;
-    counts = (int32_t*)p; p += 4 * 32;
-    lastmeas = (int32_t*)p; p += 4 * 32;
-    nsel = (int32_t*)p; p += 4 * 32;
-    lo = (int32_t*)p; p += 4 * 32;
-    cnt = (int32_t*)p; p += 4 * 32;
-    off = (int32_t*)p; p += 4 * 33;
-    Kex = (int32_t*)p; p += 4 * 33;
-  }
-};
+__device__ __forceinline__ void flush_counter(unsigned long long* dst, unsigned long long v) {
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) v += __shfl_xor_sync(0xffffffffu, v, o);
+  if ((threadIdx.x & 31) == 0 && v) atomicAdd(dst, v);
+}
 
 }  // namespace ckf

@@ -46,14 +46,18 @@ struct LayerRec {
   int32_t n_phi, n_z, offset, pad;
 };
 
-// a2 field store: uniform, or float4-padded copy of the float32 grid [ix][iy][iz] (w unused).
+// a2 field store: uniform, or the float32 grid [ix][iy][iz] widened ONCE to float64 and padded to 4 doubles
+// per node (one 32-byte sector).  The widening is exact, so the trilinear read returns the same float64 value
+// as widening at read time; it removes 24 float->double conversions per read from the RKN4 trial loop, whose
+// bottleneck on B200 is the conversion/special-function (XU) pipe (profiles/r01c).
 struct FieldDev {
   int32_t kind;
   int32_t n[3];
   double ub[3];
   double org[3];
   double inv[3];  // 1 / spacing
-  const float4* grid;
+  double nm2[3];  // (double)(n - 2): largest cell index
+  const double* grid;  // [n0 * n1 * n2][4]
 };
 
 struct CfgDev {
@@ -74,11 +78,14 @@ CKF_HD auto dot3(const A a[3], const B b[3]) -> decltype(a[0] * b[0]) {
   return a[0] * b[0] + a[1] * b[1] + a[2] * b[2];
 }
 
-CKF_HD float4 ldg4(const float4* p) {
+struct D3 { double x, y, z; };
+CKF_HD D3 ld_node(const double* p) {
 #if defined(__CUDA_ARCH__)
-  return __ldg(p);
+  const double2 a = __ldg((const double2*)p);
+  const double b = __ldg(p + 2);
+  return D3{a.x, a.y, b};
 #else
-  return *p;
+  return D3{p[0], p[1], p[2]};
 #endif
 }
 
@@ -94,27 +101,35 @@ CKF_HD void field_at(const FieldDev& f, const double r[3], double B[3]) {
 #pragma unroll
   for (int a = 0; a < 3; ++a) {
     const double g = (r[a] - f.org[a]) * f.inv[a];
-    int i = (int)floor(g);
-    i = i < 0 ? 0 : i;
-    i = i > f.n[a] - 2 ? f.n[a] - 2 : i;
-    idx[a] = i;
-    fr[a] = g - (double)i;
+    // i = clamp(floor(g), 0, n - 2) and fr = g - i with float64 adds only (no float<->int conversion
+    // instructions): adding 1.5 * 2^52 rounds g to the nearest integer and leaves that integer in the low
+    // mantissa bits.  NaN and out-of-range g fall to the clamps (fmax/fmin return the non-NaN operand).
+    const double MAGIC = 6755399441055744.0;
+    double ti = (g + MAGIC) - MAGIC;
+    if (ti > g) ti -= 1.0;
+    ti = fmin(fmax(ti, 0.0), f.nm2[a]);
+#if defined(__CUDA_ARCH__)
+    idx[a] = __double2loint(ti + MAGIC);
+#else
+    idx[a] = (int)ti;
+#endif
+    fr[a] = g - ti;
   }
   const long long s1 = f.n[2], s0 = (long long)f.n[1] * f.n[2];
-  const float4* p = f.grid + idx[0] * s0 + idx[1] * s1 + idx[2];
-  const float4 v000 = ldg4(p), v001 = ldg4(p + 1);
-  const float4 v010 = ldg4(p + s1), v011 = ldg4(p + s1 + 1);
-  const float4 v100 = ldg4(p + s0), v101 = ldg4(p + s0 + 1);
-  const float4 v110 = ldg4(p + s0 + s1), v111 = ldg4(p + s0 + s1 + 1);
-#define CKF_TRILERP(C)                                                                     \
-  {                                                                                        \
-    const double x00 = (double)v000.C + fr[0] * ((double)v100.C - (double)v000.C);         \
-    const double x10 = (double)v010.C + fr[0] * ((double)v110.C - (double)v010.C);         \
-    const double x01 = (double)v001.C + fr[0] * ((double)v101.C - (double)v001.C);         \
-    const double x11 = (double)v011.C + fr[0] * ((double)v111.C - (double)v011.C);         \
-    const double y0 = x00 + fr[1] * (x10 - x00);                                           \
-    const double y1 = x01 + fr[1] * (x11 - x01);                                           \
-    out = y0 + fr[2] * (y1 - y0);                                                          \
+  const double* p = f.grid + 4 * (idx[0] * s0 + idx[1] * s1 + idx[2]);
+  const D3 v000 = ld_node(p), v001 = ld_node(p + 4);
+  const D3 v010 = ld_node(p + 4 * s1), v011 = ld_node(p + 4 * s1 + 4);
+  const D3 v100 = ld_node(p + 4 * s0), v101 = ld_node(p + 4 * s0 + 4);
+  const D3 v110 = ld_node(p + 4 * (s0 + s1)), v111 = ld_node(p + 4 * (s0 + s1) + 4);
+#define CKF_TRILERP(C)                                              \
+  {                                                                 \
+    const double x00 = v000.C + fr[0] * (v100.C - v000.C);          \
+    const double x10 = v010.C + fr[0] * (v110.C - v010.C);          \
+    const double x01 = v001.C + fr[0] * (v101.C - v001.C);          \
+    const double x11 = v011.C + fr[0] * (v111.C - v011.C);          \
+    const double y0 = x00 + fr[1] * (x10 - x00);                    \
+    const double y1 = x01 + fr[1] * (x11 - x01);                    \
+    out = y0 + fr[2] * (y1 - y0);                                   \
   }
   double out;
   CKF_TRILERP(x) B[0] = out;
@@ -254,7 +269,7 @@ CKF_HD void jac_column_q(T lam, T h, T qf, const T B1[3], const T B2[3], const T
 // Accept a trial: D <- D_step D column by column (J2, J3), then the state (P2).  The four columns go through
 // ONE copy of the column code: a rolled loop that rotates the columns through fixed registers.
 template <typename T>
-CKF_HD void rk_accept(Traj& y, Jac<T>& J, double h, const Trial<T>& t, double mass) {
+CKF_HD void rk_accept(Traj& y, Jac<T>& J, double h, const Trial<T>& t, double ib, double dib) {
   {
     const T lamT = (T)(KAPPA * y.qop), hT = (T)h;
 #if CKF_JAC_ROLLED
@@ -281,7 +296,7 @@ CKF_HD void rk_accept(Traj& y, Jac<T>& J, double h, const Trial<T>& t, double ma
     }
     jac_column_q<T>(lamT, hT, T(1), t.B1, t.B2, t.B4, t.q1, t.q2, t.q3, t.q4, J.rq, J.dq);
 #endif
-    J.tq += (T)(h * dinvbeta_dqop(y.qop, mass));
+    J.tq += (T)(h * dib);
   }
   const double h6 = h / 6.0, hh6 = h * h / 6.0;
   double dn[3], n2 = 0.0;
@@ -294,12 +309,12 @@ CKF_HD void rk_accept(Traj& y, Jac<T>& J, double h, const Trial<T>& t, double ma
   const double nrm = sqrt(n2);
 #pragma unroll
   for (int i = 0; i < 3; ++i) y.d[i] = dn[i] / nrm;
-  y.t += h * inv_beta(y.qop, mass);
+  y.t += h * ib;
 }
 
 // P5: field-free closing step of length s.
 template <typename T>
-CKF_HD void straight_close(Traj& y, Jac<T>& J, double s, double mass) {
+CKF_HD void straight_close(Traj& y, Jac<T>& J, double s, double ib, double dib) {
   const T sT = (T)s;
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
@@ -308,8 +323,8 @@ CKF_HD void straight_close(Traj& y, Jac<T>& J, double s, double mass) {
     J.rq[i] += sT * J.dq[i];
     y.r[i] += s * y.d[i];
   }
-  J.tq += (T)(s * dinvbeta_dqop(y.qop, mass));
-  y.t += s * inv_beta(y.qop, mass);
+  J.tq += (T)(s * dib);
+  y.t += s * ib;
 }
 
 // ------------------------------------------------------------------------------------------ step control

@@ -244,45 +244,54 @@ template <typename T>
 struct Move {
   Traj y;
   Jac<T> D;
-  T dep_d[3];           // direction on departure (J1)
-  T q_phi, q_theta;     // Highland variances to add before transport (V5)
   double tc[3], tn[3];  // target plane (PH_PLANE)
   double R;             // target cylinder radius (PH_CYL)
   double h, h_ctrl;
+  double ib, dib;       // 1/beta and d(1/beta)/d(q/p): constant along the move (no energy loss)
   int phase, stop, from, tgt, lp, n_steps;
   bool retry;
 };
 
-// Validation + departure state.  Leaves the move in PH_START, or PH_FIN with stop = NUMERIC.
+// Departure state of a tip with bound parameters x on module `from` (J1, V5): global position and direction,
+// the direction as T for the bound->free Jacobian, and the Highland variances to add to C[phi][phi],
+// C[theta][theta] on leaving.  Returns STOP_NUMERIC for non-finite parameters or theta outside (0, pi).
 template <typename T>
-CKF_HD void move_init(Move<T>& m, const GeoDev& g, const CfgDev& cfg, int from, const double x[6]) {
-  m.from = from; m.tgt = -1; m.lp = 0; m.n_steps = 0; m.retry = false; m.stop = STOP_NONE;
-  m.h = 0.0; m.h_ctrl = cfg.h_max; m.R = 0.0;
-  m.q_theta = T(0); m.q_phi = T(0);
-  m.y.qop = 0.0;
+CKF_HD int departure_state(const GeoDev& g, const CfgDev& cfg, int from, const double x[6], Traj& y, T dep[5]) {
   bool ok = true;
 #pragma unroll
   for (int i = 0; i < 6; ++i) ok = ok && isfinite(x[i]);
   ok = ok && (x[3] > 0.0 && x[3] < PI_D);
-  if (!ok) { m.stop = STOP_NUMERIC; m.phase = PH_FIN; return; }
+  if (!ok) return STOP_NUMERIC;
   const ModuleRec& k = g.mod[from];
   double sp, cp, st, ct;
   sincos(x[2], &sp, &cp);
   sincos(x[3], &st, &ct);
-  m.y.d[0] = st * cp; m.y.d[1] = st * sp; m.y.d[2] = ct;
+  y.d[0] = st * cp; y.d[1] = st * sp; y.d[2] = ct;
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
-    m.y.r[i] = k.c[i] + x[0] * k.u[i] + x[1] * k.v[i];
-    m.dep_d[i] = (T)m.y.d[i];
+    y.r[i] = k.c[i] + x[0] * k.u[i] + x[1] * k.v[i];
+    dep[i] = (T)y.d[i];
   }
-  m.y.t = x[5];
-  m.y.qop = x[4];
+  y.t = x[5];
+  y.qop = x[4];
+  dep[3] = T(0);  // q_phi
+  dep[4] = T(0);  // q_theta
   if (k.xx0 > 0.0) {
-    const double th2 = highland_theta0_sq(k.xx0, fabs(dot3(m.y.d, k.n)), m.y.qop, cfg.mass);
-    m.q_theta = (T)th2;
-    m.q_phi = (T)(th2 / (st * st));
+    const double th2 = highland_theta0_sq(k.xx0, fabs(dot3(y.d, k.n)), y.qop, cfg.mass);
+    dep[4] = (T)th2;
+    dep[3] = (T)(th2 / (st * st));
   }
+  return STOP_NONE;
+}
+
+// Start of a move whose m.y holds the departure state: identity transport, fresh step control (P4, J3).
+template <typename T>
+CKF_HD void move_begin(Move<T>& m, const CfgDev& cfg, int from) {
+  m.from = from; m.tgt = -1; m.lp = 0; m.n_steps = 0; m.retry = false; m.stop = STOP_NONE;
+  m.h = 0.0; m.h_ctrl = cfg.h_max; m.R = 0.0;
   jac_identity(m.D);
+  m.ib = inv_beta(m.y.qop, cfg.mass);
+  m.dib = dinvbeta_dqop(m.y.qop, cfg.mass);
   m.phase = PH_START;
 }
 
@@ -349,7 +358,7 @@ CKF_HD void move_step(Move<T>& m, const FieldDev& fld, const CfgDev& cfg, int& n
     }
     if (!isfinite(s)) { m.stop = STOP_NUMERIC; m.phase = PH_FIN; return; }
     if (fabs(s) <= cfg.surf_tol) {
-      straight_close(m.y, m.D, s, cfg.mass);  // P5
+      straight_close(m.y, m.D, s, m.ib, m.dib);  // P5
       m.phase = (m.phase == PH_PLANE) ? PH_FIN : PH_LANDED;
       return;
     }
@@ -370,7 +379,7 @@ CKF_HD void move_step(Move<T>& m, const FieldDev& fld, const CfgDev& cfg, int& n
     f = f > 4.0 ? 4.0 : f;
   }
   if (t.eps <= cfg.rk_tol) {
-    rk_accept<T>(m.y, m.D, m.h, t, cfg.mass);
+    rk_accept<T>(m.y, m.D, m.h, t, m.ib, m.dib);
     m.h_ctrl = fabs(m.h) * f;
     ++n_accepted;
   } else {
@@ -382,13 +391,13 @@ CKF_HD void move_step(Move<T>& m, const FieldDev& fld, const CfgDev& cfg, int& n
 // Arrival (J4, J5) of a move in PH_FIN with stop == NONE: predicted bound parameters and the 5x5 Jacobian
 // block.  Returns the final stop reason (NUMERIC if a predicted parameter is not finite).
 template <typename T>
-CKF_HD int move_arrive(const Move<T>& m, const GeoDev& g, const FieldDev& fld, const CfgDev& cfg, double xp[6],
-                       T J[5][5]) {
+CKF_HD int move_arrive(const Move<T>& m, const T dep[5], const GeoDev& g, const FieldDev& fld, const CfgDev& cfg,
+                       double xp[6], T J[5][5]) {
   const ModuleRec& k = g.mod[m.tgt];
   const ModuleRec& m0 = g.mod[m.from];
   double B[3];
   field_at(fld, m.y.r, B);
-  arrival_jacobian(m.D, m0.u, m0.v, m.dep_d, k, m.y, B, cfg.mass, J);
+  arrival_jacobian(m.D, m0.u, m0.v, dep, k, m.y, B, cfg.mass, J);
   const double rel[3] = {m.y.r[0] - k.c[0], m.y.r[1] - k.c[1], m.y.r[2] - k.c[2]};
   xp[0] = dot3(rel, k.u);
   xp[1] = dot3(rel, k.v);
@@ -407,7 +416,10 @@ template <typename T>
 CKF_HD int move_to_next_module(const GeoDev& g, const FieldDev& fld, const CfgDev& cfg, int from, const double x[6],
                                int& target, double xp[6], T J[5][5], T& q_phi, T& q_theta, StepCtl& sc) {
   Move<T> m;
-  move_init(m, g, cfg, from, x);
+  T dep[5];
+  const int st0 = departure_state<T>(g, cfg, from, x, m.y, dep);
+  if (st0 != STOP_NONE) return st0;
+  move_begin(m, cfg, from);
   while (m.phase != PH_FIN) {
     if (m.phase == PH_START || m.phase == PH_LANDED) {
       PickRequest q;
@@ -418,10 +430,10 @@ CKF_HD int move_to_next_module(const GeoDev& g, const FieldDev& fld, const CfgDe
       move_step(m, fld, cfg, sc.n_trials, sc.n_accepted);
     }
   }
-  q_phi = m.q_phi;
-  q_theta = m.q_theta;
+  q_phi = dep[3];
+  q_theta = dep[4];
   if (m.stop != STOP_NONE) return m.stop;
-  const int st = move_arrive(m, g, fld, cfg, xp, J);
+  const int st = move_arrive(m, dep, g, fld, cfg, xp, J);
   if (st == STOP_NONE) target = m.tgt;
   return st;
 }

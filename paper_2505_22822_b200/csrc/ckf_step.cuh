@@ -1,0 +1,168 @@
+// ckf_step.cuh — navigation + adaptive RKN4 of every tip of a level (a4, a5): the hot kernel.
+//
+// Persistent lanes: every lane owns one Move (ckf_nav.cuh) at a time and pulls the next tip of the level
+// from a global cursor when its move is done, so lanes do not idle while a neighbour needs more RKN4 trials
+// (the imbalance the paper names).  The code that is not the trial — write-back + fetch,
+// module choice — runs at SERVICE points: lanes that finished, lanes without a tip and lanes that need a
+// module choice wait until SERVICE_MIN of them have gathered (or no lane can step), then are served together.
+// The module choice spreads its nine straight-line tests per tip over all 32 lanes.
+#pragma once
+#include "ckf_kernels.cuh"
+
+namespace ckf {
+
+// scratch of one warp for the module choice
+struct PickSmem {
+  double* hit;     // [9][32] path length of each (tip, neighbour) test; NaN = no hit
+  double* rd;      // [6][32] position and direction of the requesting tips
+  int32_t* hid;    // [9][32] module id of each test
+  int32_t *rl, *ri, *rj, *rx, *list;  // [32] request: layer, iphi, iz, exclude | s_min sign; compacted lanes
+  static constexpr size_t BYTES = 8 * 9 * 32 + 8 * 6 * 32 + 4 * 9 * 32 + 4 * 5 * 32;
+  __host__ __device__ static constexpr size_t bytes() { return BYTES; }
+  __device__ void carve(unsigned char* raw) {
+    unsigned char* p = raw;
+    hit = (double*)p; p += 8 * 9 * 32;
+    rd = (double*)p; p += 8 * 6 * 32;
+    hid = (int32_t*)p; p += 4 * 9 * 32;
+    rl = (int32_t*)p; p += 4 * 32;
+    ri = (int32_t*)p; p += 4 * 32;
+    rj = (int32_t*)p; p += 4 * 32;
+    rx = (int32_t*)p; p += 4 * 32;
+    list = (int32_t*)p; p += 4 * 32;
+  }
+};
+
+// a4: module choice for all lanes in PH_START / PH_LANDED at once (N2, N4).  The nine tests of each requesting
+// tip are flattened into (tip, neighbour) pairs over the 32 lanes; the owning lane then scans its nine
+// results in the order of the sequential rule (nearest first, tie -> lower id).
+template <typename T>
+__device__ __forceinline__ void pick_warp(const GeoDev& geo, const PickSmem& ps, Move<T>& m, int lane) {
+  const bool need = m.phase == PH_START || m.phase == PH_LANDED;
+  PickRequest q;
+  bool ok = false;
+  if (need) ok = move_pick_request(m, geo, q);
+  const unsigned breq = __ballot_sync(0xffffffffu, ok);
+  if (ok) {
+    ps.rl[lane] = q.layer; ps.ri[lane] = q.iphi; ps.rj[lane] = q.iz;
+    ps.rx[lane] = (q.exclude < 0 ? 0 : q.exclude + 1) * 2 + (q.s_min > 0.0 ? 1 : 0);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { ps.rd[i * 32 + lane] = m.y.r[i]; ps.rd[(3 + i) * 32 + lane] = m.y.d[i]; }
+    ps.list[__popc(breq & ((1u << lane) - 1u))] = lane;
+  }
+  __syncwarp();
+  const int total = 9 * __popc(breq);
+  for (int q0 = 0; q0 < total; q0 += 32) {
+    const int pr = q0 + lane;
+    if (pr < total) {
+      const int t = ps.list[pr / 9], nb = pr % 9;
+      const LayerRec L = geo.layer[ps.rl[t]];
+      int ii = ps.ri[t] + (nb / 3 - 1);
+      ii = ii < 0 ? ii + L.n_phi : (ii >= L.n_phi ? ii - L.n_phi : ii);
+      const int jj = ps.rj[t] + (nb % 3 - 1);
+      const int rx = ps.rx[t];
+      double sres = __longlong_as_double(0x7ff8000000000000LL);
+      int id = -1;
+      if (jj >= 0 && jj < L.n_z) {
+        id = L.offset + ii * L.n_z + jj;
+        if (id != (rx >> 1) - 1) {
+          const double r[3] = {ps.rd[0 * 32 + t], ps.rd[1 * 32 + t], ps.rd[2 * 32 + t]};
+          const double d[3] = {ps.rd[3 * 32 + t], ps.rd[4 * 32 + t], ps.rd[5 * 32 + t]};
+          double sv;
+          if (line_hits_module(geo.mod[id], r, d, (rx & 1) ? 1e-3 : -1e-3, sv)) sres = sv;
+        }
+      }
+      ps.hit[nb * 32 + t] = sres;
+      ps.hid[nb * 32 + t] = id;
+    }
+  }
+  __syncwarp();
+  if (need) {
+    int best = -1;
+    double best_s = 0.0;
+    if (ok) {
+#pragma unroll 1
+      for (int nb = 0; nb < 9; ++nb) {
+        const double sv = ps.hit[nb * 32 + lane];
+        const int id = ps.hid[nb * 32 + lane];
+        if (sv == sv && (best < 0 || sv < best_s || (sv == best_s && id < best))) { best = id; best_s = sv; }
+      }
+    }
+    move_pick_apply(m, geo, best);
+  }
+  __syncwarp();
+}
+
+template <typename T, int MINB>
+__global__ void __launch_bounds__(STEP_NT, MINB) ckf_step(const KParams<T> p, int level) {
+  const int n = p.g[G_NTIPS0 + (level & 1)];
+  if (n == 0 || level == 0) return;  // level 0: the seed's own module, identity transport (N6)
+  __shared__ __align__(16) unsigned char smem_raw[(STEP_NT / 32) * PickSmem::bytes()];
+  const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
+  PickSmem ps;
+  ps.carve(smem_raw + (size_t)wib * PickSmem::bytes());
+  const size_t TC = (size_t)p.tcap;
+
+  Move<T> m;
+  m.phase = PH_IDLE; m.stop = STOP_NONE; m.from = 0; m.tgt = -1; m.lp = 0; m.n_steps = 0; m.retry = false;
+  m.h = 0.0; m.h_ctrl = 0.0; m.R = 0.0; m.y.qop = 0.0; m.ib = 0.0; m.dib = 0.0;
+  int tip = -1, nt = 0, na = 0;
+  bool more = true;  // the level's cursor is not exhausted (warp-uniform)
+  for (;;) {
+    const unsigned bI = __ballot_sync(0xffffffffu, m.phase == PH_IDLE);
+    const unsigned bP = __ballot_sync(0xffffffffu, m.phase == PH_START || m.phase == PH_LANDED);
+    const unsigned bS = __ballot_sync(0xffffffffu, m.phase == PH_CYL || m.phase == PH_PLANE);
+    const unsigned bF = __ballot_sync(0xffffffffu, m.phase == PH_FIN);
+    if (!bP && !bS && !bF && !more) break;
+    const int waiting = __popc(bF) + __popc(bP) + (more ? __popc(bI) : 0);
+    if (bS == 0u || waiting >= SERVICE_MIN) {
+      // ---- write-back of finished moves
+      if (m.phase == PH_FIN) {
+        if (m.stop == STOP_NONE) {
+#pragma unroll
+          for (int i = 0; i < 3; ++i) { p.mv_y[i * TC + tip] = m.y.r[i]; p.mv_y[(3 + i) * TC + tip] = m.y.d[i]; }
+          p.mv_y[6 * TC + tip] = m.y.t;
+#pragma unroll
+          for (int i = 0; i < 3; ++i) {
+#pragma unroll
+            for (int j = 0; j < 3; ++j) {
+              p.mv_D[(i * 3 + j) * TC + tip] = m.D.Rd[i][j];
+              p.mv_D[(9 + i * 3 + j) * TC + tip] = m.D.Dd[i][j];
+            }
+            p.mv_D[(18 + i) * TC + tip] = m.D.rq[i];
+            p.mv_D[(21 + i) * TC + tip] = m.D.dq[i];
+          }
+          p.mv_D[24 * TC + tip] = m.D.tq;
+          p.mv_tgt[tip] = m.tgt;
+        }
+        p.mv_stop[tip] = m.stop;
+        m.phase = PH_IDLE;
+      }
+      // ---- fetch: idle lanes take the next tips of the level, in order
+      const unsigned idle = __ballot_sync(0xffffffffu, m.phase == PH_IDLE);
+      if (idle && more) {
+        int base = 0;
+        if (lane == 0) base = atomicAdd(p.g + G_STEP_CURSOR, __popc(idle));
+        base = __shfl_sync(0xffffffffu, base, 0);
+        if (base + __popc(idle) >= n) more = false;
+        const int t = base + __popc(idle & ((1u << lane) - 1u));
+        if (m.phase == PH_IDLE && t < n && p.mv_stop[t] == STOP_NONE) {
+          tip = t;
+#pragma unroll
+          for (int i = 0; i < 3; ++i) { m.y.r[i] = p.mv_y[i * TC + t]; m.y.d[i] = p.mv_y[(3 + i) * TC + t]; }
+          m.y.t = p.mv_y[6 * TC + t];
+          m.y.qop = p.mv_y[7 * TC + t];
+          move_begin<T>(m, p.cfg, p.mv_from[t]);
+        }
+      }
+      // ---- module choice for every lane that needs one
+      if (__ballot_sync(0xffffffffu, m.phase == PH_START || m.phase == PH_LANDED)) pick_warp<T>(p.geo, ps, m, lane);
+    }
+    // ---- one step: targeting + landing, else one RKN4 trial
+    if (m.phase == PH_CYL || m.phase == PH_PLANE) move_step<T>(m, p.fld, p.cfg, nt, na);
+    __syncwarp();
+  }
+  flush_counter(p.counters + CNT_TRIALS, (unsigned long long)nt);
+  flush_counter(p.counters + CNT_ACCEPTED, (unsigned long long)na);
+}
+
+}  // namespace ckf

@@ -15,7 +15,7 @@ namespace {
 struct Ctx {
   std::vector<ModuleRec> mods;
   std::vector<LayerRec> layers;
-  std::vector<float4> grid;
+  std::vector<double> grid;
   GeoDev geo;
   FieldDev fld;
   CfgDev cfg;
@@ -68,11 +68,13 @@ void* hm_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c) 
   for (int a = 0; a < 3; ++a) {
     x->fld.ub[a] = f->uniform_b[a]; x->fld.n[a] = f->n[a]; x->fld.org[a] = f->origin[a];
     x->fld.inv[a] = f->kind == 1 ? 1.0 / f->spacing[a] : 0.0;
+    x->fld.nm2[a] = (double)(f->n[a] - 2);
   }
   if (f->kind == 1) {
     const size_t np = (size_t)f->n[0] * f->n[1] * f->n[2];
-    x->grid.resize(np);
-    for (size_t i = 0; i < np; ++i) x->grid[i] = make_float4(f->grid[3 * i], f->grid[3 * i + 1], f->grid[3 * i + 2], 0.f);
+    x->grid.resize(4 * np);
+    for (size_t i = 0; i < np; ++i)
+      for (int k = 0; k < 3; ++k) x->grid[4 * i + k] = (double)f->grid[3 * i + k];
     x->fld.grid = x->grid.data();
   }
   x->cfg.chi2_max = c->chi2_max; x->cfg.rk_tol = c->rk_tolerance_mm; x->cfg.surf_tol = c->surface_tolerance_mm;
