@@ -34,8 +34,9 @@ E2E_STREAMS = 4
 F_FIELD_GRID = 75       # one trilinear read
 F_TRIAL = 108           # one RKN4 trial without the three field reads
 F_ACCEPT = 500          # state update 50 + four Jacobian columns 450
+F_NAV = 600             # navigation of one visit (ckf_step): ~1.7 module choices x 9 modules x 35 + targeting
 F_VISIT = 1450          # navigation 600 + arrival Jacobian, covariance transport, bound parameters 850
-F_GATE = 17             # one chi2
+F_GATE = 17             # one chi2 actually evaluated (inside a loc0 window)
 F_UPDATE = 155          # one gain-form update
 # plain-ALU peaks from the guide's unit counts: 148 SMs x 128 FP32 (64 FP64) lanes x 2 flop x 1.965 GHz
 PEAK_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
@@ -46,7 +47,7 @@ def algorithmic_flops(cnt: dict, grid_field: bool):
     """(total flop, flop the design computes in float64) for one launch, from the library's work counters."""
     f_trial = F_TRIAL + (3 * F_FIELD_GRID if grid_field else 0)
     traj = cnt["rk_trials"] * f_trial + cnt["rk_accepted"] * 50 + cnt["visits"] * 700   # float64 in both modes
-    cov = cnt["rk_accepted"] * 450 + cnt["visits"] * 750 + cnt["gate_tests"] * F_GATE + cnt["updates"] * F_UPDATE
+    cov = cnt["rk_accepted"] * 450 + cnt["visits"] * 750 + cnt["gate_tests_executed"] * F_GATE + cnt["updates"] * F_UPDATE
     return float(traj + cov), float(traj)
 
 
@@ -150,6 +151,7 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--streams", type=int, default=4, help="events kept in flight (CUDA streams) for `value`")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -172,21 +174,30 @@ def main():
     det, fld, cfg, evs = make_events(N_EVENTS, first_index=rank * N_EVENTS)
     max_s = max(e.n_seeds for e in evs)
     max_m = max(e.n_measurements for e in evs)
+    S = max(1, args.streams)
     ckf = CKF(det, fld, cfg.ckf, cfg.precision, max_seeds=max_s, max_measurements=max_m, max_tracks=8 * max_s,
-              max_track_entries=80 * max_s, n_streams=E2E_STREAMS + 1)
+              max_track_entries=80 * max_s, n_streams=max(S, E2E_STREAMS) + 1)
     devs = [ckf.upload_event(e) for e in evs]
-    out = ckf.alloc_tracks()
     stream = torch.cuda.current_stream()
+    work = [torch.cuda.Stream() for _ in range(S)]
+    outs = [ckf.alloc_tracks() for _ in range(S)]
+    out = outs[0]
 
-    def step(i):
+    # one step = one ckf_find over one event; the K steps are independent events, kept S at a time in flight on S
+    # CUDA streams (the paper's own throughput mode: one event pipeline per stream)
+    def run_steps(k):
+        for i in range(k):
+            ckf.find(devs[i % N_EVENTS], outs[i % S], work[i % S])
+
+    W = max(3, args.warmup)
+    for i in range(W):
         ckf.find(devs[i % N_EVENTS], out, stream)
-
-    for i in range(max(3, args.warmup)):
-        step(i)
     torch.cuda.synchronize()
     cnt = ckf.counters(stream)                      # of event (warmup-1) % N
     res = ckf.download(out)
-    ev_last = evs[(max(3, args.warmup) - 1) % N_EVENTS]
+    ev_last = evs[(W - 1) % N_EVENTS]
+    run_steps(S)                                    # warm the per-stream workspaces
+    torch.cuda.synchronize()
 
     sampler = ClockSampler(local)
     sampler.start()
@@ -197,8 +208,11 @@ def main():
     t0 = torch.cuda.Event(enable_timing=True)
     t1 = torch.cuda.Event(enable_timing=True)
     t0.record(stream)
-    for i in range(args.steps):
-        step(i)
+    for w in work:
+        w.wait_stream(stream)
+    run_steps(args.steps)
+    for w in work:
+        stream.wait_stream(w)
     t1.record(stream)
     torch.cuda.synchronize()
     if world > 1:
@@ -206,18 +220,25 @@ def main():
     ms_total = t0.elapsed_time(t1)
     seeds_done = sum(evs[i % N_EVENTS].n_seeds for i in range(args.steps))
 
-    # dominant kernel alone: CUDA events around the level-loop share is not separable from outside the library,
-    # so time whole finds one by one (events on the launching stream) and take the level loop's share from the
-    # committed ncu launch list (profiles/): init + scan + emit + finalize are < 3 % of a step.
+    # single-event latency (one stream, finds back to back) and the per-kernel device times of the dominant
+    # kernel, ckf_step, measured live with CUDA events on the launching stream (ckf_set_timing)
     per = []
     for i in range(min(args.steps, 8)):
         a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
         a.record(stream)
-        step(i)
+        ckf.find(devs[i % N_EVENTS], out, stream)
         b.record(stream)
         torch.cuda.synchronize()
         per.append(a.elapsed_time(b))
+    ckf.set_timing(True)
+    tim = []
+    for i in range(min(args.steps, 8)):
+        ckf.find(devs[(W - 1) % N_EVENTS], out, stream)
+        torch.cuda.synchronize()
+        tim.append(ckf.timing(stream))
+    ckf.set_timing(False)
     clocks = sampler.stop()
+    launches_per_find = int(tim[0]["launches"])
 
     # ---- e2e: host buffers through ckf_find_host on 4 streams / 4 host threads (configs[4] shape)
     hevs = [ckf.pinned_event(e) for e in evs]
@@ -254,10 +275,17 @@ def main():
     if rank == 0:
         flop, flop64 = algorithmic_flops(cnt, grid_field=cfg.inhomogeneous)
         k_ms = float(np.mean(per))
-        achieved = flop / (k_ms * 1e-3) / 1e12
-        # serial-pipe peak for this launch's fp32/fp64 mix
-        f64_share = flop64 / flop if cfg.precision == 32 else 1.0
+        # dominant kernel: ckf_step (navigation + RKN4 trials + Jacobian columns), all its launches of one find
+        step_ms = float(np.mean([t["step_ms"] for t in tim]))
+        f_trial = F_TRIAL + (3 * F_FIELD_GRID if cfg.inhomogeneous else 0)
+        step64 = cnt["rk_trials"] * f_trial + cnt["rk_accepted"] * 50 + cnt["visits"] * F_NAV
+        step32 = cnt["rk_accepted"] * 450
+        step_flop = float(step64 + step32)
+        achieved = step_flop / (step_ms * 1e-3) / 1e12
+        # serial-pipe peak for this kernel's fp32/fp64 mix
+        f64_share = step64 / step_flop if cfg.precision == 32 else 1.0
         peak = 1.0 / (f64_share / PEAK_FP64_TFLOPS + (1.0 - f64_share) / PEAK_FP32_TFLOPS)
+        step_launches = sum(1 for _ in range(cfg.ckf.max_levels))
         line = {
             "metric": "CKF seeds/sec (40k-particle event)", "value": value, "unit": "seeds/s", "n_gpus": world,
             "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms_step, "higher_is_better": True,
@@ -267,19 +295,25 @@ def main():
                                    "float32 grid field, k=10, cap=100", "seeds_per_event": ev_last.n_seeds,
                        "measurements_per_event": ev_last.n_measurements, "distinct_events_rotated": N_EVENTS,
                        "l2": "4 events rotated; each step writes a >190 MB link buffer (> 126 MB L2)",
-                       "launch": ckf.launch_info()},
+                       "events_in_flight": S, "how": "K independent events, S at a time on S CUDA streams, device "
+                       "timed from the first launch to the last completion", "launch": ckf.launch_info()},
+            "latency_ms_single_event": k_ms, "seeds_per_s_single_stream": ev_last.n_seeds / (k_ms * 1e-3),
             "events_per_s": value / ev_last.n_seeds,
             "e2e": {"value": e2e_value, "unit": "seeds/s", "h2d_bytes_per_step": int(bi), "d2h_bytes_per_step": int(bo),
                     "streams": E2E_STREAMS, "events": n_e2e, "events_per_s": e2e_value / ev_last.n_seeds,
                     "how": "ckf_find_host, pinned host buffers, 4 host threads x 4 CUDA streams, wall clock"},
-            "gpu_launches": 6 * args.steps,
+            "gpu_launches": launches_per_find * args.steps,
             "clocks": clocks,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
-                         "traffic": None, "kernel": "ckf_level_loop", "flop_per_launch": flop,
+                         "traffic": None, "kernel": "ckf_step (all %d launches of one find)" % step_launches,
+                         "flop_per_find_this_kernel": step_flop, "kernel_ms_per_find": step_ms,
+                         "share_of_find": step_ms / max(sum(v for k, v in tim[0].items() if k.endswith("_ms")), 1e-9),
+                         "whole_path_flop_per_find": flop, "whole_path_tflops": flop / (k_ms * 1e-3) / 1e12,
+                         "kernel_ms_by_phase": {k: float(np.mean([t[k] for t in tim])) for k in tim[0] if k.endswith("_ms")},
                          "fp64_share_of_flop": f64_share, "peak_fp32": PEAK_FP32_TFLOPS, "peak_fp64": PEAK_FP64_TFLOPS,
                          "peak_source": "derived from the guide's unit counts and max clock (DESIGN.md §7); "
                                         "MEASURED_PEAKS.json has no ALU peak",
-                         "hbm_gbs_achieved": (bi + bo) / (k_ms * 1e-3) / 1e9, "launch_ms": k_ms,
+                         "hbm_gbs_achieved": (bi + bo) / (k_ms * 1e-3) / 1e9,
                          "counters": cnt},
         }
         if not args.no_cpu_baseline:

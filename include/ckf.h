@@ -178,6 +178,24 @@ int ckf_find_host(ckf_handle* handle, const ckf_measurements* measurements, cons
 /* Copies the work counters of the most recent ckf_find issued on `cuda_stream` (synchronises that stream). */
 int ckf_get_counters(ckf_handle* handle, void* cuda_stream, ckf_counters* out);
 
+/* Per-kernel device times of one ckf_find, summed over the levels (CUDA events on the call's stream). */
+typedef struct {
+  float init_ms;          /* per-event reset                                                            */
+  float sort_ms;          /* gate index (slice sort)                                                    */
+  float step_ms;          /* ckf_step: navigation + adaptive RKN4 + Jacobian transport (the hot kernel) */
+  float visit_ms;         /* ckf_visit: arrival Jacobian, covariance transport, chi2 gate, k best       */
+  float scan_ms;          /* ckf_scan: per-seed cap, emission records, child offsets                    */
+  float update_ms;        /* ckf_update: Kalman update, link append, departure state                    */
+  float emit_ms;          /* emission: seed scan, backtrace, finalize                                   */
+  int32_t launches;       /* kernel launches of one ckf_find                                            */
+} ckf_timing;
+
+/* Measurement aid.  ckf_set_timing(handle, 1) makes every later ckf_find record a CUDA event after each
+ * kernel and SYNCHRONISE its stream at the end (so it is off by default); ckf_get_timing returns the times of
+ * the most recent timed ckf_find issued on `cuda_stream`. */
+int ckf_set_timing(ckf_handle* handle, int on);
+int ckf_get_timing(ckf_handle* handle, void* cuda_stream, ckf_timing* out);
+
 /* Launch configuration chosen at ckf_create for the hot kernel (ckf_step: navigation + RKN4): thread blocks,
  * threads per block, shared bytes, registers per thread (any pointer may be NULL). */
 int ckf_get_launch_info(const ckf_handle* handle, int32_t* blocks, int32_t* threads, int32_t* smem_bytes,

@@ -21,6 +21,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libckf.so")
 
 EXPORTS = ("ckf_create", "ckf_find", "ckf_find_host", "ckf_get_counters", "ckf_get_launch_info", "ckf_destroy",
+           "ckf_set_timing", "ckf_get_timing",
            "ckf_last_error", "ckf_abi_version")
 
 
@@ -59,6 +60,11 @@ class ckf_tracks(C.Structure):
                 ("chi2_sum", _vp), ("entry_chi2", _vp)]
 
 
+class ckf_timing(C.Structure):
+    _fields_ = [("init_ms", C.c_float), ("sort_ms", C.c_float), ("step_ms", C.c_float), ("visit_ms", C.c_float),
+                ("scan_ms", C.c_float), ("update_ms", C.c_float), ("emit_ms", C.c_float), ("launches", C.c_int32)]
+
+
 class ckf_counters(C.Structure):
     _fields_ = [("tips", C.c_int64), ("visits", C.c_int64), ("rk_trials", C.c_int64), ("rk_accepted", C.c_int64),
                 ("gate_tests", C.c_int64), ("updates", C.c_int64), ("links", C.c_int64), ("iterations", C.c_int64),
@@ -82,6 +88,10 @@ def load_library():
             fn = getattr(L, name)
             fn.restype = C.c_int
             fn.argtypes = [_vp, C.POINTER(ckf_measurements), C.POINTER(ckf_seeds), C.POINTER(ckf_tracks), _vp]
+        L.ckf_set_timing.restype = C.c_int
+        L.ckf_set_timing.argtypes = [_vp, C.c_int]
+        L.ckf_get_timing.restype = C.c_int
+        L.ckf_get_timing.argtypes = [_vp, _vp, C.POINTER(ckf_timing)]
         L.ckf_get_counters.restype = C.c_int
         L.ckf_get_counters.argtypes = [_vp, _vp, C.POINTER(ckf_counters)]
         L.ckf_get_launch_info.restype = C.c_int
@@ -257,6 +267,17 @@ class CKF:
                            cpu["n_holes"][:nt].copy(), cpu["last_module"][:nt].copy(), cpu["stop_reason"][:nt].copy(),
                            cpu["params"][:nt].astype(np.float64), cpu["cov"][:nt].astype(np.float64),
                            cpu["chi2_sum"][:nt].astype(np.float64))
+
+    def set_timing(self, on: bool) -> None:
+        self.lib.ckf_set_timing(self.handle, 1 if on else 0)
+
+    def timing(self, stream=None) -> dict:
+        st = stream if stream is not None else self.torch.cuda.current_stream()
+        t = ckf_timing()
+        rc = self.lib.ckf_get_timing(self.handle, _vp(st.cuda_stream), C.byref(t))
+        if rc != 0:
+            raise RuntimeError("ckf_get_timing failed: %s" % self.lib.ckf_last_error(self.handle).decode())
+        return {k: getattr(t, k) for k, _ in ckf_timing._fields_}
 
     def counters(self, stream=None) -> dict:
         st = stream if stream is not None else self.torch.cuda.current_stream()

@@ -1,13 +1,14 @@
 // ckf.cu — C ABI of the B200-native CKF track-finding library (include/ckf.h): host side.
 //
 // ckf_create uploads the geometry store (a1) and field store (a2) once and reserves every
-// workspace; ckf_find enqueues its launches (five small kernels per level) on the caller's stream and never allocates.
+// workspace; ckf_find enqueues its launches (four small kernels per level) on the caller's stream and never allocates.
 // There is no CPU path in this library: all arithmetic of the method runs in the kernels of
 // ckf_step.cuh / ckf_visit.cuh / ckf_branch.cuh / ckf_sort.cuh / ckf_emit.cuh.
 #include <cuda_runtime.h>
 
 #include <cstdarg>
 #include <cstdio>
+#include <cstdlib>
 #include <cstring>
 #include <mutex>
 #include <string>
@@ -40,7 +41,7 @@ struct Workspace {
   double *mv_y = nullptr, *pd_x = nullptr;
   void *mv_D = nullptr, *mv_dep = nullptr, *pd_C = nullptr, *sel_chi2 = nullptr;
   int32_t *mv_from = nullptr, *mv_tgt = nullptr, *mv_stop = nullptr, *sel_idx = nullptr;
-  int32_t *t_nsel = nullptr, *t_want = nullptr, *t_counts = nullptr, *t_keep = nullptr, *t_kex = nullptr, *blk_sum = nullptr;
+  int32_t *t_nsel = nullptr, *t_want = nullptr, *t_counts = nullptr, *t_keep = nullptr, *t_kex = nullptr, *blk_sum = nullptr, *t_fin = nullptr;
   void *s_loc = nullptr, *s_var = nullptr, *s_v0max = nullptr;  // gate index (ckf_sort_slices)
   int32_t* s_idx = nullptr;
   int32_t* globals = nullptr;  // GlobalId
@@ -55,6 +56,8 @@ struct Workspace {
   cudaEvent_t done = nullptr;
   void* stream_tag = nullptr;
   bool used = false;
+  float last_ms[10] = {0};  // per-kernel-kind times of the last timed ckf_find (ckf_set_timing)
+  int last_launches = 0;
 };
 
 }  // namespace
@@ -74,6 +77,8 @@ struct ckf_handle {
   std::mutex mu;
   std::string err;
   std::vector<void*> allocs;
+  bool timing_print = false;
+  bool timing = false;  // ckf_set_timing / CKF_TIMING=1: per-kernel CUDA-event times of every ckf_find on stderr (debug aid; synchronises)
 };
 
 namespace {
@@ -134,7 +139,7 @@ void fill_params(ckf_handle* h, Workspace& w, KParams<T>& p) {
   p.mv_stop = w.mv_stop;
   p.pd_x = w.pd_x; p.pd_C = (T*)w.pd_C; p.sel_chi2 = (T*)w.sel_chi2; p.sel_idx = w.sel_idx;
   p.t_nsel = w.t_nsel; p.t_want = w.t_want; p.t_counts = w.t_counts; p.t_keep = w.t_keep; p.t_kex = w.t_kex;
-  p.blk_sum = w.blk_sum;
+  p.blk_sum = w.blk_sum; p.t_fin = w.t_fin;
   p.s_loc = (typename Vec2<T>::type*)w.s_loc; p.s_var = (typename Vec2<T>::type*)w.s_var; p.s_idx = w.s_idx;
   p.s_v0max = (T*)w.s_v0max;
   p.g = w.globals;
@@ -156,21 +161,51 @@ int launch_find(ckf_handle* h, Workspace& w, const ckf_measurements* m, const ck
   p.o_seed = o->seed_id; p.o_nholes = o->n_holes; p.o_lastmod = o->last_module; p.o_stop = o->stop_reason;
   p.o_params = (T*)o->params; p.o_cov = (T*)o->cov; p.o_chi2sum = (T*)o->chi2_sum; p.o_entrychi2 = (T*)o->entry_chi2;
   const int nb = (std::max(s->n, (int)CNT_N) + 255) / 256;
-  ckf_init_event<T><<<nb, 256, 0, st>>>(p);
-  ckf_sort_slices<T><<<h->sm_count * 8, SORT_NT, 0, st>>>(p);
+  // optional per-kernel timing (debug): an event after every launch
+  std::vector<cudaEvent_t> tev;
+  std::vector<int> tkind;
+  auto mark = [&](int kind) {
+    if (!h->timing) return;
+    cudaEvent_t e;
+    cudaEventCreate(&e);
+    cudaEventRecord(e, st);
+    tev.push_back(e);
+    tkind.push_back(kind);
+  };
+  mark(-1);
+  ckf_init_event<T><<<nb, 256, 0, st>>>(p); mark(0);
+  ckf_sort_slices<T><<<h->sm_count * 8, SORT_NT, 0, st>>>(p); mark(1);
   // level loop: tips of level l were made by level l - 1; a tip at max_levels only stops (LEVEL_LIMIT) and emits.
   // Kernels of an empty level return at once, so the loop needs no host read of the level's size.
-  const int scan_blocks = h->tcap / SCAN_NT + 1, wide = h->sm_count * 8;
+  const int wide = h->sm_count * 4;
   for (int level = 0; level <= h->cfg.max_levels; ++level) {
-    if (level > 0) ckf_step<T, MinBlocks<T>::value><<<h->step_grid, STEP_NT, 0, st>>>(p, level);
-    ckf_visit<T, VisitBlocks<T>::value><<<h->visit_grid, VISIT_NT, h->visit_smem, st>>>(p, level);
-    ckf_cap<T><<<wide, SCAN_NT, 0, st>>>(p, level);
-    ckf_scan<T><<<scan_blocks, SCAN_NT, 0, st>>>(p, level);
-    ckf_update<T><<<wide, SCAN_NT, 0, st>>>(p, level);
+    if (level > 0) { ckf_step<T, MinBlocks<T>::value><<<h->step_grid, STEP_NT, 0, st>>>(p, level); mark(2); }
+    ckf_visit<T, VisitBlocks<T>::value><<<h->visit_grid, VISIT_NT, h->visit_smem, st>>>(p, level); mark(3);
+    ckf_scan<T><<<wide, SCAN_NT, 0, st>>>(p, level); mark(5);
+    ckf_update<T><<<wide, SCAN_NT, 0, st>>>(p, level); mark(6);
   }
-  ckf_scan_seeds<T><<<1, 1024, 0, st>>>(p);
-  ckf_emit_tracks<T><<<h->sm_count * 4, 256, 0, st>>>(p);
-  ckf_finalize<T><<<1, 1, 0, st>>>(p);
+  ckf_scan_seeds<T><<<1, 1024, 0, st>>>(p); mark(7);
+  ckf_emit_tracks<T><<<h->sm_count * 4, 256, 0, st>>>(p); mark(8);
+  ckf_finalize<T><<<1, 1, 0, st>>>(p); mark(9);
+  w.last_launches = 5 + 4 * (h->cfg.max_levels + 1) - 1;
+  if (h->timing) {
+    static const char* names[10] = {"init", "sort", "step", "visit", "cap", "scan", "update", "scan_seeds", "emit", "finalize"};
+    cudaStreamSynchronize(st);
+    float acc[10] = {0}, tot = 0.f;
+    for (size_t i = 1; i < tev.size(); ++i) {
+      float ms = 0.f;
+      cudaEventElapsedTime(&ms, tev[i - 1], tev[i]);
+      acc[tkind[i]] += ms;
+      tot += ms;
+    }
+    for (int k = 0; k < 10; ++k) w.last_ms[k] = acc[k];
+    if (h->timing_print) {
+      fprintf(stderr, "[ckf timing] total %.3f ms:", tot);
+      for (int k = 0; k < 10; ++k) fprintf(stderr, " %s %.3f", names[k], acc[k]);
+      fprintf(stderr, "\n");
+    }
+    for (auto e : tev) cudaEventDestroy(e);
+  }
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(h, CKF_E_CUDA, "kernel launch failed: %s", cudaGetErrorString(e));
   return CKF_OK;
@@ -234,6 +269,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     return bail(CKF_E_CUDA);
   }
   h->sm_count = prop.multiProcessorCount;
+  { const char* t = getenv("CKF_TIMING"); h->timing = h->timing_print = t && t[0] == '1'; }
   h->n_modules = g->n_modules;
   h->n_layers = g->n_layers;
 
@@ -326,6 +362,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     CKB(dalloc(h, &w.t_nsel, TC * 4)); CKB(dalloc(h, &w.t_want, TC * 4)); CKB(dalloc(h, &w.t_counts, TC * 4));
     CKB(dalloc(h, &w.t_keep, TC * 4)); CKB(dalloc(h, &w.t_kex, TC * 4));
     CKB(dalloc(h, &w.blk_sum, (TC / SCAN_NT + 2) * 4));
+    CKB(dalloc(h, &w.t_fin, 4 * TC * 4));
     CKB(dalloc(h, (char**)&w.s_loc, 2 * (size_t)c->max_measurements * ts));
     CKB(dalloc(h, (char**)&w.s_var, 2 * (size_t)c->max_measurements * ts));
     CKB(dalloc(h, &w.s_idx, (size_t)c->max_measurements * 4));
@@ -428,6 +465,29 @@ int ckf_get_counters(ckf_handle* h, void* stream, ckf_counters* out) {
   out->rk_accepted = (int64_t)c[CNT_ACCEPTED]; out->gate_tests = (int64_t)c[CNT_GATE];
   out->updates = (int64_t)c[CNT_UPDATES]; out->links = (int64_t)c[CNT_LINKS]; out->iterations = (int64_t)c[CNT_ITER];
   out->gate_tests_executed = (int64_t)c[CNT_GATE_EXEC];
+  return CKF_OK;
+}
+
+int ckf_set_timing(ckf_handle* h, int on) {
+  if (!h) return CKF_E_ARG;
+  h->timing = on != 0 || h->timing_print;
+  return CKF_OK;
+}
+
+int ckf_get_timing(ckf_handle* h, void* stream, ckf_timing* out) {
+  if (!h || !out) return CKF_E_ARG;
+  cudaStream_t st = (cudaStream_t)stream;
+  Workspace* w = nullptr;
+  {
+    std::lock_guard<std::mutex> lk(h->mu);
+    for (auto& x : h->ws)
+      if (x.used && x.stream_tag == (void*)st) { w = &x; break; }
+  }
+  if (!w) return fail(h, CKF_E_ARG, "no ckf_find was issued on this stream");
+  out->init_ms = w->last_ms[0]; out->sort_ms = w->last_ms[1]; out->step_ms = w->last_ms[2]; out->visit_ms = w->last_ms[3];
+  out->scan_ms = w->last_ms[5]; out->update_ms = w->last_ms[6];
+  out->emit_ms = w->last_ms[7] + w->last_ms[8] + w->last_ms[9];
+  out->launches = w->last_launches;
   return CKF_OK;
 }
 

@@ -5,68 +5,87 @@
 
 namespace ckf {
 
-// a10 (R10) + a11: the thread of a seed's FIRST tip of the level walks the seed's tips in order, so the greedy
-// cap and the emission slots are the sequential rule itself and only one thread touches the seed's counters.
-// Seeds hold a few tips on average (at most max_candidates_per_seed), so the walk is short.
-template <typename T>
-__global__ void __launch_bounds__(SCAN_NT) ckf_cap(const KParams<T> p, int level) {
-  const int n = p.g[G_NTIPS0 + (level & 1)];
-  if (n == 0) return;
-  const size_t TC = (size_t)p.tcap;
-  const int32_t* tlink = p.tip_link + (size_t)(level & 1) * TC;
-  const int32_t* tseed = p.tip_seed + (size_t)(level & 1) * TC;
-  const int cap = p.cfg.max_cands;
-  for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < n; t += gridDim.x * blockDim.x) {
-    const int seed = tseed[t];
-    if (t > 0 && tseed[t - 1] == seed) continue;  // not the seed's first tip
-    const int extra0 = p.sd_extra[seed];
-    const int Rm = cap - (1 + extra0);
-    int P = 0, KM = 0, nemit = p.sd_nemit[seed], nent = p.sd_nentries[seed];
-    for (int j = t; j < n && tseed[j] == seed; ++j) {
-      const int want = p.t_want[j];
-      const int e = want > 0 ? want - 1 : 0;
-      int keep = 0;
-      if (want > 0) {
-        const int room = Rm - P;
-        keep = 1 + min(e, room > 0 ? room : 0);
-      }
-      P += e;
-      KM += keep > 1 ? keep - 1 : 0;
-      p.t_keep[j] = keep;
-      // emission record of a tip that stopped at this level, in tip order within the seed
-      const int stop = p.mv_stop[j], counts = p.t_counts[j], nm = counts & 0xffff;
-      if (stop != STOP_NONE && nm >= p.cfg.min_meas) {
-        if (nemit < cap) {
-          const size_t li = (size_t)seed * cap + nemit;
-          p.leaf_link[li] = tlink[j];
-          p.leaf_meta[li] = stop | ((counts >> 16) << 8);
-          p.leaf_entry[li] = nent;
-        }
-        nemit += 1;
-        nent += nm;
-      }
-    }
-    if (KM) p.sd_extra[seed] = extra0 + KM;
-    p.sd_nemit[seed] = nemit;
-    p.sd_nentries[seed] = nent;
-  }
-}
-
-// Exclusive scan of t_keep over the level's tips: per-tile prefix (t_kex) + per-tile sums; the last tile to
-// finish turns the sums into offsets, reserves the level's links (contiguous, so link ids are deterministic)
-// and publishes the next level's size.
+// a10 (R10) + a11 + child offsets, one kernel.
+//  1. Thread per tip: the tip looks BACK over the earlier tips of its seed at this level (a few on average, at
+//     most max_candidates_per_seed) and so evaluates the sequential rules in closed form, independently of
+//     every other thread: kept children (R10: exclusive prefix of the extra wants), emission slot and entry
+//     offset (exclusive prefix of the emitting tips).  The seed's LAST tip also sees the seed's totals; it
+//     parks them in t_fin* for ckf_update to apply to the per-seed counters (no thread reads a counter that
+//     another thread of this launch writes).
+//  2. Exclusive scan of the kept children: per-tile prefix (t_kex) + per-tile sums; the last block to finish
+//     turns the sums into offsets, reserves the level's links (contiguous, so link ids are deterministic) and
+//     publishes the next level's size.
 template <typename T>
 __global__ void __launch_bounds__(SCAN_NT) ckf_scan(const KParams<T> p, int level) {
   const int n = p.g[G_NTIPS0 + (level & 1)];
-  const int nb = n > 0 ? (n + SCAN_NT - 1) / SCAN_NT : 1;
-  if ((int)blockIdx.x >= nb) return;
+  if (n == 0) {
+    if (blockIdx.x == 0 && threadIdx.x == 0) p.g[G_NTIPS0 + ((level + 1) & 1)] = 0;  // the slot held level - 1
+    return;
+  }
+  const int nb = (n + SCAN_NT - 1) / SCAN_NT;
   __shared__ int s_w[SCAN_NT / 32];
   __shared__ int s_last;
+  const size_t TC = (size_t)p.tcap;
+  const int32_t* tlink = p.tip_link + (size_t)(level & 1) * TC;
+  const int32_t* tseed = p.tip_seed + (size_t)(level & 1) * TC;
+  const int cap = p.cfg.max_cands, min_meas = p.cfg.min_meas;
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5;
-  {
-    const int t = blockIdx.x * SCAN_NT + tid;
-    const int v = t < n ? p.t_keep[t] : 0;
-    const int inc = warp_incl_scan(v, lane);
+  for (int b = blockIdx.x; b < nb; b += gridDim.x) {
+    const int t = b * SCAN_NT + tid;
+    int keep = 0;
+    if (t < n) {
+      const int seed = tseed[t];
+      const int want = p.t_want[t];
+      const int e = want > 0 ? want - 1 : 0;
+      const int stop = p.mv_stop[t], counts = p.t_counts[t], nm = counts & 0xffff;
+      const bool emit = stop != STOP_NONE && nm >= min_meas;
+      // look back over the seed's earlier tips of this level
+      int P = 0, nemit_before = 0, nent_before = 0;
+      for (int j = t - 1; j >= 0 && tseed[j] == seed; --j) {
+        const int wj = p.t_want[j];
+        P += wj > 0 ? wj - 1 : 0;
+        const int cj = p.t_counts[j], nmj = cj & 0xffff;
+        if (p.mv_stop[j] != STOP_NONE && nmj >= min_meas) { nemit_before += 1; nent_before += nmj; }
+      }
+      const int extra0 = p.sd_extra[seed];
+      if (want > 0) {
+        const int room = cap - (1 + extra0) - P;
+        keep = 1 + min(e, room > 0 ? room : 0);
+      }
+      p.t_keep[t] = keep;
+      const int nemit0 = p.sd_nemit[seed], nent0 = p.sd_nentries[seed];
+      if (emit) {
+        const int slot = nemit0 + nemit_before;
+        if (slot < cap) {
+          const size_t li = (size_t)seed * cap + slot;
+          p.leaf_link[li] = tlink[t];
+          p.leaf_meta[li] = stop | ((counts >> 16) << 8);
+          p.leaf_entry[li] = nent0 + nent_before;
+        }
+      }
+      const bool tail = (t + 1 == n) || (tseed[t + 1] != seed);
+      if (tail) {
+        // totals of the seed at this level: kept extras need every tip's keep, recomputed from the prefixes
+        int KM = 0, Pj = 0;
+        const int Rm = cap - (1 + extra0);
+        int j0 = t;
+        while (j0 > 0 && tseed[j0 - 1] == seed) --j0;
+        for (int j = j0; j <= t; ++j) {
+          const int wj = p.t_want[j];
+          const int ej = wj > 0 ? wj - 1 : 0;
+          if (wj > 0) { const int room = Rm - Pj; KM += min(ej, room > 0 ? room : 0); }
+          Pj += ej;
+        }
+        p.t_fin[t] = seed;
+        p.t_fin[TC + t] = extra0 + KM;
+        p.t_fin[2 * TC + t] = nemit0 + nemit_before + (emit ? 1 : 0);
+        p.t_fin[3 * TC + t] = nent0 + nent_before + (emit ? nm : 0);
+      } else {
+        p.t_fin[t] = -1;
+      }
+    }
+    const int inc = warp_incl_scan(keep, lane);
+    __syncthreads();
     if (lane == 31) s_w[w] = inc;
     __syncthreads();
     int base = 0, tot = 0;
@@ -76,12 +95,14 @@ __global__ void __launch_bounds__(SCAN_NT) ckf_scan(const KParams<T> p, int leve
       if (i < w) base += x;
       tot += x;
     }
-    if (t < n) p.t_kex[t] = base + inc - v;
-    if (tid == 0) p.blk_sum[blockIdx.x] = tot;
+    if (t < n) p.t_kex[t] = base + inc - keep;
+    if (tid == 0) p.blk_sum[b] = tot;
   }
   __threadfence();
   __syncthreads();
-  if (tid == 0) s_last = (atomicAdd(p.g + G_SCAN_TICKET, 1) == nb - 1) ? 1 : 0;
+  const int nblocks = min((int)gridDim.x, nb);
+  if ((int)blockIdx.x >= nb) return;
+  if (tid == 0) s_last = (atomicAdd(p.g + G_SCAN_TICKET, 1) == nblocks - 1) ? 1 : 0;
   __syncthreads();
   if (!s_last) return;
   __threadfence();
@@ -123,14 +144,46 @@ __global__ void __launch_bounds__(SCAN_NT) ckf_scan(const KParams<T> p, int leve
   }
 }
 
+// Parent tip of child c: the last tip whose global exclusive prefix (tile offset + in-tile prefix) is <= c; tips
+// that keep nothing share their prefix with their successor, so "last" skips them.
+template <typename T>
+__device__ __forceinline__ int find_parent(const KParams<T>& p, int n, int nb, int c) {
+  int lo = 0, hi = nb;  // invariant: blk_sum[lo] <= c < blk_sum[hi]  (blk_sum[nb] = total)
+  while (hi - lo > 1) {
+    const int mid = (lo + hi) >> 1;
+    if (p.blk_sum[mid] <= c) lo = mid; else hi = mid;
+  }
+  const int boff = p.blk_sum[lo];
+  int a = lo * SCAN_NT, b = min(n, a + SCAN_NT);  // invariant: kex[a] <= c - boff < kex[b] (virtual kex[b] = inf)
+  while (b - a > 1) {
+    const int mid = (a + b) >> 1;
+    if (boff + p.t_kex[mid] <= c) a = mid; else b = mid;
+  }
+  return a;
+}
+
 // a9 + a10: thread per child, in child order (parent tip order, then (chi2, index) rank): Kalman update or hole
-// copy, link append, and the departure state (J1, V5) of the child as a tip of the next level.
+// copy, link append, and the departure state (J1, V5) of the child as a tip of the next level.  Also applies the
+// per-seed totals parked by ckf_scan.  The child -> parent search is staged: two threads bracket the block's
+// 256 children in the global prefix, the bracket is copied to shared memory, every thread searches there.
+constexpr int UPD_WIN = 1024;
 template <typename T>
 __global__ void __launch_bounds__(SCAN_NT) ckf_update(const KParams<T> p, int level) {
   const int n = p.g[G_NTIPS0 + (level & 1)];
+  if (n == 0) return;
   const int nc = p.g[G_NTIPS0 + ((level + 1) & 1)];
-  if (n == 0 || nc == 0) return;
   const size_t TC = (size_t)p.tcap;
+  for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < n; t += gridDim.x * blockDim.x) {
+    const int seed = p.t_fin[t];
+    if (seed >= 0) {
+      p.sd_extra[seed] = p.t_fin[TC + t];
+      p.sd_nemit[seed] = p.t_fin[2 * TC + t];
+      p.sd_nentries[seed] = p.t_fin[3 * TC + t];
+    }
+  }
+  if (nc == 0) return;
+  __shared__ int s_gk[UPD_WIN + 1];
+  __shared__ int s_p[2];
   const int32_t* tlink = p.tip_link + (size_t)(level & 1) * TC;
   const int32_t* tseed = p.tip_seed + (size_t)(level & 1) * TC;
   int32_t* nlink = p.tip_link + (size_t)((level + 1) & 1) * TC;
@@ -138,21 +191,30 @@ __global__ void __launch_bounds__(SCAN_NT) ckf_update(const KParams<T> p, int le
   const int nb = (n + SCAN_NT - 1) / SCAN_NT;
   const int lbase = p.g[G_LBASE];
   unsigned long long my_updates = 0;
-  for (int c = blockIdx.x * blockDim.x + threadIdx.x; c < nc; c += gridDim.x * blockDim.x) {
-    // parent = last tip whose exclusive prefix is <= c (tips that keep nothing share it with their successor)
-    int lo = 0, hi = nb;  // invariant: blk_sum[lo] <= c < blk_sum[hi]  (blk_sum[nb] = total)
-    while (hi - lo > 1) {
-      const int mid = (lo + hi) >> 1;
-      if (p.blk_sum[mid] <= c) lo = mid; else hi = mid;
+  for (int c0 = blockIdx.x * SCAN_NT; c0 < nc; c0 += gridDim.x * SCAN_NT) {
+    const int c = c0 + threadIdx.x;
+    __syncthreads();
+    if (threadIdx.x == 0) s_p[0] = find_parent<T>(p, n, nb, c0);
+    if (threadIdx.x == 32) s_p[1] = find_parent<T>(p, n, nb, min(c0 + SCAN_NT, nc) - 1);
+    __syncthreads();
+    const int p0 = s_p[0], win = s_p[1] - p0 + 1;
+    int par;
+    if (win <= UPD_WIN) {
+      for (int i = threadIdx.x; i < win; i += SCAN_NT) s_gk[i] = p.blk_sum[(p0 + i) / SCAN_NT] + p.t_kex[p0 + i];
+      __syncthreads();
+      int a = 0, b = win;  // invariant: gk[a] <= c < gk[b] (virtual gk[win] = inf)
+      if (c < nc) {
+        while (b - a > 1) {
+          const int mid = (a + b) >> 1;
+          if (s_gk[mid] <= c) a = mid; else b = mid;
+        }
+      }
+      par = p0 + a;
+    } else {
+      par = c < nc ? find_parent<T>(p, n, nb, c) : 0;
     }
-    const int boff = p.blk_sum[lo];
-    int a = lo * SCAN_NT, b = min(n, a + SCAN_NT);  // invariant: kex[a] <= c - boff < kex[b] (virtual kex[b] = inf)
-    while (b - a > 1) {
-      const int mid = (a + b) >> 1;
-      if (boff + p.t_kex[mid] <= c) a = mid; else b = mid;
-    }
-    const int par = a;
-    const int j = c - (boff + p.t_kex[par]);
+    if (c >= nc) continue;
+    const int j = c - (p.blk_sum[par / SCAN_NT] + p.t_kex[par]);
     const int nl = lbase + c;
     const int plink = tlink[par], seed = tseed[par];
     const int pc = p.t_counts[par];

@@ -1,13 +1,13 @@
 // ckf_kernels.cuh — shared declarations of the CKF kernels (a3-a11).
 //
 // Design: the level loop is LEVEL-SYNCHRONOUS over the whole event and PHASE-SEPARATED into
-// small kernels, five per level:
+// small kernels, four per level:
 //   ckf_step    persistent lanes pull tips of the level from a global cursor and run the navigation +
 //               adaptive RKN4 state machine (ckf_nav.cuh) until the tip stands on its next module
 //   ckf_visit   arrival Jacobian + covariance transport (lane per tip), then the chi2 gate over the loc0
 //               windows of the sorted slices (flattened (tip, measurement) pairs) and the k best
-//   ckf_cap     per-seed cap R10 and emission records (one thread walks a seed's tips in order)
-//   ckf_scan    exclusive scan of the kept children -> child offsets, link allocation, next level's size
+//   ckf_scan    per-seed cap R10 + emission records (every tip looks back over its seed's earlier tips), then
+//               the exclusive scan of the kept children -> child offsets, link allocation, next level's size
 //   ckf_update  thread per child: Kalman update or hole, link append, departure state of the next level
 // Why not one persistent kernel: measured on B200 (profiles/r01b), the monolithic level loop is ~100 KB of
 // SASS; with the warps of an SM in different phases the SM instruction cache misses 31 % of its requests and
@@ -23,7 +23,7 @@ namespace ckf {
 constexpr int CAND = 16;          // per-tip passer buffer of the gate fast path
 constexpr int STEP_NT = 128;      // threads per block of ckf_step
 constexpr int VISIT_NT = 128;     // threads per block of ckf_visit (4 warps, 32 tips each)
-constexpr int SCAN_NT = 256;      // threads per block of ckf_cap / ckf_scan / ckf_update; tile of the scan
+constexpr int SCAN_NT = 256;      // threads per block of ckf_scan / ckf_update; tile of the scan
 constexpr int SORT_NT = 128;      // threads per block of the slice sort
 constexpr int SORT_CAP = 2048;    // largest module slice sorted in shared memory; larger ones stay unsorted
 #ifndef CKF_SERVICE_MIN
@@ -101,7 +101,8 @@ struct KParams {
   int32_t* t_counts;   // [tcap] n_meas | n_holes << 16 of the tip (fatal hole included)
   int32_t* t_keep;     // [tcap] children kept after R10
   int32_t* t_kex;      // [tcap] exclusive prefix of t_keep inside the tip's scan tile
-  int32_t* blk_sum;    // [tcap / SCAN_NT + 1] kept children per scan tile, then exclusive offsets
+  int32_t* blk_sum;    // [tcap / SCAN_NT + 2] kept children per scan tile, then exclusive offsets
+  int32_t* t_fin;      // [4][tcap] per-seed totals parked by the seed's last tip: seed (-1 none), extra, nemit, nentries
   // globals
   int32_t* g;          // [G_N]
   unsigned long long* counters;
