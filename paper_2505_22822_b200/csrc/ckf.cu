@@ -35,6 +35,7 @@ struct Workspace {
   int32_t *lk_module = nullptr, *lk_parent = nullptr, *lk_meas = nullptr, *lk_counts = nullptr, *lk_lastmeas = nullptr;
   void *lk_chi2 = nullptr, *lk_chi2sum = nullptr;
   int32_t *sd = nullptr;       // 3 * max_seeds + 2 * (max_seeds + 1)
+  int32_t* seed_tile = nullptr;  // 2 * (tiles + 1)
   int32_t* leaf = nullptr;     // 3 * max_seeds * cap
   // level state (tips, move state, predictions, selections, scan)
   int32_t *tip_link = nullptr, *tip_seed = nullptr;
@@ -131,6 +132,7 @@ void fill_params(ckf_handle* h, Workspace& w, KParams<T>& p) {
   const size_t S = (size_t)c.max_seeds;
   p.sd_extra = w.sd; p.sd_nemit = w.sd + S; p.sd_nentries = w.sd + 2 * S;
   p.sd_track_base = w.sd + 3 * S; p.sd_entry_base = w.sd + 3 * S + (S + 1);
+  p.seed_tile = w.seed_tile; p.seed_tiles_cap = (int32_t)((S + SEED_TILE - 1) / SEED_TILE);
   const size_t LC = S * (size_t)c.max_candidates_per_seed;
   p.leaf_link = w.leaf; p.leaf_meta = w.leaf + LC; p.leaf_entry = w.leaf + 2 * LC;
   p.tcap = h->tcap;
@@ -184,7 +186,7 @@ int launch_find(ckf_handle* h, Workspace& w, const ckf_measurements* m, const ck
     ckf_scan<T><<<wide, SCAN_NT, 0, st>>>(p, level); mark(5);
     ckf_update<T><<<wide, SCAN_NT, 0, st>>>(p, level); mark(6);
   }
-  ckf_scan_seeds<T><<<1, 1024, 0, st>>>(p); mark(7);
+  ckf_scan_seeds<T><<<(s->n + SEED_TILE - 1) / SEED_TILE + 1, SEED_TILE, 0, st>>>(p); mark(7);
   ckf_emit_tracks<T><<<h->sm_count * 4, 256, 0, st>>>(p); mark(8);
   ckf_finalize<T><<<1, 1, 0, st>>>(p); mark(9);
   w.last_launches = 5 + 4 * (h->cfg.max_levels + 1) - 1;
@@ -335,6 +337,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     if (per_sm < 1 || vper_sm < 1) { fail(h, CKF_E_CUDA, "kernels do not fit on an SM (visit smem %d B)", h->visit_smem); return bail(CKF_E_CUDA); }
     h->step_regs = fa.numRegs;
     h->step_grid = per_sm * h->sm_count;
+    if (const char* d = getenv("CKF_STEP_GRID_DIV")) h->step_grid = std::max(1, h->step_grid / std::max(1, atoi(d)));  // experiment knob
     h->visit_grid = vper_sm * h->sm_count;
   }
   if (h->cfg.max_tips_per_level <= 0)
@@ -351,6 +354,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     CKB(dalloc(h, &w.lk_counts, L * 4)); CKB(dalloc(h, &w.lk_lastmeas, L * 4));
     CKB(dalloc(h, (char**)&w.lk_chi2, L * ts)); CKB(dalloc(h, (char**)&w.lk_chi2sum, L * ts));
     CKB(dalloc(h, &w.sd, (3 * S + 2 * (S + 1)) * 4));
+    CKB(dalloc(h, &w.seed_tile, 2 * ((S + SEED_TILE - 1) / SEED_TILE + 2) * 4));
     CKB(dalloc(h, &w.leaf, 3 * S * (size_t)c->max_candidates_per_seed * 4));
     const size_t TC = (size_t)h->tcap, KB = (size_t)c->max_branches_per_surface;
     CKB(dalloc(h, &w.tip_link, 2 * TC * 4)); CKB(dalloc(h, &w.tip_seed, 2 * TC * 4));

@@ -24,34 +24,58 @@ __global__ void ckf_init_event(const KParams<T> p) {
   if (i < CNT_N) p.counters[i] = 0ull;
 }
 
-// Exclusive scan over seeds of (emitted candidates, their entries) -> per-seed bases.  One block: the array is
-// tens of thousands of ints, a few microseconds.  Order by seed id is what makes the output deterministic.
+// Exclusive scan over seeds of (emitted candidates, their entries) -> per-seed bases.  Order by seed id is what
+// makes the output deterministic.  One block per tile of 1024 seeds writes the in-tile prefixes; the last block
+// to finish scans the tile totals (seed_tile[2][tiles + 1]).  Global base of seed s = tile offset + prefix.
+constexpr int SEED_TILE = 1024;
 template <typename T>
-__global__ void __launch_bounds__(1024) ckf_scan_seeds(const KParams<T> p) {
-  __shared__ int s_a[1024], s_b[1024];
-  const int tid = threadIdx.x, S = p.n_seeds;
-  const int per = (S + 1023) / 1024;
-  const int lo = min(S, tid * per), hi = min(S, lo + per);
-  int a = 0, b = 0;
-  for (int i = lo; i < hi; ++i) { a += p.sd_nemit[i]; b += p.sd_nentries[i]; }
-  s_a[tid] = a; s_b[tid] = b;
+__global__ void __launch_bounds__(SEED_TILE) ckf_scan_seeds(const KParams<T> p) {
+  __shared__ unsigned long long s_w[32];
+  __shared__ int s_last;
+  const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, S = p.n_seeds;
+  const int ntiles = S > 0 ? (S + SEED_TILE - 1) / SEED_TILE : 1;
+  if ((int)blockIdx.x >= ntiles) return;
+  int32_t* tile_trk = p.seed_tile;
+  int32_t* tile_ent = p.seed_tile + (p.seed_tiles_cap + 1);
+  {
+    const int i = blockIdx.x * SEED_TILE + tid;
+    unsigned long long v = 0ull;  // (tracks << 32) | entries: both stay below 2^31
+    if (i < S) v = ((unsigned long long)(unsigned)p.sd_nemit[i] << 32) | (unsigned long long)(unsigned)p.sd_nentries[i];
+    unsigned long long inc = v;
+#pragma unroll
+    for (int o = 1; o < 32; o <<= 1) {
+      const unsigned long long n = __shfl_up_sync(0xffffffffu, inc, o);
+      if (lane >= o) inc += n;
+    }
+    if (lane == 31) s_w[w] = inc;
+    __syncthreads();
+    unsigned long long base = 0ull, tot = 0ull;
+#pragma unroll
+    for (int k = 0; k < 32; ++k) {
+      const unsigned long long x = s_w[k];
+      if (k < w) base += x;
+      tot += x;
+    }
+    const unsigned long long ex = base + inc - v;
+    if (i < S) { p.sd_track_base[i] = (int)(ex >> 32); p.sd_entry_base[i] = (int)(ex & 0xffffffffull); }
+    if (tid == 0) { tile_trk[blockIdx.x] = (int)(tot >> 32); tile_ent[blockIdx.x] = (int)(tot & 0xffffffffull); }
+  }
+  __threadfence();
   __syncthreads();
-  // Hillis-Steele inclusive scan over the 1024 partials
-  for (int o = 1; o < 1024; o <<= 1) {
-    int va = 0, vb = 0;
-    if (tid >= o) { va = s_a[tid - o]; vb = s_b[tid - o]; }
-    __syncthreads();
-    s_a[tid] += va; s_b[tid] += vb;
-    __syncthreads();
-  }
-  int ra = s_a[tid] - a, rb = s_b[tid] - b;
-  for (int i = lo; i < hi; ++i) {
-    p.sd_track_base[i] = ra; p.sd_entry_base[i] = rb;
-    ra += p.sd_nemit[i]; rb += p.sd_nentries[i];
-  }
-  if (tid == 1023) {
-    p.sd_track_base[S] = s_a[1023]; p.sd_entry_base[S] = s_b[1023];
-    p.g[G_TOTAL_TRACKS] = s_a[1023]; p.g[G_TOTAL_ENTRIES] = s_b[1023];
+  if (tid == 0) s_last = (atomicAdd(p.g + G_SEED_TICKET, 1) == ntiles - 1) ? 1 : 0;
+  __syncthreads();
+  if (!s_last) return;
+  __threadfence();
+  if (tid == 0) {
+    int a = 0, b = 0;
+    for (int k = 0; k < ntiles; ++k) {
+      const int ta = ((volatile int32_t*)tile_trk)[k], tb = ((volatile int32_t*)tile_ent)[k];
+      tile_trk[k] = a; tile_ent[k] = b;
+      a += ta; b += tb;
+    }
+    tile_trk[ntiles] = a; tile_ent[ntiles] = b;
+    p.g[G_TOTAL_TRACKS] = a; p.g[G_TOTAL_ENTRIES] = b;
+    p.g[G_SEED_TICKET] = 0;
   }
 }
 
@@ -60,17 +84,26 @@ template <typename T>
 __global__ void __launch_bounds__(256) ckf_emit_tracks(const KParams<T> p) {
   const int total = p.g[G_TOTAL_TRACKS];
   const int cap = p.cfg.max_cands;
+  const int ntiles = p.n_seeds > 0 ? (p.n_seeds + SEED_TILE - 1) / SEED_TILE : 1;
+  const int32_t* tile_trk = p.seed_tile;
+  const int32_t* tile_ent = p.seed_tile + (p.seed_tiles_cap + 1);
   for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < total; t += gridDim.x * blockDim.x) {
-    // seed = last s with track_base[s] <= t
-    int lo = 0, hi = p.n_seeds;
+    // seed = last s with (tile offset + in-tile prefix) <= t: tile first, then inside the tile
+    int lo = 0, hi = ntiles;
     while (hi - lo > 1) {
       const int mid = (lo + hi) >> 1;
-      if (p.sd_track_base[mid] <= t) lo = mid; else hi = mid;
+      if (tile_trk[mid] <= t) lo = mid; else hi = mid;
     }
-    const int seed = lo, j = t - p.sd_track_base[seed];
+    const int toff = tile_trk[lo], eoff = tile_ent[lo];
+    int a = lo * SEED_TILE, b = min(p.n_seeds, a + SEED_TILE);
+    while (b - a > 1) {
+      const int mid = (a + b) >> 1;
+      if (toff + p.sd_track_base[mid] <= t) a = mid; else b = mid;
+    }
+    const int seed = a, j = t - (toff + p.sd_track_base[seed]);
     const size_t li = (size_t)seed * cap + j;
     const int leaf = p.leaf_link[li], meta = p.leaf_meta[li];
-    const int off = p.sd_entry_base[seed] + p.leaf_entry[li];
+    const int off = eoff + p.sd_entry_base[seed] + p.leaf_entry[li];
     const int nm = p.lk_counts[leaf] & 0xffff;
     if (t >= p.max_tracks || off + nm > p.max_entries) {
       atomicMin(p.g + G_FIRST_BAD, t);

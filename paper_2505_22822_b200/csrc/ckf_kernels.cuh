@@ -40,7 +40,7 @@ enum CounterId { CNT_TIPS = 0, CNT_VISITS, CNT_TRIALS, CNT_ACCEPTED, CNT_GATE, C
 
 // per-event device globals (int32 each)
 enum GlobalId { G_LINK_COUNT = 0, G_FIRST_BAD, G_TOTAL_TRACKS, G_TOTAL_ENTRIES, G_NTIPS0, G_NTIPS1, G_STEP_CURSOR,
-                G_SCAN_TICKET, G_LBASE, G_N };
+                G_SCAN_TICKET, G_LBASE, G_SEED_TICKET, G_N };
 
 template <typename T>
 struct KParams {
@@ -78,8 +78,10 @@ struct KParams {
   int32_t* leaf_link;    // [n_seeds * cap]
   int32_t* leaf_meta;    // stop reason | n_holes << 8
   int32_t* leaf_entry;   // entry offset inside the seed
-  int32_t* sd_track_base;  // [n_seeds + 1] (emission scan)
+  int32_t* sd_track_base;  // [n_seeds + 1] (emission scan) prefix inside the seed's tile of 1024
   int32_t* sd_entry_base;  // [n_seeds + 1]
+  int32_t* seed_tile;      // [2][seed_tiles_cap + 1] tile offsets (tracks, entries)
+  int32_t seed_tiles_cap;
   // ---- tips of a level, ordered by seed then lineage; arrays [..][tcap], tip index fastest
   int32_t tcap;
   int32_t* tip_link;   // [2][tcap] (ping-pong by level parity) link the tip stands on, -1 = fresh seed

@@ -11,8 +11,50 @@
 
 namespace ckf {
 
-// One block per module (grid-stride).  Slices longer than SORT_CAP, or holding a variance that is not a
-// positive finite number, are copied through unsorted and flagged (s_v0max < 0): their tips gate the whole slice.
+// Slices of at most 32 measurements (most modules) are rank-sorted by ONE warp with shuffles, four modules per
+// block at a time; longer slices by the whole block with a bitonic sort in shared memory.  Slices longer than
+// SORT_CAP, or holding a variance that is not a positive finite number, are copied through unsorted and flagged
+// (s_v0max < 0): their tips gate the whole slice.
+template <typename T>
+__device__ __forceinline__ void sort_slice_warp(const KParams<T>& p, int m, int beg, int n, int lane) {
+  if (n <= 0) {
+    if (lane == 0) p.s_v0max[m] = T(0);
+    return;
+  }
+  T key = (T)INFINITY, vmax = T(0);
+  int id = INT_MAX;
+  bool bad = false;
+  typename Vec2<T>::type lc, vr;
+  if (lane < n) {
+    id = beg + lane;
+    lc = p.loc[id];
+    vr = p.var[id];
+    key = lc.x;
+    if (!(key == key)) key = (T)INFINITY;  // NaN sorts last; it can never pass the gate
+    bad = !(vr.x > T(0)) || !(vr.y > T(0)) || !isfinite(vr.x) || !isfinite(vr.y);
+    vmax = vr.x;
+  }
+  const bool any_bad = __any_sync(0xffffffffu, bad);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const T ov = __shfl_xor_sync(0xffffffffu, vmax, o);
+    vmax = ov > vmax ? ov : vmax;
+  }
+  int rank = 0;
+  for (int j = 0; j < n; ++j) {
+    const T kj = __shfl_sync(0xffffffffu, key, j);
+    const int ij = __shfl_sync(0xffffffffu, id, j);
+    rank += key_less<T>(kj, ij, key, id) ? 1 : 0;
+  }
+  if (any_bad) rank = lane;
+  if (lane < n) {
+    p.s_loc[beg + rank] = lc;
+    p.s_var[beg + rank] = vr;
+    p.s_idx[beg + rank] = id;
+  }
+  if (lane == 0) p.s_v0max[m] = any_bad ? T(-1) : vmax;
+}
+
 template <typename T>
 __global__ void __launch_bounds__(SORT_NT) ckf_sort_slices(const KParams<T> p) {
   __shared__ T s_key[SORT_CAP];
@@ -20,84 +62,92 @@ __global__ void __launch_bounds__(SORT_NT) ckf_sort_slices(const KParams<T> p) {
   __shared__ T s_red[SORT_NT / 32];
   __shared__ int s_bad;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  for (int m = blockIdx.x; m < p.geo.n_modules; m += gridDim.x) {
-    const int beg = __ldg(p.moff + m), end = __ldg(p.moff + m + 1), n = end - beg;
-    if (n <= 0) {
-      if (tid == 0) p.s_v0max[m] = T(0);
-      continue;
+  constexpr int MPB = SORT_NT / 32;  // small modules taken per block and round, one per warp
+  for (int m0 = blockIdx.x * MPB; m0 < p.geo.n_modules; m0 += gridDim.x * MPB) {
+    const int mw = m0 + warp;
+    if (mw < p.geo.n_modules) {
+      const int begw = __ldg(p.moff + mw), nw = __ldg(p.moff + mw + 1) - begw;
+      if (nw <= 32) sort_slice_warp<T>(p, mw, begw, nw, lane);
     }
-    if (tid == 0) s_bad = 0;
-    __syncthreads();
-    // largest var0 and validity of the slice's variances
-    T vmax = T(0);
-    bool bad = false;
-    for (int i = tid; i < n; i += SORT_NT) {
-      const auto vr = p.var[beg + i];
-      bad = bad || !(vr.x > T(0)) || !(vr.y > T(0)) || !isfinite(vr.x) || !isfinite(vr.y);
-      vmax = vr.x > vmax ? vr.x : vmax;
-    }
-#pragma unroll
-    for (int o = 16; o > 0; o >>= 1) {
-      const T ov = __shfl_xor_sync(0xffffffffu, vmax, o);
-      vmax = ov > vmax ? ov : vmax;
-    }
-    if (lane == 0) s_red[warp] = vmax;
-    if (bad) s_bad = 1;
-    __syncthreads();
-    const bool unsorted = (s_bad != 0) || n > SORT_CAP;
-    if (unsorted) {
-      for (int i = tid; i < n; i += SORT_NT) {
-        p.s_loc[beg + i] = p.loc[beg + i];
-        p.s_var[beg + i] = p.var[beg + i];
-        p.s_idx[beg + i] = beg + i;
-      }
-      if (tid == 0) p.s_v0max[m] = T(-1);
+  }
+  // long slices: one block per module, consecutive modules on different blocks (the crowded inner-layer
+  // modules have consecutive ids)
+  {
+    for (int m = blockIdx.x; m < p.geo.n_modules; m += gridDim.x) {
+      const int beg = __ldg(p.moff + m), end = __ldg(p.moff + m + 1), n = end - beg;
+      if (n <= 32) continue;
       __syncthreads();
-      continue;
-    }
-    int P = 1;
-    while (P < n) P <<= 1;
-    for (int i = tid; i < P; i += SORT_NT) {
-      T key = (T)INFINITY;
-      int id = INT_MAX;
-      if (i < n) {
-        key = p.loc[beg + i].x;
-        if (!(key == key)) key = (T)INFINITY;  // NaN sorts last; it can never pass the gate
-        id = beg + i;
+      if (tid == 0) s_bad = 0;
+      __syncthreads();
+      // largest var0 and validity of the slice's variances
+      T vmax = T(0);
+      bool bad = false;
+      for (int i = tid; i < n; i += SORT_NT) {
+        const auto vr = p.var[beg + i];
+        bad = bad || !(vr.x > T(0)) || !(vr.y > T(0)) || !isfinite(vr.x) || !isfinite(vr.y);
+        vmax = vr.x > vmax ? vr.x : vmax;
       }
-      s_key[i] = key;
-      s_id[i] = id;
-    }
-    __syncthreads();
-    // bitonic sort, ascending by (loc0, index)
-    for (int k = 2; k <= P; k <<= 1) {
-      for (int j = k >> 1; j > 0; j >>= 1) {
-        for (int i = tid; i < P; i += SORT_NT) {
-          const int ixj = i ^ j;
-          if (ixj > i) {
-            const T ka = s_key[i], kb = s_key[ixj];
-            const int ia = s_id[i], ib = s_id[ixj];
-            const bool up = (i & k) == 0;
-            const bool a_gt_b = key_less<T>(kb, ib, ka, ia);
-            if (a_gt_b == up) { s_key[i] = kb; s_key[ixj] = ka; s_id[i] = ib; s_id[ixj] = ia; }
-          }
-        }
-        __syncthreads();
-      }
-    }
-    for (int i = tid; i < n; i += SORT_NT) {
-      const int id = s_id[i];
-      p.s_loc[beg + i] = p.loc[id];
-      p.s_var[beg + i] = p.var[id];
-      p.s_idx[beg + i] = id;
-    }
-    if (tid == 0) {
-      T v = s_red[0];
 #pragma unroll
-      for (int w = 1; w < SORT_NT / 32; ++w) v = s_red[w] > v ? s_red[w] : v;
-      p.s_v0max[m] = v;
+      for (int o = 16; o > 0; o >>= 1) {
+        const T ov = __shfl_xor_sync(0xffffffffu, vmax, o);
+        vmax = ov > vmax ? ov : vmax;
+      }
+      if (lane == 0) s_red[warp] = vmax;
+      if (bad) s_bad = 1;
+      __syncthreads();
+      const bool unsorted = (s_bad != 0) || n > SORT_CAP;
+      if (unsorted) {
+        for (int i = tid; i < n; i += SORT_NT) {
+          p.s_loc[beg + i] = p.loc[beg + i];
+          p.s_var[beg + i] = p.var[beg + i];
+          p.s_idx[beg + i] = beg + i;
+        }
+        if (tid == 0) p.s_v0max[m] = T(-1);
+        continue;
+      }
+      int P = 64;
+      while (P < n) P <<= 1;
+      for (int i = tid; i < P; i += SORT_NT) {
+        T key = (T)INFINITY;
+        int id = INT_MAX;
+        if (i < n) {
+          key = p.loc[beg + i].x;
+          if (!(key == key)) key = (T)INFINITY;  // NaN sorts last; it can never pass the gate
+          id = beg + i;
+        }
+        s_key[i] = key;
+        s_id[i] = id;
+      }
+      __syncthreads();
+      // bitonic sort, ascending by (loc0, index)
+      for (int kk = 2; kk <= P; kk <<= 1) {
+        for (int j = kk >> 1; j > 0; j >>= 1) {
+          for (int i = tid; i < P; i += SORT_NT) {
+            const int ixj = i ^ j;
+            if (ixj > i) {
+              const T ka = s_key[i], kb = s_key[ixj];
+              const int ia = s_id[i], ib = s_id[ixj];
+              const bool up = (i & kk) == 0;
+              const bool a_gt_b = key_less<T>(kb, ib, ka, ia);
+              if (a_gt_b == up) { s_key[i] = kb; s_key[ixj] = ka; s_id[i] = ib; s_id[ixj] = ia; }
+            }
+          }
+          __syncthreads();
+        }
+      }
+      for (int i = tid; i < n; i += SORT_NT) {
+        const int id = s_id[i];
+        p.s_loc[beg + i] = p.loc[id];
+        p.s_var[beg + i] = p.var[id];
+        p.s_idx[beg + i] = id;
+      }
+      if (tid == 0) {
+        T v = s_red[0];
+#pragma unroll
+        for (int w = 1; w < SORT_NT / 32; ++w) v = s_red[w] > v ? s_red[w] : v;
+        p.s_v0max[m] = v;
+      }
     }
-    __syncthreads();
   }
 }
 
