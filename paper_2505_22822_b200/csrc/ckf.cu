@@ -362,7 +362,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     CKB(dalloc(h, (char**)&w.mv_D, 25 * TC * ts)); CKB(dalloc(h, (char**)&w.mv_dep, 5 * TC * ts));
     CKB(dalloc(h, (char**)&w.pd_C, 21 * TC * ts)); CKB(dalloc(h, (char**)&w.sel_chi2, KB * TC * ts));
     CKB(dalloc(h, &w.sel_idx, KB * TC * 4));
-    CKB(dalloc(h, &w.mv_from, TC * 4)); CKB(dalloc(h, &w.mv_tgt, TC * 4)); CKB(dalloc(h, &w.mv_stop, TC * 4));
+    CKB(dalloc(h, &w.mv_from, TC * 4)); CKB(dalloc(h, &w.mv_tgt, 2 * TC * 4)); CKB(dalloc(h, &w.mv_stop, TC * 4));
     CKB(dalloc(h, &w.t_nsel, TC * 4)); CKB(dalloc(h, &w.t_want, TC * 4)); CKB(dalloc(h, &w.t_counts, TC * 4));
     CKB(dalloc(h, &w.t_keep, TC * 4)); CKB(dalloc(h, &w.t_kex, TC * 4));
     CKB(dalloc(h, &w.blk_sum, (TC / SCAN_NT + 2) * 4));

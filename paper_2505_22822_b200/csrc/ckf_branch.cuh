@@ -273,6 +273,8 @@ __global__ void __launch_bounds__(SCAN_NT) ckf_update(const KParams<T> p, int le
         p.mv_y[7 * TC + c] = y.qop;
 #pragma unroll
         for (int i = 0; i < 5; ++i) p.mv_dep[i * TC + c] = dep[i];
+        // N2 here, at full lanes, instead of inside the RKN4 kernel: the overlap neighbour of the child's departure
+        p.mv_tgt[TC + c] = overlap_neighbour(p.geo, target, y.r, y.d);
       }
     }
     p.mv_stop[c] = stop;

@@ -26,10 +26,14 @@ constexpr int VISIT_NT = 128;     // threads per block of ckf_visit (4 warps, 32
 constexpr int SCAN_NT = 256;      // threads per block of ckf_scan / ckf_update; tile of the scan
 constexpr int SORT_NT = 128;      // threads per block of the slice sort
 constexpr int SORT_CAP = 2048;    // largest module slice sorted in shared memory; larger ones stay unsorted
-#ifndef CKF_SERVICE_MIN
-#define CKF_SERVICE_MIN 16
+#ifndef CKF_FETCH_MIN
+#define CKF_FETCH_MIN 4
 #endif
-constexpr int SERVICE_MIN = CKF_SERVICE_MIN;  // lanes that must wait before a ckf_step service point runs early
+#ifndef CKF_PICK_MIN
+#define CKF_PICK_MIN 8
+#endif
+constexpr int FETCH_MIN = CKF_FETCH_MIN;  // finished / tip-less lanes that must wait before write-back + fetch run early
+constexpr int PICK_MIN = CKF_PICK_MIN;    // lanes on a portal that must wait before the module choice runs early
 
 template <typename T> struct Vec2;
 template <> struct Vec2<float> { using type = float2; };
@@ -91,7 +95,7 @@ struct KParams {
   T* mv_D;             // [25][tcap] transport Jacobian (ckf_step -> ckf_visit)
   T* mv_dep;           // [5][tcap] direction on departure, Highland q_phi, q_theta
   int32_t* mv_from;    // [tcap] module the tip stands on
-  int32_t* mv_tgt;     // [tcap] module reached
+  int32_t* mv_tgt;     // [2][tcap] module reached; overlap neighbour at departure (N2, by ckf_update), -1 none
   int32_t* mv_stop;    // [tcap] stop reason so far
   // prediction + selection (ckf_visit -> ckf_cap, ckf_update)
   double* pd_x;        // [6][tcap]

@@ -103,16 +103,20 @@ CKF_HD void field_at(const FieldDev& f, const double r[3], double B[3]) {
     const double g = (r[a] - f.org[a]) * f.inv[a];
     // i = clamp(floor(g), 0, n - 2) and fr = g - i with float64 adds only (no float<->int conversion
     // instructions): adding 1.5 * 2^52 rounds g to the nearest integer and leaves that integer in the low
-    // mantissa bits.  NaN and out-of-range g fall to the clamps (fmax/fmin return the non-NaN operand).
+    // mantissa bits.  Out-of-range g falls to the clamps.
     const double MAGIC = 6755399441055744.0;
     double ti = (g + MAGIC) - MAGIC;
     if (ti > g) ti -= 1.0;
-    ti = fmin(fmax(ti, 0.0), f.nm2[a]);
+    ti = ti < 0.0 ? 0.0 : ti;
+    ti = ti > f.nm2[a] ? f.nm2[a] : ti;
 #if defined(__CUDA_ARCH__)
-    idx[a] = __double2loint(ti + MAGIC);
+    int i = __double2loint(ti + MAGIC);
 #else
-    idx[a] = (int)ti;
+    int i = (ti == ti) ? (int)ti : 0;
 #endif
+    i = i < 0 ? 0 : i;                      // only a NaN position gets here out of range: keep the loads in bounds,
+    i = i > f.n[a] - 2 ? f.n[a] - 2 : i;    // fr is NaN and the trial ends as STOP_NUMERIC
+    idx[a] = i;
     fr[a] = g - ti;
   }
   const long long s1 = f.n[2], s0 = (long long)f.n[1] * f.n[2];

@@ -301,6 +301,13 @@ struct PickRequest {
   int layer, iphi, iz, exclude;
   double s_min;
 };
+// N2 for a tip leaving module `from` at (r, d): nearest in-bounds overlap neighbour on the same layer, or -1.
+CKF_HD int overlap_neighbour(const GeoDev& g, int from, const double r[3], const double d[3]) {
+  const ModuleRec& k = g.mod[from];
+  const int iz = from - g.layer[k.layer].offset - k.iphi * g.layer[k.layer].n_z;
+  return pick_in_neighbourhood(g, k.layer, k.iphi, iz, from, r, d, 1e-3);
+}
+
 template <typename T>
 CKF_HD bool move_pick_request(const Move<T>& m, const GeoDev& g, PickRequest& q) {
   if (m.phase == PH_START) {

@@ -4,7 +4,7 @@
 // from a global cursor when its move is done, so lanes do not idle while a neighbour needs more RKN4 trials
 // (the imbalance the paper names).  The code that is not the trial — write-back + fetch,
 // module choice — runs at SERVICE points: lanes that finished, lanes without a tip and lanes that need a
-// module choice wait until SERVICE_MIN of them have gathered (or no lane can step), then are served together.
+// module choice wait until FETCH_MIN / PICK_MIN of them have gathered (or no lane can step), then are served together.
 // The module choice spreads its nine straight-line tests per tip over all 32 lanes.
 #pragma once
 #include "ckf_kernels.cuh"
@@ -113,8 +113,8 @@ __global__ void __launch_bounds__(STEP_NT, MINB) ckf_step(const KParams<T> p, in
     const unsigned bS = __ballot_sync(0xffffffffu, m.phase == PH_CYL || m.phase == PH_PLANE);
     const unsigned bF = __ballot_sync(0xffffffffu, m.phase == PH_FIN);
     if (!bP && !bS && !bF && !more) break;
-    const int waiting = __popc(bF) + __popc(bP) + (more ? __popc(bI) : 0);
-    if (bS == 0u || waiting >= SERVICE_MIN) {
+    const int waiting = __popc(bF) + (more ? __popc(bI) : 0);
+    if (bS == 0u || waiting >= FETCH_MIN || __popc(bP) >= PICK_MIN) {
       // ---- write-back of finished moves
       if (m.phase == PH_FIN) {
         if (m.stop == STOP_NONE) {
@@ -152,10 +152,15 @@ __global__ void __launch_bounds__(STEP_NT, MINB) ckf_step(const KParams<T> p, in
           m.y.t = p.mv_y[6 * TC + t];
           m.y.qop = p.mv_y[7 * TC + t];
           move_begin<T>(m, p.cfg, p.mv_from[t]);
+          move_pick_apply<T>(m, p.geo, p.mv_tgt[TC + t]);  // N2 was decided by ckf_update
         }
       }
-      // ---- module choice for every lane that needs one
-      if (__ballot_sync(0xffffffffu, m.phase == PH_START || m.phase == PH_LANDED)) pick_warp<T>(p.geo, ps, m, lane);
+      // ---- module choice at the portal (N3, N4) once enough lanes need one
+      {
+        const unsigned need = __ballot_sync(0xffffffffu, m.phase == PH_START || m.phase == PH_LANDED);
+        const unsigned step = __ballot_sync(0xffffffffu, m.phase == PH_CYL || m.phase == PH_PLANE);
+        if (need && (step == 0u || __popc(need) >= PICK_MIN)) pick_warp<T>(p.geo, ps, m, lane);
+      }
     }
     // ---- one step: targeting + landing, else one RKN4 trial
     if (m.phase == PH_CYL || m.phase == PH_PLANE) move_step<T>(m, p.fld, p.cfg, nt, na);

@@ -139,3 +139,102 @@ def test_host_buffer_path_equals_device_path():
     assert res.n_tracks == gpu.n_tracks
     assert np.array_equal(res.meas_idx, gpu.meas_idx)
     assert np.array_equal(res.params, gpu.params)
+
+
+def _inject(ev, module, loc, var):
+    """Copy of `ev` with extra measurements appended to `module`'s CSR slice (indices after it shift)."""
+    import copy
+    ev2 = copy.copy(ev)
+    off = ev.module_offsets.astype(np.int64)
+    at = int(off[module + 1])
+    k = loc.shape[0]
+    ev2.loc = np.concatenate([ev.loc[:at], loc.astype(ev.loc.dtype), ev.loc[at:]])
+    ev2.var = np.concatenate([ev.var[:at], var.astype(ev.var.dtype), ev.var[at:]])
+    ev2.meas_particle = np.concatenate([ev.meas_particle[:at], -np.ones(k, np.int32), ev.meas_particle[at:]])
+    ev2.meas_module = np.concatenate([ev.meas_module[:at], np.full(k, module, np.int32), ev.meas_module[at:]])
+    off2 = off.copy()
+    off2[module + 1:] += k
+    ev2.module_offsets = off2.astype(np.int32)
+    return ev2
+
+
+@pytest.mark.parametrize("config", [1, 2])
+def test_gate_paths_long_slices_many_passers_bad_variances(config):
+    """The gate index (slices sorted by loc0, window search) must not change any result: (a) a slice longer than
+    the in-shared-memory sort (left unsorted, gated in full), (b) more passers than the per-tip buffer (exact
+    k-round selection), (c) a slice with a non-positive variance (left unsorted), (d) exact chi2 ties (rank by
+    index) — each against the oracle, which always gates the whole slice."""
+    det, fld, cfg = synth.config_bundle(config)
+    ev = synth.make_event(config, det=det, n_particles=120)
+    rng = np.random.default_rng(7)
+    # seed 0's own module: 40 near-copies of its truth hit (> 16 passers, with exact duplicates = chi2 ties)
+    m0 = int(ev.seed_module[0])
+    sl = slice(int(ev.module_offsets[m0]), int(ev.module_offsets[m0 + 1]))
+    truth = np.nonzero(ev.meas_particle[sl] == ev.seed_particle[0])[0]
+    base = ev.loc[sl][truth[0]].astype(np.float64)
+    dup = base + rng.normal(0.0, 0.003, size=(40, 2))
+    dup[10:20] = dup[0:10]
+    ev = _inject(ev, m0, dup, np.tile(ev.var[sl][truth[0]], (40, 1)))
+    # seed 1's module: 2500 uniform hits (> SORT_CAP = 2048 -> unsorted slice)
+    m1 = int(ev.seed_module[1])
+    if m1 == m0:
+        m1 = int(ev.seed_module[2])
+    hu, hv = float(det.half_u[m1]), float(det.half_v[m1])
+    big = np.stack([rng.uniform(-hu, hu, 2500), rng.uniform(-hv, hv, 2500)], axis=1)
+    v1 = ev.var[int(ev.module_offsets[m1])]
+    ev = _inject(ev, m1, big, np.tile(v1, (2500, 1)))
+    # another seed's module: one measurement with a zero variance and one with a negative one
+    m2 = int(ev.seed_module[5])
+    assert m2 not in (m0, m1)
+    v2 = ev.var[int(ev.module_offsets[m2])].astype(np.float64)
+    ev = _inject(ev, m2, np.array([[0.0, 0.0], [1.0, 1.0]]), np.array([[0.0, v2[1]], [-v2[0], v2[1]]]))
+    ora = _run_oracle(det, fld, cfg, ev)
+    ckf, dev, out, gpu, cnt = _run_gpu(det, fld, cfg, ev)
+    assert gpu.status == 0
+    if cfg.precision == 64:
+        parity.assert_bit_exact_lists(gpu, ora)
+        rel, chi2, _ = parity.max_param_diffs(gpu, ora)
+        assert rel < 1e-9 and chi2 < 1e-8, (rel, chi2)
+    else:
+        r = parity.compare_fp32(gpu, ora, ev.n_seeds)
+        assert r["frac_identical"] >= 0.999 and r["max_param_rel"] < 1e-4 and r["max_chi2_sum_abs"] < 1e-3, r
+    assert cnt["gate_tests"] == ora.counters["gate_tests"]
+    assert cnt["gate_tests_executed"] <= cnt["gate_tests"]
+    ckf.close()
+
+
+def test_tip_capacity_overflow_is_flagged():
+    import torch
+    from paper_2505_22822_b200 import CKF
+    det, fld, cfg = synth.config_bundle(1)
+    ev = synth.make_event(1, det=det, n_particles=200)
+    rng = np.random.default_rng(3)
+    for sd in range(40):                         # 4 near-copies of the seed's own hit: 5 branches at level 0
+        m = int(ev.seed_module[sd])
+        sl = slice(int(ev.module_offsets[m]), int(ev.module_offsets[m + 1]))
+        own = np.nonzero(ev.meas_particle[sl] == ev.seed_particle[sd])[0]
+        if own.size == 0:
+            continue
+        hit = ev.loc[sl][own[0]].astype(np.float64)
+        ev = _inject(ev, m, hit + rng.normal(0.0, 0.002, size=(4, 2)), np.tile(ev.var[sl][own[0]], (4, 1)))
+    ckf = CKF(det, fld, cfg.ckf, 64, max_seeds=ev.n_seeds, max_measurements=ev.n_measurements,
+              max_tips_per_level=ev.n_seeds)     # no room for any branching
+    dev, out = ckf.upload_event(ev), ckf.alloc_tracks()
+    ckf.find(dev, out)
+    torch.cuda.synchronize()
+    assert int(out["status"][0]) & 4
+    ckf.close()
+
+
+def test_timing_abi_reports_every_phase():
+    import torch
+    det, fld, cfg = synth.config_bundle(2)
+    ev = synth.make_event(2, det=det, n_particles=500)
+    ckf, dev, out, gpu, _ = _run_gpu(det, fld, cfg, ev)
+    ckf.set_timing(True)
+    ckf.find(dev, out)
+    torch.cuda.synchronize()
+    t = ckf.timing()
+    ckf.set_timing(False)
+    assert t["launches"] > 0 and t["step_ms"] > 0 and t["visit_ms"] > 0 and t["update_ms"] > 0 and t["scan_ms"] > 0
+    ckf.close()
