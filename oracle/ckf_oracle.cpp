@@ -534,7 +534,15 @@ int move_to_next_module(const OGeometry& g, const OField& fld, const OConfig& cf
       cyl.R = g.layer_r[lp];
       int st = propagate_to(fld, cfg, cyl, y, cnt);
       if (st != STOP_NONE) return st;
-      if (std::fabs(y.r[2]) > g.layer_half_z[lp]) { ++lp; continue; }
+      if (std::fabs(y.r[2]) > g.layer_half_z[lp]) {
+        // N3 (reading D11): beyond the half-length of this layer AND of every further layer while moving
+        // away in z, the tip has left the barrel: EXIT now instead of walking the remaining portal cylinders.
+        bool gone = y.r[2] * y.d[2] > 0.0;
+        for (int l2 = lp + 1; gone && l2 < g.n_layers; ++l2) gone = std::fabs(y.r[2]) > g.layer_half_z[l2];
+        if (gone) return STOP_EXIT;
+        ++lp;
+        continue;
+      }
       const int nphi = g.n_phi[lp], nz = g.n_z[lp];
       const double len = 2.0 * g.half_v[g.module_offset[lp]];
       const double phix = std::atan2(y.r[1], y.r[0]);

@@ -235,7 +235,8 @@ CKF_HD void kalman_update(const double x[6], const T C[21], T m0, T m1, T v0, T 
 //
 //   START --pick--> PLANE | CYL | FIN(EXIT)         N2 overlap neighbour, else next layer's cylinder
 //   CYL   --step--> CYL (one RKN4 trial) | LANDED    P3-P5 toward the portal cylinder of layer lp
-//   LANDED--pick--> PLANE | CYL | FIN(EXIT)         N3/N4 module choice at the portal; a crack is not a hole
+//   LANDED--pick--> PLANE | CYL | FIN(EXIT)         N3/N4 module choice at the portal; a crack is not a hole;
+//                                                   beyond every further layer's half length = EXIT (D11)
 //   PLANE --step--> PLANE (one trial) | FIN          N5 toward the target module's plane
 //   FIN   --arrive-> predicted bound parameters + 5x5 Jacobian block (J4, J5)
 enum MovePhase : int { PH_IDLE = 0, PH_START = 1, PH_CYL = 2, PH_LANDED = 3, PH_PLANE = 4, PH_FIN = 5 };
@@ -308,29 +309,38 @@ CKF_HD int overlap_neighbour(const GeoDev& g, int from, const double r[3], const
   return pick_in_neighbourhood(g, k.layer, k.iphi, iz, from, r, d, 1e-3);
 }
 
+// What a move in PH_START / PH_LANDED needs next: PICK_TEST (test the 3x3 neighbourhood in q), PICK_SKIP (portal
+// point beyond the layer's half length: go on to the next layer), PICK_EXIT (beyond the half length of this and
+// every further layer and moving away in z: the tip has left the barrel, reading D11).
+enum PickWhat : int { PICK_TEST = 1, PICK_SKIP = 0, PICK_EXIT = -1 };
 template <typename T>
-CKF_HD bool move_pick_request(const Move<T>& m, const GeoDev& g, PickRequest& q) {
+CKF_HD int move_pick_request(const Move<T>& m, const GeoDev& g, PickRequest& q) {
   if (m.phase == PH_START) {
     const ModuleRec& k = g.mod[m.from];
     q.layer = k.layer; q.iphi = k.iphi;
     q.iz = m.from - g.layer[k.layer].offset - k.iphi * g.layer[k.layer].n_z;
     q.exclude = m.from; q.s_min = 1e-3;
-    return true;
+    return PICK_TEST;
   }
   const LayerRec L = g.layer[m.lp];
   q.layer = m.lp; q.exclude = -1; q.s_min = -1e-3; q.iphi = 0; q.iz = 0;
-  if (fabs(m.y.r[2]) > L.half_z) return false;
+  if (fabs(m.y.r[2]) > L.half_z) {
+    bool gone = m.y.r[2] * m.y.d[2] > 0.0;
+    for (int l2 = m.lp + 1; gone && l2 < g.n_layers; ++l2) gone = fabs(m.y.r[2]) > g.layer[l2].half_z;
+    return gone ? PICK_EXIT : PICK_SKIP;
+  }
   const double phix = atan2(m.y.r[1], m.y.r[0]);
   const int i = (int)nearbyint(phix * L.n_phi / (2.0 * PI_D));
   q.iphi = ((i % L.n_phi) + L.n_phi) % L.n_phi;
   const int j = (int)floor((m.y.r[2] + L.half_z) / L.len_z);
   q.iz = j < 0 ? 0 : (j > L.n_z - 1 ? L.n_z - 1 : j);
-  return true;
+  return PICK_TEST;
 }
 
 // Result of the pick (module id or -1) -> next phase.
 template <typename T>
-CKF_HD void move_pick_apply(Move<T>& m, const GeoDev& g, int tgt) {
+CKF_HD void move_pick_apply(Move<T>& m, const GeoDev& g, int tgt, bool exit_now = false) {
+  if (exit_now) { m.stop = STOP_EXIT; m.phase = PH_FIN; return; }
   if (tgt >= 0) {
     const ModuleRec& k = g.mod[tgt];
 #pragma unroll
@@ -430,9 +440,9 @@ CKF_HD int move_to_next_module(const GeoDev& g, const FieldDev& fld, const CfgDe
   while (m.phase != PH_FIN) {
     if (m.phase == PH_START || m.phase == PH_LANDED) {
       PickRequest q;
-      const bool ok = move_pick_request(m, g, q);
-      const int tgt = ok ? pick_in_neighbourhood(g, q.layer, q.iphi, q.iz, q.exclude, m.y.r, m.y.d, q.s_min) : -1;
-      move_pick_apply(m, g, tgt);
+      const int what = move_pick_request(m, g, q);
+      const int tgt = what == PICK_TEST ? pick_in_neighbourhood(g, q.layer, q.iphi, q.iz, q.exclude, m.y.r, m.y.d, q.s_min) : -1;
+      move_pick_apply(m, g, tgt, what == PICK_EXIT);
     } else {
       move_step(m, fld, cfg, sc.n_trials, sc.n_accepted);
     }

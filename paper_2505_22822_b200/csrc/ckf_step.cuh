@@ -39,8 +39,9 @@ template <typename T>
 __device__ __forceinline__ void pick_warp(const GeoDev& geo, const PickSmem& ps, Move<T>& m, int lane) {
   const bool need = m.phase == PH_START || m.phase == PH_LANDED;
   PickRequest q;
-  bool ok = false;
-  if (need) ok = move_pick_request(m, geo, q);
+  int what = PICK_SKIP;
+  if (need) what = move_pick_request(m, geo, q);
+  const bool ok = what == PICK_TEST;
   const unsigned breq = __ballot_sync(0xffffffffu, ok);
   if (ok) {
     ps.rl[lane] = q.layer; ps.ri[lane] = q.iphi; ps.rj[lane] = q.iz;
@@ -87,7 +88,7 @@ __device__ __forceinline__ void pick_warp(const GeoDev& geo, const PickSmem& ps,
         if (sv == sv && (best < 0 || sv < best_s || (sv == best_s && id < best))) { best = id; best_s = sv; }
       }
     }
-    move_pick_apply(m, geo, best);
+    move_pick_apply(m, geo, best, what == PICK_EXIT);
   }
   __syncwarp();
 }
