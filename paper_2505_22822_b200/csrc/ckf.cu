@@ -337,7 +337,6 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     if (per_sm < 1 || vper_sm < 1) { fail(h, CKF_E_CUDA, "kernels do not fit on an SM (visit smem %d B)", h->visit_smem); return bail(CKF_E_CUDA); }
     h->step_regs = fa.numRegs;
     h->step_grid = per_sm * h->sm_count;
-    if (const char* d = getenv("CKF_STEP_GRID_DIV")) h->step_grid = std::max(1, h->step_grid / std::max(1, atoi(d)));  // experiment knob
     h->visit_grid = vper_sm * h->sm_count;
   }
   if (h->cfg.max_tips_per_level <= 0)

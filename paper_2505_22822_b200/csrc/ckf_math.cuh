@@ -20,10 +20,6 @@
 #define CKF_HD inline
 #endif
 
-#ifndef CKF_JAC_ROLLED
-#define CKF_JAC_ROLLED 0
-#endif
-
 namespace ckf {
 
 constexpr double KAPPA = 2.99792458e-4;  // GeV / (T mm)
@@ -270,26 +266,11 @@ CKF_HD void jac_column_q(T lam, T h, T qf, const T B1[3], const T B2[3], const T
   }
 }
 
-// Accept a trial: D <- D_step D column by column (J2, J3), then the state (P2).  The four columns go through
-// ONE copy of the column code: a rolled loop that rotates the columns through fixed registers.
+// Accept a trial: D <- D_step D column by column (J2, J3), then the state (P2).
 template <typename T>
 CKF_HD void rk_accept(Traj& y, Jac<T>& J, double h, const Trial<T>& t, double ib, double dib) {
   {
     const T lamT = (T)(KAPPA * y.qop), hT = (T)h;
-#if CKF_JAC_ROLLED
-    // rotation: after 4 rounds every column is back in its place
-#pragma unroll 1
-    for (int c = 0; c < 4; ++c) {
-      T dr[3] = {J.Rd[0][0], J.Rd[1][0], J.Rd[2][0]};
-      T dd[3] = {J.Dd[0][0], J.Dd[1][0], J.Dd[2][0]};
-      jac_column_q<T>(lamT, hT, c == 3 ? T(1) : T(0), t.B1, t.B2, t.B4, t.q1, t.q2, t.q3, t.q4, dr, dd);
-#pragma unroll
-      for (int i = 0; i < 3; ++i) {
-        J.Rd[i][0] = J.Rd[i][1]; J.Rd[i][1] = J.Rd[i][2]; J.Rd[i][2] = J.rq[i]; J.rq[i] = dr[i];
-        J.Dd[i][0] = J.Dd[i][1]; J.Dd[i][1] = J.Dd[i][2]; J.Dd[i][2] = J.dq[i]; J.dq[i] = dd[i];
-      }
-    }
-#else
 #pragma unroll
     for (int j = 0; j < 3; ++j) {
       T dr[3] = {J.Rd[0][j], J.Rd[1][j], J.Rd[2][j]};
@@ -299,7 +280,6 @@ CKF_HD void rk_accept(Traj& y, Jac<T>& J, double h, const Trial<T>& t, double ib
       for (int i = 0; i < 3; ++i) { J.Rd[i][j] = dr[i]; J.Dd[i][j] = dd[i]; }
     }
     jac_column_q<T>(lamT, hT, T(1), t.B1, t.B2, t.B4, t.q1, t.q2, t.q3, t.q4, J.rq, J.dq);
-#endif
     J.tq += (T)(h * dib);
   }
   const double h6 = h / 6.0, hh6 = h * h / 6.0;
