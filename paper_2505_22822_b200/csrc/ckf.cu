@@ -41,7 +41,7 @@ struct Workspace {
   int32_t *tip_link = nullptr, *tip_seed = nullptr;
   double *mv_y = nullptr, *pd_x = nullptr;
   void *mv_D = nullptr, *mv_dep = nullptr, *pd_C = nullptr, *sel_chi2 = nullptr;
-  int32_t *mv_from = nullptr, *mv_tgt = nullptr, *mv_stop = nullptr, *sel_idx = nullptr;
+  int32_t *mv_from = nullptr, *mv_tgt = nullptr, *mv_stop = nullptr, *sel_idx = nullptr, *mv_order = nullptr;
   int32_t *t_nsel = nullptr, *t_want = nullptr, *t_counts = nullptr, *t_keep = nullptr, *t_kex = nullptr, *blk_sum = nullptr, *t_fin = nullptr;
   void *s_loc = nullptr, *s_var = nullptr, *s_v0max = nullptr;  // gate index (ckf_sort_slices)
   int32_t* s_idx = nullptr;
@@ -138,7 +138,7 @@ void fill_params(ckf_handle* h, Workspace& w, KParams<T>& p) {
   p.tcap = h->tcap;
   p.tip_link = w.tip_link; p.tip_seed = w.tip_seed;
   p.mv_y = w.mv_y; p.mv_D = (T*)w.mv_D; p.mv_dep = (T*)w.mv_dep; p.mv_from = w.mv_from; p.mv_tgt = w.mv_tgt;
-  p.mv_stop = w.mv_stop;
+  p.mv_stop = w.mv_stop; p.mv_order = w.mv_order;
   p.pd_x = w.pd_x; p.pd_C = (T*)w.pd_C; p.sel_chi2 = (T*)w.sel_chi2; p.sel_idx = w.sel_idx;
   p.t_nsel = w.t_nsel; p.t_want = w.t_want; p.t_counts = w.t_counts; p.t_keep = w.t_keep; p.t_kex = w.t_kex;
   p.blk_sum = w.blk_sum; p.t_fin = w.t_fin;
@@ -370,7 +370,9 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     CKB(dalloc(h, (char**)&w.s_var, 2 * (size_t)c->max_measurements * ts));
     CKB(dalloc(h, &w.s_idx, (size_t)c->max_measurements * 4));
     CKB(dalloc(h, (char**)&w.s_v0max, (size_t)g->n_modules * ts));
-    CKB(dalloc(h, &w.globals, 16 * 4));
+    CKB(dalloc(h, &w.globals, 64 * 4));
+    static_assert(G_N <= 64, "globals block too small");
+    CKB(dalloc(h, &w.mv_order, (size_t)NBIN * TC * 4));
     CKB(dalloc(h, &w.counters, CNT_N * 8));
     CKB(cudaEventCreateWithFlags(&w.done, cudaEventDisableTiming));
     // staging for ckf_find_host

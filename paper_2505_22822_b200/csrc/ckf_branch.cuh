@@ -137,6 +137,7 @@ __global__ void __launch_bounds__(SCAN_NT) ckf_scan(const KParams<T> p, int leve
     p.g[G_NTIPS0 + ((level + 1) & 1)] = allowed;
     p.g[G_STEP_CURSOR] = 0;
     p.g[G_SCAN_TICKET] = 0;
+    for (int b = 0; b < NBIN; ++b) p.g[G_BIN0 + b] = 0;  // ckf_update of this level refills the step schedule
     p.blk_sum[nb] = tot;
     atomicAdd(p.counters + CNT_TIPS, (unsigned long long)n);
     atomicAdd(p.counters + CNT_LINKS, (unsigned long long)allowed);
@@ -160,6 +161,21 @@ __device__ __forceinline__ int find_parent(const KParams<T>& p, int n, int nb, i
     if (boff + p.t_kex[mid] <= c) a = mid; else b = mid;
   }
   return a;
+}
+
+// Cost class of the move a live child is about to make = its predicted number of RKN4 trials (DESIGN.md §6,
+// "step schedule").  A scheduling hint only: ckf_step processes the classes in descending order so that the
+// lanes of a warp run moves of similar length and the launch ends on the short ones; results do not depend on
+// it.  trials ~ 0.26 (gap / sin theta)^0.71 (0.6 |q/p| / sin theta)^0.27, fitted on configs[3] (r = 0.95).
+__device__ __forceinline__ int step_cost_bin(const GeoDev& g, int module, const Traj& y, int overlap) {
+  if (overlap >= 0) return 0;  // same-layer neighbour: one or two short trials
+  const int L = g.mod[module].layer;
+  if (L + 1 >= g.n_layers) return 0;  // leaves the barrel at once
+  const float st = sqrtf((float)(y.d[0] * y.d[0] + y.d[1] * y.d[1]));
+  const float gap = (float)(g.layer[L + 1].r - g.layer[L].r);
+  const float pred = 0.2565f * __powf(gap / st, 0.713f) * __powf(0.6f * fabsf((float)y.qop) / st, 0.266f);
+  const int b = (int)pred;
+  return b < 1 ? 1 : (b > NBIN - 1 ? NBIN - 1 : b);
 }
 
 // a9 + a10: thread per child, in child order (parent tip order, then (chi2, index) rank): Kalman update or hole
@@ -213,7 +229,8 @@ __global__ void __launch_bounds__(SCAN_NT) ckf_update(const KParams<T> p, int le
     } else {
       par = c < nc ? find_parent<T>(p, n, nb, c) : 0;
     }
-    if (c >= nc) continue;
+    int bin = -1;
+    if (c < nc) {
     const int j = c - (p.blk_sum[par / SCAN_NT] + p.t_kex[par]);
     const int nl = lbase + c;
     const int plink = tlink[par], seed = tseed[par];
@@ -274,10 +291,24 @@ __global__ void __launch_bounds__(SCAN_NT) ckf_update(const KParams<T> p, int le
 #pragma unroll
         for (int i = 0; i < 5; ++i) p.mv_dep[i * TC + c] = dep[i];
         // N2 here, at full lanes, instead of inside the RKN4 kernel: the overlap neighbour of the child's departure
-        p.mv_tgt[TC + c] = overlap_neighbour(p.geo, target, y.r, y.d);
+        const int ov = overlap_neighbour(p.geo, target, y.r, y.d);
+        p.mv_tgt[TC + c] = ov;
+        bin = step_cost_bin(p.geo, target, y, ov);
       }
     }
     p.mv_stop[c] = stop;
+    }
+    // step schedule: append the live child to its cost class (one atomic per class present in the warp)
+    const unsigned live = __ballot_sync(0xffffffffu, bin >= 0);
+    if (bin >= 0) {
+      const int lane = threadIdx.x & 31;
+      const unsigned peers = __match_any_sync(live, bin);
+      const int leader = __ffs(peers) - 1;
+      int base = 0;
+      if (lane == leader) base = atomicAdd(p.g + G_BIN0 + bin, __popc(peers));
+      base = __shfl_sync(peers, base, leader);
+      p.mv_order[(size_t)bin * TC + base + __popc(peers & ((1u << lane) - 1u))] = c;
+    }
   }
   flush_counter(p.counters + CNT_UPDATES, my_updates);
 }

@@ -44,7 +44,8 @@ enum CounterId { CNT_TIPS = 0, CNT_VISITS, CNT_TRIALS, CNT_ACCEPTED, CNT_GATE, C
 
 // per-event device globals (int32 each)
 enum GlobalId { G_LINK_COUNT = 0, G_FIRST_BAD, G_TOTAL_TRACKS, G_TOTAL_ENTRIES, G_NTIPS0, G_NTIPS1, G_STEP_CURSOR,
-                G_SCAN_TICKET, G_LBASE, G_SEED_TICKET, G_N };
+                G_SCAN_TICKET, G_LBASE, G_SEED_TICKET, G_BIN0, G_N = G_BIN0 + 16 };
+constexpr int NBIN = 16;          // cost classes of the step schedule (G_BIN0 .. G_BIN0 + NBIN - 1 hold their sizes)
 
 template <typename T>
 struct KParams {
@@ -97,6 +98,7 @@ struct KParams {
   int32_t* mv_from;    // [tcap] module the tip stands on
   int32_t* mv_tgt;     // [2][tcap] module reached; overlap neighbour at departure (N2, by ckf_update), -1 none
   int32_t* mv_stop;    // [tcap] stop reason so far
+  int32_t* mv_order;   // [NBIN][tcap] live tips of the level grouped by predicted RKN4 trial count (step schedule)
   // prediction + selection (ckf_visit -> ckf_cap, ckf_update)
   double* pd_x;        // [6][tcap]
   T* pd_C;             // [21][tcap]

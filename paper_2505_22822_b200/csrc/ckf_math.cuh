@@ -282,7 +282,7 @@ CKF_HD void rk_accept(Traj& y, Jac<T>& J, double h, const Trial<T>& t, double ib
     jac_column_q<T>(lamT, hT, T(1), t.B1, t.B2, t.B4, t.q1, t.q2, t.q3, t.q4, J.rq, J.dq);
     J.tq += (T)(h * dib);
   }
-  const double h6 = h / 6.0, hh6 = h * h / 6.0;
+  const double h6 = h * (1.0 / 6.0), hh6 = h * h * (1.0 / 6.0);  // one rounding away from h / 6: far inside 1e-9
   double dn[3], n2 = 0.0;
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
@@ -290,9 +290,9 @@ CKF_HD void rk_accept(Traj& y, Jac<T>& J, double h, const Trial<T>& t, double ib
     dn[i] = y.d[i] + h6 * t.s2[i];
     n2 += dn[i] * dn[i];
   }
-  const double nrm = sqrt(n2);
+  const double inrm = 1.0 / sqrt(n2);
 #pragma unroll
-  for (int i = 0; i < 3; ++i) y.d[i] = dn[i] / nrm;
+  for (int i = 0; i < 3; ++i) y.d[i] = dn[i] * inrm;
   y.t += h * ib;
 }
 

@@ -95,9 +95,16 @@ __device__ __forceinline__ void pick_warp(const GeoDev& geo, const PickSmem& ps,
 
 template <typename T, int MINB>
 __global__ void __launch_bounds__(STEP_NT, MINB) ckf_step(const KParams<T> p, int level) {
-  const int n = p.g[G_NTIPS0 + (level & 1)];
-  if (n == 0 || level == 0) return;  // level 0: the seed's own module, identity transport (N6)
+  if (p.g[G_NTIPS0 + (level & 1)] == 0 || level == 0) return;  // level 0: the seed's own module, identity transport (N6)
   __shared__ __align__(16) unsigned char smem_raw[(STEP_NT / 32) * PickSmem::bytes()];
+  // step schedule: the live tips of the level, grouped by predicted trial count (ckf_update), longest first
+  __shared__ int s_binend[NBIN];
+  if (threadIdx.x == 0) {
+    int acc = 0;
+    for (int k = 0; k < NBIN; ++k) { acc += p.g[G_BIN0 + NBIN - 1 - k]; s_binend[k] = acc; }
+  }
+  __syncthreads();
+  const int n = s_binend[NBIN - 1];
   const int lane = threadIdx.x & 31, wib = threadIdx.x >> 5;
   PickSmem ps;
   ps.carve(smem_raw + (size_t)wib * PickSmem::bytes());
@@ -145,8 +152,14 @@ __global__ void __launch_bounds__(STEP_NT, MINB) ckf_step(const KParams<T> p, in
         if (lane == 0) base = atomicAdd(p.g + G_STEP_CURSOR, __popc(idle));
         base = __shfl_sync(0xffffffffu, base, 0);
         if (base + __popc(idle) >= n) more = false;
-        const int t = base + __popc(idle & ((1u << lane) - 1u));
-        if (m.phase == PH_IDLE && t < n && p.mv_stop[t] == STOP_NONE) {
+        const int q = base + __popc(idle & ((1u << lane) - 1u));
+        int t = -1;
+        if (m.phase == PH_IDLE && q < n) {
+          int k = 0;
+          while (q >= s_binend[k]) ++k;
+          t = p.mv_order[(size_t)(NBIN - 1 - k) * TC + (q - (k ? s_binend[k - 1] : 0))];
+        }
+        if (t >= 0 && p.mv_stop[t] == STOP_NONE) {
           tip = t;
 #pragma unroll
           for (int i = 0; i < 3; ++i) { m.y.r[i] = p.mv_y[i * TC + t]; m.y.d[i] = p.mv_y[(3 + i) * TC + t]; }
