@@ -75,6 +75,15 @@ def lib():
         L.oracle_highland_theta0.restype = C.c_double
         L.oracle_highland_theta0.argtypes = [C.c_double, C.c_double, C.c_double]
         L.oracle_add_material.argtypes = [C.POINTER(OGeometry), C.POINTER(OConfig), C.c_int32, _dp, _dp]
+        L.oracle_kf_fit.restype = None
+        L.oracle_kf_fit.argtypes = [C.POINTER(OGeometry), C.POINTER(OField), C.POINTER(OConfig), _ip, _dp, _dp, _ip, _dp,
+                                    _dp, C.c_int32, _ip, _ip, _ip, C.c_int32, _ip, _ip, _dp, _dp, _dp, _dp, _dp]
+        L.oracle_kf_fit_states.restype = C.c_int32
+        L.oracle_kf_fit_states.argtypes = [C.POINTER(OGeometry), C.POINTER(OField), C.POINTER(OConfig), _ip, _dp, _dp,
+                                           C.c_int32, _dp, _dp, C.c_int32, _ip, C.c_int32, _ip, _ip, _dp, _dp, _dp, _dp,
+                                           _dp, _dp, _dp]
+        L.oracle_rts_smooth.restype = C.c_int32
+        L.oracle_rts_smooth.argtypes = [C.c_int32, _dp, _dp, _dp, _dp, _dp, _dp, _dp]
         _lib = L
     return _lib
 
@@ -242,3 +251,63 @@ def add_material(setup: Setup, module, x, Cov):
     x, Cov = _d(x), _d(Cov).reshape(36).copy()
     lib().oracle_add_material(C.byref(setup.geometry), C.byref(setup.config), int(module), _pd(x), _pd(Cov))
     return Cov.reshape(6, 6)
+
+
+# ------------------------------------------------------------------ K: KF fit + RTS smoother
+@dataclass
+class Fits:
+    """Result of the KF fit + RTS smoother over a CSR list of candidates (layout of `ckf_fits`, include/ckf.h)."""
+    n_tracks: int
+    status: np.ndarray        # [n_tracks] 0 = fitted, else stop reason
+    n_states: np.ndarray      # [n_tracks] visited modules of the forward pass
+    chi2_sum: np.ndarray      # [n_tracks] forward (predicted-residual) chi2 sum
+    last_params: np.ndarray   # [n_tracks, 6] forward-filtered state at the last measurement
+    last_cov: np.ndarray      # [n_tracks, 36]
+    first_cov: np.ndarray     # [n_tracks, 36] smoothed covariance at the first measurement
+    entry_params: np.ndarray  # [n_entries, 6] smoothed parameters at every measurement of the list
+
+
+def kf_fit(setup: Setup, ev, track_offsets, meas_idx, seed_id, n_threads: int = 1) -> Fits:
+    L = lib()
+    mo, lo, va = _i(ev.module_offsets), _d(ev.loc), _d(ev.var)
+    sm, sp, sc = _i(ev.seed_module), _d(ev.seed_params), _d(ev.seed_cov)
+    to, mi, si = _i(track_offsets), _i(meas_idx), _i(seed_id)
+    nt = si.shape[0]
+    ne = int(to[nt]) if nt else 0
+    out = Fits(nt, np.zeros(nt, np.int32), np.zeros(nt, np.int32), np.zeros(nt), np.zeros((nt, 6)), np.zeros((nt, 36)),
+               np.zeros((nt, 36)), np.zeros((ne, 6)))
+    L.oracle_kf_fit(C.byref(setup.geometry), C.byref(setup.field), C.byref(setup.config), _pi(mo), _pd(lo), _pd(va),
+                    _pi(sm), _pd(sp), _pd(sc), nt, _pi(to), _pi(mi), _pi(si), int(n_threads), _pi(out.status),
+                    _pi(out.n_states), _pd(out.chi2_sum), _pd(out.last_params), _pd(out.last_cov), _pd(out.first_cov),
+                    _pd(out.entry_params))
+    return out
+
+
+def kf_fit_states(setup: Setup, ev, seed: int, meas, max_states: int = 64):
+    """Every state of one track's fit: dict of module, meas, xp, Cp, xf, Cf, J, xs, Cs (arrays over states)."""
+    mo, lo, va = _i(ev.module_offsets), _d(ev.loc), _d(ev.var)
+    sx, sC = _d(ev.seed_params[seed]), _d(ev.seed_cov[seed]).reshape(36)
+    me = _i(meas)
+    n = max_states
+    mod, mu = np.zeros(n, np.int32), np.zeros(n, np.int32)
+    xp, xf, xs = np.zeros((n, 6)), np.zeros((n, 6)), np.zeros((n, 6))
+    Cp, Cf, J, Cs = np.zeros((n, 36)), np.zeros((n, 36)), np.zeros((n, 36)), np.zeros((n, 36))
+    ns = lib().oracle_kf_fit_states(C.byref(setup.geometry), C.byref(setup.field), C.byref(setup.config), _pi(mo),
+                                    _pd(lo), _pd(va), int(ev.seed_module[seed]), _pd(sx), _pd(sC), me.shape[0], _pi(me),
+                                    n, _pi(mod), _pi(mu), _pd(xp), _pd(Cp), _pd(xf), _pd(Cf), _pd(J), _pd(xs), _pd(Cs))
+    if ns < 0:
+        return {"status": -ns}
+    ns = min(ns, n)
+    r6 = lambda a: a[:ns].reshape(ns, 6, 6)
+    return {"status": 0, "module": mod[:ns], "meas": mu[:ns], "xp": xp[:ns], "xf": xf[:ns], "xs": xs[:ns],
+            "Cp": r6(Cp), "Cf": r6(Cf), "J": r6(J), "Cs": r6(Cs)}
+
+
+def rts_smooth(xp, Cp, xf, Cf, J):
+    """The RTS recursion alone on given states ([n,6] / [n,6,6]; J[k] leads into state k)."""
+    xp, xf = _d(xp), _d(xf)
+    n = xp.shape[0]
+    Cp, Cf, J = _d(Cp).reshape(n, 36), _d(Cf).reshape(n, 36), _d(J).reshape(n, 36)
+    xs, Cs = np.zeros((n, 6)), np.zeros((n, 36))
+    rc = lib().oracle_rts_smooth(n, _pd(xp), _pd(Cp), _pd(xf), _pd(Cf), _pd(J), _pd(xs), _pd(Cs))
+    return rc, xs, Cs.reshape(n, 6, 6)

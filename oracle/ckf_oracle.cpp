@@ -13,6 +13,9 @@
 // Pins (tests/test_oracle_pins.py): analytic helix (P2-P5), finite-difference Jacobian (J1-J5),
 // closed-form scalar gain + information-form identity (V1-V3), Highland values (V5), multilinear field
 // (F), brute-force module sequence (N2-N5), brute-force CKF enumeration on a toy (R9-R11).
+// KF fit + RTS smoother (rules K, tests/test_oracle_fit.py): scalar random walk against its information-form
+// closed form, the smoothed states of real tracks against a dense Gaussian conditioning of the linearised
+// model (numpy), forward pass = the CKF candidate's reported state.
 // Parity unpinned (convention only, fixed by DESIGN.md): the order in which the per-seed cap R10 cuts,
 // hole-only-when-nothing-passes (A5), outward-only navigation (A7), inclusive in-bounds edges (A10),
 // min_measurements = 3 (A14).
@@ -765,6 +768,166 @@ void run_seed(const OGeometry& g, const OField& fld, const OConfig& cfg, const i
   }
 }
 
+// ====================================================================================== K: KF fit + RTS smoother
+// "a Kalman Filter-based fitting [8], which runs a smoothing algorithm called the
+// Rauch-Tung-Striebel (RTS) smoother [19], is applied additionally to the tracks to make all track parameters
+// consider all measurements in the pattern"; the parameters at the FIRST measurement are the ones it names as
+// wanted (vertex reconstruction).  The paper prints no formula; rules K1-K5 of DESIGN.md §3 restate the
+// textbook filter/smoother of its refs [8], [19] on top of the P/J/N/V rules above.
+//
+// One visited module = one STATE: predicted (xp, Cp), filtered (xf, Cf), the bound->bound Jacobian J that made
+// the prediction from the previous state's filtered one, and the measurement used (-1 = passed without one).
+struct FitState {
+  int module, meas;
+  double chi2;
+  double xp[6], Cp[6][6], xf[6], Cf[6][6], J[6][6];
+};
+
+// K2: forward filter = the CKF's own path with the branch choice replaced by the candidate's list: state 0 is the
+// seed's module with the seed's (x, C) (N6); on every visited module the next unconsumed measurement of the list
+// is used iff it lives on that module (V1 chi2, V3 update), otherwise the module is passed (filtered =
+// predicted); then the N-rules move on (V5 material on leaving, J1-J5).  Ends when the list is consumed.
+int fit_forward(const OGeometry& g, const OField& fld, const OConfig& cfg, const int32_t* moff, const double* loc,
+                const double* var, int seed_module, const double* sx, const double* sC, const int32_t* meas, int n_meas,
+                std::vector<FitState>& st, Counters& cnt) {
+  double x[6], C[6][6];
+  for (int i = 0; i < 6; ++i) {
+    x[i] = sx[i];
+    for (int j = 0; j < 6; ++j) C[i][j] = sC[6 * i + j];
+  }
+  int module = seed_module, next = 0;
+  if (n_meas < 1) return STOP_NONE;
+  for (int level = 0;; ++level) {
+    if (level >= cfg.max_levels) return STOP_LEVEL_LIMIT;
+    FitState s;
+    if (level == 0) {
+      bool ok = (x[3] > 0.0 && x[3] < PI);
+      for (int a = 0; a < 6; ++a) ok = ok && std::isfinite(x[a]);
+      if (!ok) return STOP_NUMERIC;
+      std::memcpy(s.xp, x, sizeof(x));
+      std::memcpy(s.Cp, C, sizeof(C));
+      for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) s.J[i][j] = (i == j) ? 1.0 : 0.0;
+      s.module = module;
+    } else {
+      int tg = -1;
+      const int stop = move_to_next_module(g, fld, cfg, module, x, C, tg, s.xp, s.Cp, s.J, cnt);
+      if (stop != STOP_NONE) return stop;
+      s.module = tg;
+    }
+    const int k = meas[next];
+    if (k >= moff[s.module] && k < moff[s.module + 1]) {
+      s.meas = k;
+      s.chi2 = predicted_chi2(s.xp, s.Cp, loc + 2 * k, var + 2 * k);
+      kalman_update(s.xp, s.Cp, loc + 2 * k, var + 2 * k, s.xf, s.Cf);
+      ++next;
+    } else {
+      s.meas = -1;
+      s.chi2 = 0.0;
+      std::memcpy(s.xf, s.xp, sizeof(s.xp));
+      std::memcpy(s.Cf, s.Cp, sizeof(s.Cp));
+    }
+    st.push_back(s);
+    if (next == n_meas) return STOP_NONE;
+    std::memcpy(x, s.xf, sizeof(x));
+    std::memcpy(C, s.Cf, sizeof(C));
+    module = s.module;
+  }
+}
+
+// K4 helper: X = G^-1 B for a symmetric positive definite 6x6 G, by diagonal scaling (G_ii -> 1; the bound
+// covariance mixes mm^2, rad^2 and GeV^-2, 10 orders of magnitude apart) and Cholesky G' = L L^T.
+// Returns false when G is not positive definite.
+bool spd_solve6(const double G[6][6], const double B[6][6], double X[6][6]) {
+  double s[6], L[6][6];
+  for (int i = 0; i < 6; ++i) {
+    if (!(G[i][i] > 0.0)) return false;
+    s[i] = 1.0 / std::sqrt(G[i][i]);
+  }
+  for (int j = 0; j < 6; ++j) {
+    double d = G[j][j] * s[j] * s[j];
+    for (int k = 0; k < j; ++k) d -= L[j][k] * L[j][k];
+    if (!(d > 0.0)) return false;
+    L[j][j] = std::sqrt(d);
+    for (int i = j + 1; i < 6; ++i) {
+      double v = G[i][j] * s[i] * s[j];
+      for (int k = 0; k < j; ++k) v -= L[i][k] * L[j][k];
+      L[i][j] = v / L[j][j];
+    }
+  }
+  for (int c = 0; c < 6; ++c) {
+    double z[6], w[6];
+    for (int i = 0; i < 6; ++i) {  // L z = S b
+      double v = B[i][c] * s[i];
+      for (int k = 0; k < i; ++k) v -= L[i][k] * z[k];
+      z[i] = v / L[i][i];
+    }
+    for (int i = 5; i >= 0; --i) {  // L^T w = z
+      double v = z[i];
+      for (int k = i + 1; k < 6; ++k) v -= L[k][i] * w[k];
+      w[i] = v / L[i][i];
+    }
+    for (int i = 0; i < 6; ++i) X[i][c] = w[i] * s[i];
+  }
+  return true;
+}
+
+inline double wrap_pi(double a) {
+  while (a > PI) a -= 2.0 * PI;
+  while (a <= -PI) a += 2.0 * PI;
+  return a;
+}
+
+// K4: RTS backward recursion [19] over states 0..n-1.  xs[n-1] = xf[n-1]; for k = n-2..0:
+//   A_k = Cf[k] J[k+1]^T Cp[k+1]^-1;  xs[k] = xf[k] + A_k (xs[k+1] - xp[k+1]);
+//   Cs[k] = Cf[k] + A_k (Cs[k+1] - Cp[k+1]) A_k^T   (symmetrised).
+// The process noise (V5) enters Cp[k+1] = J (Cf[k] + Q_k) J^T only; the gain uses Cf[k] without it, because the
+// noise of the step k -> k+1 is independent of state k.  Angle differences and results are wrapped to (-pi, pi].
+bool rts_smooth(int n, const FitState* st, double (*xs)[6], double (*Cs)[6][6]) {
+  if (n < 1) return true;
+  std::memcpy(xs[n - 1], st[n - 1].xf, sizeof(double) * 6);
+  std::memcpy(Cs[n - 1], st[n - 1].Cf, sizeof(double) * 36);
+  for (int k = n - 2; k >= 0; --k) {
+    const FitState& a = st[k];
+    const FitState& b = st[k + 1];
+    double M[6][6], X[6][6];  // M = J Cf[k];  X = Cp[k+1]^-1 M = A_k^T
+    for (int i = 0; i < 6; ++i)
+      for (int j = 0; j < 6; ++j) {
+        double v = 0.0;
+        for (int l = 0; l < 6; ++l) v += b.J[i][l] * a.Cf[l][j];
+        M[i][j] = v;
+      }
+    if (!spd_solve6(b.Cp, M, X)) return false;
+    double dx[6], dC[6][6], T[6][6];
+    for (int i = 0; i < 6; ++i) dx[i] = xs[k + 1][i] - b.xp[i];
+    dx[2] = wrap_pi(dx[2]);
+    for (int i = 0; i < 6; ++i) {
+      double v = 0.0;
+      for (int j = 0; j < 6; ++j) v += X[j][i] * dx[j];
+      xs[k][i] = a.xf[i] + v;
+    }
+    xs[k][2] = wrap_pi(xs[k][2]);
+    for (int i = 0; i < 6; ++i)
+      for (int j = 0; j < 6; ++j) dC[i][j] = Cs[k + 1][i][j] - b.Cp[i][j];
+    for (int i = 0; i < 6; ++i)   // T = dC X
+      for (int j = 0; j < 6; ++j) {
+        double v = 0.0;
+        for (int l = 0; l < 6; ++l) v += dC[i][l] * X[l][j];
+        T[i][j] = v;
+      }
+    double R[6][6];
+    for (int i = 0; i < 6; ++i)   // R = X^T T
+      for (int j = 0; j < 6; ++j) {
+        double v = 0.0;
+        for (int l = 0; l < 6; ++l) v += X[l][i] * T[l][j];
+        R[i][j] = a.Cf[i][j] + v;
+      }
+    for (int i = 0; i < 6; ++i)
+      for (int j = 0; j < 6; ++j) Cs[k][i][j] = 0.5 * (R[i][j] + R[j][i]);
+  }
+  return true;
+}
+
 struct Result {
   std::vector<Track> tracks;
   Counters cnt;
@@ -840,6 +1003,104 @@ void oracle_result_copy(const void* r, int32_t* track_offsets, int32_t* meas_idx
   track_offsets[R->tracks.size()] = off;
 }
 void oracle_result_free(void* r) { delete (Result*)r; }
+
+// ---- K: KF fit + RTS smoother over candidates given as a CSR list (the layout ckf_find reports).
+// Per track: status (0 = fitted, else the stop reason of the forward pass, or STOP_NUMERIC when a predicted
+// covariance is not positive definite), number of states, forward chi2 sum, the forward-filtered state at the
+// last measurement (K2: equals the CKF candidate's), the smoothed covariance at the first measurement; per
+// entry (measurement of the list): the smoothed parameters at that measurement's state.
+void oracle_kf_fit(const OGeometry* g, const OField* f, const OConfig* cfg, const int32_t* module_offsets,
+                   const double* loc, const double* var, const int32_t* seed_module, const double* seed_params,
+                   const double* seed_cov, int32_t n_tracks, const int32_t* track_offsets, const int32_t* meas_idx,
+                   const int32_t* seed_id, int32_t n_threads, int32_t* status, int32_t* n_states, double* chi2_sum,
+                   double* last_x, double* last_C, double* first_C, double* entry_xs) {
+  if (n_threads < 1) n_threads = 1;
+  if (n_threads > n_tracks) n_threads = std::max(1, n_tracks);
+  auto work = [&](int t) {
+    const long long lo = (long long)n_tracks * t / n_threads, hi = (long long)n_tracks * (t + 1) / n_threads;
+    Counters cnt;
+    std::vector<FitState> st;
+    std::vector<double> xs, Cs;
+    for (long long tr = lo; tr < hi; ++tr) {
+      const int e0 = track_offsets[tr], n = track_offsets[tr + 1] - e0, sd = seed_id[tr];
+      st.clear();
+      int rc = fit_forward(*g, *f, *cfg, module_offsets, loc, var, seed_module[sd], seed_params + 6 * sd,
+                           seed_cov + 36 * sd, meas_idx + e0, n, st, cnt);
+      const int ns = (int)st.size();
+      n_states[tr] = ns;
+      chi2_sum[tr] = 0.0;
+      for (int i = 0; i < 6; ++i) last_x[6 * tr + i] = 0.0;
+      for (int i = 0; i < 36; ++i) { last_C[36 * tr + i] = 0.0; first_C[36 * tr + i] = 0.0; }
+      for (int e = 0; e < 6 * n; ++e) entry_xs[6 * (size_t)e0 + e] = 0.0;
+      if (rc == STOP_NONE && ns > 0) {
+        xs.assign((size_t)ns * 6, 0.0);
+        Cs.assign((size_t)ns * 36, 0.0);
+        if (!rts_smooth(ns, st.data(), (double(*)[6])xs.data(), (double(*)[6][6])Cs.data())) rc = STOP_NUMERIC;
+      }
+      status[tr] = rc;
+      if (rc != STOP_NONE || ns == 0) continue;
+      double c2 = 0.0;
+      int e = 0;
+      bool first = true;
+      for (int k = 0; k < ns; ++k) {
+        if (st[k].meas < 0) continue;
+        c2 += st[k].chi2;
+        for (int i = 0; i < 6; ++i) entry_xs[6 * (size_t)(e0 + e) + i] = xs[(size_t)k * 6 + i];
+        if (first) {
+          for (int i = 0; i < 36; ++i) first_C[36 * tr + i] = Cs[(size_t)k * 36 + i];
+          first = false;
+        }
+        ++e;
+      }
+      chi2_sum[tr] = c2;
+      for (int i = 0; i < 6; ++i) last_x[6 * tr + i] = st[ns - 1].xf[i];
+      for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) last_C[36 * tr + 6 * i + j] = st[ns - 1].Cf[i][j];
+    }
+  };
+  if (n_threads == 1) work(0);
+  else {
+    std::vector<std::thread> th;
+    for (int t = 0; t < n_threads; ++t) th.emplace_back(work, t);
+    for (auto& x : th) x.join();
+  }
+}
+
+// One track, every state (for the pins): returns the number of states (<= max_states are copied) or -stop.
+int32_t oracle_kf_fit_states(const OGeometry* g, const OField* f, const OConfig* cfg, const int32_t* module_offsets,
+                             const double* loc, const double* var, int32_t seed_module, const double* sx,
+                             const double* sC, int32_t n_meas, const int32_t* meas, int32_t max_states,
+                             int32_t* module, int32_t* meas_used, double* xp, double* Cp, double* xf, double* Cf,
+                             double* J, double* xs, double* Cs) {
+  Counters cnt;
+  std::vector<FitState> st;
+  const int rc = fit_forward(*g, *f, *cfg, module_offsets, loc, var, seed_module, sx, sC, meas, n_meas, st, cnt);
+  if (rc != STOP_NONE) return -rc;
+  const int ns = (int)st.size();
+  std::vector<double> vx((size_t)ns * 6), vC((size_t)ns * 36);
+  if (!rts_smooth(ns, st.data(), (double(*)[6])vx.data(), (double(*)[6][6])vC.data())) return -STOP_NUMERIC;
+  for (int k = 0; k < ns && k < max_states; ++k) {
+    module[k] = st[k].module; meas_used[k] = st[k].meas;
+    std::memcpy(xp + 6 * k, st[k].xp, 48); std::memcpy(xf + 6 * k, st[k].xf, 48);
+    std::memcpy(Cp + 36 * k, st[k].Cp, 288); std::memcpy(Cf + 36 * k, st[k].Cf, 288);
+    std::memcpy(J + 36 * k, st[k].J, 288);
+    std::memcpy(xs + 6 * k, &vx[(size_t)k * 6], 48); std::memcpy(Cs + 36 * k, &vC[(size_t)k * 36], 288);
+  }
+  return ns;
+}
+
+// The RTS recursion alone on caller-given states (closed-form pin).  Arrays [n][6] / [n][36]; J[k] leads into k.
+int32_t oracle_rts_smooth(int32_t n, const double* xp, const double* Cp, const double* xf, const double* Cf,
+                          const double* J, double* xs, double* Cs) {
+  std::vector<FitState> st(n);
+  for (int k = 0; k < n; ++k) {
+    st[k].module = 0; st[k].meas = 0; st[k].chi2 = 0.0;
+    std::memcpy(st[k].xp, xp + 6 * k, 48); std::memcpy(st[k].xf, xf + 6 * k, 48);
+    std::memcpy(st[k].Cp, Cp + 36 * k, 288); std::memcpy(st[k].Cf, Cf + 36 * k, 288);
+    std::memcpy(st[k].J, J + 36 * k, 288);
+  }
+  return rts_smooth(n, st.data(), (double(*)[6])xs, (double(*)[6][6])Cs) ? 0 : STOP_NUMERIC;
+}
 
 // ---- pieces exposed for the pins (tests/test_oracle_pins.py)
 void oracle_field_at(const OField* f, const double r[3], double B[3]) { field_at(*f, r, B); }
