@@ -26,7 +26,7 @@
 extern "C" {
 #endif
 
-#define CKF_ABI_VERSION 2
+#define CKF_ABI_VERSION 3
 
 /* return codes */
 #define CKF_OK 0
@@ -174,6 +174,34 @@ int ckf_find(ckf_handle* handle, const ckf_measurements* measurements, const ckf
  * Output arrays are filled up to *n_tracks / track_offsets[*n_tracks] after the stream is synchronised. */
 int ckf_find_host(ckf_handle* handle, const ckf_measurements* measurements, const ckf_seeds* seeds, ckf_tracks* out,
                   void* cuda_stream);
+
+/* ---- Kalman-filter track fit + RTS smoother over candidates ----------
+ * "The filtered track parameters at the first measurement ... are estimated only with one measurement hence
+ * least accurate.  Therefore, a Kalman Filter-based fitting, which runs a smoothing algorithm called the
+ * Rauch-Tung-Striebel (RTS) smoother, is applied additionally to the tracks".
+ * Rules K1-K5 of DESIGN.md 3: the forward filter walks each candidate's own path (same navigation, RKN4,
+ * Jacobian, material and update rules as ckf_find) using the listed measurements in order; every visited
+ * module is a state; the RTS recursion then runs backward over the states in float64.
+ * Results.  DEVICE pointers, caller-owned, sized from max_tracks / max_track_entries like ckf_tracks. */
+typedef struct {
+  int32_t* status;      /* [max_tracks] 0 = fitted; else CKF_STOP_* of the forward pass, or CKF_STOP_NUMERIC when a
+                           predicted covariance was not positive definite.  A track that is not fitted has zeros
+                           in every other array                                                              */
+  int32_t* n_states;    /* [max_tracks] modules the forward pass visited                                      */
+  void* chi2_sum;       /* T[max_tracks] forward chi2 sum (equals ckf_tracks.chi2_sum)                        */
+  void* last_params;    /* T[max_tracks][6]  forward-filtered state at the last measurement (= ckf_tracks.params) */
+  void* last_cov;       /* T[max_tracks][36]                                                                  */
+  void* first_cov;      /* T[max_tracks][36] SMOOTHED covariance at the first measurement                     */
+  void* entry_params;   /* T[max_track_entries][6] SMOOTHED parameters at every measurement, parallel to
+                           ckf_tracks.meas_idx (entry track_offsets[t] is the first measurement of track t)  */
+} ckf_fits;
+
+/* Fits every candidate of `tracks` (the DEVICE arrays a ckf_find on the same measurements and seeds filled;
+ * *tracks->n_tracks is read on the device, no host synchronisation).  Asynchronous on `cuda_stream`.  The first
+ * call on a handle reserves the state store (about 1.5 GB for fp32); later calls allocate nothing.  Calls
+ * on different streams are ordered one after the other (one state store per handle). */
+int ckf_fit(ckf_handle* handle, const ckf_measurements* measurements, const ckf_seeds* seeds, const ckf_tracks* tracks,
+            ckf_fits* out, void* cuda_stream);
 
 /* Copies the work counters of the most recent ckf_find issued on `cuda_stream` (synchronises that stream). */
 int ckf_get_counters(ckf_handle* handle, void* cuda_stream, ckf_counters* out);

@@ -20,7 +20,7 @@ _vp = C.c_void_p
 HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libckf.so")
 
-EXPORTS = ("ckf_create", "ckf_find", "ckf_find_host", "ckf_get_counters", "ckf_get_launch_info", "ckf_destroy",
+EXPORTS = ("ckf_create", "ckf_find", "ckf_find_host", "ckf_fit", "ckf_get_counters", "ckf_get_launch_info", "ckf_destroy",
            "ckf_set_timing", "ckf_get_timing",
            "ckf_last_error", "ckf_abi_version")
 
@@ -60,6 +60,11 @@ class ckf_tracks(C.Structure):
                 ("chi2_sum", _vp), ("entry_chi2", _vp)]
 
 
+class ckf_fits(C.Structure):
+    _fields_ = [("status", _vp), ("n_states", _vp), ("chi2_sum", _vp), ("last_params", _vp), ("last_cov", _vp),
+                ("first_cov", _vp), ("entry_params", _vp)]
+
+
 class ckf_timing(C.Structure):
     _fields_ = [("init_ms", C.c_float), ("sort_ms", C.c_float), ("step_ms", C.c_float), ("visit_ms", C.c_float),
                 ("scan_ms", C.c_float), ("update_ms", C.c_float), ("emit_ms", C.c_float), ("launches", C.c_int32)]
@@ -88,6 +93,9 @@ def load_library():
             fn = getattr(L, name)
             fn.restype = C.c_int
             fn.argtypes = [_vp, C.POINTER(ckf_measurements), C.POINTER(ckf_seeds), C.POINTER(ckf_tracks), _vp]
+        L.ckf_fit.restype = C.c_int
+        L.ckf_fit.argtypes = [_vp, C.POINTER(ckf_measurements), C.POINTER(ckf_seeds), C.POINTER(ckf_tracks),
+                              C.POINTER(ckf_fits), _vp]
         L.ckf_set_timing.restype = C.c_int
         L.ckf_set_timing.argtypes = [_vp, C.c_int]
         L.ckf_get_timing.restype = C.c_int
@@ -240,6 +248,34 @@ class CKF:
         rc = self.lib.ckf_find(self.handle, C.byref(m), C.byref(s), C.byref(o), _vp(st.cuda_stream))
         if rc != 0:
             raise RuntimeError("ckf_find failed (%d): %s" % (rc, self.lib.ckf_last_error(self.handle).decode()))
+
+    # ------------------------------------------------------------------ KF fit + RTS smoother (ckf_fit)
+    def alloc_fits(self, device="cuda"):
+        t = self.torch
+        i32 = dict(dtype=t.int32, device=device)
+        T = dict(dtype=self.tdtype, device=device)
+        nt, ne = self.max_tracks, self.max_track_entries
+        return dict(status=t.zeros(nt, **i32), n_states=t.zeros(nt, **i32), chi2_sum=t.zeros(nt, **T),
+                    last_params=t.zeros(nt, 6, **T), last_cov=t.zeros(nt, 36, **T), first_cov=t.zeros(nt, 36, **T),
+                    entry_params=t.zeros(ne, 6, **T))
+
+    def fit(self, dev_event: dict, tracks: dict, fits: dict, stream=None):
+        """Asynchronous ckf_fit of the candidates in `tracks` (device tensors filled by `find`)."""
+        st = stream if stream is not None else self.torch.cuda.current_stream()
+        m, s, o = self._structs(dev_event, tracks, lambda x: x.data_ptr())
+        f = ckf_fits(*[fits[k].data_ptr() for k in ("status", "n_states", "chi2_sum", "last_params", "last_cov",
+                                                    "first_cov", "entry_params")])
+        rc = self.lib.ckf_fit(self.handle, C.byref(m), C.byref(s), C.byref(o), C.byref(f), _vp(st.cuda_stream))
+        if rc != 0:
+            raise RuntimeError("ckf_fit failed (%d): %s" % (rc, self.lib.ckf_last_error(self.handle).decode()))
+
+    def download_fits(self, fits: dict, n_tracks: int, n_entries: int) -> dict:
+        out = {}
+        for k, v in fits.items():
+            a = v.cpu().numpy()
+            a = a[:n_entries] if k == "entry_params" else a[:n_tracks]
+            out[k] = a.astype(np.float64) if a.dtype.kind == "f" else a.copy()
+        return out
 
     def find_host(self, host_event: dict, host_out: dict, stream=None):
         """ckf_find_host on (pinned) host tensors: H2D, find, D2H inside; synchronous on return."""

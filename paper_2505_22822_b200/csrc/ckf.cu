@@ -18,6 +18,7 @@
 #include "ckf_emit.cuh"
 #include "ckf_host_geom.h"
 #include "ckf_branch.cuh"
+#include "ckf_fit.cuh"
 #include "ckf_sort.cuh"
 #include "ckf_step.cuh"
 #include "ckf_visit.cuh"
@@ -78,6 +79,10 @@ struct ckf_handle {
   std::mutex mu;
   std::string err;
   std::vector<void*> allocs;
+  // state store of ckf_fit, reserved by the first call
+  double* fs_x = nullptr; void* fs_t = nullptr; int32_t* fs_meas = nullptr;
+  int fit_chunk = 0, fit_states = 0;
+  cudaEvent_t fit_done = nullptr;
   bool timing_print = false;
   bool timing = false;  // ckf_set_timing / CKF_TIMING=1: per-kernel CUDA-event times of every ckf_find on stderr (debug aid; synchronises)
 };
@@ -207,6 +212,35 @@ int launch_find(ckf_handle* h, Workspace& w, const ckf_measurements* m, const ck
       fprintf(stderr, "\n");
     }
     for (auto e : tev) cudaEventDestroy(e);
+  }
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(h, CKF_E_CUDA, "kernel launch failed: %s", cudaGetErrorString(e));
+  return CKF_OK;
+}
+
+template <typename T>
+int launch_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, const ckf_tracks* t, ckf_fits* o,
+               cudaStream_t st) {
+  FitParams<T> p;
+  p.geo.mod = h->d_mod; p.geo.layer = h->d_layer; p.geo.n_layers = h->n_layers; p.geo.n_modules = h->n_modules;
+  p.fld = h->fld;
+  p.cfg = h->kcfg;
+  p.moff = m->module_offsets;
+  p.loc = (const typename Vec2<T>::type*)m->loc;
+  p.var = (const typename Vec2<T>::type*)m->var;
+  p.seed_module = s->module_id; p.seed_x = (const T*)s->params; p.seed_C = (const T*)s->cov;
+  p.n_tracks = t->n_tracks; p.offsets = t->track_offsets; p.meas = t->meas_idx; p.seed = t->seed_id;
+  p.max_tracks = h->cfg.max_tracks;
+  p.chunk = h->fit_chunk; p.max_states = h->fit_states;
+  p.fs_x = h->fs_x; p.fs_t = (T*)h->fs_t; p.fs_meas = h->fs_meas;
+  p.o_status = o->status; p.o_nstates = o->n_states; p.o_chi2 = (T*)o->chi2_sum; p.o_lastx = (T*)o->last_params;
+  p.o_lastC = (T*)o->last_cov; p.o_firstC = (T*)o->first_cov; p.o_entryx = (T*)o->entry_params;
+  const int grid = (h->fit_chunk + FIT_NT - 1) / FIT_NT;
+  // passes of fit_chunk tracks; a pass beyond *n_tracks returns at once (the count is only known on the device)
+  for (int first = 0; first < h->cfg.max_tracks; first += h->fit_chunk) {
+    p.first = first;
+    ckf_fit_forward<T><<<grid, FIT_NT, 0, st>>>(p);
+    ckf_fit_smooth<T><<<grid, FIT_NT, 0, st>>>(p);
   }
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(h, CKF_E_CUDA, "kernel launch failed: %s", cudaGetErrorString(e));
@@ -453,6 +487,32 @@ int ckf_find_host(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, 
   return CKF_OK;
 }
 
+int ckf_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, const ckf_tracks* t, ckf_fits* o, void* stream) {
+  if (!h) return CKF_E_ARG;
+  if (!m || !s || !t || !o) return fail(h, CKF_E_ARG, "null argument");
+  if (!m->module_offsets || !t->n_tracks || !t->track_offsets || !t->meas_idx || !t->seed_id)
+    return fail(h, CKF_E_ARG, "null input array");
+  if (!o->status || !o->n_states || !o->chi2_sum || !o->last_params || !o->last_cov || !o->first_cov || !o->entry_params)
+    return fail(h, CKF_E_ARG, "null output array");
+  cudaStream_t st = (cudaStream_t)stream;
+  std::lock_guard<std::mutex> lk(h->mu);
+  if (!h->fs_x) {  // first call: reserve the state store
+    const int chunk = std::min(h->cfg.max_tracks, (int)FIT_CHUNK), ns = h->cfg.max_levels;
+    const size_t n = (size_t)ns * (size_t)chunk;
+    double* fx = nullptr; char* ft = nullptr; int32_t* fm = nullptr;
+    CK(dalloc(h, &fx, n * FS_X * sizeof(double)));
+    CK(dalloc(h, &ft, n * FS_T * (size_t)h->tsize));
+    CK(dalloc(h, &fm, n * 4));
+    CK(cudaEventCreateWithFlags(&h->fit_done, cudaEventDisableTiming));
+    h->fs_x = fx; h->fs_t = ft; h->fs_meas = fm; h->fit_chunk = chunk; h->fit_states = ns;
+  } else {
+    cudaStreamWaitEvent(st, h->fit_done, 0);  // one state store: fits are ordered one after the other
+  }
+  int rc = h->cfg.precision == 32 ? launch_fit<float>(h, m, s, t, o, st) : launch_fit<double>(h, m, s, t, o, st);
+  cudaEventRecord(h->fit_done, st);
+  return rc;
+}
+
 int ckf_get_counters(ckf_handle* h, void* stream, ckf_counters* out) {
   if (!h || !out) return CKF_E_ARG;
   cudaStream_t st = (cudaStream_t)stream;
@@ -512,6 +572,7 @@ int ckf_destroy(ckf_handle* h) {
     if (w.done) cudaEventDestroy(w.done);
     if (w.pinned_nt) cudaFreeHost(w.pinned_nt);
   }
+  if (h->fit_done) cudaEventDestroy(h->fit_done);
   for (void* p : h->allocs) cudaFree(p);
   delete h;
   return CKF_OK;

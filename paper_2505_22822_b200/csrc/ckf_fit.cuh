@@ -1,0 +1,328 @@
+// ckf_fit.cuh — Kalman-filter track fit + RTS smoother over the candidates ckf_find reported.
+//
+// the CKF's parameters are best at the LAST measurement; "a Kalman Filter-based fitting, which runs
+// a smoothing algorithm called the Rauch-Tung-Striebel (RTS) smoother, is applied additionally to the tracks to
+// make all track parameters consider all measurements".  Rules K1-K5 of DESIGN.md §3:
+//   ckf_fit_forward  thread per track: the forward filter walks the candidate's own path with the same per-tip
+//                    code as the CKF (navigation, RKN4 + Jacobian, arrival, covariance transport, Highland,
+//                    gain-form update: ckf_nav.cuh / ckf_math.cuh) and the branch choice replaced by the
+//                    candidate's list; every visited module is a STATE whose predicted / filtered parameters,
+//                    covariances and Jacobian go to the state store
+//   ckf_fit_smooth   thread per track: RTS backward recursion over the stored states, float64 arithmetic in
+//                    both modes (the gain needs the inverse of a predicted covariance whose entries span ten
+//                    orders of magnitude; PAPER.md:61, :100 report the float32 smoother as unstable)
+// State store: [state][component][track], track fastest, so the lanes of a warp (consecutive tracks) coalesce.
+#pragma once
+#include "ckf_kernels.cuh"
+
+namespace ckf {
+
+constexpr int FIT_NT = 128;
+constexpr int FIT_CHUNK = 131072;   // tracks per pass: bounds the state store (ckf.cu loops over the chunks)
+constexpr int FS_X = 12;            // float64 per state: xp[6], xf[6]
+constexpr int FS_T = 21 + 21 + 25;  // T per state: Cp, Cf (packed upper triangles), J (5x5 block, row-major)
+
+template <typename T>
+struct FitParams {
+  GeoDev geo;
+  FieldDev fld;
+  CfgDev cfg;
+  // event
+  const int32_t* moff;
+  const typename Vec2<T>::type* loc;
+  const typename Vec2<T>::type* var;
+  const int32_t* seed_module;
+  const T* seed_x;
+  const T* seed_C;
+  // candidates, as ckf_find wrote them (device)
+  const int32_t* n_tracks;
+  const int32_t* offsets;
+  const int32_t* meas;
+  const int32_t* seed;
+  int32_t max_tracks;   // capacity of the caller's per-track arrays
+  int32_t first;        // first track of this pass
+  int32_t chunk;        // tracks of this pass = stride of the state store
+  int32_t max_states;
+  double* fs_x;         // [max_states][FS_X][chunk]
+  T* fs_t;              // [max_states][FS_T][chunk]
+  int32_t* fs_meas;     // [max_states][chunk] measurement used by the state, -1 = module passed without one
+  // output (device, caller-owned)
+  int32_t* o_status; int32_t* o_nstates;
+  T* o_chi2; T* o_lastx; T* o_lastC; T* o_firstC; T* o_entryx;
+};
+
+template <typename T>
+__global__ void __launch_bounds__(FIT_NT) ckf_fit_forward(const FitParams<T> p) {
+  const int nt = min(*p.n_tracks, p.max_tracks);
+  const size_t CH = (size_t)p.chunk;
+  for (int s = blockIdx.x * FIT_NT + threadIdx.x; s < p.chunk; s += gridDim.x * FIT_NT) {
+    const int tr = p.first + s;
+    if (tr >= nt) return;
+    const int e0 = p.offsets[tr], n = p.offsets[tr + 1] - e0, sd = p.seed[tr];
+    double x[6], xf[6];
+    T C[21], Cf[21];
+    bool ok = true;
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+      x[i] = (double)p.seed_x[(size_t)sd * 6 + i];
+      xf[i] = 0.0;
+      ok = ok && isfinite(x[i]);
+    }
+    ok = ok && (x[3] > 0.0 && x[3] < PI_D);
+#pragma unroll
+    for (int i = 0; i < 6; ++i)
+#pragma unroll
+      for (int j = i; j < 6; ++j) { C[tri(i, j)] = p.seed_C[(size_t)sd * 36 + i * 6 + j]; Cf[tri(i, j)] = T(0); }
+    int module = p.seed_module[sd], next = 0, status = STOP_NONE, ns = 0;
+    T c2sum = T(0);
+    for (int level = 0; n > 0; ++level) {
+      if (level >= p.cfg.max_levels || level >= p.max_states) { status = STOP_LEVEL_LIMIT; break; }
+      double xp[6];
+      T Cp[21], J[5][5];
+      if (level == 0) {  // N6: the seed's own module, identity transport
+        if (!ok) { status = STOP_NUMERIC; break; }
+#pragma unroll
+        for (int i = 0; i < 6; ++i) xp[i] = x[i];
+#pragma unroll
+        for (int i = 0; i < 21; ++i) Cp[i] = C[i];
+#pragma unroll
+        for (int a = 0; a < 5; ++a)
+#pragma unroll
+          for (int b = 0; b < 5; ++b) J[a][b] = (a == b && a < 4) ? T(1) : T(0);
+      } else {
+        int tg = -1;
+        T qphi, qth;
+        StepCtl sc;
+        sc.n_trials = 0; sc.n_accepted = 0;
+        status = move_to_next_module<T>(p.geo, p.fld, p.cfg, module, x, tg, xp, J, qphi, qth, sc);
+        if (status != STOP_NONE) break;
+        C[tri(2, 2)] += qphi;  // V5 on leaving
+        C[tri(3, 3)] += qth;
+        transport_cov<T>(J, C, Cp);
+        bool fin = true;
+#pragma unroll
+        for (int i = 0; i < 21; ++i) fin = fin && isfinite(Cp[i]);
+        if (!fin) { status = STOP_NUMERIC; break; }
+        module = tg;
+      }
+      const int k = p.meas[e0 + next];
+      int used = -1;
+      if (k >= p.moff[module] && k < p.moff[module + 1]) {
+        const typename Vec2<T>::type m = p.loc[k], v = p.var[k];
+        const double c2 = predicted_chi2<double>(xp[0], xp[1], (double)Cp[tri(0, 0)], (double)Cp[tri(0, 1)],
+                                                 (double)Cp[tri(1, 1)], (double)m.x, (double)m.y, (double)v.x, (double)v.y);
+        c2sum += (T)c2;
+        kalman_update<T>(xp, Cp, m.x, m.y, v.x, v.y, xf, Cf);
+        used = k;
+        ++next;
+      } else {
+#pragma unroll
+        for (int i = 0; i < 6; ++i) xf[i] = xp[i];
+#pragma unroll
+        for (int i = 0; i < 21; ++i) Cf[i] = Cp[i];
+      }
+      double* fx = p.fs_x + (size_t)level * FS_X * CH + s;
+      T* ft = p.fs_t + (size_t)level * FS_T * CH + s;
+#pragma unroll
+      for (int i = 0; i < 6; ++i) { fx[i * CH] = xp[i]; fx[(6 + i) * CH] = xf[i]; }
+#pragma unroll
+      for (int i = 0; i < 21; ++i) { ft[i * CH] = Cp[i]; ft[(21 + i) * CH] = Cf[i]; }
+#pragma unroll
+      for (int a = 0; a < 5; ++a)
+#pragma unroll
+        for (int b = 0; b < 5; ++b) ft[(42 + a * 5 + b) * CH] = J[a][b];
+      p.fs_meas[(size_t)level * CH + s] = used;
+      ns = level + 1;
+      if (next == n) break;
+#pragma unroll
+      for (int i = 0; i < 6; ++i) x[i] = xf[i];
+#pragma unroll
+      for (int i = 0; i < 21; ++i) C[i] = Cf[i];
+    }
+    p.o_status[tr] = status;
+    p.o_nstates[tr] = ns;
+    const bool good = status == STOP_NONE && ns > 0;
+    p.o_chi2[tr] = good ? c2sum : T(0);
+#pragma unroll
+    for (int i = 0; i < 6; ++i) p.o_lastx[(size_t)tr * 6 + i] = good ? (T)xf[i] : T(0);
+#pragma unroll
+    for (int i = 0; i < 6; ++i)
+#pragma unroll
+      for (int j = 0; j < 6; ++j) p.o_lastC[(size_t)tr * 36 + i * 6 + j] = good ? Cf[tri(i, j)] : T(0);
+  }
+}
+
+// K4 helper: X = G^-1 B for a symmetric positive definite 6x6 G: scale to unit diagonal, Cholesky, two
+// triangular solves per column.  false when G is not positive definite.
+__device__ __forceinline__ bool spd_solve6(const double G[6][6], const double B[6][6], double X[6][6]) {
+  double s[6], L[6][6];
+#pragma unroll
+  for (int i = 0; i < 6; ++i) {
+    if (!(G[i][i] > 0.0)) return false;
+    s[i] = 1.0 / sqrt(G[i][i]);
+  }
+#pragma unroll
+  for (int j = 0; j < 6; ++j) {
+    double d = G[j][j] * s[j] * s[j];
+#pragma unroll
+    for (int k = 0; k < j; ++k) d -= L[j][k] * L[j][k];
+    if (!(d > 0.0)) return false;
+    L[j][j] = sqrt(d);
+#pragma unroll
+    for (int i = j + 1; i < 6; ++i) {
+      double v = G[i][j] * s[i] * s[j];
+#pragma unroll
+      for (int k = 0; k < j; ++k) v -= L[i][k] * L[j][k];
+      L[i][j] = v / L[j][j];
+    }
+  }
+#pragma unroll 1
+  for (int c = 0; c < 6; ++c) {
+    double z[6], w[6];
+#pragma unroll
+    for (int i = 0; i < 6; ++i) {
+      double v = B[i][c] * s[i];
+#pragma unroll
+      for (int k = 0; k < i; ++k) v -= L[i][k] * z[k];
+      z[i] = v / L[i][i];
+    }
+#pragma unroll
+    for (int i = 5; i >= 0; --i) {
+      double v = z[i];
+#pragma unroll
+      for (int k = i + 1; k < 6; ++k) v -= L[k][i] * w[k];
+      w[i] = v / L[i][i];
+    }
+#pragma unroll
+    for (int i = 0; i < 6; ++i) X[i][c] = w[i] * s[i];
+  }
+  return true;
+}
+
+__device__ __forceinline__ double wrap_pi(double a) {
+  while (a > PI_D) a -= 2.0 * PI_D;
+  while (a <= -PI_D) a += 2.0 * PI_D;
+  return a;
+}
+
+// packed upper triangle (T) of state `k` at component offset `c0` -> dense symmetric float64
+template <typename T>
+__device__ __forceinline__ void load_sym(const T* ft, size_t CH, int c0, double M[6][6]) {
+#pragma unroll
+  for (int i = 0; i < 6; ++i)
+#pragma unroll
+    for (int j = i; j < 6; ++j) {
+      const double v = (double)ft[(size_t)(c0 + tri(i, j)) * CH];
+      M[i][j] = v;
+      M[j][i] = v;
+    }
+}
+
+template <typename T>
+__global__ void __launch_bounds__(FIT_NT) ckf_fit_smooth(const FitParams<T> p) {
+  const int nt = min(*p.n_tracks, p.max_tracks);
+  const size_t CH = (size_t)p.chunk;
+  for (int s = blockIdx.x * FIT_NT + threadIdx.x; s < p.chunk; s += gridDim.x * FIT_NT) {
+    const int tr = p.first + s;
+    if (tr >= nt) return;
+    const int e0 = p.offsets[tr], n = p.offsets[tr + 1] - e0;
+    const int ns = p.o_nstates[tr];
+    bool good = p.o_status[tr] == STOP_NONE && ns > 0;
+    double xs[6], Cs[6][6];
+    int e = n - 1;  // entries are filled from the back: the forward pass ends on the last measurement
+    if (good) {
+      const double* fx = p.fs_x + (size_t)(ns - 1) * FS_X * CH + s;
+      const T* ft = p.fs_t + (size_t)(ns - 1) * FS_T * CH + s;
+#pragma unroll
+      for (int i = 0; i < 6; ++i) xs[i] = fx[(6 + i) * CH];
+      load_sym<T>(ft, CH, 21, Cs);
+      for (int k = ns - 1;; --k) {
+        if (p.fs_meas[(size_t)k * CH + s] >= 0) {
+#pragma unroll
+          for (int i = 0; i < 6; ++i) p.o_entryx[(size_t)(e0 + e) * 6 + i] = (T)xs[i];
+          if (e == 0) {  // first measurement of the track: the state PAPER.md:35 wants improved
+#pragma unroll
+            for (int i = 0; i < 6; ++i)
+#pragma unroll
+              for (int j = 0; j < 6; ++j) p.o_firstC[(size_t)tr * 36 + i * 6 + j] = (T)Cs[i][j];
+          }
+          --e;
+        }
+        if (k == 0 || e < 0) break;  // states before the first measurement are not reported
+        // ---- one RTS step: state k -> k - 1.  b = state k (xp, Cp, J), a = state k - 1 (xf, Cf)
+        const double* bx = p.fs_x + (size_t)k * FS_X * CH + s;
+        const T* bt = p.fs_t + (size_t)k * FS_T * CH + s;
+        const double* ax = p.fs_x + (size_t)(k - 1) * FS_X * CH + s;
+        const T* at = p.fs_t + (size_t)(k - 1) * FS_T * CH + s;
+        double G[6][6], Cfa[6][6], M[6][6], X[6][6];
+        load_sym<T>(bt, CH, 0, G);
+        load_sym<T>(at, CH, 21, Cfa);
+        // M = Jf Cf[k-1], Jf rows 0..3 = J[0..3] over columns 0..4, row 4 = e_4, row 5 = J[4] plus 1 at column 5
+#pragma unroll
+        for (int i = 0; i < 6; ++i) {
+          if (i == 4) {
+#pragma unroll
+            for (int j = 0; j < 6; ++j) M[4][j] = Cfa[4][j];
+          } else {
+            const int r = (i == 5) ? 4 : i;
+            double Jr[5];
+#pragma unroll
+            for (int l = 0; l < 5; ++l) Jr[l] = (double)bt[(size_t)(42 + r * 5 + l) * CH];
+#pragma unroll
+            for (int j = 0; j < 6; ++j) {
+              double v = (i == 5) ? Cfa[5][j] : 0.0;
+#pragma unroll
+              for (int l = 0; l < 5; ++l) v += Jr[l] * Cfa[l][j];
+              M[i][j] = v;
+            }
+          }
+        }
+        if (!spd_solve6(G, M, X)) { good = false; break; }  // X = Cp^-1 J Cf = A^T
+        double dx[6];
+#pragma unroll
+        for (int i = 0; i < 6; ++i) dx[i] = xs[i] - bx[i * CH];
+        dx[2] = wrap_pi(dx[2]);
+#pragma unroll
+        for (int i = 0; i < 6; ++i) {
+          double v = 0.0;
+#pragma unroll
+          for (int j = 0; j < 6; ++j) v += X[j][i] * dx[j];
+          xs[i] = ax[(6 + i) * CH] + v;
+        }
+        xs[2] = wrap_pi(xs[2]);
+        double Tm[6][6];
+#pragma unroll
+        for (int i = 0; i < 6; ++i)
+#pragma unroll
+          for (int j = 0; j < 6; ++j) {
+            double v = 0.0;
+#pragma unroll
+            for (int l = 0; l < 6; ++l) v += (Cs[i][l] - G[i][l]) * X[l][j];
+            Tm[i][j] = v;
+          }
+#pragma unroll
+        for (int i = 0; i < 6; ++i)
+#pragma unroll
+          for (int j = 0; j < 6; ++j) {
+            double v = 0.0;
+#pragma unroll
+            for (int l = 0; l < 6; ++l) v += X[l][i] * Tm[l][j];
+            M[i][j] = Cfa[i][j] + v;
+          }
+#pragma unroll
+        for (int i = 0; i < 6; ++i)
+#pragma unroll
+          for (int j = 0; j < 6; ++j) Cs[i][j] = 0.5 * (M[i][j] + M[j][i]);
+      }
+    }
+    if (!good) {
+      if (p.o_status[tr] == STOP_NONE && ns > 0) p.o_status[tr] = STOP_NUMERIC;  // a predicted covariance was not positive definite
+      p.o_chi2[tr] = T(0);
+      for (int i = 0; i < 6; ++i) p.o_lastx[(size_t)tr * 6 + i] = T(0);
+      for (int i = 0; i < 36; ++i) { p.o_lastC[(size_t)tr * 36 + i] = T(0); p.o_firstC[(size_t)tr * 36 + i] = T(0); }
+      for (int i = 0; i < 6 * n; ++i) p.o_entryx[(size_t)e0 * 6 + i] = T(0);
+    }
+  }
+}
+
+}  // namespace ckf

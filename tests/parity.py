@@ -10,6 +10,7 @@ def param_rel_diff(a, b):
     d = a - b
     d[..., 2] = (d[..., 2] + np.pi) % (2 * np.pi) - np.pi
     den = np.maximum(np.maximum(np.abs(a), np.abs(b)), FLOOR)
+    den = np.where(den == 0.0, 1.0, den)     # both exactly zero (q/p has no floor): difference 0
     return np.abs(d) / den
 
 
@@ -66,3 +67,25 @@ def compare_fp32(gpu, ora, n_seeds):
                 max_param_rel=float(rel.max(initial=0.0)), max_chi2_sum_abs=float(chi2.max(initial=0.0)),
                 max_entry_chi2_abs=emax,
                 table1=[float(np.mean(rel.max(axis=1) <= tol)) if gi.size else 1.0 for tol in (1e-4, 1e-3, 1e-2, 5e-2)])
+
+
+def compare_fits(gpu: dict, ora, track_offsets):
+    """CUDA ckf_fit (dict of arrays from CKF.download_fits) against oracle.kf_fit on the SAME candidate lists.
+    Integer results must be equal; returns the maximum A15 relative differences of the forward state at the last
+    measurement and of the smoothed parameters, the scaled covariance difference at the first measurement, and the
+    Table-1-style matching ratios of the smoothed parameters (fitted parameters at 0.01/0.1/1/5 %)."""
+    assert np.array_equal(gpu["status"], ora.status), np.flatnonzero(gpu["status"] != ora.status)[:10]
+    assert np.array_equal(gpu["n_states"], ora.n_states)
+    ok = ora.status == 0
+    last = param_rel_diff(gpu["last_params"][ok].copy(), ora.last_params[ok].copy())
+    ent = param_rel_diff(gpu["entry_params"].copy(), ora.entry_params.copy())
+    scale = np.sqrt(np.abs(ora.first_cov[:, [0, 7, 14, 21, 28, 35]]))
+    sc = (scale[:, :, None] * scale[:, None, :]).reshape(-1, 36)
+    cov = (np.abs(gpu["first_cov"] - ora.first_cov) / np.maximum(sc, 1e-300))[ok]
+    first = track_offsets[:-1][ok]
+    rel_first = ent[first].max(axis=1) if first.size else np.zeros(0)
+    return dict(n_fitted=int(ok.sum()), n_failed=int((~ok).sum()),
+                max_last_rel=float(last.max(initial=0.0)), max_smoothed_rel=float(ent.max(initial=0.0)),
+                max_first_cov_scaled=float(cov.max(initial=0.0)),
+                max_chi2_abs=float(np.abs(gpu["chi2_sum"] - ora.chi2_sum).max(initial=0.0)),
+                table1_first=[float(np.mean(rel_first <= tol)) if first.size else 1.0 for tol in (1e-4, 1e-3, 1e-2, 5e-2)])

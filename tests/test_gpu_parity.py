@@ -238,3 +238,83 @@ def test_timing_abi_reports_every_phase():
     ckf.set_timing(False)
     assert t["launches"] > 0 and t["step_ms"] > 0 and t["visit_ms"] > 0 and t["update_ms"] > 0 and t["scan_ms"] > 0
     ckf.close()
+
+
+# ---------------------------------------------------------------------------------- KF fit + RTS smoother (ckf_fit)
+def _fit_both(config, n_particles=None):
+    import torch
+    import oracle
+    det, fld, cfg = synth.config_bundle(config)
+    ev = synth.make_event(config, det=det, n_particles=n_particles)
+    ckf, dev, out, gpu, _ = _run_gpu(det, fld, cfg, ev)
+    fits = ckf.alloc_fits()
+    ckf.fit(dev, out, fits)
+    torch.cuda.synchronize()
+    ne = int(gpu.meas_idx.size)
+    g = ckf.download_fits(fits, gpu.n_tracks, ne)
+    # the oracle fits the SAME candidate lists (the CUDA path's), so this compares the fit alone
+    st = oracle.Setup(det, fld, cfg.ckf)
+    o = oracle.kf_fit(st, ev, gpu.track_offsets, gpu.meas_idx, gpu.seed_id, n_threads=16)
+    r = parity.compare_fits(g, o, gpu.track_offsets)
+    return ckf, dev, out, fits, gpu, g, o, r
+
+
+@pytest.mark.parametrize("config", [0, 1])
+def test_fit_fp64_parity(config):
+    ckf, dev, out, fits, gpu, g, o, r = _fit_both(config)
+    print("fit config", config, r)
+    assert r["n_fitted"] == gpu.n_tracks and gpu.n_tracks > 0
+    assert r["max_last_rel"] < 1e-9 and r["max_chi2_abs"] < 1e-8
+    assert r["max_smoothed_rel"] < 1e-9, r        # same bar as the CKF parameters (north_star, fp64)
+    assert r["max_first_cov_scaled"] < 1e-6, r
+    # K2: the forward pass ends on the state the CKF reported for the candidate
+    assert np.max(parity.param_rel_diff(g["last_params"].copy(), gpu.params.copy())) < 1e-12
+    # determinism
+    import torch
+    fits2 = ckf.alloc_fits()
+    ckf.fit(dev, out, fits2)
+    torch.cuda.synchronize()
+    n = gpu.n_tracks
+    for k in fits:
+        m = int(gpu.meas_idx.size) if k == "entry_params" else n
+        assert torch.equal(fits[k][:m], fits2[k][:m]), k
+    ckf.close()
+
+
+@pytest.mark.parametrize("config", [2, 3])
+def test_fit_fp32_parity(config):
+    ckf, dev, out, fits, gpu, g, o, r = _fit_both(config)
+    print("fit config", config, r)
+    assert r["n_fitted"] >= 0.999 * gpu.n_tracks
+    assert r["max_last_rel"] < 1e-4 and r["max_chi2_abs"] < 1e-3      # north_star's fp32 bar for parameters / chi2
+    assert r["max_smoothed_rel"] < 1e-4, r
+    assert r["table1_first"][0] == 1.0, r
+    ckf.close()
+
+
+def test_fit_incomplete_list_is_flagged_not_fitted():
+    """A list the path cannot reach (a measurement of a module the track never crosses) ends with the forward
+    pass's stop reason and zeros, on both sides."""
+    import torch
+    import oracle
+    det, fld, cfg = synth.config_bundle(1)
+    ev = synth.make_event(1, det=det, n_particles=50)
+    ckf, dev, out, gpu, _ = _run_gpu(det, fld, cfg, ev)
+    assert gpu.n_tracks > 5
+    # corrupt track 2: its last entry becomes a measurement from a far-away module
+    e = int(gpu.track_offsets[3]) - 1
+    far = int(ev.module_offsets[det.n_modules] - 1)
+    assert far != int(gpu.meas_idx[e])
+    out["meas_idx"][e] = far
+    fits = ckf.alloc_fits()
+    ckf.fit(dev, out, fits)
+    torch.cuda.synchronize()
+    g = ckf.download_fits(fits, gpu.n_tracks, int(gpu.meas_idx.size))
+    mi = gpu.meas_idx.copy()
+    mi[e] = far
+    o = oracle.kf_fit(oracle.Setup(det, fld, cfg.ckf), ev, gpu.track_offsets, mi, gpu.seed_id, n_threads=4)
+    assert o.status[2] != 0 and g["status"][2] == o.status[2]
+    assert not g["entry_params"][gpu.track_offsets[2]:gpu.track_offsets[3]].any()
+    r = parity.compare_fits(g, o, gpu.track_offsets)
+    assert r["n_failed"] >= 1 and r["max_smoothed_rel"] < 1e-9
+    ckf.close()
