@@ -38,6 +38,7 @@ F_NAV = 600             # navigation of one visit (ckf_step): ~1.7 module choice
 F_VISIT = 1450          # navigation 600 + arrival Jacobian, covariance transport, bound parameters 850
 F_GATE = 17             # one chi2 actually evaluated (inside a loc0 window)
 F_UPDATE = 155          # one gain-form update
+F_RTS = 1950            # one RTS step (ckf_fit_smooth): J Cf 300, scaled Cholesky 150, 6 column solves 430, gain products 1070
 # plain-ALU peaks from the guide's unit counts: 148 SMs x 128 FP32 (64 FP64) lanes x 2 flop x 1.965 GHz
 PEAK_FP32_TFLOPS = 148 * 128 * 2 * 1.965e9 / 1e12
 PEAK_FP64_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12
@@ -237,6 +238,23 @@ def main():
         torch.cuda.synchronize()
         tim.append(ckf.timing(stream))
     ckf.set_timing(False)
+    # ---- next row: KF fit + RTS smoother of that event's candidates (ckf_fit)
+    fits = ckf.alloc_fits()
+    dev_last = devs[(W - 1) % N_EVENTS]
+    for _ in range(2):
+        ckf.fit(dev_last, out, fits, stream)
+    torch.cuda.synchronize()
+    n_fit = 5
+    fa, fb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    fa.record(stream)
+    for _ in range(n_fit):
+        ckf.fit(dev_last, out, fits, stream)
+    fb.record(stream)
+    torch.cuda.synchronize()
+    fit_ms = fa.elapsed_time(fb) / n_fit
+    fit_ok = int((fits["status"][:res.n_tracks] == 0).sum().item())
+    fit_work = [int(v) // (n_fit + 2) for v in fits["work"].cpu().tolist()]   # trials, accepted, moves, updates per call
+    fit_states = int(fits["n_states"][:res.n_tracks].sum().item())
     clocks = sampler.stop()
     launches_per_find = int(tim[0]["launches"])
 
@@ -286,6 +304,8 @@ def main():
         f64_share = step64 / step_flop if cfg.precision == 32 else 1.0
         peak = 1.0 / (f64_share / PEAK_FP64_TFLOPS + (1.0 - f64_share) / PEAK_FP32_TFLOPS)
         step_launches = sum(1 for _ in range(cfg.ckf.max_levels))
+        fit_flop = float(fit_work[0] * f_trial + fit_work[1] * F_ACCEPT + fit_work[2] * F_VISIT + fit_work[3] * F_UPDATE +
+                         max(fit_states - res.n_tracks, 0) * F_RTS)
         line = {
             "metric": "CKF seeds/sec (40k-particle event)", "value": value, "unit": "seeds/s", "n_gpus": world,
             "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms_step, "higher_is_better": True,
@@ -302,6 +322,13 @@ def main():
             "e2e": {"value": e2e_value, "unit": "seeds/s", "h2d_bytes_per_step": int(bi), "d2h_bytes_per_step": int(bo),
                     "streams": E2E_STREAMS, "events": n_e2e, "events_per_s": e2e_value / ev_last.n_seeds,
                     "how": "ckf_find_host, pinned host buffers, 4 host threads x 4 CUDA streams, wall clock"},
+            "fit": {"what": "ckf_fit: Kalman-filter fit + RTS smoother of every candidate of one configs[3] event "
+                            "(next row, SURVEY.md 8(f) rank 1); device-resident, CUDA events, mean of 5",
+                    "value": res.n_tracks / (fit_ms * 1e-3), "unit": "tracks/s", "ms_per_event": fit_ms,
+                    "tracks": res.n_tracks, "fitted": fit_ok, "entries": int(res.meas_idx.size),
+                    "work": dict(zip(("rk_trials", "rk_accepted", "moves", "updates"), fit_work)), "states": fit_states,
+                    "flop_per_event": fit_flop, "achieved_tflops": fit_flop / (fit_ms * 1e-3) / 1e12,
+                    "launches": "2 kernels (forward filter, RTS smoother) per pass of 131,072 candidates"},
             "gpu_launches": launches_per_find * args.steps,
             "clocks": clocks,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,

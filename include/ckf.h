@@ -194,6 +194,8 @@ typedef struct {
   void* first_cov;      /* T[max_tracks][36] SMOOTHED covariance at the first measurement                     */
   void* entry_params;   /* T[max_track_entries][6] SMOOTHED parameters at every measurement, parallel to
                            ckf_tracks.meas_idx (entry track_offsets[t] is the first measurement of track t)  */
+  int64_t* work;        /* [4] or NULL: the call ADDS its RKN4 trials, accepted steps, module-to-module moves and
+                           Kalman updates here (zero it before the call; roofline accounting)    */
 } ckf_fits;
 
 /* Fits every candidate of `tracks` (the DEVICE arrays a ckf_find on the same measurements and seeds filled;

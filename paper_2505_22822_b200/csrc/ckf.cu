@@ -235,6 +235,7 @@ int launch_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, con
   p.fs_x = h->fs_x; p.fs_t = (T*)h->fs_t; p.fs_meas = h->fs_meas;
   p.o_status = o->status; p.o_nstates = o->n_states; p.o_chi2 = (T*)o->chi2_sum; p.o_lastx = (T*)o->last_params;
   p.o_lastC = (T*)o->last_cov; p.o_firstC = (T*)o->first_cov; p.o_entryx = (T*)o->entry_params;
+  p.o_work = (unsigned long long*)o->work;
   const int grid = (h->fit_chunk + FIT_NT - 1) / FIT_NT;
   // passes of fit_chunk tracks; a pass beyond *n_tracks returns at once (the count is only known on the device)
   for (int first = 0; first < h->cfg.max_tracks; first += h->fit_chunk) {

@@ -49,15 +49,17 @@ struct FitParams {
   // output (device, caller-owned)
   int32_t* o_status; int32_t* o_nstates;
   T* o_chi2; T* o_lastx; T* o_lastC; T* o_firstC; T* o_entryx;
+  unsigned long long* o_work;  // [4] or null: RKN4 trials, accepted steps, moves, updates are ADDED here
 };
 
 template <typename T>
 __global__ void __launch_bounds__(FIT_NT) ckf_fit_forward(const FitParams<T> p) {
   const int nt = min(*p.n_tracks, p.max_tracks);
   const size_t CH = (size_t)p.chunk;
+  unsigned long long w_trials = 0, w_acc = 0, w_moves = 0, w_upd = 0;
   for (int s = blockIdx.x * FIT_NT + threadIdx.x; s < p.chunk; s += gridDim.x * FIT_NT) {
     const int tr = p.first + s;
-    if (tr >= nt) return;
+    if (tr >= nt) break;
     const int e0 = p.offsets[tr], n = p.offsets[tr + 1] - e0, sd = p.seed[tr];
     double x[6], xf[6];
     T C[21], Cf[21];
@@ -95,6 +97,7 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_forward(const FitParams<T> p) 
         StepCtl sc;
         sc.n_trials = 0; sc.n_accepted = 0;
         status = move_to_next_module<T>(p.geo, p.fld, p.cfg, module, x, tg, xp, J, qphi, qth, sc);
+        w_trials += sc.n_trials; w_acc += sc.n_accepted; w_moves += 1;
         if (status != STOP_NONE) break;
         C[tri(2, 2)] += qphi;  // V5 on leaving
         C[tri(3, 3)] += qth;
@@ -115,6 +118,7 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_forward(const FitParams<T> p) 
         kalman_update<T>(xp, Cp, m.x, m.y, v.x, v.y, xf, Cf);
         used = k;
         ++next;
+        w_upd += 1;
       } else {
 #pragma unroll
         for (int i = 0; i < 6; ++i) xf[i] = xp[i];
@@ -149,6 +153,13 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_forward(const FitParams<T> p) 
     for (int i = 0; i < 6; ++i)
 #pragma unroll
       for (int j = 0; j < 6; ++j) p.o_lastC[(size_t)tr * 36 + i * 6 + j] = good ? Cf[tri(i, j)] : T(0);
+  }
+  if (p.o_work) {
+    __syncwarp();
+    flush_counter(p.o_work + 0, w_trials);
+    flush_counter(p.o_work + 1, w_acc);
+    flush_counter(p.o_work + 2, w_moves);
+    flush_counter(p.o_work + 3, w_upd);
   }
 }
 

@@ -278,6 +278,9 @@ def test_fit_fp64_parity(config):
     for k in fits:
         m = int(gpu.meas_idx.size) if k == "entry_params" else n
         assert torch.equal(fits[k][:m], fits2[k][:m]), k
+    # work counters: one update per entry, one move per state after the first
+    w = g["work"]
+    assert w[3] == gpu.meas_idx.size and w[2] == int(g["n_states"].sum()) - n and w[0] >= w[1] > 0
     ckf.close()
 
 
