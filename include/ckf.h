@@ -196,6 +196,9 @@ typedef struct {
                            ckf_tracks.meas_idx (entry track_offsets[t] is the first measurement of track t)  */
   int64_t* work;        /* [4] or NULL: the call ADDS its RKN4 trials, accepted steps, module-to-module moves and
                            Kalman updates here (zero it before the call; roofline accounting)    */
+  int32_t smoother_precision; /* INPUT.  0 or 64: the RTS recursion runs in float64 (the product's choice, K5).
+                           32 (handles of precision 32 only): it runs in float32 -- kept to study the instability
+                           of the float32 smoother that PAPER.md:61, :100 report, not for production             */
 } ckf_fits;
 
 /* Fits every candidate of `tracks` (the DEVICE arrays a ckf_find on the same measurements and seeds filled;

@@ -241,7 +241,8 @@ int launch_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, con
   for (int first = 0; first < h->cfg.max_tracks; first += h->fit_chunk) {
     p.first = first;
     ckf_fit_forward<T><<<grid, FIT_NT, 0, st>>>(p);
-    ckf_fit_smooth<T><<<grid, FIT_NT, 0, st>>>(p);
+    if (sizeof(T) == 4 && o->smoother_precision == 32) ckf_fit_smooth<T, float><<<grid, FIT_NT, 0, st>>>(p);
+    else ckf_fit_smooth<T, double><<<grid, FIT_NT, 0, st>>>(p);
   }
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(h, CKF_E_CUDA, "kernel launch failed: %s", cudaGetErrorString(e));
@@ -493,6 +494,10 @@ int ckf_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, const 
   if (!m || !s || !t || !o) return fail(h, CKF_E_ARG, "null argument");
   if (!m->module_offsets || !t->n_tracks || !t->track_offsets || !t->meas_idx || !t->seed_id)
     return fail(h, CKF_E_ARG, "null input array");
+  if (o->smoother_precision != 0 && o->smoother_precision != 32 && o->smoother_precision != 64)
+    return fail(h, CKF_E_ARG, "smoother_precision must be 0, 32 or 64");
+  if (o->smoother_precision == 32 && h->cfg.precision != 32)
+    return fail(h, CKF_E_ARG, "smoother_precision 32 needs a handle of precision 32");
   if (!o->status || !o->n_states || !o->chi2_sum || !o->last_params || !o->last_cov || !o->first_cov || !o->entry_params)
     return fail(h, CKF_E_ARG, "null output array");
   cudaStream_t st = (cudaStream_t)stream;

@@ -165,23 +165,24 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_forward(const FitParams<T> p) 
 
 // K4 helper: X = G^-1 B for a symmetric positive definite 6x6 G: scale to unit diagonal, Cholesky, two
 // triangular solves per column.  false when G is not positive definite.
-__device__ __forceinline__ bool spd_solve6(const double G[6][6], const double B[6][6], double X[6][6]) {
-  double s[6], L[6][6];
+template <typename A>
+__device__ __forceinline__ bool spd_solve6(const A G[6][6], const A B[6][6], A X[6][6]) {
+  A s[6], L[6][6];
 #pragma unroll
   for (int i = 0; i < 6; ++i) {
-    if (!(G[i][i] > 0.0)) return false;
-    s[i] = 1.0 / sqrt(G[i][i]);
+    if (!(G[i][i] > A(0))) return false;
+    s[i] = A(1) / sqrt(G[i][i]);
   }
 #pragma unroll
   for (int j = 0; j < 6; ++j) {
-    double d = G[j][j] * s[j] * s[j];
+    A d = G[j][j] * s[j] * s[j];
 #pragma unroll
     for (int k = 0; k < j; ++k) d -= L[j][k] * L[j][k];
-    if (!(d > 0.0)) return false;
+    if (!(d > A(0))) return false;
     L[j][j] = sqrt(d);
 #pragma unroll
     for (int i = j + 1; i < 6; ++i) {
-      double v = G[i][j] * s[i] * s[j];
+      A v = G[i][j] * s[i] * s[j];
 #pragma unroll
       for (int k = 0; k < j; ++k) v -= L[i][k] * L[j][k];
       L[i][j] = v / L[j][j];
@@ -189,17 +190,17 @@ __device__ __forceinline__ bool spd_solve6(const double G[6][6], const double B[
   }
 #pragma unroll 1
   for (int c = 0; c < 6; ++c) {
-    double z[6], w[6];
+    A z[6], w[6];
 #pragma unroll
     for (int i = 0; i < 6; ++i) {
-      double v = B[i][c] * s[i];
+      A v = B[i][c] * s[i];
 #pragma unroll
       for (int k = 0; k < i; ++k) v -= L[i][k] * z[k];
       z[i] = v / L[i][i];
     }
 #pragma unroll
     for (int i = 5; i >= 0; --i) {
-      double v = z[i];
+      A v = z[i];
 #pragma unroll
       for (int k = i + 1; k < 6; ++k) v -= L[k][i] * w[k];
       w[i] = v / L[i][i];
@@ -210,26 +211,29 @@ __device__ __forceinline__ bool spd_solve6(const double G[6][6], const double B[
   return true;
 }
 
-__device__ __forceinline__ double wrap_pi(double a) {
-  while (a > PI_D) a -= 2.0 * PI_D;
-  while (a <= -PI_D) a += 2.0 * PI_D;
+template <typename A>
+__device__ __forceinline__ A wrap_pi(A a) {
+  while (a > (A)PI_D) a -= (A)(2.0 * PI_D);
+  while (a <= -(A)PI_D) a += (A)(2.0 * PI_D);
   return a;
 }
 
-// packed upper triangle (T) of state `k` at component offset `c0` -> dense symmetric float64
-template <typename T>
-__device__ __forceinline__ void load_sym(const T* ft, size_t CH, int c0, double M[6][6]) {
+// packed upper triangle (T) of a state at component offset `c0` -> dense symmetric matrix of the arithmetic type
+template <typename T, typename A>
+__device__ __forceinline__ void load_sym(const T* ft, size_t CH, int c0, A M[6][6]) {
 #pragma unroll
   for (int i = 0; i < 6; ++i)
 #pragma unroll
     for (int j = i; j < 6; ++j) {
-      const double v = (double)ft[(size_t)(c0 + tri(i, j)) * CH];
+      const A v = (A)ft[(size_t)(c0 + tri(i, j)) * CH];
       M[i][j] = v;
       M[j][i] = v;
     }
 }
 
-template <typename T>
+// A = arithmetic type of the recursion: double (the product's choice, K5), or float for the study of the float32
+// smoother's instability that PAPER.md:61, :100 report (fp32 mode only).
+template <typename T, typename A>
 __global__ void __launch_bounds__(FIT_NT) ckf_fit_smooth(const FitParams<T> p) {
   const int nt = min(*p.n_tracks, p.max_tracks);
   const size_t CH = (size_t)p.chunk;
@@ -239,14 +243,14 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_smooth(const FitParams<T> p) {
     const int e0 = p.offsets[tr], n = p.offsets[tr + 1] - e0;
     const int ns = p.o_nstates[tr];
     bool good = p.o_status[tr] == STOP_NONE && ns > 0;
-    double xs[6], Cs[6][6];
+    A xs[6], Cs[6][6];
     int e = n - 1;  // entries are filled from the back: the forward pass ends on the last measurement
     if (good) {
       const double* fx = p.fs_x + (size_t)(ns - 1) * FS_X * CH + s;
       const T* ft = p.fs_t + (size_t)(ns - 1) * FS_T * CH + s;
 #pragma unroll
-      for (int i = 0; i < 6; ++i) xs[i] = fx[(6 + i) * CH];
-      load_sym<T>(ft, CH, 21, Cs);
+      for (int i = 0; i < 6; ++i) xs[i] = (A)fx[(6 + i) * CH];
+      load_sym<T, A>(ft, CH, 21, Cs);
       for (int k = ns - 1;; --k) {
         if (p.fs_meas[(size_t)k * CH + s] >= 0) {
 #pragma unroll
@@ -265,9 +269,9 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_smooth(const FitParams<T> p) {
         const T* bt = p.fs_t + (size_t)k * FS_T * CH + s;
         const double* ax = p.fs_x + (size_t)(k - 1) * FS_X * CH + s;
         const T* at = p.fs_t + (size_t)(k - 1) * FS_T * CH + s;
-        double G[6][6], Cfa[6][6], M[6][6], X[6][6];
-        load_sym<T>(bt, CH, 0, G);
-        load_sym<T>(at, CH, 21, Cfa);
+        A G[6][6], Cfa[6][6], M[6][6], X[6][6];
+        load_sym<T, A>(bt, CH, 0, G);
+        load_sym<T, A>(at, CH, 21, Cfa);
         // M = Jf Cf[k-1], Jf rows 0..3 = J[0..3] over columns 0..4, row 4 = e_4, row 5 = J[4] plus 1 at column 5
 #pragma unroll
         for (int i = 0; i < 6; ++i) {
@@ -276,37 +280,37 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_smooth(const FitParams<T> p) {
             for (int j = 0; j < 6; ++j) M[4][j] = Cfa[4][j];
           } else {
             const int r = (i == 5) ? 4 : i;
-            double Jr[5];
+            A Jr[5];
 #pragma unroll
-            for (int l = 0; l < 5; ++l) Jr[l] = (double)bt[(size_t)(42 + r * 5 + l) * CH];
+            for (int l = 0; l < 5; ++l) Jr[l] = (A)bt[(size_t)(42 + r * 5 + l) * CH];
 #pragma unroll
             for (int j = 0; j < 6; ++j) {
-              double v = (i == 5) ? Cfa[5][j] : 0.0;
+              A v = (i == 5) ? Cfa[5][j] : A(0);
 #pragma unroll
               for (int l = 0; l < 5; ++l) v += Jr[l] * Cfa[l][j];
               M[i][j] = v;
             }
           }
         }
-        if (!spd_solve6(G, M, X)) { good = false; break; }  // X = Cp^-1 J Cf = A^T
-        double dx[6];
+        if (!spd_solve6<A>(G, M, X)) { good = false; break; }  // X = Cp^-1 J Cf = A^T
+        A dx[6];
 #pragma unroll
-        for (int i = 0; i < 6; ++i) dx[i] = xs[i] - bx[i * CH];
-        dx[2] = wrap_pi(dx[2]);
+        for (int i = 0; i < 6; ++i) dx[i] = xs[i] - (A)bx[i * CH];
+        dx[2] = wrap_pi<A>(dx[2]);
 #pragma unroll
         for (int i = 0; i < 6; ++i) {
-          double v = 0.0;
+          A v = A(0);
 #pragma unroll
           for (int j = 0; j < 6; ++j) v += X[j][i] * dx[j];
-          xs[i] = ax[(6 + i) * CH] + v;
+          xs[i] = (A)ax[(6 + i) * CH] + v;
         }
-        xs[2] = wrap_pi(xs[2]);
-        double Tm[6][6];
+        xs[2] = wrap_pi<A>(xs[2]);
+        A Tm[6][6];
 #pragma unroll
         for (int i = 0; i < 6; ++i)
 #pragma unroll
           for (int j = 0; j < 6; ++j) {
-            double v = 0.0;
+            A v = A(0);
 #pragma unroll
             for (int l = 0; l < 6; ++l) v += (Cs[i][l] - G[i][l]) * X[l][j];
             Tm[i][j] = v;
@@ -315,7 +319,7 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_smooth(const FitParams<T> p) {
         for (int i = 0; i < 6; ++i)
 #pragma unroll
           for (int j = 0; j < 6; ++j) {
-            double v = 0.0;
+            A v = A(0);
 #pragma unroll
             for (int l = 0; l < 6; ++l) v += X[l][i] * Tm[l][j];
             M[i][j] = Cfa[i][j] + v;
@@ -323,7 +327,7 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_smooth(const FitParams<T> p) {
 #pragma unroll
         for (int i = 0; i < 6; ++i)
 #pragma unroll
-          for (int j = 0; j < 6; ++j) Cs[i][j] = 0.5 * (M[i][j] + M[j][i]);
+          for (int j = 0; j < 6; ++j) Cs[i][j] = A(0.5) * (M[i][j] + M[j][i]);
       }
     }
     if (!good) {
