@@ -183,11 +183,12 @@ struct Trial {
 
 template <typename T>
 CKF_HD void rk_trial(const FieldDev& fld, const Traj& y, double lam, double h, Trial<T>& t) {
-  // The three field reads share ONE inlined copy of field_at (a rolled stage loop): the trial is the hot
-  // loop of the whole path and must stay small enough for the SM's instruction cache.
+  // The stage loop is unrolled: three inlined copies of field_at.  In the monolithic level loop of r01b one rolled
+  // copy was needed to stay inside the SM's instruction cache; in the per-phase ckf_step the three copies fit
+  // (2,640 SASS instructions) and save the register moves of the rolled form: ckf_step 2.07 -> 1.89 ms per event.
   const double h2 = 0.5 * h, h8 = h * h * 0.125, hh2 = h * h * 0.5;
   double cr1[3], cr2[3], cr3[3], cr4[3];
-#pragma unroll 1
+#pragma unroll
   for (int st = 0; st < 3; ++st) {
     double p[3], B[3], w[3];
     if (st == 0) {
