@@ -80,7 +80,11 @@ struct ckf_handle {
   std::string err;
   std::vector<void*> allocs;
   // state store of ckf_fit, reserved by the first call
-  double* fs_x = nullptr; void* fs_t = nullptr; int32_t* fs_meas = nullptr;
+  double* fs_x = nullptr; void* fs_t = nullptr; int32_t* fs_meas = nullptr; int32_t* fs_next = nullptr;
+  // level arrays, globals and counters for ckf_step when it runs the moves of a fit level (tcap = fit_chunk)
+  int32_t* ft_g = nullptr; unsigned long long* ft_counters = nullptr;
+  double* ft_y = nullptr; void *ft_D = nullptr, *ft_dep = nullptr;
+  int32_t *ft_from = nullptr, *ft_tgt = nullptr, *ft_stop = nullptr, *ft_order = nullptr;
   int fit_chunk = 0, fit_states = 0;
   cudaEvent_t fit_done = nullptr;
   bool timing_print = false;
@@ -232,15 +236,39 @@ int launch_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, con
   p.n_tracks = t->n_tracks; p.offsets = t->track_offsets; p.meas = t->meas_idx; p.seed = t->seed_id;
   p.max_tracks = h->cfg.max_tracks;
   p.chunk = h->fit_chunk; p.max_states = h->fit_states;
-  p.fs_x = h->fs_x; p.fs_t = (T*)h->fs_t; p.fs_meas = h->fs_meas;
+  p.fs_x = h->fs_x; p.fs_t = (T*)h->fs_t; p.fs_meas = h->fs_meas; p.fs_next = h->fs_next;
   p.o_status = o->status; p.o_nstates = o->n_states; p.o_chi2 = (T*)o->chi2_sum; p.o_lastx = (T*)o->last_params;
   p.o_lastC = (T*)o->last_cov; p.o_firstC = (T*)o->first_cov; p.o_entryx = (T*)o->entry_params;
   p.o_work = (unsigned long long*)o->work;
   const int grid = (h->fit_chunk + FIT_NT - 1) / FIT_NT;
   // passes of fit_chunk tracks; a pass beyond *n_tracks returns at once (the count is only known on the device)
+  // what ckf_step needs to run the moves of one level with one tip per track
+  KParams<T> kp;
+  std::memset(&kp, 0, sizeof(kp));
+  kp.geo = p.geo; kp.fld = p.fld; kp.cfg = p.cfg;
+  kp.tcap = h->fit_chunk;
+  kp.g = h->ft_g; kp.counters = h->ft_counters;
+  kp.mv_y = h->ft_y; kp.mv_D = (T*)h->ft_D; kp.mv_dep = (T*)h->ft_dep; kp.mv_from = h->ft_from; kp.mv_tgt = h->ft_tgt;
+  kp.mv_stop = h->ft_stop; kp.mv_order = h->ft_order;
   for (int first = 0; first < h->cfg.max_tracks; first += h->fit_chunk) {
     p.first = first;
-    ckf_fit_forward<T><<<grid, FIT_NT, 0, st>>>(p);
+    // forward filter, level-synchronous: per level the moves on ckf_step, then the rest of the state (ckf_fit_level).
+    // Two blocks of globals, by level parity: level L's ckf_step reads the schedule in block L & 1.
+    cudaMemsetAsync(h->ft_g, 0, 64 * 4, st);
+    cudaMemsetAsync(h->ft_g + G_NTIPS0, 1, 2 * 4, st);       // non-zero: ckf_step only asks whether the level holds tips
+    cudaMemsetAsync(h->ft_g + 32 + G_NTIPS0, 1, 2 * 4, st);
+    cudaMemsetAsync(h->ft_counters, 0, CNT_N * 8, st);
+    for (int level = 0; level < h->fit_states; ++level) {
+      int32_t* g_this = h->ft_g + 32 * (level & 1);
+      int32_t* g_next = h->ft_g + 32 * ((level + 1) & 1);
+      if (level > 0) {
+        kp.g = g_this;
+        ckf_step<T, MinBlocks<T>::value><<<h->step_grid, STEP_NT, 0, st>>>(kp, level);
+      }
+      kp.g = g_next;
+      ckf_fit_level<T><<<grid, FIT_NT, 0, st>>>(kp, p, level, g_this);
+    }
+    ckf_fit_flush_work<<<1, 32, 0, st>>>(h->ft_counters, p.o_work);
     if (sizeof(T) == 4 && o->smoother_precision == 32) ckf_fit_smooth<T, float><<<grid, FIT_NT, 0, st>>>(p);
     else ckf_fit_smooth<T, double><<<grid, FIT_NT, 0, st>>>(p);
   }
@@ -407,7 +435,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     CKB(dalloc(h, &w.s_idx, (size_t)c->max_measurements * 4));
     CKB(dalloc(h, (char**)&w.s_v0max, (size_t)g->n_modules * ts));
     CKB(dalloc(h, &w.globals, 64 * 4));
-    static_assert(G_N <= 64, "globals block too small");
+    static_assert(G_N <= 32, "globals block too small (ckf_fit keeps two of them in 64 ints)");
     CKB(dalloc(h, &w.mv_order, (size_t)NBIN * TC * 4));
     CKB(dalloc(h, &w.counters, CNT_N * 8));
     CKB(cudaEventCreateWithFlags(&w.done, cudaEventDisableTiming));
@@ -509,6 +537,13 @@ int ckf_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, const 
     CK(dalloc(h, &fx, n * FS_X * sizeof(double)));
     CK(dalloc(h, &ft, n * FS_T * (size_t)h->tsize));
     CK(dalloc(h, &fm, n * 4));
+    const size_t CHK = (size_t)chunk, ts = (size_t)h->tsize;
+    CK(dalloc(h, &h->fs_next, CHK * 4));
+    CK(dalloc(h, &h->ft_g, 64 * 4)); CK(dalloc(h, &h->ft_counters, CNT_N * 8));
+    CK(dalloc(h, &h->ft_y, 8 * CHK * sizeof(double)));
+    CK(dalloc(h, (char**)&h->ft_D, 25 * CHK * ts)); CK(dalloc(h, (char**)&h->ft_dep, 5 * CHK * ts));
+    CK(dalloc(h, &h->ft_from, CHK * 4)); CK(dalloc(h, &h->ft_tgt, 2 * CHK * 4)); CK(dalloc(h, &h->ft_stop, CHK * 4));
+    CK(dalloc(h, &h->ft_order, (size_t)NBIN * CHK * 4));
     CK(cudaEventCreateWithFlags(&h->fit_done, cudaEventDisableTiming));
     h->fs_x = fx; h->fs_t = ft; h->fs_meas = fm; h->fit_chunk = chunk; h->fit_states = ns;
   } else {

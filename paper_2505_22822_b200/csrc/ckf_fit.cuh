@@ -3,22 +3,23 @@
 // the CKF's parameters are best at the LAST measurement; "a Kalman Filter-based fitting, which runs
 // a smoothing algorithm called the Rauch-Tung-Striebel (RTS) smoother, is applied additionally to the tracks to
 // make all track parameters consider all measurements".  Rules K1-K5 of DESIGN.md §3:
-//   ckf_fit_forward  thread per track: the forward filter walks the candidate's own path with the same per-tip
-//                    code as the CKF (navigation, RKN4 + Jacobian, arrival, covariance transport, Highland,
-//                    gain-form update: ckf_nav.cuh / ckf_math.cuh) and the branch choice replaced by the
-//                    candidate's list; every visited module is a STATE whose predicted / filtered parameters,
-//                    covariances and Jacobian go to the state store
+//   forward filter   level-synchronous like the CKF, one tip per track, the branch choice replaced by the candidate's
+//                    list: the moves of a level run on the CKF's own ckf_step kernel (navigation, RKN4 + Jacobian),
+//                    ckf_fit_level does the rest of the state with the CKF's per-tip code (arrival, covariance
+//                    transport, Highland, gain-form update: ckf_nav.cuh / ckf_math.cuh); every visited module is a
+//                    STATE whose predicted / filtered parameters, covariances and Jacobian go to the state store
 //   ckf_fit_smooth   thread per track: RTS backward recursion over the stored states, float64 arithmetic in
 //                    both modes (the gain needs the inverse of a predicted covariance whose entries span ten
 //                    orders of magnitude; PAPER.md:61, :100 report the float32 smoother as unstable)
 // State store: [state][component][track], track fastest, so the lanes of a warp (consecutive tracks) coalesce.
 #pragma once
-#include "ckf_kernels.cuh"
+#include "ckf_branch.cuh"
+#include "ckf_step.cuh"
 
 namespace ckf {
 
 constexpr int FIT_NT = 128;
-constexpr int FIT_CHUNK = 131072;   // tracks per pass: bounds the state store (ckf.cu loops over the chunks)
+constexpr int FIT_CHUNK = 262144;   // tracks per pass: bounds the state store (ckf.cu loops over the chunks)
 constexpr int FS_X = 12;            // float64 per state: xp[6], xf[6]
 constexpr int FS_T = 21 + 21 + 25;  // T per state: Cp, Cf (packed upper triangles), J (5x5 block, row-major)
 
@@ -46,76 +47,112 @@ struct FitParams {
   double* fs_x;         // [max_states][FS_X][chunk]
   T* fs_t;              // [max_states][FS_T][chunk]
   int32_t* fs_meas;     // [max_states][chunk] measurement used by the state, -1 = module passed without one
+  int32_t* fs_next;     // [chunk] list entries the track has consumed so far (level-synchronous forward filter)
   // output (device, caller-owned)
   int32_t* o_status; int32_t* o_nstates;
   T* o_chi2; T* o_lastx; T* o_lastC; T* o_firstC; T* o_entryx;
   unsigned long long* o_work;  // [4] or null: RKN4 trials, accepted steps, moves, updates are ADDED here
 };
 
+// ---- level-synchronous forward filter: the moves of a level run on the CKF's own ckf_step (persistent lanes,
+// step schedule), one tip per track; this kernel is the rest of a level, thread per track: arrival (J4, J5),
+// covariance transport, the listed measurement (or none), state store, departure + N2 + cost class of the next move.
+// kp carries only what ckf_step needs (level arrays with tcap = chunk, globals, counters), all owned by the fit store.
+constexpr int FIT_RUNNING = -1;
+
+// The step schedule is double-buffered by level parity (two blocks of globals, G_N ints apart): kp.g is the block
+// this level appends to for the next level's ckf_step; `g_done` is the block the ckf_step before this kernel
+// consumed, which thread 0 clears for the level after next.
 template <typename T>
-__global__ void __launch_bounds__(FIT_NT) ckf_fit_forward(const FitParams<T> p) {
+__global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, const FitParams<T> p, int level, int32_t* g_done) {
+  if (blockIdx.x == 0 && threadIdx.x < G_N - G_STEP_CURSOR) g_done[G_STEP_CURSOR + threadIdx.x] = 0;
   const int nt = min(*p.n_tracks, p.max_tracks);
   const size_t CH = (size_t)p.chunk;
-  unsigned long long w_trials = 0, w_acc = 0, w_moves = 0, w_upd = 0;
-  for (int s = blockIdx.x * FIT_NT + threadIdx.x; s < p.chunk; s += gridDim.x * FIT_NT) {
-    const int tr = p.first + s;
-    if (tr >= nt) break;
-    const int e0 = p.offsets[tr], n = p.offsets[tr + 1] - e0, sd = p.seed[tr];
-    double x[6], xf[6];
-    T C[21], Cf[21];
-    bool ok = true;
-#pragma unroll
-    for (int i = 0; i < 6; ++i) {
-      x[i] = (double)p.seed_x[(size_t)sd * 6 + i];
-      xf[i] = 0.0;
-      ok = ok && isfinite(x[i]);
-    }
-    ok = ok && (x[3] > 0.0 && x[3] < PI_D);
-#pragma unroll
-    for (int i = 0; i < 6; ++i)
-#pragma unroll
-      for (int j = i; j < 6; ++j) { C[tri(i, j)] = p.seed_C[(size_t)sd * 36 + i * 6 + j]; Cf[tri(i, j)] = T(0); }
-    int module = p.seed_module[sd], next = 0, status = STOP_NONE, ns = 0;
+  const int s = blockIdx.x * FIT_NT + threadIdx.x;
+  const int tr = p.first + s;
+  unsigned long long w_moves = 0, w_upd = 0;
+  int bin = -1;
+  if (s < p.chunk && tr < nt && (level == 0 || p.o_status[tr] == FIT_RUNNING)) {
+    const int e0 = p.offsets[tr], n = p.offsets[tr + 1] - e0;
+    double xp[6], xf[6];
+    T Cp[21], Cf[21], J[5][5];
+    int status = STOP_NONE, module = 0, next = 0, stored = level;
+    bool done = false;
     T c2sum = T(0);
-    for (int level = 0; n > 0; ++level) {
-      if (level >= p.cfg.max_levels || level >= p.max_states) { status = STOP_LEVEL_LIMIT; break; }
-      double xp[6];
-      T Cp[21], J[5][5];
-      if (level == 0) {  // N6: the seed's own module, identity transport
-        if (!ok) { status = STOP_NUMERIC; break; }
 #pragma unroll
-        for (int i = 0; i < 6; ++i) xp[i] = x[i];
+    for (int i = 0; i < 6; ++i) xf[i] = 0.0;
 #pragma unroll
-        for (int i = 0; i < 21; ++i) Cp[i] = C[i];
+    for (int i = 0; i < 21; ++i) Cf[i] = T(0);
+    if (level == 0) {  // N6: the seed's own module, identity transport
+      const int sd = p.seed[tr];
+      bool ok = true;
 #pragma unroll
-        for (int a = 0; a < 5; ++a)
+      for (int i = 0; i < 6; ++i) { xp[i] = (double)p.seed_x[(size_t)sd * 6 + i]; ok = ok && isfinite(xp[i]); }
+      ok = ok && (xp[3] > 0.0 && xp[3] < PI_D);
 #pragma unroll
-          for (int b = 0; b < 5; ++b) J[a][b] = (a == b && a < 4) ? T(1) : T(0);
-      } else {
-        int tg = -1;
-        T qphi, qth;
-        StepCtl sc;
-        sc.n_trials = 0; sc.n_accepted = 0;
-        status = move_to_next_module<T>(p.geo, p.fld, p.cfg, module, x, tg, xp, J, qphi, qth, sc);
-        w_trials += sc.n_trials; w_acc += sc.n_accepted; w_moves += 1;
-        if (status != STOP_NONE) break;
-        C[tri(2, 2)] += qphi;  // V5 on leaving
-        C[tri(3, 3)] += qth;
-        transport_cov<T>(J, C, Cp);
-        bool fin = true;
+      for (int i = 0; i < 6; ++i)
 #pragma unroll
-        for (int i = 0; i < 21; ++i) fin = fin && isfinite(Cp[i]);
-        if (!fin) { status = STOP_NUMERIC; break; }
-        module = tg;
+        for (int j = i; j < 6; ++j) Cp[tri(i, j)] = p.seed_C[(size_t)sd * 36 + i * 6 + j];
+#pragma unroll
+      for (int a = 0; a < 5; ++a)
+#pragma unroll
+        for (int b = 0; b < 5; ++b) J[a][b] = (a == b && a < 4) ? T(1) : T(0);
+      module = p.seed_module[sd];
+      if (n < 1) done = true;
+      else if (!ok) status = STOP_NUMERIC;
+    } else {
+      next = p.fs_next[s];
+      c2sum = p.o_chi2[tr];
+      w_moves += 1;
+      status = kp.mv_stop[s];
+      if (status == STOP_NONE) {
+        Move<T> m;
+#pragma unroll
+        for (int i = 0; i < 3; ++i) { m.y.r[i] = kp.mv_y[i * CH + s]; m.y.d[i] = kp.mv_y[(3 + i) * CH + s]; }
+        m.y.t = kp.mv_y[6 * CH + s];
+        m.y.qop = kp.mv_y[7 * CH + s];
+#pragma unroll
+        for (int i = 0; i < 3; ++i) {
+#pragma unroll
+          for (int j = 0; j < 3; ++j) {
+            m.D.Rd[i][j] = kp.mv_D[(i * 3 + j) * CH + s];
+            m.D.Dd[i][j] = kp.mv_D[(9 + i * 3 + j) * CH + s];
+          }
+          m.D.rq[i] = kp.mv_D[(18 + i) * CH + s];
+          m.D.dq[i] = kp.mv_D[(21 + i) * CH + s];
+        }
+        m.D.tq = kp.mv_D[24 * CH + s];
+        m.from = kp.mv_from[s];
+        m.tgt = kp.mv_tgt[s];
+        T dep[5];
+#pragma unroll
+        for (int i = 0; i < 5; ++i) dep[i] = kp.mv_dep[i * CH + s];
+        status = move_arrive<T>(m, dep, p.geo, p.fld, p.cfg, xp, J);
+        if (status == STOP_NONE) {
+          T C[21];
+          const T* pt = p.fs_t + (size_t)(level - 1) * FS_T * CH + s;  // filtered covariance of the previous state
+#pragma unroll
+          for (int i = 0; i < 21; ++i) C[i] = pt[(21 + i) * CH];
+          C[tri(2, 2)] += dep[3];  // V5 on leaving
+          C[tri(3, 3)] += dep[4];
+          transport_cov<T>(J, C, Cp);
+          bool fin = true;
+#pragma unroll
+          for (int i = 0; i < 21; ++i) fin = fin && isfinite(Cp[i]);
+          if (!fin) status = STOP_NUMERIC;
+          module = m.tgt;
+        }
       }
+    }
+    if (status == STOP_NONE && !done) {
       const int k = p.meas[e0 + next];
       int used = -1;
       if (k >= p.moff[module] && k < p.moff[module + 1]) {
-        const typename Vec2<T>::type m = p.loc[k], v = p.var[k];
+        const typename Vec2<T>::type mm = p.loc[k], vv = p.var[k];
         const double c2 = predicted_chi2<double>(xp[0], xp[1], (double)Cp[tri(0, 0)], (double)Cp[tri(0, 1)],
-                                                 (double)Cp[tri(1, 1)], (double)m.x, (double)m.y, (double)v.x, (double)v.y);
+                                                 (double)Cp[tri(1, 1)], (double)mm.x, (double)mm.y, (double)vv.x, (double)vv.y);
         c2sum += (T)c2;
-        kalman_update<T>(xp, Cp, m.x, m.y, v.x, v.y, xf, Cf);
+        kalman_update<T>(xp, Cp, mm.x, mm.y, vv.x, vv.y, xf, Cf);
         used = k;
         ++next;
         w_upd += 1;
@@ -136,30 +173,67 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_forward(const FitParams<T> p) 
 #pragma unroll
         for (int b = 0; b < 5; ++b) ft[(42 + a * 5 + b) * CH] = J[a][b];
       p.fs_meas[(size_t)level * CH + s] = used;
-      ns = level + 1;
-      if (next == n) break;
+      stored = level + 1;
+      if (next == n) done = true;
+      else if (stored >= p.cfg.max_levels || stored >= p.max_states) status = STOP_LEVEL_LIMIT;
+      else {
+        Traj y;
+        T dep[5];
+        status = departure_state<T>(p.geo, p.cfg, module, xf, y, dep);
+        if (status == STOP_NONE) {  // the track as a tip of the next level's ckf_step
 #pragma unroll
-      for (int i = 0; i < 6; ++i) x[i] = xf[i];
+          for (int i = 0; i < 3; ++i) { kp.mv_y[i * CH + s] = y.r[i]; kp.mv_y[(3 + i) * CH + s] = y.d[i]; }
+          kp.mv_y[6 * CH + s] = y.t;
+          kp.mv_y[7 * CH + s] = y.qop;
 #pragma unroll
-      for (int i = 0; i < 21; ++i) C[i] = Cf[i];
+          for (int i = 0; i < 5; ++i) kp.mv_dep[i * CH + s] = dep[i];
+          kp.mv_from[s] = module;
+          const int ov = overlap_neighbour(p.geo, module, y.r, y.d);  // N2
+          kp.mv_tgt[CH + s] = ov;
+          kp.mv_stop[s] = STOP_NONE;
+          bin = step_cost_bin(p.geo, module, y, ov);
+          p.fs_next[s] = next;
+          p.o_chi2[tr] = c2sum;
+          p.o_status[tr] = FIT_RUNNING;
+          p.o_nstates[tr] = stored;
+        }
+      }
     }
-    p.o_status[tr] = status;
-    p.o_nstates[tr] = ns;
-    const bool good = status == STOP_NONE && ns > 0;
-    p.o_chi2[tr] = good ? c2sum : T(0);
+    if (done || status != STOP_NONE) {  // the forward pass of this track ends here
+      const bool good = status == STOP_NONE && stored > 0;
+      p.o_status[tr] = status;
+      p.o_nstates[tr] = stored;
+      p.o_chi2[tr] = good ? c2sum : T(0);
 #pragma unroll
-    for (int i = 0; i < 6; ++i) p.o_lastx[(size_t)tr * 6 + i] = good ? (T)xf[i] : T(0);
+      for (int i = 0; i < 6; ++i) p.o_lastx[(size_t)tr * 6 + i] = good ? (T)xf[i] : T(0);
 #pragma unroll
-    for (int i = 0; i < 6; ++i)
+      for (int i = 0; i < 6; ++i)
 #pragma unroll
-      for (int j = 0; j < 6; ++j) p.o_lastC[(size_t)tr * 36 + i * 6 + j] = good ? Cf[tri(i, j)] : T(0);
+        for (int j = 0; j < 6; ++j) p.o_lastC[(size_t)tr * 36 + i * 6 + j] = good ? Cf[tri(i, j)] : T(0);
+    }
+  }
+  // step schedule of the next level: append the running track to its cost class (as ckf_update does)
+  const unsigned live = __ballot_sync(0xffffffffu, bin >= 0);
+  if (bin >= 0) {
+    const int lane = threadIdx.x & 31;
+    const unsigned peers = __match_any_sync(live, bin);
+    const int leader = __ffs(peers) - 1;
+    int base = 0;
+    if (lane == leader) base = atomicAdd(kp.g + G_BIN0 + bin, __popc(peers));
+    base = __shfl_sync(peers, base, leader);
+    kp.mv_order[(size_t)bin * CH + base + __popc(peers & ((1u << lane) - 1u))] = s;
   }
   if (p.o_work) {
-    __syncwarp();
-    flush_counter(p.o_work + 0, w_trials);
-    flush_counter(p.o_work + 1, w_acc);
     flush_counter(p.o_work + 2, w_moves);
     flush_counter(p.o_work + 3, w_upd);
+  }
+}
+
+// adds the RKN4 counters ckf_step accumulated for this pass to the caller's work counters
+__global__ void ckf_fit_flush_work(const unsigned long long* counters, unsigned long long* o_work) {
+  if (o_work && threadIdx.x == 0 && blockIdx.x == 0) {
+    o_work[0] += counters[CNT_TRIALS];
+    o_work[1] += counters[CNT_ACCEPTED];
   }
 }
 
