@@ -237,54 +237,8 @@ __global__ void ckf_fit_flush_work(const unsigned long long* counters, unsigned 
   }
 }
 
-// K4 helper: X = G^-1 B for a symmetric positive definite 6x6 G: scale to unit diagonal, Cholesky, two
-// triangular solves per column.  false when G is not positive definite.
-template <typename A>
-__device__ __forceinline__ bool spd_solve6(const A G[6][6], const A B[6][6], A X[6][6]) {
-  A s[6], L[6][6];
-#pragma unroll
-  for (int i = 0; i < 6; ++i) {
-    if (!(G[i][i] > A(0))) return false;
-    s[i] = A(1) / sqrt(G[i][i]);
-  }
-#pragma unroll
-  for (int j = 0; j < 6; ++j) {
-    A d = G[j][j] * s[j] * s[j];
-#pragma unroll
-    for (int k = 0; k < j; ++k) d -= L[j][k] * L[j][k];
-    if (!(d > A(0))) return false;
-    L[j][j] = sqrt(d);
-#pragma unroll
-    for (int i = j + 1; i < 6; ++i) {
-      A v = G[i][j] * s[i] * s[j];
-#pragma unroll
-      for (int k = 0; k < j; ++k) v -= L[i][k] * L[j][k];
-      L[i][j] = v / L[j][j];
-    }
-  }
-#pragma unroll 1
-  for (int c = 0; c < 6; ++c) {
-    A z[6], w[6];
-#pragma unroll
-    for (int i = 0; i < 6; ++i) {
-      A v = B[i][c] * s[i];
-#pragma unroll
-      for (int k = 0; k < i; ++k) v -= L[i][k] * z[k];
-      z[i] = v / L[i][i];
-    }
-#pragma unroll
-    for (int i = 5; i >= 0; --i) {
-      A v = z[i];
-#pragma unroll
-      for (int k = i + 1; k < 6; ++k) v -= L[k][i] * w[k];
-      w[i] = v / L[i][i];
-    }
-#pragma unroll
-    for (int i = 0; i < 6; ++i) X[i][c] = w[i] * s[i];
-  }
-  return true;
-}
-
+// ---- RTS smoother (K4).  Register-resident: the symmetric matrices stay packed (21 numbers), the gain is solved
+// column by column in place, every loop is unrolled with constant indices (no local memory).
 template <typename A>
 __device__ __forceinline__ A wrap_pi(A a) {
   while (a > (A)PI_D) a -= (A)(2.0 * PI_D);
@@ -292,23 +246,62 @@ __device__ __forceinline__ A wrap_pi(A a) {
   return a;
 }
 
-// packed upper triangle (T) of a state at component offset `c0` -> dense symmetric matrix of the arithmetic type
-template <typename T, typename A>
-__device__ __forceinline__ void load_sym(const T* ft, size_t CH, int c0, A M[6][6]) {
+// Cholesky of G scaled to unit diagonal: G' = S G S = L L^T, S = diag(1 / sqrt(G_ii)).  L is packed by rows
+// (L[i][j], j <= i, at tri(j, i)).  false when G is not positive definite.
+template <typename A>
+__device__ __forceinline__ bool chol6_scaled(const A G[21], A s[6], A L[21]) {
 #pragma unroll
-  for (int i = 0; i < 6; ++i)
+  for (int i = 0; i < 6; ++i) {
+    if (!(G[tri(i, i)] > A(0))) return false;
+    s[i] = A(1) / sqrt(G[tri(i, i)]);
+  }
 #pragma unroll
-    for (int j = i; j < 6; ++j) {
-      const A v = (A)ft[(size_t)(c0 + tri(i, j)) * CH];
-      M[i][j] = v;
-      M[j][i] = v;
+  for (int j = 0; j < 6; ++j) {
+    A d = G[tri(j, j)] * s[j] * s[j];
+#pragma unroll
+    for (int k = 0; k < j; ++k) d -= L[tri(k, j)] * L[tri(k, j)];
+    if (!(d > A(0))) return false;
+    L[tri(j, j)] = sqrt(d);
+#pragma unroll
+    for (int i = j + 1; i < 6; ++i) {
+      A v = G[tri(i, j)] * s[i] * s[j];
+#pragma unroll
+      for (int k = 0; k < j; ++k) v -= L[tri(k, i)] * L[tri(k, j)];
+      L[tri(j, i)] = v / L[tri(j, j)];
     }
+  }
+  return true;
+}
+
+// one column: b <- G^-1 b with the factor above (L z = S b, L^T w = z, x = S w)
+template <typename A>
+__device__ __forceinline__ void chol6_solve(const A s[6], const A L[21], A b[6]) {
+  A z[6];
+#pragma unroll
+  for (int i = 0; i < 6; ++i) {
+    A v = b[i] * s[i];
+#pragma unroll
+    for (int k = 0; k < i; ++k) v -= L[tri(k, i)] * z[k];
+    z[i] = v / L[tri(i, i)];
+  }
+#pragma unroll
+  for (int i = 5; i >= 0; --i) {
+    A v = z[i];
+#pragma unroll
+    for (int k = i + 1; k < 6; ++k) v -= L[tri(i, k)] * b[k];
+    b[i] = v / L[tri(i, i)];   // b[i..5] now hold w[i..5]
+  }
+#pragma unroll
+  for (int i = 0; i < 6; ++i) b[i] *= s[i];
 }
 
 // A = arithmetic type of the recursion: double (the product's choice, K5), or float for the study of the float32
 // smoother's instability that PAPER.md:61, :100 report (fp32 mode only).
+#ifndef CKF_SMOOTH_MINB
+#define CKF_SMOOTH_MINB 2
+#endif
 template <typename T, typename A>
-__global__ void __launch_bounds__(FIT_NT) ckf_fit_smooth(const FitParams<T> p) {
+__global__ void __launch_bounds__(FIT_NT, CKF_SMOOTH_MINB) ckf_fit_smooth(const FitParams<T> p) {
   const int nt = min(*p.n_tracks, p.max_tracks);
   const size_t CH = (size_t)p.chunk;
   for (int s = blockIdx.x * FIT_NT + threadIdx.x; s < p.chunk; s += gridDim.x * FIT_NT) {
@@ -317,14 +310,15 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_smooth(const FitParams<T> p) {
     const int e0 = p.offsets[tr], n = p.offsets[tr + 1] - e0;
     const int ns = p.o_nstates[tr];
     bool good = p.o_status[tr] == STOP_NONE && ns > 0;
-    A xs[6], Cs[6][6];
+    A xs[6], Cs[21];
     int e = n - 1;  // entries are filled from the back: the forward pass ends on the last measurement
     if (good) {
       const double* fx = p.fs_x + (size_t)(ns - 1) * FS_X * CH + s;
       const T* ft = p.fs_t + (size_t)(ns - 1) * FS_T * CH + s;
 #pragma unroll
       for (int i = 0; i < 6; ++i) xs[i] = (A)fx[(6 + i) * CH];
-      load_sym<T, A>(ft, CH, 21, Cs);
+#pragma unroll
+      for (int i = 0; i < 21; ++i) Cs[i] = (A)ft[(size_t)(21 + i) * CH];
       for (int k = ns - 1;; --k) {
         if (p.fs_meas[(size_t)k * CH + s] >= 0) {
 #pragma unroll
@@ -333,7 +327,7 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_smooth(const FitParams<T> p) {
 #pragma unroll
             for (int i = 0; i < 6; ++i)
 #pragma unroll
-              for (int j = 0; j < 6; ++j) p.o_firstC[(size_t)tr * 36 + i * 6 + j] = (T)Cs[i][j];
+              for (int j = 0; j < 6; ++j) p.o_firstC[(size_t)tr * 36 + i * 6 + j] = (T)Cs[tri(i, j)];
           }
           --e;
         }
@@ -343,30 +337,43 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_smooth(const FitParams<T> p) {
         const T* bt = p.fs_t + (size_t)k * FS_T * CH + s;
         const double* ax = p.fs_x + (size_t)(k - 1) * FS_X * CH + s;
         const T* at = p.fs_t + (size_t)(k - 1) * FS_T * CH + s;
-        A G[6][6], Cfa[6][6], M[6][6], X[6][6];
-        load_sym<T, A>(bt, CH, 0, G);
-        load_sym<T, A>(at, CH, 21, Cfa);
-        // M = Jf Cf[k-1], Jf rows 0..3 = J[0..3] over columns 0..4, row 4 = e_4, row 5 = J[4] plus 1 at column 5
+        A sc[6], L[21], dC[21], Cf[21];
+        {
+          A G[21];
 #pragma unroll
-        for (int i = 0; i < 6; ++i) {
-          if (i == 4) {
+          for (int i = 0; i < 21; ++i) { G[i] = (A)bt[(size_t)i * CH]; dC[i] = Cs[i] - G[i]; }
+          if (!chol6_scaled<A>(G, sc, L)) { good = false; break; }
+        }
 #pragma unroll
-            for (int j = 0; j < 6; ++j) M[4][j] = Cfa[4][j];
-          } else {
-            const int r = (i == 5) ? 4 : i;
-            A Jr[5];
+        for (int i = 0; i < 21; ++i) Cf[i] = (A)at[(size_t)(21 + i) * CH];
+        // X = Cp^-1 (Jf Cf) = A_k^T, column by column.  Jf rows 0..3 = J[0..3] over columns 0..4, row 4 = e_4,
+        // row 5 = J[4] plus 1 at column 5
+        A X[6][6];
+        {
+          A Jb[5][5];
 #pragma unroll
-            for (int l = 0; l < 5; ++l) Jr[l] = (A)bt[(size_t)(42 + r * 5 + l) * CH];
+          for (int r = 0; r < 5; ++r)
 #pragma unroll
-            for (int j = 0; j < 6; ++j) {
-              A v = (i == 5) ? Cfa[5][j] : A(0);
+            for (int l = 0; l < 5; ++l) Jb[r][l] = (A)bt[(size_t)(42 + r * 5 + l) * CH];
 #pragma unroll
-              for (int l = 0; l < 5; ++l) v += Jr[l] * Cfa[l][j];
-              M[i][j] = v;
+          for (int c = 0; c < 6; ++c) {
+            A col[6];
+#pragma unroll
+            for (int i = 0; i < 6; ++i) {
+              if (i == 4) col[i] = Cf[tri(4, c)];
+              else {
+                const int r = (i == 5) ? 4 : i;
+                A v = (i == 5) ? Cf[tri(5, c)] : A(0);
+#pragma unroll
+                for (int l = 0; l < 5; ++l) v += Jb[r][l] * Cf[tri(l, c)];
+                col[i] = v;
+              }
             }
+            chol6_solve<A>(sc, L, col);
+#pragma unroll
+            for (int i = 0; i < 6; ++i) X[i][c] = col[i];
           }
         }
-        if (!spd_solve6<A>(G, M, X)) { good = false; break; }  // X = Cp^-1 J Cf = A^T
         A dx[6];
 #pragma unroll
         for (int i = 0; i < 6; ++i) dx[i] = xs[i] - (A)bx[i * CH];
@@ -379,29 +386,30 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_smooth(const FitParams<T> p) {
           xs[i] = (A)ax[(6 + i) * CH] + v;
         }
         xs[2] = wrap_pi<A>(xs[2]);
-        A Tm[6][6];
+        // Cs <- sym(Cf + X^T (dC X)), one column of dC X at a time
+        A R[6][6];
 #pragma unroll
-        for (int i = 0; i < 6; ++i)
+        for (int j = 0; j < 6; ++j) {
+          A t[6];
 #pragma unroll
-          for (int j = 0; j < 6; ++j) {
+          for (int i = 0; i < 6; ++i) {
             A v = A(0);
 #pragma unroll
-            for (int l = 0; l < 6; ++l) v += (Cs[i][l] - G[i][l]) * X[l][j];
-            Tm[i][j] = v;
+            for (int l = 0; l < 6; ++l) v += dC[tri(i, l)] * X[l][j];
+            t[i] = v;
           }
 #pragma unroll
-        for (int i = 0; i < 6; ++i)
-#pragma unroll
-          for (int j = 0; j < 6; ++j) {
+          for (int i = 0; i < 6; ++i) {
             A v = A(0);
 #pragma unroll
-            for (int l = 0; l < 6; ++l) v += X[l][i] * Tm[l][j];
-            M[i][j] = Cfa[i][j] + v;
+            for (int l = 0; l < 6; ++l) v += X[l][i] * t[l];
+            R[i][j] = Cf[tri(i, j)] + v;
           }
+        }
 #pragma unroll
         for (int i = 0; i < 6; ++i)
 #pragma unroll
-          for (int j = 0; j < 6; ++j) Cs[i][j] = A(0.5) * (M[i][j] + M[j][i]);
+          for (int j = i; j < 6; ++j) Cs[tri(i, j)] = A(0.5) * (R[i][j] + R[j][i]);
       }
     }
     if (!good) {
