@@ -26,7 +26,7 @@
 extern "C" {
 #endif
 
-#define CKF_ABI_VERSION 3
+#define CKF_ABI_VERSION 4
 
 /* return codes */
 #define CKF_OK 0
@@ -104,21 +104,34 @@ typedef struct {
   int32_t max_links;                /* candidate-link buffer entries; 0 = 48 * max_seeds                 */
   int32_t max_tips_per_level;       /* live branch tips of one level, whole event; 0 = 8 * max_seeds     */
   int32_t n_streams;                /* independent workspaces; concurrent ckf_find calls up to this many */
+  int32_t max_events_per_find;      /* largest batch of events one ckf_find may carry; 0 = 1 (see ckf_measurements) */
 } ckf_config;
 
 /* Measurements of one event: CSR by module id (north_star).  DEVICE pointers, caller-owned, read-only.
- * A measurement's index is its position in loc/var and is what ckf_tracks.meas_idx reports. */
+ * A measurement's index is its position in loc/var and is what ckf_tracks.meas_idx reports.
+ *
+ * Batch of events (n_events = B > 1, at most config.max_events_per_find).  Events are independent,
+ * so B of them may share ONE ckf_find: the caller concatenates their measurements (event 0 first) and their seeds and
+ * addresses modules by the VIRTUAL id  event * n_modules + module  -- in module_offsets, which then has
+ * B * n_modules + 1 entries over the concatenated arrays, and in ckf_seeds.module_id.  The library treats the batch as
+ * one event in B replicas of the detector: every level of the branch loop then runs over the tips of all B events
+ * (the per-level cost of the level-synchronous loop is shared), and nothing else changes: meas_idx reports positions
+ * in the concatenated arrays, seed_id positions in the concatenated seeds (so the candidates of event e are those
+ * whose seed_id lies in its seed range, contiguous in the output), last_module the real module id.  Capacities
+ * (max_seeds, max_measurements, max_tracks, ...) count the whole batch.  Results per event are identical to those
+ * of B separate calls (tested). */
 typedef struct {
   int32_t n;
-  const int32_t* module_offsets; /* [n_modules + 1]; module m owns [off[m], off[m+1])  */
+  const int32_t* module_offsets; /* [n_events * n_modules + 1]; (virtual) module m owns [off[m], off[m+1]) */
   const void* loc;               /* T[n][2] local position (loc0, loc1) mm             */
   const void* var;               /* T[n][2] variances mm^2                             */
+  int32_t n_events;              /* 0 or 1: one event; B > 1: a batch, see above       */
 } ckf_measurements;
 
 /* Seeds: bound parameters + covariance on a module.  DEVICE pointers, caller-owned, read-only. */
 typedef struct {
   int32_t n;
-  const int32_t* module_id; /* [n]                                               */
+  const int32_t* module_id; /* [n]  (virtual id event * n_modules + module in a batch)  */
   const void* params;       /* T[n][6]  loc0 loc1 phi theta q/p t                */
   const void* cov;          /* T[n][36] row-major, symmetric                     */
 } ckf_seeds;

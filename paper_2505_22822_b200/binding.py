@@ -43,11 +43,11 @@ class ckf_config(C.Structure):
                 ("particle_mass_gev", C.c_double), ("max_rk_steps_per_surface", C.c_int32), ("max_levels", C.c_int32),
                 ("max_seeds", C.c_int32), ("max_measurements", C.c_int32), ("max_tracks", C.c_int32),
                 ("max_track_entries", C.c_int32), ("max_links", C.c_int32), ("max_tips_per_level", C.c_int32),
-                ("n_streams", C.c_int32)]
+                ("n_streams", C.c_int32), ("max_events_per_find", C.c_int32)]
 
 
 class ckf_measurements(C.Structure):
-    _fields_ = [("n", C.c_int32), ("module_offsets", _vp), ("loc", _vp), ("var", _vp)]
+    _fields_ = [("n", C.c_int32), ("module_offsets", _vp), ("loc", _vp), ("var", _vp), ("n_events", C.c_int32)]
 
 
 class ckf_seeds(C.Structure):
@@ -150,7 +150,8 @@ def make_field(fld, keep: list) -> ckf_field:
 
 
 def make_config(ckf, precision: int, max_seeds: int, max_measurements: int, max_tracks: int, max_track_entries: int,
-                max_links: int = 0, n_streams: int = 1, max_tips_per_level: int = 0) -> ckf_config:
+                max_links: int = 0, n_streams: int = 1, max_tips_per_level: int = 0,
+                max_events_per_find: int = 1) -> ckf_config:
     c = ckf_config()
     c.precision = int(precision)
     for name in ("chi2_max", "max_branches_per_surface", "max_candidates_per_seed", "max_holes", "min_measurements",
@@ -161,7 +162,49 @@ def make_config(ckf, precision: int, max_seeds: int, max_measurements: int, max_
     c.max_tracks, c.max_track_entries = int(max_tracks), int(max_track_entries)
     c.max_links, c.n_streams = int(max_links), int(n_streams)
     c.max_tips_per_level = int(max_tips_per_level)
+    c.max_events_per_find = int(max_events_per_find)
     return c
+
+
+@dataclass
+class EventBatch:
+    """B events concatenated for one ckf_find (include/ckf.h, ckf_measurements): virtual module ids
+    event * n_modules + module in `module_offsets` and `seed_module`; `seed_ranges` / `meas_ranges` split the results."""
+    n_events: int
+    module_offsets: np.ndarray
+    loc: np.ndarray
+    var: np.ndarray
+    seed_module: np.ndarray
+    seed_params: np.ndarray
+    seed_cov: np.ndarray
+    seed_ranges: list
+    meas_ranges: list
+
+    @property
+    def n_seeds(self) -> int:
+        return int(self.seed_module.shape[0])
+
+    @property
+    def n_measurements(self) -> int:
+        return int(self.loc.shape[0])
+
+
+def concat_events(evs, n_modules: int) -> EventBatch:
+    """Argument marshalling only: concatenates the arrays of independent events into one batch."""
+    offs, mo, so = [], 0, 0
+    seed_ranges, meas_ranges, smod = [], [], []
+    for e, ev in enumerate(evs):
+        off = np.asarray(ev.module_offsets, np.int64)
+        offs.append(off[:-1] + mo if e < len(evs) - 1 else off + mo)
+        meas_ranges.append((mo, mo + ev.n_measurements))
+        seed_ranges.append((so, so + ev.n_seeds))
+        smod.append(np.asarray(ev.seed_module, np.int64) + e * n_modules)
+        mo += ev.n_measurements
+        so += ev.n_seeds
+    return EventBatch(len(evs), np.concatenate(offs).astype(np.int32), np.concatenate([ev.loc for ev in evs]),
+                      np.concatenate([ev.var for ev in evs]), np.concatenate(smod).astype(np.int32),
+                      np.concatenate([ev.seed_params for ev in evs]), np.concatenate([ev.seed_cov for ev in evs]),
+                      seed_ranges, meas_ranges)
 
 
 @dataclass
@@ -189,7 +232,7 @@ class CKF:
 
     def __init__(self, det, fld, ckf, precision: int, max_seeds: int, max_measurements: int,
                  max_tracks: Optional[int] = None, max_track_entries: Optional[int] = None, max_links: int = 0,
-                 n_streams: int = 1, max_tips_per_level: int = 0):
+                 n_streams: int = 1, max_tips_per_level: int = 0, max_events_per_find: int = 1):
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: paper_2505_22822_b200 has no CPU fallback")
@@ -205,7 +248,7 @@ class CKF:
         g = make_geometry(det, keep)
         f = make_field(fld, keep)
         self.config = make_config(ckf, precision, max_seeds, max_measurements, self.max_tracks, self.max_track_entries,
-                                  max_links, n_streams, max_tips_per_level)
+                                  max_links, n_streams, max_tips_per_level, max_events_per_find)
         h = _vp()
         rc = self.lib.ckf_create(C.byref(g), C.byref(f), C.byref(self.config), C.byref(h))
         if rc != 0:
@@ -226,6 +269,7 @@ class CKF:
     def upload_event(self, ev, device="cuda"):
         t = self.torch
         return dict(
+            n_events=int(getattr(ev, "n_events", 1)),
             module_offsets=t.from_numpy(np.ascontiguousarray(ev.module_offsets, np.int32)).to(device),
             loc=t.from_numpy(np.ascontiguousarray(ev.loc, self.ndtype)).to(device),
             var=t.from_numpy(np.ascontiguousarray(ev.var, self.ndtype)).to(device),
@@ -234,7 +278,8 @@ class CKF:
             seed_cov=t.from_numpy(np.ascontiguousarray(ev.seed_cov, self.ndtype)).to(device))
 
     def _structs(self, d, out, ptr):
-        m = ckf_measurements(int(d["loc"].shape[0]), ptr(d["module_offsets"]), ptr(d["loc"]), ptr(d["var"]))
+        m = ckf_measurements(int(d["loc"].shape[0]), ptr(d["module_offsets"]), ptr(d["loc"]), ptr(d["var"]),
+                             int(d.get("n_events", 1)))
         s = ckf_seeds(int(d["seed_module"].shape[0]), ptr(d["seed_module"]), ptr(d["seed_params"]), ptr(d["seed_cov"]))
         o = ckf_tracks(*[ptr(out[k]) for k in ("n_tracks", "status", "track_offsets", "meas_idx", "seed_id", "n_holes",
                                                "last_module", "stop_reason", "params", "cov", "chi2_sum",
@@ -289,7 +334,7 @@ class CKF:
 
     def pinned_event(self, ev):
         d = self.upload_event(ev, device="cpu")
-        return {k: v.pin_memory() for k, v in d.items()}
+        return {k: (v.pin_memory() if hasattr(v, "pin_memory") else v) for k, v in d.items()}
 
     def pinned_tracks(self):
         d = self.alloc_tracks(device="cpu")

@@ -141,6 +141,7 @@ void fill_params(ckf_handle* h, Workspace& w, KParams<T>& p) {
   const size_t S = (size_t)c.max_seeds;
   p.sd_extra = w.sd; p.sd_nemit = w.sd + S; p.sd_nentries = w.sd + 2 * S;
   p.sd_track_base = w.sd + 3 * S; p.sd_entry_base = w.sd + 3 * S + (S + 1);
+  p.sd_eoff = w.sd + 3 * S + 2 * (S + 1);
   p.seed_tile = w.seed_tile; p.seed_tiles_cap = (int32_t)((S + SEED_TILE - 1) / SEED_TILE);
   const size_t LC = S * (size_t)c.max_candidates_per_seed;
   p.leaf_link = w.leaf; p.leaf_meta = w.leaf + LC; p.leaf_entry = w.leaf + 2 * LC;
@@ -165,6 +166,7 @@ int launch_find(ckf_handle* h, Workspace& w, const ckf_measurements* m, const ck
   fill_params<T>(h, w, p);
   p.n_meas = m->n; p.n_seeds = s->n;
   p.moff = m->module_offsets;
+  p.n_vmod = std::max(1, m->n_events) * h->n_modules;
   p.loc = (const typename Vec2<T>::type*)m->loc;
   p.var = (const typename Vec2<T>::type*)m->var;
   p.seed_module = s->module_id; p.seed_x = (const T*)s->params; p.seed_C = (const T*)s->cov;
@@ -326,6 +328,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     return fail(h, CKF_E_CUDA, "no CUDA device: this library has no CPU fallback");
   h = new ckf_handle();
   h->cfg = *c;
+  if (h->cfg.max_events_per_find <= 0) h->cfg.max_events_per_find = 1;
   if (h->cfg.max_links <= 0) h->cfg.max_links = (int32_t)std::min<long long>(48LL * c->max_seeds, 0x7ffffff0LL);
   h->tsize = c->precision == 32 ? 4 : 8;
   auto bail = [&](int code) { std::string e = h->err; ckf_destroy(h); g_create_error = e; return code; };
@@ -416,7 +419,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     CKB(dalloc(h, &w.lk_module, L * 4)); CKB(dalloc(h, &w.lk_parent, L * 4)); CKB(dalloc(h, &w.lk_meas, L * 4));
     CKB(dalloc(h, &w.lk_counts, L * 4)); CKB(dalloc(h, &w.lk_lastmeas, L * 4));
     CKB(dalloc(h, (char**)&w.lk_chi2, L * ts)); CKB(dalloc(h, (char**)&w.lk_chi2sum, L * ts));
-    CKB(dalloc(h, &w.sd, (3 * S + 2 * (S + 1)) * 4));
+    CKB(dalloc(h, &w.sd, (4 * S + 2 * (S + 1)) * 4));
     CKB(dalloc(h, &w.seed_tile, 2 * ((S + SEED_TILE - 1) / SEED_TILE + 2) * 4));
     CKB(dalloc(h, &w.leaf, 3 * S * (size_t)c->max_candidates_per_seed * 4));
     const size_t TC = (size_t)h->tcap, KB = (size_t)c->max_branches_per_surface;
@@ -433,7 +436,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     CKB(dalloc(h, (char**)&w.s_loc, 2 * (size_t)c->max_measurements * ts));
     CKB(dalloc(h, (char**)&w.s_var, 2 * (size_t)c->max_measurements * ts));
     CKB(dalloc(h, &w.s_idx, (size_t)c->max_measurements * 4));
-    CKB(dalloc(h, (char**)&w.s_v0max, (size_t)g->n_modules * ts));
+    CKB(dalloc(h, (char**)&w.s_v0max, (size_t)g->n_modules * (size_t)h->cfg.max_events_per_find * ts));
     CKB(dalloc(h, &w.globals, 64 * 4));
     static_assert(G_N <= 32, "globals block too small (ckf_fit keeps two of them in 64 ints)");
     CKB(dalloc(h, &w.mv_order, (size_t)NBIN * TC * 4));
@@ -441,7 +444,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     CKB(cudaEventCreateWithFlags(&w.done, cudaEventDisableTiming));
     // staging for ckf_find_host
     const size_t M = (size_t)c->max_measurements, NTK = (size_t)c->max_tracks, NE = (size_t)c->max_track_entries;
-    CKB(dalloc(h, &w.h_moff, ((size_t)g->n_modules + 1) * 4));
+    CKB(dalloc(h, &w.h_moff, ((size_t)g->n_modules * (size_t)h->cfg.max_events_per_find + 1) * 4));
     CKB(dalloc(h, (char**)&w.h_loc, 2 * M * ts)); CKB(dalloc(h, (char**)&w.h_var, 2 * M * ts));
     CKB(dalloc(h, &w.h_smod, S * 4)); CKB(dalloc(h, (char**)&w.h_sx, 6 * S * ts)); CKB(dalloc(h, (char**)&w.h_sC, 36 * S * ts));
     CKB(dalloc(h, &w.o_nt, 2 * 4)); CKB(dalloc(h, &w.o_off, (NTK + 1) * 4)); CKB(dalloc(h, &w.o_meas, NE * 4));
@@ -460,6 +463,8 @@ int ckf_find(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, ckf_t
   if (!h) return CKF_E_ARG;
   if (!m || !s || !o) return fail(h, CKF_E_ARG, "null argument");
   if (m->n < 0 || s->n < 0) return fail(h, CKF_E_ARG, "negative size");
+  if (m->n_events < 0 || m->n_events > h->cfg.max_events_per_find)
+    return fail(h, CKF_E_CAPACITY, "n_events %d exceeds max_events_per_find %d", m->n_events, h->cfg.max_events_per_find);
   if (s->n > h->cfg.max_seeds || m->n > h->cfg.max_measurements)
     return fail(h, CKF_E_CAPACITY, "n_seeds %d / n_measurements %d exceed capacity %d / %d", s->n, m->n,
                 h->cfg.max_seeds, h->cfg.max_measurements);
@@ -480,16 +485,19 @@ int ckf_find_host(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, 
   if (!m || !s || !o) return fail(h, CKF_E_ARG, "null argument");
   if (m->n < 0 || s->n < 0 || s->n > h->cfg.max_seeds || m->n > h->cfg.max_measurements)
     return fail(h, CKF_E_CAPACITY, "n_seeds %d / n_measurements %d exceed capacity", s->n, m->n);
+  if (m->n_events < 0 || m->n_events > h->cfg.max_events_per_find)
+    return fail(h, CKF_E_CAPACITY, "n_events %d exceeds max_events_per_find %d", m->n_events, h->cfg.max_events_per_find);
   cudaStream_t st = (cudaStream_t)stream;
   Workspace* w = acquire_ws(h, st);
   const size_t ts = (size_t)h->tsize;
-  CK(cudaMemcpyAsync(w->h_moff, m->module_offsets, ((size_t)h->n_modules + 1) * 4, cudaMemcpyHostToDevice, st));
+  CK(cudaMemcpyAsync(w->h_moff, m->module_offsets, ((size_t)h->n_modules * (size_t)std::max(1, m->n_events) + 1) * 4,
+                     cudaMemcpyHostToDevice, st));
   CK(cudaMemcpyAsync(w->h_loc, m->loc, 2 * (size_t)m->n * ts, cudaMemcpyHostToDevice, st));
   CK(cudaMemcpyAsync(w->h_var, m->var, 2 * (size_t)m->n * ts, cudaMemcpyHostToDevice, st));
   CK(cudaMemcpyAsync(w->h_smod, s->module_id, (size_t)s->n * 4, cudaMemcpyHostToDevice, st));
   CK(cudaMemcpyAsync(w->h_sx, s->params, 6 * (size_t)s->n * ts, cudaMemcpyHostToDevice, st));
   CK(cudaMemcpyAsync(w->h_sC, s->cov, 36 * (size_t)s->n * ts, cudaMemcpyHostToDevice, st));
-  ckf_measurements dm = {m->n, w->h_moff, w->h_loc, w->h_var};
+  ckf_measurements dm = {m->n, w->h_moff, w->h_loc, w->h_var, m->n_events};
   ckf_seeds ds = {s->n, w->h_smod, w->h_sx, w->h_sC};
   ckf_tracks dt = {w->o_nt, w->o_nt + 1, w->o_off, w->o_meas, w->o_seed, w->o_nh, w->o_lm, w->o_stop,
                    w->o_par, w->o_cov, w->o_c2, w->o_ec2};

@@ -12,6 +12,7 @@ __global__ void ckf_init_event(const KParams<T> p) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < p.n_seeds) {
     p.sd_extra[i] = 0; p.sd_nemit[i] = 0; p.sd_nentries[i] = 0;
+    p.sd_eoff[i] = (p.seed_module[i] / p.geo.n_modules) * p.geo.n_modules;
     if (i < p.tcap) { p.tip_link[i] = -1; p.tip_seed[i] = i; p.mv_stop[i] = STOP_NONE; }
   }
   if (i == 0) {

@@ -74,6 +74,8 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, con
   int bin = -1;
   if (s < p.chunk && tr < nt && (level == 0 || p.o_status[tr] == FIT_RUNNING)) {
     const int e0 = p.offsets[tr], n = p.offsets[tr + 1] - e0;
+    const int sd0 = p.seed[tr];
+    const int eoff = (p.seed_module[sd0] / p.geo.n_modules) * p.geo.n_modules;  // batch of events: see KParams::n_vmod
     double xp[6], xf[6];
     T Cp[21], Cf[21], J[5][5];
     int status = STOP_NONE, module = 0, next = 0, stored = level;
@@ -84,7 +86,7 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, con
 #pragma unroll
     for (int i = 0; i < 21; ++i) Cf[i] = T(0);
     if (level == 0) {  // N6: the seed's own module, identity transport
-      const int sd = p.seed[tr];
+      const int sd = sd0;
       bool ok = true;
 #pragma unroll
       for (int i = 0; i < 6; ++i) { xp[i] = (double)p.seed_x[(size_t)sd * 6 + i]; ok = ok && isfinite(xp[i]); }
@@ -97,7 +99,7 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, con
       for (int a = 0; a < 5; ++a)
 #pragma unroll
         for (int b = 0; b < 5; ++b) J[a][b] = (a == b && a < 4) ? T(1) : T(0);
-      module = p.seed_module[sd];
+      module = p.seed_module[sd] - eoff;
       if (n < 1) done = true;
       else if (!ok) status = STOP_NUMERIC;
     } else {
@@ -147,7 +149,7 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, con
     if (status == STOP_NONE && !done) {
       const int k = p.meas[e0 + next];
       int used = -1;
-      if (k >= p.moff[module] && k < p.moff[module + 1]) {
+      if (k >= p.moff[eoff + module] && k < p.moff[eoff + module + 1]) {
         const typename Vec2<T>::type mm = p.loc[k], vv = p.var[k];
         const double c2 = predicted_chi2<double>(xp[0], xp[1], (double)Cp[tri(0, 0)], (double)Cp[tri(0, 1)],
                                                  (double)Cp[tri(1, 1)], (double)mm.x, (double)mm.y, (double)vv.x, (double)vv.y);

@@ -54,7 +54,10 @@ struct KParams {
   CfgDev cfg;
   // event (caller's device buffers)
   int32_t n_meas, n_seeds;
-  const int32_t* moff;
+  const int32_t* moff;             // [n_vmod + 1]
+  int32_t n_vmod;                  // n_events * n_modules: a batch of events is ONE find over replicas of the detector
+                                   // (virtual module id = event * n_modules + module; only the CSR of measurements and
+                                   // the seeds' module ids use virtual ids, geometry and navigation use real ones)
   const typename Vec2<T>::type* loc;
   const typename Vec2<T>::type* var;
   const int32_t* seed_module;
@@ -64,7 +67,7 @@ struct KParams {
   typename Vec2<T>::type* s_loc;   // [n_meas]
   typename Vec2<T>::type* s_var;   // [n_meas]
   int32_t* s_idx;                  // [n_meas] position in the caller's arrays (what meas_idx reports)
-  T* s_v0max;                      // [n_modules] largest var0 of the slice; < 0 = slice left unsorted
+  T* s_v0max;                      // [n_vmod] largest var0 of the slice; < 0 = slice left unsorted
   // candidate-link buffer (a10): SoA, one entry per child ever made; a level's links are contiguous
   int32_t max_links;
   double* lk_x;        // [6][max_links]   bound parameters after the visit
@@ -77,6 +80,7 @@ struct KParams {
   int32_t* lk_counts;  // n_meas | n_holes << 16
   int32_t* lk_lastmeas;  // link of the branch's last measurement (state reported on emission)
   // per seed
+  int32_t* sd_eoff;      // event * n_modules of the seed's event: real module id + sd_eoff = virtual module id
   int32_t* sd_extra;     // leaves - 1 (R10)
   int32_t* sd_nemit;     // emitted candidates so far
   int32_t* sd_nentries;  // their measurement entries so far

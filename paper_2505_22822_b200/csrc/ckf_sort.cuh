@@ -63,9 +63,9 @@ __global__ void __launch_bounds__(SORT_NT) ckf_sort_slices(const KParams<T> p) {
   __shared__ int s_bad;
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
   constexpr int MPB = SORT_NT / 32;  // small modules taken per block and round, one per warp
-  for (int m0 = blockIdx.x * MPB; m0 < p.geo.n_modules; m0 += gridDim.x * MPB) {
+  for (int m0 = blockIdx.x * MPB; m0 < p.n_vmod; m0 += gridDim.x * MPB) {
     const int mw = m0 + warp;
-    if (mw < p.geo.n_modules) {
+    if (mw < p.n_vmod) {
       const int begw = __ldg(p.moff + mw), nw = __ldg(p.moff + mw + 1) - begw;
       if (nw <= 32) sort_slice_warp<T>(p, mw, begw, nw, lane);
     }
@@ -73,7 +73,7 @@ __global__ void __launch_bounds__(SORT_NT) ckf_sort_slices(const KParams<T> p) {
   // long slices: one block per module, consecutive modules on different blocks (the crowded inner-layer
   // modules have consecutive ids)
   {
-    for (int m = blockIdx.x; m < p.geo.n_modules; m += gridDim.x) {
+    for (int m = blockIdx.x; m < p.n_vmod; m += gridDim.x) {
       const int beg = __ldg(p.moff + m), end = __ldg(p.moff + m + 1), n = end - beg;
       if (n <= 32) continue;
       __syncthreads();

@@ -190,7 +190,7 @@ __global__ void __launch_bounds__(VISIT_NT, MINB) ckf_visit(const KParams<T> p, 
             s.pC[tri(i, j) * 32 + lane] = c;
             p.pd_C[tri(i, j) * TC + t] = c;
           }
-        target = p.seed_module[seed];
+        target = p.seed_module[seed] - p.sd_eoff[seed];
         p.mv_tgt[t] = target;
         if (!ok) stop = STOP_NUMERIC;
       } else {
@@ -240,11 +240,12 @@ __global__ void __launch_bounds__(VISIT_NT, MINB) ckf_visit(const KParams<T> p, 
         }
       }
     }
-    s.target[lane] = target;
+    const int vtarget = (act && target >= 0) ? target + p.sd_eoff[tseed[t]] : target;  // slice of the tip's own event
+    s.target[lane] = vtarget;
     __syncwarp();
     const bool visit = act && stop == STOP_NONE;
     if (visit) {
-      my_gate += (unsigned long long)(__ldg(p.moff + target + 1) - __ldg(p.moff + target));
+      my_gate += (unsigned long long)(__ldg(p.moff + vtarget + 1) - __ldg(p.moff + vtarget));
       my_visits += 1ull;
     }
     const int nsel = gate_chunk<T>(p, s, lane, visit, K, w_exec);

@@ -89,3 +89,22 @@ def compare_fits(gpu: dict, ora, track_offsets):
                 max_first_cov_scaled=float(cov.max(initial=0.0)),
                 max_chi2_abs=float(np.abs(gpu["chi2_sum"] - ora.chi2_sum).max(initial=0.0)),
                 table1_first=[float(np.mean(rel_first <= tol)) if first.size else 1.0 for tol in (1e-4, 1e-3, 1e-2, 5e-2)])
+
+
+def split_batch(tr, batch):
+    """Per-event views of the candidates of a batched ckf_find (paper_2505_22822_b200.EventBatch): seed ids, entry
+    offsets and measurement indices rebased to the event's own arrays.  Returns [(TrackArrays-like, t0, t1, e0)]."""
+    from types import SimpleNamespace
+    out = []
+    for (s0, s1), (m0, _m1) in zip(batch.seed_ranges, batch.meas_ranges):
+        t0 = int(np.searchsorted(tr.seed_id, s0, side="left"))
+        t1 = int(np.searchsorted(tr.seed_id, s1, side="left"))
+        e0, e1 = int(tr.track_offsets[t0]), int(tr.track_offsets[t1])
+        v = SimpleNamespace(n_tracks=t1 - t0, track_offsets=tr.track_offsets[t0:t1 + 1] - e0,
+                            meas_idx=tr.meas_idx[e0:e1] - m0, entry_chi2=tr.entry_chi2[e0:e1],
+                            seed_id=tr.seed_id[t0:t1] - s0, n_holes=tr.n_holes[t0:t1], last_module=tr.last_module[t0:t1],
+                            stop_reason=tr.stop_reason[t0:t1], params=tr.params[t0:t1], cov=tr.cov[t0:t1],
+                            chi2_sum=tr.chi2_sum[t0:t1])
+        v.meas_list = lambda t, v=v: v.meas_idx[v.track_offsets[t]:v.track_offsets[t + 1]]
+        out.append((v, t0, t1, e0))
+    return out

@@ -346,3 +346,63 @@ def test_fit_float32_smoother_study():
     # the forward pass does not depend on the smoother's arithmetic
     assert np.array_equal(g32["last_params"][both], g64["last_params"][both])
     ckf.close()
+
+
+# ---------------------------------------------------------------------------------- batches of events in one ckf_find
+def _batch_run(config, sizes):
+    import torch
+    from paper_2505_22822_b200 import CKF, concat_events
+    det, fld, cfg = synth.config_bundle(config)
+    evs = [synth.make_event(config, event_index=7 + i, det=det, n_particles=n) for i, n in enumerate(sizes)]
+    batch = concat_events(evs, det.n_modules)
+    ckf = CKF(det, fld, cfg.ckf, cfg.precision, max_seeds=batch.n_seeds, max_measurements=batch.n_measurements,
+              max_events_per_find=len(evs))
+    dev, out = ckf.upload_event(batch), ckf.alloc_tracks()
+    ckf.find(dev, out)
+    torch.cuda.synchronize()
+    return det, fld, cfg, evs, batch, ckf, dev, out, ckf.download(out)
+
+
+def test_batch_of_events_equals_separate_events_fp64():
+    """include/ckf.h, ckf_measurements: B events in one ckf_find (virtual module ids) give, per event, exactly the
+    candidates of the event alone -- checked against the oracle run on each event separately; ckf_fit likewise."""
+    import torch
+    import oracle
+    det, fld, cfg, evs, batch, ckf, dev, out, gpu = _batch_run(1, (300, 500, 200))
+    assert gpu.status == 0
+    fits = ckf.alloc_fits()
+    ckf.fit(dev, out, fits)
+    torch.cuda.synchronize()
+    gf = ckf.download_fits(fits, gpu.n_tracks, int(gpu.meas_idx.size))
+    st = oracle.Setup(det, fld, cfg.ckf)
+    total = 0
+    for ev, (v, t0, t1, e0) in zip(evs, parity.split_batch(gpu, batch)):
+        ora = oracle.find_event(st, ev, n_threads=8)
+        parity.assert_bit_exact_lists(v, ora)
+        rel, chi2, _ = parity.max_param_diffs(v, ora)
+        assert rel < 1e-9 and chi2 < 1e-8, (rel, chi2)
+        of = oracle.kf_fit(st, ev, ora.track_offsets, ora.meas_idx, ora.seed_id, n_threads=8)
+        ne = int(ora.meas_idx.size)
+        g = {k: (a[e0:e0 + ne] if k == "entry_params" else a[t0:t1]) for k, a in gf.items() if k != "work"}
+        r = parity.compare_fits(g, of, ora.track_offsets)
+        assert r["n_failed"] == 0 and r["max_smoothed_rel"] < 1e-9, r
+        total += ora.n_tracks
+    assert total == gpu.n_tracks
+    # more events than the handle was created for is refused
+    import pytest
+    dev["n_events"] = 4
+    with pytest.raises(RuntimeError, match="max_events_per_find"):
+        ckf.find(dev, out)
+    ckf.close()
+
+
+def test_batch_of_events_fp32():
+    import oracle
+    det, fld, cfg, evs, batch, ckf, dev, out, gpu = _batch_run(2, (1500, 2500))
+    assert gpu.status == 0
+    st = oracle.Setup(det, fld, cfg.ckf)
+    for ev, (v, t0, t1, e0) in zip(evs, parity.split_batch(gpu, batch)):
+        ora = oracle.find_event(st, ev, n_threads=8)
+        r = parity.compare_fp32(v, ora, ev.n_seeds)
+        assert r["frac_identical"] >= 0.999 and r["max_param_rel"] < 1e-4 and r["max_chi2_sum_abs"] < 1e-3, r
+    ckf.close()
