@@ -152,7 +152,8 @@ def main():
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--no-cpu-baseline", action="store_true")
-    ap.add_argument("--streams", type=int, default=4, help="events kept in flight (CUDA streams) for `value`")
+    ap.add_argument("--streams", type=int, default=2, help="batches kept in flight (CUDA streams) for `value`")
+    ap.add_argument("--batch", type=int, default=4, help="independent events per ckf_find (one step = one batch)")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -176,27 +177,36 @@ def main():
     max_s = max(e.n_seeds for e in evs)
     max_m = max(e.n_measurements for e in evs)
     S = max(1, args.streams)
-    ckf = CKF(det, fld, cfg.ckf, cfg.precision, max_seeds=max_s, max_measurements=max_m, max_tracks=8 * max_s,
-              max_track_entries=80 * max_s, n_streams=max(S, E2E_STREAMS) + 1)
+    B = max(1, min(args.batch, N_EVENTS))
+    # one step = one ckf_find over a BATCH of B independent events (include/ckf.h, ckf_measurements.n_events): the
+    # level loop then runs over the tips of all B events, which shares its per-level cost
+    from paper_2505_22822_b200 import concat_events
+    batches = [concat_events([evs[(i + j) % N_EVENTS] for j in range(B)], det.n_modules) for i in range(N_EVENTS)]
+    ckf = CKF(det, fld, cfg.ckf, cfg.precision, max_seeds=B * max_s, max_measurements=B * max_m, max_tracks=8 * B * max_s,
+              max_track_entries=80 * B * max_s, n_streams=max(S, E2E_STREAMS) + 1, max_events_per_find=B)
     devs = [ckf.upload_event(e) for e in evs]
+    bdevs = [ckf.upload_event(b) for b in batches]
     stream = torch.cuda.current_stream()
     work = [torch.cuda.Stream() for _ in range(S)]
     outs = [ckf.alloc_tracks() for _ in range(S)]
     out = outs[0]
 
-    # one step = one ckf_find over one event; the K steps are independent events, kept S at a time in flight on S
-    # CUDA streams (the paper's own throughput mode: one event pipeline per stream)
+    # the K steps are independent batches, kept S at a time in flight on S CUDA streams (the paper's own throughput
+    # mode: one event pipeline per stream)
     def run_steps(k):
         for i in range(k):
-            ckf.find(devs[i % N_EVENTS], outs[i % S], work[i % S])
+            ckf.find(bdevs[i % N_EVENTS], outs[i % S], work[i % S])
 
     W = max(3, args.warmup)
-    for i in range(W):
-        ckf.find(devs[i % N_EVENTS], out, stream)
-    torch.cuda.synchronize()
-    cnt = ckf.counters(stream)                      # of event (warmup-1) % N
-    res = ckf.download(out)
     ev_last = evs[(W - 1) % N_EVENTS]
+    ckf.find(devs[(W - 1) % N_EVENTS], out, stream)  # that event alone: parity check and e2e byte counts below
+    torch.cuda.synchronize()
+    res1 = ckf.download(out)
+    for i in range(W):
+        ckf.find(bdevs[i % N_EVENTS], out, stream)
+    torch.cuda.synchronize()
+    cnt = ckf.counters(stream)                      # of batch (warmup-1) % N: the B events starting at ev_last
+    res = ckf.download(out)
     run_steps(S)                                    # warm the per-stream workspaces
     torch.cuda.synchronize()
 
@@ -219,7 +229,7 @@ def main():
     if world > 1:
         dist.barrier()
     ms_total = t0.elapsed_time(t1)
-    seeds_done = sum(evs[i % N_EVENTS].n_seeds for i in range(args.steps))
+    seeds_done = sum(batches[i % N_EVENTS].n_seeds for i in range(args.steps))
 
     # single-event latency (one stream, finds back to back) and the per-kernel device times of the dominant
     # kernel, ckf_step, measured live with CUDA events on the launching stream (ckf_set_timing)
@@ -234,13 +244,13 @@ def main():
     ckf.set_timing(True)
     tim = []
     for i in range(min(args.steps, 8)):
-        ckf.find(devs[(W - 1) % N_EVENTS], out, stream)
+        ckf.find(bdevs[(W - 1) % N_EVENTS], out, stream)
         torch.cuda.synchronize()
         tim.append(ckf.timing(stream))
     ckf.set_timing(False)
     # ---- next row: KF fit + RTS smoother of that event's candidates (ckf_fit)
     fits = ckf.alloc_fits()
-    dev_last = devs[(W - 1) % N_EVENTS]
+    dev_last = bdevs[(W - 1) % N_EVENTS]
     for _ in range(2):
         ckf.fit(dev_last, out, fits, stream)
     torch.cuda.synchronize()
@@ -285,7 +295,7 @@ def main():
     dt_e2e = run_e2e(n_e2e)
     e2e_seeds = sum(evs[i % N_EVENTS].n_seeds for i in range(n_e2e))
     tsize = 4 if cfg.precision == 32 else 8
-    bi, bo = algorithmic_bytes(ev_last, res.n_tracks, int(res.meas_idx.size), tsize)
+    bi, bo = algorithmic_bytes(ev_last, res1.n_tracks, int(res1.meas_idx.size), tsize)
 
     value, ms_step = aggregate_throughput(seeds_done, ms_total, args.steps, world)
     e2e_value, _ = aggregate_throughput(e2e_seeds, dt_e2e * 1e3, n_e2e, world)
@@ -311,31 +321,36 @@ def main():
             "steps": args.steps, "warmup": max(3, args.warmup), "ms_per_step": ms_step, "higher_is_better": True,
             "scaling": "weak", "vs_baseline": None, "dtype": "f32 covariance/Jacobian + f64 trajectory",
             "data": "synthetic",
-            "config": {"workload": "configs[3]: 40,000 particles + 4,000 fake seeds, 1 event per step, fp32 arrays, "
+            "config": {"workload": "configs[3]: 40,000 particles + 4,000 fake seeds per event, %d independent events per "
+                                   "step (one batched ckf_find), fp32 arrays, " % B +
                                    "float32 grid field, k=10, cap=100", "seeds_per_event": ev_last.n_seeds,
                        "measurements_per_event": ev_last.n_measurements, "distinct_events_rotated": N_EVENTS,
                        "l2": "4 events rotated; each step writes a >190 MB link buffer (> 126 MB L2)",
-                       "events_in_flight": S, "how": "K independent events, S at a time on S CUDA streams, device "
+                       "events_per_step": B, "batches_in_flight": S,
+                       "how": "K independent batches of B events, S at a time on S CUDA streams, device "
                        "timed from the first launch to the last completion", "launch": ckf.launch_info()},
             "latency_ms_single_event": k_ms, "seeds_per_s_single_stream": ev_last.n_seeds / (k_ms * 1e-3),
             "events_per_s": value / ev_last.n_seeds,
             "e2e": {"value": e2e_value, "unit": "seeds/s", "h2d_bytes_per_step": int(bi), "d2h_bytes_per_step": int(bo),
                     "streams": E2E_STREAMS, "events": n_e2e, "events_per_s": e2e_value / ev_last.n_seeds,
                     "how": "ckf_find_host, pinned host buffers, 4 host threads x 4 CUDA streams, wall clock"},
-            "fit": {"what": "ckf_fit: Kalman-filter fit + RTS smoother of every candidate of one configs[3] event "
-                            "(next row, SURVEY.md 8(f) rank 1); device-resident, CUDA events, mean of 5",
-                    "value": res.n_tracks / (fit_ms * 1e-3), "unit": "tracks/s", "ms_per_event": fit_ms,
+            "fit": {"what": "ckf_fit: Kalman-filter fit + RTS smoother of every candidate of one step's batch of configs[3] "
+                            "events (next row, SURVEY.md 8(f) rank 1); device-resident, CUDA events, mean of 5",
+                    "value": res.n_tracks / (fit_ms * 1e-3), "unit": "tracks/s", "ms_per_event": fit_ms / B,
+                    "ms_per_step": fit_ms,
                     "tracks": res.n_tracks, "fitted": fit_ok, "entries": int(res.meas_idx.size),
                     "work": dict(zip(("rk_trials", "rk_accepted", "moves", "updates"), fit_work)), "states": fit_states,
                     "flop_per_event": fit_flop, "achieved_tflops": fit_flop / (fit_ms * 1e-3) / 1e12,
-                    "launches": "2 kernels (forward filter, RTS smoother) per pass of 131,072 candidates"},
+                    "launches": "per pass of 262,144 candidates: ckf_step + ckf_fit_level per level, then ckf_fit_smooth"},
+            "ms_per_event": ms_step / B,
             "gpu_launches": launches_per_find * args.steps,
             "clocks": clocks,
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                          "traffic": None, "kernel": "ckf_step (all %d launches of one find)" % step_launches,
                          "flop_per_find_this_kernel": step_flop, "kernel_ms_per_find": step_ms,
                          "share_of_find": step_ms / max(sum(v for k, v in tim[0].items() if k.endswith("_ms")), 1e-9),
-                         "whole_path_flop_per_find": flop, "whole_path_tflops": flop / (k_ms * 1e-3) / 1e12,
+                         "whole_path_flop_per_find": flop,
+                         "whole_path_tflops": flop / max(sum(v for k, v in tim[0].items() if k.endswith("_ms")) * 1e-3, 1e-12) / 1e12,
                          "kernel_ms_by_phase": {k: float(np.mean([t[k] for t in tim])) for k in tim[0] if k.endswith("_ms")},
                          "fp64_share_of_flop": f64_share, "peak_fp32": PEAK_FP32_TFLOPS, "peak_fp64": PEAK_FP64_TFLOPS,
                          "peak_source": "derived from the guide's unit counts and max clock (DESIGN.md §7); "
@@ -353,9 +368,9 @@ def main():
             line["cpu_baseline"] = {"value": ev_last.n_seeds / dt, "unit": "seeds/s", "cores": cores, "kind": "oracle",
                                     "sample": "one full configs[3] event (%d seeds), %d host threads, %.2f s" %
                                               (ev_last.n_seeds, cores, dt)}
-            line["parity_in_bench"] = {"n_tracks_gpu": res.n_tracks, "n_tracks_oracle": ora.n_tracks,
-                                       "index_lists_identical": bool(res.n_tracks == ora.n_tracks and
-                                                                     np.array_equal(res.meas_idx, ora.meas_idx))}
+            line["parity_in_bench"] = {"n_tracks_gpu": res1.n_tracks, "n_tracks_oracle": ora.n_tracks,
+                                       "index_lists_identical": bool(res1.n_tracks == ora.n_tracks and
+                                                                     np.array_equal(res1.meas_idx, ora.meas_idx))}
         print(json.dumps(line))
     ckf.close()
     if world > 1:
