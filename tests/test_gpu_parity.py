@@ -263,7 +263,7 @@ def _fit_both(config, n_particles=None):
 def test_fit_fp64_parity(config):
     ckf, dev, out, fits, gpu, g, o, r = _fit_both(config)
     print("fit config", config, r)
-    assert r["n_fitted"] == gpu.n_tracks and gpu.n_tracks > 0
+    assert r["n_fitted"] == gpu.n_tracks and gpu.n_tracks > 0 and r["n_not_pd_gpu_only"] == 0
     assert r["max_last_rel"] < 1e-9 and r["max_chi2_abs"] < 1e-8
     assert r["max_smoothed_rel"] < 1e-9, r        # same bar as the CKF parameters (north_star, fp64)
     assert r["max_first_cov_scaled"] < 1e-6, r
@@ -288,7 +288,7 @@ def test_fit_fp64_parity(config):
 def test_fit_fp32_parity(config):
     ckf, dev, out, fits, gpu, g, o, r = _fit_both(config)
     print("fit config", config, r)
-    assert r["n_fitted"] >= 0.999 * gpu.n_tracks
+    assert r["n_fitted"] >= 0.999 * gpu.n_tracks and r["n_not_pd_gpu_only"] <= 1e-4 * gpu.n_tracks
     assert r["max_last_rel"] < 1e-4 and r["max_chi2_abs"] < 1e-3      # north_star's fp32 bar for parameters / chi2
     assert r["max_smoothed_rel"] < 1e-4, r
     assert r["table1_first"][0] == 1.0, r
@@ -405,4 +405,28 @@ def test_batch_of_events_fp32():
         ora = oracle.find_event(st, ev, n_threads=8)
         r = parity.compare_fp32(v, ora, ev.n_seeds)
         assert r["frac_identical"] >= 0.999 and r["max_param_rel"] < 1e-4 and r["max_chi2_sum_abs"] < 1e-3, r
+    ckf.close()
+
+
+def test_fit_fp32_covariance_not_positive_definite_is_flagged():
+    """configs[3], event index 1: three candidates of one fake seed (3 measurements, 4 holes) have a float32-stored
+    predicted covariance that is not positive definite any more; ckf_fit must flag them NUMERIC with zeros (never
+    report numbers), the float64 oracle fits them; everything else agrees as usual."""
+    import torch
+    import oracle
+    det, fld, cfg = synth.config_bundle(3)
+    ev = synth.make_event(3, event_index=1, det=det)
+    ckf, dev, out, gpu, _ = _run_gpu(det, fld, cfg, ev)
+    fits = ckf.alloc_fits()
+    ckf.fit(dev, out, fits)
+    torch.cuda.synchronize()
+    g = ckf.download_fits(fits, gpu.n_tracks, int(gpu.meas_idx.size))
+    o = oracle.kf_fit(oracle.Setup(det, fld, cfg.ckf), ev, gpu.track_offsets, gpu.meas_idx, gpu.seed_id, n_threads=16)
+    r = parity.compare_fits(g, o, gpu.track_offsets)
+    print("fit config 3 event 1", r)
+    assert 0 < r["n_not_pd_gpu_only"] <= 1e-4 * gpu.n_tracks
+    bad = np.flatnonzero((g["status"] == 5) & (o.status == 0))
+    for t in bad:
+        assert not g["entry_params"][gpu.track_offsets[t]:gpu.track_offsets[t + 1]].any() and not g["first_cov"][t].any()
+    assert r["max_smoothed_rel"] < 1e-4 and r["max_last_rel"] < 1e-4
     ckf.close()
