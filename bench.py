@@ -154,6 +154,7 @@ def main():
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--streams", type=int, default=2, help="batches kept in flight (CUDA streams) for `value`")
     ap.add_argument("--batch", type=int, default=4, help="independent events per ckf_find (one step = one batch)")
+    ap.add_argument("--e2e-batch", type=int, default=4, help="events per ckf_find_host call of the e2e leg")
     args = ap.parse_args()
     rank = int(os.environ.get("RANK", "0"))
     world = int(os.environ.get("WORLD_SIZE", "1"))
@@ -269,7 +270,10 @@ def main():
     launches_per_find = int(tim[0]["launches"])
 
     # ---- e2e: host buffers through ckf_find_host on 4 streams / 4 host threads (configs[4] shape)
-    hevs = [ckf.pinned_event(e) for e in evs]
+    EB = max(1, min(args.e2e_batch, B))
+    e2e_src = evs if EB == 1 else [concat_events([evs[(i + j) % N_EVENTS] for j in range(EB)], det.n_modules)
+                                   for i in range(N_EVENTS)]
+    hevs = [ckf.pinned_event(e) for e in e2e_src]
     houts = [ckf.pinned_tracks() for _ in range(E2E_STREAMS)]
     streams = [torch.cuda.Stream() for _ in range(E2E_STREAMS)]
     n_e2e = max(E2E_STREAMS * 2, min(args.steps, 16))
@@ -293,7 +297,7 @@ def main():
 
     run_e2e(E2E_STREAMS)
     dt_e2e = run_e2e(n_e2e)
-    e2e_seeds = sum(evs[i % N_EVENTS].n_seeds for i in range(n_e2e))
+    e2e_seeds = sum(e2e_src[i % N_EVENTS].n_seeds for i in range(n_e2e))
     tsize = 4 if cfg.precision == 32 else 8
     bi, bo = algorithmic_bytes(ev_last, res1.n_tracks, int(res1.meas_idx.size), tsize)
 
@@ -332,8 +336,9 @@ def main():
             "latency_ms_single_event": k_ms, "seeds_per_s_single_stream": ev_last.n_seeds / (k_ms * 1e-3),
             "events_per_s": value / ev_last.n_seeds,
             "e2e": {"value": e2e_value, "unit": "seeds/s", "h2d_bytes_per_step": int(bi), "d2h_bytes_per_step": int(bo),
-                    "streams": E2E_STREAMS, "events": n_e2e, "events_per_s": e2e_value / ev_last.n_seeds,
-                    "how": "ckf_find_host, pinned host buffers, 4 host threads x 4 CUDA streams, wall clock"},
+                    "streams": E2E_STREAMS, "calls": n_e2e, "events_per_call": EB, "events": n_e2e * EB, "events_per_s": e2e_value / ev_last.n_seeds,
+                    "how": "ckf_find_host on batches of events_per_call events, pinned host buffers, 4 host threads x 4 CUDA "
+                           "streams (configs[4]: 64 events over 4 streams), H2D and D2H inside, wall clock"},
             "fit": {"what": "ckf_fit: Kalman-filter fit + RTS smoother of every candidate of one step's batch of configs[3] "
                             "events (next row, SURVEY.md 8(f) rank 1); device-resident, CUDA events, mean of 5",
                     "value": res.n_tracks / (fit_ms * 1e-3), "unit": "tracks/s", "ms_per_event": fit_ms / B,

@@ -430,3 +430,17 @@ def test_fit_fp32_covariance_not_positive_definite_is_flagged():
         assert not g["entry_params"][gpu.track_offsets[t]:gpu.track_offsets[t + 1]].any() and not g["first_cov"][t].any()
     assert r["max_smoothed_rel"] < 1e-4 and r["max_last_rel"] < 1e-4
     ckf.close()
+
+
+def test_find_host_on_a_batch_equals_device_path():
+    """ckf_find_host (pinned host buffers, H2D + D2H inside) on a batch of events returns what ckf_find returns."""
+    import torch
+    det, fld, cfg, evs, batch, ckf, dev, out, gpu = _batch_run(2, (400, 700, 300))
+    hev, hout = ckf.pinned_event(batch), ckf.pinned_tracks()
+    ckf.find_host(hev, hout, torch.cuda.current_stream())
+    host = ckf.download(hout)
+    assert host.n_tracks == gpu.n_tracks and host.status == gpu.status
+    for k in ("track_offsets", "meas_idx", "seed_id", "n_holes", "last_module", "stop_reason", "params", "cov", "chi2_sum",
+              "entry_chi2"):
+        assert np.array_equal(getattr(host, k), getattr(gpu, k)), k
+    ckf.close()
