@@ -183,6 +183,29 @@ __device__ __forceinline__ int step_cost_bin(const GeoDev& g, int module, const 
 // per-seed totals parked by ckf_scan.  The child -> parent search is staged: two threads bracket the block's
 // 256 children in the global prefix, the bracket is copied to shared memory, every thread searches there.
 constexpr int UPD_WIN = 1024;
+// The same search by one WARP: every round probes 32 evenly spaced keys at once and keeps the sub-range that brackets c,
+// so a range of n keys costs ceil(log32 n) dependent loads instead of log2 n.  key(i) must be non-decreasing and
+// key(lo) <= c; returns the last i in [lo, hi) with key(i) <= c.
+template <typename F>
+__device__ __forceinline__ int warp_last_le(F key, int lo, int hi, int c, int lane) {
+  while (hi - lo > 1) {
+    const int step = (hi - lo + 31) / 32;
+    const int idx = lo + (lane + 1) * step;
+    const bool le = idx < hi && key(idx) <= c;
+    const int m = __popc(__ballot_sync(0xffffffffu, le));  // the probes that are <= c form a prefix
+    const int nlo = lo + m * step;
+    hi = min(hi, nlo + step);
+    lo = nlo;
+  }
+  return lo;
+}
+template <typename T>
+__device__ __forceinline__ int find_parent_warp(const KParams<T>& p, int n, int nb, int c, int lane) {
+  const int tile = warp_last_le([&](int i) { return p.blk_sum[i]; }, 0, nb, c, lane);
+  const int boff = p.blk_sum[tile];
+  const int a = tile * SCAN_NT, b = min(n, a + SCAN_NT);
+  return warp_last_le([&](int i) { return boff + p.t_kex[i]; }, a, b, c, lane);
+}
 template <typename T>
 __global__ void __launch_bounds__(SCAN_NT) ckf_update(const KParams<T> p, int level) {
   const int n = p.g[G_NTIPS0 + (level & 1)];
@@ -210,8 +233,11 @@ __global__ void __launch_bounds__(SCAN_NT) ckf_update(const KParams<T> p, int le
   for (int c0 = blockIdx.x * SCAN_NT; c0 < nc; c0 += gridDim.x * SCAN_NT) {
     const int c = c0 + threadIdx.x;
     __syncthreads();
-    if (threadIdx.x == 0) s_p[0] = find_parent<T>(p, n, nb, c0);
-    if (threadIdx.x == 32) s_p[1] = find_parent<T>(p, n, nb, min(c0 + SCAN_NT, nc) - 1);
+    if (threadIdx.x < 64) {  // warp 0 brackets the block's first child, warp 1 its last
+      const int w = threadIdx.x >> 5;
+      const int r = find_parent_warp<T>(p, n, nb, w == 0 ? c0 : min(c0 + SCAN_NT, nc) - 1, threadIdx.x & 31);
+      if ((threadIdx.x & 31) == 0) s_p[w] = r;
+    }
     __syncthreads();
     const int p0 = s_p[0], win = s_p[1] - p0 + 1;
     int par;

@@ -28,25 +28,47 @@ CKF_HD bool line_hits_module(const ModuleRec& k, const double r[3], const double
   return true;
 }
 
-// Nearest in-bounds module of the 3x3 neighbourhood (phi wraps, z clamps) of (iphi, iz) on `layer`: the
-// sequential form (host harness).  The kernel evaluates the same nine tests cooperatively, see pick_warp.
+// The same test without early exits: path length, or NaN for "no hit".  Nine of these in a row have no control
+// dependence between them, so the loads of the nine module records overlap (thread-per-tip callers: ckf_update's N2,
+// ckf_fit_level; a chain of nine dependent L2 round trips was 25 % of ckf_update's stall samples).
+CKF_HD double line_test_module(const ModuleRec& k, const double r[3], const double d[3], double s_min) {
+  const double dn = dot3(d, k.n);
+  const double rel[3] = {k.c[0] - r[0], k.c[1] - r[1], k.c[2] - r[2]};
+  const double s = dot3(rel, k.n) / dn;
+  const double q[3] = {r[0] + s * d[0] - k.c[0], r[1] + s * d[1] - k.c[1], r[2] + s * d[2] - k.c[2]};
+  const bool ok = dn > 1e-6 && fabs(dot3(q, k.u)) <= k.half_u && fabs(dot3(q, k.v)) <= k.half_v && s > s_min;
+#if defined(__CUDA_ARCH__)
+  return ok ? s : __longlong_as_double(0x7ff8000000000000LL);
+#else
+  return ok ? s : NAN;
+#endif
+}
+
+// Nearest in-bounds module of the 3x3 neighbourhood (phi wraps, z clamps) of (iphi, iz) on `layer`, one tip per
+// thread.  ckf_step evaluates the same nine tests cooperatively over a warp, see pick_warp.
 CKF_HD int pick_in_neighbourhood(const GeoDev& g, int layer, int iphi, int iz, int exclude, const double r[3],
                                  const double d[3], double s_min) {
   const LayerRec L = g.layer[layer];
+  double sv[9];
+  int idv[9];
+#pragma unroll
+  for (int nb = 0; nb < 9; ++nb) {
+    int ii = iphi + (nb / 3 - 1);
+    ii = ii < 0 ? ii + L.n_phi : (ii >= L.n_phi ? ii - L.n_phi : ii);
+    const int jj = iz + (nb % 3 - 1);
+    const bool valid = jj >= 0 && jj < L.n_z;
+    const int id = L.offset + ii * L.n_z + (valid ? jj : iz);   // an in-range record is read either way
+    const double s = line_test_module(g.mod[id], r, d, s_min);
+    idv[nb] = (valid && id != exclude) ? id : -1;
+    sv[nb] = s;
+  }
   int best = -1;
   double best_s = 0.0;
-  for (int di = -1; di <= 1; ++di) {
-    int ii = iphi + di;
-    ii = ii < 0 ? ii + L.n_phi : (ii >= L.n_phi ? ii - L.n_phi : ii);
-    for (int dj = -1; dj <= 1; ++dj) {
-      const int jj = iz + dj;
-      if (jj < 0 || jj >= L.n_z) continue;
-      const int id = L.offset + ii * L.n_z + jj;
-      if (id == exclude) continue;
-      double s;
-      if (!line_hits_module(g.mod[id], r, d, s_min, s)) continue;
-      if (best < 0 || s < best_s || (s == best_s && id < best)) { best = id; best_s = s; }
-    }
+#pragma unroll
+  for (int nb = 0; nb < 9; ++nb) {   // the sequential rule's order: nearest first, tie -> lower id
+    const double s = sv[nb];
+    const int id = idv[nb];
+    if (id >= 0 && s == s && (best < 0 || s < best_s || (s == best_s && id < best))) { best = id; best_s = s; }
   }
   return best;
 }
