@@ -27,10 +27,10 @@ constexpr int SCAN_NT = 256;      // threads per block of ckf_scan / ckf_update;
 constexpr int SORT_NT = 128;      // threads per block of the slice sort
 constexpr int SORT_CAP = 2048;    // largest module slice sorted in shared memory; larger ones stay unsorted
 #ifndef CKF_FETCH_MIN
-#define CKF_FETCH_MIN 16
+#define CKF_FETCH_MIN 32
 #endif
 #ifndef CKF_PICK_MIN
-#define CKF_PICK_MIN 16
+#define CKF_PICK_MIN 32
 #endif
 constexpr int FETCH_MIN = CKF_FETCH_MIN;  // finished / tip-less lanes that must wait before write-back + fetch run early
 constexpr int PICK_MIN = CKF_PICK_MIN;    // lanes on a portal that must wait before the module choice runs early
