@@ -126,7 +126,10 @@ cudaError_t dalloc(ckf_handle* h, P** p, size_t bytes) {
 #endif
 template <typename T> struct MinBlocks { static constexpr int value = CKF_MINB; };
 template <> struct MinBlocks<double> { static constexpr int value = 2; };
-template <typename T> struct VisitBlocks { static constexpr int value = 4; };
+#ifndef CKF_VISIT_MINB
+#define CKF_VISIT_MINB 4
+#endif
+template <typename T> struct VisitBlocks { static constexpr int value = CKF_VISIT_MINB; };
 template <> struct VisitBlocks<double> { static constexpr int value = 2; };
 
 template <typename T>

@@ -207,7 +207,10 @@ __device__ __forceinline__ int find_parent_warp(const KParams<T>& p, int n, int 
   return warp_last_le([&](int i) { return boff + p.t_kex[i]; }, a, b, c, lane);
 }
 template <typename T>
-__global__ void __launch_bounds__(SCAN_NT) ckf_update(const KParams<T> p, int level) {
+#ifndef CKF_UPDATE_MINB
+#define CKF_UPDATE_MINB 3
+#endif
+__global__ void __launch_bounds__(SCAN_NT, CKF_UPDATE_MINB) ckf_update(const KParams<T> p, int level) {
   const int n = p.g[G_NTIPS0 + (level & 1)];
   if (n == 0) return;
   const int nc = p.g[G_NTIPS0 + ((level + 1) & 1)];
