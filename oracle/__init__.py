@@ -77,11 +77,11 @@ def lib():
         L.oracle_add_material.argtypes = [C.POINTER(OGeometry), C.POINTER(OConfig), C.c_int32, _dp, _dp]
         L.oracle_kf_fit.restype = None
         L.oracle_kf_fit.argtypes = [C.POINTER(OGeometry), C.POINTER(OField), C.POINTER(OConfig), _ip, _dp, _dp, _ip, _dp,
-                                    _dp, C.c_int32, _ip, _ip, _ip, C.c_int32, _ip, _ip, _dp, _dp, _dp, _dp, _dp]
+                                    _dp, C.c_int32, _ip, _ip, _ip, C.c_int32, _ip, _ip, _dp, _dp, _dp, _dp, _dp, C.c_int32]
         L.oracle_kf_fit_states.restype = C.c_int32
         L.oracle_kf_fit_states.argtypes = [C.POINTER(OGeometry), C.POINTER(OField), C.POINTER(OConfig), _ip, _dp, _dp,
                                            C.c_int32, _dp, _dp, C.c_int32, _ip, C.c_int32, _ip, _ip, _dp, _dp, _dp, _dp,
-                                           _dp, _dp, _dp]
+                                           _dp, _dp, _dp, C.c_int32]
         L.oracle_rts_smooth.restype = C.c_int32
         L.oracle_rts_smooth.argtypes = [C.c_int32, _dp, _dp, _dp, _dp, _dp, _dp, _dp]
         _lib = L
@@ -267,7 +267,8 @@ class Fits:
     entry_params: np.ndarray  # [n_entries, 6] smoothed parameters at every measurement of the list
 
 
-def kf_fit(setup: Setup, ev, track_offsets, meas_idx, seed_id, n_threads: int = 1) -> Fits:
+def kf_fit(setup: Setup, ev, track_offsets, meas_idx, seed_id, n_threads: int = 1, smoother: int = 0) -> Fits:
+    """smoother: 0 = RTS recursion (K4), 1 = two-filter 'optimal' smoother (K4')."""
     L = lib()
     mo, lo, va = _i(ev.module_offsets), _d(ev.loc), _d(ev.var)
     sm, sp, sc = _i(ev.seed_module), _d(ev.seed_params), _d(ev.seed_cov)
@@ -279,11 +280,11 @@ def kf_fit(setup: Setup, ev, track_offsets, meas_idx, seed_id, n_threads: int = 
     L.oracle_kf_fit(C.byref(setup.geometry), C.byref(setup.field), C.byref(setup.config), _pi(mo), _pd(lo), _pd(va),
                     _pi(sm), _pd(sp), _pd(sc), nt, _pi(to), _pi(mi), _pi(si), int(n_threads), _pi(out.status),
                     _pi(out.n_states), _pd(out.chi2_sum), _pd(out.last_params), _pd(out.last_cov), _pd(out.first_cov),
-                    _pd(out.entry_params))
+                    _pd(out.entry_params), int(smoother))
     return out
 
 
-def kf_fit_states(setup: Setup, ev, seed: int, meas, max_states: int = 64):
+def kf_fit_states(setup: Setup, ev, seed: int, meas, max_states: int = 64, smoother: int = 0):
     """Every state of one track's fit: dict of module, meas, xp, Cp, xf, Cf, J, xs, Cs (arrays over states)."""
     mo, lo, va = _i(ev.module_offsets), _d(ev.loc), _d(ev.var)
     sx, sC = _d(ev.seed_params[seed]), _d(ev.seed_cov[seed]).reshape(36)
@@ -294,7 +295,8 @@ def kf_fit_states(setup: Setup, ev, seed: int, meas, max_states: int = 64):
     Cp, Cf, J, Cs = np.zeros((n, 36)), np.zeros((n, 36)), np.zeros((n, 36)), np.zeros((n, 36))
     ns = lib().oracle_kf_fit_states(C.byref(setup.geometry), C.byref(setup.field), C.byref(setup.config), _pi(mo),
                                     _pd(lo), _pd(va), int(ev.seed_module[seed]), _pd(sx), _pd(sC), me.shape[0], _pi(me),
-                                    n, _pi(mod), _pi(mu), _pd(xp), _pd(Cp), _pd(xf), _pd(Cf), _pd(J), _pd(xs), _pd(Cs))
+                                    n, _pi(mod), _pi(mu), _pd(xp), _pd(Cp), _pd(xf), _pd(Cf), _pd(J), _pd(xs), _pd(Cs),
+                                    int(smoother))
     if ns < 0:
         return {"status": -ns}
     ns = min(ns, n)

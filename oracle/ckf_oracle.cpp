@@ -781,6 +781,7 @@ struct FitState {
   int module, meas;
   double chi2;
   double xp[6], Cp[6][6], xf[6], Cf[6][6], J[6][6];
+  double qphi, qtheta;  // V5 variances added on leaving the PREVIOUS state (what made Cp = J (Cf + Q) J^T); 0 at state 0
 };
 
 // K2: forward filter = the CKF's own path with the branch choice replaced by the candidate's list: state 0 is the
@@ -809,8 +810,15 @@ int fit_forward(const OGeometry& g, const OField& fld, const OConfig& cfg, const
       for (int i = 0; i < 6; ++i)
         for (int j = 0; j < 6; ++j) s.J[i][j] = (i == j) ? 1.0 : 0.0;
       s.module = module;
+      s.qphi = 0.0; s.qtheta = 0.0;
     } else {
       int tg = -1;
+      {
+        double Q[6][6];
+        std::memset(Q, 0, sizeof(Q));
+        add_material(cfg, get_module(g, module), x, Q);
+        s.qphi = Q[2][2]; s.qtheta = Q[3][3];
+      }
       const int stop = move_to_next_module(g, fld, cfg, module, x, C, tg, s.xp, s.Cp, s.J, cnt);
       if (stop != STOP_NONE) return stop;
       s.module = tg;
@@ -928,6 +936,145 @@ bool rts_smooth(int n, const FitState* st, double (*xs)[6], double (*Cs)[6][6]) 
   return true;
 }
 
+// K4': two-filter ("optimal") smoother, the variant PAPER.md:100 names as the more stable one [23, 24]: the smoothed
+// state is the combination of the forward-filtered state with the information a BACKWARD filter has gathered from
+// the later measurements.  It is run on the same linearised model as the RTS recursion (the stored J, xp, xf, Cf and
+// the V5 noise), in deviations d_k = z_k - xf[k], so it needs no second propagation and must give the RTS result
+// (pinned).  No difference of nearly equal covariances appears anywhere.
+//   backward information (Y, y) about d_k from the measurements of the states after k; (0, 0) at the last state;
+//   smoothed: Cf = B B^T (scaled Cholesky);  A = I + B^T Y B;  Cs = B A^-1 B^T;  xs = xf + B A^-1 B^T y;
+//   step k -> k-1: add the measurement of state k (Y += H^T V^-1 H, y += H^T V^-1 (m - H xf[k]));
+//     d_k = c + J (d_{k-1} + u), c = xp[k] - xf[k], u ~ N(0, Q) on (phi, theta):  Yz = J^T Y J, yz = J^T (y - Y c);
+//     marginalise u:  Y' = Yz - Yz G (Qr^-1 + G^T Yz G)^-1 G^T Yz,  y' likewise  (2 x 2 inverse).
+bool two_filter_smooth(int n, const FitState* st, const double* loc, const double* var, double (*xs)[6],
+                       double (*Cs)[6][6]) {
+  double Y[6][6], y[6];
+  std::memset(Y, 0, sizeof(Y));
+  std::memset(y, 0, sizeof(y));
+  for (int k = n - 1; k >= 0; --k) {
+    const FitState& a = st[k];
+    // ---- smoothed state k
+    double s[6], L[6][6], B[6][6];
+    std::memset(L, 0, sizeof(L));
+    for (int i = 0; i < 6; ++i) {
+      if (!(a.Cf[i][i] > 0.0)) return false;
+      s[i] = 1.0 / std::sqrt(a.Cf[i][i]);
+    }
+    for (int j = 0; j < 6; ++j) {  // Cholesky of S Cf S
+      double d = a.Cf[j][j] * s[j] * s[j];
+      for (int l = 0; l < j; ++l) d -= L[j][l] * L[j][l];
+      if (!(d > 0.0)) return false;
+      L[j][j] = std::sqrt(d);
+      for (int i = j + 1; i < 6; ++i) {
+        double v = a.Cf[i][j] * s[i] * s[j];
+        for (int l = 0; l < j; ++l) v -= L[i][l] * L[j][l];
+        L[i][j] = v / L[j][j];
+      }
+    }
+    for (int i = 0; i < 6; ++i)
+      for (int j = 0; j < 6; ++j) B[i][j] = L[i][j] / s[i];  // Cf = B B^T, B lower triangular
+    double A[6][6], YB[6][6], t[6];
+    for (int i = 0; i < 6; ++i)
+      for (int j = 0; j < 6; ++j) {
+        double v = 0.0;
+        for (int l = 0; l < 6; ++l) v += Y[i][l] * B[l][j];
+        YB[i][j] = v;
+      }
+    for (int i = 0; i < 6; ++i) {
+      for (int j = 0; j < 6; ++j) {
+        double v = (i == j) ? 1.0 : 0.0;
+        for (int l = 0; l < 6; ++l) v += B[l][i] * YB[l][j];
+        A[i][j] = v;
+      }
+      double v = 0.0;
+      for (int l = 0; l < 6; ++l) v += B[l][i] * y[l];
+      t[i] = v;
+    }
+    // X = A^-1 [B^T | t]: A is symmetric, >= I
+    double R[6][6], Xm[6][6];
+    for (int i = 0; i < 6; ++i)
+      for (int j = 0; j < 6; ++j) R[i][j] = B[j][i];  // B^T
+    if (!spd_solve6(A, R, Xm)) return false;   // Xm = A^-1 B^T
+    double tt[6][6], Xt[6][6];
+    for (int i = 0; i < 6; ++i)
+      for (int j = 0; j < 6; ++j) tt[i][j] = (j == 0) ? t[i] : 0.0;
+    if (!spd_solve6(A, tt, Xt)) return false;  // first column = A^-1 t
+    for (int i = 0; i < 6; ++i) {
+      double v = 0.0;
+      for (int l = 0; l < 6; ++l) v += B[i][l] * Xt[l][0];
+      xs[k][i] = a.xf[i] + v;
+    }
+    xs[k][2] = wrap_pi(xs[k][2]);
+    double Rm[6][6];
+    for (int i = 0; i < 6; ++i)
+      for (int j = 0; j < 6; ++j) {
+        double v = 0.0;
+        for (int l = 0; l < 6; ++l) v += B[i][l] * Xm[l][j];
+        Rm[i][j] = v;
+      }
+    for (int i = 0; i < 6; ++i)
+      for (int j = 0; j < 6; ++j) Cs[k][i][j] = 0.5 * (Rm[i][j] + Rm[j][i]);
+    if (k == 0) break;
+    // ---- backward step k -> k - 1
+    if (a.meas >= 0) {
+      const double* m = loc + 2 * a.meas;
+      const double* v = var + 2 * a.meas;
+      for (int c = 0; c < 2; ++c) {
+        Y[c][c] += 1.0 / v[c];
+        y[c] += (m[c] - a.xf[c]) / v[c];
+      }
+    }
+    double c6[6], yc[6];
+    for (int i = 0; i < 6; ++i) c6[i] = a.xp[i] - a.xf[i];
+    c6[2] = wrap_pi(c6[2]);
+    for (int i = 0; i < 6; ++i) {
+      double v = y[i];
+      for (int l = 0; l < 6; ++l) v -= Y[i][l] * c6[l];
+      yc[i] = v;
+    }
+    double YJ[6][6], Yz[6][6], yz[6];
+    for (int i = 0; i < 6; ++i)
+      for (int j = 0; j < 6; ++j) {
+        double v = 0.0;
+        for (int l = 0; l < 6; ++l) v += Y[i][l] * a.J[l][j];
+        YJ[i][j] = v;
+      }
+    for (int i = 0; i < 6; ++i) {
+      for (int j = 0; j < 6; ++j) {
+        double v = 0.0;
+        for (int l = 0; l < 6; ++l) v += a.J[l][i] * YJ[l][j];
+        Yz[i][j] = v;
+      }
+      double v = 0.0;
+      for (int l = 0; l < 6; ++l) v += a.J[l][i] * yc[l];
+      yz[i] = v;
+    }
+    for (int i = 0; i < 6; ++i)
+      for (int j = i + 1; j < 6; ++j) { const double m2 = 0.5 * (Yz[i][j] + Yz[j][i]); Yz[i][j] = m2; Yz[j][i] = m2; }
+    if (a.qphi > 0.0 && a.qtheta > 0.0) {
+      const double s00 = 1.0 / a.qphi + Yz[2][2], s01 = Yz[2][3], s11 = 1.0 / a.qtheta + Yz[3][3];
+      const double det = s00 * s11 - s01 * s01;
+      if (!(det > 0.0)) return false;
+      const double i00 = s11 / det, i01 = -s01 / det, i11 = s00 / det;
+      double K2[6], K3[6];   // Kg = Yz G Sg^-1
+      for (int i = 0; i < 6; ++i) {
+        K2[i] = Yz[i][2] * i00 + Yz[i][3] * i01;
+        K3[i] = Yz[i][2] * i01 + Yz[i][3] * i11;
+      }
+      for (int i = 0; i < 6; ++i) {
+        for (int j = 0; j < 6; ++j) Y[i][j] = Yz[i][j] - (K2[i] * Yz[2][j] + K3[i] * Yz[3][j]);
+        y[i] = yz[i] - (K2[i] * yz[2] + K3[i] * yz[3]);
+      }
+      for (int i = 0; i < 6; ++i)
+        for (int j = i + 1; j < 6; ++j) { const double m2 = 0.5 * (Y[i][j] + Y[j][i]); Y[i][j] = m2; Y[j][i] = m2; }
+    } else {
+      std::memcpy(Y, Yz, sizeof(Y));
+      std::memcpy(y, yz, sizeof(y));
+    }
+  }
+  return true;
+}
+
 struct Result {
   std::vector<Track> tracks;
   Counters cnt;
@@ -1013,7 +1160,7 @@ void oracle_kf_fit(const OGeometry* g, const OField* f, const OConfig* cfg, cons
                    const double* loc, const double* var, const int32_t* seed_module, const double* seed_params,
                    const double* seed_cov, int32_t n_tracks, const int32_t* track_offsets, const int32_t* meas_idx,
                    const int32_t* seed_id, int32_t n_threads, int32_t* status, int32_t* n_states, double* chi2_sum,
-                   double* last_x, double* last_C, double* first_C, double* entry_xs) {
+                   double* last_x, double* last_C, double* first_C, double* entry_xs, int32_t smoother) {
   if (n_threads < 1) n_threads = 1;
   if (n_threads > n_tracks) n_threads = std::max(1, n_tracks);
   auto work = [&](int t) {
@@ -1035,7 +1182,10 @@ void oracle_kf_fit(const OGeometry* g, const OField* f, const OConfig* cfg, cons
       if (rc == STOP_NONE && ns > 0) {
         xs.assign((size_t)ns * 6, 0.0);
         Cs.assign((size_t)ns * 36, 0.0);
-        if (!rts_smooth(ns, st.data(), (double(*)[6])xs.data(), (double(*)[6][6])Cs.data())) rc = STOP_NUMERIC;
+        const bool ok = smoother == 1
+            ? two_filter_smooth(ns, st.data(), loc, var, (double(*)[6])xs.data(), (double(*)[6][6])Cs.data())
+            : rts_smooth(ns, st.data(), (double(*)[6])xs.data(), (double(*)[6][6])Cs.data());
+        if (!ok) rc = STOP_NUMERIC;
       }
       status[tr] = rc;
       if (rc != STOP_NONE || ns == 0) continue;
@@ -1071,14 +1221,16 @@ int32_t oracle_kf_fit_states(const OGeometry* g, const OField* f, const OConfig*
                              const double* loc, const double* var, int32_t seed_module, const double* sx,
                              const double* sC, int32_t n_meas, const int32_t* meas, int32_t max_states,
                              int32_t* module, int32_t* meas_used, double* xp, double* Cp, double* xf, double* Cf,
-                             double* J, double* xs, double* Cs) {
+                             double* J, double* xs, double* Cs, int32_t smoother) {
   Counters cnt;
   std::vector<FitState> st;
   const int rc = fit_forward(*g, *f, *cfg, module_offsets, loc, var, seed_module, sx, sC, meas, n_meas, st, cnt);
   if (rc != STOP_NONE) return -rc;
   const int ns = (int)st.size();
   std::vector<double> vx((size_t)ns * 6), vC((size_t)ns * 36);
-  if (!rts_smooth(ns, st.data(), (double(*)[6])vx.data(), (double(*)[6][6])vC.data())) return -STOP_NUMERIC;
+  const bool ok = smoother == 1 ? two_filter_smooth(ns, st.data(), loc, var, (double(*)[6])vx.data(), (double(*)[6][6])vC.data())
+                                : rts_smooth(ns, st.data(), (double(*)[6])vx.data(), (double(*)[6][6])vC.data());
+  if (!ok) return -STOP_NUMERIC;
   for (int k = 0; k < ns && k < max_states; ++k) {
     module[k] = st[k].module; meas_used[k] = st[k].meas;
     std::memcpy(xp + 6 * k, st[k].xp, 48); std::memcpy(xf + 6 * k, st[k].xf, 48);
