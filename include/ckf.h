@@ -26,7 +26,7 @@
 extern "C" {
 #endif
 
-#define CKF_ABI_VERSION 4
+#define CKF_ABI_VERSION 5
 
 /* return codes */
 #define CKF_OK 0
@@ -212,6 +212,9 @@ typedef struct {
   int32_t smoother_precision; /* INPUT.  0 or 64: the RTS recursion runs in float64 (the product's choice, K5).
                            32 (handles of precision 32 only): it runs in float32 -- kept to study the instability
                            of the float32 smoother that PAPER.md:61, :100 report, not for production             */
+  int32_t smoother;     /* INPUT.  0: RTS recursion (K4).  1: two-filter "optimal" smoother (K4'): the
+                           forward-filtered state combined with a backward information filter over the same stored
+                           states; same result (tested), no differences of nearly equal covariances                 */
 } ckf_fits;
 
 /* Fits every candidate of `tracks` (the DEVICE arrays a ckf_find on the same measurements and seeds filled;

@@ -274,8 +274,14 @@ int launch_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, con
       ckf_fit_level<T><<<grid, FIT_NT, 0, st>>>(kp, p, level, g_this);
     }
     ckf_fit_flush_work<<<1, 32, 0, st>>>(h->ft_counters, p.o_work);
-    if (sizeof(T) == 4 && o->smoother_precision == 32) ckf_fit_smooth<T, float><<<grid, FIT_NT, 0, st>>>(p);
-    else ckf_fit_smooth<T, double><<<grid, FIT_NT, 0, st>>>(p);
+    const bool f32 = sizeof(T) == 4 && o->smoother_precision == 32;
+    if (o->smoother == 1) {
+      if (f32) ckf_fit_smooth_tf<T, float><<<grid, FIT_NT, 0, st>>>(p);
+      else ckf_fit_smooth_tf<T, double><<<grid, FIT_NT, 0, st>>>(p);
+    } else {
+      if (f32) ckf_fit_smooth<T, float><<<grid, FIT_NT, 0, st>>>(p);
+      else ckf_fit_smooth<T, double><<<grid, FIT_NT, 0, st>>>(p);
+    }
   }
   cudaError_t e = cudaGetLastError();
   if (e != cudaSuccess) return fail(h, CKF_E_CUDA, "kernel launch failed: %s", cudaGetErrorString(e));
@@ -535,6 +541,7 @@ int ckf_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, const 
     return fail(h, CKF_E_ARG, "null input array");
   if (o->smoother_precision != 0 && o->smoother_precision != 32 && o->smoother_precision != 64)
     return fail(h, CKF_E_ARG, "smoother_precision must be 0, 32 or 64");
+  if (o->smoother != 0 && o->smoother != 1) return fail(h, CKF_E_ARG, "smoother must be 0 (RTS) or 1 (two-filter)");
   if (o->smoother_precision == 32 && h->cfg.precision != 32)
     return fail(h, CKF_E_ARG, "smoother_precision 32 needs a handle of precision 32");
   if (!o->status || !o->n_states || !o->chi2_sum || !o->last_params || !o->last_cov || !o->first_cov || !o->entry_params)

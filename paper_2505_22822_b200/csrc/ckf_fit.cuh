@@ -21,7 +21,8 @@ namespace ckf {
 constexpr int FIT_NT = 128;
 constexpr int FIT_CHUNK = 262144;   // tracks per pass: bounds the state store (ckf.cu loops over the chunks)
 constexpr int FS_X = 12;            // float64 per state: xp[6], xf[6]
-constexpr int FS_T = 21 + 21 + 25;  // T per state: Cp, Cf (packed upper triangles), J (5x5 block, row-major)
+constexpr int FS_T = 21 + 21 + 25 + 2;  // T per state: Cp, Cf (packed upper triangles), J (5x5 block, row-major),
+                                        // V5 variances (phi, theta) added on leaving the previous state
 
 template <typename T>
 struct FitParams {
@@ -80,7 +81,7 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, con
     T Cp[21], Cf[21], J[5][5];
     int status = STOP_NONE, module = 0, next = 0, stored = level;
     bool done = false;
-    T c2sum = T(0);
+    T c2sum = T(0), q_in[2] = {T(0), T(0)};
 #pragma unroll
     for (int i = 0; i < 6; ++i) xf[i] = 0.0;
 #pragma unroll
@@ -137,6 +138,7 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, con
           for (int i = 0; i < 21; ++i) C[i] = pt[(21 + i) * CH];
           C[tri(2, 2)] += dep[3];  // V5 on leaving
           C[tri(3, 3)] += dep[4];
+          q_in[0] = dep[3]; q_in[1] = dep[4];
           transport_cov<T>(J, C, Cp);
           bool fin = true;
 #pragma unroll
@@ -174,6 +176,8 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, con
       for (int a = 0; a < 5; ++a)
 #pragma unroll
         for (int b = 0; b < 5; ++b) ft[(42 + a * 5 + b) * CH] = J[a][b];
+      ft[67 * CH] = q_in[0];
+      ft[68 * CH] = q_in[1];
       p.fs_meas[(size_t)level * CH + s] = used;
       stored = level + 1;
       if (next == n) done = true;
@@ -416,6 +420,235 @@ __global__ void __launch_bounds__(FIT_NT, CKF_SMOOTH_MINB) ckf_fit_smooth(const 
     }
     if (!good) {
       if (p.o_status[tr] == STOP_NONE && ns > 0) p.o_status[tr] = STOP_NUMERIC;  // a predicted covariance was not positive definite
+      p.o_chi2[tr] = T(0);
+      for (int i = 0; i < 6; ++i) p.o_lastx[(size_t)tr * 6 + i] = T(0);
+      for (int i = 0; i < 36; ++i) { p.o_lastC[(size_t)tr * 36 + i] = T(0); p.o_firstC[(size_t)tr * 36 + i] = T(0); }
+      for (int i = 0; i < 6 * n; ++i) p.o_entryx[(size_t)e0 * 6 + i] = T(0);
+    }
+  }
+}
+
+// ---- two-filter ("optimal") smoother K4' (the variant the paper names as more stable than RTS).
+// The smoothed state = forward-filtered state combined with the information (Y, y) a BACKWARD filter has gathered from
+// the later measurements, on the same linearised model as the RTS recursion (stored J, xp, xf, Cf, V5 noise), in
+// deviations from xf[k].  No difference of nearly equal covariances appears:
+//   Cf = B B^T (scaled Cholesky), A = I + B^T Y B = La La^T, U = La^-1 B^T:  Cs = U^T U,  xs = xf + U^T La^-1 B^T y.
+// plain Cholesky of a packed symmetric 6x6 (lower factor packed by rows, L[i][j] at tri(j, i)); false if not p.d.
+template <typename A>
+__device__ __forceinline__ bool chol6(const A G[21], A L[21]) {
+#pragma unroll
+  for (int j = 0; j < 6; ++j) {
+    A d = G[tri(j, j)];
+#pragma unroll
+    for (int k = 0; k < j; ++k) d -= L[tri(k, j)] * L[tri(k, j)];
+    if (!(d > A(0))) return false;
+    L[tri(j, j)] = sqrt(d);
+#pragma unroll
+    for (int i = j + 1; i < 6; ++i) {
+      A v = G[tri(i, j)];
+#pragma unroll
+      for (int k = 0; k < j; ++k) v -= L[tri(k, i)] * L[tri(k, j)];
+      L[tri(j, i)] = v / L[tri(j, j)];
+    }
+  }
+  return true;
+}
+
+template <typename T, typename A>
+__global__ void __launch_bounds__(FIT_NT, CKF_SMOOTH_MINB) ckf_fit_smooth_tf(const FitParams<T> p) {
+  const int nt = min(*p.n_tracks, p.max_tracks);
+  const size_t CH = (size_t)p.chunk;
+  for (int s = blockIdx.x * FIT_NT + threadIdx.x; s < p.chunk; s += gridDim.x * FIT_NT) {
+    const int tr = p.first + s;
+    if (tr >= nt) return;
+    const int e0 = p.offsets[tr], n = p.offsets[tr + 1] - e0;
+    const int ns = p.o_nstates[tr];
+    bool good = p.o_status[tr] == STOP_NONE && ns > 0;
+    int e = n - 1;
+    if (good) {
+      A Y[21], y[6];  // backward information about the deviation of state k, from the measurements after k
+#pragma unroll
+      for (int i = 0; i < 21; ++i) Y[i] = A(0);
+#pragma unroll
+      for (int i = 0; i < 6; ++i) y[i] = A(0);
+      for (int k = ns - 1;; --k) {
+        const double* fx = p.fs_x + (size_t)k * FS_X * CH + s;
+        const T* ft = p.fs_t + (size_t)k * FS_T * CH + s;
+        const int used = p.fs_meas[(size_t)k * CH + s];
+        if (used >= 0) {  // a reported state: combine
+          A B[21];  // Cf = B B^T, B lower triangular, packed like a Cholesky factor
+          {
+            A Cf[21], sc[6], L[21];
+#pragma unroll
+            for (int i = 0; i < 21; ++i) Cf[i] = (A)ft[(size_t)(21 + i) * CH];
+            if (!chol6_scaled<A>(Cf, sc, L)) { good = false; break; }
+#pragma unroll
+            for (int i = 0; i < 6; ++i)
+#pragma unroll
+              for (int j = 0; j <= i; ++j) B[tri(j, i)] = L[tri(j, i)] / sc[i];
+          }
+          A Am[21], t[6];
+          {
+            A YB[6][6];  // Y B
+#pragma unroll
+            for (int i = 0; i < 6; ++i)
+#pragma unroll
+              for (int j = 0; j < 6; ++j) {
+                A v = A(0);
+#pragma unroll
+                for (int l = j; l < 6; ++l) v += Y[tri(i, l)] * B[tri(j, l)];  // B[l][j], l >= j
+                YB[i][j] = v;
+              }
+#pragma unroll
+            for (int i = 0; i < 6; ++i) {
+#pragma unroll
+              for (int j = i; j < 6; ++j) {
+                A v = (i == j) ? A(1) : A(0);
+#pragma unroll
+                for (int l = i; l < 6; ++l) v += B[tri(i, l)] * YB[l][j];  // B^T[i][l] = B[l][i], l >= i
+                Am[tri(i, j)] = v;
+              }
+              A v = A(0);
+#pragma unroll
+              for (int l = i; l < 6; ++l) v += B[tri(i, l)] * y[l];
+              t[i] = v;
+            }
+          }
+          A La[21];
+          if (!chol6<A>(Am, La)) { good = false; break; }
+          // U = La^-1 B^T (forward substitution, column j of B^T = row j of B), w = La^-1 t
+          A U[6][6], w[6];
+#pragma unroll
+          for (int i = 0; i < 6; ++i) {
+#pragma unroll
+            for (int j = 0; j < 6; ++j) {
+              A v = (i <= j) ? B[tri(i, j)] : A(0);  // B^T[i][j] = B[j][i], non-zero for i <= j
+#pragma unroll
+              for (int l = 0; l < i; ++l) v -= La[tri(l, i)] * U[l][j];
+              U[i][j] = v / La[tri(i, i)];
+            }
+            A v = t[i];
+#pragma unroll
+            for (int l = 0; l < i; ++l) v -= La[tri(l, i)] * w[l];
+            w[i] = v / La[tri(i, i)];
+          }
+          A xs[6];
+#pragma unroll
+          for (int i = 0; i < 6; ++i) {
+            A v = A(0);
+#pragma unroll
+            for (int l = 0; l < 6; ++l) v += U[l][i] * w[l];
+            xs[i] = (A)fx[(6 + i) * CH] + v;
+          }
+          xs[2] = wrap_pi<A>(xs[2]);
+#pragma unroll
+          for (int i = 0; i < 6; ++i) p.o_entryx[(size_t)(e0 + e) * 6 + i] = (T)xs[i];
+          if (e == 0) {
+#pragma unroll
+            for (int i = 0; i < 6; ++i)
+#pragma unroll
+              for (int j = i; j < 6; ++j) {
+                A v = A(0);
+#pragma unroll
+                for (int l = 0; l < 6; ++l) v += U[l][i] * U[l][j];
+                p.o_firstC[(size_t)tr * 36 + i * 6 + j] = (T)v;
+                p.o_firstC[(size_t)tr * 36 + j * 6 + i] = (T)v;
+              }
+          }
+          --e;
+        }
+        if (k == 0 || e < 0) break;
+        // ---- backward step k -> k - 1: measurement of state k, then back through d_k = c + Jf (d_{k-1} + u)
+        if (used >= 0) {
+          const typename Vec2<T>::type mm = p.loc[used], vv = p.var[used];
+          Y[tri(0, 0)] += A(1) / (A)vv.x;
+          Y[tri(1, 1)] += A(1) / (A)vv.y;
+          y[0] += (A)((double)mm.x - fx[6 * CH]) / (A)vv.x;
+          y[1] += (A)((double)mm.y - fx[7 * CH]) / (A)vv.y;
+        }
+        A yc[6];
+        {
+          A c6[6];
+#pragma unroll
+          for (int i = 0; i < 6; ++i) c6[i] = (A)(fx[i * CH] - fx[(6 + i) * CH]);
+          c6[2] = wrap_pi<A>(c6[2]);
+#pragma unroll
+          for (int i = 0; i < 6; ++i) {
+            A v = y[i];
+#pragma unroll
+            for (int l = 0; l < 6; ++l) v -= Y[tri(i, l)] * c6[l];
+            yc[i] = v;
+          }
+        }
+        // Jf: rows 0..3 = J[0..3] over columns 0..4, row 4 = e_4, row 5 = J[4] plus 1 at column 5
+        A Jf[6][6];
+#pragma unroll
+        for (int i = 0; i < 6; ++i)
+#pragma unroll
+          for (int j = 0; j < 6; ++j) {
+            if (i == 4) Jf[i][j] = (j == 4) ? A(1) : A(0);
+            else if (j == 5) Jf[i][j] = (i == 5) ? A(1) : A(0);
+            else Jf[i][j] = (A)ft[(size_t)(42 + ((i == 5) ? 4 : i) * 5 + j) * CH];
+          }
+        A Yz[21], yz[6];
+        {
+          A YJ[6][6];
+#pragma unroll
+          for (int i = 0; i < 6; ++i)
+#pragma unroll
+            for (int j = 0; j < 6; ++j) {
+              A v = A(0);
+#pragma unroll
+              for (int l = 0; l < 6; ++l) v += Y[tri(i, l)] * Jf[l][j];
+              YJ[i][j] = v;
+            }
+#pragma unroll
+          for (int i = 0; i < 6; ++i) {
+#pragma unroll
+            for (int j = i; j < 6; ++j) {
+              A v = A(0), u = A(0);
+#pragma unroll
+              for (int l = 0; l < 6; ++l) { v += Jf[l][i] * YJ[l][j]; u += Jf[l][j] * YJ[l][i]; }
+              Yz[tri(i, j)] = A(0.5) * (v + u);
+            }
+            A v = A(0);
+#pragma unroll
+            for (int l = 0; l < 6; ++l) v += Jf[l][i] * yc[l];
+            yz[i] = v;
+          }
+        }
+        const A qp = (A)ft[67 * CH], qt = (A)ft[68 * CH];
+        if (qp > A(0) && qt > A(0)) {  // marginalise the scattering angles u ~ N(0, diag(qp, qt)) on (phi, theta)
+          const A s00 = A(1) / qp + Yz[tri(2, 2)], s01 = Yz[tri(2, 3)], s11 = A(1) / qt + Yz[tri(3, 3)];
+          const A det = s00 * s11 - s01 * s01;
+          if (!(det > A(0))) { good = false; break; }
+          const A i00 = s11 / det, i01 = -s01 / det, i11 = s00 / det;
+          A K2[6], K3[6];
+#pragma unroll
+          for (int i = 0; i < 6; ++i) {
+            K2[i] = Yz[tri(i, 2)] * i00 + Yz[tri(i, 3)] * i01;
+            K3[i] = Yz[tri(i, 2)] * i01 + Yz[tri(i, 3)] * i11;
+          }
+#pragma unroll
+          for (int i = 0; i < 6; ++i) {
+#pragma unroll
+            for (int j = i; j < 6; ++j) {
+              const A a = Yz[tri(i, j)] - (K2[i] * Yz[tri(2, j)] + K3[i] * Yz[tri(3, j)]);
+              const A b = Yz[tri(i, j)] - (K2[j] * Yz[tri(2, i)] + K3[j] * Yz[tri(3, i)]);
+              Y[tri(i, j)] = A(0.5) * (a + b);
+            }
+            y[i] = yz[i] - (K2[i] * yz[2] + K3[i] * yz[3]);
+          }
+        } else {
+#pragma unroll
+          for (int i = 0; i < 21; ++i) Y[i] = Yz[i];
+#pragma unroll
+          for (int i = 0; i < 6; ++i) y[i] = yz[i];
+        }
+      }
+    }
+    if (!good) {
+      if (p.o_status[tr] == STOP_NONE && ns > 0) p.o_status[tr] = STOP_NUMERIC;
       p.o_chi2[tr] = T(0);
       for (int i = 0; i < 6; ++i) p.o_lastx[(size_t)tr * 6 + i] = T(0);
       for (int i = 0; i < 36; ++i) { p.o_lastC[(size_t)tr * 36 + i] = T(0); p.o_firstC[(size_t)tr * 36 + i] = T(0); }
