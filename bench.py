@@ -263,8 +263,16 @@ def main():
     fb.record(stream)
     torch.cuda.synchronize()
     fit_ms = fa.elapsed_time(fb) / n_fit
+    fa.record(stream)
+    for _ in range(n_fit):
+        ckf.fit(dev_last, out, fits, stream, smoother=1)
+    fb.record(stream)
+    torch.cuda.synchronize()
+    fit_tf_ms = fa.elapsed_time(fb) / n_fit
+    ckf.fit(dev_last, out, fits, stream)            # leave the RTS result in `fits` for the counts below
+    torch.cuda.synchronize()
     fit_ok = int((fits["status"][:res.n_tracks] == 0).sum().item())
-    fit_work = [int(v) // (n_fit + 2) for v in fits["work"].cpu().tolist()]   # trials, accepted, moves, updates per call
+    fit_work = [int(v) // (2 * n_fit + 3) for v in fits["work"].cpu().tolist()]   # trials, accepted, moves, updates per call
     fit_states = int(fits["n_states"][:res.n_tracks].sum().item())
     clocks = sampler.stop()
     launches_per_find = int(tim[0]["launches"])
@@ -342,7 +350,7 @@ def main():
             "fit": {"what": "ckf_fit: Kalman-filter fit + RTS smoother of every candidate of one step's batch of configs[3] "
                             "events (next row, SURVEY.md 8(f) rank 1); device-resident, CUDA events, mean of 5",
                     "value": res.n_tracks / (fit_ms * 1e-3), "unit": "tracks/s", "ms_per_event": fit_ms / B,
-                    "ms_per_step": fit_ms,
+                    "ms_per_step": fit_ms, "ms_per_event_two_filter_smoother": fit_tf_ms / B,
                     "tracks": res.n_tracks, "fitted": fit_ok, "entries": int(res.meas_idx.size),
                     "work": dict(zip(("rk_trials", "rk_accepted", "moves", "updates"), fit_work)), "states": fit_states,
                     "flop_per_event": fit_flop, "achieved_tflops": fit_flop / (fit_ms * 1e-3) / 1e12,

@@ -429,6 +429,14 @@ def test_fit_fp32_covariance_not_positive_definite_is_flagged():
     for t in bad:
         assert not g["entry_params"][gpu.track_offsets[t]:gpu.track_offsets[t + 1]].any() and not g["first_cov"][t].any()
     assert r["max_smoothed_rel"] < 1e-4 and r["max_last_rel"] < 1e-4
+    # the two-filter smoother factors the FILTERED covariance instead of the predicted one
+    f2 = ckf.alloc_fits()
+    ckf.fit(dev, out, f2, smoother=1)
+    torch.cuda.synchronize()
+    g2 = ckf.download_fits(f2, gpu.n_tracks, int(gpu.meas_idx.size))
+    r2 = parity.compare_fits(g2, o, gpu.track_offsets)
+    print("fit config 3 event 1, two-filter", r2)
+    assert r2["n_not_pd_gpu_only"] <= r["n_not_pd_gpu_only"] and r2["max_smoothed_rel"] < 1e-4
     ckf.close()
 
 
