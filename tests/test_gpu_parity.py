@@ -491,3 +491,38 @@ def test_fit_two_filter_smoother(config):
         print("float32 smoother study config 2: RTS", res[0], "two-filter", res[1])
         assert res[1][0][0] >= res[0][0][0]          # the two-filter form matches at least as often at 0.01 %
     ckf.close()
+
+
+def test_batch_with_an_empty_event_and_fit_of_nothing():
+    """Edge cases of the batch and of ckf_fit: an event without seeds and measurements inside a batch; a find that
+    yields no candidate at all (ckf_fit must return without touching anything)."""
+    import torch
+    from types import SimpleNamespace
+    from paper_2505_22822_b200 import CKF, concat_events
+    det, fld, cfg = synth.config_bundle(1)
+    ev = synth.make_event(1, det=det, n_particles=200)
+    empty = SimpleNamespace(module_offsets=np.zeros(det.n_modules + 1, np.int32), loc=ev.loc[:0], var=ev.var[:0],
+                            seed_module=ev.seed_module[:0], seed_params=ev.seed_params[:0], seed_cov=ev.seed_cov[:0],
+                            n_measurements=0, n_seeds=0)
+    batch = concat_events([ev, empty, ev], det.n_modules)
+    ckf = CKF(det, fld, cfg.ckf, cfg.precision, max_seeds=batch.n_seeds, max_measurements=batch.n_measurements,
+              max_events_per_find=3)
+    dev, out = ckf.upload_event(batch), ckf.alloc_tracks()
+    ckf.find(dev, out)
+    torch.cuda.synchronize()
+    gpu = ckf.download(out)
+    parts = parity.split_batch(gpu, batch)
+    a, b = parts[0][0], parts[2][0]
+    assert parts[1][0].n_tracks == 0 and a.n_tracks == b.n_tracks > 0
+    assert np.array_equal(a.meas_idx, b.meas_idx) and np.array_equal(a.params, b.params)   # the same event twice
+    # a find without seeds: no candidate, and the fit of nothing leaves its outputs alone
+    dev0 = ckf.upload_event(concat_events([empty], det.n_modules))
+    out0 = ckf.alloc_tracks()
+    ckf.find(dev0, out0)
+    fits = ckf.alloc_fits()
+    fits["status"].fill_(77)
+    ckf.fit(dev0, out0, fits)
+    torch.cuda.synchronize()
+    assert int(out0["n_tracks"][0]) == 0 and int(out0["status"][0]) == 0
+    assert bool((fits["status"] == 77).all()) and int(fits["work"].sum()) == 0
+    ckf.close()
