@@ -62,18 +62,18 @@ __device__ __forceinline__ int gate_chunk(const KParams<T>& p, const VSmem<T>& s
         if (isfinite(w)) {
           const double l0 = s.px[0 * 32 + lane];
           const double a = l0 - w, b = l0 + w;
+          // both ends of the window at once: the two chains of dependent loads overlap
           int x0 = beg, x1 = end;  // first k with loc0[k] >= a
-          while (x0 < x1) {
-            const int mid = (x0 + x1) >> 1;
-            if ((double)p.s_loc[mid].x < a) x0 = mid + 1; else x1 = mid;
+          int y0 = beg, y1 = end;  // first k with loc0[k] > b
+          while (x0 < x1 || y0 < y1) {
+            const int mx = (x0 + x1) >> 1, my = (y0 + y1) >> 1;
+            const double vx = x0 < x1 ? (double)p.s_loc[mx].x : 0.0;
+            const double vy = y0 < y1 ? (double)p.s_loc[my].x : 0.0;
+            if (x0 < x1) { if (vx < a) x0 = mx + 1; else x1 = mx; }
+            if (y0 < y1) { if (vy <= b) y0 = my + 1; else y1 = my; }
           }
           lo = x0;
-          x1 = end;  // first k with loc0[k] > b
-          while (x0 < x1) {
-            const int mid = (x0 + x1) >> 1;
-            if ((double)p.s_loc[mid].x <= b) x0 = mid + 1; else x1 = mid;
-          }
-          hi = x0;
+          hi = y0;
         }
       }
     }
