@@ -95,13 +95,14 @@ __device__ __forceinline__ int gate_chunk(const KParams<T>& p, const VSmem<T>& s
       const int k = s.lo[t] + (q - s.off[t]);
       const auto lc = p.s_loc[k];
       const auto vr = p.s_var[k];
+      const int oi = p.s_idx[k];  // loaded with the rest (coalesced), not after the test by the few lanes that pass
       T c2 = T(0);
       const bool pass = gate_chi2<T>(s.px[0 * 32 + t], s.px[1 * 32 + t], s.pC[tri(0, 0) * 32 + t],
                                      s.pC[tri(0, 1) * 32 + t], s.pC[tri(1, 1) * 32 + t], lc.x, lc.y, vr.x, vr.y,
                                      chi2_max, c2);
       if (pass) {
         const int pos = atomicAdd(&s.cnt[t], 1);
-        if (pos < CAND) { s.candchi2[pos * 32 + t] = c2; s.candidx[pos * 32 + t] = p.s_idx[k]; }
+        if (pos < CAND) { s.candchi2[pos * 32 + t] = c2; s.candidx[pos * 32 + t] = oi; }
       }
     }
   }
