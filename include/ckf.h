@@ -219,7 +219,7 @@ typedef struct {
 
 /* Fits every candidate of `tracks` (the DEVICE arrays a ckf_find on the same measurements and seeds filled;
  * *tracks->n_tracks is read on the device, no host synchronisation).  Asynchronous on `cuda_stream`.  The first
- * call on a handle reserves the state store (about 1.5 GB for fp32); later calls allocate nothing.  Calls
+ * call on a handle reserves the state store (up to 3 GB in fp32: 32 states of min(max_tracks, 262,144) candidates); later calls allocate nothing.  Calls
  * on different streams are ordered one after the other (one state store per handle). */
 int ckf_fit(ckf_handle* handle, const ckf_measurements* measurements, const ckf_seeds* seeds, const ckf_tracks* tracks,
             ckf_fits* out, void* cuda_stream);
