@@ -259,13 +259,13 @@ int launch_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, con
     p.first = first;
     // forward filter, level-synchronous: per level the moves on ckf_step, then the rest of the state (ckf_fit_level).
     // Two blocks of globals, by level parity: level L's ckf_step reads the schedule in block L & 1.
-    cudaMemsetAsync(h->ft_g, 0, 64 * 4, st);
+    cudaMemsetAsync(h->ft_g, 0, 2 * GBLK * 4, st);
     cudaMemsetAsync(h->ft_g + G_NTIPS0, 1, 2 * 4, st);       // non-zero: ckf_step only asks whether the level holds tips
-    cudaMemsetAsync(h->ft_g + 32 + G_NTIPS0, 1, 2 * 4, st);
+    cudaMemsetAsync(h->ft_g + GBLK + G_NTIPS0, 1, 2 * 4, st);
     cudaMemsetAsync(h->ft_counters, 0, CNT_N * 8, st);
     for (int level = 0; level < h->fit_states; ++level) {
-      int32_t* g_this = h->ft_g + 32 * (level & 1);
-      int32_t* g_next = h->ft_g + 32 * ((level + 1) & 1);
+      int32_t* g_this = h->ft_g + GBLK * (level & 1);
+      int32_t* g_next = h->ft_g + GBLK * ((level + 1) & 1);
       if (level > 0) {
         kp.g = g_this;
         ckf_step<T, MinBlocks<T>::value><<<h->step_grid, STEP_NT, 0, st>>>(kp, level);
@@ -446,8 +446,8 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     CKB(dalloc(h, (char**)&w.s_var, 2 * (size_t)c->max_measurements * ts));
     CKB(dalloc(h, &w.s_idx, (size_t)c->max_measurements * 4));
     CKB(dalloc(h, (char**)&w.s_v0max, (size_t)g->n_modules * (size_t)h->cfg.max_events_per_find * ts));
-    CKB(dalloc(h, &w.globals, 64 * 4));
-    static_assert(G_N <= 32, "globals block too small (ckf_fit keeps two of them in 64 ints)");
+    CKB(dalloc(h, &w.globals, GBLK * 4));
+    static_assert(G_N <= GBLK, "globals block too small");
     CKB(dalloc(h, &w.mv_order, (size_t)NBIN * TC * 4));
     CKB(dalloc(h, &w.counters, CNT_N * 8));
     CKB(cudaEventCreateWithFlags(&w.done, cudaEventDisableTiming));
@@ -557,7 +557,7 @@ int ckf_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, const 
     CK(dalloc(h, &fm, n * 4));
     const size_t CHK = (size_t)chunk, ts = (size_t)h->tsize;
     CK(dalloc(h, &h->fs_next, CHK * 4));
-    CK(dalloc(h, &h->ft_g, 64 * 4)); CK(dalloc(h, &h->ft_counters, CNT_N * 8));
+    CK(dalloc(h, &h->ft_g, 2 * GBLK * 4)); CK(dalloc(h, &h->ft_counters, CNT_N * 8));
     CK(dalloc(h, &h->ft_y, 8 * CHK * sizeof(double)));
     CK(dalloc(h, (char**)&h->ft_D, 25 * CHK * ts)); CK(dalloc(h, (char**)&h->ft_dep, 5 * CHK * ts));
     CK(dalloc(h, &h->ft_from, CHK * 4)); CK(dalloc(h, &h->ft_tgt, 2 * CHK * 4)); CK(dalloc(h, &h->ft_stop, CHK * 4));

@@ -174,7 +174,7 @@ __device__ __forceinline__ int step_cost_bin(const GeoDev& g, int module, const 
   const float st = sqrtf((float)(y.d[0] * y.d[0] + y.d[1] * y.d[1]));
   const float gap = (float)(g.layer[L + 1].r - g.layer[L].r);
   const float pred = 0.2565f * __powf(gap / st, 0.713f) * __powf(0.6f * fabsf((float)y.qop) / st, 0.266f);
-  const int b = (int)pred;
+  const int b = (int)(pred * ((float)NBIN / 16.0f));  // NBIN / 16 classes per predicted trial
   return b < 1 ? 1 : (b > NBIN - 1 ? NBIN - 1 : b);
 }
 

@@ -43,9 +43,13 @@ enum CounterId { CNT_TIPS = 0, CNT_VISITS, CNT_TRIALS, CNT_ACCEPTED, CNT_GATE, C
                  CNT_GATE_EXEC, CNT_N };
 
 // per-event device globals (int32 each)
+#ifndef CKF_NBIN
+#define CKF_NBIN 8
+#endif
 enum GlobalId { G_LINK_COUNT = 0, G_FIRST_BAD, G_TOTAL_TRACKS, G_TOTAL_ENTRIES, G_NTIPS0, G_NTIPS1, G_STEP_CURSOR,
-                G_SCAN_TICKET, G_LBASE, G_SEED_TICKET, G_BIN0, G_N = G_BIN0 + 16 };
-constexpr int NBIN = 16;          // cost classes of the step schedule (G_BIN0 .. G_BIN0 + NBIN - 1 hold their sizes)
+                G_SCAN_TICKET, G_LBASE, G_SEED_TICKET, G_BIN0, G_N = G_BIN0 + CKF_NBIN };
+constexpr int NBIN = CKF_NBIN;    // cost classes of the step schedule (G_BIN0 .. G_BIN0 + NBIN - 1 hold their sizes)
+constexpr int GBLK = 64;          // ints reserved for one block of globals
 
 template <typename T>
 struct KParams {
