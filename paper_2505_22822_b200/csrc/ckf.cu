@@ -434,7 +434,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     const size_t TC = (size_t)h->tcap, KB = (size_t)c->max_branches_per_surface;
     CKB(dalloc(h, &w.tip_link, 2 * TC * 4)); CKB(dalloc(h, &w.tip_seed, 2 * TC * 4));
     CKB(dalloc(h, &w.mv_y, 8 * TC * sizeof(double))); CKB(dalloc(h, &w.pd_x, 6 * TC * sizeof(double)));
-    CKB(dalloc(h, (char**)&w.mv_D, 25 * TC * ts)); CKB(dalloc(h, (char**)&w.mv_dep, 5 * TC * ts));
+    CKB(dalloc(h, (char**)&w.mv_D, (size_t)MVD * TC * ts)); CKB(dalloc(h, (char**)&w.mv_dep, 5 * TC * ts));
     CKB(dalloc(h, (char**)&w.pd_C, 21 * TC * ts)); CKB(dalloc(h, (char**)&w.sel_chi2, KB * TC * ts));
     CKB(dalloc(h, &w.sel_idx, KB * TC * 4));
     CKB(dalloc(h, &w.mv_from, TC * 4)); CKB(dalloc(h, &w.mv_tgt, 2 * TC * 4)); CKB(dalloc(h, &w.mv_stop, TC * 4));
@@ -559,7 +559,7 @@ int ckf_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, const 
     CK(dalloc(h, &h->fs_next, CHK * 4));
     CK(dalloc(h, &h->ft_g, 2 * GBLK * 4)); CK(dalloc(h, &h->ft_counters, CNT_N * 8));
     CK(dalloc(h, &h->ft_y, 8 * CHK * sizeof(double)));
-    CK(dalloc(h, (char**)&h->ft_D, 25 * CHK * ts)); CK(dalloc(h, (char**)&h->ft_dep, 5 * CHK * ts));
+    CK(dalloc(h, (char**)&h->ft_D, (size_t)MVD * CHK * ts)); CK(dalloc(h, (char**)&h->ft_dep, 5 * CHK * ts));
     CK(dalloc(h, &h->ft_from, CHK * 4)); CK(dalloc(h, &h->ft_tgt, 2 * CHK * 4)); CK(dalloc(h, &h->ft_stop, CHK * 4));
     CK(dalloc(h, &h->ft_order, (size_t)NBIN * CHK * 4));
     CK(cudaEventCreateWithFlags(&h->fit_done, cudaEventDisableTiming));

@@ -313,10 +313,7 @@ __global__ void __launch_bounds__(SCAN_NT, CKF_UPDATE_MINB) ckf_update(const KPa
       T dep[5];
       stop = departure_state<T>(p.geo, p.cfg, target, xo, y, dep);
       if (stop == STOP_NONE) {
-#pragma unroll
-        for (int i = 0; i < 3; ++i) { p.mv_y[i * TC + c] = y.r[i]; p.mv_y[(3 + i) * TC + c] = y.d[i]; }
-        p.mv_y[6 * TC + c] = y.t;
-        p.mv_y[7 * TC + c] = y.qop;
+        store_traj(p.mv_y, (size_t)c, y);
 #pragma unroll
         for (int i = 0; i < 5; ++i) p.mv_dep[i * TC + c] = dep[i];
         // N2 here, at full lanes, instead of inside the RKN4 kernel: the overlap neighbour of the child's departure

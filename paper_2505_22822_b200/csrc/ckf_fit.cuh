@@ -110,21 +110,8 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, con
       status = kp.mv_stop[s];
       if (status == STOP_NONE) {
         Move<T> m;
-#pragma unroll
-        for (int i = 0; i < 3; ++i) { m.y.r[i] = kp.mv_y[i * CH + s]; m.y.d[i] = kp.mv_y[(3 + i) * CH + s]; }
-        m.y.t = kp.mv_y[6 * CH + s];
-        m.y.qop = kp.mv_y[7 * CH + s];
-#pragma unroll
-        for (int i = 0; i < 3; ++i) {
-#pragma unroll
-          for (int j = 0; j < 3; ++j) {
-            m.D.Rd[i][j] = kp.mv_D[(i * 3 + j) * CH + s];
-            m.D.Dd[i][j] = kp.mv_D[(9 + i * 3 + j) * CH + s];
-          }
-          m.D.rq[i] = kp.mv_D[(18 + i) * CH + s];
-          m.D.dq[i] = kp.mv_D[(21 + i) * CH + s];
-        }
-        m.D.tq = kp.mv_D[24 * CH + s];
+        load_traj(kp.mv_y, (size_t)s, m.y);
+        load_jac(kp.mv_D, (size_t)s, m.D);
         m.from = kp.mv_from[s];
         m.tgt = kp.mv_tgt[s];
         T dep[5];
@@ -187,10 +174,7 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, con
         T dep[5];
         status = departure_state<T>(p.geo, p.cfg, module, xf, y, dep);
         if (status == STOP_NONE) {  // the track as a tip of the next level's ckf_step
-#pragma unroll
-          for (int i = 0; i < 3; ++i) { kp.mv_y[i * CH + s] = y.r[i]; kp.mv_y[(3 + i) * CH + s] = y.d[i]; }
-          kp.mv_y[6 * CH + s] = y.t;
-          kp.mv_y[7 * CH + s] = y.qop;
+          store_traj(kp.mv_y, (size_t)s, y);
 #pragma unroll
           for (int i = 0; i < 5; ++i) kp.mv_dep[i * CH + s] = dep[i];
           kp.mv_from[s] = module;

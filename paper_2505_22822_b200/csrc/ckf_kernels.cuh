@@ -100,8 +100,8 @@ struct KParams {
   int32_t* tip_link;   // [2][tcap] (ping-pong by level parity) link the tip stands on, -1 = fresh seed
   int32_t* tip_seed;   // [2][tcap]
   // departure / arrival state of the move (ckf_update -> ckf_step -> ckf_visit)
-  double* mv_y;        // [8][tcap] r, d, t, q/p
-  T* mv_D;             // [25][tcap] transport Jacobian (ckf_step -> ckf_visit)
+  double* mv_y;        // [tcap][8] r, d, t, q/p (move records, see below)
+  T* mv_D;             // [tcap][MVD] transport Jacobian (ckf_step -> ckf_visit)
   T* mv_dep;           // [5][tcap] direction on departure, Highland q_phi, q_theta
   int32_t* mv_from;    // [tcap] module the tip stands on
   int32_t* mv_tgt;     // [2][tcap] module reached; overlap neighbour at departure (N2, by ckf_update), -1 none
@@ -128,6 +128,68 @@ struct KParams {
   int32_t* o_lastmod; int32_t* o_stop;
   T* o_params; T* o_cov; T* o_chi2sum; T* o_entrychi2;
 };
+
+// ------------------------------------------------------------------------------------------ move records
+// The state of a move is kept per tip as two contiguous records (AoS), not [component][tip]: ckf_step reaches its tips
+// through the step schedule, i.e. in scattered order, and a contiguous record costs whole sectors whatever the order
+// (the [component][tip] form cost 33 partial-sector accesses per tip there); the lane-per-tip readers (ckf_visit,
+// ckf_update, ckf_fit_level) read the same bytes either way.
+//   mv_y[t * 8 ..)    r[3], d[3], t, q/p   float64 (one 64-byte record)
+//   mv_D[t * MVD ..)  Rd[9], Dd[9], rq[3], dq[3], tq, padding   T (one 128- / 256-byte record)
+constexpr int MVD = 32;
+__device__ __forceinline__ void store_traj(double* mv_y, size_t t, const Traj& y) {
+  double2* q = reinterpret_cast<double2*>(mv_y + t * 8);
+  q[0] = make_double2(y.r[0], y.r[1]); q[1] = make_double2(y.r[2], y.d[0]);
+  q[2] = make_double2(y.d[1], y.d[2]); q[3] = make_double2(y.t, y.qop);
+}
+__device__ __forceinline__ void load_traj(const double* mv_y, size_t t, Traj& y) {
+  const double2* q = reinterpret_cast<const double2*>(mv_y + t * 8);
+  const double2 a = q[0], b = q[1], c = q[2], d = q[3];
+  y.r[0] = a.x; y.r[1] = a.y; y.r[2] = b.x; y.d[0] = b.y; y.d[1] = c.x; y.d[2] = c.y; y.t = d.x; y.qop = d.y;
+}
+__device__ __forceinline__ void store_jac(float* mv_D, size_t t, const Jac<float>& D) {
+  float4* q = reinterpret_cast<float4*>(mv_D + t * MVD);
+  q[0] = make_float4(D.Rd[0][0], D.Rd[0][1], D.Rd[0][2], D.Rd[1][0]);
+  q[1] = make_float4(D.Rd[1][1], D.Rd[1][2], D.Rd[2][0], D.Rd[2][1]);
+  q[2] = make_float4(D.Rd[2][2], D.Dd[0][0], D.Dd[0][1], D.Dd[0][2]);
+  q[3] = make_float4(D.Dd[1][0], D.Dd[1][1], D.Dd[1][2], D.Dd[2][0]);
+  q[4] = make_float4(D.Dd[2][1], D.Dd[2][2], D.rq[0], D.rq[1]);
+  q[5] = make_float4(D.rq[2], D.dq[0], D.dq[1], D.dq[2]);
+  q[6] = make_float4(D.tq, 0.f, 0.f, 0.f);
+}
+__device__ __forceinline__ void load_jac(const float* mv_D, size_t t, Jac<float>& D) {
+  const float4* q = reinterpret_cast<const float4*>(mv_D + t * MVD);
+  const float4 a = q[0], b = q[1], c = q[2], d = q[3], e = q[4], f = q[5], g = q[6];
+  D.Rd[0][0] = a.x; D.Rd[0][1] = a.y; D.Rd[0][2] = a.z; D.Rd[1][0] = a.w;
+  D.Rd[1][1] = b.x; D.Rd[1][2] = b.y; D.Rd[2][0] = b.z; D.Rd[2][1] = b.w;
+  D.Rd[2][2] = c.x; D.Dd[0][0] = c.y; D.Dd[0][1] = c.z; D.Dd[0][2] = c.w;
+  D.Dd[1][0] = d.x; D.Dd[1][1] = d.y; D.Dd[1][2] = d.z; D.Dd[2][0] = d.w;
+  D.Dd[2][1] = e.x; D.Dd[2][2] = e.y; D.rq[0] = e.z; D.rq[1] = e.w;
+  D.rq[2] = f.x; D.dq[0] = f.y; D.dq[1] = f.z; D.dq[2] = f.w;
+  D.tq = g.x;
+}
+__device__ __forceinline__ void store_jac(double* mv_D, size_t t, const Jac<double>& D) {
+  double2* q = reinterpret_cast<double2*>(mv_D + t * MVD);
+  const double v[26] = {D.Rd[0][0], D.Rd[0][1], D.Rd[0][2], D.Rd[1][0], D.Rd[1][1], D.Rd[1][2], D.Rd[2][0], D.Rd[2][1],
+                        D.Rd[2][2], D.Dd[0][0], D.Dd[0][1], D.Dd[0][2], D.Dd[1][0], D.Dd[1][1], D.Dd[1][2], D.Dd[2][0],
+                        D.Dd[2][1], D.Dd[2][2], D.rq[0], D.rq[1], D.rq[2], D.dq[0], D.dq[1], D.dq[2], D.tq, 0.0};
+#pragma unroll
+  for (int i = 0; i < 13; ++i) q[i] = make_double2(v[2 * i], v[2 * i + 1]);
+}
+__device__ __forceinline__ void load_jac(const double* mv_D, size_t t, Jac<double>& D) {
+  const double2* q = reinterpret_cast<const double2*>(mv_D + t * MVD);
+  double v[26];
+#pragma unroll
+  for (int i = 0; i < 13; ++i) { const double2 a = q[i]; v[2 * i] = a.x; v[2 * i + 1] = a.y; }
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+#pragma unroll
+    for (int j = 0; j < 3; ++j) { D.Rd[i][j] = v[i * 3 + j]; D.Dd[i][j] = v[9 + i * 3 + j]; }
+    D.rq[i] = v[18 + i];
+    D.dq[i] = v[21 + i];
+  }
+  D.tq = v[24];
+}
 
 // ------------------------------------------------------------------------------------------ warp primitives
 __device__ __forceinline__ int warp_incl_scan(int v, int lane) {

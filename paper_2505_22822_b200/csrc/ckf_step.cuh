@@ -126,20 +126,8 @@ __global__ void __launch_bounds__(STEP_NT, MINB) ckf_step(const KParams<T> p, in
       // ---- write-back of finished moves
       if (m.phase == PH_FIN) {
         if (m.stop == STOP_NONE) {
-#pragma unroll
-          for (int i = 0; i < 3; ++i) { p.mv_y[i * TC + tip] = m.y.r[i]; p.mv_y[(3 + i) * TC + tip] = m.y.d[i]; }
-          p.mv_y[6 * TC + tip] = m.y.t;
-#pragma unroll
-          for (int i = 0; i < 3; ++i) {
-#pragma unroll
-            for (int j = 0; j < 3; ++j) {
-              p.mv_D[(i * 3 + j) * TC + tip] = m.D.Rd[i][j];
-              p.mv_D[(9 + i * 3 + j) * TC + tip] = m.D.Dd[i][j];
-            }
-            p.mv_D[(18 + i) * TC + tip] = m.D.rq[i];
-            p.mv_D[(21 + i) * TC + tip] = m.D.dq[i];
-          }
-          p.mv_D[24 * TC + tip] = m.D.tq;
+          store_traj(p.mv_y, (size_t)tip, m.y);
+          store_jac(p.mv_D, (size_t)tip, m.D);
           p.mv_tgt[tip] = m.tgt;
         }
         p.mv_stop[tip] = m.stop;
@@ -161,10 +149,7 @@ __global__ void __launch_bounds__(STEP_NT, MINB) ckf_step(const KParams<T> p, in
         }
         if (t >= 0 && p.mv_stop[t] == STOP_NONE) {
           tip = t;
-#pragma unroll
-          for (int i = 0; i < 3; ++i) { m.y.r[i] = p.mv_y[i * TC + t]; m.y.d[i] = p.mv_y[(3 + i) * TC + t]; }
-          m.y.t = p.mv_y[6 * TC + t];
-          m.y.qop = p.mv_y[7 * TC + t];
+          load_traj(p.mv_y, (size_t)t, m.y);
           move_begin<T>(m, p.cfg, p.mv_from[t]);
           move_pick_apply<T>(m, p.geo, p.mv_tgt[TC + t]);  // N2 was decided by ckf_update
         }

@@ -200,21 +200,8 @@ __global__ void __launch_bounds__(VISIT_NT, MINB) ckf_visit(const KParams<T> p, 
         if (stop == STOP_NONE) {
           // arrival (J4, J5) and covariance transport
           Move<T> m;
-#pragma unroll
-          for (int i = 0; i < 3; ++i) { m.y.r[i] = p.mv_y[i * TC + t]; m.y.d[i] = p.mv_y[(3 + i) * TC + t]; }
-          m.y.t = p.mv_y[6 * TC + t];
-          m.y.qop = p.mv_y[7 * TC + t];
-#pragma unroll
-          for (int i = 0; i < 3; ++i) {
-#pragma unroll
-            for (int j = 0; j < 3; ++j) {
-              m.D.Rd[i][j] = p.mv_D[(i * 3 + j) * TC + t];
-              m.D.Dd[i][j] = p.mv_D[(9 + i * 3 + j) * TC + t];
-            }
-            m.D.rq[i] = p.mv_D[(18 + i) * TC + t];
-            m.D.dq[i] = p.mv_D[(21 + i) * TC + t];
-          }
-          m.D.tq = p.mv_D[24 * TC + t];
+          load_traj(p.mv_y, (size_t)t, m.y);
+          load_jac(p.mv_D, (size_t)t, m.D);
           m.from = p.mv_from[t];
           m.tgt = p.mv_tgt[t];
           T dep[5];
