@@ -361,10 +361,11 @@ def main():
             "roofline": {"bound": "alu", "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak,
                          # DRAM bytes of ONE ckf_step launch (level 4 of a batched find of 4 events, ~360,000 tips), from the
                          # committed ncu --set full capture; only valid for the default batch of 4
-                         "traffic": 256.3e6 if (B == 4 and cfg.precision == 32) else None,
-                         "traffic_source": "profiles/r01h_step_and_launches.md: dram__bytes_read.sum + dram__bytes_write.sum "
-                                           "of one ckf_step launch; its algorithmic bytes (tip state in and out: 8 + 8 "
-                                           "float64 and 25 float32 per tip) are 228 B x 360,000 = 82 MB",
+                         "traffic": 139.1e6 if (B == 4 and cfg.precision == 32) else None,
+                         "traffic_source": "profiles/r01i_step_and_launches.md: dram__bytes_read.sum + dram__bytes_write.sum "
+                                           "of one ckf_step launch (level 4 of a batched find, ~360,000 tips); its algorithmic "
+                                           "bytes (tip state in and out: 8 + 8 float64 and 25 float32 per tip) are 228 B x "
+                                           "360,000 = 82 MB",
                          "kernel": "ckf_step (all %d launches of one find)" % step_launches,
                          "flop_per_find_this_kernel": step_flop, "kernel_ms_per_find": step_ms,
                          "share_of_find": step_ms / max(sum(v for k, v in tim[0].items() if k.endswith("_ms")), 1e-9),
