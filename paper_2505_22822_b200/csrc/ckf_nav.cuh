@@ -56,11 +56,10 @@ CKF_HD int pick_in_neighbourhood(const GeoDev& g, int layer, int iphi, int iz, i
     int ii = iphi + (nb / 3 - 1);
     ii = ii < 0 ? ii + L.n_phi : (ii >= L.n_phi ? ii - L.n_phi : ii);
     const int jj = iz + (nb % 3 - 1);
-    const bool valid = jj >= 0 && jj < L.n_z;
-    const int id = L.offset + ii * L.n_z + (valid ? jj : iz);   // an in-range record is read either way
-    const double s = line_test_module(g.mod[id], r, d, s_min);
-    idv[nb] = (valid && id != exclude) ? id : -1;
-    sv[nb] = s;
+    const int id = L.offset + ii * L.n_z + jj;
+    const bool test = jj >= 0 && jj < L.n_z && id != exclude;   // a predicate, not a branch around the loads
+    sv[nb] = test ? line_test_module(g.mod[id], r, d, s_min) : 0.0;
+    idv[nb] = test ? id : -1;
   }
   int best = -1;
   double best_s = 0.0;
