@@ -147,7 +147,7 @@ __global__ void __launch_bounds__(STEP_NT, MINB) ckf_step(const KParams<T> p, in
           while (q >= s_binend[k]) ++k;
           t = p.mv_order[(size_t)(NBIN - 1 - k) * TC + (q - (k ? s_binend[k - 1] : 0))];
         }
-        if (t >= 0 && p.mv_stop[t] == STOP_NONE) {
+        if (t >= 0) {  // every tip of the schedule is live (ckf_update / ckf_fit_level only append live ones)
           tip = t;
           load_traj(p.mv_y, (size_t)t, m.y);
           move_begin<T>(m, p.cfg, p.mv_from[t]);
