@@ -59,6 +59,7 @@ def lib():
         L.oracle_result_copy.argtypes = [C.c_void_p, _ip, _ip, _dp, _ip, _ip, _ip, _ip, _dp, _dp, _dp]
         L.oracle_result_free.argtypes = [C.c_void_p]
         L.oracle_field_at.argtypes = [C.POINTER(OField), _dp, _dp]
+        L.oracle_set_n3_literal_walk.argtypes = [C.c_int32]
         L.oracle_propagate_free.restype = C.c_int32
         L.oracle_propagate_free.argtypes = [C.POINTER(OField), C.POINTER(OConfig), C.c_int32, _dp, _dp, C.c_double, _dp,
                                             _dp, _ip]
@@ -185,6 +186,11 @@ def find_event(setup: Setup, ev, n_threads: int = 1) -> Tracks:
 
 
 # ------------------------------------------------------------------ pieces for the pins
+def set_n3_literal_walk(on: bool):
+    """Pin hook: navigate past the barrel ends as SURVEY.md N3 words it (True) instead of reading D11 (False, default)."""
+    lib().oracle_set_n3_literal_walk(1 if on else 0)
+
+
 def field_at(setup: Setup, r):
     r = _d(r)
     b = np.zeros(3)

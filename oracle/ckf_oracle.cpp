@@ -16,7 +16,12 @@
 // KF fit + RTS smoother (rules K, tests/test_oracle_fit.py): scalar random walk against its information-form
 // closed form, the smoothed states of real tracks against a dense Gaussian conditioning of the linearised
 // model (numpy), forward pass = the CKF candidate's reported state.
-// Parity unpinned (convention only, fixed by DESIGN.md): the order in which the per-seed cap R10 cuts,
+// Round-2 pins (tests/test_oracle_pins2.py): RKN4 stage points and field per stage in a NON-uniform field against
+// an independent DOP853 integration (analytic map through the pin hook `field kind 2`, and the float32 grid through
+// scipy's multilinear interpolator); the material path factor x/X0 / |d.n| for inclined tracks; the closed form of
+// R10 against a literal one-child-at-a-time greedy (which children survive, with branches finishing at different
+// levels); reading D11 against the literal N3 walk (pin hook oracle_set_n3_literal_walk): same candidates.
+// Parity unpinned (convention only, fixed by DESIGN.md): that R10 cuts in TIP order (the closed form itself is pinned),
 // hole-only-when-nothing-passes (A5), outward-only navigation (A7), inclusive in-bounds edges (A10),
 // min_measurements = 3 (A14).
 #include <cmath>
@@ -106,6 +111,17 @@ inline void mat3_mul(const double A[3][3], const double B[3][3], double O[3][3])
 void field_at(const OField& f, const double r[3], double B[3]) {
   if (f.kind == 0) {
     B[0] = f.uniform_b[0]; B[1] = f.uniform_b[1]; B[2] = f.uniform_b[2];
+    return;
+  }
+  if (f.kind == 2) {
+    // PIN HOOK (tests only; the product has no such field kind): the analytic map behind configs[2]'s grid,
+    // Bz = B0 (1 - a z^2), Br = a B0 r z (BASELINE.json configs[2]), with B0 = uniform_b[2] and a = origin[0].
+    // A smooth non-uniform field lets the stepping (P2-P5) be compared with an independent ODE integrator and
+    // the Jacobian with finite differences without the kinks of the trilinear interpolant.
+    const double B0 = f.uniform_b[2], a = f.origin[0];
+    B[0] = a * B0 * r[0] * r[2];
+    B[1] = a * B0 * r[1] * r[2];
+    B[2] = B0 * (1.0 - a * r[2] * r[2]);
     return;
   }
   int idx[3];
@@ -472,6 +488,11 @@ void add_material(const OConfig& cfg, const Module& m, const double x[6], double
 }
 
 // ---------------------------------------------------------------------------------- N: navigation
+// PIN HOOK: 1 = walk the remaining portal cylinders literally as SURVEY.md N3 words it ("l' <- l' + 1 and repeat"),
+// 0 (default) = reading D11: a tip beyond every further half-length and moving away in z stops EXIT at
+// once.  tests/test_oracle_pins.py runs both and checks that the candidates are the same.
+int g_n3_literal_walk = 0;
+
 // straight-line test of one module from the point (r, d): N2 / N4
 bool line_hits_module(const Module& k, const double r[3], const double d[3], double s_min, double& s_out) {
   const double dn = dot(d, k.n);
@@ -540,7 +561,7 @@ int move_to_next_module(const OGeometry& g, const OField& fld, const OConfig& cf
       if (std::fabs(y.r[2]) > g.layer_half_z[lp]) {
         // N3 (reading D11): beyond the half-length of this layer AND of every further layer while moving
         // away in z, the tip has left the barrel: EXIT now instead of walking the remaining portal cylinders.
-        bool gone = y.r[2] * y.d[2] > 0.0;
+        bool gone = !g_n3_literal_walk && y.r[2] * y.d[2] > 0.0;
         for (int l2 = lp + 1; gone && l2 < g.n_layers; ++l2) gone = std::fabs(y.r[2]) > g.layer_half_z[l2];
         if (gone) return STOP_EXIT;
         ++lp;
@@ -1255,6 +1276,8 @@ int32_t oracle_rts_smooth(int32_t n, const double* xp, const double* Cp, const d
 }
 
 // ---- pieces exposed for the pins (tests/test_oracle_pins.py)
+void oracle_set_n3_literal_walk(int32_t on) { g_n3_literal_walk = on ? 1 : 0; }
+
 void oracle_field_at(const OField* f, const double r[3], double B[3]) { field_at(*f, r, B); }
 
 // Free-state propagation to a plane (kind 0: c, n) or cylinder (kind 1: R).  y = (r, t, d, q/p) in/out;
