@@ -11,7 +11,14 @@
  * Conventions
  *   - Units: mm, GeV, tesla, c = 1 (time in mm).  Bound parameters (loc0, loc1, phi, theta, q/p, t).
  *   - All structs are POD and passed by const pointer; no C++ types or exceptions cross the ABI.
- *   - Return value: 0 (CKF_OK) on success, negative CKF_E_* otherwise; ckf_last_error() gives text.
+ *   - Return value: 0 (CKF_OK) on success, negative CKF_E_* otherwise; ckf_last_error() gives the text of the
+ *     calling thread's last failure.
+ *   - Threads: several host threads may call ckf_find / ckf_find_host on one handle, each on its own stream
+ *     (one host thread per event pipeline).  With more streams than n_streams a workspace is recycled:
+ *     the later call waits on the host until the earlier one has finished enqueuing and is ordered on the device
+ *     after its work.
+ *   - Malformed input (a seed module id out of range, a module_offsets array that is not monotonic or points beyond
+ *     n) never causes an out-of-bounds access: the seed stops, the slice is clamped, and CKF_STATUS_BAD_INPUT is set.
  *   - ckf_find is ASYNCHRONOUS on `cuda_stream` and never allocates: every workspace is reserved in
  *     ckf_create from the max_* capacities (PAPER.md:84, :102 blame in-pipeline allocation for the lack of
  *     stream scaling).  Capacity overflow is never silent: it sets a bit in *status.
@@ -26,7 +33,7 @@
 extern "C" {
 #endif
 
-#define CKF_ABI_VERSION 5
+#define CKF_ABI_VERSION 6
 
 /* return codes */
 #define CKF_OK 0
@@ -38,6 +45,8 @@ extern "C" {
 #define CKF_STATUS_TRACK_OVERFLOW 1  /* more candidates than max_tracks: the first max_tracks are kept       */
 #define CKF_STATUS_ENTRY_OVERFLOW 2  /* meas_idx capacity max_track_entries exceeded: later tracks dropped   */
 #define CKF_STATUS_LINK_OVERFLOW 4   /* max_links or max_tips_per_level exhausted: some branches were cut    */
+#define CKF_STATUS_BAD_INPUT 8       /* a seed's module id was out of range (that seed yields nothing), or
+                                        module_offsets was not a valid CSR over [0, n] (slices were clamped)  */
 
 /* stop reasons reported per candidate */
 #define CKF_STOP_EXIT 1         /* left the detector (past the last layer / beyond half-z everywhere) */
@@ -105,6 +114,9 @@ typedef struct {
   int32_t max_tips_per_level;       /* live branch tips of one level, whole event; 0 = 8 * max_seeds     */
   int32_t n_streams;                /* independent workspaces; concurrent ckf_find calls up to this many */
   int32_t max_events_per_find;      /* largest batch of events one ckf_find may carry; 0 = 1 (see ckf_measurements) */
+  int32_t max_fit_tracks;           /* ckf_fit: candidates fitted per pass; sizes the state store reserved in ckf_create
+                                       (max_levels states x min(max_fit_tracks, max_tracks, 262144) candidates x
+                                       (12 float64 + 69 T): 3 GB at 262,144 in fp32).  0 = no ckf_fit on this handle */
 } ckf_config;
 
 /* Measurements of one event: CSR by module id (north_star).  DEVICE pointers, caller-owned, read-only.
@@ -177,14 +189,17 @@ int ckf_create(const ckf_geometry* geometry, const ckf_field* field, const ckf_c
 /* Runs CKF track finding for one event on `cuda_stream` (a cudaStream_t; NULL = default stream).
  * Asynchronous; all pointers in measurements/seeds/out are DEVICE pointers that must stay valid until the
  * stream reaches the end of the call's work.  Up to n_streams calls may be in flight on different streams;
- * further streams are ordered after the call that last used the recycled workspace. */
+ * further streams are ordered after the call that last used the recycled workspace (also when that call is still
+ * being enqueued by another host thread). */
 int ckf_find(ckf_handle* handle, const ckf_measurements* measurements, const ckf_seeds* seeds, ckf_tracks* out,
              void* cuda_stream);
 
 /* Same work with HOST buffers: copies measurements and seeds host->device, runs ckf_find, copies the
  * candidates device->host, all on `cuda_stream` (PAPER.md:51 transfer policy; BASELINE config 4).  Buffers
  * should be pinned for the copies to be asynchronous.  Device staging buffers belong to the handle.
- * Output arrays are filled up to *n_tracks / track_offsets[*n_tracks] after the stream is synchronised. */
+ * SYNCHRONOUS: when it returns, the stream has been synchronised and the output arrays are filled up to *n_tracks /
+ * track_offsets[*n_tracks] (what lies beyond is unspecified: the copies are sized from a guess, the previous call's
+ * result + 1/8, so that one synchronisation per call suffices; the host arrays need their full capacity). */
 int ckf_find_host(ckf_handle* handle, const ckf_measurements* measurements, const ckf_seeds* seeds, ckf_tracks* out,
                   void* cuda_stream);
 
@@ -218,9 +233,10 @@ typedef struct {
 } ckf_fits;
 
 /* Fits every candidate of `tracks` (the DEVICE arrays a ckf_find on the same measurements and seeds filled;
- * *tracks->n_tracks is read on the device, no host synchronisation).  Asynchronous on `cuda_stream`.  The first
- * call on a handle reserves the state store (up to 3 GB in fp32: 32 states of min(max_tracks, 262,144) candidates); later calls allocate nothing.  Calls
- * on different streams are ordered one after the other (one state store per handle). */
+ * *tracks->n_tracks is read on the device, no host synchronisation).  Asynchronous on `cuda_stream`; allocates
+ * nothing: the state store was reserved by ckf_create (config.max_fit_tracks; CKF_E_CAPACITY if that was 0).  All
+ * candidates are fitted, in passes of the store's size.  Calls on different streams are ordered one after the other
+ * (one state store per handle). */
 int ckf_fit(ckf_handle* handle, const ckf_measurements* measurements, const ckf_seeds* seeds, const ckf_tracks* tracks,
             ckf_fits* out, void* cuda_stream);
 
@@ -252,7 +268,7 @@ int ckf_get_launch_info(const ckf_handle* handle, int32_t* blocks, int32_t* thre
 
 int ckf_destroy(ckf_handle* handle);
 
-/* Text of the last error on this handle (or of the last failed ckf_create when handle is NULL). */
+/* Text of the calling thread's last failed call (handle may be NULL; it is not used). */
 const char* ckf_last_error(const ckf_handle* handle);
 
 int ckf_abi_version(void);

@@ -43,7 +43,7 @@ class ckf_config(C.Structure):
                 ("particle_mass_gev", C.c_double), ("max_rk_steps_per_surface", C.c_int32), ("max_levels", C.c_int32),
                 ("max_seeds", C.c_int32), ("max_measurements", C.c_int32), ("max_tracks", C.c_int32),
                 ("max_track_entries", C.c_int32), ("max_links", C.c_int32), ("max_tips_per_level", C.c_int32),
-                ("n_streams", C.c_int32), ("max_events_per_find", C.c_int32)]
+                ("n_streams", C.c_int32), ("max_events_per_find", C.c_int32), ("max_fit_tracks", C.c_int32)]
 
 
 class ckf_measurements(C.Structure):
@@ -151,7 +151,7 @@ def make_field(fld, keep: list) -> ckf_field:
 
 def make_config(ckf, precision: int, max_seeds: int, max_measurements: int, max_tracks: int, max_track_entries: int,
                 max_links: int = 0, n_streams: int = 1, max_tips_per_level: int = 0,
-                max_events_per_find: int = 1) -> ckf_config:
+                max_events_per_find: int = 1, max_fit_tracks: int = 0) -> ckf_config:
     c = ckf_config()
     c.precision = int(precision)
     for name in ("chi2_max", "max_branches_per_surface", "max_candidates_per_seed", "max_holes", "min_measurements",
@@ -163,6 +163,7 @@ def make_config(ckf, precision: int, max_seeds: int, max_measurements: int, max_
     c.max_links, c.n_streams = int(max_links), int(n_streams)
     c.max_tips_per_level = int(max_tips_per_level)
     c.max_events_per_find = int(max_events_per_find)
+    c.max_fit_tracks = int(max_fit_tracks)
     return c
 
 
@@ -232,7 +233,10 @@ class CKF:
 
     def __init__(self, det, fld, ckf, precision: int, max_seeds: int, max_measurements: int,
                  max_tracks: Optional[int] = None, max_track_entries: Optional[int] = None, max_links: int = 0,
-                 n_streams: int = 1, max_tips_per_level: int = 0, max_events_per_find: int = 1):
+                 n_streams: int = 1, max_tips_per_level: int = 0, max_events_per_find: int = 1,
+                 max_fit_tracks: Optional[int] = None):
+        """max_fit_tracks: candidates per ckf_fit pass (sizes the state store reserved by ckf_create); None = all of
+        max_tracks up to the library's pass limit, 0 = this handle never fits."""
         import torch
         if not torch.cuda.is_available():
             raise RuntimeError("no CUDA device: paper_2505_22822_b200 has no CPU fallback")
@@ -248,7 +252,8 @@ class CKF:
         g = make_geometry(det, keep)
         f = make_field(fld, keep)
         self.config = make_config(ckf, precision, max_seeds, max_measurements, self.max_tracks, self.max_track_entries,
-                                  max_links, n_streams, max_tips_per_level, max_events_per_find)
+                                  max_links, n_streams, max_tips_per_level, max_events_per_find,
+                                  self.max_tracks if max_fit_tracks is None else max_fit_tracks)
         h = _vp()
         rc = self.lib.ckf_create(C.byref(g), C.byref(f), C.byref(self.config), C.byref(h))
         if rc != 0:

@@ -10,6 +10,8 @@
 #include <cstdio>
 #include <cstdlib>
 #include <cstring>
+#include <atomic>
+#include <deque>
 #include <mutex>
 #include <string>
 #include <vector>
@@ -27,7 +29,9 @@ using namespace ckf;
 
 namespace {
 
-thread_local std::string g_create_error;
+// Error text is per calling THREAD (several host threads may drive one handle, configs[4]): a failing call stores its
+// message here and ckf_last_error returns the calling thread's last message.
+thread_local std::string g_error;
 
 struct Workspace {
   // link buffer
@@ -54,8 +58,15 @@ struct Workspace {
   int32_t *o_nt = nullptr, *o_off = nullptr, *o_meas = nullptr, *o_seed = nullptr, *o_nh = nullptr, *o_lm = nullptr,
           *o_stop = nullptr;
   void *o_par = nullptr, *o_cov = nullptr, *o_c2 = nullptr, *o_ec2 = nullptr;
-  int32_t* pinned_nt = nullptr;  // host pinned [2]
-  cudaEvent_t done = nullptr;
+  int32_t* pinned_nt = nullptr;  // host pinned [3]: candidates, status, entries of the last ckf_find_host
+  cudaEvent_t done = nullptr;    // recorded after the last piece of work that uses this workspace
+  // Ownership.  `stream_tag` / `used` (which stream's finds map to this workspace) change under the handle mutex;
+  // `busy` is held by a host thread from before its first enqueue to after it has recorded `done`, so a thread that
+  // recycles the workspace for another stream waits (on the host) until the previous owner has finished ENQUEUING and
+  // then (on the device, cudaStreamWaitEvent) until that work has finished RUNNING.  `done_stream` is written under busy.
+  std::mutex busy;
+  void* done_stream = nullptr;
+  bool done_valid = false;
   void* stream_tag = nullptr;
   bool used = false;
   float last_ms[10] = {0};  // per-kernel-kind times of the last timed ckf_find (ckf_set_timing)
@@ -74,12 +85,13 @@ struct ckf_handle {
   FieldDev fld;
   CfgDev kcfg;
   int step_grid = 0, step_regs = 0, visit_grid = 0, visit_smem = 0, tcap = 0, tsize = 4;
-  std::vector<Workspace> ws;
+  std::deque<Workspace> ws;
   int next_ws = 0;
   std::mutex mu;
-  std::string err;
   std::vector<void*> allocs;
-  // state store of ckf_fit, reserved by the first call
+  // sizes of the last ckf_find_host result, the guess for the next call's device->host copies
+  std::atomic<int> hint_tracks{-1}, hint_entries{-1};
+  // state store of ckf_fit, reserved in ckf_create (config.max_fit_tracks)
   double* fs_x = nullptr; void* fs_t = nullptr; int32_t* fs_meas = nullptr; int32_t* fs_next = nullptr;
   // level arrays, globals and counters for ckf_step when it runs the moves of a fit level (tcap = fit_chunk)
   int32_t* ft_g = nullptr; unsigned long long* ft_counters = nullptr;
@@ -99,8 +111,8 @@ int fail(ckf_handle* h, int code, const char* fmt, ...) {
   va_start(ap, fmt);
   vsnprintf(buf, sizeof(buf), fmt, ap);
   va_end(ap);
-  if (h) h->err = buf;
-  else g_create_error = buf;
+  (void)h;
+  g_error = buf;
   return code;
 }
 
@@ -119,7 +131,8 @@ cudaError_t dalloc(ckf_handle* h, P** p, size_t bytes) {
 }
 
 // Resident blocks per SM ckf_step / ckf_visit are compiled for: 3 x 128 threads at <= 168 registers (float step:
-// measured faster than 4 x 128 at 128 registers with 300 B of spills), 4 x 128 at <= 128 registers (float visit),
+// measured faster than 4 x 128 at 128 registers with 300 B of spills), 3 x 128 at <= 168 registers (float visit: its
+// arrival algebra is float64 since r02; 4 blocks spill 360 B and run 3 % slower, 2 blocks 2 % slower),
 // 2 x 128 threads at <= 255 registers (double: the covariance algebra doubles its register footprint).
 #ifndef CKF_MINB
 #define CKF_MINB 3
@@ -127,7 +140,7 @@ cudaError_t dalloc(ckf_handle* h, P** p, size_t bytes) {
 template <typename T> struct MinBlocks { static constexpr int value = CKF_MINB; };
 template <> struct MinBlocks<double> { static constexpr int value = 2; };
 #ifndef CKF_VISIT_MINB
-#define CKF_VISIT_MINB 4
+#define CKF_VISIT_MINB 3
 #endif
 template <typename T> struct VisitBlocks { static constexpr int value = CKF_VISIT_MINB; };
 template <> struct VisitBlocks<double> { static constexpr int value = 2; };
@@ -139,8 +152,8 @@ void fill_params(ckf_handle* h, Workspace& w, KParams<T>& p) {
   p.fld = h->fld;
   p.cfg = h->kcfg;
   p.max_links = c.max_links;
-  p.lk_x = w.lk_x; p.lk_C = (T*)w.lk_C; p.lk_module = w.lk_module; p.lk_parent = w.lk_parent; p.lk_meas = w.lk_meas;
-  p.lk_chi2 = (T*)w.lk_chi2; p.lk_chi2sum = (T*)w.lk_chi2sum; p.lk_counts = w.lk_counts; p.lk_lastmeas = w.lk_lastmeas;
+  p.lk_x = w.lk_x; p.lk_C = (double*)w.lk_C; p.lk_module = w.lk_module; p.lk_parent = w.lk_parent; p.lk_meas = w.lk_meas;
+  p.lk_chi2 = (T*)w.lk_chi2; p.lk_chi2sum = (double*)w.lk_chi2sum; p.lk_counts = w.lk_counts; p.lk_lastmeas = w.lk_lastmeas;
   const size_t S = (size_t)c.max_seeds;
   p.sd_extra = w.sd; p.sd_nemit = w.sd + S; p.sd_nentries = w.sd + 2 * S;
   p.sd_track_base = w.sd + 3 * S; p.sd_entry_base = w.sd + 3 * S + (S + 1);
@@ -150,9 +163,9 @@ void fill_params(ckf_handle* h, Workspace& w, KParams<T>& p) {
   p.leaf_link = w.leaf; p.leaf_meta = w.leaf + LC; p.leaf_entry = w.leaf + 2 * LC;
   p.tcap = h->tcap;
   p.tip_link = w.tip_link; p.tip_seed = w.tip_seed;
-  p.mv_y = w.mv_y; p.mv_D = (T*)w.mv_D; p.mv_dep = (T*)w.mv_dep; p.mv_from = w.mv_from; p.mv_tgt = w.mv_tgt;
+  p.mv_y = w.mv_y; p.mv_D = (T*)w.mv_D; p.mv_dep = (double*)w.mv_dep; p.mv_from = w.mv_from; p.mv_tgt = w.mv_tgt;
   p.mv_stop = w.mv_stop; p.mv_order = w.mv_order;
-  p.pd_x = w.pd_x; p.pd_C = (T*)w.pd_C; p.sel_chi2 = (T*)w.sel_chi2; p.sel_idx = w.sel_idx;
+  p.pd_x = w.pd_x; p.pd_C = (double*)w.pd_C; p.sel_chi2 = (T*)w.sel_chi2; p.sel_idx = w.sel_idx;
   p.t_nsel = w.t_nsel; p.t_want = w.t_want; p.t_counts = w.t_counts; p.t_keep = w.t_keep; p.t_kex = w.t_kex;
   p.blk_sum = w.blk_sum; p.t_fin = w.t_fin;
   p.s_loc = (typename Vec2<T>::type*)w.s_loc; p.s_var = (typename Vec2<T>::type*)w.s_var; p.s_idx = w.s_idx;
@@ -160,13 +173,15 @@ void fill_params(ckf_handle* h, Workspace& w, KParams<T>& p) {
   p.g = w.globals;
   p.counters = w.counters;
   p.max_tracks = c.max_tracks; p.max_entries = c.max_track_entries;
+  p.o_summary = nullptr;
 }
 
 template <typename T>
 int launch_find(ckf_handle* h, Workspace& w, const ckf_measurements* m, const ckf_seeds* s, ckf_tracks* o,
-                cudaStream_t st) {
+                cudaStream_t st, int32_t* summary = nullptr) {
   KParams<T> p;
   fill_params<T>(h, w, p);
+  p.o_summary = summary;
   p.n_meas = m->n; p.n_seeds = s->n;
   p.moff = m->module_offsets;
   p.n_vmod = std::max(1, m->n_events) * h->n_modules;
@@ -253,7 +268,7 @@ int launch_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, con
   kp.geo = p.geo; kp.fld = p.fld; kp.cfg = p.cfg;
   kp.tcap = h->fit_chunk;
   kp.g = h->ft_g; kp.counters = h->ft_counters;
-  kp.mv_y = h->ft_y; kp.mv_D = (T*)h->ft_D; kp.mv_dep = (T*)h->ft_dep; kp.mv_from = h->ft_from; kp.mv_tgt = h->ft_tgt;
+  kp.mv_y = h->ft_y; kp.mv_D = (T*)h->ft_D; kp.mv_dep = (double*)h->ft_dep; kp.mv_from = h->ft_from; kp.mv_tgt = h->ft_tgt;
   kp.mv_stop = h->ft_stop; kp.mv_order = h->ft_order;
   for (int first = 0; first < h->cfg.max_tracks; first += h->fit_chunk) {
     p.first = first;
@@ -288,21 +303,38 @@ int launch_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, con
   return CKF_OK;
 }
 
-// Picks (or recycles) the workspace for this stream; orders the stream after the workspace's last user.
+// Picks (or recycles) the workspace for this stream and returns it with `busy` LOCKED; the stream is ordered after the
+// workspace's previous work when that ran on another stream.  The caller enqueues, then calls release_ws, which
+// records `done` and unlocks -- on every exit path (WsGuard).
 Workspace* acquire_ws(ckf_handle* h, cudaStream_t st) {
-  std::lock_guard<std::mutex> lk(h->mu);
   Workspace* w = nullptr;
-  for (auto& x : h->ws)
-    if (x.used && x.stream_tag == (void*)st) { w = &x; break; }
-  if (!w)
+  {
+    std::lock_guard<std::mutex> lk(h->mu);
     for (auto& x : h->ws)
-      if (!x.used) { w = &x; break; }
-  if (!w) { w = &h->ws[h->next_ws]; h->next_ws = (h->next_ws + 1) % (int)h->ws.size(); }
-  if (w->used && w->stream_tag != (void*)st) cudaStreamWaitEvent(st, w->done, 0);
-  w->used = true;
-  w->stream_tag = (void*)st;
+      if (x.used && x.stream_tag == (void*)st) { w = &x; break; }
+    if (!w)
+      for (auto& x : h->ws)
+        if (!x.used) { w = &x; break; }
+    if (!w) { w = &h->ws[h->next_ws]; h->next_ws = (h->next_ws + 1) % (int)h->ws.size(); }
+    w->used = true;
+    w->stream_tag = (void*)st;
+  }
+  w->busy.lock();  // a previous owner still enqueuing: wait for it (and for its cudaEventRecord) on the host
+  if (w->done_valid && w->done_stream != (void*)st) cudaStreamWaitEvent(st, w->done, 0);
   return w;
 }
+
+void release_ws(Workspace* w, cudaStream_t st) {
+  cudaEventRecord(w->done, st);
+  w->done_stream = (void*)st;
+  w->done_valid = true;
+  w->busy.unlock();
+}
+
+struct WsGuard {
+  Workspace* w; cudaStream_t st;
+  ~WsGuard() { release_ws(w, st); }
+};
 
 }  // namespace
 
@@ -310,7 +342,7 @@ extern "C" {
 
 int ckf_abi_version(void) { return CKF_ABI_VERSION; }
 
-const char* ckf_last_error(const ckf_handle* h) { return h ? h->err.c_str() : g_create_error.c_str(); }
+const char* ckf_last_error(const ckf_handle* h) { (void)h; return g_error.c_str(); }
 
 int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, ckf_handle** out) {
   ckf_handle* h = nullptr;
@@ -323,7 +355,8 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     return fail(h, CKF_E_ARG, "max_candidates_per_seed must be in 1..256");
   if (c->max_levels < 1 || c->max_levels > 64) return fail(h, CKF_E_ARG, "max_levels must be in 1..64");
   if (c->min_measurements < 1) return fail(h, CKF_E_ARG, "min_measurements must be >= 1");
-  if (c->max_seeds < 1 || c->max_measurements < 0 || c->max_tracks < 1 || c->max_track_entries < 1 || c->n_streams < 1)
+  if (c->max_seeds < 1 || c->max_measurements < 0 || c->max_tracks < 1 || c->max_track_entries < 1 || c->n_streams < 1 ||
+      c->max_fit_tracks < 0)
     return fail(h, CKF_E_ARG, "capacities must be positive");
   if (g->n_layers < 1 || g->n_modules < 1) return fail(h, CKF_E_ARG, "empty geometry");
   if (f->kind != 0 && f->kind != 1) return fail(h, CKF_E_ARG, "field kind must be 0 or 1");
@@ -340,7 +373,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
   if (h->cfg.max_events_per_find <= 0) h->cfg.max_events_per_find = 1;
   if (h->cfg.max_links <= 0) h->cfg.max_links = (int32_t)std::min<long long>(48LL * c->max_seeds, 0x7ffffff0LL);
   h->tsize = c->precision == 32 ? 4 : 8;
-  auto bail = [&](int code) { std::string e = h->err; ckf_destroy(h); g_create_error = e; return code; };
+  auto bail = [&](int code) { std::string e = g_error; ckf_destroy(h); g_error = e; return code; };
   cudaDeviceProp prop;
   if (cudaGetDevice(&h->device) != cudaSuccess || cudaGetDeviceProperties(&prop, h->device) != cudaSuccess) {
     fail(h, CKF_E_CUDA, "cudaGetDeviceProperties failed");
@@ -421,21 +454,21 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
   h->tcap = h->cfg.max_tips_per_level;
   // ---- workspaces
   const size_t L = (size_t)h->cfg.max_links, S = (size_t)c->max_seeds, ts = (size_t)h->tsize;
-  h->ws.resize(c->n_streams);
+  for (int i = 0; i < c->n_streams; ++i) h->ws.emplace_back();
   for (auto& w : h->ws) {
     CKB(dalloc(h, &w.lk_x, 6 * L * sizeof(double)));
-    CKB(dalloc(h, (char**)&w.lk_C, 21 * L * ts));
+    CKB(dalloc(h, (char**)&w.lk_C, 21 * L * sizeof(double)));
     CKB(dalloc(h, &w.lk_module, L * 4)); CKB(dalloc(h, &w.lk_parent, L * 4)); CKB(dalloc(h, &w.lk_meas, L * 4));
     CKB(dalloc(h, &w.lk_counts, L * 4)); CKB(dalloc(h, &w.lk_lastmeas, L * 4));
-    CKB(dalloc(h, (char**)&w.lk_chi2, L * ts)); CKB(dalloc(h, (char**)&w.lk_chi2sum, L * ts));
+    CKB(dalloc(h, (char**)&w.lk_chi2, L * ts)); CKB(dalloc(h, (char**)&w.lk_chi2sum, L * sizeof(double)));
     CKB(dalloc(h, &w.sd, (4 * S + 2 * (S + 1)) * 4));
     CKB(dalloc(h, &w.seed_tile, 2 * ((S + SEED_TILE - 1) / SEED_TILE + 2) * 4));
     CKB(dalloc(h, &w.leaf, 3 * S * (size_t)c->max_candidates_per_seed * 4));
     const size_t TC = (size_t)h->tcap, KB = (size_t)c->max_branches_per_surface;
     CKB(dalloc(h, &w.tip_link, 2 * TC * 4)); CKB(dalloc(h, &w.tip_seed, 2 * TC * 4));
     CKB(dalloc(h, &w.mv_y, 8 * TC * sizeof(double))); CKB(dalloc(h, &w.pd_x, 6 * TC * sizeof(double)));
-    CKB(dalloc(h, (char**)&w.mv_D, (size_t)MVD * TC * ts)); CKB(dalloc(h, (char**)&w.mv_dep, 5 * TC * ts));
-    CKB(dalloc(h, (char**)&w.pd_C, 21 * TC * ts)); CKB(dalloc(h, (char**)&w.sel_chi2, KB * TC * ts));
+    CKB(dalloc(h, (char**)&w.mv_D, (size_t)MVD * TC * ts)); CKB(dalloc(h, (char**)&w.mv_dep, 5 * TC * sizeof(double)));
+    CKB(dalloc(h, (char**)&w.pd_C, 21 * TC * sizeof(double))); CKB(dalloc(h, (char**)&w.sel_chi2, KB * TC * ts));
     CKB(dalloc(h, &w.sel_idx, KB * TC * 4));
     CKB(dalloc(h, &w.mv_from, TC * 4)); CKB(dalloc(h, &w.mv_tgt, 2 * TC * 4)); CKB(dalloc(h, &w.mv_stop, TC * 4));
     CKB(dalloc(h, &w.t_nsel, TC * 4)); CKB(dalloc(h, &w.t_want, TC * 4)); CKB(dalloc(h, &w.t_counts, TC * 4));
@@ -447,6 +480,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     CKB(dalloc(h, &w.s_idx, (size_t)c->max_measurements * 4));
     CKB(dalloc(h, (char**)&w.s_v0max, (size_t)g->n_modules * (size_t)h->cfg.max_events_per_find * ts));
     CKB(dalloc(h, &w.globals, GBLK * 4));
+    CKB(cudaMemset(w.globals, 0, GBLK * 4));
     static_assert(G_N <= GBLK, "globals block too small");
     CKB(dalloc(h, &w.mv_order, (size_t)NBIN * TC * 4));
     CKB(dalloc(h, &w.counters, CNT_N * 8));
@@ -456,12 +490,28 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     CKB(dalloc(h, &w.h_moff, ((size_t)g->n_modules * (size_t)h->cfg.max_events_per_find + 1) * 4));
     CKB(dalloc(h, (char**)&w.h_loc, 2 * M * ts)); CKB(dalloc(h, (char**)&w.h_var, 2 * M * ts));
     CKB(dalloc(h, &w.h_smod, S * 4)); CKB(dalloc(h, (char**)&w.h_sx, 6 * S * ts)); CKB(dalloc(h, (char**)&w.h_sC, 36 * S * ts));
-    CKB(dalloc(h, &w.o_nt, 2 * 4)); CKB(dalloc(h, &w.o_off, (NTK + 1) * 4)); CKB(dalloc(h, &w.o_meas, NE * 4));
+    CKB(dalloc(h, &w.o_nt, 8 * 4)); CKB(dalloc(h, &w.o_off, (NTK + 1) * 4)); CKB(dalloc(h, &w.o_meas, NE * 4));
     CKB(dalloc(h, &w.o_seed, NTK * 4)); CKB(dalloc(h, &w.o_nh, NTK * 4)); CKB(dalloc(h, &w.o_lm, NTK * 4));
     CKB(dalloc(h, &w.o_stop, NTK * 4));
     CKB(dalloc(h, (char**)&w.o_par, 6 * NTK * ts)); CKB(dalloc(h, (char**)&w.o_cov, 36 * NTK * ts));
     CKB(dalloc(h, (char**)&w.o_c2, NTK * ts)); CKB(dalloc(h, (char**)&w.o_ec2, NE * ts));
-    CKB(cudaMallocHost((void**)&w.pinned_nt, 2 * 4));
+    CKB(cudaMallocHost((void**)&w.pinned_nt, 4 * 4));
+  }
+  // ---- state store of ckf_fit (row f1): reserved here, so that ckf_fit allocates nothing
+  if (c->max_fit_tracks > 0) {
+    const int chunk = std::min(std::min(c->max_fit_tracks, c->max_tracks), (int)FIT_CHUNK), ns = c->max_levels;
+    const size_t n = (size_t)ns * (size_t)chunk, CHK = (size_t)chunk;
+    CKB(dalloc(h, &h->fs_x, n * FS_X * sizeof(double)));
+    CKB(dalloc(h, (char**)&h->fs_t, n * FS_T * ts));
+    CKB(dalloc(h, &h->fs_meas, n * 4));
+    CKB(dalloc(h, &h->fs_next, CHK * 4));
+    CKB(dalloc(h, &h->ft_g, 2 * GBLK * 4)); CKB(dalloc(h, &h->ft_counters, CNT_N * 8));
+    CKB(dalloc(h, &h->ft_y, 8 * CHK * sizeof(double)));
+    CKB(dalloc(h, (char**)&h->ft_D, (size_t)MVD * CHK * ts)); CKB(dalloc(h, (char**)&h->ft_dep, 5 * CHK * sizeof(double)));
+    CKB(dalloc(h, &h->ft_from, CHK * 4)); CKB(dalloc(h, &h->ft_tgt, 2 * CHK * 4)); CKB(dalloc(h, &h->ft_stop, CHK * 4));
+    CKB(dalloc(h, &h->ft_order, (size_t)NBIN * CHK * 4));
+    CKB(cudaEventCreateWithFlags(&h->fit_done, cudaEventDisableTiming));
+    h->fit_chunk = chunk; h->fit_states = ns;
   }
 #undef CKB
   *out = h;
@@ -483,10 +533,8 @@ int ckf_find(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, ckf_t
       !o->stop_reason || !o->params || !o->cov || !o->chi2_sum || !o->entry_chi2)
     return fail(h, CKF_E_ARG, "null output array");
   cudaStream_t st = (cudaStream_t)stream;
-  Workspace* w = acquire_ws(h, st);
-  int rc = h->cfg.precision == 32 ? launch_find<float>(h, *w, m, s, o, st) : launch_find<double>(h, *w, m, s, o, st);
-  cudaEventRecord(w->done, st);
-  return rc;
+  WsGuard g{acquire_ws(h, st), st};
+  return h->cfg.precision == 32 ? launch_find<float>(h, *g.w, m, s, o, st) : launch_find<double>(h, *g.w, m, s, o, st);
 }
 
 int ckf_find_host(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, ckf_tracks* o, void* stream) {
@@ -496,8 +544,14 @@ int ckf_find_host(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, 
     return fail(h, CKF_E_CAPACITY, "n_seeds %d / n_measurements %d exceed capacity", s->n, m->n);
   if (m->n_events < 0 || m->n_events > h->cfg.max_events_per_find)
     return fail(h, CKF_E_CAPACITY, "n_events %d exceeds max_events_per_find %d", m->n_events, h->cfg.max_events_per_find);
+  if (!m->module_offsets || (m->n > 0 && (!m->loc || !m->var)) || (s->n > 0 && (!s->module_id || !s->params || !s->cov)))
+    return fail(h, CKF_E_ARG, "null input array");
+  if (!o->n_tracks || !o->status || !o->track_offsets || !o->meas_idx || !o->seed_id || !o->n_holes || !o->last_module ||
+      !o->stop_reason || !o->params || !o->cov || !o->chi2_sum || !o->entry_chi2)
+    return fail(h, CKF_E_ARG, "null output array");
   cudaStream_t st = (cudaStream_t)stream;
-  Workspace* w = acquire_ws(h, st);
+  WsGuard g{acquire_ws(h, st), st};
+  Workspace* w = g.w;
   const size_t ts = (size_t)h->tsize;
   CK(cudaMemcpyAsync(w->h_moff, m->module_offsets, ((size_t)h->n_modules * (size_t)std::max(1, m->n_events) + 1) * 4,
                      cudaMemcpyHostToDevice, st));
@@ -510,27 +564,52 @@ int ckf_find_host(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, 
   ckf_seeds ds = {s->n, w->h_smod, w->h_sx, w->h_sC};
   ckf_tracks dt = {w->o_nt, w->o_nt + 1, w->o_off, w->o_meas, w->o_seed, w->o_nh, w->o_lm, w->o_stop,
                    w->o_par, w->o_cov, w->o_c2, w->o_ec2};
-  int rc = h->cfg.precision == 32 ? launch_find<float>(h, *w, &dm, &ds, &dt, st) : launch_find<double>(h, *w, &dm, &ds, &dt, st);
+  // ckf_finalize leaves (candidates, status, entries) in o_nt[4..6] (o_nt[0], o_nt[1] are *n_tracks and *status)
+  int rc = h->cfg.precision == 32 ? launch_find<float>(h, *w, &dm, &ds, &dt, st, w->o_nt + 4)
+                                  : launch_find<double>(h, *w, &dm, &ds, &dt, st, w->o_nt + 4);
   if (rc != CKF_OK) return rc;
-  CK(cudaMemcpyAsync(w->pinned_nt, w->o_nt, 8, cudaMemcpyDeviceToHost, st));
+  CK(cudaMemcpyAsync(w->pinned_nt, w->o_nt + 4, 12, cudaMemcpyDeviceToHost, st));
+  // The result sizes are only known on the device.  Instead of stopping the stream to learn them, the copies are
+  // issued at once for a GUESS (the sizes of the handle's previous ckf_find_host result + 1/8), the stream is
+  // synchronised once, and only a result that outgrew the guess costs a second round for its tail.  The first call on
+  // a handle has no guess and takes two rounds.
+  auto copy_tracks = [&](size_t t0, size_t t1) -> int {   // per-track arrays, tracks [t0, t1); offsets [t0, t1]
+    if (t1 <= t0) return CKF_OK;
+    const size_t n = t1 - t0;
+    CK(cudaMemcpyAsync(o->track_offsets + t0, w->o_off + t0, (n + 1) * 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(o->seed_id + t0, w->o_seed + t0, n * 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(o->n_holes + t0, w->o_nh + t0, n * 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(o->last_module + t0, w->o_lm + t0, n * 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync(o->stop_reason + t0, w->o_stop + t0, n * 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync((char*)o->params + 6 * t0 * ts, (char*)w->o_par + 6 * t0 * ts, 6 * n * ts, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync((char*)o->cov + 36 * t0 * ts, (char*)w->o_cov + 36 * t0 * ts, 36 * n * ts, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync((char*)o->chi2_sum + t0 * ts, (char*)w->o_c2 + t0 * ts, n * ts, cudaMemcpyDeviceToHost, st));
+    return CKF_OK;
+  };
+  auto copy_entries = [&](size_t e0, size_t e1) -> int {
+    if (e1 <= e0) return CKF_OK;
+    CK(cudaMemcpyAsync(o->meas_idx + e0, w->o_meas + e0, (e1 - e0) * 4, cudaMemcpyDeviceToHost, st));
+    CK(cudaMemcpyAsync((char*)o->entry_chi2 + e0 * ts, (char*)w->o_ec2 + e0 * ts, (e1 - e0) * ts, cudaMemcpyDeviceToHost, st));
+    return CKF_OK;
+  };
+  size_t gt = 0, ge = 0;
+  const int ht = h->hint_tracks.load(), he = h->hint_entries.load();
+  if (ht >= 0) {
+    gt = std::min<size_t>((size_t)h->cfg.max_tracks, (size_t)ht + (size_t)ht / 8 + 256);
+    ge = std::min<size_t>((size_t)h->cfg.max_track_entries, (size_t)he + (size_t)he / 8 + 4096);
+    if ((rc = copy_tracks(0, gt)) != CKF_OK || (rc = copy_entries(0, ge)) != CKF_OK) return rc;
+  }
   CK(cudaStreamSynchronize(st));
-  const size_t nt = (size_t)w->pinned_nt[0];
+  const size_t nt = (size_t)w->pinned_nt[0], ne = (size_t)w->pinned_nt[2];
   *o->n_tracks = w->pinned_nt[0];
   *o->status = w->pinned_nt[1];
-  CK(cudaMemcpyAsync(o->track_offsets, w->o_off, (nt + 1) * 4, cudaMemcpyDeviceToHost, st));
-  CK(cudaMemcpyAsync(o->seed_id, w->o_seed, nt * 4, cudaMemcpyDeviceToHost, st));
-  CK(cudaMemcpyAsync(o->n_holes, w->o_nh, nt * 4, cudaMemcpyDeviceToHost, st));
-  CK(cudaMemcpyAsync(o->last_module, w->o_lm, nt * 4, cudaMemcpyDeviceToHost, st));
-  CK(cudaMemcpyAsync(o->stop_reason, w->o_stop, nt * 4, cudaMemcpyDeviceToHost, st));
-  CK(cudaMemcpyAsync(o->params, w->o_par, 6 * nt * ts, cudaMemcpyDeviceToHost, st));
-  CK(cudaMemcpyAsync(o->cov, w->o_cov, 36 * nt * ts, cudaMemcpyDeviceToHost, st));
-  CK(cudaMemcpyAsync(o->chi2_sum, w->o_c2, nt * ts, cudaMemcpyDeviceToHost, st));
-  CK(cudaStreamSynchronize(st));  // track_offsets[nt] is needed for the entry count
-  const size_t ne = nt ? (size_t)o->track_offsets[nt] : 0;
-  CK(cudaMemcpyAsync(o->meas_idx, w->o_meas, ne * 4, cudaMemcpyDeviceToHost, st));
-  CK(cudaMemcpyAsync(o->entry_chi2, w->o_ec2, ne * ts, cudaMemcpyDeviceToHost, st));
-  CK(cudaStreamSynchronize(st));
-  cudaEventRecord(w->done, st);
+  if (nt > gt || ne > ge) {
+    if ((rc = copy_tracks(gt, nt)) != CKF_OK || (rc = copy_entries(ge, ne)) != CKF_OK) return rc;
+    CK(cudaStreamSynchronize(st));
+  }
+  if (nt == 0) o->track_offsets[0] = 0;
+  h->hint_tracks.store((int)nt);
+  h->hint_entries.store((int)ne);
   return CKF_OK;
 }
 
@@ -546,27 +625,12 @@ int ckf_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, const 
     return fail(h, CKF_E_ARG, "smoother_precision 32 needs a handle of precision 32");
   if (!o->status || !o->n_states || !o->chi2_sum || !o->last_params || !o->last_cov || !o->first_cov || !o->entry_params)
     return fail(h, CKF_E_ARG, "null output array");
+  if ((m->n > 0 && (!m->loc || !m->var)) || (s->n > 0 && (!s->module_id || !s->params || !s->cov)))
+    return fail(h, CKF_E_ARG, "null input array");
+  if (!h->fs_x) return fail(h, CKF_E_CAPACITY, "ckf_fit needs a state store: create the handle with max_fit_tracks > 0");
   cudaStream_t st = (cudaStream_t)stream;
   std::lock_guard<std::mutex> lk(h->mu);
-  if (!h->fs_x) {  // first call: reserve the state store
-    const int chunk = std::min(h->cfg.max_tracks, (int)FIT_CHUNK), ns = h->cfg.max_levels;
-    const size_t n = (size_t)ns * (size_t)chunk;
-    double* fx = nullptr; char* ft = nullptr; int32_t* fm = nullptr;
-    CK(dalloc(h, &fx, n * FS_X * sizeof(double)));
-    CK(dalloc(h, &ft, n * FS_T * (size_t)h->tsize));
-    CK(dalloc(h, &fm, n * 4));
-    const size_t CHK = (size_t)chunk, ts = (size_t)h->tsize;
-    CK(dalloc(h, &h->fs_next, CHK * 4));
-    CK(dalloc(h, &h->ft_g, 2 * GBLK * 4)); CK(dalloc(h, &h->ft_counters, CNT_N * 8));
-    CK(dalloc(h, &h->ft_y, 8 * CHK * sizeof(double)));
-    CK(dalloc(h, (char**)&h->ft_D, (size_t)MVD * CHK * ts)); CK(dalloc(h, (char**)&h->ft_dep, 5 * CHK * ts));
-    CK(dalloc(h, &h->ft_from, CHK * 4)); CK(dalloc(h, &h->ft_tgt, 2 * CHK * 4)); CK(dalloc(h, &h->ft_stop, CHK * 4));
-    CK(dalloc(h, &h->ft_order, (size_t)NBIN * CHK * 4));
-    CK(cudaEventCreateWithFlags(&h->fit_done, cudaEventDisableTiming));
-    h->fs_x = fx; h->fs_t = ft; h->fs_meas = fm; h->fit_chunk = chunk; h->fit_states = ns;
-  } else {
-    cudaStreamWaitEvent(st, h->fit_done, 0);  // one state store: fits are ordered one after the other
-  }
+  cudaStreamWaitEvent(st, h->fit_done, 0);  // one state store: fits are ordered one after the other
   int rc = h->cfg.precision == 32 ? launch_fit<float>(h, m, s, t, o, st) : launch_fit<double>(h, m, s, t, o, st);
   cudaEventRecord(h->fit_done, st);
   return rc;

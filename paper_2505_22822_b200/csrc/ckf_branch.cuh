@@ -266,13 +266,14 @@ __global__ void __launch_bounds__(SCAN_NT, CKF_UPDATE_MINB) ckf_update(const KPa
     const int pc = p.t_counts[par];
     const int target = p.mv_tgt[par];
     double x[6], xo[6];
-    T C[21];
+    double C[21];
 #pragma unroll
     for (int i = 0; i < 6; ++i) x[i] = p.pd_x[i * TC + par];
 #pragma unroll
     for (int i = 0; i < 21; ++i) C[i] = p.pd_C[i * TC + par];
     int meas = -1, ncounts, nlast = plink >= 0 ? p.lk_lastmeas[plink] : -1;
-    T chi2 = T(0), nc2s = plink >= 0 ? p.lk_chi2sum[plink] : T(0);
+    T chi2 = T(0);
+    double nc2s = plink >= 0 ? p.lk_chi2sum[plink] : 0.0;
     if (p.t_nsel[par] == 0) {
       ncounts = pc + (1 << 16);
 #pragma unroll
@@ -284,12 +285,12 @@ __global__ void __launch_bounds__(SCAN_NT, CKF_UPDATE_MINB) ckf_update(const KPa
       chi2 = p.sel_chi2[j * TC + par];
       const auto lc = __ldg(p.loc + meas);
       const auto vr = __ldg(p.var + meas);
-      T Co[21];
-      kalman_update<T>(x, C, lc.x, lc.y, vr.x, vr.y, xo, Co);
+      double Co[21];
+      kalman_update(x, C, lc.x, lc.y, vr.x, vr.y, xo, Co);
       ncounts = pc + 1;
       nlast = nl;
       my_updates += 1ull;
-      nc2s += chi2;
+      nc2s += (double)chi2;
 #pragma unroll
       for (int i = 0; i < 6; ++i) p.lk_x[(size_t)i * p.max_links + nl] = xo[i];
 #pragma unroll
@@ -310,8 +311,8 @@ __global__ void __launch_bounds__(SCAN_NT, CKF_UPDATE_MINB) ckf_update(const KPa
     if ((ncounts & 0xffff) + (ncounts >> 16) >= p.cfg.max_levels) stop = STOP_LEVEL_LIMIT;
     else {
       Traj y;
-      T dep[5];
-      stop = departure_state<T>(p.geo, p.cfg, target, xo, y, dep);
+      double dep[5];
+      stop = departure_state(p.geo, p.cfg, target, xo, y, dep);
       if (stop == STOP_NONE) {
         store_traj(p.mv_y, (size_t)c, y);
 #pragma unroll

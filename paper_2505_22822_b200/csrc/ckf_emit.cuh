@@ -12,11 +12,17 @@ __global__ void ckf_init_event(const KParams<T> p) {
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < p.n_seeds) {
     p.sd_extra[i] = 0; p.sd_nemit[i] = 0; p.sd_nentries[i] = 0;
-    p.sd_eoff[i] = (p.seed_module[i] / p.geo.n_modules) * p.geo.n_modules;
+    // a seed whose (virtual) module id is out of range is malformed input: it is flagged (sd_eoff < 0), stops NUMERIC
+    // at level 0 and sets CKF_STATUS_BAD_INPUT; nothing is ever indexed with its module id
+    const int sm = p.seed_module[i];
+    const bool bad = sm < 0 || sm >= p.n_vmod;
+    p.sd_eoff[i] = bad ? -1 : (sm / p.geo.n_modules) * p.geo.n_modules;
+    if (bad) atomicOr(p.g + G_BAD_INPUT, 1);
     if (i < p.tcap) { p.tip_link[i] = -1; p.tip_seed[i] = i; p.mv_stop[i] = STOP_NONE; }
   }
   if (i == 0) {
-    for (int k = 0; k < G_N; ++k) p.g[k] = 0;
+    for (int k = 0; k < G_N; ++k)
+      if (k != G_BAD_INPUT) p.g[k] = 0;   // G_BAD_INPUT is cleared by ckf_finalize (other threads of this launch set it)
     p.g[G_FIRST_BAD] = INT_MAX;
     p.g[G_NTIPS0] = p.n_seeds < p.tcap ? p.n_seeds : p.tcap;
     *p.o_status = p.n_seeds > p.tcap ? 4 : 0;
@@ -123,13 +129,13 @@ __global__ void __launch_bounds__(256) ckf_emit_tracks(const KParams<T> p) {
     p.o_nholes[t] = meta >> 8;
     p.o_stop[t] = meta & 0xff;
     p.o_lastmod[t] = p.lk_module[ls];
-    p.o_chi2sum[t] = p.lk_chi2sum[leaf];
+    p.o_chi2sum[t] = (T)p.lk_chi2sum[leaf];
 #pragma unroll
     for (int i = 0; i < 6; ++i) p.o_params[(size_t)t * 6 + i] = (T)p.lk_x[(size_t)i * p.max_links + ls];
 #pragma unroll
     for (int i = 0; i < 6; ++i)
 #pragma unroll
-      for (int k = 0; k < 6; ++k) p.o_cov[(size_t)t * 36 + i * 6 + k] = p.lk_C[(size_t)tri(i, k) * p.max_links + ls];
+      for (int k = 0; k < 6; ++k) p.o_cov[(size_t)t * 36 + i * 6 + k] = (T)p.lk_C[(size_t)tri(i, k) * p.max_links + ls];
   }
 }
 
@@ -139,6 +145,9 @@ __global__ void ckf_finalize(const KParams<T> p) {
   const int n = total < bad ? total : bad;
   *p.o_ntracks = n;
   if (n == 0) p.o_offsets[0] = 0;
+  if (p.g[G_BAD_INPUT]) { atomicOr(p.o_status, 8); p.g[G_BAD_INPUT] = 0; }
+  // what ckf_find_host needs to size its copies: candidates, status, entries
+  if (p.o_summary) { p.o_summary[0] = n; p.o_summary[1] = *p.o_status; p.o_summary[2] = n > 0 ? p.o_offsets[n] : 0; }
 }
 
 }  // namespace ckf

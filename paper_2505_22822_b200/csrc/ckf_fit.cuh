@@ -20,9 +20,10 @@ namespace ckf {
 
 constexpr int FIT_NT = 128;
 constexpr int FIT_CHUNK = 262144;   // tracks per pass: bounds the state store (ckf.cu loops over the chunks)
-constexpr int FS_X = 12;            // float64 per state: xp[6], xf[6]
-constexpr int FS_T = 21 + 21 + 25 + 2;  // T per state: Cp, Cf (packed upper triangles), J (5x5 block, row-major),
-                                        // V5 variances (phi, theta) added on leaving the previous state
+// float64 per state: xp[6], xf[6], Cp[21], Cf[21] (packed upper triangles), the V5 variances (phi, theta) added on
+// leaving the previous state -- the covariance algebra is float64 in both modes
+constexpr int FS_XP = 0, FS_XF = 6, FS_CP = 12, FS_CF = 33, FS_Q = 54, FS_X = 56;
+constexpr int FS_T = 25;            // T per state: J (5x5 block, row-major), built from the T-typed transport Jacobian
 
 template <typename T>
 struct FitParams {
@@ -78,14 +79,15 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, con
     const int sd0 = p.seed[tr];
     const int eoff = (p.seed_module[sd0] / p.geo.n_modules) * p.geo.n_modules;  // batch of events: see KParams::n_vmod
     double xp[6], xf[6];
-    T Cp[21], Cf[21], J[5][5];
+    double Cp[21], Cf[21], J[5][5];
     int status = STOP_NONE, module = 0, next = 0, stored = level;
     bool done = false;
-    T c2sum = T(0), q_in[2] = {T(0), T(0)};
+    T c2sum = T(0);
+    double q_in[2] = {0.0, 0.0};
 #pragma unroll
     for (int i = 0; i < 6; ++i) xf[i] = 0.0;
 #pragma unroll
-    for (int i = 0; i < 21; ++i) Cf[i] = T(0);
+    for (int i = 0; i < 21; ++i) Cf[i] = 0.0;
     if (level == 0) {  // N6: the seed's own module, identity transport
       const int sd = sd0;
       bool ok = true;
@@ -95,11 +97,11 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, con
 #pragma unroll
       for (int i = 0; i < 6; ++i)
 #pragma unroll
-        for (int j = i; j < 6; ++j) Cp[tri(i, j)] = p.seed_C[(size_t)sd * 36 + i * 6 + j];
+        for (int j = i; j < 6; ++j) Cp[tri(i, j)] = (double)p.seed_C[(size_t)sd * 36 + i * 6 + j];
 #pragma unroll
       for (int a = 0; a < 5; ++a)
 #pragma unroll
-        for (int b = 0; b < 5; ++b) J[a][b] = (a == b && a < 4) ? T(1) : T(0);
+        for (int b = 0; b < 5; ++b) J[a][b] = (a == b && a < 4) ? 1.0 : 0.0;
       module = p.seed_module[sd] - eoff;
       if (n < 1) done = true;
       else if (!ok) status = STOP_NUMERIC;
@@ -114,19 +116,19 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, con
         load_jac(kp.mv_D, (size_t)s, m.D);
         m.from = kp.mv_from[s];
         m.tgt = kp.mv_tgt[s];
-        T dep[5];
+        double dep[5];
 #pragma unroll
         for (int i = 0; i < 5; ++i) dep[i] = kp.mv_dep[i * CH + s];
         status = move_arrive<T>(m, dep, p.geo, p.fld, p.cfg, xp, J);
         if (status == STOP_NONE) {
-          T C[21];
-          const T* pt = p.fs_t + (size_t)(level - 1) * FS_T * CH + s;  // filtered covariance of the previous state
+          double C[21];
+          const double* pt = p.fs_x + (size_t)(level - 1) * FS_X * CH + s;  // filtered covariance of the previous state
 #pragma unroll
-          for (int i = 0; i < 21; ++i) C[i] = pt[(21 + i) * CH];
+          for (int i = 0; i < 21; ++i) C[i] = pt[(FS_CF + i) * CH];
           C[tri(2, 2)] += dep[3];  // V5 on leaving
           C[tri(3, 3)] += dep[4];
           q_in[0] = dep[3]; q_in[1] = dep[4];
-          transport_cov<T>(J, C, Cp);
+          transport_cov<double>(J, C, Cp);
           bool fin = true;
 #pragma unroll
           for (int i = 0; i < 21; ++i) fin = fin && isfinite(Cp[i]);
@@ -140,10 +142,10 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, con
       int used = -1;
       if (k >= p.moff[eoff + module] && k < p.moff[eoff + module + 1]) {
         const typename Vec2<T>::type mm = p.loc[k], vv = p.var[k];
-        const double c2 = predicted_chi2<double>(xp[0], xp[1], (double)Cp[tri(0, 0)], (double)Cp[tri(0, 1)],
-                                                 (double)Cp[tri(1, 1)], (double)mm.x, (double)mm.y, (double)vv.x, (double)vv.y);
+        const double c2 = predicted_chi2<double>(xp[0], xp[1], Cp[tri(0, 0)], Cp[tri(0, 1)], Cp[tri(1, 1)], (double)mm.x,
+                                                 (double)mm.y, (double)vv.x, (double)vv.y);
         c2sum += (T)c2;
-        kalman_update<T>(xp, Cp, mm.x, mm.y, vv.x, vv.y, xf, Cf);
+        kalman_update(xp, Cp, mm.x, mm.y, vv.x, vv.y, xf, Cf);
         used = k;
         ++next;
         w_upd += 1;
@@ -156,23 +158,23 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, con
       double* fx = p.fs_x + (size_t)level * FS_X * CH + s;
       T* ft = p.fs_t + (size_t)level * FS_T * CH + s;
 #pragma unroll
-      for (int i = 0; i < 6; ++i) { fx[i * CH] = xp[i]; fx[(6 + i) * CH] = xf[i]; }
+      for (int i = 0; i < 6; ++i) { fx[(FS_XP + i) * CH] = xp[i]; fx[(FS_XF + i) * CH] = xf[i]; }
 #pragma unroll
-      for (int i = 0; i < 21; ++i) { ft[i * CH] = Cp[i]; ft[(21 + i) * CH] = Cf[i]; }
+      for (int i = 0; i < 21; ++i) { fx[(FS_CP + i) * CH] = Cp[i]; fx[(FS_CF + i) * CH] = Cf[i]; }
 #pragma unroll
       for (int a = 0; a < 5; ++a)
 #pragma unroll
-        for (int b = 0; b < 5; ++b) ft[(42 + a * 5 + b) * CH] = J[a][b];
-      ft[67 * CH] = q_in[0];
-      ft[68 * CH] = q_in[1];
+        for (int b = 0; b < 5; ++b) ft[(a * 5 + b) * CH] = (T)J[a][b];
+      fx[(FS_Q + 0) * CH] = q_in[0];
+      fx[(FS_Q + 1) * CH] = q_in[1];
       p.fs_meas[(size_t)level * CH + s] = used;
       stored = level + 1;
       if (next == n) done = true;
       else if (stored >= p.cfg.max_levels || stored >= p.max_states) status = STOP_LEVEL_LIMIT;
       else {
         Traj y;
-        T dep[5];
-        status = departure_state<T>(p.geo, p.cfg, module, xf, y, dep);
+        double dep[5];
+        status = departure_state(p.geo, p.cfg, module, xf, y, dep);
         if (status == STOP_NONE) {  // the track as a tip of the next level's ckf_step
           store_traj(kp.mv_y, (size_t)s, y);
 #pragma unroll
@@ -199,7 +201,7 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, con
 #pragma unroll
       for (int i = 0; i < 6; ++i)
 #pragma unroll
-        for (int j = 0; j < 6; ++j) p.o_lastC[(size_t)tr * 36 + i * 6 + j] = good ? Cf[tri(i, j)] : T(0);
+        for (int j = 0; j < 6; ++j) p.o_lastC[(size_t)tr * 36 + i * 6 + j] = good ? (T)Cf[tri(i, j)] : T(0);
     }
   }
   // step schedule of the next level: append the running track to its cost class (as ckf_update does)
@@ -306,9 +308,9 @@ __global__ void __launch_bounds__(FIT_NT, CKF_SMOOTH_MINB) ckf_fit_smooth(const 
       const double* fx = p.fs_x + (size_t)(ns - 1) * FS_X * CH + s;
       const T* ft = p.fs_t + (size_t)(ns - 1) * FS_T * CH + s;
 #pragma unroll
-      for (int i = 0; i < 6; ++i) xs[i] = (A)fx[(6 + i) * CH];
+      for (int i = 0; i < 6; ++i) xs[i] = (A)fx[(FS_XF + i) * CH];
 #pragma unroll
-      for (int i = 0; i < 21; ++i) Cs[i] = (A)ft[(size_t)(21 + i) * CH];
+      for (int i = 0; i < 21; ++i) Cs[i] = (A)fx[(size_t)(FS_CF + i) * CH];
       for (int k = ns - 1;; --k) {
         if (p.fs_meas[(size_t)k * CH + s] >= 0) {
 #pragma unroll
@@ -331,11 +333,11 @@ __global__ void __launch_bounds__(FIT_NT, CKF_SMOOTH_MINB) ckf_fit_smooth(const 
         {
           A G[21];
 #pragma unroll
-          for (int i = 0; i < 21; ++i) { G[i] = (A)bt[(size_t)i * CH]; dC[i] = Cs[i] - G[i]; }
+          for (int i = 0; i < 21; ++i) { G[i] = (A)bx[(size_t)(FS_CP + i) * CH]; dC[i] = Cs[i] - G[i]; }
           if (!chol6_scaled<A>(G, sc, L)) { good = false; break; }
         }
 #pragma unroll
-        for (int i = 0; i < 21; ++i) Cf[i] = (A)at[(size_t)(21 + i) * CH];
+        for (int i = 0; i < 21; ++i) Cf[i] = (A)ax[(size_t)(FS_CF + i) * CH];
         // X = Cp^-1 (Jf Cf) = A_k^T, column by column.  Jf rows 0..3 = J[0..3] over columns 0..4, row 4 = e_4,
         // row 5 = J[4] plus 1 at column 5
         A X[6][6];
@@ -344,7 +346,7 @@ __global__ void __launch_bounds__(FIT_NT, CKF_SMOOTH_MINB) ckf_fit_smooth(const 
 #pragma unroll
           for (int r = 0; r < 5; ++r)
 #pragma unroll
-            for (int l = 0; l < 5; ++l) Jb[r][l] = (A)bt[(size_t)(42 + r * 5 + l) * CH];
+            for (int l = 0; l < 5; ++l) Jb[r][l] = (A)bt[(size_t)(r * 5 + l) * CH];
 #pragma unroll
           for (int c = 0; c < 6; ++c) {
             A col[6];
@@ -366,14 +368,14 @@ __global__ void __launch_bounds__(FIT_NT, CKF_SMOOTH_MINB) ckf_fit_smooth(const 
         }
         A dx[6];
 #pragma unroll
-        for (int i = 0; i < 6; ++i) dx[i] = xs[i] - (A)bx[i * CH];
+        for (int i = 0; i < 6; ++i) dx[i] = xs[i] - (A)bx[(FS_XP + i) * CH];
         dx[2] = wrap_pi<A>(dx[2]);
 #pragma unroll
         for (int i = 0; i < 6; ++i) {
           A v = A(0);
 #pragma unroll
           for (int j = 0; j < 6; ++j) v += X[j][i] * dx[j];
-          xs[i] = (A)ax[(6 + i) * CH] + v;
+          xs[i] = (A)ax[(FS_XF + i) * CH] + v;
         }
         xs[2] = wrap_pi<A>(xs[2]);
         // Cs <- sym(Cf + X^T (dC X)), one column of dC X at a time
@@ -464,7 +466,7 @@ __global__ void __launch_bounds__(FIT_NT, CKF_SMOOTH_MINB) ckf_fit_smooth_tf(con
           {
             A Cf[21], sc[6], L[21];
 #pragma unroll
-            for (int i = 0; i < 21; ++i) Cf[i] = (A)ft[(size_t)(21 + i) * CH];
+            for (int i = 0; i < 21; ++i) Cf[i] = (A)fx[(size_t)(FS_CF + i) * CH];
             if (!chol6_scaled<A>(Cf, sc, L)) { good = false; break; }
 #pragma unroll
             for (int i = 0; i < 6; ++i)
@@ -522,7 +524,7 @@ __global__ void __launch_bounds__(FIT_NT, CKF_SMOOTH_MINB) ckf_fit_smooth_tf(con
             A v = A(0);
 #pragma unroll
             for (int l = 0; l < 6; ++l) v += U[l][i] * w[l];
-            xs[i] = (A)fx[(6 + i) * CH] + v;
+            xs[i] = (A)fx[(FS_XF + i) * CH] + v;
           }
           xs[2] = wrap_pi<A>(xs[2]);
 #pragma unroll
@@ -547,14 +549,14 @@ __global__ void __launch_bounds__(FIT_NT, CKF_SMOOTH_MINB) ckf_fit_smooth_tf(con
           const typename Vec2<T>::type mm = p.loc[used], vv = p.var[used];
           Y[tri(0, 0)] += A(1) / (A)vv.x;
           Y[tri(1, 1)] += A(1) / (A)vv.y;
-          y[0] += (A)((double)mm.x - fx[6 * CH]) / (A)vv.x;
-          y[1] += (A)((double)mm.y - fx[7 * CH]) / (A)vv.y;
+          y[0] += (A)((double)mm.x - fx[(FS_XF + 0) * CH]) / (A)vv.x;
+          y[1] += (A)((double)mm.y - fx[(FS_XF + 1) * CH]) / (A)vv.y;
         }
         A yc[6];
         {
           A c6[6];
 #pragma unroll
-          for (int i = 0; i < 6; ++i) c6[i] = (A)(fx[i * CH] - fx[(6 + i) * CH]);
+          for (int i = 0; i < 6; ++i) c6[i] = (A)(fx[(FS_XP + i) * CH] - fx[(FS_XF + i) * CH]);
           c6[2] = wrap_pi<A>(c6[2]);
 #pragma unroll
           for (int i = 0; i < 6; ++i) {
@@ -572,7 +574,7 @@ __global__ void __launch_bounds__(FIT_NT, CKF_SMOOTH_MINB) ckf_fit_smooth_tf(con
           for (int j = 0; j < 6; ++j) {
             if (i == 4) Jf[i][j] = (j == 4) ? A(1) : A(0);
             else if (j == 5) Jf[i][j] = (i == 5) ? A(1) : A(0);
-            else Jf[i][j] = (A)ft[(size_t)(42 + ((i == 5) ? 4 : i) * 5 + j) * CH];
+            else Jf[i][j] = (A)ft[(size_t)(((i == 5) ? 4 : i) * 5 + j) * CH];
           }
         A Yz[21], yz[6];
         {
@@ -601,7 +603,7 @@ __global__ void __launch_bounds__(FIT_NT, CKF_SMOOTH_MINB) ckf_fit_smooth_tf(con
             yz[i] = v;
           }
         }
-        const A qp = (A)ft[67 * CH], qt = (A)ft[68 * CH];
+        const A qp = (A)fx[(FS_Q + 0) * CH], qt = (A)fx[(FS_Q + 1) * CH];
         if (qp > A(0) && qt > A(0)) {  // marginalise the scattering angles u ~ N(0, diag(qp, qt)) on (phi, theta)
           const A s00 = A(1) / qp + Yz[tri(2, 2)], s01 = Yz[tri(2, 3)], s11 = A(1) / qt + Yz[tri(3, 3)];
           const A det = s00 * s11 - s01 * s01;

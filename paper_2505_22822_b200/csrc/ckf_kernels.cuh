@@ -47,7 +47,7 @@ enum CounterId { CNT_TIPS = 0, CNT_VISITS, CNT_TRIALS, CNT_ACCEPTED, CNT_GATE, C
 #define CKF_NBIN 8
 #endif
 enum GlobalId { G_LINK_COUNT = 0, G_FIRST_BAD, G_TOTAL_TRACKS, G_TOTAL_ENTRIES, G_NTIPS0, G_NTIPS1, G_STEP_CURSOR,
-                G_SCAN_TICKET, G_LBASE, G_SEED_TICKET, G_BIN0, G_N = G_BIN0 + CKF_NBIN };
+                G_SCAN_TICKET, G_LBASE, G_SEED_TICKET, G_BAD_INPUT, G_BIN0, G_N = G_BIN0 + CKF_NBIN };
 constexpr int NBIN = CKF_NBIN;    // cost classes of the step schedule (G_BIN0 .. G_BIN0 + NBIN - 1 hold their sizes)
 constexpr int GBLK = 64;          // ints reserved for one block of globals
 
@@ -75,12 +75,12 @@ struct KParams {
   // candidate-link buffer (a10): SoA, one entry per child ever made; a level's links are contiguous
   int32_t max_links;
   double* lk_x;        // [6][max_links]   bound parameters after the visit
-  T* lk_C;             // [21][max_links]  packed covariance after the visit
+  double* lk_C;        // [21][max_links]  packed covariance after the visit (float64 in both modes)
   int32_t* lk_module;  // module visited
   int32_t* lk_parent;  // previous link of the branch, -1 = seed
   int32_t* lk_meas;    // measurement index, -1 = hole
   T* lk_chi2;          // predicted chi2 of that measurement
-  T* lk_chi2sum;
+  double* lk_chi2sum;
   int32_t* lk_counts;  // n_meas | n_holes << 16
   int32_t* lk_lastmeas;  // link of the branch's last measurement (state reported on emission)
   // per seed
@@ -102,14 +102,14 @@ struct KParams {
   // departure / arrival state of the move (ckf_update -> ckf_step -> ckf_visit)
   double* mv_y;        // [tcap][8] r, d, t, q/p (move records, see below)
   T* mv_D;             // [tcap][MVD] transport Jacobian (ckf_step -> ckf_visit)
-  T* mv_dep;           // [5][tcap] direction on departure, Highland q_phi, q_theta
+  double* mv_dep;      // [5][tcap] direction on departure, Highland q_phi, q_theta
   int32_t* mv_from;    // [tcap] module the tip stands on
   int32_t* mv_tgt;     // [2][tcap] module reached; overlap neighbour at departure (N2, by ckf_update), -1 none
   int32_t* mv_stop;    // [tcap] stop reason so far
   int32_t* mv_order;   // [NBIN][tcap] live tips of the level grouped by predicted RKN4 trial count (step schedule)
   // prediction + selection (ckf_visit -> ckf_cap, ckf_update)
   double* pd_x;        // [6][tcap]
-  T* pd_C;             // [21][tcap]
+  double* pd_C;        // [21][tcap]
   T* sel_chi2;         // [K][tcap]
   int32_t* sel_idx;    // [K][tcap]
   int32_t* t_nsel;     // [tcap]
@@ -127,7 +127,18 @@ struct KParams {
   int32_t* o_ntracks; int32_t* o_status; int32_t* o_offsets; int32_t* o_meas; int32_t* o_seed; int32_t* o_nholes;
   int32_t* o_lastmod; int32_t* o_stop;
   T* o_params; T* o_cov; T* o_chi2sum; T* o_entrychi2;
+  int32_t* o_summary;  // [3] or null (ckf_find_host): n_tracks, status, entries, written last by ckf_finalize
 };
+
+// CSR slice of (virtual) module m, clamped into [0, n_meas]: a malformed module_offsets array (not monotonic, or an
+// offset beyond n) shortens slices, it never reads outside loc / var (ckf_sort_slices flags it CKF_STATUS_BAD_INPUT).
+template <typename T>
+__device__ __forceinline__ void slice_of(const KParams<T>& p, int m, int& beg, int& end) {
+  int b = __ldg(p.moff + m), e = __ldg(p.moff + m + 1);
+  b = b < 0 ? 0 : (b > p.n_meas ? p.n_meas : b);
+  e = e < b ? b : (e > p.n_meas ? p.n_meas : e);
+  beg = b; end = e;
+}
 
 // ------------------------------------------------------------------------------------------ move records
 // The state of a move is kept per tip as two contiguous records (AoS), not [component][tip]: ckf_step reaches its tips

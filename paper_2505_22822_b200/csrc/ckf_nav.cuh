@@ -85,8 +85,10 @@ CKF_HD double highland_theta0_sq(double xx0, double cosi, double qop, double mas
 // (l0, l1, phi, theta, q/p); the full 6x6 has row q/p = e_4, column t = e_5.
 //   dep_u, dep_v : axes of the departure module;  dep_d : direction at departure (gives d d/d phi, d d/d theta)
 //   arr          : arrival module;  y : state on its plane;  B : field there
-template <typename T>
-CKF_HD void arrival_jacobian(const Jac<T>& D, const double dep_u[3], const double dep_v[3], const T dep_d[3],
+// T = arithmetic type of the bound->bound block (float64 in the product), TD = type the running
+// transport Jacobian D was accumulated in (float32 in fp32 mode).
+template <typename T, typename TD>
+CKF_HD void arrival_jacobian(const Jac<TD>& D, const double dep_u[3], const double dep_v[3], const T dep_d[3],
                              const ModuleRec& arr, const Traj& y, const double Bd[3], double mass, T J[5][5]) {
   const double lam = KAPPA * y.qop;
   double kd[3];
@@ -115,7 +117,7 @@ CKF_HD void arrival_jacobian(const Jac<T>& D, const double dep_u[3], const doubl
   T nR[3];
 #pragma unroll
   for (int j = 0; j < 3; ++j) nR[j] = n[0] * D.Rd[0][j] + n[1] * D.Rd[1][j] + n[2] * D.Rd[2][j];
-  const T nrq = dot3(n, D.rq), nu0 = dot3(n, u0), nv0 = dot3(n, v0);
+  const T nrq = (T)dot3(n, D.rq), nu0 = dot3(n, u0), nv0 = dot3(n, v0);
   const T nRgphi = dot3(nR, gphi), nRgth = dot3(nR, gth);
   // rows l0, l1
 #pragma unroll
@@ -133,7 +135,7 @@ CKF_HD void arrival_jacobian(const Jac<T>& D, const double dep_u[3], const doubl
     J[a][1] = dot3(wp, v0);
     J[a][2] = dot3(wR, gphi);
     J[a][3] = dot3(wR, gth);
-    J[a][4] = dot3(wp, D.rq);
+    J[a][4] = (T)dot3(wp, D.rq);
   }
   // rows phi, theta
 #pragma unroll
@@ -149,7 +151,7 @@ CKF_HD void arrival_jacobian(const Jac<T>& D, const double dep_u[3], const doubl
     J[2 + a][1] = -fk * nv0;
     J[2 + a][2] = dot3(row, gphi);
     J[2 + a][3] = dot3(row, gth);
-    J[2 + a][4] = dot3(f, D.dq) - fk * nrq;
+    J[2 + a][4] = (T)dot3(f, D.dq) - fk * nrq;
   }
   // row t
   const T c = ib / nd;
@@ -157,7 +159,7 @@ CKF_HD void arrival_jacobian(const Jac<T>& D, const double dep_u[3], const doubl
   J[4][1] = -c * nv0;
   J[4][2] = -c * nRgphi;
   J[4][3] = -c * nRgth;
-  J[4][4] = D.tq - c * nrq;
+  J[4][4] = (T)D.tq - c * nrq;
 }
 
 // C' = Jf C Jf^T on the packed upper triangle, Jf = full 6x6 built from the 5x5 block (see arrival_jacobian).
@@ -204,37 +206,35 @@ CKF_HD T predicted_chi2(double l0, double l1, T C00, T C01, T C11, T m0, T m1, T
   return (r0 * r0 * S11 - T(2) * r0 * r1 * C01 + r1 * r1 * S00) / det;
 }
 
-// V1 + V2 gate of one measurement.  T = float: a float32 pre-filter with a generous margin rejects the bulk
-// of the slice; the few survivors are re-evaluated in float64 so that the decision and the reported chi2 do
-// not carry float32 cancellation error.  T = double: one evaluation.
-template <typename T>
-CKF_HD bool gate_chi2(double l0, double l1, T C00, T C01, T C11, T m0, T m1, T v0, T v1, T chi2_max, T& chi2) {
-  const T c = predicted_chi2<T>(l0, l1, C00, C01, C11, m0, m1, v0, v1);
-  if (sizeof(T) == 8) {
-    chi2 = c;
-    return c < chi2_max;
+// V1 + V2 gate of one measurement against a float64 prediction (l0, l1, C00, C01, C11).  M = element type of the
+// measurement arrays.  M = float: a float32 pre-filter with a generous margin rejects the bulk of the slice; the few
+// survivors are re-evaluated in float64, so the decision and the reported chi2 are float64 functions of the inputs
+// (DESIGN.md §4).  M = double: one evaluation.
+template <typename M>
+CKF_HD bool gate_chi2(double l0, double l1, double C00, double C01, double C11, M m0, M m1, M v0, M v1, double chi2_max,
+                      double& chi2) {
+  if (sizeof(M) == 4) {
+    const float c = predicted_chi2<float>(l0, l1, (float)C00, (float)C01, (float)C11, (float)m0, (float)m1, (float)v0, (float)v1);
+    if (!(c < (float)chi2_max * 1.01f + 0.01f)) return false;
   }
-  if (!(c < chi2_max * T(1.01) + T(0.01))) return false;
-  const double cd = predicted_chi2<double>(l0, l1, (double)C00, (double)C01, (double)C11, (double)m0, (double)m1,
-                                           (double)v0, (double)v1);
-  chi2 = (T)cd;
-  return cd < (double)chi2_max;
+  const double cd = predicted_chi2<double>(l0, l1, C00, C01, C11, (double)m0, (double)m1, (double)v0, (double)v1);
+  chi2 = cd;
+  return cd < chi2_max;
 }
 
-// V3: gain-form update.  x float64 in/out, C packed upper triangle in/out (stored as T).  The arithmetic is
-// float64 in both modes: C' = C - K H C cancels two to three digits when a precise hit meets a loose
-// prediction, and the update is < 2 % of the work, so it is not worth a float32 error budget.
-template <typename T>
-CKF_HD void kalman_update(const double x[6], const T C[21], T m0, T m1, T v0, T v1, double xo[6], T Co[21]) {
+// V3: gain-form update, float64 in both modes (x, C packed upper triangle); M = element type of the measurement.
+// C' = C - K H C cancels two to three digits when a precise hit meets a loose prediction.
+template <typename M>
+CKF_HD void kalman_update(const double x[6], const double C[21], M m0, M m1, M v0, M v1, double xo[6], double Co[21]) {
   const double r0 = (double)m0 - x[0], r1 = (double)m1 - x[1];
-  const double S00 = (double)C[tri(0, 0)] + (double)v0, S01 = (double)C[tri(0, 1)], S11 = (double)C[tri(1, 1)] + (double)v1;
+  const double S00 = C[tri(0, 0)] + (double)v0, S01 = C[tri(0, 1)], S11 = C[tri(1, 1)] + (double)v1;
   const double det = S00 * S11 - S01 * S01;
   const double I00 = S11 / det, I01 = -S01 / det, I11 = S00 / det;
   double K0[6], K1[6];
 #pragma unroll
   for (int i = 0; i < 6; ++i) {
-    K0[i] = (double)C[tri(i, 0)] * I00 + (double)C[tri(i, 1)] * I01;
-    K1[i] = (double)C[tri(i, 0)] * I01 + (double)C[tri(i, 1)] * I11;
+    K0[i] = C[tri(i, 0)] * I00 + C[tri(i, 1)] * I01;
+    K1[i] = C[tri(i, 0)] * I01 + C[tri(i, 1)] * I11;
   }
 #pragma unroll
   for (int i = 0; i < 6; ++i) xo[i] = x[i] + (K0[i] * r0 + K1[i] * r1);
@@ -242,7 +242,7 @@ CKF_HD void kalman_update(const double x[6], const T C[21], T m0, T m1, T v0, T 
   for (int i = 0; i < 6; ++i)
 #pragma unroll
     for (int j = i; j < 6; ++j)
-      Co[tri(i, j)] = (T)((double)C[tri(i, j)] - (K0[i] * (double)C[tri(0, j)] + K1[i] * (double)C[tri(1, j)]));
+      Co[tri(i, j)] = C[tri(i, j)] - (K0[i] * C[tri(0, j)] + K1[i] * C[tri(1, j)]);
   while (xo[2] > PI_D) xo[2] -= 2.0 * PI_D;
   while (xo[2] <= -PI_D) xo[2] += 2.0 * PI_D;
 }
@@ -275,10 +275,9 @@ struct Move {
 };
 
 // Departure state of a tip with bound parameters x on module `from` (J1, V5): global position and direction,
-// the direction as T for the bound->free Jacobian, and the Highland variances to add to C[phi][phi],
+// the direction again for the bound->free Jacobian, and the Highland variances to add to C[phi][phi],
 // C[theta][theta] on leaving.  Returns STOP_NUMERIC for non-finite parameters or theta outside (0, pi).
-template <typename T>
-CKF_HD int departure_state(const GeoDev& g, const CfgDev& cfg, int from, const double x[6], Traj& y, T dep[5]) {
+CKF_HD int departure_state(const GeoDev& g, const CfgDev& cfg, int from, const double x[6], Traj& y, double dep[5]) {
   bool ok = true;
 #pragma unroll
   for (int i = 0; i < 6; ++i) ok = ok && isfinite(x[i]);
@@ -292,16 +291,16 @@ CKF_HD int departure_state(const GeoDev& g, const CfgDev& cfg, int from, const d
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
     y.r[i] = k.c[i] + x[0] * k.u[i] + x[1] * k.v[i];
-    dep[i] = (T)y.d[i];
+    dep[i] = y.d[i];
   }
   y.t = x[5];
   y.qop = x[4];
-  dep[3] = T(0);  // q_phi
-  dep[4] = T(0);  // q_theta
+  dep[3] = 0.0;  // q_phi
+  dep[4] = 0.0;  // q_theta
   if (k.xx0 > 0.0) {
     const double th2 = highland_theta0_sq(k.xx0, fabs(dot3(y.d, k.n)), y.qop, cfg.mass);
-    dep[4] = (T)th2;
-    dep[3] = (T)(th2 / (st * st));
+    dep[4] = th2;
+    dep[3] = th2 / (st * st);
   }
   return STOP_NONE;
 }
@@ -429,13 +428,13 @@ CKF_HD void move_step(Move<T>& m, const FieldDev& fld, const CfgDev& cfg, int& n
 // Arrival (J4, J5) of a move in PH_FIN with stop == NONE: predicted bound parameters and the 5x5 Jacobian
 // block.  Returns the final stop reason (NUMERIC if a predicted parameter is not finite).
 template <typename T>
-CKF_HD int move_arrive(const Move<T>& m, const T dep[5], const GeoDev& g, const FieldDev& fld, const CfgDev& cfg,
-                       double xp[6], T J[5][5]) {
+CKF_HD int move_arrive(const Move<T>& m, const double dep[5], const GeoDev& g, const FieldDev& fld, const CfgDev& cfg,
+                       double xp[6], double J[5][5]) {
   const ModuleRec& k = g.mod[m.tgt];
   const ModuleRec& m0 = g.mod[m.from];
   double B[3];
   field_at(fld, m.y.r, B);
-  arrival_jacobian(m.D, m0.u, m0.v, dep, k, m.y, B, cfg.mass, J);
+  arrival_jacobian<double, T>(m.D, m0.u, m0.v, dep, k, m.y, B, cfg.mass, J);
   const double rel[3] = {m.y.r[0] - k.c[0], m.y.r[1] - k.c[1], m.y.r[2] - k.c[2]};
   xp[0] = dot3(rel, k.u);
   xp[1] = dot3(rel, k.v);
@@ -452,10 +451,10 @@ CKF_HD int move_arrive(const Move<T>& m, const T dep[5], const GeoDev& g, const 
 // One tip at a time (host test harness): the transitions above in their natural order.
 template <typename T>
 CKF_HD int move_to_next_module(const GeoDev& g, const FieldDev& fld, const CfgDev& cfg, int from, const double x[6],
-                               int& target, double xp[6], T J[5][5], T& q_phi, T& q_theta, StepCtl& sc) {
+                               int& target, double xp[6], double J[5][5], double& q_phi, double& q_theta, StepCtl& sc) {
   Move<T> m;
-  T dep[5];
-  const int st0 = departure_state<T>(g, cfg, from, x, m.y, dep);
+  double dep[5];
+  const int st0 = departure_state(g, cfg, from, x, m.y, dep);
   if (st0 != STOP_NONE) return st0;
   move_begin(m, cfg, from);
   while (m.phase != PH_FIN) {

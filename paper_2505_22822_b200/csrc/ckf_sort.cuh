@@ -66,7 +66,13 @@ __global__ void __launch_bounds__(SORT_NT) ckf_sort_slices(const KParams<T> p) {
   for (int m0 = blockIdx.x * MPB; m0 < p.n_vmod; m0 += gridDim.x * MPB) {
     const int mw = m0 + warp;
     if (mw < p.n_vmod) {
-      const int begw = __ldg(p.moff + mw), nw = __ldg(p.moff + mw + 1) - begw;
+      int begw, endw;
+      slice_of<T>(p, mw, begw, endw);
+      const int nw = endw - begw;
+      if (lane == 0) {  // malformed CSR: flagged, and every reader clamps the slice the same way
+        const int rb = __ldg(p.moff + mw), re = __ldg(p.moff + mw + 1);
+        if (rb != begw || re != endw) atomicOr(p.g + G_BAD_INPUT, 1);
+      }
       if (nw <= 32) sort_slice_warp<T>(p, mw, begw, nw, lane);
     }
   }
@@ -74,7 +80,9 @@ __global__ void __launch_bounds__(SORT_NT) ckf_sort_slices(const KParams<T> p) {
   // modules have consecutive ids)
   {
     for (int m = blockIdx.x; m < p.n_vmod; m += gridDim.x) {
-      const int beg = __ldg(p.moff + m), end = __ldg(p.moff + m + 1), n = end - beg;
+      int beg, end;
+      slice_of<T>(p, m, beg, end);
+      const int n = end - beg;
       if (n <= 32) continue;
       __syncthreads();
       if (tid == 0) s_bad = 0;

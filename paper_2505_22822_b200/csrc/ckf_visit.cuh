@@ -11,7 +11,7 @@ namespace ckf {
 template <typename T>
 struct VSmem {
   double* px;       // [6][32] predicted bound parameters
-  T* pC;            // [21][32] predicted packed covariance
+  double* pC;       // [21][32] predicted packed covariance
   T* selchi2;       // [K][32]
   int32_t* selidx;  // [K][32]
   T* candchi2;      // [CAND][32]
@@ -19,14 +19,14 @@ struct VSmem {
   int32_t *target, *lo, *cnt;  // [32] each
   int32_t* off;     // [33]
   __host__ __device__ static size_t bytes(int K) {
-    size_t b = sizeof(double) * 6 * 32 + sizeof(T) * 21 * 32 + (sizeof(T) + 4) * (size_t)K * 32 +
+    size_t b = sizeof(double) * 6 * 32 + sizeof(double) * 21 * 32 + (sizeof(T) + 4) * (size_t)K * 32 +
                (sizeof(T) + 4) * (size_t)CAND * 32 + 4 * 3 * 32 + 4 * 33;
     return (b + 15) & ~(size_t)15;
   }
   __device__ void carve(unsigned char* raw, int K) {
     unsigned char* p = raw;
     px = (double*)p; p += sizeof(double) * 6 * 32;
-    pC = (T*)p; p += sizeof(T) * 21 * 32;
+    pC = (double*)p; p += sizeof(double) * 21 * 32;
     selchi2 = (T*)p; p += sizeof(T) * (size_t)K * 32;
     candchi2 = (T*)p; p += sizeof(T) * (size_t)CAND * 32;
     selidx = (int32_t*)p; p += 4 * (size_t)K * 32;
@@ -46,19 +46,20 @@ struct VSmem {
 template <typename T>
 __device__ __forceinline__ int gate_chunk(const KParams<T>& p, const VSmem<T>& s, int lane, bool visit, int K,
                                           unsigned long long& n_exec) {
-  const T chi2_max = (T)p.cfg.chi2_max;
+  const double chi2_max = p.cfg.chi2_max;
   int lo = 0, len = 0;
   if (visit) {
     const int m = s.target[lane];
-    const int beg = __ldg(p.moff + m), end = __ldg(p.moff + m + 1);
+    int beg, end;
+    slice_of<T>(p, m, beg, end);
     int hi = end;
     lo = beg;
     if (end > beg) {
       const T v0max = p.s_v0max[m];
-      const T C00 = s.pC[tri(0, 0) * 32 + lane], C01 = s.pC[tri(0, 1) * 32 + lane], C11 = s.pC[tri(1, 1) * 32 + lane];
-      if (v0max >= T(0) && C00 > T(0) && C11 > T(0) && C00 * C11 - C01 * C01 > T(0)) {
+      const double C00 = s.pC[tri(0, 0) * 32 + lane], C01 = s.pC[tri(0, 1) * 32 + lane], C11 = s.pC[tri(1, 1) * 32 + lane];
+      if (v0max >= T(0) && C00 > 0.0 && C11 > 0.0 && C00 * C11 - C01 * C01 > 0.0) {
         // chi2 >= r0^2 / S00 and S00 <= C00 + v0max: nothing outside |loc0 - l0| <= w can pass
-        const double w = sqrt(p.cfg.chi2_max * ((double)C00 + (double)v0max)) * (1.0 + 1e-6) + 1e-9;
+        const double w = sqrt(p.cfg.chi2_max * (C00 + (double)v0max)) * (1.0 + 1e-6) + 1e-9;
         if (isfinite(w)) {
           const double l0 = s.px[0 * 32 + lane];
           const double a = l0 - w, b = l0 + w;
@@ -96,13 +97,13 @@ __device__ __forceinline__ int gate_chunk(const KParams<T>& p, const VSmem<T>& s
       const auto lc = p.s_loc[k];
       const auto vr = p.s_var[k];
       const int oi = p.s_idx[k];  // loaded with the rest (coalesced), not after the test by the few lanes that pass
-      T c2 = T(0);
+      double c2 = 0.0;
       const bool pass = gate_chi2<T>(s.px[0 * 32 + t], s.px[1 * 32 + t], s.pC[tri(0, 0) * 32 + t],
                                      s.pC[tri(0, 1) * 32 + t], s.pC[tri(1, 1) * 32 + t], lc.x, lc.y, vr.x, vr.y,
                                      chi2_max, c2);
       if (pass) {
         const int pos = atomicAdd(&s.cnt[t], 1);
-        if (pos < CAND) { s.candchi2[pos * 32 + t] = c2; s.candidx[pos * 32 + t] = oi; }
+        if (pos < CAND) { s.candchi2[pos * 32 + t] = (T)c2; s.candidx[pos * 32 + t] = oi; }
       }
     }
   }
@@ -124,7 +125,7 @@ __device__ __forceinline__ int gate_chunk(const KParams<T>& p, const VSmem<T>& s
     } else {
       // rare: more than CAND passers.  K rounds of "smallest key above the last one" over the window.
       const double l0 = s.px[0 * 32 + lane], l1 = s.px[1 * 32 + lane];
-      const T C00 = s.pC[tri(0, 0) * 32 + lane], C01 = s.pC[tri(0, 1) * 32 + lane], C11 = s.pC[tri(1, 1) * 32 + lane];
+      const double C00 = s.pC[tri(0, 0) * 32 + lane], C01 = s.pC[tri(0, 1) * 32 + lane], C11 = s.pC[tri(1, 1) * 32 + lane];
       T last_c = T(-1);
       int last_i = -1;
       nsel = count < K ? count : K;
@@ -134,8 +135,9 @@ __device__ __forceinline__ int gate_chunk(const KParams<T>& p, const VSmem<T>& s
         for (int k = lo; k < lo + len; ++k) {
           const auto lc = p.s_loc[k];
           const auto vr = p.s_var[k];
-          T c2 = T(0);
-          const bool ok = gate_chi2<T>(l0, l1, C00, C01, C11, lc.x, lc.y, vr.x, vr.y, chi2_max, c2);
+          double c2d = 0.0;
+          const bool ok = gate_chi2<T>(l0, l1, C00, C01, C11, lc.x, lc.y, vr.x, vr.y, chi2_max, c2d);
+          const T c2 = (T)c2d;
           const int id = p.s_idx[k];
           if (ok && key_less<T>(last_c, last_i, c2, id) && (bi == 0x7fffffff || key_less<T>(c2, id, bc, bi))) {
             bc = c2; bi = id;
@@ -187,11 +189,13 @@ __global__ void __launch_bounds__(VISIT_NT, MINB) ckf_visit(const KParams<T> p, 
         for (int i = 0; i < 6; ++i)
 #pragma unroll
           for (int j = i; j < 6; ++j) {
-            const T c = p.seed_C[(size_t)seed * 36 + i * 6 + j];
+            const double c = (double)p.seed_C[(size_t)seed * 36 + i * 6 + j];
             s.pC[tri(i, j) * 32 + lane] = c;
             p.pd_C[tri(i, j) * TC + t] = c;
           }
-        target = p.seed_module[seed] - p.sd_eoff[seed];
+        const int eoff = p.sd_eoff[seed];
+        if (eoff < 0) ok = false;     // seed module out of range (flagged by ckf_init_event): never used as an index
+        target = ok ? p.seed_module[seed] - eoff : -1;
         p.mv_tgt[t] = target;
         if (!ok) stop = STOP_NUMERIC;
       } else {
@@ -204,20 +208,20 @@ __global__ void __launch_bounds__(VISIT_NT, MINB) ckf_visit(const KParams<T> p, 
           load_jac(p.mv_D, (size_t)t, m.D);
           m.from = p.mv_from[t];
           m.tgt = p.mv_tgt[t];
-          T dep[5];
+          double dep[5];
 #pragma unroll
           for (int i = 0; i < 5; ++i) dep[i] = p.mv_dep[i * TC + t];
           double xp[6];
-          T J[5][5];
+          double J[5][5];
           stop = move_arrive<T>(m, dep, p.geo, p.fld, p.cfg, xp, J);
           if (stop == STOP_NONE) {
             target = m.tgt;
-            T C[21], Co[21];
+            double C[21], Co[21];
 #pragma unroll
             for (int i = 0; i < 21; ++i) C[i] = p.lk_C[(size_t)i * p.max_links + link];
             C[tri(2, 2)] += dep[3];
             C[tri(3, 3)] += dep[4];
-            transport_cov<T>(J, C, Co);
+            transport_cov<double>(J, C, Co);
             bool fin = true;
 #pragma unroll
             for (int i = 0; i < 21; ++i) { s.pC[i * 32 + lane] = Co[i]; p.pd_C[i * TC + t] = Co[i]; fin = fin && isfinite(Co[i]); }
@@ -233,7 +237,9 @@ __global__ void __launch_bounds__(VISIT_NT, MINB) ckf_visit(const KParams<T> p, 
     __syncwarp();
     const bool visit = act && stop == STOP_NONE;
     if (visit) {
-      my_gate += (unsigned long long)(__ldg(p.moff + vtarget + 1) - __ldg(p.moff + vtarget));
+      int sb, se;
+      slice_of<T>(p, vtarget, sb, se);
+      my_gate += (unsigned long long)(se - sb);
       my_visits += 1ull;
     }
     const int nsel = gate_chunk<T>(p, s, lane, visit, K, w_exec);

@@ -23,7 +23,7 @@ struct Ctx {
 
 template <typename T>
 int move_t(Ctx* c, int from, const double* x, const double* C36, int* target, double* xp, double* Cp36, int* trials) {
-  T J[5][5], qphi, qth;
+  double J[5][5], qphi, qth;
   StepCtl sc;
   sc.n_trials = 0; sc.n_accepted = 0;
   int tg = -1;
@@ -31,12 +31,12 @@ int move_t(Ctx* c, int from, const double* x, const double* C36, int* target, do
   *target = tg;
   if (trials) *trials = sc.n_trials;
   if (st != STOP_NONE) return st;
-  T C[21], Co[21];
+  double C[21], Co[21];
   for (int i = 0; i < 6; ++i)
-    for (int j = i; j < 6; ++j) C[tri(i, j)] = (T)C36[6 * i + j];
+    for (int j = i; j < 6; ++j) C[tri(i, j)] = C36[6 * i + j];
   C[tri(2, 2)] += qphi;
   C[tri(3, 3)] += qth;
-  transport_cov<T>(J, C, Co);
+  transport_cov<double>(J, C, Co);
   for (int i = 0; i < 6; ++i)
     for (int j = 0; j < 6; ++j) Cp36[6 * i + j] = (double)Co[tri(i, j)];
   return st;
@@ -45,12 +45,12 @@ int move_t(Ctx* c, int from, const double* x, const double* C36, int* target, do
 template <typename T>
 void update_t(const double* x, const double* C36, const double* loc, const double* var, double* xo, double* Co36,
               double* chi2) {
-  T C[21], Co[21];
+  double C[21], Co[21];
   for (int i = 0; i < 6; ++i)
-    for (int j = i; j < 6; ++j) C[tri(i, j)] = (T)C36[6 * i + j];
-  T c2 = T(0);
-  gate_chi2<T>(x[0], x[1], C[tri(0, 0)], C[tri(0, 1)], C[tri(1, 1)], (T)loc[0], (T)loc[1], (T)var[0], (T)var[1], T(1e30), c2);
-  *chi2 = (double)c2;
+    for (int j = i; j < 6; ++j) C[tri(i, j)] = C36[6 * i + j];
+  double c2 = 0.0;
+  gate_chi2<T>(x[0], x[1], C[tri(0, 0)], C[tri(0, 1)], C[tri(1, 1)], (T)loc[0], (T)loc[1], (T)var[0], (T)var[1], 1e30, c2);
+  *chi2 = c2;
   kalman_update<T>(x, C, (T)loc[0], (T)loc[1], (T)var[0], (T)var[1], xo, Co);
   for (int i = 0; i < 6; ++i)
     for (int j = 0; j < 6; ++j) Co36[6 * i + j] = (double)Co[tri(i, j)];

@@ -66,12 +66,9 @@ def test_fp32_parity(config):
     ora = _run_oracle(det, fld, cfg, ev)
     ckf, dev, out, gpu, cnt = _run_gpu(det, fld, cfg, ev)
     assert gpu.status == 0
-    r = parity.compare_fp32(gpu, ora, ev.n_seeds)
+    # north_star: >= 99.9 % identical lists, every mismatch traced to a gate-edge chi2 or a ranking tie, 1e-4, 1e-3
+    r = parity.assert_fp32_parity(gpu, ora, ev.n_seeds, cfg.ckf.chi2_max, "configs[%d]" % config)
     print("config", config, {k: v for k, v in r.items() if k != "bad_seeds"}, "n_bad", len(r["bad_seeds"]))
-    assert r["frac_identical"] >= 0.999          # north_star
-    assert r["max_param_rel"] < 1e-4
-    assert r["max_chi2_sum_abs"] < 1e-3
-    assert r["max_entry_chi2_abs"] < 1e-3
 
 
 def test_edge_cases():
@@ -408,10 +405,11 @@ def test_batch_of_events_fp32():
     ckf.close()
 
 
-def test_fit_fp32_covariance_not_positive_definite_is_flagged():
-    """configs[3], event index 1: three candidates of one fake seed (3 measurements, 4 holes) have a float32-stored
-    predicted covariance that is not positive definite any more; ckf_fit must flag them NUMERIC with zeros (never
-    report numbers), the float64 oracle fits them; everything else agrees as usual."""
+def test_fit_fp32_ill_conditioned_covariances_are_fitted():
+    """configs[3], event index 1: three candidates of one fake seed (3 measurements, 4 holes) have predicted covariances
+    so ill-conditioned that their float32-STORED copy was no longer positive definite (round 1 flagged them NUMERIC).
+    Since the covariance algebra and storage are float64 in both modes every candidate the float64
+    oracle fits is fitted here too."""
     import torch
     import oracle
     det, fld, cfg = synth.config_bundle(3)
@@ -424,11 +422,8 @@ def test_fit_fp32_covariance_not_positive_definite_is_flagged():
     o = oracle.kf_fit(oracle.Setup(det, fld, cfg.ckf), ev, gpu.track_offsets, gpu.meas_idx, gpu.seed_id, n_threads=16)
     r = parity.compare_fits(g, o, gpu.track_offsets)
     print("fit config 3 event 1", r)
-    assert 0 < r["n_not_pd_gpu_only"] <= 1e-4 * gpu.n_tracks
-    bad = np.flatnonzero((g["status"] == 5) & (o.status == 0))
-    for t in bad:
-        assert not g["entry_params"][gpu.track_offsets[t]:gpu.track_offsets[t + 1]].any() and not g["first_cov"][t].any()
-    assert r["max_smoothed_rel"] < 1e-4 and r["max_last_rel"] < 1e-4
+    assert r["n_not_pd_gpu_only"] == 0 and np.array_equal(g["status"], o.status)
+    assert r["max_smoothed_rel"] < 1e-5 and r["max_last_rel"] < 1e-5
     # the two-filter smoother factors the FILTERED covariance instead of the predicted one
     f2 = ckf.alloc_fits()
     ckf.fit(dev, out, f2, smoother=1)
@@ -526,3 +521,125 @@ def test_batch_with_an_empty_event_and_fit_of_nothing():
     assert int(out0["n_tracks"][0]) == 0 and int(out0["status"][0]) == 0
     assert bool((fits["status"] == 77).all()) and int(fits["work"].sum()) == 0
     ckf.close()
+
+
+def test_malformed_input_is_flagged_not_read_out_of_bounds():
+    """a seed module id out of range and a broken measurement CSR end in CKF_STATUS_BAD_INPUT (8); the
+    other seeds are unaffected."""
+    import torch
+    det, fld, cfg = synth.config_bundle(1)
+    ev = synth.make_event(1, det=det, n_particles=200)
+    ora = _run_oracle(det, fld, cfg, ev)
+    ckf, dev, out, gpu, _ = _run_gpu(det, fld, cfg, ev)
+    assert gpu.status == 0
+    bad = dict(dev)
+    sm = dev["seed_module"].clone()
+    sm[3] = det.n_modules + 12345          # beyond the detector (and beyond n_events * n_modules)
+    sm[7] = -5
+    bad["seed_module"] = sm
+    ckf.find(bad, out)
+    torch.cuda.synchronize()
+    res = ckf.download(out)
+    assert res.status & 8
+    assert 3 not in res.seed_id and 7 not in res.seed_id
+    keep = ~np.isin(ora.seed_id, [3, 7])
+    assert np.array_equal(res.seed_id, ora.seed_id[keep])
+    assert res.n_tracks == int(keep.sum())
+    # a CSR that is not monotonic and points beyond n: flagged, slices clamped, no fault; the next call is clean again
+    off = dev["module_offsets"].clone()
+    m = int(ev.meas_module[ev.n_measurements // 2])
+    off[m] = ev.n_measurements + 1000
+    off[m + 3] = -7
+    broken = dict(dev)
+    broken["module_offsets"] = off
+    ckf.find(broken, out)
+    torch.cuda.synchronize()
+    assert int(out["status"][0]) & 8
+    ckf.find(dev, out)
+    torch.cuda.synchronize()
+    again = ckf.download(out)
+    assert again.status == 0
+    parity.assert_bit_exact_lists(again, ora)
+    ckf.close()
+
+
+def _streamed(ckf, hevs, n_threads, streams_per_thread=1):
+    """configs[4] shape: host threads, each with its own CUDA stream(s) and pinned output buffers, call ckf_find_host
+    concurrently; returns the downloaded result of every event."""
+    import threading
+    import torch
+    results = [None] * len(hevs)
+    errors = []
+
+    def worker(k):
+        try:
+            torch.cuda.set_device(0)
+            sts = [torch.cuda.Stream() for _ in range(streams_per_thread)]
+            hout = ckf.pinned_tracks()
+            for j, i in enumerate(range(k, len(hevs), n_threads)):
+                ckf.find_host(hevs[i], hout, sts[j % streams_per_thread])
+                results[i] = ckf.download(hout)
+        except Exception as e:  # noqa
+            errors.append(e)
+
+    ths = [threading.Thread(target=worker, args=(k,)) for k in range(n_threads)]
+    for t in ths:
+        t.start()
+    for t in ths:
+        t.join()
+    assert not errors, errors
+    return results
+
+
+def _make_event4(i):
+    return synth.make_event(4, event_index=i)
+
+
+def test_config4_streamed_parity():
+    """BASELINE.json configs[4] as written: 64 DISTINCT events (event_index 0..63), 4 host threads x 4 CUDA streams,
+    pinned host buffers through ckf_find_host (H2D + D2H inside), every event compared with the oracle."""
+    import os
+    from concurrent.futures import ProcessPoolExecutor
+    import oracle
+    from paper_2505_22822_b200 import CKF
+    det, fld, cfg = synth.config_bundle(4)
+    n_ev = 64
+    with ProcessPoolExecutor(max_workers=min(16, os.cpu_count() or 1)) as ex:
+        evs = list(ex.map(_make_event4, range(n_ev)))
+    assert len({e.n_measurements for e in evs}) > 32          # distinct events, not a rotation
+    ms, mm = max(e.n_seeds for e in evs), max(e.n_measurements for e in evs)
+    ckf = CKF(det, fld, cfg.ckf, cfg.precision, max_seeds=ms, max_measurements=mm, max_tracks=8 * ms,
+              max_track_entries=80 * ms, n_streams=4, max_fit_tracks=0)
+    hevs = [ckf.pinned_event(e) for e in evs]
+    res = _streamed(ckf, hevs, n_threads=4)
+    ckf.close()
+    st = oracle.Setup(det, fld, cfg.ckf)
+    worst = dict(frac=1.0, rel=0.0, chi2=0.0, echi2=0.0, traced=0)
+    for i, ev in enumerate(evs):
+        ora = oracle.find_event(st, ev, n_threads=os.cpu_count() or 8)
+        assert res[i].status == 0
+        r = parity.assert_fp32_parity(res[i], ora, ev.n_seeds, cfg.ckf.chi2_max, "configs[4] event %d" % i)
+        worst["frac"] = min(worst["frac"], r["frac_identical"])
+        worst["rel"] = max(worst["rel"], r["max_param_rel"])
+        worst["chi2"] = max(worst["chi2"], r["max_chi2_sum_abs"])
+        worst["echi2"] = max(worst["echi2"], r["max_entry_chi2_abs"])
+        worst["traced"] += r["n_mismatch_traced"]
+    print("configs[4], 64 events on 4 threads x 4 streams, worst over events:", worst)
+
+
+def test_more_streams_than_workspaces_is_ordered():
+    """6 host threads x 2 streams each on a handle with n_streams = 2: workspaces are recycled while other threads are
+    still enqueuing (acquire_ws); every result must still be the oracle's."""
+    import oracle
+    from paper_2505_22822_b200 import CKF
+    det, fld, cfg = synth.config_bundle(2)
+    evs = [synth.make_event(2, event_index=i, det=det, n_particles=1500 + 100 * i) for i in range(6)]
+    ms, mm = max(e.n_seeds for e in evs), max(e.n_measurements for e in evs)
+    ckf = CKF(det, fld, cfg.ckf, cfg.precision, max_seeds=ms, max_measurements=mm, n_streams=2, max_fit_tracks=0)
+    hevs = [ckf.pinned_event(evs[i % 6]) for i in range(48)]
+    res = _streamed(ckf, hevs, n_threads=6, streams_per_thread=2)
+    ckf.close()
+    st = oracle.Setup(det, fld, cfg.ckf)
+    oras = [oracle.find_event(st, e, n_threads=8) for e in evs]
+    for i, r in enumerate(res):
+        parity.assert_fp32_parity(r, oras[i % 6], evs[i % 6].n_seeds, cfg.ckf.chi2_max, "call %d" % i)
