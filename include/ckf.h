@@ -266,6 +266,14 @@ int ckf_get_timing(ckf_handle* handle, void* cuda_stream, ckf_timing* out);
 int ckf_get_launch_info(const ckf_handle* handle, int32_t* blocks, int32_t* threads, int32_t* smem_bytes,
                         int32_t* regs);
 
+/* Measurement aid: the plain-ALU FMA peak of the current device, the roofline denominator of this path (north_star:
+ * "% of FP pipe peak"; the method does not use the tensor cores).  FMA chains in registers on every SM, launched back
+ * to back for at least `seconds` on the default stream, synchronous.  mix 0: float32 chains only; 1: float64 only;
+ * 2: 8 float32 + 4 float64 chains per thread at once.  *tflops_f32 / *tflops_f64: flop rates over the whole run (an
+ * FMA counts 2); *best_f32 / *best_f64 (may be NULL): rates of the fastest single launch.  Needs no handle. */
+int ckf_measure_alu_peak(int mix, double seconds, double* tflops_f32, double* tflops_f64, double* best_f32,
+                         double* best_f64);
+
 int ckf_destroy(ckf_handle* handle);
 
 /* Text of the calling thread's last failed call (handle may be NULL; it is not used). */

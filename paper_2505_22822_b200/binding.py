@@ -21,7 +21,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libckf.so")
 
 EXPORTS = ("ckf_create", "ckf_find", "ckf_find_host", "ckf_fit", "ckf_get_counters", "ckf_get_launch_info", "ckf_destroy",
-           "ckf_set_timing", "ckf_get_timing",
+           "ckf_set_timing", "ckf_get_timing", "ckf_measure_alu_peak",
            "ckf_last_error", "ckf_abi_version")
 
 
@@ -109,6 +109,8 @@ def load_library():
         L.ckf_last_error.restype = C.c_char_p
         L.ckf_last_error.argtypes = [_vp]
         L.ckf_abi_version.restype = C.c_int
+        L.ckf_measure_alu_peak.restype = C.c_int
+        L.ckf_measure_alu_peak.argtypes = [C.c_int, C.c_double, _dp, _dp, _dp, _dp]
         _lib = L
     return _lib
 
@@ -165,6 +167,15 @@ def make_config(ckf, precision: int, max_seeds: int, max_measurements: int, max_
     c.max_events_per_find = int(max_events_per_find)
     c.max_fit_tracks = int(max_fit_tracks)
     return c
+
+
+def measure_alu_peak(mix: int, seconds: float = 1.0) -> dict:
+    """ckf_measure_alu_peak: FMA-chain throughput of the current device (mix 0 float32, 1 float64, 2 both)."""
+    v = [C.c_double(0.0) for _ in range(4)]
+    rc = load_library().ckf_measure_alu_peak(int(mix), float(seconds), *[C.byref(x) for x in v])
+    if rc != 0:
+        raise RuntimeError("ckf_measure_alu_peak failed (%d): %s" % (rc, load_library().ckf_last_error(None).decode()))
+    return dict(tflops_f32=v[0].value, tflops_f64=v[1].value, best_f32=v[2].value, best_f64=v[3].value)
 
 
 @dataclass

@@ -21,6 +21,7 @@
 #include "ckf_host_geom.h"
 #include "ckf_branch.cuh"
 #include "ckf_fit.cuh"
+#include "ckf_peak.cuh"
 #include "ckf_sort.cuh"
 #include "ckf_step.cuh"
 #include "ckf_visit.cuh"
@@ -685,6 +686,58 @@ int ckf_get_launch_info(const ckf_handle* h, int32_t* blocks, int32_t* threads, 
   if (threads) *threads = STEP_NT;
   if (smem) *smem = (int32_t)((STEP_NT / 32) * PickSmem::bytes());
   if (regs) *regs = h->step_regs;
+  return CKF_OK;
+}
+
+// Measured plain-ALU peak (see ckf_peak.cuh).  mix: 0 = float32 FMA chains only, 1 = float64 only, 2 = both at once
+// (8 float + 4 double chains per thread: the two pipes fed together).  Launches back to back for at least `seconds`
+// on the default stream; *tflops_f32 / *tflops_f64 receive the flop rates over the whole run (an FMA = 2 flop),
+// *best_* the rates of the fastest single launch.
+int ckf_measure_alu_peak(int mix, double seconds, double* tflops_f32, double* tflops_f64, double* best_f32, double* best_f64) {
+  ckf_handle* h = nullptr;
+  if (mix < 0 || mix > 2 || !(seconds > 0.0) || !tflops_f32 || !tflops_f64) return fail(h, CKF_E_ARG, "bad argument");
+  int dev = 0, sms = 0;
+  CK(cudaGetDevice(&dev));
+  CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+  const int blocks = sms * 8, threads = 256, iters = 4096;
+  double* out = nullptr;
+  CK(cudaMalloc(&out, (size_t)blocks * threads * sizeof(double)));
+  const int nf = mix == 0 ? 8 : (mix == 2 ? 8 : 0), nd = mix == 1 ? 8 : (mix == 2 ? 4 : 0);
+  auto launch = [&]() {
+    if (mix == 0) ckf_fma_chain<8, 0><<<blocks, threads>>>(out, iters, 0.999f, 1e-3f, 0.999, 1e-3);
+    else if (mix == 1) ckf_fma_chain<0, 8><<<blocks, threads>>>(out, iters, 0.999f, 1e-3f, 0.999, 1e-3);
+    else ckf_fma_chain<8, 4><<<blocks, threads>>>(out, iters, 0.999f, 1e-3f, 0.999, 1e-3);
+  };
+  cudaEvent_t e0, e1, a, b;
+  cudaEventCreate(&e0); cudaEventCreate(&e1); cudaEventCreate(&a); cudaEventCreate(&b);
+  for (int i = 0; i < 3; ++i) launch();
+  cudaDeviceSynchronize();
+  const double per_launch = (double)blocks * threads * (double)iters * 8.0 * 2.0;   // flop per chain kind per chain
+  double total_ms = 0.0, best_ms = 1e30;
+  long n = 0;
+  cudaEventRecord(e0);
+  while (total_ms < seconds * 1e3) {
+    cudaEventRecord(a);
+    for (int i = 0; i < 8; ++i) launch();
+    cudaEventRecord(b);
+    cudaEventSynchronize(b);
+    float ms = 0.f;
+    cudaEventElapsedTime(&ms, a, b);
+    best_ms = ms / 8.0 < best_ms ? ms / 8.0 : best_ms;
+    n += 8;
+    cudaEventRecord(e1);
+    cudaEventSynchronize(e1);
+    cudaEventElapsedTime(&ms, e0, e1);
+    total_ms = ms;
+  }
+  cudaError_t e = cudaGetLastError();
+  cudaEventDestroy(e0); cudaEventDestroy(e1); cudaEventDestroy(a); cudaEventDestroy(b);
+  cudaFree(out);
+  if (e != cudaSuccess) return fail(h, CKF_E_CUDA, "fma chain failed: %s", cudaGetErrorString(e));
+  *tflops_f32 = nf * per_launch * (double)n / (total_ms * 1e-3) / 1e12;
+  *tflops_f64 = nd * per_launch * (double)n / (total_ms * 1e-3) / 1e12;
+  if (best_f32) *best_f32 = nf * per_launch / (best_ms * 1e-3) / 1e12;
+  if (best_f64) *best_f64 = nd * per_launch / (best_ms * 1e-3) / 1e12;
   return CKF_OK;
 }
 

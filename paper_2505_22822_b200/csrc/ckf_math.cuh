@@ -181,8 +181,10 @@ struct Trial {
   double eps;
 };
 
+// B1 = field at y.r, read by the caller (move_target): it is the same for every retry of a rejected trial, and after an
+// accepted step its loads are issued before the Jacobian columns are computed, which hides their latency.
 template <typename T>
-CKF_HD void rk_trial(const FieldDev& fld, const Traj& y, double lam, double h, Trial<T>& t) {
+CKF_HD void rk_trial(const FieldDev& fld, const Traj& y, const double B1[3], double lam, double h, Trial<T>& t) {
   // The stage loop is unrolled: three inlined copies of field_at.  In the monolithic level loop of r01b one rolled
   // copy was needed to stay inside the SM's instruction cache; in the per-phase ckf_step the three copies fit
   // (2,640 SASS instructions) and save the register moves of the rolled form: ckf_step 2.07 -> 1.89 ms per event.
@@ -193,7 +195,7 @@ CKF_HD void rk_trial(const FieldDev& fld, const Traj& y, double lam, double h, T
     double p[3], B[3], w[3];
     if (st == 0) {
 #pragma unroll
-      for (int i = 0; i < 3; ++i) p[i] = y.r[i];
+      for (int i = 0; i < 3; ++i) B[i] = B1[i];
     } else if (st == 1) {
 #pragma unroll
       for (int i = 0; i < 3; ++i) p[i] = y.r[i] + h2 * y.d[i] + h8 * (lam * cr1[i]);
@@ -201,7 +203,7 @@ CKF_HD void rk_trial(const FieldDev& fld, const Traj& y, double lam, double h, T
 #pragma unroll
       for (int i = 0; i < 3; ++i) p[i] = y.r[i] + h * y.d[i] + hh2 * (lam * cr3[i]);
     }
-    field_at(fld, p, B);
+    if (st != 0) field_at(fld, p, B);
     if (st == 0) {
 #pragma unroll
       for (int i = 0; i < 3; ++i) t.B1[i] = (T)B[i];
@@ -267,9 +269,10 @@ CKF_HD void jac_column_q(T lam, T h, T qf, const T B1[3], const T B2[3], const T
   }
 }
 
-// Accept a trial: D <- D_step D column by column (J2, J3), then the state (P2).
+// Accept a trial, in two halves so that the caller can put the next field read between them: the state (P2), and
+// D <- D_step D column by column (J2, J3).  The Jacobian half does not read the state's position or direction.
 template <typename T>
-CKF_HD void rk_accept(Traj& y, Jac<T>& J, double h, const Trial<T>& t, double ib, double dib) {
+CKF_HD void rk_accept_jac(const Traj& y, Jac<T>& J, double h, const Trial<T>& t, double dib) {
   {
     const T lamT = (T)(KAPPA * y.qop), hT = (T)h;
 #pragma unroll
@@ -283,6 +286,9 @@ CKF_HD void rk_accept(Traj& y, Jac<T>& J, double h, const Trial<T>& t, double ib
     jac_column_q<T>(lamT, hT, T(1), t.B1, t.B2, t.B4, t.q1, t.q2, t.q3, t.q4, J.rq, J.dq);
     J.tq += (T)(h * dib);
   }
+}
+template <typename T>
+CKF_HD void rk_accept_state(Traj& y, double h, const Trial<T>& t, double ib) {
   const double h6 = h * (1.0 / 6.0), hh6 = h * h * (1.0 / 6.0);  // one rounding away from h / 6: far inside 1e-9
   double dn[3], n2 = 0.0;
 #pragma unroll

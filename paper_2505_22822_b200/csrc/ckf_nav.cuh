@@ -270,8 +270,9 @@ struct Move {
   double R;             // target cylinder radius (PH_CYL)
   double h, h_ctrl;
   double ib, dib;       // 1/beta and d(1/beta)/d(q/p): constant along the move (no energy loss)
+  double B1[3];         // field at y.r, valid while `targeted` (read once per position, see move_target)
   int phase, stop, from, tgt, lp, n_steps;
-  bool retry;
+  bool targeted;        // the next trial's length m.h and B1 are set (P4 done for the current position)
 };
 
 // Departure state of a tip with bound parameters x on module `from` (J1, V5): global position and direction,
@@ -308,7 +309,7 @@ CKF_HD int departure_state(const GeoDev& g, const CfgDev& cfg, int from, const d
 // Start of a move whose m.y holds the departure state: identity transport, fresh step control (P4, J3).
 template <typename T>
 CKF_HD void move_begin(Move<T>& m, const CfgDev& cfg, int from) {
-  m.from = from; m.tgt = -1; m.lp = 0; m.n_steps = 0; m.retry = false; m.stop = STOP_NONE;
+  m.from = from; m.tgt = -1; m.lp = 0; m.n_steps = 0; m.targeted = false; m.stop = STOP_NONE;
   m.h = 0.0; m.h_ctrl = cfg.h_max; m.R = 0.0;
   jac_identity(m.D);
   m.ib = inv_beta(m.y.qop, cfg.mass);
@@ -375,37 +376,58 @@ CKF_HD void move_pick_apply(Move<T>& m, const GeoDev& g, int tgt, bool exit_now 
   m.phase = PH_CYL;
 }
 
-// One step of a move in PH_CYL / PH_PLANE: targeting + landing (P4, P5), else one RKN4 trial (P2, P3).
+// P4: signed straight-line distance from the move's position to its target (plane or cylinder) along d.
+// Returns STOP_NONE and s, or the stop reason (P6).
+template <typename T>
+CKF_HD int target_distance(const Move<T>& m, double& s) {
+  if (m.phase == PH_PLANE) {
+    const double dn = dot3(m.y.d, m.tn);
+    if (!(fabs(dn) > 1e-12)) return STOP_NUMERIC;
+    const double rel[3] = {m.tc[0] - m.y.r[0], m.tc[1] - m.y.r[1], m.tc[2] - m.y.r[2]};
+    s = dot3(rel, m.tn) / dn;
+  } else {
+    const double a = m.y.d[0] * m.y.d[0] + m.y.d[1] * m.y.d[1];
+    const double b = m.y.r[0] * m.y.d[0] + m.y.r[1] * m.y.d[1];
+    const double cc = m.y.r[0] * m.y.r[0] + m.y.r[1] * m.y.r[1] - m.R * m.R;
+    const double disc = b * b - a * cc;
+    if (!(b > 0.0) || !(disc >= 0.0)) return STOP_NOT_OUTGOING;
+    s = -cc / (b + sqrt(disc));
+  }
+  return isfinite(s) ? STOP_NONE : STOP_NUMERIC;
+}
+
+// The next trial from the current position: its length (P4) and the field there -- stage 1 of that trial and of every
+// retry of it (a rejected trial restarts from the same point).
+template <typename T>
+CKF_HD void set_trial(Move<T>& m, const FieldDev& fld, const CfgDev& cfg, double s) {
+  const double hlim = fmin(m.h_ctrl, cfg.h_max);
+  m.h = (fabs(s) <= hlim) ? s : (s > 0.0 ? hlim : -hlim);
+  field_at(fld, m.y.r, m.B1);
+  m.targeted = true;
+}
+
+// P5 / P6 once no further trial follows: stop, or close onto the surface with a field-free step.
+template <typename T>
+CKF_HD void land_or_stop(Move<T>& m, int st, double s) {
+  if (st != STOP_NONE) { m.stop = st; m.phase = PH_FIN; return; }
+  straight_close(m.y, m.D, s, m.ib, m.dib);
+  m.phase = (m.phase == PH_PLANE) ? PH_FIN : PH_LANDED;
+}
+
+// One step of a move in PH_CYL / PH_PLANE: targeting + landing (P4, P5), else one RKN4 trial (P2, P3).  After an
+// accepted trial the next one is targeted at once and its stage-1 field read is issued BEFORE the Jacobian columns of
+// the accepted step are computed, so that the loads fly during that arithmetic.
 template <typename T>
 CKF_HD void move_step(Move<T>& m, const FieldDev& fld, const CfgDev& cfg, int& n_trials, int& n_accepted) {
-  if (!m.retry) {
-    double s;
-    if (m.phase == PH_PLANE) {
-      const double dn = dot3(m.y.d, m.tn);
-      if (!(fabs(dn) > 1e-12)) { m.stop = STOP_NUMERIC; m.phase = PH_FIN; return; }
-      const double rel[3] = {m.tc[0] - m.y.r[0], m.tc[1] - m.y.r[1], m.tc[2] - m.y.r[2]};
-      s = dot3(rel, m.tn) / dn;
-    } else {
-      const double a = m.y.d[0] * m.y.d[0] + m.y.d[1] * m.y.d[1];
-      const double b = m.y.r[0] * m.y.d[0] + m.y.r[1] * m.y.d[1];
-      const double cc = m.y.r[0] * m.y.r[0] + m.y.r[1] * m.y.r[1] - m.R * m.R;
-      const double disc = b * b - a * cc;
-      if (!(b > 0.0) || !(disc >= 0.0)) { m.stop = STOP_NOT_OUTGOING; m.phase = PH_FIN; return; }
-      s = -cc / (b + sqrt(disc));
-    }
-    if (!isfinite(s)) { m.stop = STOP_NUMERIC; m.phase = PH_FIN; return; }
-    if (fabs(s) <= cfg.surf_tol) {
-      straight_close(m.y, m.D, s, m.ib, m.dib);  // P5
-      m.phase = (m.phase == PH_PLANE) ? PH_FIN : PH_LANDED;
-      return;
-    }
-    const double hlim = fmin(m.h_ctrl, cfg.h_max);  // P4
-    m.h = (fabs(s) <= hlim) ? s : (s > 0.0 ? hlim : -hlim);
+  if (!m.targeted) {   // a fresh position (start of a phase)
+    double s = 0.0;
+    const int st = target_distance(m, s);
+    if (st != STOP_NONE || fabs(s) <= cfg.surf_tol) { land_or_stop(m, st, s); return; }
+    set_trial(m, fld, cfg, s);
   }
-  m.retry = false;
   if (++m.n_steps > cfg.max_rk_steps) { m.stop = STOP_STEP_LIMIT; m.phase = PH_FIN; return; }
   Trial<T> t;
-  rk_trial<T>(fld, m.y, KAPPA * m.y.qop, m.h, t);
+  rk_trial<T>(fld, m.y, m.B1, KAPPA * m.y.qop, m.h, t);
   ++n_trials;
   if (!isfinite(t.eps)) { m.stop = STOP_NUMERIC; m.phase = PH_FIN; return; }
   double f;
@@ -416,12 +438,19 @@ CKF_HD void move_step(Move<T>& m, const FieldDev& fld, const CfgDev& cfg, int& n
     f = f > 4.0 ? 4.0 : f;
   }
   if (t.eps <= cfg.rk_tol) {
-    rk_accept<T>(m.y, m.D, m.h, t, m.ib, m.dib);
-    m.h_ctrl = fabs(m.h) * f;
+    const double h = m.h;
+    rk_accept_state<T>(m.y, h, t, m.ib);
+    m.h_ctrl = fabs(h) * f;
     ++n_accepted;
+    m.targeted = false;
+    double s = 0.0;
+    const int st = target_distance(m, s);
+    const bool more = st == STOP_NONE && fabs(s) > cfg.surf_tol;
+    if (more) set_trial(m, fld, cfg, s);            // the loads of the next trial's stage 1 start here ...
+    rk_accept_jac<T>(m.y, m.D, h, t, m.dib);        // ... and fly while D <- D_step D is computed
+    if (!more) land_or_stop(m, st, s);              // the closing drift acts on the updated D
   } else {
-    m.h = m.h * f;
-    m.retry = true;
+    m.h = m.h * f;                                  // retry from the same position: same B1
   }
 }
 

@@ -111,7 +111,8 @@ __global__ void __launch_bounds__(STEP_NT, MINB) ckf_step(const KParams<T> p, in
   const size_t TC = (size_t)p.tcap;
 
   Move<T> m;
-  m.phase = PH_IDLE; m.stop = STOP_NONE; m.from = 0; m.tgt = -1; m.lp = 0; m.n_steps = 0; m.retry = false;
+  m.phase = PH_IDLE; m.stop = STOP_NONE; m.from = 0; m.tgt = -1; m.lp = 0; m.n_steps = 0; m.targeted = false;
+  m.B1[0] = m.B1[1] = m.B1[2] = 0.0;
   m.h = 0.0; m.h_ctrl = 0.0; m.R = 0.0; m.y.qop = 0.0; m.ib = 0.0; m.dib = 0.0;
   int tip = -1, nt = 0, na = 0;
   bool more = true;  // the level's cursor is not exhausted (warp-uniform)
