@@ -60,6 +60,8 @@ def lib():
         L.oracle_result_free.argtypes = [C.c_void_p]
         L.oracle_field_at.argtypes = [C.POINTER(OField), _dp, _dp]
         L.oracle_set_n3_literal_walk.argtypes = [C.c_int32]
+        L.oracle_resolve_ambiguity.restype = None
+        L.oracle_resolve_ambiguity.argtypes = [C.c_int32, _ip, _ip, _dp, C.c_int32, C.c_int32, C.c_double, _ip, _ip]
         L.oracle_propagate_free.restype = C.c_int32
         L.oracle_propagate_free.argtypes = [C.POINTER(OField), C.POINTER(OConfig), C.c_int32, _dp, _dp, C.c_double, _dp,
                                             _dp, _ip]
@@ -319,3 +321,15 @@ def rts_smooth(xp, Cp, xf, Cf, J):
     xs, Cs = np.zeros((n, 6)), np.zeros((n, 36))
     rc = lib().oracle_rts_smooth(n, _pd(xp), _pd(Cp), _pd(xf), _pd(Cf), _pd(J), _pd(xs), _pd(Cs))
     return rc, xs, Cs.reshape(n, 6, 6)
+
+
+# ------------------------------------------------------------------ AR: ambiguity resolution
+def resolve_ambiguity(track_offsets, meas_idx, chi2_sum, n_measurements: int, max_shared_hits: int = 1,
+                      max_shared_fraction: float = 1.0):
+    """Greedy shared-hit resolver (rules AR1-AR3).  Returns (accepted[n_tracks] in {0,1}, n_shared[n_tracks])."""
+    to, mi, c2 = _i(track_offsets), _i(meas_idx), _d(chi2_sum)
+    nt = c2.shape[0]
+    acc, ns = np.zeros(nt, np.int32), np.zeros(nt, np.int32)
+    lib().oracle_resolve_ambiguity(nt, _pi(to), _pi(mi), _pd(c2), int(n_measurements), int(max_shared_hits),
+                                   float(max_shared_fraction), _pi(acc), _pi(ns))
+    return acc, ns

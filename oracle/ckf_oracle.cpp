@@ -21,6 +21,8 @@
 // scipy's multilinear interpolator); the material path factor x/X0 / |d.n| for inclined tracks; the closed form of
 // R10 against a literal one-child-at-a-time greedy (which children survive, with branches finishing at different
 // levels); reading D11 against the literal N3 walk (pin hook oracle_set_n3_literal_walk): same candidates.
+// Ambiguity resolution (rules AR, tests/test_oracle_resolve.py): the greedy's result against the unique fixed point of
+// its defining property found by brute force over all subsets of a small candidate set; limits k = 0 and k = infinity.
 // Parity unpinned (convention only, fixed by DESIGN.md): that R10 cuts in TIP order (the closed form itself is pinned),
 // hole-only-when-nothing-passes (A5), outward-only navigation (A7), inclusive in-bounds edges (A10),
 // min_measurements = 3 (A14).
@@ -1101,6 +1103,45 @@ struct Result {
   Counters cnt;
 };
 
+// ====================================================================================== AR: ambiguity resolution
+// PAPER.md:98 (section 4): "Duplicate tracks arise when multiple tracks share the same or very similar hit patterns ...
+// an additional algorithm -- known as ambiguity resolution -- will be integrated into the reconstruction chain to
+// remove such tracks after the CKF stage."  The paper names the stage and gives no algorithm; rules AR1-AR3 of
+// DESIGN.md 3 (readings) define a greedy shared-hit resolver over the candidates ckf_find reported:
+//   AR1  a candidate's quality key is (number of measurements DESCENDING, chi2 sum rounded to float32 ASCENDING,
+//        candidate index ASCENDING): longer first, then better chi2; the index makes the order total.
+//   AR2  candidates are visited in that order; a measurement belongs to the first ACCEPTED candidate that holds it.
+//   AR3  a candidate is accepted iff the number s of its measurements that already belong to accepted candidates
+//        satisfies s <= max_shared_hits and s <= max_shared_fraction * n_meas; an accepted candidate then takes its
+//        free measurements; a rejected one takes nothing.
+// Written out as exactly that loop.
+void resolve_ambiguity(int n_tracks, const int32_t* offsets, const int32_t* meas, const double* chi2_sum, int n_meas_total,
+                       int max_shared_hits, double max_shared_fraction, int32_t* accepted, int32_t* n_shared) {
+  std::vector<int> order(n_tracks);
+  for (int t = 0; t < n_tracks; ++t) order[t] = t;
+  std::stable_sort(order.begin(), order.end(), [&](int a, int b) {
+    const int na = offsets[a + 1] - offsets[a], nb = offsets[b + 1] - offsets[b];
+    if (na != nb) return na > nb;
+    const float ca = (float)chi2_sum[a], cb = (float)chi2_sum[b];
+    if (ca != cb) return ca < cb;
+    return a < b;
+  });
+  std::vector<int> owner(n_meas_total, -1);
+  for (int k = 0; k < n_tracks; ++k) {
+    const int t = order[k];
+    const int n = offsets[t + 1] - offsets[t];
+    int s = 0;
+    for (int e = offsets[t]; e < offsets[t + 1]; ++e)
+      if (owner[meas[e]] >= 0) ++s;
+    const bool ok = s <= max_shared_hits && (double)s <= max_shared_fraction * (double)n;
+    accepted[t] = ok ? 1 : 0;
+    n_shared[t] = s;
+    if (ok)
+      for (int e = offsets[t]; e < offsets[t + 1]; ++e)
+        if (owner[meas[e]] < 0) owner[meas[e]] = t;
+  }
+}
+
 }  // namespace
 
 // ====================================================================================== C interface
@@ -1276,6 +1317,14 @@ int32_t oracle_rts_smooth(int32_t n, const double* xp, const double* Cp, const d
 }
 
 // ---- pieces exposed for the pins (tests/test_oracle_pins.py)
+// AR1-AR3 on a CSR list of candidates (HOST arrays); accepted[t] in {0, 1}, n_shared[t] = s at the decision.
+void oracle_resolve_ambiguity(int32_t n_tracks, const int32_t* track_offsets, const int32_t* meas_idx, const double* chi2_sum,
+                              int32_t n_measurements, int32_t max_shared_hits, double max_shared_fraction,
+                              int32_t* accepted, int32_t* n_shared) {
+  resolve_ambiguity(n_tracks, track_offsets, meas_idx, chi2_sum, n_measurements, max_shared_hits, max_shared_fraction,
+                    accepted, n_shared);
+}
+
 void oracle_set_n3_literal_walk(int32_t on) { g_n3_literal_walk = on ? 1 : 0; }
 
 void oracle_field_at(const OField* f, const double r[3], double B[3]) { field_at(*f, r, B); }
