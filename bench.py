@@ -353,6 +353,19 @@ def main():
     fit_work = [int(v) // (2 * n_fit + 3) for v in fits["work"].cpu().tolist()]   # trials, accepted, moves, updates per call
     fit_states = int(fits["n_states"][:res1.n_tracks].sum().item())
 
+    # ---- row f4: shared-hit ambiguity resolution of the same candidates (ckf_resolve)
+    ckf.find(devs[(W - 1) % N_EVENTS], out, stream)
+    reso = ckf.alloc_resolution()
+    ckf.resolve(out, ev_chk.n_measurements, reso, 1, 1.0, stream)
+    torch.cuda.synchronize()
+    fa.record(stream)
+    for _ in range(n_fit):
+        ckf.resolve(out, ev_chk.n_measurements, reso, 1, 1.0, stream)
+    fb.record(stream)
+    torch.cuda.synchronize()
+    resolve_ms = fa.elapsed_time(fb) / n_fit
+    resolve_kept, resolve_rounds = [int(v) for v in reso["summary"].cpu()]
+
     # ---- e2e = BASELINE.json configs[4]: 64 distinct events, pinned host buffers, 4 host threads x 4 streams
     e2e = None
     if n_e2e_ev:
@@ -458,6 +471,10 @@ def main():
                     "flop_per_event": fit_flop, "achieved_tflops": fit_flop / (fit_ms * 1e-3) / 1e12,
                     "launches_per_call": "per pass of <= 262,144 candidates: 4 memsets + (ckf_step + ckf_fit_level) per level "
                                          "(max_levels = %d) + 2" % cfg.ckf.max_levels},
+            "resolve": {"what": "ckf_resolve: greedy shared-hit ambiguity resolution (PAPER.md:98, rules AR1-AR3) of ONE "
+                                "configs[3] event's candidates, max_shared_hits = 1; one cooperative launch",
+                        "ms_per_event": resolve_ms, "candidates": res1.n_tracks, "kept": resolve_kept,
+                        "rounds": resolve_rounds, "value": res1.n_tracks / (resolve_ms * 1e-3), "unit": "candidates/s"},
             "gpu_launches": launches_per_find * args.steps,
             "gpu_launches_per_find": launches_per_find,
             "clocks": clocks,

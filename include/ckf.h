@@ -240,6 +240,30 @@ typedef struct {
 int ckf_fit(ckf_handle* handle, const ckf_measurements* measurements, const ckf_seeds* seeds, const ckf_tracks* tracks,
             ckf_fits* out, void* cuda_stream);
 
+/* ---- Ambiguity resolution after the CKF ----------------------------------
+ * "Duplicate tracks arise when multiple tracks share the same or very similar hit patterns ... an additional
+ * algorithm -- known as ambiguity resolution -- will be integrated into the reconstruction chain to remove such tracks
+ * after the CKF stage".  The paper gives no algorithm; rules AR1-AR3 of DESIGN.md 3 define a greedy
+ * shared-hit resolver: candidates are ranked by (more measurements, smaller chi2_sum rounded to float32, lower
+ * index); visited in that order, a candidate is ACCEPTED iff the number s of its measurements that already belong to
+ * accepted candidates satisfies s <= max_shared_hits and s <= max_shared_fraction * n_meas; an accepted candidate
+ * takes its free measurements.  The result equals that sequential greedy exactly and is deterministic.
+ * DEVICE pointers, caller-owned, sized from max_tracks. */
+typedef struct {
+  int32_t* accepted;           /* [max_tracks] 1 = kept, 0 = removed                                        */
+  int32_t* n_shared;           /* [max_tracks] s of the candidate's decision                                */
+  int32_t* summary;            /* [2] number of accepted candidates, rounds the parallel resolution took    */
+  int32_t max_shared_hits;     /* INPUT                                                                      */
+  double max_shared_fraction;  /* INPUT; 1.0 = no fractional limit                                           */
+} ckf_resolution;
+
+/* Resolves the candidates of `tracks` (the DEVICE arrays ckf_find filled; *tracks->n_tracks is read on the device).
+ * n_measurements = ckf_measurements.n of that find.  Asynchronous on `cuda_stream`, allocates nothing (20 bytes per
+ * measurement and 12 per candidate were reserved by ckf_create); at most 2^24 candidates.  Calls on different streams
+ * are ordered one after the other (one workspace per handle). */
+int ckf_resolve(ckf_handle* handle, const ckf_tracks* tracks, int32_t n_measurements, ckf_resolution* out,
+                void* cuda_stream);
+
 /* Copies the work counters of the most recent ckf_find issued on `cuda_stream` (synchronises that stream). */
 int ckf_get_counters(ckf_handle* handle, void* cuda_stream, ckf_counters* out);
 

@@ -21,7 +21,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libckf.so")
 
 EXPORTS = ("ckf_create", "ckf_find", "ckf_find_host", "ckf_fit", "ckf_get_counters", "ckf_get_launch_info", "ckf_destroy",
-           "ckf_set_timing", "ckf_get_timing", "ckf_measure_alu_peak",
+           "ckf_set_timing", "ckf_get_timing", "ckf_measure_alu_peak", "ckf_resolve",
            "ckf_last_error", "ckf_abi_version")
 
 
@@ -65,6 +65,11 @@ class ckf_fits(C.Structure):
                 ("first_cov", _vp), ("entry_params", _vp), ("work", _vp), ("smoother_precision", C.c_int32), ("smoother", C.c_int32)]
 
 
+class ckf_resolution(C.Structure):
+    _fields_ = [("accepted", _vp), ("n_shared", _vp), ("summary", _vp), ("max_shared_hits", C.c_int32),
+                ("max_shared_fraction", C.c_double)]
+
+
 class ckf_timing(C.Structure):
     _fields_ = [("init_ms", C.c_float), ("sort_ms", C.c_float), ("step_ms", C.c_float), ("visit_ms", C.c_float),
                 ("scan_ms", C.c_float), ("update_ms", C.c_float), ("emit_ms", C.c_float), ("launches", C.c_int32)]
@@ -96,6 +101,8 @@ def load_library():
         L.ckf_fit.restype = C.c_int
         L.ckf_fit.argtypes = [_vp, C.POINTER(ckf_measurements), C.POINTER(ckf_seeds), C.POINTER(ckf_tracks),
                               C.POINTER(ckf_fits), _vp]
+        L.ckf_resolve.restype = C.c_int
+        L.ckf_resolve.argtypes = [_vp, C.POINTER(ckf_tracks), C.c_int32, C.POINTER(ckf_resolution), _vp]
         L.ckf_set_timing.restype = C.c_int
         L.ckf_set_timing.argtypes = [_vp, C.c_int]
         L.ckf_get_timing.restype = C.c_int
@@ -339,6 +346,26 @@ class CKF:
                 a = a[:n_entries] if k == "entry_params" else a[:n_tracks]
             out[k] = a.astype(np.float64) if a.dtype.kind == "f" else a.copy()
         return out
+
+    # ------------------------------------------------------------------ ambiguity resolution (ckf_resolve)
+    def alloc_resolution(self, device="cuda"):
+        t = self.torch
+        i32 = dict(dtype=t.int32, device=device)
+        return dict(accepted=t.zeros(self.max_tracks, **i32), n_shared=t.zeros(self.max_tracks, **i32),
+                    summary=t.zeros(2, **i32))
+
+    def resolve(self, tracks: dict, n_measurements: int, res: dict, max_shared_hits: int = 1,
+                max_shared_fraction: float = 1.0, stream=None):
+        """Asynchronous ckf_resolve of the candidates in `tracks` (device tensors filled by `find`)."""
+        st = stream if stream is not None else self.torch.cuda.current_stream()
+        o = ckf_tracks(*[tracks[k].data_ptr() for k in ("n_tracks", "status", "track_offsets", "meas_idx", "seed_id",
+                                                        "n_holes", "last_module", "stop_reason", "params", "cov",
+                                                        "chi2_sum", "entry_chi2")])
+        r = ckf_resolution(res["accepted"].data_ptr(), res["n_shared"].data_ptr(), res["summary"].data_ptr(),
+                           int(max_shared_hits), float(max_shared_fraction))
+        rc = self.lib.ckf_resolve(self.handle, C.byref(o), int(n_measurements), C.byref(r), _vp(st.cuda_stream))
+        if rc != 0:
+            raise RuntimeError("ckf_resolve failed (%d): %s" % (rc, self.lib.ckf_last_error(self.handle).decode()))
 
     def find_host(self, host_event: dict, host_out: dict, stream=None):
         """ckf_find_host on (pinned) host tensors: H2D, find, D2H inside; synchronous on return."""

@@ -22,6 +22,7 @@
 #include "ckf_branch.cuh"
 #include "ckf_fit.cuh"
 #include "ckf_peak.cuh"
+#include "ckf_resolve.cuh"
 #include "ckf_sort.cuh"
 #include "ckf_step.cuh"
 #include "ckf_visit.cuh"
@@ -100,6 +101,11 @@ struct ckf_handle {
   int32_t *ft_from = nullptr, *ft_tgt = nullptr, *ft_stop = nullptr, *ft_order = nullptr;
   int fit_chunk = 0, fit_states = 0;
   cudaEvent_t fit_done = nullptr;
+  // workspace of ckf_resolve (one per handle; calls are ordered one after the other)
+  unsigned long long *rs_key = nullptr, *rs_best = nullptr;
+  int32_t *rs_owner = nullptr, *rs_state = nullptr, *rs_g = nullptr;
+  int resolve_grid = 0;
+  cudaEvent_t resolve_done = nullptr;
   bool timing_print = false;
   bool timing = false;  // ckf_set_timing / CKF_TIMING=1: per-kernel CUDA-event times of every ckf_find on stderr (debug aid; synchronises)
 };
@@ -514,6 +520,17 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     CKB(cudaEventCreateWithFlags(&h->fit_done, cudaEventDisableTiming));
     h->fit_chunk = chunk; h->fit_states = ns;
   }
+  // ---- workspace of ckf_resolve (row f4): 20 B per measurement + 12 B per candidate
+  {
+    const size_t M = (size_t)c->max_measurements, NTK = (size_t)c->max_tracks;
+    CKB(dalloc(h, &h->rs_key, NTK * 8)); CKB(dalloc(h, &h->rs_best, 2 * M * 8));
+    CKB(dalloc(h, &h->rs_owner, M * 4)); CKB(dalloc(h, &h->rs_state, NTK * 4)); CKB(dalloc(h, &h->rs_g, 4 * 4));
+    CKB(cudaEventCreateWithFlags(&h->resolve_done, cudaEventDisableTiming));
+    int per_sm = 0;
+    if (c->precision == 32) CKB(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ckf_resolve_kernel<float>, RESOLVE_NT, 0));
+    else CKB(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ckf_resolve_kernel<double>, RESOLVE_NT, 0));
+    h->resolve_grid = std::max(1, per_sm) * h->sm_count;   // a cooperative launch needs every block resident
+  }
 #undef CKB
   *out = h;
   return CKF_OK;
@@ -637,6 +654,37 @@ int ckf_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, const 
   return rc;
 }
 
+int ckf_resolve(ckf_handle* h, const ckf_tracks* t, int32_t n_measurements, ckf_resolution* o, void* stream) {
+  if (!h) return CKF_E_ARG;
+  if (!t || !o) return fail(h, CKF_E_ARG, "null argument");
+  if (!t->n_tracks || !t->track_offsets || !t->meas_idx || !t->chi2_sum) return fail(h, CKF_E_ARG, "null input array");
+  if (!o->accepted || !o->n_shared || !o->summary) return fail(h, CKF_E_ARG, "null output array");
+  if (n_measurements < 0 || n_measurements > h->cfg.max_measurements)
+    return fail(h, CKF_E_CAPACITY, "n_measurements %d exceeds capacity %d", n_measurements, h->cfg.max_measurements);
+  if (h->cfg.max_tracks > (1 << 24)) return fail(h, CKF_E_CAPACITY, "ckf_resolve ranks at most 2^24 candidates");
+  if (o->max_shared_hits < 0 || !(o->max_shared_fraction >= 0.0)) return fail(h, CKF_E_ARG, "bad sharing limits");
+  cudaStream_t st = (cudaStream_t)stream;
+  std::lock_guard<std::mutex> lk(h->mu);
+  cudaStreamWaitEvent(st, h->resolve_done, 0);   // one workspace: resolutions are ordered one after the other
+  cudaError_t e;
+  if (h->cfg.precision == 32) {
+    ResolveParams<float> p{t->n_tracks, t->track_offsets, t->meas_idx, (const float*)t->chi2_sum, h->cfg.max_tracks,
+                           n_measurements, o->max_shared_hits, o->max_shared_fraction, h->rs_key, h->rs_best, h->rs_owner,
+                           h->rs_state, h->rs_g, o->accepted, o->n_shared, o->summary};
+    void* args[] = {&p};
+    e = cudaLaunchCooperativeKernel((void*)ckf_resolve_kernel<float>, dim3(h->resolve_grid), dim3(RESOLVE_NT), args, 0, st);
+  } else {
+    ResolveParams<double> p{t->n_tracks, t->track_offsets, t->meas_idx, (const double*)t->chi2_sum, h->cfg.max_tracks,
+                            n_measurements, o->max_shared_hits, o->max_shared_fraction, h->rs_key, h->rs_best, h->rs_owner,
+                            h->rs_state, h->rs_g, o->accepted, o->n_shared, o->summary};
+    void* args[] = {&p};
+    e = cudaLaunchCooperativeKernel((void*)ckf_resolve_kernel<double>, dim3(h->resolve_grid), dim3(RESOLVE_NT), args, 0, st);
+  }
+  cudaEventRecord(h->resolve_done, st);
+  if (e != cudaSuccess) return fail(h, CKF_E_CUDA, "ckf_resolve launch failed: %s", cudaGetErrorString(e));
+  return CKF_OK;
+}
+
 int ckf_get_counters(ckf_handle* h, void* stream, ckf_counters* out) {
   if (!h || !out) return CKF_E_ARG;
   cudaStream_t st = (cudaStream_t)stream;
@@ -749,6 +797,7 @@ int ckf_destroy(ckf_handle* h) {
     if (w.pinned_nt) cudaFreeHost(w.pinned_nt);
   }
   if (h->fit_done) cudaEventDestroy(h->fit_done);
+  if (h->resolve_done) cudaEventDestroy(h->resolve_done);
   for (void* p : h->allocs) cudaFree(p);
   delete h;
   return CKF_OK;

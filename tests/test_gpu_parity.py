@@ -643,3 +643,76 @@ def test_more_streams_than_workspaces_is_ordered():
     oras = [oracle.find_event(st, e, n_threads=8) for e in evs]
     for i, r in enumerate(res):
         parity.assert_fp32_parity(r, oras[i % 6], evs[i % 6].n_seeds, cfg.ckf.chi2_max, "call %d" % i)
+
+
+@pytest.mark.parametrize("config,limits", [(1, (1, 1.0)), (1, (0, 1.0)), (2, (2, 0.25)), (3, (1, 1.0)), (3, (3, 0.5))])
+def test_resolve_ambiguity_parity(config, limits):
+    """ckf_resolve (row f4) against the oracle's sequential greedy on the SAME candidates (the CUDA
+    path's own lists and chi2 sums): accepted flags and shared-hit counts bit-exact; twice the same result."""
+    import torch
+    import oracle
+    det, fld, cfg = synth.config_bundle(config)
+    ev = synth.make_event(config, det=det)
+    ckf, dev, out, gpu, _ = _run_gpu(det, fld, cfg, ev)
+    res = ckf.alloc_resolution()
+    ckf.resolve(out, ev.n_measurements, res, *limits)
+    torch.cuda.synchronize()
+    acc = res["accepted"][:gpu.n_tracks].cpu().numpy()
+    ns = res["n_shared"][:gpu.n_tracks].cpu().numpy()
+    n_acc, rounds = [int(v) for v in res["summary"].cpu()]
+    # the oracle ranks by the float32-rounded chi2 sum: feed it the values the CUDA path reported
+    chi2 = out["chi2_sum"][:gpu.n_tracks].cpu().numpy().astype(np.float64)
+    o_acc, o_ns = oracle.resolve_ambiguity(gpu.track_offsets, gpu.meas_idx, chi2, ev.n_measurements, *limits)
+    assert np.array_equal(acc, o_acc)
+    assert np.array_equal(ns, o_ns)
+    assert n_acc == int(o_acc.sum())
+    res2 = ckf.alloc_resolution()
+    ckf.resolve(out, ev.n_measurements, res2, *limits)
+    torch.cuda.synchronize()
+    assert torch.equal(res["accepted"][:gpu.n_tracks], res2["accepted"][:gpu.n_tracks])
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(5):
+        ckf.resolve(out, ev.n_measurements, res2, *limits)
+    b.record()
+    torch.cuda.synchronize()
+    print("resolve configs[%d] limits %s: %d of %d candidates kept, %d rounds, %.3f ms" %
+          (config, limits, n_acc, gpu.n_tracks, rounds, a.elapsed_time(b) / 5))
+    ckf.close()
+
+
+def test_resolve_edge_cases():
+    """No candidates at all; a limit that keeps everything; exact duplicates keep one."""
+    import torch
+    from paper_2505_22822_b200 import CKF
+    det, fld, cfg = synth.config_bundle(1)
+    ev = synth.make_event(1, det=det, n_particles=60)
+    ckf, dev, out, gpu, _ = _run_gpu(det, fld, cfg, ev)
+    res = ckf.alloc_resolution()
+    ckf.resolve(out, ev.n_measurements, res, 1000, 1.0)
+    torch.cuda.synchronize()
+    assert int(res["summary"][0]) == gpu.n_tracks and bool(res["accepted"][:gpu.n_tracks].all())
+    empty = dict(dev)
+    for k in ("seed_module", "seed_params", "seed_cov"):
+        empty[k] = dev[k][:0]
+    ckf.find(empty, out)
+    ckf.resolve(out, ev.n_measurements, res, 1, 1.0)
+    torch.cuda.synchronize()
+    assert int(res["summary"][0]) == 0
+    # the same seed twice gives every candidate twice: with no sharing allowed exactly one copy of each survives
+    twice = dict(dev)
+    for k in ("seed_module", "seed_params", "seed_cov"):
+        twice[k] = torch.cat([dev[k][:20], dev[k][:20]])
+    ckf.find(twice, out)
+    torch.cuda.synchronize()
+    t2 = ckf.download(out)
+    ckf.resolve(out, ev.n_measurements, res, 0, 1.0)
+    torch.cuda.synchronize()
+    acc = res["accepted"][:t2.n_tracks].cpu().numpy().astype(bool)
+    kept = {tuple(t2.meas_list(t).tolist()) for t in np.flatnonzero(acc)}
+    assert len(kept) == int(acc.sum())                        # no list twice among the survivors
+    first = t2.seed_id < 20
+    assert not (acc[~first] & np.array([tuple(t2.meas_list(t).tolist()) in
+                                         {tuple(t2.meas_list(u).tolist()) for u in np.flatnonzero(acc & first)}
+                                         for t in np.flatnonzero(~first)])).any()
+    ckf.close()
