@@ -33,7 +33,7 @@
 extern "C" {
 #endif
 
-#define CKF_ABI_VERSION 6
+#define CKF_ABI_VERSION 7
 
 /* return codes */
 #define CKF_OK 0
@@ -114,6 +114,11 @@ typedef struct {
   int32_t max_tips_per_level;       /* live branch tips of one level, whole event; 0 = 8 * max_seeds     */
   int32_t n_streams;                /* independent workspaces; concurrent ckf_find calls up to this many */
   int32_t max_events_per_find;      /* largest batch of events one ckf_find may carry; 0 = 1 (see ckf_measurements) */
+  int32_t energy_loss;              /* 1: mean energy loss of the muon hypothesis (Bethe, silicon, DESIGN.md rule E) in every
+                                       crossed module of x_over_x0 > 0: q/p changes on leaving the module and the
+                                       covariance is transported with d(q/p)'/d(q/p).  0: none (BASELINE configs)     */
+  int32_t field_gradient;           /* must be 0: the field-gradient terms of the transport Jacobian (PAPER.md ref
+                                       [18]) exist in the oracle only (reading A13)                          */
   int32_t max_fit_tracks;           /* ckf_fit: candidates fitted per pass; sizes the state store reserved in ckf_create
                                        (max_levels states x min(max_fit_tracks, max_tracks, 262144) candidates x
                                        (12 float64 + 69 T): 3 GB at 262,144 in fp32).  0 = no ckf_fit on this handle */

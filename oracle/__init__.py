@@ -36,7 +36,8 @@ class OConfig(C.Structure):
     _fields_ = [("chi2_max", C.c_double), ("max_branches_per_surface", C.c_int32),
                 ("max_candidates_per_seed", C.c_int32), ("max_holes", C.c_int32), ("min_measurements", C.c_int32),
                 ("rk_tolerance_mm", C.c_double), ("surface_tolerance_mm", C.c_double), ("h_max_mm", C.c_double),
-                ("particle_mass_gev", C.c_double), ("max_rk_steps_per_surface", C.c_int32), ("max_levels", C.c_int32)]
+                ("particle_mass_gev", C.c_double), ("max_rk_steps_per_surface", C.c_int32), ("max_levels", C.c_int32),
+                ("energy_loss", C.c_int32), ("field_gradient", C.c_int32)]
 
 
 STOP_NAMES = {0: "NONE", 1: "EXIT", 2: "HOLES", 3: "NOT_OUTGOING", 4: "STEP_LIMIT", 5: "NUMERIC", 6: "LEVEL_LIMIT"}
@@ -78,6 +79,10 @@ def lib():
         L.oracle_highland_theta0.restype = C.c_double
         L.oracle_highland_theta0.argtypes = [C.c_double, C.c_double, C.c_double]
         L.oracle_add_material.argtypes = [C.POINTER(OGeometry), C.POINTER(OConfig), C.c_int32, _dp, _dp]
+        L.oracle_bethe_dedx.restype = C.c_double
+        L.oracle_bethe_dedx.argtypes = [C.c_double, C.c_double]
+        L.oracle_energy_loss.restype = C.c_double
+        L.oracle_energy_loss.argtypes = [C.POINTER(OGeometry), C.POINTER(OConfig), C.c_int32, _dp, _dp, _dp]
         L.oracle_kf_fit.restype = None
         L.oracle_kf_fit.argtypes = [C.POINTER(OGeometry), C.POINTER(OField), C.POINTER(OConfig), _ip, _dp, _dp, _ip, _dp,
                                     _dp, C.c_int32, _ip, _ip, _ip, C.c_int32, _ip, _ip, _dp, _dp, _dp, _dp, _dp, C.c_int32]
@@ -135,7 +140,7 @@ class Setup:
             f.grid = grid.ctypes.data_as(_fp)
         c = OConfig()
         for name, _t in OConfig._fields_:
-            setattr(c, name, getattr(ckf, name))
+            setattr(c, name, getattr(ckf, name, 0))
         self.geometry, self.field, self.config = g, f, c
         self.det = det
 
@@ -259,6 +264,19 @@ def add_material(setup: Setup, module, x, Cov):
     x, Cov = _d(x), _d(Cov).reshape(36).copy()
     lib().oracle_add_material(C.byref(setup.geometry), C.byref(setup.config), int(module), _pd(x), _pd(Cov))
     return Cov.reshape(6, 6)
+
+
+def bethe_dedx(p, mass):
+    """Mean stopping power [GeV cm^2 / g] of the oracle's rule E (silicon, no density correction)."""
+    return lib().oracle_bethe_dedx(float(p), float(mass))
+
+
+def energy_loss(setup: Setup, module, x):
+    """Rule E on leaving `module`: (dE [GeV], parameters after the loss, g = d(q/p)'/d(q/p))."""
+    x = _d(x)
+    xo, g = np.zeros(6), C.c_double(1.0)
+    dE = lib().oracle_energy_loss(C.byref(setup.geometry), C.byref(setup.config), int(module), _pd(x), _pd(xo), C.byref(g))
+    return dE, xo, g.value
 
 
 # ------------------------------------------------------------------ K: KF fit + RTS smoother (PAPER.md:35)

@@ -76,6 +76,8 @@ struct OConfig {
   double particle_mass_gev;
   int32_t max_rk_steps_per_surface;
   int32_t max_levels;
+  int32_t energy_loss;      // 1: mean energy loss of rule E in every crossed module (0 = BASELINE configs: "no energy loss")
+  int32_t field_gradient;   // 1: transport Jacobian with the field-gradient terms of PAPER.md ref [18] (reading A13; 0 = ref [17])
 };
 
 enum StopReason { STOP_NONE = 0, STOP_EXIT = 1, STOP_HOLES = 2, STOP_NOT_OUTGOING = 3, STOP_STEP_LIMIT = 4,
@@ -489,6 +491,53 @@ void add_material(const OConfig& cfg, const Module& m, const double x[6], double
   C[2][2] += th0 * th0 / (st * st);
 }
 
+// ---------------------------------------------------------------------------------- E: mean energy loss
+// "effects from material interactions are evaluated by assuming muon trajectories".  BASELINE configs
+// switch energy loss off; rule E adds the MEAN loss of the muon hypothesis in
+// every crossed module, next to V5.  Mean stopping power of a heavy charged particle (Bethe, as tabulated by the PDG
+// review "Passage of particles through matter"), density-effect correction neglected (reading):
+//   -dE/dx = K (Z/A) / beta^2 [ 1/2 ln(2 me beta^2 gamma^2 Wmax / I^2) - beta^2 ],
+//   Wmax = 2 me (beta gamma)^2 / (1 + 2 gamma me/M + (me/M)^2),      K = 0.307075 MeV cm^2 / mol.
+// The modules are silicon (configs[0]: "0.15 mm silicon (x/X0 = 0.0016)"): Z/A = 0.49848 mol/g, I = 173 eV,
+// X0 = 21.82 g/cm^2, so a module of x/X0 crossed at incidence |d.n| is (x/X0) / |d.n| * 21.82 g/cm^2 of silicon.
+constexpr double EL_K = 0.307075e-3;      // GeV cm^2 / mol
+constexpr double EL_Z_OVER_A = 0.49848;   // mol / g   (silicon)
+constexpr double EL_I = 173.0e-9;         // GeV       (silicon mean excitation energy)
+constexpr double EL_X0 = 21.82;           // g / cm^2  (silicon radiation length)
+constexpr double EL_ME = 0.51099895e-3;   // GeV
+
+// mean stopping power [GeV cm^2 / g] of a singly charged particle of mass M and momentum p in silicon
+double bethe_dedx(double p, double M) {
+  const double bg2 = (p * p) / (M * M);
+  const double E = std::sqrt(p * p + M * M);
+  const double beta2 = (p * p) / (E * E), gamma = E / M;
+  const double r = EL_ME / M;
+  const double wmax = 2.0 * EL_ME * bg2 / (1.0 + 2.0 * gamma * r + r * r);
+  return EL_K * EL_Z_OVER_A / beta2 * (0.5 * std::log(2.0 * EL_ME * bg2 * wmax / (EL_I * EL_I)) - beta2);
+}
+
+// Rule E on leaving module m with bound parameters x: returns dE [GeV]; xo = x with q/p after the loss
+// (E' = E - dE, p' = sqrt(E'^2 - M^2); not finite if the particle would stop), g = d(q/p)'/d(q/p) with dE held
+// fixed (reading: like the field gradient in J2, the slow dependence of dE on p is neglected):
+//   dE' = dE = (p/E) dp,  dp' = (E'/p') dE'   =>   g = (p/p')^3 (E'/E).
+double energy_loss(const OConfig& cfg, const Module& m, const double x[6], double xo[6], double& g) {
+  for (int i = 0; i < 6; ++i) xo[i] = x[i];
+  g = 1.0;
+  if (!cfg.energy_loss || !(m.x_over_x0 > 0.0)) return 0.0;
+  const double M = cfg.particle_mass_gev;
+  const double st = std::sin(x[3]), ct = std::cos(x[3]);
+  const double d[3] = {st * std::cos(x[2]), st * std::sin(x[2]), ct};
+  const double cosi = std::fabs(dot(d, m.n));
+  const double p = 1.0 / std::fabs(x[4]);
+  const double E = std::sqrt(p * p + M * M);
+  const double dE = bethe_dedx(p, M) * (m.x_over_x0 / cosi) * EL_X0;
+  const double E2 = E - dE;
+  const double p2 = std::sqrt(E2 * E2 - M * M);     // NaN if E' < M: the tip then stops NUMERIC
+  xo[4] = (x[4] < 0.0 ? -1.0 : 1.0) / p2;
+  g = (p / p2) * (p / p2) * (p / p2) * (E2 / E);
+  return dE;
+}
+
 // ---------------------------------------------------------------------------------- N: navigation
 // PIN HOOK: 1 = walk the remaining portal cylinders literally as SURVEY.md N3 words it ("l' <- l' + 1 and repeat"),
 // 0 (default) = reading D11: a tip beyond every further half-length and moving away in z stops EXIT at
@@ -541,10 +590,14 @@ int move_to_next_module(const OGeometry& g, const OField& fld, const OConfig& cf
   const Module m = get_module(g, from);
   double C[6][6];
   std::memcpy(C, Cin, sizeof(C));
-  add_material(cfg, m, x, C);
+  add_material(cfg, m, x, C);              // V5, with the momentum the tip arrived with
+  double xd[6], gE = 1.0;                  // E: departure parameters after the mean energy loss, J_E = diag(1,1,1,1,gE,1)
+  energy_loss(cfg, m, x, xd, gE);
+  if (!std::isfinite(xd[4])) return STOP_NUMERIC;
+  for (int i = 0; i < 6; ++i) { C[i][4] *= gE; C[4][i] *= gE; }   // C <- J_E C J_E^T (C[4][4] gets gE twice)
   FreeState y;
   double B2F[8][6];
-  bound_to_free(m, x, y, B2F);
+  bound_to_free(m, xd, y, B2F);
   set_identity8(y.D);
   y.h_ctrl = cfg.h_max_mm;
   y.n_steps = 0;
@@ -595,7 +648,7 @@ int move_to_next_module(const OGeometry& g, const OField& fld, const OConfig& cf
   for (int i = 0; i < 6; ++i) {
     if (!std::isfinite(xp[i])) return STOP_NUMERIC;
     for (int j = 0; j < 6; ++j) {
-      if (Jout) Jout[i][j] = J[i][j];
+      if (Jout) Jout[i][j] = J[i][j] * (j == 4 ? gE : 1.0);   // d(arrival) / d(parameters before the loss) = J J_E
       if (!std::isfinite(Cp[i][j])) return STOP_NUMERIC;
     }
   }
@@ -1409,6 +1462,13 @@ void oracle_kalman_update(const double x[6], const double C[36], const double lo
 }
 
 double oracle_highland_theta0(double p, double x_eff, double mass) { return highland_theta0(p, x_eff, mass); }
+
+double oracle_bethe_dedx(double p, double mass) { return bethe_dedx(p, mass); }
+
+// rule E on module `module`: returns dE [GeV], xo[6] = parameters after the loss, *g = d(q/p)'/d(q/p)
+double oracle_energy_loss(const OGeometry* g, const OConfig* cfg, int32_t module, const double x[6], double xo[6], double* gE) {
+  return energy_loss(*cfg, get_module(*g, module), x, xo, *gE);
+}
 
 void oracle_add_material(const OGeometry* g, const OConfig* cfg, int32_t module, const double x[6], double C[36]) {
   double Cm[6][6];

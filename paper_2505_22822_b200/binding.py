@@ -43,7 +43,8 @@ class ckf_config(C.Structure):
                 ("particle_mass_gev", C.c_double), ("max_rk_steps_per_surface", C.c_int32), ("max_levels", C.c_int32),
                 ("max_seeds", C.c_int32), ("max_measurements", C.c_int32), ("max_tracks", C.c_int32),
                 ("max_track_entries", C.c_int32), ("max_links", C.c_int32), ("max_tips_per_level", C.c_int32),
-                ("n_streams", C.c_int32), ("max_events_per_find", C.c_int32), ("max_fit_tracks", C.c_int32)]
+                ("n_streams", C.c_int32), ("max_events_per_find", C.c_int32), ("energy_loss", C.c_int32),
+                ("field_gradient", C.c_int32), ("max_fit_tracks", C.c_int32)]
 
 
 class ckf_measurements(C.Structure):
@@ -173,6 +174,8 @@ def make_config(ckf, precision: int, max_seeds: int, max_measurements: int, max_
     c.max_tips_per_level = int(max_tips_per_level)
     c.max_events_per_find = int(max_events_per_find)
     c.max_fit_tracks = int(max_fit_tracks)
+    c.energy_loss = int(getattr(ckf, "energy_loss", 0))
+    c.field_gradient = int(getattr(ckf, "field_gradient", 0))
     return c
 
 

@@ -367,6 +367,8 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     return fail(h, CKF_E_ARG, "capacities must be positive");
   if (g->n_layers < 1 || g->n_modules < 1) return fail(h, CKF_E_ARG, "empty geometry");
   if (f->kind != 0 && f->kind != 1) return fail(h, CKF_E_ARG, "field kind must be 0 or 1");
+  if (c->field_gradient != 0)
+    return fail(h, CKF_E_ARG, "field_gradient = 1 (gradient terms in the transport Jacobian) is not built in the CUDA path");
   if (f->kind == 1 && (!f->grid || f->n[0] < 2 || f->n[1] < 2 || f->n[2] < 2))
     return fail(h, CKF_E_ARG, "field grid needs >= 2 nodes per axis");
   for (int l = 0; l < g->n_layers; ++l)
@@ -433,6 +435,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
   h->kcfg.h_max = c->h_max_mm; h->kcfg.mass = c->particle_mass_gev; h->kcfg.max_branches = c->max_branches_per_surface;
   h->kcfg.max_cands = c->max_candidates_per_seed; h->kcfg.max_holes = c->max_holes; h->kcfg.min_meas = c->min_measurements;
   h->kcfg.max_rk_steps = c->max_rk_steps_per_surface; h->kcfg.max_levels = c->max_levels;
+  h->kcfg.energy_loss = c->energy_loss ? 1 : 0;
   // ---- launch configuration: ckf_step is persistent (one wave of resident blocks), ckf_visit grid-strides
   {
     int per_sm = 0, vper_sm = 0;
@@ -474,7 +477,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     const size_t TC = (size_t)h->tcap, KB = (size_t)c->max_branches_per_surface;
     CKB(dalloc(h, &w.tip_link, 2 * TC * 4)); CKB(dalloc(h, &w.tip_seed, 2 * TC * 4));
     CKB(dalloc(h, &w.mv_y, 8 * TC * sizeof(double))); CKB(dalloc(h, &w.pd_x, 6 * TC * sizeof(double)));
-    CKB(dalloc(h, (char**)&w.mv_D, (size_t)MVD * TC * ts)); CKB(dalloc(h, (char**)&w.mv_dep, 5 * TC * sizeof(double)));
+    CKB(dalloc(h, (char**)&w.mv_D, (size_t)MVD * TC * ts)); CKB(dalloc(h, (char**)&w.mv_dep, (size_t)NDEP * TC * sizeof(double)));
     CKB(dalloc(h, (char**)&w.pd_C, 21 * TC * sizeof(double))); CKB(dalloc(h, (char**)&w.sel_chi2, KB * TC * ts));
     CKB(dalloc(h, &w.sel_idx, KB * TC * 4));
     CKB(dalloc(h, &w.mv_from, TC * 4)); CKB(dalloc(h, &w.mv_tgt, 2 * TC * 4)); CKB(dalloc(h, &w.mv_stop, TC * 4));
@@ -514,7 +517,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     CKB(dalloc(h, &h->fs_next, CHK * 4));
     CKB(dalloc(h, &h->ft_g, 2 * GBLK * 4)); CKB(dalloc(h, &h->ft_counters, CNT_N * 8));
     CKB(dalloc(h, &h->ft_y, 8 * CHK * sizeof(double)));
-    CKB(dalloc(h, (char**)&h->ft_D, (size_t)MVD * CHK * ts)); CKB(dalloc(h, (char**)&h->ft_dep, 5 * CHK * sizeof(double)));
+    CKB(dalloc(h, (char**)&h->ft_D, (size_t)MVD * CHK * ts)); CKB(dalloc(h, (char**)&h->ft_dep, (size_t)NDEP * CHK * sizeof(double)));
     CKB(dalloc(h, &h->ft_from, CHK * 4)); CKB(dalloc(h, &h->ft_tgt, 2 * CHK * 4)); CKB(dalloc(h, &h->ft_stop, CHK * 4));
     CKB(dalloc(h, &h->ft_order, (size_t)NBIN * CHK * 4));
     CKB(cudaEventCreateWithFlags(&h->fit_done, cudaEventDisableTiming));

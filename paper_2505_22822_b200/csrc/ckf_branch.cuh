@@ -311,12 +311,12 @@ __global__ void __launch_bounds__(SCAN_NT, CKF_UPDATE_MINB) ckf_update(const KPa
     if ((ncounts & 0xffff) + (ncounts >> 16) >= p.cfg.max_levels) stop = STOP_LEVEL_LIMIT;
     else {
       Traj y;
-      double dep[5];
+      double dep[NDEP];
       stop = departure_state(p.geo, p.cfg, target, xo, y, dep);
       if (stop == STOP_NONE) {
         store_traj(p.mv_y, (size_t)c, y);
 #pragma unroll
-        for (int i = 0; i < 5; ++i) p.mv_dep[i * TC + c] = dep[i];
+        for (int i = 0; i < NDEP; ++i) p.mv_dep[i * TC + c] = dep[i];
         // N2 here, at full lanes, instead of inside the RKN4 kernel: the overlap neighbour of the child's departure
         const int ov = overlap_neighbour(p.geo, target, y.r, y.d);
         p.mv_tgt[TC + c] = ov;

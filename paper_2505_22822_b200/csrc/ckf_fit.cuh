@@ -22,7 +22,8 @@ constexpr int FIT_NT = 128;
 constexpr int FIT_CHUNK = 262144;   // tracks per pass: bounds the state store (ckf.cu loops over the chunks)
 // float64 per state: xp[6], xf[6], Cp[21], Cf[21] (packed upper triangles), the V5 variances (phi, theta) added on
 // leaving the previous state -- the covariance algebra is float64 in both modes
-constexpr int FS_XP = 0, FS_XF = 6, FS_CP = 12, FS_CF = 33, FS_Q = 54, FS_X = 56;
+// (FS_Q: q_phi, q_theta, and the energy-loss factor g of rule E, the q/p row of the full Jacobian being g e_4)
+constexpr int FS_XP = 0, FS_XF = 6, FS_CP = 12, FS_CF = 33, FS_Q = 54, FS_X = 57;
 constexpr int FS_T = 25;            // T per state: J (5x5 block, row-major), built from the T-typed transport Jacobian
 
 template <typename T>
@@ -83,7 +84,7 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, con
     int status = STOP_NONE, module = 0, next = 0, stored = level;
     bool done = false;
     T c2sum = T(0);
-    double q_in[2] = {0.0, 0.0};
+    double q_in[3] = {0.0, 0.0, 1.0};
 #pragma unroll
     for (int i = 0; i < 6; ++i) xf[i] = 0.0;
 #pragma unroll
@@ -116,18 +117,17 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, con
         load_jac(kp.mv_D, (size_t)s, m.D);
         m.from = kp.mv_from[s];
         m.tgt = kp.mv_tgt[s];
-        double dep[5];
+        double dep[NDEP];
 #pragma unroll
-        for (int i = 0; i < 5; ++i) dep[i] = kp.mv_dep[i * CH + s];
+        for (int i = 0; i < NDEP; ++i) dep[i] = kp.mv_dep[i * CH + s];
         status = move_arrive<T>(m, dep, p.geo, p.fld, p.cfg, xp, J);
         if (status == STOP_NONE) {
           double C[21];
           const double* pt = p.fs_x + (size_t)(level - 1) * FS_X * CH + s;  // filtered covariance of the previous state
 #pragma unroll
           for (int i = 0; i < 21; ++i) C[i] = pt[(FS_CF + i) * CH];
-          C[tri(2, 2)] += dep[3];  // V5 on leaving
-          C[tri(3, 3)] += dep[4];
-          q_in[0] = dep[3]; q_in[1] = dep[4];
+          leave_module_cov(C, dep);  // V5 and rule E on leaving
+          q_in[0] = dep[3]; q_in[1] = dep[4]; q_in[2] = dep[5];
           transport_cov<double>(J, C, Cp);
           bool fin = true;
 #pragma unroll
@@ -167,18 +167,19 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, con
         for (int b = 0; b < 5; ++b) ft[(a * 5 + b) * CH] = (T)J[a][b];
       fx[(FS_Q + 0) * CH] = q_in[0];
       fx[(FS_Q + 1) * CH] = q_in[1];
+      fx[(FS_Q + 2) * CH] = q_in[2];
       p.fs_meas[(size_t)level * CH + s] = used;
       stored = level + 1;
       if (next == n) done = true;
       else if (stored >= p.cfg.max_levels || stored >= p.max_states) status = STOP_LEVEL_LIMIT;
       else {
         Traj y;
-        double dep[5];
+        double dep[NDEP];
         status = departure_state(p.geo, p.cfg, module, xf, y, dep);
         if (status == STOP_NONE) {  // the track as a tip of the next level's ckf_step
           store_traj(kp.mv_y, (size_t)s, y);
 #pragma unroll
-          for (int i = 0; i < 5; ++i) kp.mv_dep[i * CH + s] = dep[i];
+          for (int i = 0; i < NDEP; ++i) kp.mv_dep[i * CH + s] = dep[i];
           kp.mv_from[s] = module;
           const int ov = overlap_neighbour(p.geo, module, y.r, y.d);  // N2
           kp.mv_tgt[CH + s] = ov;
@@ -347,12 +348,16 @@ __global__ void __launch_bounds__(FIT_NT, CKF_SMOOTH_MINB) ckf_fit_smooth(const 
           for (int r = 0; r < 5; ++r)
 #pragma unroll
             for (int l = 0; l < 5; ++l) Jb[r][l] = (A)bt[(size_t)(r * 5 + l) * CH];
+          // rule E: the full Jacobian is J_arrival J_E, J_E = diag(1,1,1,1,g,1): column q/p times g, row q/p = g e_4
+          const A gE = (A)bx[(size_t)(FS_Q + 2) * CH];
+#pragma unroll
+          for (int r = 0; r < 5; ++r) Jb[r][4] *= gE;
 #pragma unroll
           for (int c = 0; c < 6; ++c) {
             A col[6];
 #pragma unroll
             for (int i = 0; i < 6; ++i) {
-              if (i == 4) col[i] = Cf[tri(4, c)];
+              if (i == 4) col[i] = gE * Cf[tri(4, c)];
               else {
                 const int r = (i == 5) ? 4 : i;
                 A v = (i == 5) ? Cf[tri(5, c)] : A(0);
@@ -567,14 +572,15 @@ __global__ void __launch_bounds__(FIT_NT, CKF_SMOOTH_MINB) ckf_fit_smooth_tf(con
           }
         }
         // Jf: rows 0..3 = J[0..3] over columns 0..4, row 4 = e_4, row 5 = J[4] plus 1 at column 5
+        const A gE = (A)fx[(size_t)(FS_Q + 2) * CH];
         A Jf[6][6];
 #pragma unroll
         for (int i = 0; i < 6; ++i)
 #pragma unroll
           for (int j = 0; j < 6; ++j) {
-            if (i == 4) Jf[i][j] = (j == 4) ? A(1) : A(0);
+            if (i == 4) Jf[i][j] = (j == 4) ? gE : A(0);     // rule E: J_arrival J_E
             else if (j == 5) Jf[i][j] = (i == 5) ? A(1) : A(0);
-            else Jf[i][j] = (A)ft[(size_t)(((i == 5) ? 4 : i) * 5 + j) * CH];
+            else Jf[i][j] = (A)ft[(size_t)(((i == 5) ? 4 : i) * 5 + j) * CH] * ((j == 4) ? gE : A(1));
           }
         A Yz[21], yz[6];
         {

@@ -102,7 +102,7 @@ struct KParams {
   // departure / arrival state of the move (ckf_update -> ckf_step -> ckf_visit)
   double* mv_y;        // [tcap][8] r, d, t, q/p (move records, see below)
   T* mv_D;             // [tcap][MVD] transport Jacobian (ckf_step -> ckf_visit)
-  double* mv_dep;      // [5][tcap] direction on departure, Highland q_phi, q_theta
+  double* mv_dep;      // [NDEP][tcap] direction on departure, Highland q_phi, q_theta, energy-loss factor g
   int32_t* mv_from;    // [tcap] module the tip stands on
   int32_t* mv_tgt;     // [2][tcap] module reached; overlap neighbour at departure (N2, by ckf_update), -1 none
   int32_t* mv_stop;    // [tcap] stop reason so far

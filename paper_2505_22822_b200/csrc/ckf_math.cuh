@@ -60,6 +60,7 @@ struct CfgDev {
   double chi2_max;
   double rk_tol, surf_tol, h_max, mass;
   int32_t max_branches, max_cands, max_holes, min_meas, max_rk_steps, max_levels;
+  int32_t energy_loss;   // rule E: mean energy loss in every crossed module (BASELINE configs: 0)
 };
 
 // ------------------------------------------------------------------------------------------ small algebra

@@ -11,6 +11,8 @@ struct GeoDev {
   int32_t n_layers, n_modules;
 };
 
+constexpr int NDEP = 6;  // numbers of a departure record (departure_state): direction[3], q_phi, q_theta, g
+
 // Packed upper triangle of a symmetric 6x6: index of (i, j), i <= j.
 CKF_HD constexpr int tri(int i, int j) { return i <= j ? i * 6 - (i * (i - 1)) / 2 + (j - i) : j * 6 - (j * (j - 1)) / 2 + (i - j); }
 
@@ -79,6 +81,18 @@ CKF_HD double highland_theta0_sq(double xx0, double cosi, double qop, double mas
   const double X = xx0 / cosi;
   const double th0 = 0.0136 / (beta * p) * sqrt(X) * (1.0 + 0.038 * log(X / (beta * beta)));
   return th0 * th0;
+}
+
+// E: mean energy loss of the muon hypothesis in a silicon module (rule E).  Mean stopping power
+// of a heavy singly charged particle (Bethe, PDG review "Passage of particles through matter"), density correction
+// neglected, in GeV cm^2 / g:  K (Z/A) / beta^2 [ 1/2 ln(2 me (beta gamma)^2 Wmax / I^2) - beta^2 ],
+// Wmax = 2 me (beta gamma)^2 / (1 + 2 gamma me/M + (me/M)^2);  silicon: Z/A 0.49848, I 173 eV, X0 21.82 g/cm^2.
+CKF_HD double mean_dedx_silicon(double p, double M) {
+  const double me = 0.51099895e-3, I = 173.0e-9, KZA = 0.307075e-3 * 0.49848;
+  const double E = sqrt(p * p + M * M);
+  const double bg2 = (p * p) / (M * M), beta2 = (p * p) / (E * E), rm = me / M;
+  const double wmax = 2.0 * me * bg2 / (1.0 + 2.0 * (E / M) * rm + rm * rm);
+  return KZA / beta2 * (0.5 * log(2.0 * me * bg2 * wmax / (I * I)) - beta2);
 }
 
 // J4 + J5: the non-trivial 5x5 block of the bound->bound Jacobian.  Rows (l0, l1, phi, theta, t), columns
@@ -160,6 +174,17 @@ CKF_HD void arrival_jacobian(const Jac<TD>& D, const double dep_u[3], const doub
   J[4][2] = -c * nRgphi;
   J[4][3] = -c * nRgth;
   J[4][4] = (T)D.tq - c * nrq;
+}
+
+// Covariance of a tip on LEAVING its module: V5 noise on (phi, theta), then rule E, C <- J_E C J_E^T with
+// J_E = diag(1, 1, 1, 1, g, 1).
+CKF_HD void leave_module_cov(double C[21], const double dep[NDEP]) {
+  C[tri(2, 2)] += dep[3];
+  C[tri(3, 3)] += dep[4];
+  const double g = dep[5];
+#pragma unroll
+  for (int i = 0; i < 6; ++i) C[tri(i, 4)] *= g;
+  C[tri(4, 4)] *= g;
 }
 
 // C' = Jf C Jf^T on the packed upper triangle, Jf = full 6x6 built from the 5x5 block (see arrival_jacobian).
@@ -276,9 +301,11 @@ struct Move {
 };
 
 // Departure state of a tip with bound parameters x on module `from` (J1, V5): global position and direction,
-// the direction again for the bound->free Jacobian, and the Highland variances to add to C[phi][phi],
-// C[theta][theta] on leaving.  Returns STOP_NUMERIC for non-finite parameters or theta outside (0, pi).
-CKF_HD int departure_state(const GeoDev& g, const CfgDev& cfg, int from, const double x[6], Traj& y, double dep[5]) {
+// the direction again for the bound->free Jacobian, the Highland variances to add to C[phi][phi], C[theta][theta] on
+// leaving (dep[3], dep[4]) and, with rule E, q/p after the mean energy loss in the module (y.qop) with
+// dep[5] = g = d(q/p)'/d(q/p) = (p/p')^3 (E'/E), the energy lost held fixed (1 when rule E is off).
+// Returns STOP_NUMERIC for non-finite parameters, theta outside (0, pi), or a particle that would stop in the module.
+CKF_HD int departure_state(const GeoDev& g, const CfgDev& cfg, int from, const double x[6], Traj& y, double dep[NDEP]) {
   bool ok = true;
 #pragma unroll
   for (int i = 0; i < 6; ++i) ok = ok && isfinite(x[i]);
@@ -298,10 +325,20 @@ CKF_HD int departure_state(const GeoDev& g, const CfgDev& cfg, int from, const d
   y.qop = x[4];
   dep[3] = 0.0;  // q_phi
   dep[4] = 0.0;  // q_theta
+  dep[5] = 1.0;  // g
   if (k.xx0 > 0.0) {
-    const double th2 = highland_theta0_sq(k.xx0, fabs(dot3(y.d, k.n)), y.qop, cfg.mass);
+    const double cosi = fabs(dot3(y.d, k.n));
+    const double th2 = highland_theta0_sq(k.xx0, cosi, y.qop, cfg.mass);   // V5: with the momentum the tip arrived with
     dep[4] = th2;
     dep[3] = th2 / (st * st);
+    if (cfg.energy_loss) {
+      const double p = 1.0 / fabs(y.qop), E = sqrt(p * p + cfg.mass * cfg.mass);
+      const double dE = mean_dedx_silicon(p, cfg.mass) * (k.xx0 / cosi) * 21.82;
+      const double E2 = E - dE, p2 = sqrt(E2 * E2 - cfg.mass * cfg.mass);
+      y.qop = (y.qop < 0.0 ? -1.0 : 1.0) / p2;
+      dep[5] = (p / p2) * (p / p2) * (p / p2) * (E2 / E);
+      if (!isfinite(y.qop)) return STOP_NUMERIC;
+    }
   }
   return STOP_NONE;
 }
@@ -457,7 +494,7 @@ CKF_HD void move_step(Move<T>& m, const FieldDev& fld, const CfgDev& cfg, int& n
 // Arrival (J4, J5) of a move in PH_FIN with stop == NONE: predicted bound parameters and the 5x5 Jacobian
 // block.  Returns the final stop reason (NUMERIC if a predicted parameter is not finite).
 template <typename T>
-CKF_HD int move_arrive(const Move<T>& m, const double dep[5], const GeoDev& g, const FieldDev& fld, const CfgDev& cfg,
+CKF_HD int move_arrive(const Move<T>& m, const double dep[NDEP], const GeoDev& g, const FieldDev& fld, const CfgDev& cfg,
                        double xp[6], double J[5][5]) {
   const ModuleRec& k = g.mod[m.tgt];
   const ModuleRec& m0 = g.mod[m.from];
@@ -480,9 +517,10 @@ CKF_HD int move_arrive(const Move<T>& m, const double dep[5], const GeoDev& g, c
 // One tip at a time (host test harness): the transitions above in their natural order.
 template <typename T>
 CKF_HD int move_to_next_module(const GeoDev& g, const FieldDev& fld, const CfgDev& cfg, int from, const double x[6],
-                               int& target, double xp[6], double J[5][5], double& q_phi, double& q_theta, StepCtl& sc) {
+                               int& target, double xp[6], double J[5][5], double& q_phi, double& q_theta, double& g_e,
+                               StepCtl& sc) {
   Move<T> m;
-  double dep[5];
+  double dep[NDEP];
   const int st0 = departure_state(g, cfg, from, x, m.y, dep);
   if (st0 != STOP_NONE) return st0;
   move_begin(m, cfg, from);
@@ -498,6 +536,7 @@ CKF_HD int move_to_next_module(const GeoDev& g, const FieldDev& fld, const CfgDe
   }
   q_phi = dep[3];
   q_theta = dep[4];
+  g_e = dep[5];
   if (m.stop != STOP_NONE) return m.stop;
   const int st = move_arrive(m, dep, g, fld, cfg, xp, J);
   if (st == STOP_NONE) target = m.tgt;

@@ -208,9 +208,9 @@ __global__ void __launch_bounds__(VISIT_NT, MINB) ckf_visit(const KParams<T> p, 
           load_jac(p.mv_D, (size_t)t, m.D);
           m.from = p.mv_from[t];
           m.tgt = p.mv_tgt[t];
-          double dep[5];
+          double dep[NDEP];
 #pragma unroll
-          for (int i = 0; i < 5; ++i) dep[i] = p.mv_dep[i * TC + t];
+          for (int i = 0; i < NDEP; ++i) dep[i] = p.mv_dep[i * TC + t];
           double xp[6];
           double J[5][5];
           stop = move_arrive<T>(m, dep, p.geo, p.fld, p.cfg, xp, J);
@@ -219,8 +219,7 @@ __global__ void __launch_bounds__(VISIT_NT, MINB) ckf_visit(const KParams<T> p, 
             double C[21], Co[21];
 #pragma unroll
             for (int i = 0; i < 21; ++i) C[i] = p.lk_C[(size_t)i * p.max_links + link];
-            C[tri(2, 2)] += dep[3];
-            C[tri(3, 3)] += dep[4];
+            leave_module_cov(C, dep);
             transport_cov<double>(J, C, Co);
             bool fin = true;
 #pragma unroll

@@ -42,6 +42,8 @@ class CKFSettings:
     particle_mass_gev: float = M_MUON
     max_rk_steps_per_surface: int = 64
     max_levels: int = 32
+    energy_loss: int = 0          # rule E (mean energy loss per module); BASELINE configs: off
+    field_gradient: int = 0       # transport Jacobian with field-gradient terms (oracle only); BASELINE configs: off
 
 
 @dataclass

@@ -23,19 +23,19 @@ struct Ctx {
 
 template <typename T>
 int move_t(Ctx* c, int from, const double* x, const double* C36, int* target, double* xp, double* Cp36, int* trials) {
-  double J[5][5], qphi, qth;
+  double J[5][5], qphi, qth, ge;
   StepCtl sc;
   sc.n_trials = 0; sc.n_accepted = 0;
   int tg = -1;
-  int st = move_to_next_module<T>(c->geo, c->fld, c->cfg, from, x, tg, xp, J, qphi, qth, sc);
+  int st = move_to_next_module<T>(c->geo, c->fld, c->cfg, from, x, tg, xp, J, qphi, qth, ge, sc);
   *target = tg;
   if (trials) *trials = sc.n_trials;
   if (st != STOP_NONE) return st;
   double C[21], Co[21];
   for (int i = 0; i < 6; ++i)
     for (int j = i; j < 6; ++j) C[tri(i, j)] = C36[6 * i + j];
-  C[tri(2, 2)] += qphi;
-  C[tri(3, 3)] += qth;
+  const double dep[NDEP] = {0.0, 0.0, 0.0, qphi, qth, ge};
+  leave_module_cov(C, dep);
   transport_cov<double>(J, C, Co);
   for (int i = 0; i < 6; ++i)
     for (int j = 0; j < 6; ++j) Cp36[6 * i + j] = (double)Co[tri(i, j)];
@@ -81,6 +81,7 @@ void* hm_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c) 
   x->cfg.h_max = c->h_max_mm; x->cfg.mass = c->particle_mass_gev; x->cfg.max_branches = c->max_branches_per_surface;
   x->cfg.max_cands = c->max_candidates_per_seed; x->cfg.max_holes = c->max_holes; x->cfg.min_meas = c->min_measurements;
   x->cfg.max_rk_steps = c->max_rk_steps_per_surface; x->cfg.max_levels = c->max_levels;
+  x->cfg.energy_loss = c->energy_loss ? 1 : 0;
   return x;
 }
 void hm_destroy(void* p) { delete (Ctx*)p; }

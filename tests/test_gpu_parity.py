@@ -716,3 +716,51 @@ def test_resolve_edge_cases():
                                          {tuple(t2.meas_list(u).tolist()) for u in np.flatnonzero(acc & first)}
                                          for t in np.flatnonzero(~first)])).any()
     ckf.close()
+
+
+@pytest.mark.parametrize("config", [1, 2])
+def test_energy_loss_parity(config):
+    """Rule E (row f3: mean energy loss of the muon hypothesis in every crossed module) switched on: ckf_find and ckf_fit
+    against the oracle with the same switch; the candidates really differ from the run without it."""
+    import copy
+    import torch
+    import oracle
+    det, fld, cfg = synth.config_bundle(config)
+    cfg = copy.deepcopy(cfg)
+    cfg.ckf.energy_loss = 1
+    ev = synth.make_event(config, det=det, n_particles=3000 if config == 2 else None)
+    ora = _run_oracle(det, fld, cfg, ev)
+    ckf, dev, out, gpu, cnt = _run_gpu(det, fld, cfg, ev)
+    assert gpu.status == 0
+    if cfg.precision == 64:
+        parity.assert_bit_exact_lists(gpu, ora)
+        rel, chi2, cov = parity.max_param_diffs(gpu, ora)
+        assert rel < 1e-9 and chi2 < 1e-8 and cov < 1e-7, (rel, chi2, cov)
+        for k in ("visits", "rk_trials", "rk_accepted", "gate_tests", "updates", "tips"):
+            assert cnt[k] == ora.counters[k], k
+    else:
+        r = parity.assert_fp32_parity(gpu, ora, ev.n_seeds, cfg.ckf.chi2_max, "energy loss, configs[%d]" % config)
+        print("energy loss config", config, {k: v for k, v in r.items() if k != "bad_seeds"})
+    # q/p at the last measurement is larger in magnitude than without the loss (the same lists mostly survive)
+    cfg0 = copy.deepcopy(cfg)
+    cfg0.ckf.energy_loss = 0
+    ora0 = _run_oracle(det, fld, cfg0, ev)
+    same = ora0.n_tracks == ora.n_tracks and np.array_equal(ora0.meas_idx, ora.meas_idx)
+    if same:
+        assert np.mean(np.abs(ora.params[:, 4]) > np.abs(ora0.params[:, 4])) > 0.95
+    # the fit follows the same rule: forward pass ends on the CKF's state, smoothed parameters equal the oracle's
+    fits = ckf.alloc_fits()
+    ckf.fit(dev, out, fits)
+    torch.cuda.synchronize()
+    g = ckf.download_fits(fits, gpu.n_tracks, int(gpu.meas_idx.size))
+    for smoother in (0, 1):
+        if smoother == 1:
+            ckf.fit(dev, out, fits, smoother=1)
+            torch.cuda.synchronize()
+            g = ckf.download_fits(fits, gpu.n_tracks, int(gpu.meas_idx.size))
+        o = oracle.kf_fit(oracle.Setup(det, fld, cfg.ckf), ev, gpu.track_offsets, gpu.meas_idx, gpu.seed_id, n_threads=8,
+                          smoother=smoother)
+        rf = parity.compare_fits(g, o, gpu.track_offsets)
+        tol = 1e-9 if cfg.precision == 64 else 1e-5
+        assert rf["n_not_pd_gpu_only"] == 0 and rf["max_smoothed_rel"] < tol and rf["max_last_rel"] < tol, (smoother, rf)
+    ckf.close()

@@ -13,10 +13,14 @@ def _rel(a, b, floor):
     return np.abs(a - b) / np.maximum(np.maximum(np.abs(a), np.abs(b)), floor)
 
 
-@pytest.mark.parametrize("config,precision,tol_x,tol_c", [(0, 64, 1e-10, 1e-9), (2, 64, 1e-10, 1e-9),
-                                                          (2, 32, 1e-9, 2e-6)])
-def test_moves_and_updates_match_oracle(config, precision, tol_x, tol_c):
+@pytest.mark.parametrize("config,precision,tol_x,tol_c,eloss", [(0, 64, 1e-10, 1e-9, 0), (2, 64, 1e-10, 1e-9, 0),
+                                                                (2, 32, 1e-9, 2e-6, 0), (1, 64, 1e-10, 1e-9, 1),
+                                                                (2, 32, 1e-9, 2e-6, 1)])
+def test_moves_and_updates_match_oracle(config, precision, tol_x, tol_c, eloss):
+    import copy
     det, fld, cfg = synth.config_bundle(config)
+    cfg = copy.deepcopy(cfg)
+    cfg.ckf.energy_loss = eloss        # rule E (mean energy loss per module), off in the BASELINE configs
     ev = synth.make_event(config, det=det, n_particles=60, n_fake_seeds=0)
     st = oracle.Setup(det, fld, cfg.ckf)
     hm = HostMath(det, fld, cfg.ckf)
