@@ -21,6 +21,11 @@
 // scipy's multilinear interpolator); the material path factor x/X0 / |d.n| for inclined tracks; the closed form of
 // R10 against a literal one-child-at-a-time greedy (which children survive, with branches finishing at different
 // levels); reading D11 against the literal N3 walk (pin hook oracle_set_n3_literal_walk): same candidates.
+// Energy loss (rule E, tests/test_oracle_eloss.py): minimum of the Bethe curve against the PDG table value for silicon
+// (golden file), non-relativistic limit, energy conservation, g against finite differences of the kinematics, the
+// whole move's Jacobian against finite differences.  Field-gradient Jacobian (J2', tests/test_oracle_pins2.py): finite
+// differences of the bound->bound map in the analytic non-uniform field to 1e-5 with the terms on; the default
+// matrix form of J2 against the tangent form with G = 0 (pin hook field_gradient = 2) in that field.
 // Ambiguity resolution (rules AR, tests/test_oracle_resolve.py): the greedy's result against the unique fixed point of
 // its defining property found by brute force over all subsets of a small candidate set; limits k = 0 and k = infinity.
 // Parity unpinned (convention only, fixed by DESIGN.md): that R10 cuts in TIP order (the closed form itself is pinned),
@@ -154,6 +159,47 @@ void field_at(const OField& f, const double r[3], double B[3]) {
   }
 }
 
+// Gradient of the field, G[i][j] = dB_i / dr_j, for the optional gradient terms of the transport Jacobian (J2'):
+// zero for a uniform field; the exact derivative of the trilinear interpolant inside its cell for a grid (piecewise
+// constant along the differentiated axis); analytic for the pin hook `kind 2`.
+void field_gradient_at(const OField& f, const double r[3], double G[3][3]) {
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) G[i][j] = 0.0;
+  if (f.kind == 0) return;
+  if (f.kind == 2) {
+    const double B0 = f.uniform_b[2], a = f.origin[0];
+    G[0][0] = a * B0 * r[2]; G[0][2] = a * B0 * r[0];
+    G[1][1] = a * B0 * r[2]; G[1][2] = a * B0 * r[1];
+    G[2][2] = -2.0 * a * B0 * r[2];
+    return;
+  }
+  int idx[3];
+  double fr[3];
+  for (int a = 0; a < 3; ++a) {
+    double g = (r[a] - f.origin[a]) / f.spacing[a];
+    int i = (int)std::floor(g);
+    if (i < 0) i = 0;
+    if (i > f.n[a] - 2) i = f.n[a] - 2;
+    idx[a] = i;
+    fr[a] = g - (double)i;
+  }
+  const long long st[3] = {(long long)f.n[1] * f.n[2] * 3, (long long)f.n[2] * 3, 3};
+  const float* p = f.grid + idx[0] * st[0] + idx[1] * st[1] + idx[2] * st[2];
+  for (int c = 0; c < 3; ++c)
+    for (int ax = 0; ax < 3; ++ax) {
+      // d/d(axis ax): difference along ax of the corner values, bilinear in the other two axes
+      const int o1 = (ax + 1) % 3, o2 = (ax + 2) % 3;
+      double acc = 0.0;
+      for (int b1 = 0; b1 < 2; ++b1)
+        for (int b2 = 0; b2 < 2; ++b2) {
+          const long long base = b1 * st[o1] + b2 * st[o2];
+          const double diff = (double)p[base + st[ax] + c] - (double)p[base + c];
+          acc += (b1 ? fr[o1] : 1.0 - fr[o1]) * (b2 ? fr[o2] : 1.0 - fr[o2]) * diff;
+        }
+      G[c][ax] = acc / f.spacing[ax];
+    }
+}
+
 // ---------------------------------------------------------------------------------- free state + transport Jacobian
 // Free vector y = (r[0..2], t, d[0..2], q/p)  (U);  D = d y / d y_departure (8x8, J3)
 struct FreeState {
@@ -188,6 +234,7 @@ inline double dinvbeta_dqop(double qop, double mass) {
 // P2 + P3 + J2: one RKN4 trial of signed length h.  Returns the error estimate eps; on request applies it.
 struct Trial {
   double k1[3], k2[3], k3[3], k4[3], B1[3], B2[3], B4[3];
+  double rm[3], re[3];   // stage points (for the gradient terms of J2')
   double eps;
 };
 
@@ -198,6 +245,7 @@ void rk_trial(const OField& fld, const FreeState& y, double h, Trial& T) {
   cross(y.d, T.B1, tmp);
   for (int i = 0; i < 3; ++i) T.k1[i] = lam * tmp[i];
   for (int i = 0; i < 3; ++i) rm[i] = y.r[i] + 0.5 * h * y.d[i] + h * h / 8.0 * T.k1[i];
+  for (int i = 0; i < 3; ++i) T.rm[i] = rm[i];
   field_at(fld, rm, T.B2);
   for (int i = 0; i < 3; ++i) dd[i] = y.d[i] + 0.5 * h * T.k1[i];
   cross(dd, T.B2, tmp);
@@ -206,6 +254,7 @@ void rk_trial(const OField& fld, const FreeState& y, double h, Trial& T) {
   cross(dd, T.B2, tmp);
   for (int i = 0; i < 3; ++i) T.k3[i] = lam * tmp[i];
   for (int i = 0; i < 3; ++i) re[i] = y.r[i] + h * y.d[i] + h * h / 2.0 * T.k3[i];
+  for (int i = 0; i < 3; ++i) T.re[i] = re[i];
   field_at(fld, re, T.B4);
   for (int i = 0; i < 3; ++i) dd[i] = y.d[i] + h * T.k3[i];
   cross(dd, T.B4, tmp);
@@ -218,8 +267,82 @@ void rk_trial(const OField& fld, const FreeState& y, double h, Trial& T) {
   T.eps = h * h * std::sqrt(e2);
 }
 
-void rk_accept(FreeState& y, double h, const Trial& T, double mass) {
+// J2' (config.field_gradient = 1; reading A13, PAPER.md ref [18]): the step map of P2 differentiated stage by stage
+// with h fixed INCLUDING the dependence of the field on the stage points.  Written as seven tangent vectors
+// (dr, dd, dlam) -- one per column r_x, r_y, r_z, d_x, d_y, d_z, lambda -- pushed through the four stages:
+//   dk1 = lam [dd x B1 + d x (G1 dr)] + dlam (d x B1)
+//   drm = dr + h/2 dd + h^2/8 dk1
+//   dk2 = lam [(dd + h/2 dk1) x B2 + (d + h/2 k1) x (G2 drm)] + dlam ((d + h/2 k1) x B2)      dk3 likewise from k2
+//   dre = dr + h dd + h^2/2 dk3
+//   dk4 = lam [(dd + h dk3) x B4 + (d + h k3) x (G4 dre)] + dlam ((d + h k3) x B4)
+//   dr' = dr + h dd + h^2/6 (dk1 + dk2 + dk3),   dd' = dd + h/6 (dk1 + 2 dk2 + 2 dk3 + dk4)
+// With G = 0 this is J2 (dr'/dr = I, dd'/dr = 0).
+void step_jacobian_with_gradient(const OField& fld, const FreeState& y, double h, const Trial& T, double mass,
+                                 bool zero_gradient, double Ds[8][8]) {
   const double lam = KAPPA * y.qop;
+  double G1[3][3], G2[3][3], G4[3][3];
+  field_gradient_at(fld, y.r, G1);
+  field_gradient_at(fld, T.rm, G2);
+  field_gradient_at(fld, T.re, G4);
+  if (zero_gradient)   // PIN HOOK (field_gradient = 2): this tangent form with G = 0 must equal the matrix form of J2
+    for (int i = 0; i < 3; ++i)
+      for (int j = 0; j < 3; ++j) G1[i][j] = G2[i][j] = G4[i][j] = 0.0;
+  set_identity8(Ds);
+  auto gmul = [](const double G[3][3], const double v[3], double o[3]) {
+    for (int i = 0; i < 3; ++i) o[i] = G[i][0] * v[0] + G[i][1] * v[1] + G[i][2] * v[2];
+  };
+  for (int c = 0; c < 7; ++c) {
+    double dr[3] = {0, 0, 0}, dd[3] = {0, 0, 0}, dlam = 0.0;
+    if (c < 3) dr[c] = 1.0;
+    else if (c < 6) dd[c - 3] = 1.0;
+    else dlam = 1.0;
+    double dk1[3], dk2[3], dk3[3], dk4[3], drm[3], dre[3], w[3], dw[3], a[3], b[3], gb[3];
+    // stage 1
+    cross(dd, T.B1, a);
+    gmul(G1, dr, gb);
+    cross(y.d, gb, b);
+    cross(y.d, T.B1, w);
+    for (int i = 0; i < 3; ++i) dk1[i] = lam * (a[i] + b[i]) + dlam * w[i];
+    for (int i = 0; i < 3; ++i) drm[i] = dr[i] + 0.5 * h * dd[i] + h * h / 8.0 * dk1[i];
+    // stage 2
+    for (int i = 0; i < 3; ++i) { w[i] = y.d[i] + 0.5 * h * T.k1[i]; dw[i] = dd[i] + 0.5 * h * dk1[i]; }
+    cross(dw, T.B2, a);
+    gmul(G2, drm, gb);
+    cross(w, gb, b);
+    cross(w, T.B2, gb);
+    for (int i = 0; i < 3; ++i) dk2[i] = lam * (a[i] + b[i]) + dlam * gb[i];
+    // stage 3
+    for (int i = 0; i < 3; ++i) { w[i] = y.d[i] + 0.5 * h * T.k2[i]; dw[i] = dd[i] + 0.5 * h * dk2[i]; }
+    cross(dw, T.B2, a);
+    gmul(G2, drm, gb);
+    cross(w, gb, b);
+    cross(w, T.B2, gb);
+    for (int i = 0; i < 3; ++i) dk3[i] = lam * (a[i] + b[i]) + dlam * gb[i];
+    for (int i = 0; i < 3; ++i) dre[i] = dr[i] + h * dd[i] + h * h / 2.0 * dk3[i];
+    // stage 4
+    for (int i = 0; i < 3; ++i) { w[i] = y.d[i] + h * T.k3[i]; dw[i] = dd[i] + h * dk3[i]; }
+    cross(dw, T.B4, a);
+    gmul(G4, dre, gb);
+    cross(w, gb, b);
+    cross(w, T.B4, gb);
+    for (int i = 0; i < 3; ++i) dk4[i] = lam * (a[i] + b[i]) + dlam * gb[i];
+    const int col = c < 3 ? c : (c < 6 ? 4 + (c - 3) : 7);
+    const double scale = (c == 6) ? KAPPA : 1.0;   // d/d(q/p) = kappa d/dlam
+    for (int i = 0; i < 3; ++i) {
+      Ds[i][col] = scale * (dr[i] + h * dd[i] + h * h / 6.0 * (dk1[i] + dk2[i] + dk3[i]));
+      Ds[4 + i][col] = scale * (dd[i] + h / 6.0 * (dk1[i] + 2.0 * dk2[i] + 2.0 * dk3[i] + dk4[i]));
+    }
+  }
+  Ds[3][7] = h * dinvbeta_dqop(y.qop, mass);
+}
+
+void rk_accept(const OField& fld, const OConfig& cfg, FreeState& y, double h, const Trial& T, double mass) {
+  const double lam = KAPPA * y.qop;
+  if (cfg.field_gradient) {
+    double Dg[8][8];
+    step_jacobian_with_gradient(fld, y, h, T, mass, cfg.field_gradient == 2, Dg);
+    apply_step_jacobian(y.D, Dg);
+  } else {
   // ---- J2: step Jacobian, field gradient neglected, h fixed
   double M1[3][3], M2[3][3], M4[3][3], A1[3][3], A2[3][3], A3[3][3], A4[3][3], W[3][3], X[3][3];
   double a1[3], a2[3], a3[3], a4[3], dd[3], t1[3], t2[3];
@@ -275,6 +398,7 @@ void rk_accept(FreeState& y, double h, const Trial& T, double mass) {
   }
   Ds[3][7] = h * dinvbeta_dqop(y.qop, mass);
   apply_step_jacobian(y.D, Ds);
+  }
 
   // ---- P2: the state
   double dn[3], nrm2 = 0.0;
@@ -350,7 +474,7 @@ int propagate_to(const OField& fld, const OConfig& cfg, const Target& tg, FreeSt
         if (f > 4.0) f = 4.0;
       }
       if (T.eps <= cfg.rk_tolerance_mm) {
-        rk_accept(y, h, T, mass);
+        rk_accept(fld, cfg, y, h, T, mass);
         y.h_ctrl = std::fabs(h) * f;
         ++cnt.rk_accepted;
         break;

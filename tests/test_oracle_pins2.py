@@ -221,3 +221,94 @@ def test_d11_early_exit_changes_no_candidate():
     assert set(np.unique(lit.stop_reason[diff]).tolist()) <= {3, 4}
     assert d11.counters["rk_trials"] <= lit.counters["rk_trials"]
     assert d11.counters["visits"] == lit.counters["visits"] and d11.counters["updates"] == lit.counters["updates"]
+
+
+# ------------------------------------------------------------------ J2': field-gradient terms of the transport Jacobian
+def _fd_jacobian(st, m_from, m_to, x0):
+    steps = np.array([1e-3, 1e-3, 1e-6, 1e-6, 1e-6 * abs(x0[4]), 1e-3])
+    Jfd = np.zeros((6, 6))
+    for k in range(6):
+        xa, xb = x0.copy(), x0.copy()
+        xa[k] += steps[k]
+        xb[k] -= steps[k]
+        ca, pa, _ = oracle.bound_to_bound(st, m_from, m_to, xa)
+        cb, pb, _ = oracle.bound_to_bound(st, m_from, m_to, xb)
+        assert ca == 0 and cb == 0
+        Jfd[:, k] = (pa - pb) / (2 * steps[k])
+    return Jfd
+
+
+@pytest.mark.parametrize("qop,layers", [(1.0 / 0.7, (4, 5)), (-1.0 / 1.5, (6, 7)), (1.0 / 0.6, (7, 8))])
+def test_jacobian_with_field_gradient_vs_finite_differences(detector, qop, layers):
+    """In the analytic NON-uniform field the Jacobian with the gradient terms (config.field_gradient = 1, reading A13)
+    equals central finite differences of the bound->bound map to 1e-5; without them it is off at the 1e-3..1e-2 level
+    (SURVEY.md pin table J1-J5).  This also pins which field value each stage of J2 uses: B1 = B2 = B4 only in a uniform
+    field."""
+    det = detector
+    l0, l1 = layers
+    m_from = int(det.module_offset[l0] + 0 * det.n_z[l0] + int(det.n_z[l0] * 0.8))     # z ~ +600 mm: dB/dz is large there
+    m_to = int(det.module_offset[l1] + 0 * det.n_z[l1] + int(det.n_z[l1] * 0.8))
+    x0 = np.array([2.0, 10.0, 0.03, 1.45, qop, 3.0])
+    kw = dict(rk_tolerance_mm=1e-9, surface_tolerance_mm=1e-11, max_rk_steps_per_surface=100000)
+    on = oracle.Setup(det, _analytic_field_spec(), CKFSettings(field_gradient=1, **kw))
+    off = oracle.Setup(det, _analytic_field_spec(), CKFSettings(field_gradient=0, **kw))
+    code, xp, J_on = oracle.bound_to_bound(on, m_from, m_to, x0)
+    code2, xp2, J_off = oracle.bound_to_bound(off, m_from, m_to, x0)
+    assert code == 0 and code2 == 0 and np.array_equal(xp, xp2)        # the flag never touches the state
+    Jfd = _fd_jacobian(on, m_from, m_to, x0)
+    scale = np.maximum(np.abs(Jfd), np.max(np.abs(Jfd), axis=1, keepdims=True) * 1e-3 + 1e-12)
+    err_on = np.max(np.abs(J_on - Jfd) / scale)
+    err_off = np.max(np.abs(J_off - Jfd) / scale)
+    assert err_on < 1e-5, err_on
+    assert err_off > 30 * err_on and err_off > 2e-4, (err_on, err_off)
+
+
+def test_field_gradient_flag_is_neutral_in_a_uniform_field(detector):
+    """G = 0: the tangent form of J2' must reproduce the matrix form of J2 (rounding apart), on every element."""
+    det = detector
+    m_from = int(det.module_offset[4] + det.n_z[4] // 2)
+    m_to = int(det.module_offset[5] + det.n_z[5] // 2)
+    x0 = np.array([2.0, 10.0, 0.05, 1.35, -1.0 / 0.8, 3.0])
+    Js = []
+    for flag in (0, 1):
+        st = oracle.Setup(det, synth.uniform_field(), CKFSettings(field_gradient=flag))
+        code, xp, J = oracle.bound_to_bound(st, m_from, m_to, x0)
+        assert code == 0
+        Js.append(J)
+    assert np.allclose(Js[0], Js[1], rtol=1e-12, atol=1e-13)
+
+
+def test_grid_field_gradient_is_the_derivative_of_the_interpolant(detector):
+    """With the flag on in the float32 GRID field the Jacobian matches finite differences of the map through the same
+    trilinear interpolant, as long as no stage point changes its cell under the perturbation (one short move)."""
+    det = detector
+    m_from = int(det.module_offset[2] + 0 * det.n_z[2] + int(det.n_z[2] * 0.7))
+    m_to = int(det.module_offset[3] + 0 * det.n_z[3] + int(det.n_z[3] * 0.7))
+    x0 = np.array([1.0, 3.0, 0.02, 1.5, 1.0 / 0.9, 0.0])
+    kw = dict(rk_tolerance_mm=1e-9, surface_tolerance_mm=1e-11, max_rk_steps_per_surface=100000)
+    on = oracle.Setup(det, synth.grid_field(), CKFSettings(field_gradient=1, **kw))
+    code, xp, J = oracle.bound_to_bound(on, m_from, m_to, x0)
+    assert code == 0
+    Jfd = _fd_jacobian(on, m_from, m_to, x0)
+    scale = np.maximum(np.abs(Jfd), np.max(np.abs(Jfd), axis=1, keepdims=True) * 1e-3 + 1e-12)
+    assert np.max(np.abs(J - Jfd) / scale) < 5e-5
+
+
+def test_matrix_form_of_j2_equals_tangent_form_without_gradient_in_a_nonuniform_field(detector):
+    """The default Jacobian (J2, matrix form, gradient neglected) against the tangent form with G forced to zero (pin
+    hook field_gradient = 2) where B1 != B2 != B4: pins which field value each stage of the DEFAULT path uses through
+    the tangent form, which finite differences pin with the gradient on."""
+    det = detector
+    kw = dict(rk_tolerance_mm=1e-6, surface_tolerance_mm=1e-8)
+    for l0, qop in ((4, 1.0 / 0.7), (7, -1.0 / 0.6)):
+        m_from = int(det.module_offset[l0] + int(det.n_z[l0] * 0.8))
+        m_to = int(det.module_offset[l0 + 1] + int(det.n_z[l0 + 1] * 0.8))
+        x0 = np.array([2.0, 10.0, 0.03, 1.45, qop, 3.0])
+        Js = []
+        for flag in (0, 2):
+            st = oracle.Setup(det, _analytic_field_spec(), CKFSettings(field_gradient=flag, **kw))
+            code, _, J = oracle.bound_to_bound(st, m_from, m_to, x0)
+            assert code == 0
+            Js.append(J)
+        scale = np.maximum(np.abs(Js[1]), np.max(np.abs(Js[1]), axis=1, keepdims=True) * 1e-6 + 1e-14)
+        assert np.max(np.abs(Js[0] - Js[1]) / scale) < 1e-9
