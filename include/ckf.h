@@ -33,7 +33,7 @@
 extern "C" {
 #endif
 
-#define CKF_ABI_VERSION 7
+#define CKF_ABI_VERSION 8
 
 /* return codes */
 #define CKF_OK 0
@@ -77,6 +77,13 @@ typedef struct {
   const double* half_u;         /* [n_modules] mm                                    */
   const double* half_v;         /* [n_modules] mm                                    */
   const double* x_over_x0;      /* [n_modules]; 0 = no material                      */
+  /* Endcap discs ("barrel + endcaps").  Both NULL = barrel only.  Barrel layers
+   * come first, by increasing radius, the disc layers follow in any order.  For a disc layer l: layer_half_z[l] = signed
+   * z of its plane, layer_r_min[l] .. layer_r[l] its radial acceptance, n_z[l] = number of rings, module id =
+   * module_offset[l] + i_phi * n_z[l] + i_ring, ring pitch = 2 * half_v of the layer's first module; its modules lie in
+   * the plane with loc1 (axis_v) radial and the normal axis_u x axis_v pointing away from z = 0. */
+  const int32_t* layer_kind;    /* [n_layers] 0 barrel cylinder, 1 disc              */
+  const double* layer_r_min;    /* [n_layers] inner radius of a disc (barrel: unused) */
 } ckf_geometry;
 
 /* Magnetic field (north_star "magnetic-field store").  HOST pointers, copied during ckf_create.

@@ -24,7 +24,7 @@ _fp = C.POINTER(C.c_float)
 class OGeometry(C.Structure):
     _fields_ = [("n_layers", C.c_int32), ("layer_r", _dp), ("layer_half_z", _dp), ("n_phi", _ip), ("n_z", _ip),
                 ("module_offset", _ip), ("n_modules", C.c_int32), ("center", _dp), ("axis_u", _dp), ("axis_v", _dp),
-                ("half_u", _dp), ("half_v", _dp), ("x_over_x0", _dp)]
+                ("half_u", _dp), ("half_v", _dp), ("x_over_x0", _dp), ("layer_kind", _ip), ("layer_r_min", _dp)]
 
 
 class OField(C.Structure):
@@ -69,6 +69,7 @@ def lib():
         L.oracle_move.restype = C.c_int32
         L.oracle_move.argtypes = [C.POINTER(OGeometry), C.POINTER(OField), C.POINTER(OConfig), C.c_int32, _dp, _dp, _ip,
                                   _dp, _dp, _dp]
+        L.oracle_last_move_trials.restype = C.c_int64
         L.oracle_bound_to_bound.restype = C.c_int32
         L.oracle_bound_to_bound.argtypes = [C.POINTER(OGeometry), C.POINTER(OField), C.POINTER(OConfig), C.c_int32,
                                             C.c_int32, _dp, _dp, _dp]
@@ -127,6 +128,10 @@ class Setup:
             arr = conv(getattr(det, name))
             k.append(arr)
             setattr(g, name, _pd(arr) if conv is _d else _pi(arr))
+        if getattr(det, "layer_kind", None) is not None:      # endcap discs (row f3)
+            lk, rm = _i(det.layer_kind), _d(det.layer_r_min)
+            k.extend([lk, rm])
+            g.layer_kind, g.layer_r_min = _pi(lk), _pd(rm)
         f = OField()
         f.kind = int(fld.kind)
         for a in range(3):
@@ -227,6 +232,11 @@ def move(setup: Setup, module, x, Cov):
     st = lib().oracle_move(C.byref(setup.geometry), C.byref(setup.field), C.byref(setup.config), int(module), _pd(x),
                            _pd(Cov), C.byref(tg), _pd(xp), _pd(Cp), _pd(J))
     return st, tg.value, xp, Cp.reshape(6, 6), J.reshape(6, 6)
+
+
+def last_move_trials() -> int:
+    """RKN4 trials of this thread's last `move` (also of moves that ended in a stop)."""
+    return int(lib().oracle_last_move_trials())
 
 
 def bound_to_bound(setup: Setup, m_from, m_to, x):

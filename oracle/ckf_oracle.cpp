@@ -58,6 +58,11 @@ struct OGeometry {
   const double* half_u;
   const double* half_v;
   const double* x_over_x0;
+  // endcap discs (row f3; both NULL = barrel only).  Barrel layers come first, by increasing radius.  For a disc layer
+  // l: layer_half_z[l] = signed z of its plane, layer_r_min[l] .. layer_r[l] its radial acceptance, n_z[l] = rings,
+  // module id = module_offset[l] + i_phi * n_z[l] + i_ring, ring pitch = 2 * half_v of its modules.
+  const int32_t* layer_kind;   // [n_layers] 0 barrel cylinder, 1 disc
+  const double* layer_r_min;   // [n_layers]
 };
 
 struct OField {
@@ -728,35 +733,100 @@ int move_to_next_module(const OGeometry& g, const OField& fld, const OConfig& cf
   // N2: overlap neighbour on the same layer
   int tgt = pick_in_neighbourhood(g, m.layer, m.iphi, m.iz, m.id, y.r, y.d, 1e-3);
   if (tgt < 0) {
-    // N3: next layer's cylinder, then N4 module choice at the portal
-    int lp = m.layer + 1;
-    for (;;) {
-      if (lp >= g.n_layers) return STOP_EXIT;
-      Target cyl;
-      cyl.kind = 1;
-      cyl.R = g.layer_r[lp];
-      int st = propagate_to(fld, cfg, cyl, y, cnt);
-      if (st != STOP_NONE) return st;
-      if (std::fabs(y.r[2]) > g.layer_half_z[lp]) {
-        // N3 (reading D11): beyond the half-length of this layer AND of every further layer while moving
-        // away in z, the tip has left the barrel: EXIT now instead of walking the remaining portal cylinders.
-        bool gone = !g_n3_literal_walk && y.r[2] * y.d[2] > 0.0;
-        for (int l2 = lp + 1; gone && l2 < g.n_layers; ++l2) gone = std::fabs(y.r[2]) > g.layer_half_z[l2];
-        if (gone) return STOP_EXIT;
-        ++lp;
-        continue;
+    // N3': the next PORTAL -- the cylinder of the next barrel layer, or the plane of the next disc in the direction of
+    // d_z, whichever the straight line from here reaches first -- then N4 module choice on it.  Barrel only, this is
+    // SURVEY's N3 with reading D11; discs (row f3) add the second family of portals.
+    const bool has_discs = g.layer_kind != nullptr;
+    auto is_disc = [&](int l) { return has_discs && g.layer_kind[l] == 1; };
+    int n_barrel = 0;
+    while (n_barrel < g.n_layers && !is_disc(n_barrel)) ++n_barrel;
+    // next disc after disc layer `l` on its side (larger |z|), or the first disc ahead of z when l < 0
+    auto disc_after = [&](int l, double z, double dz) {
+      int best = -1;
+      for (int k = n_barrel; k < g.n_layers; ++k) {
+        const double zk = g.layer_half_z[k];
+        bool ahead;
+        if (l >= 0) ahead = (zk > 0.0) == (g.layer_half_z[l] > 0.0) && std::fabs(zk) > std::fabs(g.layer_half_z[l]);
+        else ahead = dz != 0.0 && (zk - z) * dz > 0.0;
+        if (ahead && (best < 0 || std::fabs(zk - z) < std::fabs(g.layer_half_z[best] - z))) best = k;
       }
+      return best;
+    };
+    int lb, ld;   // last barrel cylinder passed (the next one is lb + 1); next disc candidate (-1 = none)
+    if (is_disc(m.layer)) {
+      const double rho = std::hypot(y.r[0], y.r[1]);
+      lb = -1;
+      while (lb + 1 < n_barrel && g.layer_r[lb + 1] <= rho) ++lb;
+      ld = disc_after(m.layer, y.r[2], y.d[2]);
+    } else {
+      lb = m.layer;
+      ld = disc_after(-1, y.r[2], y.d[2]);
+    }
+    for (;;) {
+      // a barrel layer whose half length is already behind a tip that moves away in z cannot be crossed inside its
+      // acceptance: it is passed without propagating to it (reading D11, per layer)
+      while (!g_n3_literal_walk && lb + 1 < n_barrel && std::fabs(y.r[2]) > g.layer_half_z[lb + 1] &&
+             y.r[2] * y.d[2] > 0.0)
+        ++lb;
+      // likewise a disc whose plane is not ahead (any more), or whose outer radius is already behind a tip that moves
+      // outward radially, is passed
+      {
+        const double rho2 = y.r[0] * y.r[0] + y.r[1] * y.r[1], bxy = y.r[0] * y.d[0] + y.r[1] * y.d[1];
+        while (ld >= 0 && ((g.layer_half_z[ld] - y.r[2]) * y.d[2] <= 0.0 ||
+                           (rho2 > g.layer_r[ld] * g.layer_r[ld] && bxy > 0.0)))
+          ld = disc_after(ld, y.r[2], y.d[2]);
+      }
+      const int lc = lb + 1 < n_barrel ? lb + 1 : -1;
+      if (lc < 0 && ld < 0) return STOP_EXIT;
+      bool to_disc = false;
+      if (ld >= 0) {
+        const double s_d = (g.layer_half_z[ld] - y.r[2]) / y.d[2];
+        double s_c = INFINITY;   // straight-line distance to the cylinder (P4), infinite when it is not ahead
+        if (lc >= 0) {
+          const double a = y.d[0] * y.d[0] + y.d[1] * y.d[1], b = y.r[0] * y.d[0] + y.r[1] * y.d[1];
+          const double cc = y.r[0] * y.r[0] + y.r[1] * y.r[1] - g.layer_r[lc] * g.layer_r[lc];
+          const double disc = b * b - a * cc;
+          if (b > 0.0 && disc >= 0.0) s_c = -cc / (b + std::sqrt(disc));
+        }
+        to_disc = lc < 0 || s_d < s_c;   // tie -> the cylinder
+      }
+      int lp;
+      if (!to_disc) {
+        lp = lc;
+        Target cyl;
+        cyl.kind = 1;
+        cyl.R = g.layer_r[lp];
+        int st = propagate_to(fld, cfg, cyl, y, cnt);
+        if (st != STOP_NONE) return st;
+        lb = lp;
+        if (std::fabs(y.r[2]) > g.layer_half_z[lp]) continue;   // outside the layer's acceptance: on to the next portal
+      } else {
+        lp = ld;
+        Target pl;
+        pl.kind = 0;
+        pl.c[0] = 0.0; pl.c[1] = 0.0; pl.c[2] = g.layer_half_z[lp];
+        pl.n[0] = 0.0; pl.n[1] = 0.0; pl.n[2] = g.layer_half_z[lp] > 0.0 ? 1.0 : -1.0;
+        int st = propagate_to(fld, cfg, pl, y, cnt);
+        if (st != STOP_NONE) return st;
+        ld = disc_after(lp, y.r[2], y.d[2]);
+        const double rho = std::hypot(y.r[0], y.r[1]);
+        lb = -1;
+        while (lb + 1 < n_barrel && g.layer_r[lb + 1] <= rho) ++lb;
+        if (rho < g.layer_r_min[lp] || rho > g.layer_r[lp]) continue;   // outside the disc's acceptance
+      }
+      // N4: module choice at the portal point, 3x3 around its (phi, z) or (phi, ring) bin
       const int nphi = g.n_phi[lp], nz = g.n_z[lp];
       const double len = 2.0 * g.half_v[g.module_offset[lp]];
       const double phix = std::atan2(y.r[1], y.r[0]);
       int i = (int)std::nearbyint(phix * nphi / (2.0 * PI));
       i = ((i % nphi) + nphi) % nphi;
-      int j = (int)std::floor((y.r[2] + g.layer_half_z[lp]) / len);
+      const double along = is_disc(lp) ? std::hypot(y.r[0], y.r[1]) - g.layer_r_min[lp] : y.r[2] + g.layer_half_z[lp];
+      int j = (int)std::floor(along / len);
       if (j < 0) j = 0;
       if (j > nz - 1) j = nz - 1;
       tgt = pick_in_neighbourhood(g, lp, i, j, -1, y.r, y.d, -1e-3);
       if (tgt >= 0) break;
-      ++lp;  // a crack is not a hole
+      // a crack is not a hole: on to the next portal
     }
   }
   // N5: to the target's plane
@@ -1321,6 +1391,8 @@ void resolve_ambiguity(int n_tracks, const int32_t* offsets, const int32_t* meas
 
 }  // namespace
 
+thread_local long long g_last_move_trials = 0;
+
 // ====================================================================================== C interface
 extern "C" {
 
@@ -1536,12 +1608,16 @@ int32_t oracle_move(const OGeometry* g, const OField* f, const OConfig* cfg, int
   int tg = -1;
   int st = move_to_next_module(*g, *f, *cfg, from, x, Ci, tg, xp, Co, Jo, cnt);
   *target = tg;
+  g_last_move_trials = cnt.rk_trials;
   if (st == STOP_NONE) {
     std::memcpy(Cp, Co, sizeof(Co));
     if (J) std::memcpy(J, Jo, sizeof(Jo));
   }
   return st;
 }
+
+// RKN4 trials of the calling thread's last oracle_move (for the per-move comparison of the host-math test)
+int64_t oracle_last_move_trials(void) { return g_last_move_trials; }
 
 // Bound -> bound transport between two given modules, no navigation, no material (for the FD pin of J1-J5).
 int32_t oracle_bound_to_bound(const OGeometry* g, const OField* f, const OConfig* cfg, int32_t from, int32_t to,

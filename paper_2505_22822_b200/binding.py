@@ -28,7 +28,7 @@ EXPORTS = ("ckf_create", "ckf_find", "ckf_find_host", "ckf_fit", "ckf_get_counte
 class ckf_geometry(C.Structure):
     _fields_ = [("n_layers", C.c_int32), ("layer_r", _dp), ("layer_half_z", _dp), ("n_phi", _ip), ("n_z", _ip),
                 ("module_offset", _ip), ("n_modules", C.c_int32), ("center", _dp), ("axis_u", _dp), ("axis_v", _dp),
-                ("half_u", _dp), ("half_v", _dp), ("x_over_x0", _dp)]
+                ("half_u", _dp), ("half_v", _dp), ("x_over_x0", _dp), ("layer_kind", _ip), ("layer_r_min", _dp)]
 
 
 class ckf_field(C.Structure):
@@ -141,6 +141,10 @@ def make_geometry(det, keep: list) -> ckf_geometry:
         arr = conv(getattr(det, name))
         keep.append(arr)
         setattr(g, name, arr.ctypes.data_as(pt))
+    if getattr(det, "layer_kind", None) is not None:      # endcap discs
+        lk, rm = _i(det.layer_kind), _d(det.layer_r_min)
+        keep.extend([lk, rm])
+        g.layer_kind, g.layer_r_min = lk.ctypes.data_as(_ip), rm.ctypes.data_as(_dp)
     return g
 
 

@@ -83,6 +83,7 @@ struct ckf_handle {
   int n_modules = 0, n_layers = 0;
   ModuleRec* d_mod = nullptr;
   LayerRec* d_layer = nullptr;
+  GeoDev geo;   // device pointers + layer summary (barrel count, first discs)
   double* d_grid = nullptr;
   FieldDev fld;
   CfgDev kcfg;
@@ -155,7 +156,7 @@ template <> struct VisitBlocks<double> { static constexpr int value = 2; };
 template <typename T>
 void fill_params(ckf_handle* h, Workspace& w, KParams<T>& p) {
   const ckf_config& c = h->cfg;
-  p.geo.mod = h->d_mod; p.geo.layer = h->d_layer; p.geo.n_layers = h->n_layers; p.geo.n_modules = h->n_modules;
+  p.geo = h->geo;
   p.fld = h->fld;
   p.cfg = h->kcfg;
   p.max_links = c.max_links;
@@ -253,7 +254,7 @@ template <typename T>
 int launch_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, const ckf_tracks* t, ckf_fits* o,
                cudaStream_t st) {
   FitParams<T> p;
-  p.geo.mod = h->d_mod; p.geo.layer = h->d_layer; p.geo.n_layers = h->n_layers; p.geo.n_modules = h->n_modules;
+  p.geo = h->geo;
   p.fld = h->fld;
   p.cfg = h->kcfg;
   p.moff = m->module_offsets;
@@ -373,6 +374,21 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     return fail(h, CKF_E_ARG, "field grid needs >= 2 nodes per axis");
   for (int l = 0; l < g->n_layers; ++l)
     if (g->n_phi[l] < 3 || g->n_z[l] < 1) return fail(h, CKF_E_ARG, "layer %d: n_phi >= 3 and n_z >= 1 required", l);
+  if (g->layer_kind) {   // row f3: barrel layers first, by increasing radius, then the discs
+    bool disc_seen = false;
+    for (int l = 0; l < g->n_layers; ++l) {
+      const int k = g->layer_kind[l];
+      if (k != 0 && k != 1) return fail(h, CKF_E_ARG, "layer %d: kind must be 0 (barrel) or 1 (disc)", l);
+      if (k == 1) disc_seen = true;
+      else if (disc_seen) return fail(h, CKF_E_ARG, "barrel layers must precede the disc layers");
+      if (k == 1 && (!g->layer_r_min || !(g->layer_r_min[l] >= 0.0) || !(g->layer_r_min[l] < g->layer_r[l]) || g->layer_half_z[l] == 0.0))
+        return fail(h, CKF_E_ARG, "disc layer %d: needs 0 <= r_min < r and a plane z != 0", l);
+    }
+  }
+  for (int l = 1; l < g->n_layers; ++l)
+    if ((!g->layer_kind || (g->layer_kind[l] == 0 && g->layer_kind[l - 1] == 0)) && !(g->layer_r[l] > g->layer_r[l - 1]))
+      return fail(h, CKF_E_ARG, "barrel layer radii must increase");
+  if (g->layer_kind && g->layer_kind[0] != 0) return fail(h, CKF_E_ARG, "the first layer must be a barrel layer");
 
   int ndev = 0;
   if (cudaGetDeviceCount(&ndev) != cudaSuccess || ndev < 1)
@@ -409,6 +425,8 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
   CKB(dalloc(h, &h->d_layer, layers.size() * sizeof(LayerRec)));
   CKB(cudaMemcpy(h->d_mod, mods.data(), mods.size() * sizeof(ModuleRec), cudaMemcpyHostToDevice));
   CKB(cudaMemcpy(h->d_layer, layers.data(), layers.size() * sizeof(LayerRec), cudaMemcpyHostToDevice));
+  h->geo.mod = h->d_mod; h->geo.layer = h->d_layer; h->geo.n_layers = g->n_layers; h->geo.n_modules = g->n_modules;
+  fill_geo_summary(layers, h->geo);
   // ---- a2 field store
   std::memset(&h->fld, 0, sizeof(h->fld));
   h->fld.kind = f->kind;

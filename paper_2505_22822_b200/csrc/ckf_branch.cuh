@@ -170,10 +170,17 @@ __device__ __forceinline__ int find_parent(const KParams<T>& p, int n, int nb, i
 __device__ __forceinline__ int step_cost_bin(const GeoDev& g, int module, const Traj& y, int overlap) {
   if (overlap >= 0) return 0;  // same-layer neighbour: one or two short trials
   const int L = g.mod[module].layer;
-  if (L + 1 >= g.n_layers) return 0;  // leaves the barrel at once
+  const LayerRec LR = g.layer[L];
   const float st = sqrtf((float)(y.d[0] * y.d[0] + y.d[1] * y.d[1]));
-  const float gap = (float)(g.layer[L + 1].r - g.layer[L].r);
-  const float pred = 0.2565f * __powf(gap / st, 0.713f) * __powf(0.6f * fabsf((float)y.qop) / st, 0.266f);
+  float path;  // rough length of the move: to the next cylinder, or from a disc to the next disc of its side
+  if (LR.kind == 0) {
+    if (L + 1 >= g.n_barrel) return 0;  // leaves the barrel at once
+    path = (float)(g.layer[L + 1].r - LR.r) / st;
+  } else {
+    if (LR.next_disc < 0) return 0;
+    path = fabsf((float)(g.layer[LR.next_disc].half_z - LR.half_z)) / fmaxf(fabsf((float)y.d[2]), 0.05f);
+  }
+  const float pred = 0.2565f * __powf(path, 0.713f) * __powf(0.6f * fabsf((float)y.qop) / st, 0.266f);
   const int b = (int)(pred * ((float)NBIN / 16.0f));  // NBIN / 16 classes per predicted trial
   return b < 1 ? 1 : (b > NBIN - 1 ? NBIN - 1 : b);
 }

@@ -1,9 +1,10 @@
 // ckf_host_geom.h — host-side packing of ckf_geometry into the device geometry store (a1).
 #pragma once
+#include <cmath>
 #include <vector>
 
 #include "../../include/ckf.h"
-#include "ckf_math.cuh"
+#include "ckf_nav.cuh"
 
 namespace ckf {
 
@@ -18,6 +19,19 @@ inline void build_geometry_records(const ckf_geometry& g, std::vector<ModuleRec>
     L.offset = g.module_offset[l];
     L.len_z = 2.0 * g.half_v[g.module_offset[l]];
     L.pad = 0;
+    L.kind = g.layer_kind ? g.layer_kind[l] : 0;
+    L.r_min = (g.layer_kind && g.layer_r_min) ? g.layer_r_min[l] : 0.0;
+    L.next_disc = -1;
+  }
+  // next disc of the same side: the one with the smallest |z| beyond this disc's
+  for (int l = 0; l < g.n_layers; ++l) {
+    if (layers[l].kind != 1) continue;
+    for (int k = 0; k < g.n_layers; ++k) {
+      if (layers[k].kind != 1 || (layers[k].half_z > 0.0) != (layers[l].half_z > 0.0)) continue;
+      if (!(std::fabs(layers[k].half_z) > std::fabs(layers[l].half_z))) continue;
+      if (layers[l].next_disc < 0 || std::fabs(layers[k].half_z) < std::fabs(layers[layers[l].next_disc].half_z))
+        layers[l].next_disc = k;
+    }
   }
   mods.resize(g.n_modules);
   int l = 0;
@@ -37,6 +51,19 @@ inline void build_geometry_records(const ckf_geometry& g, std::vector<ModuleRec>
     m.xx0 = g.x_over_x0[id];
     m.layer = l;
     m.iphi = (id - g.module_offset[l]) / g.n_z[l];
+  }
+}
+
+// barrel layers first (n_barrel of them), innermost disc of each side
+inline void fill_geo_summary(const std::vector<LayerRec>& layers, GeoDev& geo) {
+  geo.n_barrel = 0;
+  while (geo.n_barrel < (int)layers.size() && layers[geo.n_barrel].kind == 0) ++geo.n_barrel;
+  geo.first_disc[0] = geo.first_disc[1] = -1;
+  for (int l = 0; l < (int)layers.size(); ++l) {
+    if (layers[l].kind != 1) continue;
+    const int side = layers[l].half_z > 0.0 ? 0 : 1;
+    if (geo.first_disc[side] < 0 || std::fabs(layers[l].half_z) < std::fabs(layers[geo.first_disc[side]].half_z))
+      geo.first_disc[side] = l;
   }
 }
 

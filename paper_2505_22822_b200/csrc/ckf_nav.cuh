@@ -9,6 +9,8 @@ struct GeoDev {
   const ModuleRec* mod;
   const LayerRec* layer;
   int32_t n_layers, n_modules;
+  int32_t n_barrel;        // barrel layers come first, by increasing radius; disc layers follow
+  int32_t first_disc[2];   // innermost disc of the +z side, of the -z side (-1 = none)
 };
 
 constexpr int NDEP = 6;  // numbers of a departure record (departure_state): direction[3], q_phi, q_theta, g
@@ -285,7 +287,10 @@ CKF_HD void kalman_update(const double x[6], const double C[21], M m0, M m1, M v
 //                                                   beyond every further layer's half length = EXIT (D11)
 //   PLANE --step--> PLANE (one trial) | FIN          N5 toward the target module's plane
 //   FIN   --arrive-> predicted bound parameters + 5x5 Jacobian block (J4, J5)
-enum MovePhase : int { PH_IDLE = 0, PH_START = 1, PH_CYL = 2, PH_LANDED = 3, PH_PLANE = 4, PH_FIN = 5 };
+//   DISC  --step--> DISC | LANDED                   like CYL toward the plane of a disc layer (row f3)
+enum MovePhase : int { PH_IDLE = 0, PH_START = 1, PH_CYL = 2, PH_LANDED = 3, PH_PLANE = 4, PH_FIN = 5, PH_DISC = 6 };
+
+CKF_HD bool is_stepping(int phase) { return phase == PH_CYL || phase == PH_PLANE || phase == PH_DISC; }
 
 template <typename T>
 struct Move {
@@ -297,6 +302,7 @@ struct Move {
   double ib, dib;       // 1/beta and d(1/beta)/d(q/p): constant along the move (no energy loss)
   double B1[3];         // field at y.r, valid while `targeted` (read once per position, see move_target)
   int phase, stop, from, tgt, lp, n_steps;
+  int lb, ld;           // portals (N3'): last barrel cylinder passed (the next is lb + 1); next disc candidate, -1 none
   bool targeted;        // the next trial's length m.h and B1 are set (P4 done for the current position)
 };
 
@@ -346,7 +352,7 @@ CKF_HD int departure_state(const GeoDev& g, const CfgDev& cfg, int from, const d
 // Start of a move whose m.y holds the departure state: identity transport, fresh step control (P4, J3).
 template <typename T>
 CKF_HD void move_begin(Move<T>& m, const CfgDev& cfg, int from) {
-  m.from = from; m.tgt = -1; m.lp = 0; m.n_steps = 0; m.targeted = false; m.stop = STOP_NONE;
+  m.from = from; m.tgt = -1; m.lp = 0; m.lb = -1; m.ld = -1; m.n_steps = 0; m.targeted = false; m.stop = STOP_NONE;
   m.h = 0.0; m.h_ctrl = cfg.h_max; m.R = 0.0;
   jac_identity(m.D);
   m.ib = inv_beta(m.y.qop, cfg.mass);
@@ -367,12 +373,17 @@ CKF_HD int overlap_neighbour(const GeoDev& g, int from, const double r[3], const
   return pick_in_neighbourhood(g, k.layer, k.iphi, iz, from, r, d, 1e-3);
 }
 
-// What a move in PH_START / PH_LANDED needs next: PICK_TEST (test the 3x3 neighbourhood in q), PICK_SKIP (portal
-// point beyond the layer's half length: go on to the next layer), PICK_EXIT (beyond the half length of this and
-// every further layer and moving away in z: the tip has left the barrel, reading D11).
-enum PickWhat : int { PICK_TEST = 1, PICK_SKIP = 0, PICK_EXIT = -1 };
+// What a move in PH_START / PH_LANDED needs next: PICK_TEST (test the 3x3 neighbourhood in q) or PICK_SKIP (the portal
+// point lies outside the layer's acceptance: on to the next portal).  For a move that has just LANDED on a portal this
+// also books the landing: the cylinder is passed (lb), the next disc of the side becomes the candidate (ld).
+enum PickWhat : int { PICK_TEST = 1, PICK_SKIP = 0 };
+CKF_HD int barrel_index_inside(const GeoDev& g, double rho) {   // last barrel layer with r <= rho, -1 if none
+  int lb = -1;
+  while (lb + 1 < g.n_barrel && g.layer[lb + 1].r <= rho) ++lb;
+  return lb;
+}
 template <typename T>
-CKF_HD int move_pick_request(const Move<T>& m, const GeoDev& g, PickRequest& q) {
+CKF_HD int move_pick_request(Move<T>& m, const GeoDev& g, PickRequest& q) {
   if (m.phase == PH_START) {
     const ModuleRec& k = g.mod[m.from];
     q.layer = k.layer; q.iphi = k.iphi;
@@ -382,23 +393,79 @@ CKF_HD int move_pick_request(const Move<T>& m, const GeoDev& g, PickRequest& q) 
   }
   const LayerRec L = g.layer[m.lp];
   q.layer = m.lp; q.exclude = -1; q.s_min = -1e-3; q.iphi = 0; q.iz = 0;
-  if (fabs(m.y.r[2]) > L.half_z) {
-    bool gone = m.y.r[2] * m.y.d[2] > 0.0;
-    for (int l2 = m.lp + 1; gone && l2 < g.n_layers; ++l2) gone = fabs(m.y.r[2]) > g.layer[l2].half_z;
-    return gone ? PICK_EXIT : PICK_SKIP;
+  double along;
+  if (L.kind == 0) {
+    m.lb = m.lp;
+    if (fabs(m.y.r[2]) > L.half_z) return PICK_SKIP;
+    along = m.y.r[2] + L.half_z;
+  } else {
+    const double rho = sqrt(m.y.r[0] * m.y.r[0] + m.y.r[1] * m.y.r[1]);
+    m.ld = L.next_disc;
+    m.lb = barrel_index_inside(g, rho);
+    if (rho < L.r_min || rho > L.r) return PICK_SKIP;
+    along = rho - L.r_min;
   }
   const double phix = atan2(m.y.r[1], m.y.r[0]);
   const int i = (int)nearbyint(phix * L.n_phi / (2.0 * PI_D));
   q.iphi = ((i % L.n_phi) + L.n_phi) % L.n_phi;
-  const int j = (int)floor((m.y.r[2] + L.half_z) / L.len_z);
+  const int j = (int)floor(along / L.len_z);
   q.iz = j < 0 ? 0 : (j > L.n_z - 1 ? L.n_z - 1 : j);
   return PICK_TEST;
 }
 
+// N3': the next PORTAL of a move that has no module to go to -- the cylinder of the next barrel layer or the plane of
+// the next disc in the direction of d_z, whichever the straight line from here reaches first (tie -> the cylinder).
+// A barrel layer whose half length is already behind a tip that moves away in z, and a disc whose plane is not ahead
+// or whose outer radius is behind a tip that moves outward radially, are passed without propagating to them (reading
+// D11, per layer).  No portal left = the tip has left the detector (EXIT).
+template <typename T>
+CKF_HD void choose_portal(Move<T>& m, const GeoDev& g) {
+  const double z = m.y.r[2], dz = m.y.d[2];
+  const double rho2 = m.y.r[0] * m.y.r[0] + m.y.r[1] * m.y.r[1], bxy = m.y.r[0] * m.y.d[0] + m.y.r[1] * m.y.d[1];
+  if (m.phase == PH_START) {   // leaving a module: where the tip stands in the two families of portals
+    const LayerRec L0 = g.layer[g.mod[m.from].layer];
+    if (L0.kind == 0) {
+      m.lb = g.mod[m.from].layer;
+      m.ld = dz > 0.0 ? g.first_disc[0] : (dz < 0.0 ? g.first_disc[1] : -1);
+    } else {
+      m.lb = barrel_index_inside(g, sqrt(rho2));
+      m.ld = L0.next_disc;
+    }
+  }
+  while (m.lb + 1 < g.n_barrel && fabs(z) > g.layer[m.lb + 1].half_z && z * dz > 0.0) ++m.lb;
+  while (m.ld >= 0 && ((g.layer[m.ld].half_z - z) * dz <= 0.0 || (rho2 > g.layer[m.ld].r * g.layer[m.ld].r && bxy > 0.0)))
+    m.ld = g.layer[m.ld].next_disc;
+  const int lc = m.lb + 1 < g.n_barrel ? m.lb + 1 : -1;
+  if (lc < 0 && m.ld < 0) { m.stop = STOP_EXIT; m.phase = PH_FIN; return; }
+  bool to_disc = false;
+  if (m.ld >= 0) {
+    const double s_d = (g.layer[m.ld].half_z - z) / dz;
+    double s_c = INFINITY;
+    if (lc >= 0) {
+      const double a = m.y.d[0] * m.y.d[0] + m.y.d[1] * m.y.d[1];
+      const double cc = rho2 - g.layer[lc].r * g.layer[lc].r;
+      const double disc = bxy * bxy - a * cc;
+      if (bxy > 0.0 && disc >= 0.0) s_c = -cc / (bxy + sqrt(disc));
+    }
+    to_disc = lc < 0 || s_d < s_c;
+  }
+  m.targeted = false;
+  if (!to_disc) {
+    m.lp = lc;
+    m.R = g.layer[lc].r;
+    m.phase = PH_CYL;
+  } else {
+    m.lp = m.ld;
+    const double zd = g.layer[m.ld].half_z;
+    m.tc[0] = 0.0; m.tc[1] = 0.0; m.tc[2] = zd;
+    m.tn[0] = 0.0; m.tn[1] = 0.0; m.tn[2] = zd > 0.0 ? 1.0 : -1.0;
+    m.phase = PH_DISC;
+  }
+}
+
 // Result of the pick (module id or -1) -> next phase.
 template <typename T>
-CKF_HD void move_pick_apply(Move<T>& m, const GeoDev& g, int tgt, bool exit_now = false) {
-  if (exit_now) { m.stop = STOP_EXIT; m.phase = PH_FIN; return; }
+CKF_HD void move_pick_apply(Move<T>& m, const GeoDev& g, int tgt) {
   if (tgt >= 0) {
     const ModuleRec& k = g.mod[tgt];
 #pragma unroll
@@ -407,17 +474,14 @@ CKF_HD void move_pick_apply(Move<T>& m, const GeoDev& g, int tgt, bool exit_now 
     m.phase = PH_PLANE;
     return;
   }
-  m.lp = (m.phase == PH_START) ? g.mod[m.from].layer + 1 : m.lp + 1;
-  if (m.lp >= g.n_layers) { m.stop = STOP_EXIT; m.phase = PH_FIN; return; }
-  m.R = g.layer[m.lp].r;
-  m.phase = PH_CYL;
+  choose_portal(m, g);   // no module here (no overlap neighbour / outside the acceptance / a crack): the next portal
 }
 
 // P4: signed straight-line distance from the move's position to its target (plane or cylinder) along d.
 // Returns STOP_NONE and s, or the stop reason (P6).
 template <typename T>
 CKF_HD int target_distance(const Move<T>& m, double& s) {
-  if (m.phase == PH_PLANE) {
+  if (m.phase == PH_PLANE || m.phase == PH_DISC) {
     const double dn = dot3(m.y.d, m.tn);
     if (!(fabs(dn) > 1e-12)) return STOP_NUMERIC;
     const double rel[3] = {m.tc[0] - m.y.r[0], m.tc[1] - m.y.r[1], m.tc[2] - m.y.r[2]};
@@ -529,7 +593,7 @@ CKF_HD int move_to_next_module(const GeoDev& g, const FieldDev& fld, const CfgDe
       PickRequest q;
       const int what = move_pick_request(m, g, q);
       const int tgt = what == PICK_TEST ? pick_in_neighbourhood(g, q.layer, q.iphi, q.iz, q.exclude, m.y.r, m.y.d, q.s_min) : -1;
-      move_pick_apply(m, g, tgt, what == PICK_EXIT);
+      move_pick_apply(m, g, tgt);
     } else {
       move_step(m, fld, cfg, sc.n_trials, sc.n_accepted);
     }

@@ -88,7 +88,7 @@ __device__ __forceinline__ void pick_warp(const GeoDev& geo, const PickSmem& ps,
         if (sv == sv && (best < 0 || sv < best_s || (sv == best_s && id < best))) { best = id; best_s = sv; }
       }
     }
-    move_pick_apply(m, geo, best, what == PICK_EXIT);
+    move_pick_apply(m, geo, best);
   }
   __syncwarp();
 }
@@ -111,7 +111,7 @@ __global__ void __launch_bounds__(STEP_NT, MINB) ckf_step(const KParams<T> p, in
   const size_t TC = (size_t)p.tcap;
 
   Move<T> m;
-  m.phase = PH_IDLE; m.stop = STOP_NONE; m.from = 0; m.tgt = -1; m.lp = 0; m.n_steps = 0; m.targeted = false;
+  m.phase = PH_IDLE; m.stop = STOP_NONE; m.from = 0; m.tgt = -1; m.lp = 0; m.lb = -1; m.ld = -1; m.n_steps = 0; m.targeted = false;
   m.B1[0] = m.B1[1] = m.B1[2] = 0.0;
   m.h = 0.0; m.h_ctrl = 0.0; m.R = 0.0; m.y.qop = 0.0; m.ib = 0.0; m.dib = 0.0;
   int tip = -1, nt = 0, na = 0;
@@ -119,7 +119,7 @@ __global__ void __launch_bounds__(STEP_NT, MINB) ckf_step(const KParams<T> p, in
   for (;;) {
     const unsigned bI = __ballot_sync(0xffffffffu, m.phase == PH_IDLE);
     const unsigned bP = __ballot_sync(0xffffffffu, m.phase == PH_START || m.phase == PH_LANDED);
-    const unsigned bS = __ballot_sync(0xffffffffu, m.phase == PH_CYL || m.phase == PH_PLANE);
+    const unsigned bS = __ballot_sync(0xffffffffu, is_stepping(m.phase));
     const unsigned bF = __ballot_sync(0xffffffffu, m.phase == PH_FIN);
     if (!bP && !bS && !bF && !more) break;
     const int waiting = __popc(bF) + (more ? __popc(bI) : 0);
@@ -158,12 +158,12 @@ __global__ void __launch_bounds__(STEP_NT, MINB) ckf_step(const KParams<T> p, in
       // ---- module choice at the portal (N3, N4) once enough lanes need one
       {
         const unsigned need = __ballot_sync(0xffffffffu, m.phase == PH_START || m.phase == PH_LANDED);
-        const unsigned step = __ballot_sync(0xffffffffu, m.phase == PH_CYL || m.phase == PH_PLANE);
+        const unsigned step = __ballot_sync(0xffffffffu, is_stepping(m.phase));
         if (need && (step == 0u || __popc(need) >= PICK_MIN)) pick_warp<T>(p.geo, ps, m, lane);
       }
     }
     // ---- one step: targeting + landing, else one RKN4 trial
-    if (m.phase == PH_CYL || m.phase == PH_PLANE) move_step<T>(m, p.fld, p.cfg, nt, na);
+    if (is_stepping(m.phase)) move_step<T>(m, p.fld, p.cfg, nt, na);
     __syncwarp();
   }
   flush_counter(p.counters + CNT_TRIALS, (unsigned long long)nt);

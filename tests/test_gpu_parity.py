@@ -764,3 +764,57 @@ def test_energy_loss_parity(config):
         tol = 1e-9 if cfg.precision == 64 else 1e-5
         assert rf["n_not_pd_gpu_only"] == 0 and rf["max_smoothed_rel"] < tol and rf["max_last_rel"] < tol, (smoother, rf)
     ckf.close()
+
+
+ENDCAP_DISC_Z = (560.0, 640.0, 740.0, 860.0, 1000.0)
+
+
+@pytest.mark.parametrize("precision,inhom", [(64, False), (32, True)])
+def test_endcap_discs_parity(precision, inhom):
+    """Row f3: a barrel closed by endcap discs, particles up to |eta| = 3, noise and fake seeds:
+    ckf_find, ckf_fit and ckf_resolve against the oracle.  fp64 in the uniform field, fp32 through the float32 grid
+    (barrel half length 500 mm and discs up to |z| = 1000 mm stay inside the grid of configs[2])."""
+    import torch
+    import oracle
+    from paper_2505_22822_b200 import CKF
+    from synth.events import CKFSettings
+    det = synth.build_detector(half_z=500.0, disc_z=ENDCAP_DISC_Z)
+    fld = synth.grid_field() if inhom else synth.uniform_field()
+    ckfs = CKFSettings(max_branches_per_surface=5, max_candidates_per_seed=50,
+                       surface_tolerance_mm=1e-5 if precision == 64 else 1e-2)
+    ev = synth.make_endcap_event(det, 6000, seed=21 + precision, n_fake_seeds=600, inhomogeneous=inhom, precision=precision)
+    ora = oracle.find_event(oracle.Setup(det, fld, ckfs), ev, n_threads=8)
+    ckf = CKF(det, fld, ckfs, precision, max_seeds=ev.n_seeds, max_measurements=ev.n_measurements)
+    dev, out = ckf.upload_event(ev), ckf.alloc_tracks()
+    ckf.find(dev, out)
+    torch.cuda.synchronize()
+    gpu = ckf.download(out)
+    cnt = ckf.counters()
+    assert gpu.status == 0 and gpu.n_tracks > 6000
+    lay = det.layer_kind[det.module_layer[gpu.last_module]]
+    assert 0.3 < lay.mean() < 0.9                       # many candidates end on a disc, many in the barrel
+    if precision == 64:
+        parity.assert_bit_exact_lists(gpu, ora)
+        rel, chi2, cov = parity.max_param_diffs(gpu, ora)
+        assert rel < 1e-9 and chi2 < 1e-8 and cov < 1e-7, (rel, chi2, cov)
+        for k in ("visits", "rk_trials", "rk_accepted", "gate_tests", "updates", "tips"):
+            assert cnt[k] == ora.counters[k], (k, cnt[k], ora.counters[k])
+    else:
+        r = parity.assert_fp32_parity(gpu, ora, ev.n_seeds, ckfs.chi2_max, "endcap fp32")
+        print("endcap fp32", {k: v for k, v in r.items() if k != "bad_seeds"})
+    fits = ckf.alloc_fits()
+    ckf.fit(dev, out, fits)
+    torch.cuda.synchronize()
+    g = ckf.download_fits(fits, gpu.n_tracks, int(gpu.meas_idx.size))
+    o = oracle.kf_fit(oracle.Setup(det, fld, ckfs), ev, gpu.track_offsets, gpu.meas_idx, gpu.seed_id, n_threads=8)
+    rf = parity.compare_fits(g, o, gpu.track_offsets)
+    assert rf["n_not_pd_gpu_only"] == 0 and rf["max_smoothed_rel"] < (1e-9 if precision == 64 else 1e-5), rf
+    res = ckf.alloc_resolution()
+    ckf.resolve(out, ev.n_measurements, res, 1, 1.0)
+    torch.cuda.synchronize()
+    chi2 = out["chi2_sum"][:gpu.n_tracks].cpu().numpy().astype(np.float64)
+    o_acc, _ = oracle.resolve_ambiguity(gpu.track_offsets, gpu.meas_idx, chi2, ev.n_measurements, 1, 1.0)
+    assert np.array_equal(res["accepted"][:gpu.n_tracks].cpu().numpy(), o_acc)
+    print("endcap precision %d: %d seeds -> %d candidates (%d kept), fit %d" %
+          (precision, ev.n_seeds, gpu.n_tracks, int(o_acc.sum()), rf["n_fitted"]))
+    ckf.close()

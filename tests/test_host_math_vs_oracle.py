@@ -73,3 +73,40 @@ def test_field_read_matches_oracle():
     for _ in range(300):
         r = rng.uniform(-1090, 1090, 3)
         assert np.max(np.abs(oracle.field_at(st, r) - hm.field(r))) < 1e-12
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_moves_with_endcap_discs_match_oracle(precision):
+    """Row f3: barrel -> disc -> disc navigation (N3' portals) of the CUDA path's per-tip code against the oracle, move by
+    move along the truth of forward and central particles (|eta| up to 3)."""
+    from synth.events import CKFSettings
+    det = synth.build_detector(half_z=500.0, disc_z=(560.0, 640.0, 740.0, 860.0, 1000.0))
+    fld = synth.uniform_field()
+    ev = synth.make_endcap_event(det, 150, seed=11, noise_fraction=0.0)
+    ckf = CKFSettings(surface_tolerance_mm=1e-5 if precision == 64 else 1e-2)
+    st = oracle.Setup(det, fld, ckf)
+    hm = HostMath(det, fld, ckf)
+    floor_x = np.array([1.0, 1.0, 1.0, 1.0, 0.0, 1.0])
+    n_moves = n_disc = n_exit = 0
+    for s in range(ev.n_seeds):
+        x = ev.seed_params[s].astype(np.float64)
+        Cm = ev.seed_cov[s].reshape(6, 6).astype(np.float64)
+        m = int(ev.seed_module[s])
+        for level in range(30):
+            co, tgo, xo, Co, _ = oracle.move(st, m, x, Cm)
+            ch, tgh, xh, Ch, trials = hm.move(precision, m, x, Cm)
+            assert co == ch, (s, level, co, ch)
+            assert trials == oracle.last_move_trials(), (s, level)     # same sequence of RKN4 trials, stops included
+            if co != 0:
+                n_exit += oracle.STOP_NAMES[co] == "EXIT"
+                break
+            assert tgo == tgh, (s, level, tgo, tgh)
+            fl = floor_x.copy()
+            fl[4] = abs(xo[4])
+            assert np.max(_rel(xo, xh, fl)) < (1e-10 if precision == 64 else 1e-9)
+            scale = np.sqrt(np.outer(np.diag(Co), np.diag(Co)))
+            assert np.max(np.abs(Co - Ch) / scale) < (1e-9 if precision == 64 else 2e-6)
+            n_moves += 1
+            n_disc += int(det.layer_kind[det.module_layer[tgo]])
+            x, Cm, m = xo, Co, tgo
+    assert n_moves > 900 and n_disc > 300 and n_exit > 100
