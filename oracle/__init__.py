@@ -37,7 +37,7 @@ class OConfig(C.Structure):
                 ("max_candidates_per_seed", C.c_int32), ("max_holes", C.c_int32), ("min_measurements", C.c_int32),
                 ("rk_tolerance_mm", C.c_double), ("surface_tolerance_mm", C.c_double), ("h_max_mm", C.c_double),
                 ("particle_mass_gev", C.c_double), ("max_rk_steps_per_surface", C.c_int32), ("max_levels", C.c_int32),
-                ("energy_loss", C.c_int32), ("field_gradient", C.c_int32)]
+                ("energy_loss", C.c_int32), ("field_gradient", C.c_int32), ("bidirectional", C.c_int32)]
 
 
 STOP_NAMES = {0: "NONE", 1: "EXIT", 2: "HOLES", 3: "NOT_OUTGOING", 4: "STEP_LIMIT", 5: "NUMERIC", 6: "LEVEL_LIMIT"}

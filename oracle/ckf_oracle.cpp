@@ -88,6 +88,8 @@ struct OConfig {
   int32_t max_levels;
   int32_t energy_loss;      // 1: mean energy loss of rule E in every crossed module (0 = BASELINE configs: "no energy loss")
   int32_t field_gradient;   // 1: transport Jacobian with the field-gradient terms of PAPER.md ref [18] (reading A13; 0 = ref [17])
+  int32_t bidirectional;    // 1: tips that move radially INWARD are navigated too (rules N3'' below); 0 = reading A7:
+                            //    outward-only, such tips stop NOT_OUTGOING (BASELINE configs)
 };
 
 enum StopReason { STOP_NONE = 0, STOP_EXIT = 1, STOP_HOLES = 2, STOP_NOT_OUTGOING = 3, STOP_STEP_LIMIT = 4,
@@ -429,7 +431,8 @@ void straight_close(FreeState& y, double s, double mass) {
 }
 
 struct Target {
-  int kind;      // 0 plane (c, n), 1 cylinder radius R around z
+  int kind;      // 0 plane (c, n); cylinder of radius R around z: 1 crossed outward, 2 crossed INWARD from outside,
+                 // 3 FAR crossing (the tip is inside or on it and leaves through its far side)
   double c[3], n[3], R;
 };
 
@@ -446,6 +449,20 @@ bool target_distance(const Target& tg, const FreeState& y, double& s, int& why) 
   const double b = y.r[0] * y.d[0] + y.r[1] * y.d[1];
   const double cc = y.r[0] * y.r[0] + y.r[1] * y.r[1] - tg.R * tg.R;
   const double disc = b * b - a * cc;
+  if (tg.kind == 2) {
+    // N3'': the cylinder is inside the tip's radius and the tip moves inward: near root of a s^2 + 2 b s + cc = 0,
+    // s = cc / (-b + sqrt(disc)) (signed: negative once the tip has overshot to the inside)
+    if (!(b < 0.0) || !(disc >= 0.0)) { why = STOP_NOT_OUTGOING; return false; }   // it turned before reaching it
+    s = cc / (-b + std::sqrt(disc));
+    return true;
+  }
+  if (tg.kind == 3) {
+    // N3'': far root (-b + sqrt(disc)) / a, written without cancellation for either sign of b
+    if (!(disc >= 0.0)) { why = STOP_NOT_OUTGOING; return false; }
+    const double sq = std::sqrt(disc);
+    s = b < 0.0 ? (-b + sq) / a : -cc / (b + sq);
+    return true;
+  }
   if (!(b > 0.0) || !(disc >= 0.0)) { why = STOP_NOT_OUTGOING; return false; }
   s = -cc / (b + std::sqrt(disc));
   return true;
@@ -674,9 +691,11 @@ double energy_loss(const OConfig& cfg, const Module& m, const double x[6], doubl
 int g_n3_literal_walk = 0;
 
 // straight-line test of one module from the point (r, d): N2 / N4
+// (g_bidirectional, set per call from config.bidirectional: a module may also be crossed AGAINST its normal)
+thread_local int g_bidirectional = 0;
 bool line_hits_module(const Module& k, const double r[3], const double d[3], double s_min, double& s_out) {
   const double dn = dot(d, k.n);
-  if (dn <= 1e-6) return false;
+  if (g_bidirectional ? std::fabs(dn) <= 1e-6 : dn <= 1e-6) return false;
   double rel[3] = {k.c[0] - r[0], k.c[1] - r[1], k.c[2] - r[2]};
   const double s = dot(rel, k.n) / dn;
   double q[3] = {r[0] + s * d[0] - k.c[0], r[1] + s * d[1] - k.c[1], r[2] + s * d[2] - k.c[2]};
@@ -717,6 +736,7 @@ int move_to_next_module(const OGeometry& g, const OField& fld, const OConfig& cf
     if (!std::isfinite(x[i])) return STOP_NUMERIC;
   if (!(x[3] > 0.0 && x[3] < PI)) return STOP_NUMERIC;
   const Module m = get_module(g, from);
+  g_bidirectional = cfg.bidirectional;
   double C[6][6];
   std::memcpy(C, Cin, sizeof(C));
   add_material(cfg, m, x, C);              // V5, with the momentum the tip arrived with
@@ -752,7 +772,9 @@ int move_to_next_module(const OGeometry& g, const OField& fld, const OConfig& cf
       }
       return best;
     };
-    int lb, ld;   // last barrel cylinder passed (the next one is lb + 1); next disc candidate (-1 = none)
+    int lb, ld;   // radial shell: last barrel cylinder inside the tip (the next one outward is lb + 1, the next one
+                  // inward is lb itself); next disc candidate (-1 = none)
+    const bool bidir = cfg.bidirectional != 0;
     if (is_disc(m.layer)) {
       const double rho = std::hypot(y.r[0], y.r[1]);
       lb = -1;
@@ -760,33 +782,54 @@ int move_to_next_module(const OGeometry& g, const OField& fld, const OConfig& cf
       ld = disc_after(m.layer, y.r[2], y.d[2]);
     } else {
       lb = m.layer;
+      // N3'': a tip that leaves a barrel module INWARD has its own layer's cylinder behind it already
+      if (bidir && y.r[0] * y.d[0] + y.r[1] * y.d[1] < 0.0) lb = m.layer - 1;
       ld = disc_after(-1, y.r[2], y.d[2]);
     }
     for (;;) {
       // a barrel layer whose half length is already behind a tip that moves away in z cannot be crossed inside its
       // acceptance: it is passed without propagating to it (reading D11, per layer)
-      while (!g_n3_literal_walk && lb + 1 < n_barrel && std::fabs(y.r[2]) > g.layer_half_z[lb + 1] &&
+      const double a = y.d[0] * y.d[0] + y.d[1] * y.d[1], b = y.r[0] * y.d[0] + y.r[1] * y.d[1];
+      const double rho2 = y.r[0] * y.r[0] + y.r[1] * y.r[1];
+      const bool inward = bidir && b < 0.0;
+      while (!inward && !g_n3_literal_walk && lb + 1 < n_barrel && std::fabs(y.r[2]) > g.layer_half_z[lb + 1] &&
              y.r[2] * y.d[2] > 0.0)
         ++lb;
       // likewise a disc whose plane is not ahead (any more), or whose outer radius is already behind a tip that moves
       // outward radially, is passed
-      {
-        const double rho2 = y.r[0] * y.r[0] + y.r[1] * y.r[1], bxy = y.r[0] * y.d[0] + y.r[1] * y.d[1];
-        while (ld >= 0 && ((g.layer_half_z[ld] - y.r[2]) * y.d[2] <= 0.0 ||
-                           (rho2 > g.layer_r[ld] * g.layer_r[ld] && bxy > 0.0)))
-          ld = disc_after(ld, y.r[2], y.d[2]);
+      while (ld >= 0 && ((g.layer_half_z[ld] - y.r[2]) * y.d[2] <= 0.0 ||
+                         (rho2 > g.layer_r[ld] * g.layer_r[ld] && b > 0.0)))
+        ld = disc_after(ld, y.r[2], y.d[2]);
+      int lc = lb + 1 < n_barrel ? lb + 1 : -1;
+      int cyl_kind = 1;   // how the cylinder candidate is crossed: 1 outward, 2 inward, 3 through its far side
+      double r_target = 0.0;
+      if (inward) {
+        // N3'': moving inward.  The candidate is the next inner cylinder (lb, or the first one below it whose half
+        // length is not behind a tip moving away in z) if the straight line reaches it; otherwise the tip turns inside
+        // its shell and leaves through the FAR side of the cylinder that bounds the shell from outside (lb + 1).
+        // The flat modules of a layer lie OUTSIDE its cylinder, between r and hypot(r, half_u): a tip coming from
+        // outside meets them before it meets the cylinder, so the inward portal of a layer is its outer envelope.
+        int li = lb;
+        while (!g_n3_literal_walk && li >= 0 && std::fabs(y.r[2]) > g.layer_half_z[li] && y.r[2] * y.d[2] > 0.0) --li;
+        if (li >= 0) r_target = std::hypot(g.layer_r[li], g.half_u[g.module_offset[li]]);
+        if (li >= 0 && b * b - a * (rho2 - r_target * r_target) >= 0.0) { lc = li; cyl_kind = 2; }
+        else {
+          cyl_kind = 3;   // first cylinder from lb + 1 outward that the straight line meets at all
+          while (lc >= 0 && b * b - a * (rho2 - g.layer_r[lc] * g.layer_r[lc]) < 0.0) lc = lc + 1 < n_barrel ? lc + 1 : -1;
+        }
       }
-      const int lc = lb + 1 < n_barrel ? lb + 1 : -1;
+      if (cyl_kind != 2 && lc >= 0) r_target = g.layer_r[lc];
       if (lc < 0 && ld < 0) return STOP_EXIT;
       bool to_disc = false;
       if (ld >= 0) {
         const double s_d = (g.layer_half_z[ld] - y.r[2]) / y.d[2];
         double s_c = INFINITY;   // straight-line distance to the cylinder (P4), infinite when it is not ahead
         if (lc >= 0) {
-          const double a = y.d[0] * y.d[0] + y.d[1] * y.d[1], b = y.r[0] * y.d[0] + y.r[1] * y.d[1];
-          const double cc = y.r[0] * y.r[0] + y.r[1] * y.r[1] - g.layer_r[lc] * g.layer_r[lc];
+          const double cc = rho2 - r_target * r_target;
           const double disc = b * b - a * cc;
-          if (b > 0.0 && disc >= 0.0) s_c = -cc / (b + std::sqrt(disc));
+          if (cyl_kind == 1) { if (b > 0.0 && disc >= 0.0) s_c = -cc / (b + std::sqrt(disc)); }
+          else if (cyl_kind == 2) s_c = cc / (-b + std::sqrt(disc));
+          else if (disc >= 0.0) s_c = (-b + std::sqrt(disc)) / a;
         }
         to_disc = lc < 0 || s_d < s_c;   // tie -> the cylinder
       }
@@ -794,11 +837,11 @@ int move_to_next_module(const OGeometry& g, const OField& fld, const OConfig& cf
       if (!to_disc) {
         lp = lc;
         Target cyl;
-        cyl.kind = 1;
-        cyl.R = g.layer_r[lp];
+        cyl.kind = cyl_kind;
+        cyl.R = r_target;
         int st = propagate_to(fld, cfg, cyl, y, cnt);
         if (st != STOP_NONE) return st;
-        lb = lp;
+        lb = cyl_kind == 2 ? lp - 1 : lp;   // crossed inward: the shell below it
         if (std::fabs(y.r[2]) > g.layer_half_z[lp]) continue;   // outside the layer's acceptance: on to the next portal
       } else {
         lp = ld;

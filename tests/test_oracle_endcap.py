@@ -124,3 +124,77 @@ def test_barrel_only_detector_is_unchanged_by_the_portal_rule(detector):
                 break
             assert cb == 0 and ta == tb and np.array_equal(xa, xb2) and np.array_equal(Ca, Cb)
             xm, mm, xb, mb = xa, ta, xb2, tb
+
+
+def _crossings_any_direction(det, stt, y0, start_module, margin=150.0):
+    """Brute force for tips that may cross modules against their normal: every module whose centre lies within `margin`
+    of the straight line ahead is tried with the tight-tolerance trajectory."""
+    normal = np.cross(det.axis_u, det.axis_v)
+    r0, d0 = y0[:3], y0[4:7]
+    rel = det.center - r0
+    along = rel @ d0
+    perp = np.linalg.norm(rel - along[:, None] * d0, axis=1)
+    crossed, near_edge = [], False
+    for k in np.flatnonzero((along > -50.0) & (perp < margin)):
+        if k == start_module:
+            continue
+        code, y1, _, _ = oracle.propagate_free(stt, y0, plane=(det.center[k], normal[k]))
+        if code != 0 or y1[3] < 1e-6:
+            continue
+        q = y1[:3] - det.center[k]
+        mu = det.half_u[k] - abs(np.dot(q, det.axis_u[k]))
+        mv = det.half_v[k] - abs(np.dot(q, det.axis_v[k]))
+        if mu >= 0 and mv >= 0:
+            crossed.append((y1[3], int(k)))
+        if min(abs(mu), abs(mv)) < 0.02 and max(-mu, -mv) < 0.02:
+            near_edge = True
+    crossed.sort()
+    return [k for _, k in crossed], near_edge
+
+
+def test_bidirectional_navigation_equals_brute_force(detector):
+    """config.bidirectional = 1 (rules N3''): tips that leave a barrel module INWARD cross the inner layers against
+    their normals, pass the beam line and leave through the far side -- the visited-module sequence equals the brute
+    force; with the flag off (reading A7, BASELINE configs) the same tips stop NOT_OUTGOING."""
+    det = detector
+    kw = dict(max_rk_steps_per_surface=100000)
+    on = oracle.Setup(det, synth.uniform_field(), CKFSettings(bidirectional=1, rk_tolerance_mm=1e-6, surface_tolerance_mm=1e-8, **kw))
+    off = oracle.Setup(det, synth.uniform_field(), CKFSettings(rk_tolerance_mm=1e-6, surface_tolerance_mm=1e-8, **kw))
+    stt = oracle.Setup(det, synth.uniform_field(), CKFSettings(rk_tolerance_mm=1e-8, surface_tolerance_mm=1e-10, **kw))
+    rng = np.random.default_rng(9)
+    n_cmp = n_inward_visits = n_turned = 0
+    for trial in range(10):
+        layer = int(rng.integers(0, 6))
+        m = int(det.module_offset[layer] + rng.integers(0, det.n_phi[layer]) * det.n_z[layer] + det.n_z[layer] // 2 +
+                rng.integers(-3, 4))
+        n = np.cross(det.axis_u[m], det.axis_v[m])
+        # pointing inward: opposite to the module normal, up to 1.2 rad off (so that some tips miss the inner layers)
+        phi = math.atan2(-n[1], -n[0]) + rng.uniform(-1.2, 1.2)
+        theta = rng.uniform(1.0, 2.1)
+        pt = math.exp(rng.uniform(math.log(5.0), math.log(50.0)))     # stiff: the pre-filter is a tube around a line
+        q = 1.0 if rng.random() < 0.5 else -1.0
+        x = np.array([rng.uniform(-5, 5), rng.uniform(-10, 10), phi, theta, q * math.sin(theta) / pt, 0.0])
+        d0 = np.array([math.sin(theta) * math.cos(phi), math.sin(theta) * math.sin(phi), math.cos(theta)])
+        r0 = det.center[m] + x[0] * det.axis_u[m] + x[1] * det.axis_v[m]
+        y0 = np.concatenate([r0, [0.0], d0, [x[4]]])
+        want, near_edge = _crossings_any_direction(det, stt, y0, m)
+        if near_edge:
+            continue
+        code0, *_ = oracle.move(off, m, x, np.eye(6) * 1e-6)
+        assert oracle.STOP_NAMES[code0] == "NOT_OUTGOING"          # reading A7 without the flag
+        visited, mm, xm = [], m, x
+        while True:
+            code, tg, xp, Cp, _ = oracle.move(on, mm, xm, np.eye(6) * 1e-6)
+            if code != 0:
+                assert oracle.STOP_NAMES[code] == "EXIT", (trial, oracle.STOP_NAMES[code])
+                break
+            visited.append(tg)
+            xm, mm = xp, tg
+        assert visited == want, (trial, layer, visited, want)
+        n_cmp += 1
+        normals = np.cross(det.axis_u[want], det.axis_v[want]) if want else np.zeros((0, 3))
+        lay = det.module_layer[np.array(want, int)] if want else np.zeros(0, int)
+        n_inward_visits += int(np.sum(lay < layer)) if want else 0
+        n_turned += int(want != [] and lay.min() >= layer)          # turned inside its shell: left through the far side
+    print("bidirectional pin: compared", n_cmp, "inward visits", n_inward_visits, "turned", n_turned)
+    assert n_cmp >= 8 and n_inward_visits >= 10 and n_turned >= 1
