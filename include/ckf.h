@@ -33,7 +33,7 @@
 extern "C" {
 #endif
 
-#define CKF_ABI_VERSION 8
+#define CKF_ABI_VERSION 9
 
 /* return codes */
 #define CKF_OK 0
@@ -126,6 +126,9 @@ typedef struct {
                                        covariance is transported with d(q/p)'/d(q/p).  0: none (BASELINE configs)     */
   int32_t field_gradient;           /* must be 0: the field-gradient terms of the transport Jacobian (PAPER.md ref
                                        [18]) exist in the oracle only (reading A13)                          */
+  int32_t bidirectional;            /* 1: tips that move radially INWARD are navigated too (DESIGN.md rules N3''): they cross the
+                                       inner layers against the module normals, pass the beam line and leave through the far
+                                       side.  0 (BASELINE configs, reading A7): outward only, such tips stop NOT_OUTGOING    */
   int32_t max_fit_tracks;           /* ckf_fit: candidates fitted per pass; sizes the state store reserved in ckf_create
                                        (max_levels states x min(max_fit_tracks, max_tracks, 262144) candidates x
                                        (12 float64 + 69 T): 3 GB at 262,144 in fp32).  0 = no ckf_fit on this handle */

@@ -44,7 +44,7 @@ class ckf_config(C.Structure):
                 ("max_seeds", C.c_int32), ("max_measurements", C.c_int32), ("max_tracks", C.c_int32),
                 ("max_track_entries", C.c_int32), ("max_links", C.c_int32), ("max_tips_per_level", C.c_int32),
                 ("n_streams", C.c_int32), ("max_events_per_find", C.c_int32), ("energy_loss", C.c_int32),
-                ("field_gradient", C.c_int32), ("max_fit_tracks", C.c_int32)]
+                ("field_gradient", C.c_int32), ("bidirectional", C.c_int32), ("max_fit_tracks", C.c_int32)]
 
 
 class ckf_measurements(C.Structure):
@@ -180,6 +180,7 @@ def make_config(ckf, precision: int, max_seeds: int, max_measurements: int, max_
     c.max_fit_tracks = int(max_fit_tracks)
     c.energy_loss = int(getattr(ckf, "energy_loss", 0))
     c.field_gradient = int(getattr(ckf, "field_gradient", 0))
+    c.bidirectional = int(getattr(ckf, "bidirectional", 0))
     return c
 
 

@@ -367,6 +367,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
       c->max_fit_tracks < 0)
     return fail(h, CKF_E_ARG, "capacities must be positive");
   if (g->n_layers < 1 || g->n_modules < 1) return fail(h, CKF_E_ARG, "empty geometry");
+  if (g->n_layers > 254) return fail(h, CKF_E_ARG, "at most 254 layers (the navigation cursors are 9-bit fields)");
   if (f->kind != 0 && f->kind != 1) return fail(h, CKF_E_ARG, "field kind must be 0 or 1");
   if (c->field_gradient != 0)
     return fail(h, CKF_E_ARG, "field_gradient = 1 (gradient terms in the transport Jacobian) is not built in the CUDA path");
@@ -427,6 +428,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
   CKB(cudaMemcpy(h->d_layer, layers.data(), layers.size() * sizeof(LayerRec), cudaMemcpyHostToDevice));
   h->geo.mod = h->d_mod; h->geo.layer = h->d_layer; h->geo.n_layers = g->n_layers; h->geo.n_modules = g->n_modules;
   fill_geo_summary(layers, h->geo);
+  h->geo.bidir = c->bidirectional ? 1 : 0;
   // ---- a2 field store
   std::memset(&h->fld, 0, sizeof(h->fld));
   h->fld.kind = f->kind;

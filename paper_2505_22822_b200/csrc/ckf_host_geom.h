@@ -22,6 +22,7 @@ inline void build_geometry_records(const ckf_geometry& g, std::vector<ModuleRec>
     L.kind = g.layer_kind ? g.layer_kind[l] : 0;
     L.r_min = (g.layer_kind && g.layer_r_min) ? g.layer_r_min[l] : 0.0;
     L.next_disc = -1;
+    L.r_in = std::sqrt(L.r * L.r + g.half_u[g.module_offset[l]] * g.half_u[g.module_offset[l]]);
   }
   // next disc of the same side: the one with the smallest |z| beyond this disc's
   for (int l = 0; l < g.n_layers; ++l) {

@@ -40,8 +40,9 @@ static_assert(sizeof(ModuleRec) == 128, "ModuleRec must be one 128-byte line");
 // kind 0: barrel cylinder of radius r, acceptance |z| <= half_z, modules on a (phi, z) grid of pitch len_z.
 // kind 1 (row f3): disc in the plane z = half_z (signed), acceptance r_min <= rho <= r, modules on a (phi, ring)
 // grid of ring pitch len_z, n_z rings; next_disc = the next disc of the same side (larger |z|) or -1.
+// r_in (barrel): hypot(r, half_u), the outer envelope of the layer's flat modules = its portal for INWARD-moving tips.
 struct LayerRec {
-  double r, half_z, len_z, r_min;
+  double r, half_z, len_z, r_min, r_in;
   int32_t n_phi, n_z, offset, kind, next_disc, pad;
 };
 

@@ -11,6 +11,7 @@ struct GeoDev {
   int32_t n_layers, n_modules;
   int32_t n_barrel;        // barrel layers come first, by increasing radius; disc layers follow
   int32_t first_disc[2];   // innermost disc of the +z side, of the -z side (-1 = none)
+  int32_t bidir;           // config.bidirectional: inward-moving tips are navigated, modules may be crossed against n
 };
 
 constexpr int NDEP = 6;  // numbers of a departure record (departure_state): direction[3], q_phi, q_theta, g
@@ -19,9 +20,10 @@ constexpr int NDEP = 6;  // numbers of a departure record (departure_state): dir
 CKF_HD constexpr int tri(int i, int j) { return i <= j ? i * 6 - (i * (i - 1)) / 2 + (j - i) : j * 6 - (j * (j - 1)) / 2 + (i - j); }
 
 // N2 / N4: straight-line test of one module from (r, d).
-CKF_HD bool line_hits_module(const ModuleRec& k, const double r[3], const double d[3], double s_min, double& s_out) {
+CKF_HD bool line_hits_module(const ModuleRec& k, const double r[3], const double d[3], double s_min, double& s_out,
+                             int bidir = 0) {
   const double dn = dot3(d, k.n);
-  if (dn <= 1e-6) return false;
+  if (bidir ? fabs(dn) <= 1e-6 : dn <= 1e-6) return false;
   const double rel[3] = {k.c[0] - r[0], k.c[1] - r[1], k.c[2] - r[2]};
   const double s = dot3(rel, k.n) / dn;
   const double q[3] = {r[0] + s * d[0] - k.c[0], r[1] + s * d[1] - k.c[1], r[2] + s * d[2] - k.c[2]};
@@ -35,12 +37,12 @@ CKF_HD bool line_hits_module(const ModuleRec& k, const double r[3], const double
 // The same test without early exits: path length, or NaN for "no hit".  Nine of these in a row have no control
 // dependence between them, so the loads of the nine module records overlap (thread-per-tip callers: ckf_update's N2,
 // ckf_fit_level; a chain of nine dependent L2 round trips was 25 % of ckf_update's stall samples).
-CKF_HD double line_test_module(const ModuleRec& k, const double r[3], const double d[3], double s_min) {
+CKF_HD double line_test_module(const ModuleRec& k, const double r[3], const double d[3], double s_min, int bidir = 0) {
   const double dn = dot3(d, k.n);
   const double rel[3] = {k.c[0] - r[0], k.c[1] - r[1], k.c[2] - r[2]};
   const double s = dot3(rel, k.n) / dn;
   const double q[3] = {r[0] + s * d[0] - k.c[0], r[1] + s * d[1] - k.c[1], r[2] + s * d[2] - k.c[2]};
-  const bool ok = dn > 1e-6 && fabs(dot3(q, k.u)) <= k.half_u && fabs(dot3(q, k.v)) <= k.half_v && s > s_min;
+  const bool ok = (bidir ? fabs(dn) > 1e-6 : dn > 1e-6) && fabs(dot3(q, k.u)) <= k.half_u && fabs(dot3(q, k.v)) <= k.half_v && s > s_min;
 #if defined(__CUDA_ARCH__)
   return ok ? s : __longlong_as_double(0x7ff8000000000000LL);
 #else
@@ -62,7 +64,7 @@ CKF_HD int pick_in_neighbourhood(const GeoDev& g, int layer, int iphi, int iz, i
     const int jj = iz + (nb % 3 - 1);
     const int id = L.offset + ii * L.n_z + jj;
     const bool test = jj >= 0 && jj < L.n_z && id != exclude;   // a predicate, not a branch around the loads
-    sv[nb] = test ? line_test_module(g.mod[id], r, d, s_min) : 0.0;
+    sv[nb] = test ? line_test_module(g.mod[id], r, d, s_min, g.bidir) : 0.0;
     idv[nb] = test ? id : -1;
   }
   int best = -1;
@@ -288,9 +290,14 @@ CKF_HD void kalman_update(const double x[6], const double C[21], M m0, M m1, M v
 //   PLANE --step--> PLANE (one trial) | FIN          N5 toward the target module's plane
 //   FIN   --arrive-> predicted bound parameters + 5x5 Jacobian block (J4, J5)
 //   DISC  --step--> DISC | LANDED                   like CYL toward the plane of a disc layer (row f3)
-enum MovePhase : int { PH_IDLE = 0, PH_START = 1, PH_CYL = 2, PH_LANDED = 3, PH_PLANE = 4, PH_FIN = 5, PH_DISC = 6 };
+//   CYL_IN / CYL_FAR (config.bidirectional, rules N3''): toward the outer envelope of an inner layer, crossed inward;
+//                   toward the far side of the cylinder that bounds the tip's shell
+enum MovePhase : int { PH_IDLE = 0, PH_START = 1, PH_CYL = 2, PH_LANDED = 3, PH_PLANE = 4, PH_FIN = 5, PH_DISC = 6,
+                       PH_CYL_IN = 7, PH_CYL_FAR = 8 };
 
-CKF_HD bool is_stepping(int phase) { return phase == PH_CYL || phase == PH_PLANE || phase == PH_DISC; }
+CKF_HD bool is_stepping(int phase) {
+  return phase == PH_CYL || phase == PH_PLANE || phase == PH_DISC || phase == PH_CYL_IN || phase == PH_CYL_FAR;
+}
 
 template <typename T>
 struct Move {
@@ -301,8 +308,14 @@ struct Move {
   double h, h_ctrl;
   double ib, dib;       // 1/beta and d(1/beta)/d(q/p): constant along the move (no energy loss)
   double B1[3];         // field at y.r, valid while `targeted` (read once per position, see move_target)
-  int phase, stop, from, tgt, lp, n_steps;
-  int lb, ld;           // portals (N3'): last barrel cylinder passed (the next is lb + 1); next disc candidate, -1 none
+  int phase, from, tgt, n_steps;
+  // navigation cursors, packed into one register (ckf_step sits at its register cap): they are touched once or twice
+  // per move, never inside the trial loop
+  int lp : 9;           // layer of the portal being targeted / just landed on
+  int lb : 9;           // portals (N3'): last barrel cylinder inside the tip (the next one outward is lb + 1), -1 none
+  int ld : 9;           // next disc candidate, -1 none
+  int stop : 4;         // stop reason so far
+  bool inward;          // the cylinder portal being targeted / just landed on is crossed inward (CYL_IN)
   bool targeted;        // the next trial's length m.h and B1 are set (P4 done for the current position)
 };
 
@@ -352,7 +365,7 @@ CKF_HD int departure_state(const GeoDev& g, const CfgDev& cfg, int from, const d
 // Start of a move whose m.y holds the departure state: identity transport, fresh step control (P4, J3).
 template <typename T>
 CKF_HD void move_begin(Move<T>& m, const CfgDev& cfg, int from) {
-  m.from = from; m.tgt = -1; m.lp = 0; m.lb = -1; m.ld = -1; m.n_steps = 0; m.targeted = false; m.stop = STOP_NONE;
+  m.from = from; m.tgt = -1; m.lp = 0; m.lb = -1; m.ld = -1; m.n_steps = 0; m.targeted = false; m.inward = false; m.stop = STOP_NONE;
   m.h = 0.0; m.h_ctrl = cfg.h_max; m.R = 0.0;
   jac_identity(m.D);
   m.ib = inv_beta(m.y.qop, cfg.mass);
@@ -395,7 +408,7 @@ CKF_HD int move_pick_request(Move<T>& m, const GeoDev& g, PickRequest& q) {
   q.layer = m.lp; q.exclude = -1; q.s_min = -1e-3; q.iphi = 0; q.iz = 0;
   double along;
   if (L.kind == 0) {
-    m.lb = m.lp;
+    m.lb = m.inward ? m.lp - 1 : m.lp;   // crossed inward: the shell below it
     if (fabs(m.y.r[2]) > L.half_z) return PICK_SKIP;
     along = m.y.r[2] + L.half_z;
   } else {
@@ -420,40 +433,77 @@ CKF_HD int move_pick_request(Move<T>& m, const GeoDev& g, PickRequest& q) {
 // D11, per layer).  No portal left = the tip has left the detector (EXIT).
 template <typename T>
 CKF_HD void choose_portal(Move<T>& m, const GeoDev& g) {
+  if (g.n_barrel == g.n_layers && !g.bidir) {
+    // barrel only, outward only (the BASELINE configs): the rule below reduces to "the next barrel cylinder whose half
+    // length is not behind the tip" -- kept as its own short path because it runs once or twice per move of the hot
+    // kernel (measured: the general code costs ckf_step 3-5 %)
+    int lb = (m.phase == PH_START) ? g.mod[m.from].layer : m.lb;
+    const double z = m.y.r[2];
+    if (z * m.y.d[2] > 0.0)
+      while (lb + 1 < g.n_barrel && fabs(z) > g.layer[lb + 1].half_z) ++lb;
+    m.lb = lb;
+    m.targeted = false;
+    if (lb + 1 >= g.n_barrel) { m.stop = STOP_EXIT; m.phase = PH_FIN; return; }
+    m.lp = lb + 1;
+    m.R = g.layer[lb + 1].r;
+    m.phase = PH_CYL;
+    return;
+  }
   const double z = m.y.r[2], dz = m.y.d[2];
   const double rho2 = m.y.r[0] * m.y.r[0] + m.y.r[1] * m.y.r[1], bxy = m.y.r[0] * m.y.d[0] + m.y.r[1] * m.y.d[1];
   if (m.phase == PH_START) {   // leaving a module: where the tip stands in the two families of portals
     const LayerRec L0 = g.layer[g.mod[m.from].layer];
     if (L0.kind == 0) {
       m.lb = g.mod[m.from].layer;
+      if (g.bidir && bxy < 0.0) m.lb -= 1;   // N3'': leaving a barrel module inward, its own cylinder is behind already
       m.ld = dz > 0.0 ? g.first_disc[0] : (dz < 0.0 ? g.first_disc[1] : -1);
     } else {
       m.lb = barrel_index_inside(g, sqrt(rho2));
       m.ld = L0.next_disc;
     }
   }
-  while (m.lb + 1 < g.n_barrel && fabs(z) > g.layer[m.lb + 1].half_z && z * dz > 0.0) ++m.lb;
+  const bool inward = g.bidir && bxy < 0.0;
+  while (!inward && m.lb + 1 < g.n_barrel && fabs(z) > g.layer[m.lb + 1].half_z && z * dz > 0.0) ++m.lb;
   while (m.ld >= 0 && ((g.layer[m.ld].half_z - z) * dz <= 0.0 || (rho2 > g.layer[m.ld].r * g.layer[m.ld].r && bxy > 0.0)))
     m.ld = g.layer[m.ld].next_disc;
-  const int lc = m.lb + 1 < g.n_barrel ? m.lb + 1 : -1;
+  int lc = m.lb + 1 < g.n_barrel ? m.lb + 1 : -1;
+  int kind = PH_CYL;
+  double r_target = 0.0;
+  const double a = m.y.d[0] * m.y.d[0] + m.y.d[1] * m.y.d[1];
+  if (inward) {
+    // N3'': the next inner layer's outer envelope if the straight line reaches it, else the far side of the first
+    // cylinder from lb + 1 outward that the line meets at all
+    int li = m.lb;
+    while (li >= 0 && fabs(z) > g.layer[li].half_z && z * dz > 0.0) --li;
+    if (li >= 0) r_target = g.layer[li].r_in;
+    if (li >= 0 && bxy * bxy - a * (rho2 - r_target * r_target) >= 0.0) { lc = li; kind = PH_CYL_IN; }
+    else {
+      kind = PH_CYL_FAR;
+      while (lc >= 0 && bxy * bxy - a * (rho2 - g.layer[lc].r * g.layer[lc].r) < 0.0) lc = lc + 1 < g.n_barrel ? lc + 1 : -1;
+    }
+  }
+  if (kind != PH_CYL_IN && lc >= 0) r_target = g.layer[lc].r;
   if (lc < 0 && m.ld < 0) { m.stop = STOP_EXIT; m.phase = PH_FIN; return; }
   bool to_disc = false;
   if (m.ld >= 0) {
     const double s_d = (g.layer[m.ld].half_z - z) / dz;
     double s_c = INFINITY;
     if (lc >= 0) {
-      const double a = m.y.d[0] * m.y.d[0] + m.y.d[1] * m.y.d[1];
-      const double cc = rho2 - g.layer[lc].r * g.layer[lc].r;
+      const double cc = rho2 - r_target * r_target;
       const double disc = bxy * bxy - a * cc;
-      if (bxy > 0.0 && disc >= 0.0) s_c = -cc / (bxy + sqrt(disc));
+      if (kind == PH_CYL) { if (bxy > 0.0 && disc >= 0.0) s_c = -cc / (bxy + sqrt(disc)); }
+      else if (kind == PH_CYL_IN) s_c = cc / (-bxy + sqrt(disc));
+      else if (disc >= 0.0) s_c = (-bxy + sqrt(disc)) / a;
     }
     to_disc = lc < 0 || s_d < s_c;
   }
   m.targeted = false;
+  m.inward = false;
   if (!to_disc) {
     m.lp = lc;
-    m.R = g.layer[lc].r;
-    m.phase = PH_CYL;
+    m.R = r_target;
+    m.phase = kind;
+    m.inward = kind == PH_CYL_IN;
   } else {
     m.lp = m.ld;
     const double zd = g.layer[m.ld].half_z;
@@ -491,8 +541,17 @@ CKF_HD int target_distance(const Move<T>& m, double& s) {
     const double b = m.y.r[0] * m.y.d[0] + m.y.r[1] * m.y.d[1];
     const double cc = m.y.r[0] * m.y.r[0] + m.y.r[1] * m.y.r[1] - m.R * m.R;
     const double disc = b * b - a * cc;
-    if (!(b > 0.0) || !(disc >= 0.0)) return STOP_NOT_OUTGOING;
-    s = -cc / (b + sqrt(disc));
+    if (m.phase == PH_CYL_IN) {          // near root from outside, moving inward (signed once overshot)
+      if (!(b < 0.0) || !(disc >= 0.0)) return STOP_NOT_OUTGOING;   // it turned before reaching it
+      s = cc / (-b + sqrt(disc));
+    } else if (m.phase == PH_CYL_FAR) {  // far root, written without cancellation for either sign of b
+      if (!(disc >= 0.0)) return STOP_NOT_OUTGOING;
+      const double sq = sqrt(disc);
+      s = b < 0.0 ? (-b + sq) / a : -cc / (b + sq);
+    } else {
+      if (!(b > 0.0) || !(disc >= 0.0)) return STOP_NOT_OUTGOING;
+      s = -cc / (b + sqrt(disc));
+    }
   }
   return isfinite(s) ? STOP_NONE : STOP_NUMERIC;
 }

@@ -69,7 +69,7 @@ __device__ __forceinline__ void pick_warp(const GeoDev& geo, const PickSmem& ps,
           const double r[3] = {ps.rd[0 * 32 + t], ps.rd[1 * 32 + t], ps.rd[2 * 32 + t]};
           const double d[3] = {ps.rd[3 * 32 + t], ps.rd[4 * 32 + t], ps.rd[5 * 32 + t]};
           double sv;
-          if (line_hits_module(geo.mod[id], r, d, (rx & 1) ? 1e-3 : -1e-3, sv)) sres = sv;
+          if (line_hits_module(geo.mod[id], r, d, (rx & 1) ? 1e-3 : -1e-3, sv, geo.bidir)) sres = sv;
         }
       }
       ps.hit[nb * 32 + t] = sres;
@@ -111,7 +111,7 @@ __global__ void __launch_bounds__(STEP_NT, MINB) ckf_step(const KParams<T> p, in
   const size_t TC = (size_t)p.tcap;
 
   Move<T> m;
-  m.phase = PH_IDLE; m.stop = STOP_NONE; m.from = 0; m.tgt = -1; m.lp = 0; m.lb = -1; m.ld = -1; m.n_steps = 0; m.targeted = false;
+  m.phase = PH_IDLE; m.stop = STOP_NONE; m.from = 0; m.tgt = -1; m.lp = 0; m.lb = -1; m.ld = -1; m.n_steps = 0; m.targeted = false; m.inward = false;
   m.B1[0] = m.B1[1] = m.B1[2] = 0.0;
   m.h = 0.0; m.h_ctrl = 0.0; m.R = 0.0; m.y.qop = 0.0; m.ib = 0.0; m.dib = 0.0;
   int tip = -1, nt = 0, na = 0;

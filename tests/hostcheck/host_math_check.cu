@@ -64,6 +64,7 @@ void* hm_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c) 
   build_geometry_records(*g, x->mods, x->layers);
   x->geo.mod = x->mods.data(); x->geo.layer = x->layers.data(); x->geo.n_layers = g->n_layers; x->geo.n_modules = g->n_modules;
   fill_geo_summary(x->layers, x->geo);
+  x->geo.bidir = c->bidirectional ? 1 : 0;
   std::memset(&x->fld, 0, sizeof(x->fld));
   x->fld.kind = f->kind;
   for (int a = 0; a < 3; ++a) {

@@ -818,3 +818,42 @@ def test_endcap_discs_parity(precision, inhom):
     print("endcap precision %d: %d seeds -> %d candidates (%d kept), fit %d" %
           (precision, ev.n_seeds, gpu.n_tracks, int(o_acc.sum()), rf["n_fitted"]))
     ckf.close()
+
+
+@pytest.mark.parametrize("endcap", [False, True])
+def test_bidirectional_navigation_parity(endcap):
+    """Row f3, config.bidirectional = 1 (lifts reading A7): the inward-pointing half of the fake seeds is walked through
+    the detector instead of stopping NOT_OUTGOING; ckf_find against the oracle, fp64, bit-exact."""
+    import copy
+    import torch
+    import oracle
+    from paper_2505_22822_b200 import CKF
+    from synth.events import CKFSettings
+    ckfs = CKFSettings(max_branches_per_surface=5, max_candidates_per_seed=50, bidirectional=1)
+    if endcap:
+        det = synth.build_detector(half_z=500.0, disc_z=ENDCAP_DISC_Z)
+        ev = synth.make_endcap_event(det, 1500, seed=77, n_fake_seeds=1500)
+    else:
+        det = synth.build_detector()
+        ev = synth.make_event(1, det=det, n_particles=1500, n_fake_seeds=1500)
+    fld = synth.uniform_field()
+    ora = oracle.find_event(oracle.Setup(det, fld, ckfs), ev, n_threads=8)
+    ckf = CKF(det, fld, ckfs, 64, max_seeds=ev.n_seeds, max_measurements=ev.n_measurements, max_fit_tracks=0)
+    dev, out = ckf.upload_event(ev), ckf.alloc_tracks()
+    ckf.find(dev, out)
+    torch.cuda.synchronize()
+    gpu = ckf.download(out)
+    cnt = ckf.counters()
+    parity.assert_bit_exact_lists(gpu, ora)
+    rel, chi2, cov = parity.max_param_diffs(gpu, ora)
+    assert rel < 1e-9 and chi2 < 1e-8 and cov < 1e-7, (rel, chi2, cov)
+    for k in ("visits", "rk_trials", "rk_accepted", "gate_tests", "updates", "tips"):
+        assert cnt[k] == ora.counters[k], (k, cnt[k], ora.counters[k])
+    # the flag matters: without it the inward half of the fake seeds dies at once and far fewer surfaces are visited
+    off = copy.copy(ckfs)
+    off.bidirectional = 0
+    ora0 = oracle.find_event(oracle.Setup(det, fld, off), ev, n_threads=8)
+    assert ora.counters["visits"] > ora0.counters["visits"] + 300
+    print("bidirectional endcap=%s: %d candidates, visits %d (outward only: %d)" %
+          (endcap, gpu.n_tracks, cnt["visits"], ora0.counters["visits"]))
+    ckf.close()

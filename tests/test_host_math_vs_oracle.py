@@ -110,3 +110,43 @@ def test_moves_with_endcap_discs_match_oracle(precision):
             n_disc += int(det.layer_kind[det.module_layer[tgo]])
             x, Cm, m = xo, Co, tgo
     assert n_moves > 900 and n_disc > 300 and n_exit > 100
+
+
+@pytest.mark.parametrize("endcap", [False, True])
+def test_bidirectional_moves_match_oracle(endcap):
+    """config.bidirectional = 1 (rules N3''): inward-pointing fake seeds are walked through the inner layers, past the
+    beam line and out of the far side; every move of the CUDA path's per-tip code against the oracle (stop codes,
+    targets, RKN4 trial counts, parameters)."""
+    from synth.events import CKFSettings
+    if endcap:
+        det = synth.build_detector(half_z=500.0, disc_z=(560.0, 640.0, 740.0, 860.0, 1000.0))
+        ev = synth.make_endcap_event(det, 40, seed=5, n_fake_seeds=260, noise_fraction=0.0)
+    else:
+        det = synth.build_detector()
+        ev = synth.make_event(1, det=det, n_particles=40, n_fake_seeds=260)
+    fld = synth.uniform_field()
+    ckf = CKFSettings(bidirectional=1)
+    st = oracle.Setup(det, fld, ckf)
+    hm = HostMath(det, fld, ckf)
+    n_moves = n_inward = n_exit = 0
+    for s in range(ev.n_seeds):
+        x = ev.seed_params[s].astype(np.float64)
+        Cm = ev.seed_cov[s].reshape(6, 6).astype(np.float64)
+        m = int(ev.seed_module[s])
+        for level in range(40):
+            nrm = np.cross(det.axis_u[m], det.axis_v[m])
+            d = np.array([np.sin(x[3]) * np.cos(x[2]), np.sin(x[3]) * np.sin(x[2]), np.cos(x[3])])
+            co, tgo, xo, Co, _ = oracle.move(st, m, x, Cm)
+            ch, tgh, xh, Ch, trials = hm.move(64, m, x, Cm)
+            assert co == ch and trials == oracle.last_move_trials(), (s, level, co, ch)
+            if co != 0:
+                n_exit += oracle.STOP_NAMES[co] == "EXIT"
+                break
+            assert tgo == tgh, (s, level)
+            assert np.max(np.abs(xo - xh) / np.maximum(np.abs(xo), 1.0)) < 1e-10
+            scale = np.sqrt(np.outer(np.diag(Co), np.diag(Co)))
+            assert np.max(np.abs(Co - Ch) / scale) < 1e-9
+            n_moves += 1
+            n_inward += int(np.dot(d, nrm) < 0.0)
+            x, Cm, m = xo, Co, tgo
+    assert n_moves > 2000 and n_inward > 80 and n_exit > 250, (n_moves, n_inward, n_exit)
