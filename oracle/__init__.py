@@ -40,6 +40,13 @@ class OConfig(C.Structure):
                 ("energy_loss", C.c_int32), ("field_gradient", C.c_int32), ("bidirectional", C.c_int32)]
 
 
+class OSeedConfig(C.Structure):
+    _fields_ = [("layer_b", C.c_int32), ("layer_m", C.c_int32), ("layer_t", C.c_int32), ("dphi_max", C.c_double),
+                ("cot_max", C.c_double), ("z0_max", C.c_double), ("dcot_max", C.c_double), ("pt_min", C.c_double),
+                ("d0_max", C.c_double), ("sigma_angle", C.c_double), ("rel_sigma_qop", C.c_double),
+                ("cov_scale", C.c_double)]
+
+
 STOP_NAMES = {0: "NONE", 1: "EXIT", 2: "HOLES", 3: "NOT_OUTGOING", 4: "STEP_LIMIT", 5: "NUMERIC", 6: "LEVEL_LIMIT"}
 
 _lib = None
@@ -70,6 +77,13 @@ def lib():
         L.oracle_move.argtypes = [C.POINTER(OGeometry), C.POINTER(OField), C.POINTER(OConfig), C.c_int32, _dp, _dp, _ip,
                                   _dp, _dp, _dp]
         L.oracle_last_move_trials.restype = C.c_int64
+        L.oracle_seed_find.restype = C.c_void_p
+        L.oracle_seed_find.argtypes = [C.POINTER(OGeometry), C.POINTER(OField), C.POINTER(OSeedConfig), C.c_int32, _ip,
+                                       _dp, _dp, C.c_int32]
+        L.oracle_seed_count.restype = C.c_int32
+        L.oracle_seed_count.argtypes = [C.c_void_p]
+        L.oracle_seed_copy.argtypes = [C.c_void_p, _ip, _ip, _dp, _dp]
+        L.oracle_seed_free.argtypes = [C.c_void_p]
         L.oracle_bound_to_bound.restype = C.c_int32
         L.oracle_bound_to_bound.argtypes = [C.POINTER(OGeometry), C.POINTER(OField), C.POINTER(OConfig), C.c_int32,
                                             C.c_int32, _dp, _dp, _dp]
@@ -361,3 +375,23 @@ def resolve_ambiguity(track_offsets, meas_idx, chi2_sum, n_measurements: int, ma
     lib().oracle_resolve_ambiguity(nt, _pi(to), _pi(mi), _pd(c2), int(n_measurements), int(max_shared_hits),
                                    float(max_shared_fraction), _pi(acc), _pi(ns))
     return acc, ns
+
+
+# ------------------------------------------------------------------ S: triplet seeding + parameter estimation
+def seed_find(setup: Setup, seeding, module_offsets, loc, var, n_threads: int = 1):
+    """Rules S0-S6 over all combinations.  Returns dict(triplets [n,3] measurement indices (bottom, middle, top),
+    module [n], params [n,6], cov [n,36]), ordered by (bottom, middle, top)."""
+    c = OSeedConfig()
+    for name, _t in OSeedConfig._fields_:
+        setattr(c, name, getattr(seeding, name))
+    mo, lo, va = _i(module_offsets), _d(loc), _d(var)
+    r = lib().oracle_seed_find(C.byref(setup.geometry), C.byref(setup.field), C.byref(c), lo.shape[0], _pi(mo), _pd(lo),
+                               _pd(va), int(n_threads))
+    try:
+        n = lib().oracle_seed_count(r)
+        out = dict(triplets=np.zeros((n, 3), np.int32), module=np.zeros(n, np.int32), params=np.zeros((n, 6)),
+                   cov=np.zeros((n, 36)))
+        lib().oracle_seed_copy(r, _pi(out["triplets"]), _pi(out["module"]), _pd(out["params"]), _pd(out["cov"]))
+    finally:
+        lib().oracle_seed_free(r)
+    return out

@@ -26,6 +26,10 @@
 // whole move's Jacobian against finite differences.  Field-gradient Jacobian (J2', tests/test_oracle_pins2.py): finite
 // differences of the bound->bound map in the analytic non-uniform field to 1e-5 with the terms on; the default
 // matrix form of J2 against the tangent form with G = 0 (pin hook field_gradient = 2) in that field.
+// Seeding + parameter estimation (rules S, tests/test_oracle_seed.py): S5 exact on three points of an analytic helix
+// (tangent, theta, q/p at the bottom point to 1e-9); S1-S4 against an enumeration of all combinations with other
+// textbook formulas (R = abc / 4A, circle centre from the bisectors), default and binding cuts.  Navigation with discs
+// and bidirectional navigation (tests/test_oracle_endcap.py): visited-module sequences against brute force.
 // Ambiguity resolution (rules AR, tests/test_oracle_resolve.py): the greedy's result against the unique fixed point of
 // its defining property found by brute force over all subsets of a small candidate set; limits k = 0 and k = infinity.
 // Parity unpinned (convention only, fixed by DESIGN.md): that R10 cuts in TIP order (the closed form itself is pinned),
@@ -1436,6 +1440,119 @@ void resolve_ambiguity(int n_tracks, const int32_t* offsets, const int32_t* meas
 
 thread_local long long g_last_move_trials = 0;
 
+// ====================================================================================== S: seeding + parameter estimation
+// "The spacepoints are used in the seeding algorithm where triplets, a set of three spacepoints which can
+// approximately form a helix, are found.  In the track parameter estimation algorithm, the position and momentum of
+// tracks, called a seed, are estimated at the first spacepoint using the helix model."  The paper gives no cut and no
+// formula; rules S0-S6 of DESIGN.md 3 (readings) are written out here as plain loops over all combinations.
+struct OSeedConfig {
+  int32_t layer_b, layer_m, layer_t;   // barrel layers of the bottom / middle / top spacepoint
+  double dphi_max;     // S1: |phi_outer - phi_inner| of a doublet
+  double cot_max;      // S1: |cot theta| of a doublet
+  double z0_max;       // S1: |z at rho = 0| of a doublet's straight line in (rho, z)
+  double dcot_max;     // S2: |cot theta (bottom, middle) - cot theta (middle, top)|
+  double pt_min;       // S3: transverse momentum of the circle through the three points, GeV
+  double d0_max;       // S4: distance of that circle from the z axis, mm
+  double sigma_angle;  // S6: phi / theta standard deviation of a seed, rad
+  double rel_sigma_qop;  // S6: relative standard deviation of q/p added to the sagitta-resolution term
+  double cov_scale;    // S6: inflation of every variance (BASELINE seeds: 10)
+};
+
+struct SeedOut {
+  int b, m, t;   // measurement indices
+  int module;
+  double x[6], C[36];
+};
+
+struct SpacePoint { int meas; double x, y, z, rho, phi; };
+
+// S0: spacepoints of one layer = global positions of its measurements
+std::vector<SpacePoint> layer_spacepoints(const OGeometry& g, int layer, const int32_t* moff, const double* loc) {
+  std::vector<SpacePoint> out;
+  for (int id = g.module_offset[layer]; id < g.module_offset[layer + 1]; ++id) {
+    const Module k = get_module(g, id);
+    for (int i = moff[id]; i < moff[id + 1]; ++i) {
+      SpacePoint p;
+      p.meas = i;
+      p.x = k.c[0] + loc[2 * i] * k.u[0] + loc[2 * i + 1] * k.v[0];
+      p.y = k.c[1] + loc[2 * i] * k.u[1] + loc[2 * i + 1] * k.v[1];
+      p.z = k.c[2] + loc[2 * i] * k.u[2] + loc[2 * i + 1] * k.v[2];
+      p.rho = std::hypot(p.x, p.y);
+      p.phi = std::atan2(p.y, p.x);
+      out.push_back(p);
+    }
+  }
+  return out;
+}
+
+// S1: doublet (inner, outer) -> cot theta, or false
+bool doublet_ok(const OSeedConfig& c, const SpacePoint& in, const SpacePoint& out, double& cot) {
+  double dphi = out.phi - in.phi;
+  while (dphi > PI) dphi -= 2.0 * PI;
+  while (dphi <= -PI) dphi += 2.0 * PI;
+  if (!(std::fabs(dphi) <= c.dphi_max)) return false;
+  const double drho = out.rho - in.rho;
+  if (!(drho > 0.0)) return false;
+  cot = (out.z - in.z) / drho;
+  if (!(std::fabs(cot) <= c.cot_max)) return false;
+  const double z0 = in.z - in.rho * cot;
+  return std::fabs(z0) <= c.z0_max;
+}
+
+// S3-S6 for one triplet that passed S1, S2: false if a cut fails
+bool triplet_seed(const OGeometry& g, const OField& fld, const OSeedConfig& c, const int32_t* meas_module,
+                  const double* loc, const double* var, const SpacePoint& B, const SpacePoint& M, const SpacePoint& T,
+                  SeedOut& s) {
+  // S3: circle through the three transverse points
+  const double d = 2.0 * (B.x * (M.y - T.y) + M.x * (T.y - B.y) + T.x * (B.y - M.y));
+  if (d == 0.0) return false;   // exactly collinear: no curvature to estimate
+  const double b2 = B.x * B.x + B.y * B.y, m2 = M.x * M.x + M.y * M.y, t2 = T.x * T.x + T.y * T.y;
+  const double xc = (b2 * (M.y - T.y) + m2 * (T.y - B.y) + t2 * (B.y - M.y)) / d;
+  const double yc = (b2 * (T.x - M.x) + m2 * (B.x - T.x) + t2 * (M.x - B.x)) / d;
+  const double R = std::hypot(B.x - xc, B.y - yc);
+  const double rB[3] = {B.x, B.y, B.z};
+  double Bf[3];
+  field_at(fld, rB, Bf);
+  const double pt = KAPPA * std::fabs(Bf[2]) * R;
+  if (!(pt >= c.pt_min)) return false;
+  // S4: distance of the circle from the z axis
+  if (!(std::fabs(std::hypot(xc, yc) - R) <= c.d0_max)) return false;
+  // S5: helix parameters at the bottom spacepoint
+  double tx = -(B.y - yc) / R, ty = (B.x - xc) / R;   // tangent, oriented toward the middle point
+  if (tx * (M.x - B.x) + ty * (M.y - B.y) < 0.0) { tx = -tx; ty = -ty; }
+  const double cz = (M.x - B.x) * (T.y - M.y) - (M.y - B.y) * (T.x - M.x);   // turning sense of B -> M -> T
+  const double q = (cz * Bf[2] < 0.0) ? 1.0 : -1.0;      // a positive charge turns clockwise in a field along +z (P1)
+  const double chord = std::hypot(T.x - B.x, T.y - B.y);
+  const double arc = 2.0 * R * std::asin(std::min(1.0, chord / (2.0 * R)));
+  const double cot = (T.z - B.z) / arc;
+  const double theta = std::atan2(1.0, cot);
+  s.b = B.meas; s.m = M.meas; s.t = T.meas;
+  s.module = meas_module[B.meas];
+  s.x[0] = loc[2 * B.meas]; s.x[1] = loc[2 * B.meas + 1];
+  s.x[2] = std::atan2(ty, tx);
+  s.x[3] = theta;
+  s.x[4] = q * std::sin(theta) / pt;
+  s.x[5] = 0.0;
+  // S6: diagonal covariance
+  for (int i = 0; i < 36; ++i) s.C[i] = 0.0;
+  s.C[0] = c.cov_scale * var[2 * B.meas];
+  s.C[7] = c.cov_scale * var[2 * B.meas + 1];
+  s.C[14] = c.cov_scale * c.sigma_angle * c.sigma_angle;
+  s.C[21] = c.cov_scale * c.sigma_angle * c.sigma_angle;
+  // q/p: what three points resolve -- the sagitta sag = M - (B + T) / 2 across the chord L has variance
+  // var_M + (var_B + var_T) / 4 in the measured transverse coordinate, 1/R = 8 sag / L^2 -- plus a relative term for
+  // the scattering between the layers
+  const double var_sag = var[2 * M.meas] + 0.25 * (var[2 * B.meas] + var[2 * T.meas]);
+  const double dcurv = 8.0 * std::sqrt(var_sag) / (chord * chord);                    // sigma(1/R), 1/mm
+  const double sq_res = std::sin(theta) * dcurv / (KAPPA * std::fabs(Bf[2]));          // sigma(q/p) from the resolution
+  s.C[28] = c.cov_scale * (sq_res * sq_res + (c.rel_sigma_qop * s.x[4]) * (c.rel_sigma_qop * s.x[4]));
+  s.C[35] = 1.0;
+  (void)g;
+  return true;
+}
+
+struct SeedResult { std::vector<SeedOut> seeds; };
+
 // ====================================================================================== C interface
 extern "C" {
 
@@ -1658,6 +1775,61 @@ int32_t oracle_move(const OGeometry* g, const OField* f, const OConfig* cfg, int
   }
   return st;
 }
+
+// S: every triplet (bottom, middle, top) of spacepoints on the three seeding layers that passes S1-S4, as a seed (S5, S6).
+// Order: by (bottom, middle, top) measurement index.  Threads split the bottom spacepoints.
+void* oracle_seed_find(const OGeometry* g, const OField* f, const OSeedConfig* c, int32_t n_meas, const int32_t* module_offsets,
+                       const double* loc, const double* var, int32_t n_threads) {
+  std::vector<int32_t> meas_module(n_meas, -1);
+  for (int id = 0; id < g->n_modules; ++id)
+    for (int i = module_offsets[id]; i < module_offsets[id + 1]; ++i) meas_module[i] = id;
+  const std::vector<SpacePoint> Bs = layer_spacepoints(*g, c->layer_b, module_offsets, loc);
+  const std::vector<SpacePoint> Ms = layer_spacepoints(*g, c->layer_m, module_offsets, loc);
+  const std::vector<SpacePoint> Ts = layer_spacepoints(*g, c->layer_t, module_offsets, loc);
+  if (n_threads < 1) n_threads = 1;
+  std::vector<std::vector<SeedOut>> parts(n_threads);
+  auto work = [&](int th) {
+    const size_t lo = Bs.size() * th / n_threads, hi = Bs.size() * (th + 1) / n_threads;
+    std::vector<std::pair<int, double>> tops;
+    for (size_t ib = lo; ib < hi; ++ib)
+      for (size_t im = 0; im < Ms.size(); ++im) {
+        double cot_bm;
+        if (!doublet_ok(*c, Bs[ib], Ms[im], cot_bm)) continue;
+        for (size_t it = 0; it < Ts.size(); ++it) {
+          double cot_mt;
+          if (!doublet_ok(*c, Ms[im], Ts[it], cot_mt)) continue;
+          if (!(std::fabs(cot_bm - cot_mt) <= c->dcot_max)) continue;   // S2
+          SeedOut s;
+          if (triplet_seed(*g, *f, *c, meas_module.data(), loc, var, Bs[ib], Ms[im], Ts[it], s)) parts[th].push_back(s);
+        }
+      }
+  };
+  if (n_threads == 1) work(0);
+  else {
+    std::vector<std::thread> th;
+    for (int t = 0; t < n_threads; ++t) th.emplace_back(work, t);
+    for (auto& x : th) x.join();
+  }
+  SeedResult* R = new SeedResult();
+  for (auto& p : parts)
+    for (auto& s : p) R->seeds.push_back(s);
+  std::sort(R->seeds.begin(), R->seeds.end(), [](const SeedOut& a, const SeedOut& b) {
+    return a.b != b.b ? a.b < b.b : (a.m != b.m ? a.m < b.m : a.t < b.t);
+  });
+  return R;
+}
+int32_t oracle_seed_count(const void* r) { return (int32_t)((const SeedResult*)r)->seeds.size(); }
+void oracle_seed_copy(const void* r, int32_t* triplets, int32_t* module, double* params, double* cov) {
+  const SeedResult* R = (const SeedResult*)r;
+  for (size_t i = 0; i < R->seeds.size(); ++i) {
+    const SeedOut& s = R->seeds[i];
+    triplets[3 * i] = s.b; triplets[3 * i + 1] = s.m; triplets[3 * i + 2] = s.t;
+    module[i] = s.module;
+    std::memcpy(params + 6 * i, s.x, sizeof(s.x));
+    std::memcpy(cov + 36 * i, s.C, sizeof(s.C));
+  }
+}
+void oracle_seed_free(void* r) { delete (SeedResult*)r; }
 
 // RKN4 trials of the calling thread's last oracle_move (for the per-move comparison of the host-math test)
 int64_t oracle_last_move_trials(void) { return g_last_move_trials; }

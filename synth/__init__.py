@@ -11,10 +11,10 @@ Recipe: BASELINE.json configs[0..4]; stated in DESIGN.md §5.
 """
 from .detector import Detector, build_detector
 from .field import FieldSpec, uniform_field, grid_field, analytic_b
-from .events import Event, EventConfig, CKFSettings, CONFIGS, make_event, config_bundle
+from .events import Event, EventConfig, CKFSettings, SeedSettings, CONFIGS, make_event, config_bundle
 from .endcap import make_endcap_event
 
 __all__ = [
     "Detector", "build_detector", "FieldSpec", "uniform_field", "grid_field", "analytic_b",
-    "Event", "EventConfig", "CKFSettings", "CONFIGS", "make_event", "config_bundle", "make_endcap_event",
+    "Event", "EventConfig", "CKFSettings", "SeedSettings", "CONFIGS", "make_event", "config_bundle", "make_endcap_event",
 ]
