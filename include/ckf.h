@@ -33,7 +33,7 @@
 extern "C" {
 #endif
 
-#define CKF_ABI_VERSION 9
+#define CKF_ABI_VERSION 10
 
 /* return codes */
 #define CKF_OK 0
@@ -129,6 +129,8 @@ typedef struct {
   int32_t bidirectional;            /* 1: tips that move radially INWARD are navigated too (DESIGN.md rules N3''): they cross the
                                        inner layers against the module normals, pass the beam line and leave through the far
                                        side.  0 (BASELINE configs, reading A7): outward only, such tips stop NOT_OUTGOING    */
+  int32_t max_seed_doublets;        /* ckf_seed: capacity of its middle-top doublet lists; its workspace (48 B per measurement
+                                       + 12 B per doublet) is reserved in ckf_create.  0 = no ckf_seed on this handle */
   int32_t max_fit_tracks;           /* ckf_fit: candidates fitted per pass; sizes the state store reserved in ckf_create
                                        (max_levels states x min(max_fit_tracks, max_tracks, 262144) candidates x
                                        (12 float64 + 69 T): 3 GB at 262,144 in fp32).  0 = no ckf_fit on this handle */
@@ -278,6 +280,52 @@ typedef struct {
  * are ordered one after the other (one workspace per handle). */
 int ckf_resolve(ckf_handle* handle, const ckf_tracks* tracks, int32_t n_measurements, ckf_resolution* out,
                 void* cuda_stream);
+
+/* ---- Triplet seeding + track-parameter estimation, the stage in front of the CKF ---
+ * "The spacepoints are used in the seeding algorithm where triplets, a set of three spacepoints which can approximately
+ * form a helix, are found.  In the track parameter estimation algorithm, the position and momentum of tracks, called a
+ * seed, are estimated at the first spacepoint using the helix model".  The paper gives no cut and no
+ * formula; rules S0-S6 of DESIGN.md 3: spacepoints = global positions of the measurements of three barrel layers;
+ * doublets (inner, outer) with |dphi| <= dphi_max, |cot theta| <= cot_max, |z0| <= z0_max; triplets with
+ * |cot(b,m) - cot(m,t)| <= dcot_max whose circle through the three transverse points has pT >= pt_min (field at the
+ * bottom point) and passes within d0_max of the z axis; every such triplet is a seed: bound parameters on the bottom
+ * measurement's module (its loc0, loc1; tangent direction, arc-length cot theta, charge from the turning sense, q/p) and
+ * a diagonal covariance cov_scale x (measurement variances, sigma_angle^2 twice, what the sagitta resolves in q/p plus
+ * (rel_sigma_qop q/p)^2, and 1 for t unscaled). */
+typedef struct {
+  int32_t layer_b;       /* barrel layers, bottom < middle < top */
+  int32_t layer_m;
+  int32_t layer_t;
+  double dphi_max;       /* doublet cuts: rad                    */
+  double cot_max;
+  double z0_max;         /* mm                                   */
+  double dcot_max;       /* triplet cuts                         */
+  double pt_min;         /* GeV                                  */
+  double d0_max;         /* mm                                   */
+  double sigma_angle;    /* covariance recipe, see above         */
+  double rel_sigma_qop;
+  double cov_scale;
+} ckf_seeding;
+
+/* Seeds in the layout of ckf_seeds.  DEVICE pointers, caller-owned, sized from `capacity`.  Order: by (bottom, middle,
+ * top) measurement index; deterministic.  *n_seeds is written on the device: read it (after the stream) to fill
+ * ckf_seeds.n for ckf_find. */
+typedef struct {
+  int32_t* n_seeds;    /* [1]                                                                    */
+  int32_t* status;     /* [1] 1 = more seeds than capacity (the first `capacity` are kept), 2 = the doublet lists did
+                          not fit config.max_seed_doublets (no seed is reported)                 */
+  int32_t* module_id;  /* [capacity] module of the bottom measurement                             */
+  void* params;        /* T[capacity][6]                                                          */
+  void* cov;           /* T[capacity][36]                                                         */
+  int32_t* triplets;   /* [capacity][3] measurement indices (bottom, middle, top)                 */
+  int32_t capacity;    /* INPUT                                                                   */
+} ckf_seed_out;
+
+/* Seeds of one event's measurements (DEVICE arrays as for ckf_find, one event).  Asynchronous on `cuda_stream`,
+ * allocates nothing (CKF_E_CAPACITY if config.max_seed_doublets was 0).  Calls on different streams are ordered one
+ * after the other (one workspace per handle). */
+int ckf_seed(ckf_handle* handle, const ckf_measurements* measurements, const ckf_seeding* seeding, ckf_seed_out* out,
+             void* cuda_stream);
 
 /* Copies the work counters of the most recent ckf_find issued on `cuda_stream` (synchronises that stream). */
 int ckf_get_counters(ckf_handle* handle, void* cuda_stream, ckf_counters* out);

@@ -9,7 +9,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(HERE, "libckf.so")
 SOURCES = ["ckf.cu"]
-DEPS = ["ckf.cu", "ckf_math.cuh", "ckf_nav.cuh", "ckf_kernels.cuh", "ckf_step.cuh", "ckf_fit.cuh", "ckf_visit.cuh", "ckf_branch.cuh", "ckf_emit.cuh", "ckf_sort.cuh", "ckf_peak.cuh", "ckf_resolve.cuh",
+DEPS = ["ckf.cu", "ckf_math.cuh", "ckf_nav.cuh", "ckf_kernels.cuh", "ckf_step.cuh", "ckf_fit.cuh", "ckf_visit.cuh", "ckf_branch.cuh", "ckf_emit.cuh", "ckf_sort.cuh", "ckf_peak.cuh", "ckf_resolve.cuh", "ckf_seed.cuh",
         "ckf_host_geom.h", os.path.join("..", "..", "include", "ckf.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17", "-shared",
               "-Xcompiler", "-fPIC", "-Xptxas", "-v"]

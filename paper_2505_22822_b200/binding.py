@@ -21,7 +21,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libckf.so")
 
 EXPORTS = ("ckf_create", "ckf_find", "ckf_find_host", "ckf_fit", "ckf_get_counters", "ckf_get_launch_info", "ckf_destroy",
-           "ckf_set_timing", "ckf_get_timing", "ckf_measure_alu_peak", "ckf_resolve",
+           "ckf_set_timing", "ckf_get_timing", "ckf_measure_alu_peak", "ckf_resolve", "ckf_seed",
            "ckf_last_error", "ckf_abi_version")
 
 
@@ -44,7 +44,7 @@ class ckf_config(C.Structure):
                 ("max_seeds", C.c_int32), ("max_measurements", C.c_int32), ("max_tracks", C.c_int32),
                 ("max_track_entries", C.c_int32), ("max_links", C.c_int32), ("max_tips_per_level", C.c_int32),
                 ("n_streams", C.c_int32), ("max_events_per_find", C.c_int32), ("energy_loss", C.c_int32),
-                ("field_gradient", C.c_int32), ("bidirectional", C.c_int32), ("max_fit_tracks", C.c_int32)]
+                ("field_gradient", C.c_int32), ("bidirectional", C.c_int32), ("max_seed_doublets", C.c_int32), ("max_fit_tracks", C.c_int32)]
 
 
 class ckf_measurements(C.Structure):
@@ -69,6 +69,18 @@ class ckf_fits(C.Structure):
 class ckf_resolution(C.Structure):
     _fields_ = [("accepted", _vp), ("n_shared", _vp), ("summary", _vp), ("max_shared_hits", C.c_int32),
                 ("max_shared_fraction", C.c_double)]
+
+
+class ckf_seeding(C.Structure):
+    _fields_ = [("layer_b", C.c_int32), ("layer_m", C.c_int32), ("layer_t", C.c_int32), ("dphi_max", C.c_double),
+                ("cot_max", C.c_double), ("z0_max", C.c_double), ("dcot_max", C.c_double), ("pt_min", C.c_double),
+                ("d0_max", C.c_double), ("sigma_angle", C.c_double), ("rel_sigma_qop", C.c_double),
+                ("cov_scale", C.c_double)]
+
+
+class ckf_seed_out(C.Structure):
+    _fields_ = [("n_seeds", _vp), ("status", _vp), ("module_id", _vp), ("params", _vp), ("cov", _vp), ("triplets", _vp),
+                ("capacity", C.c_int32)]
 
 
 class ckf_timing(C.Structure):
@@ -104,6 +116,8 @@ def load_library():
                               C.POINTER(ckf_fits), _vp]
         L.ckf_resolve.restype = C.c_int
         L.ckf_resolve.argtypes = [_vp, C.POINTER(ckf_tracks), C.c_int32, C.POINTER(ckf_resolution), _vp]
+        L.ckf_seed.restype = C.c_int
+        L.ckf_seed.argtypes = [_vp, C.POINTER(ckf_measurements), C.POINTER(ckf_seeding), C.POINTER(ckf_seed_out), _vp]
         L.ckf_set_timing.restype = C.c_int
         L.ckf_set_timing.argtypes = [_vp, C.c_int]
         L.ckf_get_timing.restype = C.c_int
@@ -165,7 +179,7 @@ def make_field(fld, keep: list) -> ckf_field:
 
 def make_config(ckf, precision: int, max_seeds: int, max_measurements: int, max_tracks: int, max_track_entries: int,
                 max_links: int = 0, n_streams: int = 1, max_tips_per_level: int = 0,
-                max_events_per_find: int = 1, max_fit_tracks: int = 0) -> ckf_config:
+                max_events_per_find: int = 1, max_fit_tracks: int = 0, max_seed_doublets: int = 0) -> ckf_config:
     c = ckf_config()
     c.precision = int(precision)
     for name in ("chi2_max", "max_branches_per_surface", "max_candidates_per_seed", "max_holes", "min_measurements",
@@ -178,6 +192,7 @@ def make_config(ckf, precision: int, max_seeds: int, max_measurements: int, max_
     c.max_tips_per_level = int(max_tips_per_level)
     c.max_events_per_find = int(max_events_per_find)
     c.max_fit_tracks = int(max_fit_tracks)
+    c.max_seed_doublets = int(max_seed_doublets)
     c.energy_loss = int(getattr(ckf, "energy_loss", 0))
     c.field_gradient = int(getattr(ckf, "field_gradient", 0))
     c.bidirectional = int(getattr(ckf, "bidirectional", 0))
@@ -260,7 +275,7 @@ class CKF:
     def __init__(self, det, fld, ckf, precision: int, max_seeds: int, max_measurements: int,
                  max_tracks: Optional[int] = None, max_track_entries: Optional[int] = None, max_links: int = 0,
                  n_streams: int = 1, max_tips_per_level: int = 0, max_events_per_find: int = 1,
-                 max_fit_tracks: Optional[int] = None):
+                 max_fit_tracks: Optional[int] = None, max_seed_doublets: int = 0):
         """max_fit_tracks: candidates per ckf_fit pass (sizes the state store reserved by ckf_create); None = all of
         max_tracks up to the library's pass limit, 0 = this handle never fits."""
         import torch
@@ -279,7 +294,7 @@ class CKF:
         f = make_field(fld, keep)
         self.config = make_config(ckf, precision, max_seeds, max_measurements, self.max_tracks, self.max_track_entries,
                                   max_links, n_streams, max_tips_per_level, max_events_per_find,
-                                  self.max_tracks if max_fit_tracks is None else max_fit_tracks)
+                                  self.max_tracks if max_fit_tracks is None else max_fit_tracks, max_seed_doublets)
         h = _vp()
         rc = self.lib.ckf_create(C.byref(g), C.byref(f), C.byref(self.config), C.byref(h))
         if rc != 0:
@@ -354,6 +369,26 @@ class CKF:
                 a = a[:n_entries] if k == "entry_params" else a[:n_tracks]
             out[k] = a.astype(np.float64) if a.dtype.kind == "f" else a.copy()
         return out
+
+    # ------------------------------------------------------------------ seeding + parameter estimation (ckf_seed)
+    def alloc_seeds(self, capacity: int, device="cuda"):
+        t = self.torch
+        i32 = dict(dtype=t.int32, device=device)
+        T = dict(dtype=self.tdtype, device=device)
+        return dict(n_seeds=t.zeros(1, **i32), status=t.zeros(1, **i32), module_id=t.zeros(capacity, **i32),
+                    params=t.zeros(capacity, 6, **T), cov=t.zeros(capacity, 36, **T), triplets=t.zeros(capacity, 3, **i32))
+
+    def seed(self, dev_event: dict, seeding, seeds: dict, stream=None):
+        """Asynchronous ckf_seed on the measurements of `dev_event` (device tensors); `seeding` = synth.SeedSettings."""
+        st = stream if stream is not None else self.torch.cuda.current_stream()
+        m = ckf_measurements(int(dev_event["loc"].shape[0]), dev_event["module_offsets"].data_ptr(),
+                             dev_event["loc"].data_ptr(), dev_event["var"].data_ptr(), 1)
+        sc = ckf_seeding(*[getattr(seeding, n) for n, _ in ckf_seeding._fields_])
+        o = ckf_seed_out(*[seeds[k].data_ptr() for k in ("n_seeds", "status", "module_id", "params", "cov", "triplets")],
+                         int(seeds["module_id"].shape[0]))
+        rc = self.lib.ckf_seed(self.handle, C.byref(m), C.byref(sc), C.byref(o), _vp(st.cuda_stream))
+        if rc != 0:
+            raise RuntimeError("ckf_seed failed (%d): %s" % (rc, self.lib.ckf_last_error(self.handle).decode()))
 
     # ------------------------------------------------------------------ ambiguity resolution (ckf_resolve)
     def alloc_resolution(self, device="cuda"):

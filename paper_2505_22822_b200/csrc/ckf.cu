@@ -23,6 +23,7 @@
 #include "ckf_fit.cuh"
 #include "ckf_peak.cuh"
 #include "ckf_resolve.cuh"
+#include "ckf_seed.cuh"
 #include "ckf_sort.cuh"
 #include "ckf_step.cuh"
 #include "ckf_visit.cuh"
@@ -107,6 +108,10 @@ struct ckf_handle {
   int32_t *rs_owner = nullptr, *rs_state = nullptr, *rs_g = nullptr;
   int resolve_grid = 0;
   cudaEvent_t resolve_done = nullptr;
+  // workspace of ckf_seed (one per handle; reserved when config.max_seed_doublets > 0)
+  double *sd_sp = nullptr, *sd_cot = nullptr;
+  int32_t *sd_cnt = nullptr, *sd_off = nullptr, *sd_t = nullptr, *sd_g = nullptr;
+  cudaEvent_t seed_done = nullptr;
   bool timing_print = false;
   bool timing = false;  // ckf_set_timing / CKF_TIMING=1: per-kernel CUDA-event times of every ckf_find on stderr (debug aid; synchronises)
 };
@@ -344,6 +349,35 @@ struct WsGuard {
   ~WsGuard() { release_ws(w, st); }
 };
 
+template <typename T>
+int launch_seed(ckf_handle* h, const ckf_measurements* m, const ckf_seeding* sc, ckf_seed_out* o, cudaStream_t st) {
+  SeedParams<T> p;
+  p.geo = h->geo; p.fld = h->fld;
+  p.cfg.layer_b = sc->layer_b; p.cfg.layer_m = sc->layer_m; p.cfg.layer_t = sc->layer_t;
+  p.cfg.dphi_max = sc->dphi_max; p.cfg.cot_max = sc->cot_max; p.cfg.z0_max = sc->z0_max; p.cfg.dcot_max = sc->dcot_max;
+  p.cfg.pt_min = sc->pt_min; p.cfg.d0_max = sc->d0_max; p.cfg.sigma_angle = sc->sigma_angle;
+  p.cfg.rel_sigma_qop = sc->rel_sigma_qop; p.cfg.cov_scale = sc->cov_scale;
+  p.n_meas = m->n; p.moff = m->module_offsets; p.loc = (const T*)m->loc; p.var = (const T*)m->var;
+  p.sp = h->sd_sp; p.n_cap = h->cfg.max_measurements; p.cnt = h->sd_cnt; p.mt_off = h->sd_off; p.mt_t = h->sd_t;
+  p.mt_cot = h->sd_cot; p.max_doublets = h->cfg.max_seed_doublets; p.g = h->sd_g;
+  p.capacity = o->capacity; p.o_n = o->n_seeds; p.o_status = o->status; p.o_module = o->module_id;
+  p.o_params = (T*)o->params; p.o_cov = (T*)o->cov; p.o_triplets = o->triplets;
+  const int wide = h->sm_count * 8, n = m->n;
+  seed_spacepoints<T><<<wide, 128, 0, st>>>(p);
+  cudaMemsetAsync(p.cnt, 0, ((size_t)n + 1) * 4, st);
+  seed_doublets_mt<T, false><<<wide, 128, 0, st>>>(p);
+  seed_scan<<<1, 1024, 0, st>>>(p.cnt, p.mt_off, n, p.g + 0);
+  seed_doublets_mt<T, true><<<wide, 128, 0, st>>>(p);
+  cudaMemsetAsync(p.cnt, 0, ((size_t)n + 1) * 4, st);
+  seed_triplets<T, false><<<wide, 128, 0, st>>>(p);
+  seed_scan<<<1, 1024, 0, st>>>(p.cnt, p.cnt, n, p.g + 1);
+  seed_triplets<T, true><<<wide, 128, 0, st>>>(p);
+  seed_finish<T><<<1, 1, 0, st>>>(p);
+  cudaError_t e = cudaGetLastError();
+  if (e != cudaSuccess) return fail(h, CKF_E_CUDA, "ckf_seed launch failed: %s", cudaGetErrorString(e));
+  return CKF_OK;
+}
+
 }  // namespace
 
 extern "C" {
@@ -364,7 +398,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
   if (c->max_levels < 1 || c->max_levels > 64) return fail(h, CKF_E_ARG, "max_levels must be in 1..64");
   if (c->min_measurements < 1) return fail(h, CKF_E_ARG, "min_measurements must be >= 1");
   if (c->max_seeds < 1 || c->max_measurements < 0 || c->max_tracks < 1 || c->max_track_entries < 1 || c->n_streams < 1 ||
-      c->max_fit_tracks < 0)
+      c->max_fit_tracks < 0 || c->max_seed_doublets < 0)
     return fail(h, CKF_E_ARG, "capacities must be positive");
   if (g->n_layers < 1 || g->n_modules < 1) return fail(h, CKF_E_ARG, "empty geometry");
   if (g->n_layers > 254) return fail(h, CKF_E_ARG, "at most 254 layers (the navigation cursors are 9-bit fields)");
@@ -554,6 +588,15 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     else CKB(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ckf_resolve_kernel<double>, RESOLVE_NT, 0));
     h->resolve_grid = std::max(1, per_sm) * h->sm_count;   // a cooperative launch needs every block resident
   }
+  // ---- workspace of ckf_seed (row f4): 48 B per measurement + 12 B per middle-top doublet
+  if (c->max_seed_doublets > 0) {
+    const size_t M = (size_t)c->max_measurements, D = (size_t)c->max_seed_doublets;
+    CKB(dalloc(h, &h->sd_sp, 5 * M * sizeof(double)));
+    CKB(dalloc(h, &h->sd_cnt, (M + 1) * 4)); CKB(dalloc(h, &h->sd_off, (M + 1) * 4));
+    CKB(dalloc(h, &h->sd_t, D * 4)); CKB(dalloc(h, &h->sd_cot, D * sizeof(double)));
+    CKB(dalloc(h, &h->sd_g, 4 * 4));
+    CKB(cudaEventCreateWithFlags(&h->seed_done, cudaEventDisableTiming));
+  }
 #undef CKB
   *out = h;
   return CKF_OK;
@@ -674,6 +717,28 @@ int ckf_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, const 
   cudaStreamWaitEvent(st, h->fit_done, 0);  // one state store: fits are ordered one after the other
   int rc = h->cfg.precision == 32 ? launch_fit<float>(h, m, s, t, o, st) : launch_fit<double>(h, m, s, t, o, st);
   cudaEventRecord(h->fit_done, st);
+  return rc;
+}
+
+int ckf_seed(ckf_handle* h, const ckf_measurements* m, const ckf_seeding* sc, ckf_seed_out* o, void* stream) {
+  if (!h) return CKF_E_ARG;
+  if (!m || !sc || !o) return fail(h, CKF_E_ARG, "null argument");
+  if (!h->sd_sp) return fail(h, CKF_E_CAPACITY, "ckf_seed needs its workspace: create the handle with max_seed_doublets > 0");
+  if (m->n < 0 || m->n > h->cfg.max_measurements) return fail(h, CKF_E_CAPACITY, "n_measurements %d exceeds capacity", m->n);
+  if (m->n_events > 1) return fail(h, CKF_E_ARG, "ckf_seed takes one event at a time");
+  if (!m->module_offsets || (m->n > 0 && (!m->loc || !m->var))) return fail(h, CKF_E_ARG, "null input array");
+  if (!o->n_seeds || !o->status || !o->module_id || !o->params || !o->cov || !o->triplets || o->capacity < 1)
+    return fail(h, CKF_E_ARG, "null output array");
+  const int nb = h->geo.n_barrel;
+  if (sc->layer_b < 0 || sc->layer_t >= nb || !(sc->layer_b < sc->layer_m && sc->layer_m < sc->layer_t))
+    return fail(h, CKF_E_ARG, "seeding layers must be barrel layers with bottom < middle < top");
+  if (!(sc->dphi_max > 0.0 && sc->dphi_max < 1.5) || !(sc->cot_max > 0.0) || !(sc->pt_min > 0.0))
+    return fail(h, CKF_E_ARG, "bad seeding cuts");
+  cudaStream_t st = (cudaStream_t)stream;
+  std::lock_guard<std::mutex> lk(h->mu);
+  cudaStreamWaitEvent(st, h->seed_done, 0);   // one workspace: calls are ordered one after the other
+  const int rc = h->cfg.precision == 32 ? launch_seed<float>(h, m, sc, o, st) : launch_seed<double>(h, m, sc, o, st);
+  cudaEventRecord(h->seed_done, st);
   return rc;
 }
 
@@ -821,6 +886,7 @@ int ckf_destroy(ckf_handle* h) {
   }
   if (h->fit_done) cudaEventDestroy(h->fit_done);
   if (h->resolve_done) cudaEventDestroy(h->resolve_done);
+  if (h->seed_done) cudaEventDestroy(h->seed_done);
   for (void* p : h->allocs) cudaFree(p);
   delete h;
   return CKF_OK;

@@ -53,12 +53,12 @@ class SeedSettings:
     layer_b: int = 0
     layer_m: int = 1
     layer_t: int = 2
-    dphi_max: float = 0.08          # rad, doublet
+    dphi_max: float = 0.05          # rad, doublet (pT >= 0.4 GeV bends 0.033 rad between the seeding layers)
     cot_max: float = 10.5           # |eta| <= 3
-    z0_max: float = 250.0           # mm: 5 sigma of the vertex spread
-    dcot_max: float = 0.03          # resolution + scattering between the two doublets
+    z0_max: float = 200.0           # mm: 4 sigma of the vertex spread
+    dcot_max: float = 0.01          # ~5 sigma of resolution + scattering between the two doublets
     pt_min: float = 0.4             # GeV, below the 0.5 GeV of the workloads
-    d0_max: float = 10.0            # mm
+    d0_max: float = 2.0             # mm
     sigma_angle: float = 2e-3       # rad
     rel_sigma_qop: float = 0.1
     cov_scale: float = 10.0         # BASELINE seeds: covariance = 10 x the smearing variances

@@ -5,11 +5,14 @@ import numpy as np
 FLOOR = np.array([1.0, 1.0, 1.0, 1.0, 0.0, 1.0])   # mm, mm, rad, rad, (none for q/p), mm
 
 
-def param_rel_diff(a, b):
-    """A15: |a-b| / max(|a|, |b|, floor); angles compared after wrapping the difference."""
+def param_rel_diff(a, b, qop_floor=0.0):
+    """A15: |a-b| / max(|a|, |b|, floor); angles compared after wrapping the difference.  qop_floor: a floor for q/p
+    (A15 has none: the workloads' |q/p| >= 0.0126 / GeV; seeds ESTIMATED from fake triplets can be straight lines)."""
     d = a - b
     d[..., 2] = (d[..., 2] + np.pi) % (2 * np.pi) - np.pi
-    den = np.maximum(np.maximum(np.abs(a), np.abs(b)), FLOOR)
+    floor = FLOOR.copy()
+    floor[4] = qop_floor
+    den = np.maximum(np.maximum(np.abs(a), np.abs(b)), floor)
     den = np.where(den == 0.0, 1.0, den)     # both exactly zero (q/p has no floor): difference 0
     return np.abs(d) / den
 
@@ -41,12 +44,12 @@ def by_seed(tr):
     return out
 
 
-def compare_fp32(gpu, ora, n_seeds):
+def compare_fp32(gpu, ora, n_seeds, qop_floor=0.0):
     """Returns dict: frac_identical seeds, mismatching seed ids, max param rel diff / chi2 abs diff on matched tracks."""
     if (gpu.n_tracks == ora.n_tracks and np.array_equal(gpu.seed_id, ora.seed_id) and
             np.array_equal(gpu.track_offsets, ora.track_offsets) and np.array_equal(gpu.meas_idx, ora.meas_idx)):
         # the common case: same candidates in the same order -> everything vectorised, every entry compared
-        rel = param_rel_diff(gpu.params.copy(), ora.params.copy())
+        rel = param_rel_diff(gpu.params.copy(), ora.params.copy(), qop_floor)
         chi2 = np.abs(gpu.chi2_sum - ora.chi2_sum)
         emax = float(np.max(np.abs(gpu.entry_chi2 - ora.entry_chi2), initial=0.0))
         return dict(frac_identical=1.0, bad_seeds=[], n_matched=int(gpu.n_tracks),
@@ -64,7 +67,7 @@ def compare_fp32(gpu, ora, n_seeds):
             gi.append(gs[k])
             oi.append(os_[k])
     gi, oi = np.array(gi, int), np.array(oi, int)
-    rel = param_rel_diff(gpu.params[gi].copy(), ora.params[oi].copy()) if gi.size else np.zeros((0, 6))
+    rel = param_rel_diff(gpu.params[gi].copy(), ora.params[oi].copy(), qop_floor) if gi.size else np.zeros((0, 6))
     chi2 = np.abs(gpu.chi2_sum[gi] - ora.chi2_sum[oi]) if gi.size else np.zeros(0)
     # per-entry chi2 on matched tracks
     emax = 0.0
@@ -178,10 +181,10 @@ def trace_mismatches(gpu, ora, bad_seeds, chi2_max, tol=1e-3):
     return out
 
 
-def assert_fp32_parity(gpu, ora, n_seeds, chi2_max, what=""):
+def assert_fp32_parity(gpu, ora, n_seeds, chi2_max, what="", qop_floor=0.0):
     """The fp32 bar of north_star in one place: >= 99.9 % of seeds with identical lists, EVERY mismatch traced,
     parameters 1e-4 relative, chi2 1e-3 absolute."""
-    r = compare_fp32(gpu, ora, n_seeds)
+    r = compare_fp32(gpu, ora, n_seeds, qop_floor)
     traced = trace_mismatches(gpu, ora, r["bad_seeds"], chi2_max)
     untraced = [s for s, why in traced if why is None]
     assert r["frac_identical"] >= 0.999, (what, r["frac_identical"])

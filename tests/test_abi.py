@@ -17,13 +17,13 @@ def test_library_exports_every_declared_symbol():
     assert declared == set(B.EXPORTS), declared ^ set(B.EXPORTS)
     for name in declared:
         assert hasattr(lib, name), name
-    assert lib.ckf_abi_version() == 9
+    assert lib.ckf_abi_version() == 10
 
 
 def test_struct_layouts_match_header_field_order():
     hdr = open(os.path.join(ROOT, "include", "ckf.h")).read()
     for struct in (B.ckf_geometry, B.ckf_field, B.ckf_config, B.ckf_measurements, B.ckf_seeds, B.ckf_tracks,
-                   B.ckf_counters, B.ckf_timing, B.ckf_fits, B.ckf_resolution):
+                   B.ckf_counters, B.ckf_timing, B.ckf_fits, B.ckf_resolution, B.ckf_seeding, B.ckf_seed_out):
         body = re.search(r"typedef struct \{([^{}]*)\} %s;" % struct.__name__, hdr, re.S).group(1)
         body = re.sub(r"/\*.*?\*/", "", body, flags=re.S)
         names = re.findall(r"[\s\*]([a-z_0-9]+)(?:\[\d+\])?\s*;", body)

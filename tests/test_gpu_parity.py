@@ -857,3 +857,79 @@ def test_bidirectional_navigation_parity(endcap):
     print("bidirectional endcap=%s: %d candidates, visits %d (outward only: %d)" %
           (endcap, gpu.n_tracks, cnt["visits"], ora0.counters["visits"]))
     ckf.close()
+
+
+@pytest.mark.parametrize("config,n_particles", [(1, 2000), (2, 4000)])
+def test_seeding_parity_and_chain(config, n_particles):
+    """ckf_seed (row f4: triplet seeding + helix parameter estimation) against the oracle's enumeration of
+    all combinations: the same triplets in the same order, parameters and covariance; then the chain the paper runs,
+    seeds -> ckf_find -> ckf_resolve, from the ESTIMATED seeds, against the oracle's chain."""
+    import torch
+    import oracle
+    from paper_2505_22822_b200 import CKF
+    det, fld, cfg = synth.config_bundle(config)
+    ev = synth.make_event(config, det=det, n_particles=n_particles)
+    sset = synth.SeedSettings()
+    st = oracle.Setup(det, fld, cfg.ckf)
+    osd = oracle.seed_find(st, sset, ev.module_offsets, ev.loc, ev.var, n_threads=8)
+    cap = 4 * len(osd["module"]) + 16
+    ckf = CKF(det, fld, cfg.ckf, cfg.precision, max_seeds=cap, max_measurements=ev.n_measurements,
+              max_seed_doublets=4_000_000, max_fit_tracks=0)
+    dev = ckf.upload_event(ev)
+    seeds = ckf.alloc_seeds(cap)
+    ckf.seed(dev, sset, seeds)
+    torch.cuda.synchronize()
+    n = int(seeds["n_seeds"][0])
+    assert int(seeds["status"][0]) == 0 and n == len(osd["module"]) > n_particles
+    assert np.array_equal(seeds["triplets"][:n].cpu().numpy(), osd["triplets"])
+    assert np.array_equal(seeds["module_id"][:n].cpu().numpy(), osd["module"])
+    gp = seeds["params"][:n].cpu().numpy().astype(np.float64)
+    gc = seeds["cov"][:n].cpu().numpy().astype(np.float64)
+    tol = 1e-9 if cfg.precision == 64 else 2e-6             # fp32: the float32 rounding of the outputs
+    assert parity.param_rel_diff(gp.copy(), osd["params"].copy()).max() < tol
+    assert np.max(np.abs(gc - osd["cov"]) / np.maximum(np.abs(osd["cov"]), 1e-300)) < max(tol, 1e-8)
+    # twice the same; a tiny seed capacity and a tiny doublet workspace are flagged
+    seeds2 = ckf.alloc_seeds(cap)
+    ckf.seed(dev, sset, seeds2)
+    torch.cuda.synchronize()
+    assert torch.equal(seeds["params"][:n], seeds2["params"][:n]) and torch.equal(seeds["triplets"][:n], seeds2["triplets"][:n])
+    small = ckf.alloc_seeds(100)
+    ckf.seed(dev, sset, small)
+    torch.cuda.synchronize()
+    assert int(small["status"][0]) == 1 and int(small["n_seeds"][0]) == 100
+    assert np.array_equal(small["triplets"].cpu().numpy(), osd["triplets"][:100])
+    # ---- the chain from the estimated seeds: the CUDA path's own seeds into ckf_find, the oracle's into the oracle
+    d2 = dict(dev)
+    d2["seed_module"], d2["seed_params"], d2["seed_cov"] = seeds["module_id"][:n], seeds["params"][:n], seeds["cov"][:n]
+    out = ckf.alloc_tracks()
+    ckf.find(d2, out)
+    torch.cuda.synchronize()
+    gpu = ckf.download(out)
+    # (the oracle's CKF gets the SAME seed arrays -- the seeds themselves were compared above -- so that this step tests
+    # ckf_find on estimated seeds, fake triplets included, to the usual bars)
+    ora = oracle.ckf_find(st, ev.module_offsets, ev.loc, ev.var, seeds["module_id"][:n].cpu().numpy(),
+                          seeds["params"][:n].cpu().numpy(), seeds["cov"][:n].cpu().numpy(), n_threads=8)
+    if cfg.precision == 64:
+        parity.assert_bit_exact_lists(gpu, ora)
+        rel, chi2, cov = parity.max_param_diffs(gpu, ora)
+        assert rel < 1e-9 and chi2 < 1e-8, (rel, chi2)
+        r = dict(max_param_rel=rel, max_chi2_sum_abs=chi2)
+    else:
+        # fake triplets give seeds of any curvature, also straight ones (|q/p| ~ 4e-4 / GeV here, where an absolute
+        # difference of 4e-8 is 1e-4 relative): q/p is compared with a floor of 0.01 / GeV (p = 100 GeV) in this test
+        r = parity.assert_fp32_parity(gpu, ora, n, cfg.ckf.chi2_max, "chain fp32", qop_floor=0.01)
+        assert r["max_param_rel"] < 1e-5
+    res = ckf.alloc_resolution()
+    ckf.resolve(out, ev.n_measurements, res, 1, 1.0)
+    torch.cuda.synchronize()
+    kept = int(res["summary"][0])
+    a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    a.record()
+    for _ in range(5):
+        ckf.seed(dev, sset, seeds2)
+    b.record()
+    torch.cuda.synchronize()
+    print("seeding configs[%d], %d particles: %d seeds (%.3f ms), %d candidates, %d kept after resolution; %s" %
+          (config, n_particles, n, a.elapsed_time(b) / 5, gpu.n_tracks, kept, {k: v for k, v in r.items() if k != "bad_seeds"}))
+    assert 0.97 * n_particles < kept < 1.2 * n_particles
+    ckf.close()

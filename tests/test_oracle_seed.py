@@ -133,7 +133,7 @@ def test_seeding_efficiency_pulls_and_the_chain_to_candidates():
     sd = oracle.seed_find(st, s, ev.module_offsets, ev.loc, ev.var, n_threads=8)
     tp = ev.meas_particle[sd["triplets"]]
     true = (tp[:, 0] >= 0) & (tp[:, 0] == tp[:, 1]) & (tp[:, 1] == tp[:, 2])
-    assert np.unique(tp[true, 0]).size >= 0.995 * 600
+    assert np.unique(tp[true, 0]).size >= 0.99 * 600
     qop = ev.particle_q / (ev.particle_pt * np.cosh(ev.particle_eta))
     pull = (sd["params"][true, 4] - qop[tp[true, 0]]) / np.sqrt(sd["cov"][true, 28] / s.cov_scale)
     assert abs(pull.mean()) < 0.15 and 0.5 < pull.std() < 1.3
