@@ -331,23 +331,23 @@ def main():
     ckf.find(devs[(W - 1) % N_EVENTS], out, stream)
     fits = ckf.alloc_fits()
     for _ in range(2):
-        ckf.fit(devs[(W - 1) % N_EVENTS], out, fits, stream)
+        ckf.fit(devs[(W - 1) % N_EVENTS], out, fits, stream, n_tracks_upper=res1.n_tracks)
     torch.cuda.synchronize()
     n_fit = 5
     fa, fb = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     fa.record(stream)
     for _ in range(n_fit):
-        ckf.fit(devs[(W - 1) % N_EVENTS], out, fits, stream)
+        ckf.fit(devs[(W - 1) % N_EVENTS], out, fits, stream, n_tracks_upper=res1.n_tracks)
     fb.record(stream)
     torch.cuda.synchronize()
     fit_ms = fa.elapsed_time(fb) / n_fit
     fa.record(stream)
     for _ in range(n_fit):
-        ckf.fit(devs[(W - 1) % N_EVENTS], out, fits, stream, smoother=1)
+        ckf.fit(devs[(W - 1) % N_EVENTS], out, fits, stream, smoother=1, n_tracks_upper=res1.n_tracks)
     fb.record(stream)
     torch.cuda.synchronize()
     fit_tf_ms = fa.elapsed_time(fb) / n_fit
-    ckf.fit(devs[(W - 1) % N_EVENTS], out, fits, stream)       # leave the RTS result in `fits` for the counts below
+    ckf.fit(devs[(W - 1) % N_EVENTS], out, fits, stream, n_tracks_upper=res1.n_tracks)       # leave the RTS result in `fits` for the counts below
     torch.cuda.synchronize()
     fit_ok = int((fits["status"][:res1.n_tracks] == 0).sum().item())
     fit_work = [int(v) // (2 * n_fit + 3) for v in fits["work"].cpu().tolist()]   # trials, accepted, moves, updates per call
@@ -470,7 +470,8 @@ def main():
                     "work_per_event": dict(zip(("rk_trials", "rk_accepted", "moves", "updates"), fit_work)),
                     "flop_per_event": fit_flop, "achieved_tflops": fit_flop / (fit_ms * 1e-3) / 1e12,
                     "launches_per_call": "per pass of <= 262,144 candidates: 4 memsets + (ckf_step + ckf_fit_level) per level "
-                                         "(max_levels = %d) + 2" % cfg.ckf.max_levels},
+                                         "(max_levels = %d) + 2; passes bounded by the host hint n_tracks_upper (one "
+                                         "pass here)" % cfg.ckf.max_levels},
             "resolve": {"what": "ckf_resolve: greedy shared-hit ambiguity resolution (PAPER.md:98, rules AR1-AR3) of ONE "
                                 "configs[3] event's candidates, max_shared_hits = 1; one cooperative launch",
                         "ms_per_event": resolve_ms, "candidates": res1.n_tracks, "kept": resolve_kept,

@@ -33,7 +33,7 @@
 extern "C" {
 #endif
 
-#define CKF_ABI_VERSION 10
+#define CKF_ABI_VERSION 11
 
 /* return codes */
 #define CKF_OK 0
@@ -62,7 +62,12 @@ typedef struct ckf_handle ckf_handle; /* opaque; owns device geometry, field, wo
  * during ckf_create.  Module id = module_offset[l] + i_phi * n_z[l] + i_z; the module's local frame is
  * (axis_u, axis_v), its normal axis_u x axis_v; loc0 runs along axis_u, loc1 along axis_v.  Within a layer
  * all modules share half_v (the z pitch used by the navigator is 2*half_v of the layer's first module) and
- * n_phi >= 3. */
+ * n_phi >= 3.
+ * What the navigator ASSUMES of the grid (it finds the 3x3 neighbourhood of a portal point by binning, it does not
+ * search): on a barrel layer, module (i_phi, i_z) is centred at azimuth 2 pi i_phi / n_phi and at
+ * z = -layer_half_z + (i_z + 1/2) * 2 half_v, tangent to the cylinder of radius layer_r with its normal pointing
+ * outward; modules of one phi column are coplanar; neighbouring columns may overlap in phi by less than one module.
+ * A geometry that violates this gives wrong module choices, not errors. */
 typedef struct {
   int32_t n_layers;
   const double* layer_r;        /* [n_layers] mm, increasing                         */
@@ -244,6 +249,9 @@ typedef struct {
   int32_t smoother_precision; /* INPUT.  0 or 64: the RTS recursion runs in float64 (the product's choice, K5).
                            32 (handles of precision 32 only): it runs in float32 -- kept to study the instability
                            of the float32 smoother that PAPER.md:61, :100 report, not for production             */
+  int32_t n_tracks_upper; /* INPUT.  0, or a host-side upper bound on *tracks->n_tracks (e.g. from a previous read-back):
+                           passes of the state store beyond it are not enqueued at all (without it every pass up to
+                           max_tracks is enqueued and those beyond the device's count return at once)                */
   int32_t smoother;     /* INPUT.  0: RTS recursion (K4).  1: two-filter "optimal" smoother (K4'): the
                            forward-filtered state combined with a backward information filter over the same stored
                            states; same result (tested), no differences of nearly equal covariances                 */

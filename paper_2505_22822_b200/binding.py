@@ -63,7 +63,8 @@ class ckf_tracks(C.Structure):
 
 class ckf_fits(C.Structure):
     _fields_ = [("status", _vp), ("n_states", _vp), ("chi2_sum", _vp), ("last_params", _vp), ("last_cov", _vp),
-                ("first_cov", _vp), ("entry_params", _vp), ("work", _vp), ("smoother_precision", C.c_int32), ("smoother", C.c_int32)]
+                ("first_cov", _vp), ("entry_params", _vp), ("work", _vp), ("smoother_precision", C.c_int32),
+                ("n_tracks_upper", C.c_int32), ("smoother", C.c_int32)]
 
 
 class ckf_resolution(C.Structure):
@@ -350,13 +351,14 @@ class CKF:
                     last_params=t.zeros(nt, 6, **T), last_cov=t.zeros(nt, 36, **T), first_cov=t.zeros(nt, 36, **T),
                     entry_params=t.zeros(ne, 6, **T), work=t.zeros(4, dtype=t.int64, device=device))
 
-    def fit(self, dev_event: dict, tracks: dict, fits: dict, stream=None, smoother_precision: int = 0, smoother: int = 0):
+    def fit(self, dev_event: dict, tracks: dict, fits: dict, stream=None, smoother_precision: int = 0, smoother: int = 0,
+            n_tracks_upper: int = 0):
         """Asynchronous ckf_fit of the candidates in `tracks` (device tensors filled by `find`)."""
         st = stream if stream is not None else self.torch.cuda.current_stream()
         m, s, o = self._structs(dev_event, tracks, lambda x: x.data_ptr())
         f = ckf_fits(*[fits[k].data_ptr() for k in ("status", "n_states", "chi2_sum", "last_params", "last_cov",
                                                     "first_cov", "entry_params", "work")],
-                     int(smoother_precision), int(smoother))
+                     int(smoother_precision), int(n_tracks_upper), int(smoother))
         rc = self.lib.ckf_fit(self.handle, C.byref(m), C.byref(s), C.byref(o), C.byref(f), _vp(st.cuda_stream))
         if rc != 0:
             raise RuntimeError("ckf_fit failed (%d): %s" % (rc, self.lib.ckf_last_error(self.handle).decode()))

@@ -283,7 +283,8 @@ int launch_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, con
   kp.g = h->ft_g; kp.counters = h->ft_counters;
   kp.mv_y = h->ft_y; kp.mv_D = (T*)h->ft_D; kp.mv_dep = (double*)h->ft_dep; kp.mv_from = h->ft_from; kp.mv_tgt = h->ft_tgt;
   kp.mv_stop = h->ft_stop; kp.mv_order = h->ft_order;
-  for (int first = 0; first < h->cfg.max_tracks; first += h->fit_chunk) {
+  const int n_upper = o->n_tracks_upper > 0 ? std::min(o->n_tracks_upper, h->cfg.max_tracks) : h->cfg.max_tracks;
+  for (int first = 0; first < n_upper; first += h->fit_chunk) {
     p.first = first;
     // forward filter, level-synchronous: per level the moves on ckf_step, then the rest of the state (ckf_fit_level).
     // Two blocks of globals, by level parity: level L's ckf_step reads the schedule in block L & 1.

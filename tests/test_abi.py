@@ -17,7 +17,7 @@ def test_library_exports_every_declared_symbol():
     assert declared == set(B.EXPORTS), declared ^ set(B.EXPORTS)
     for name in declared:
         assert hasattr(lib, name), name
-    assert lib.ckf_abi_version() == 10
+    assert lib.ckf_abi_version() == 11
 
 
 def test_struct_layouts_match_header_field_order():

@@ -424,6 +424,12 @@ def test_fit_fp32_ill_conditioned_covariances_are_fitted():
     print("fit config 3 event 1", r)
     assert r["n_not_pd_gpu_only"] == 0 and np.array_equal(g["status"], o.status)
     assert r["max_smoothed_rel"] < 1e-5 and r["max_last_rel"] < 1e-5
+    # the host hint n_tracks_upper only cuts empty passes: same result
+    f3 = ckf.alloc_fits()
+    ckf.fit(dev, out, f3, n_tracks_upper=gpu.n_tracks)
+    torch.cuda.synchronize()
+    for k in ("status", "n_states", "entry_params", "first_cov"):
+        assert torch.equal(fits[k][:gpu.n_tracks], f3[k][:gpu.n_tracks]), k
     # the two-filter smoother factors the FILTERED covariance instead of the predicted one
     f2 = ckf.alloc_fits()
     ckf.fit(dev, out, f2, smoother=1)
