@@ -82,9 +82,12 @@ CKF_HD auto dot3(const A a[3], const B b[3]) -> decltype(a[0] * b[0]) {
 struct D3 { double x, y, z; };
 CKF_HD D3 ld_node(const double* p) {
 #if defined(__CUDA_ARCH__)
-  const double2 a = __ldg((const double2*)p);
-  const double b = __ldg(p + 2);
-  return D3{a.x, a.y, b};
+  // one 256-bit load per node (sm_100a: LDG.E.256): the node is a 32-byte-aligned sector of 4 doubles.  Against a
+  // 128-bit + a 64-bit load this halves the load instructions and the L1 wavefronts of the field read, the busiest
+  // unit of ckf_step (l1tex data-pipe wavefronts 62 % of peak, profiles/r02_step_visit_update.md)
+  double x, y, z, w;
+  asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(x), "=d"(y), "=d"(z), "=d"(w) : "l"(p));
+  return D3{x, y, z};
 #else
   return D3{p[0], p[1], p[2]};
 #endif

@@ -939,3 +939,51 @@ def test_seeding_parity_and_chain(config, n_particles):
           (config, n_particles, n, a.elapsed_time(b) / 5, gpu.n_tracks, kept, {k: v for k, v in r.items() if k != "bad_seeds"}))
     assert 0.97 * n_particles < kept < 1.2 * n_particles
     ckf.close()
+
+
+def test_fp64_parity_over_many_events():
+    """Round 2 found the fp32 chi2 bar broken on events round 1 had not sampled; the fp64 claim (bit-exact lists, equal
+    counters, 1e-9) is therefore checked on a dozen further configs[1] events, and the general navigation (discs,
+    bidirectional, energy loss together) on three endcap events."""
+    import copy
+    import torch
+    import oracle
+    from paper_2505_22822_b200 import CKF
+    from synth.events import CKFSettings
+    det, fld, cfg = synth.config_bundle(1)
+    st = oracle.Setup(det, fld, cfg.ckf)
+    evs = [synth.make_event(1, event_index=i, det=det) for i in range(1, 13)]
+    ckf = CKF(det, fld, cfg.ckf, 64, max_seeds=max(e.n_seeds for e in evs), max_measurements=max(e.n_measurements for e in evs),
+              max_fit_tracks=0)
+    out = ckf.alloc_tracks()
+    worst = 0.0
+    for ev in evs:
+        ckf.find(ckf.upload_event(ev), out)
+        torch.cuda.synchronize()
+        gpu, cnt = ckf.download(out), ckf.counters()
+        ora = oracle.find_event(st, ev, n_threads=8)
+        parity.assert_bit_exact_lists(gpu, ora)
+        rel, chi2, cov = parity.max_param_diffs(gpu, ora)
+        assert rel < 1e-9 and chi2 < 1e-8 and cov < 1e-7, (ev.event_index, rel, chi2, cov)
+        for k in ("visits", "rk_trials", "rk_accepted", "gate_tests", "updates", "tips"):
+            assert cnt[k] == ora.counters[k], (ev.event_index, k)
+        worst = max(worst, rel)
+    ckf.close()
+    det = synth.build_detector(half_z=500.0, disc_z=ENDCAP_DISC_Z)
+    cks = CKFSettings(max_branches_per_surface=5, max_candidates_per_seed=50, bidirectional=1, energy_loss=1)
+    st = oracle.Setup(det, synth.uniform_field(), cks)
+    for seed in (101, 102, 103):
+        ev = synth.make_endcap_event(det, 2500, seed=seed, n_fake_seeds=800)
+        ckf = CKF(det, synth.uniform_field(), cks, 64, max_seeds=ev.n_seeds, max_measurements=ev.n_measurements, max_fit_tracks=0)
+        out = ckf.alloc_tracks()
+        ckf.find(ckf.upload_event(ev), out)
+        torch.cuda.synchronize()
+        gpu, cnt = ckf.download(out), ckf.counters()
+        ora = oracle.find_event(st, ev, n_threads=8)
+        parity.assert_bit_exact_lists(gpu, ora)
+        rel, chi2, cov = parity.max_param_diffs(gpu, ora)
+        assert rel < 1e-9 and chi2 < 1e-8 and cov < 1e-7, (seed, rel, chi2, cov)
+        for k in ("visits", "rk_trials", "rk_accepted", "gate_tests", "updates", "tips"):
+            assert cnt[k] == ora.counters[k], (seed, k)
+        ckf.close()
+    print("fp64 over 12 configs[1] events and 3 endcap events (discs + bidirectional + energy loss): worst param rel %.1e" % worst)
