@@ -215,7 +215,7 @@ __device__ __forceinline__ int find_parent_warp(const KParams<T>& p, int n, int 
 }
 template <typename T>
 #ifndef CKF_UPDATE_MINB
-#define CKF_UPDATE_MINB 3
+#define CKF_UPDATE_MINB 2
 #endif
 __global__ void __launch_bounds__(SCAN_NT, CKF_UPDATE_MINB) ckf_update(const KParams<T> p, int level) {
   const int n = p.g[G_NTIPS0 + (level & 1)];
