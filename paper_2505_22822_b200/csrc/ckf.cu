@@ -68,8 +68,9 @@ struct Workspace {
   // recycles the workspace for another stream waits (on the host) until the previous owner has finished ENQUEUING and
   // then (on the device, cudaStreamWaitEvent) until that work has finished RUNNING.  `done_stream` is written under busy.
   std::mutex busy;
-  void* done_stream = nullptr;
-  bool done_valid = false;
+  std::atomic<void*> done_stream{nullptr};
+  std::atomic<bool> done_valid{false};
+  std::atomic<bool> enqueuing{false};  // a host thread is between acquire_ws and release_ws (hint for others_in_flight)
   void* stream_tag = nullptr;
   bool used = false;
   float last_ms[10] = {0};  // per-kernel-kind times of the last timed ckf_find (ckf_set_timing)
@@ -113,6 +114,11 @@ struct ckf_handle {
   int32_t *sd_cnt = nullptr, *sd_off = nullptr, *sd_t = nullptr, *sd_g = nullptr;
   cudaEvent_t seed_done = nullptr;
   bool timing_print = false;
+  // which kernels of a find are launched with overlap (launch_chain): bit 1 sort, 2 step, 4 visit, 8 scan, 16 update,
+  // 32 emission, 64 ckf_fit_level.  Measured (profiles/r02_launch_overlap.md): step + visit + update is best; with ckf_scan in the chain as
+  // well the whole level loop is one cascade of waiting blocks and a batched find gets 10 % slower.  CKF_CHAIN_OVERLAP=<mask>
+  // overrides (0 = plain launches), for A/B measurements.
+  int chain_overlap = 2 | 4 | 16 | 64;
   bool timing = false;  // ckf_set_timing / CKF_TIMING=1: per-kernel CUDA-event times of every ckf_find on stderr (debug aid; synchronises)
 };
 
@@ -189,6 +195,34 @@ void fill_params(ckf_handle* h, Workspace& w, KParams<T>& p) {
   p.o_summary = nullptr;
 }
 
+// One kernel of a find's chain.  With `overlap` the launch carries programmatic stream serialisation: the kernel's blocks
+// become resident while the previous kernel of the stream drains and wait in chain_enter() for its completion, which
+// takes the launch latency out of the ~136 dependent launches of a find.
+template <typename... KArgs, typename... Args>
+void launch_chain(void (*kernel)(KArgs...), int grid, int block, size_t smem, cudaStream_t st, bool overlap, Args&&... args) {
+  cudaLaunchConfig_t lc = {};
+  lc.gridDim = dim3((unsigned)grid); lc.blockDim = dim3((unsigned)block); lc.dynamicSmemBytes = smem; lc.stream = st;
+  cudaLaunchAttribute at[1];
+  at[0].id = cudaLaunchAttributeProgrammaticStreamSerialization;
+  at[0].val.programmaticStreamSerializationAllowed = 1;
+  lc.attrs = at; lc.numAttrs = overlap ? 1 : 0;
+  cudaLaunchKernelEx(&lc, kernel, KArgs(args)...);
+}
+
+// Is a find of this handle being enqueued or still running on ANOTHER stream (work of `st` itself is ordered before
+// whatever is enqueued next, never beside it)?  A hint, read without locks: it only selects the launch policy.
+bool others_in_flight(ckf_handle* h, const Workspace* self, cudaStream_t st) {
+  for (auto& o : h->ws) {
+    if (&o == self) continue;
+    if (o.enqueuing.load()) return true;
+    if (o.done_valid.load() && o.done_stream.load() != (void*)st && cudaEventQuery(o.done) == cudaErrorNotReady) {
+      (void)cudaGetLastError();  // 'not ready' is an answer, not an error of this call
+      return true;
+    }
+  }
+  return false;
+}
+
 template <typename T>
 int launch_find(ckf_handle* h, Workspace& w, const ckf_measurements* m, const ckf_seeds* s, ckf_tracks* o,
                 cudaStream_t st, int32_t* summary = nullptr) {
@@ -217,20 +251,25 @@ int launch_find(ckf_handle* h, Workspace& w, const ckf_measurements* m, const ck
     tkind.push_back(kind);
   };
   mark(-1);
-  ckf_init_event<T><<<nb, 256, 0, st>>>(p); mark(0);
-  ckf_sort_slices<T><<<h->sm_count * 8, SORT_NT, 0, st>>>(p); mark(1);
+  // Launch policy.  Alone on the GPU a find is a chain of ~70 short dependent kernels and overlapped launches take the
+  // launch latency out of it (3.70 -> 3.45 ms).  With other finds in flight the SMs are shared, blocks that sit resident
+  // waiting for their predecessor take room from the other streams' kernels (2 batches in flight: 20.4 -> 19.2 M
+  // seeds/s), so the launches stay plain.  Timing mode puts an event between the kernels, which serialises them anyway.
+  const int ovm = (h->timing || others_in_flight(h, &w, st)) ? 0 : h->chain_overlap;
+  ckf_init_event<T><<<nb, 256, 0, st>>>(p); mark(0);  // plain launch: whatever precedes the find in the stream is not ours
+  launch_chain(ckf_sort_slices<T>, h->sm_count * 8, SORT_NT, 0, st, ovm & 1, p); mark(1);
   // level loop: tips of level l were made by level l - 1; a tip at max_levels only stops (LEVEL_LIMIT) and emits.
   // Kernels of an empty level return at once, so the loop needs no host read of the level's size.
   const int wide = h->sm_count * 4;
   for (int level = 0; level <= h->cfg.max_levels; ++level) {
-    if (level > 0) { ckf_step<T, MinBlocks<T>::value><<<h->step_grid, STEP_NT, 0, st>>>(p, level); mark(2); }
-    ckf_visit<T, VisitBlocks<T>::value><<<h->visit_grid, VISIT_NT, h->visit_smem, st>>>(p, level); mark(3);
-    ckf_scan<T><<<wide, SCAN_NT, 0, st>>>(p, level); mark(5);
-    ckf_update<T><<<wide, SCAN_NT, 0, st>>>(p, level); mark(6);
+    if (level > 0) { launch_chain(ckf_step<T, MinBlocks<T>::value>, h->step_grid, STEP_NT, 0, st, ovm & 2, p, level); mark(2); }
+    launch_chain(ckf_visit<T, VisitBlocks<T>::value>, h->visit_grid, VISIT_NT, h->visit_smem, st, ovm & 4, p, level); mark(3);
+    launch_chain(ckf_scan<T>, wide, SCAN_NT, 0, st, ovm & 8, p, level); mark(5);
+    launch_chain(ckf_update<T>, wide, SCAN_NT, 0, st, ovm & 16, p, level); mark(6);
   }
-  ckf_scan_seeds<T><<<(s->n + SEED_TILE - 1) / SEED_TILE + 1, SEED_TILE, 0, st>>>(p); mark(7);
-  ckf_emit_tracks<T><<<h->sm_count * 4, 256, 0, st>>>(p); mark(8);
-  ckf_finalize<T><<<1, 1, 0, st>>>(p); mark(9);
+  launch_chain(ckf_scan_seeds<T>, (s->n + SEED_TILE - 1) / SEED_TILE + 1, SEED_TILE, 0, st, ovm & 32, p); mark(7);
+  launch_chain(ckf_emit_tracks<T>, h->sm_count * 4, 256, 0, st, ovm & 32, p); mark(8);
+  launch_chain(ckf_finalize<T>, 1, 1, 0, st, ovm & 32, p); mark(9);
   w.last_launches = 5 + 4 * (h->cfg.max_levels + 1) - 1;
   if (h->timing) {
     static const char* names[10] = {"init", "sort", "step", "visit", "cap", "scan", "update", "scan_seeds", "emit", "finalize"};
@@ -284,6 +323,7 @@ int launch_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, con
   kp.mv_y = h->ft_y; kp.mv_D = (T*)h->ft_D; kp.mv_dep = (double*)h->ft_dep; kp.mv_from = h->ft_from; kp.mv_tgt = h->ft_tgt;
   kp.mv_stop = h->ft_stop; kp.mv_order = h->ft_order;
   const int n_upper = o->n_tracks_upper > 0 ? std::min(o->n_tracks_upper, h->cfg.max_tracks) : h->cfg.max_tracks;
+  const int ovm = others_in_flight(h, nullptr, st) ? 0 : h->chain_overlap;  // launch policy as in launch_find
   for (int first = 0; first < n_upper; first += h->fit_chunk) {
     p.first = first;
     // forward filter, level-synchronous: per level the moves on ckf_step, then the rest of the state (ckf_fit_level).
@@ -297,10 +337,10 @@ int launch_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, con
       int32_t* g_next = h->ft_g + GBLK * ((level + 1) & 1);
       if (level > 0) {
         kp.g = g_this;
-        ckf_step<T, MinBlocks<T>::value><<<h->step_grid, STEP_NT, 0, st>>>(kp, level);
+        launch_chain(ckf_step<T, MinBlocks<T>::value>, h->step_grid, STEP_NT, 0, st, ovm & 2, kp, level);
       }
       kp.g = g_next;
-      ckf_fit_level<T><<<grid, FIT_NT, 0, st>>>(kp, p, level, g_this);
+      launch_chain(ckf_fit_level<T>, grid, FIT_NT, 0, st, ovm & 64, kp, p, level, g_this);
     }
     ckf_fit_flush_work<<<1, 32, 0, st>>>(h->ft_counters, p.o_work);
     const bool f32 = sizeof(T) == 4 && o->smoother_precision == 32;
@@ -334,6 +374,7 @@ Workspace* acquire_ws(ckf_handle* h, cudaStream_t st) {
     w->stream_tag = (void*)st;
   }
   w->busy.lock();  // a previous owner still enqueuing: wait for it (and for its cudaEventRecord) on the host
+  w->enqueuing = true;
   if (w->done_valid && w->done_stream != (void*)st) cudaStreamWaitEvent(st, w->done, 0);
   return w;
 }
@@ -342,6 +383,7 @@ void release_ws(Workspace* w, cudaStream_t st) {
   cudaEventRecord(w->done, st);
   w->done_stream = (void*)st;
   w->done_valid = true;
+  w->enqueuing = false;
   w->busy.unlock();
 }
 
@@ -442,6 +484,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
   }
   h->sm_count = prop.multiProcessorCount;
   { const char* t = getenv("CKF_TIMING"); h->timing = h->timing_print = t && t[0] == '1'; }
+  { const char* t = getenv("CKF_CHAIN_OVERLAP"); if (t && t[0]) h->chain_overlap = atoi(t); }
   h->n_modules = g->n_modules;
   h->n_layers = g->n_layers;
 
@@ -483,6 +526,16 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     }
     CKB(dalloc(h, &h->d_grid, 4 * np * sizeof(double)));
     CKB(cudaMemcpy(h->d_grid, pad.data(), 4 * np * sizeof(double), cudaMemcpyHostToDevice));
+    h->fld.grid = h->d_grid;
+  } else {
+    // a uniform field still owns a 2 x 2 x 2 grid of its value: field_at never reads it (kind 0 returns first), but
+    // ld_node is a plain asm load which the compiler may hoist above that test, so every address field_at can form
+    // must be readable -- with n = 2 the index clamps leave only cell 0
+    std::vector<double> pad(4 * 8, 0.0);
+    for (int i = 0; i < 8; ++i) for (int a = 0; a < 3; ++a) pad[4 * i + a] = f->uniform_b[a];
+    for (int a = 0; a < 3; ++a) { h->fld.n[a] = 2; h->fld.nm2[a] = 0.0; h->fld.org[a] = 0.0; h->fld.inv[a] = 0.0; }
+    CKB(dalloc(h, &h->d_grid, pad.size() * sizeof(double)));
+    CKB(cudaMemcpy(h->d_grid, pad.data(), pad.size() * sizeof(double), cudaMemcpyHostToDevice));
     h->fld.grid = h->d_grid;
   }
   // ---- config

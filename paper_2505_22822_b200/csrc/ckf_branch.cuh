@@ -17,6 +17,7 @@ namespace ckf {
 //     publishes the next level's size.
 template <typename T>
 __global__ void __launch_bounds__(SCAN_NT) ckf_scan(const KParams<T> p, int level) {
+  chain_enter();
   const int n = p.g[G_NTIPS0 + (level & 1)];
   if (n == 0) {
     if (blockIdx.x == 0 && threadIdx.x == 0) p.g[G_NTIPS0 + ((level + 1) & 1)] = 0;  // the slot held level - 1
@@ -218,6 +219,7 @@ template <typename T>
 #define CKF_UPDATE_MINB 2
 #endif
 __global__ void __launch_bounds__(SCAN_NT, CKF_UPDATE_MINB) ckf_update(const KParams<T> p, int level) {
+  chain_enter();
   const int n = p.g[G_NTIPS0 + (level & 1)];
   if (n == 0) return;
   const int nc = p.g[G_NTIPS0 + ((level + 1) & 1)];

@@ -9,6 +9,7 @@ namespace ckf {
 // (No allocation, no memset calls in ckf_find.)
 template <typename T>
 __global__ void ckf_init_event(const KParams<T> p) {
+  chain_enter();
   const int i = blockIdx.x * blockDim.x + threadIdx.x;
   if (i < p.n_seeds) {
     p.sd_extra[i] = 0; p.sd_nemit[i] = 0; p.sd_nentries[i] = 0;
@@ -37,6 +38,7 @@ __global__ void ckf_init_event(const KParams<T> p) {
 constexpr int SEED_TILE = 1024;
 template <typename T>
 __global__ void __launch_bounds__(SEED_TILE) ckf_scan_seeds(const KParams<T> p) {
+  chain_enter();
   __shared__ unsigned long long s_w[32];
   __shared__ int s_last;
   const int tid = threadIdx.x, lane = tid & 31, w = tid >> 5, S = p.n_seeds;
@@ -89,6 +91,7 @@ __global__ void __launch_bounds__(SEED_TILE) ckf_scan_seeds(const KParams<T> p) 
 // Thread per candidate: backtrace the links into the index list, copy the state at the last measurement.
 template <typename T>
 __global__ void __launch_bounds__(256) ckf_emit_tracks(const KParams<T> p) {
+  chain_enter();
   const int total = p.g[G_TOTAL_TRACKS];
   const int cap = p.cfg.max_cands;
   const int ntiles = p.n_seeds > 0 ? (p.n_seeds + SEED_TILE - 1) / SEED_TILE : 1;
@@ -141,6 +144,7 @@ __global__ void __launch_bounds__(256) ckf_emit_tracks(const KParams<T> p) {
 
 template <typename T>
 __global__ void ckf_finalize(const KParams<T> p) {
+  chain_enter();
   const int total = p.g[G_TOTAL_TRACKS], bad = p.g[G_FIRST_BAD];
   const int n = total < bad ? total : bad;
   *p.o_ntracks = n;

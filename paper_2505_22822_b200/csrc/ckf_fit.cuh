@@ -68,6 +68,7 @@ constexpr int FIT_RUNNING = -1;
 // consumed, which thread 0 clears for the level after next.
 template <typename T>
 __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, const FitParams<T> p, int level, int32_t* g_done) {
+  chain_enter();
   if (blockIdx.x == 0 && threadIdx.x < G_N - G_STEP_CURSOR) g_done[G_STEP_CURSOR + threadIdx.x] = 0;
   const int nt = min(*p.n_tracks, p.max_tracks);
   const size_t CH = (size_t)p.chunk;

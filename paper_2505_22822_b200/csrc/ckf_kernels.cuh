@@ -202,6 +202,15 @@ __device__ __forceinline__ void load_jac(const double* mv_D, size_t t, Jac<doubl
   D.tq = v[24];
 }
 
+// ------------------------------------------------------------------------------------------ launch chain
+// Every kernel of a find is launched with programmatic stream serialisation (ckf.cu, launch_chain): its blocks may become
+// resident while the previous kernel of the stream drains, and they wait HERE until that kernel has completed and its
+// writes are visible.  Nothing is read or written before this call.  Under a plain launch both instructions are no-ops.
+__device__ __forceinline__ void chain_enter() {
+  asm volatile("griddepcontrol.launch_dependents;");
+  asm volatile("griddepcontrol.wait;" ::: "memory");
+}
+
 // ------------------------------------------------------------------------------------------ warp primitives
 __device__ __forceinline__ int warp_incl_scan(int v, int lane) {
 #pragma unroll

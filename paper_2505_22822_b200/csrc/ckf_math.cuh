@@ -85,6 +85,9 @@ CKF_HD D3 ld_node(const double* p) {
   // one 256-bit load per node (sm_100a: LDG.E.256): the node is a 32-byte-aligned sector of 4 doubles.  Against a
   // 128-bit + a 64-bit load this halves the load instructions and the L1 wavefronts of the field read, the busiest
   // unit of ckf_step (l1tex data-pipe wavefronts 62 % of peak, profiles/r02_step_visit_update.md)
+  // NOT volatile (that costs ckf_step 4 %): to the compiler this is a pure function of p, which it may hoist above the
+  // field-kind test of field_at -- it did in ckf_seed.  Hence every address field_at can form is readable: the index
+  // clamps keep it inside the grid, and a uniform field owns a 2 x 2 x 2 grid of its value (ckf_create).
   double x, y, z, w;
   asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(x), "=d"(y), "=d"(z), "=d"(w) : "l"(p));
   return D3{x, y, z};

@@ -57,6 +57,7 @@ __device__ __forceinline__ void sort_slice_warp(const KParams<T>& p, int m, int 
 
 template <typename T>
 __global__ void __launch_bounds__(SORT_NT) ckf_sort_slices(const KParams<T> p) {
+  chain_enter();
   __shared__ T s_key[SORT_CAP];
   __shared__ int32_t s_id[SORT_CAP];
   __shared__ T s_red[SORT_NT / 32];

@@ -95,6 +95,7 @@ __device__ __forceinline__ void pick_warp(const GeoDev& geo, const PickSmem& ps,
 
 template <typename T, int MINB>
 __global__ void __launch_bounds__(STEP_NT, MINB) ckf_step(const KParams<T> p, int level) {
+  chain_enter();
   if (p.g[G_NTIPS0 + (level & 1)] == 0 || level == 0) return;  // level 0: the seed's own module, identity transport (N6)
   __shared__ __align__(16) unsigned char smem_raw[(STEP_NT / 32) * PickSmem::bytes()];
   // step schedule: the live tips of the level, grouped by predicted trial count (ckf_update), longest first

@@ -154,6 +154,7 @@ __device__ __forceinline__ int gate_chunk(const KParams<T>& p, const VSmem<T>& s
 
 template <typename T, int MINB>
 __global__ void __launch_bounds__(VISIT_NT, MINB) ckf_visit(const KParams<T> p, int level) {
+  chain_enter();
   const int n = p.g[G_NTIPS0 + (level & 1)];
   if (n == 0) return;
   extern __shared__ __align__(16) unsigned char smem_raw[];

@@ -987,3 +987,37 @@ def test_fp64_parity_over_many_events():
             assert cnt[k] == ora.counters[k], (seed, k)
         ckf.close()
     print("fp64 over 12 configs[1] events and 3 endcap events (discs + bidirectional + energy loss): worst param rel %.1e" % worst)
+
+
+def test_launch_overlap_policy_same_result(monkeypatch):
+    """The kernels of a find are launched with programmatic stream serialisation when the handle has no other find in
+    flight (ckf.cu, launch_chain / others_in_flight).  The policy must not change a single output byte: plain launches,
+    the default mask and every kernel overlapped give identical candidate arrays, and so do repeated finds."""
+    import torch
+    from paper_2505_22822_b200 import CKF
+    det, fld, cfg = synth.config_bundle(2)
+    ev = synth.make_event(2, det=det)
+    ref = None
+    for mask in ("0", None, "63"):
+        if mask is None:
+            monkeypatch.delenv("CKF_CHAIN_OVERLAP", raising=False)
+        else:
+            monkeypatch.setenv("CKF_CHAIN_OVERLAP", mask)
+        ckf = CKF(det, fld, cfg.ckf, cfg.precision, max_seeds=ev.n_seeds, max_measurements=ev.n_measurements, max_fit_tracks=0)
+        dev, out = ckf.upload_event(ev), ckf.alloc_tracks()
+        for rep in range(3):
+            ckf.find(dev, out)
+            torch.cuda.synchronize()
+            n = int(out["n_tracks"][0])
+            ne = int(out["track_offsets"][n])
+            got = {k: out[k][:n].cpu().numpy().tobytes() for k in ("seed_id", "n_holes", "last_module", "stop_reason", "params", "cov", "chi2_sum")}
+            got["offsets"] = out["track_offsets"][:n + 1].cpu().numpy().tobytes()
+            got["meas"] = out["meas_idx"][:ne].cpu().numpy().tobytes()
+            got["entry_chi2"] = out["entry_chi2"][:ne].cpu().numpy().tobytes()
+            got["counters"] = ckf.counters()
+            if ref is None:
+                ref = got
+                assert n > ev.n_seeds // 2
+            for k in ref:
+                assert got[k] == ref[k], (mask, rep, k)
+        ckf.close()
