@@ -129,8 +129,10 @@ typedef struct {
   int32_t energy_loss;              /* 1: mean energy loss of the muon hypothesis (Bethe, silicon, DESIGN.md rule E) in every
                                        crossed module of x_over_x0 > 0: q/p changes on leaving the module and the
                                        covariance is transported with d(q/p)'/d(q/p).  0: none (BASELINE configs)     */
-  int32_t field_gradient;           /* must be 0: the field-gradient terms of the transport Jacobian (PAPER.md ref
-                                       [18]) exist in the oracle only (reading A13)                          */
+  int32_t field_gradient;           /* 1: the transport Jacobian carries the field-gradient terms of PAPER.md ref [18]
+                                       (DESIGN.md rule J2', reading A13): the step map is differentiated stage by stage
+                                       including dB/dr of the interpolated field, and D gains its two position columns.
+                                       No effect in a uniform field.  0 (BASELINE configs): ref [17], gradient neglected  */
   int32_t bidirectional;            /* 1: tips that move radially INWARD are navigated too (DESIGN.md rules N3''): they cross the
                                        inner layers against the module normals, pass the beam line and leave through the far
                                        side.  0 (BASELINE configs, reading A7): outward only, such tips stop NOT_OUTGOING    */

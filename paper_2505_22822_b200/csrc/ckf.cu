@@ -48,7 +48,7 @@ struct Workspace {
   // level state (tips, move state, predictions, selections, scan)
   int32_t *tip_link = nullptr, *tip_seed = nullptr;
   double *mv_y = nullptr, *pd_x = nullptr;
-  void *mv_D = nullptr, *mv_dep = nullptr, *pd_C = nullptr, *sel_chi2 = nullptr;
+  void *mv_D = nullptr, *mv_Dr = nullptr, *mv_dep = nullptr, *pd_C = nullptr, *sel_chi2 = nullptr;
   int32_t *mv_from = nullptr, *mv_tgt = nullptr, *mv_stop = nullptr, *sel_idx = nullptr, *mv_order = nullptr;
   int32_t *t_nsel = nullptr, *t_want = nullptr, *t_counts = nullptr, *t_keep = nullptr, *t_kex = nullptr, *blk_sum = nullptr, *t_fin = nullptr;
   void *s_loc = nullptr, *s_var = nullptr, *s_v0max = nullptr;  // gate index (ckf_sort_slices)
@@ -100,7 +100,7 @@ struct ckf_handle {
   double* fs_x = nullptr; void* fs_t = nullptr; int32_t* fs_meas = nullptr; int32_t* fs_next = nullptr;
   // level arrays, globals and counters for ckf_step when it runs the moves of a fit level (tcap = fit_chunk)
   int32_t* ft_g = nullptr; unsigned long long* ft_counters = nullptr;
-  double* ft_y = nullptr; void *ft_D = nullptr, *ft_dep = nullptr;
+  double* ft_y = nullptr; void *ft_D = nullptr, *ft_Dr = nullptr, *ft_dep = nullptr;
   int32_t *ft_from = nullptr, *ft_tgt = nullptr, *ft_stop = nullptr, *ft_order = nullptr;
   int fit_chunk = 0, fit_states = 0;
   cudaEvent_t fit_done = nullptr;
@@ -118,6 +118,7 @@ struct ckf_handle {
   // 32 emission, 64 ckf_fit_level.  Measured (profiles/r02_launch_overlap.md): step + visit + update is best; with ckf_scan in the chain as
   // well the whole level loop is one cascade of waiting blocks and a batched find gets 10 % slower.  CKF_CHAIN_OVERLAP=<mask>
   // overrides (0 = plain launches), for A/B measurements.
+  bool grad = false;  // J2': config.field_gradient on an interpolated field (a uniform field has no gradient: the default kernels)
   int chain_overlap = 2 | 4 | 16 | 64;
   bool timing = false;  // ckf_set_timing / CKF_TIMING=1: per-kernel CUDA-event times of every ckf_find on stderr (debug aid; synchronises)
 };
@@ -182,7 +183,7 @@ void fill_params(ckf_handle* h, Workspace& w, KParams<T>& p) {
   p.leaf_link = w.leaf; p.leaf_meta = w.leaf + LC; p.leaf_entry = w.leaf + 2 * LC;
   p.tcap = h->tcap;
   p.tip_link = w.tip_link; p.tip_seed = w.tip_seed;
-  p.mv_y = w.mv_y; p.mv_D = (T*)w.mv_D; p.mv_dep = (double*)w.mv_dep; p.mv_from = w.mv_from; p.mv_tgt = w.mv_tgt;
+  p.mv_y = w.mv_y; p.mv_D = (T*)w.mv_D; p.mv_Dr = (T*)w.mv_Dr; p.mv_dep = (double*)w.mv_dep; p.mv_from = w.mv_from; p.mv_tgt = w.mv_tgt;
   p.mv_stop = w.mv_stop; p.mv_order = w.mv_order;
   p.pd_x = w.pd_x; p.pd_C = (double*)w.pd_C; p.sel_chi2 = (T*)w.sel_chi2; p.sel_idx = w.sel_idx;
   p.t_nsel = w.t_nsel; p.t_want = w.t_want; p.t_counts = w.t_counts; p.t_keep = w.t_keep; p.t_kex = w.t_kex;
@@ -193,6 +194,29 @@ void fill_params(ckf_handle* h, Workspace& w, KParams<T>& p) {
   p.counters = w.counters;
   p.max_tracks = c.max_tracks; p.max_entries = c.max_track_entries;
   p.o_summary = nullptr;
+}
+
+// ckf_step with the gradient terms (J2') carries 27 + 12 more live numbers: two resident blocks per SM instead of three.
+template <typename T, bool GRAD> struct StepBlocks { static constexpr int value = GRAD ? 2 : MinBlocks<T>::value; };
+
+// Launch configuration: ckf_step is persistent (one wave of resident blocks), ckf_visit grid-strides.
+template <typename T, bool GRAD>
+int setup_launch(ckf_handle* h, const ckf_config* c) {
+  int per_sm = 0, vper_sm = 0;
+  cudaFuncAttributes fa;
+  auto step = ckf_step<T, StepBlocks<T, GRAD>::value, GRAD>;
+  auto visit = ckf_visit<T, VisitBlocks<T>::value, GRAD>;
+  h->visit_smem = (int)((VISIT_NT / 32) * VSmem<T>::bytes(c->max_branches_per_surface));
+  if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, step, STEP_NT, 0) != cudaSuccess ||
+      cudaFuncGetAttributes(&fa, step) != cudaSuccess ||
+      cudaFuncSetAttribute(visit, cudaFuncAttributeMaxDynamicSharedMemorySize, h->visit_smem) != cudaSuccess ||
+      cudaOccupancyMaxActiveBlocksPerMultiprocessor(&vper_sm, visit, VISIT_NT, h->visit_smem) != cudaSuccess)
+    return fail(h, CKF_E_CUDA, "launch configuration failed: %s", cudaGetErrorString(cudaGetLastError()));
+  if (per_sm < 1 || vper_sm < 1) return fail(h, CKF_E_CUDA, "kernels do not fit on an SM (visit smem %d B)", h->visit_smem);
+  h->step_regs = fa.numRegs;
+  h->step_grid = per_sm * h->sm_count;
+  h->visit_grid = vper_sm * h->sm_count;
+  return CKF_OK;
 }
 
 // One kernel of a find's chain.  With `overlap` the launch carries programmatic stream serialisation: the kernel's blocks
@@ -262,8 +286,13 @@ int launch_find(ckf_handle* h, Workspace& w, const ckf_measurements* m, const ck
   // Kernels of an empty level return at once, so the loop needs no host read of the level's size.
   const int wide = h->sm_count * 4;
   for (int level = 0; level <= h->cfg.max_levels; ++level) {
-    if (level > 0) { launch_chain(ckf_step<T, MinBlocks<T>::value>, h->step_grid, STEP_NT, 0, st, ovm & 2, p, level); mark(2); }
-    launch_chain(ckf_visit<T, VisitBlocks<T>::value>, h->visit_grid, VISIT_NT, h->visit_smem, st, ovm & 4, p, level); mark(3);
+    if (h->grad) {
+      if (level > 0) { launch_chain(ckf_step<T, StepBlocks<T, true>::value, true>, h->step_grid, STEP_NT, 0, st, ovm & 2, p, level); mark(2); }
+      launch_chain(ckf_visit<T, VisitBlocks<T>::value, true>, h->visit_grid, VISIT_NT, h->visit_smem, st, ovm & 4, p, level); mark(3);
+    } else {
+      if (level > 0) { launch_chain(ckf_step<T, MinBlocks<T>::value>, h->step_grid, STEP_NT, 0, st, ovm & 2, p, level); mark(2); }
+      launch_chain(ckf_visit<T, VisitBlocks<T>::value>, h->visit_grid, VISIT_NT, h->visit_smem, st, ovm & 4, p, level); mark(3);
+    }
     launch_chain(ckf_scan<T>, wide, SCAN_NT, 0, st, ovm & 8, p, level); mark(5);
     launch_chain(ckf_update<T>, wide, SCAN_NT, 0, st, ovm & 16, p, level); mark(6);
   }
@@ -320,7 +349,7 @@ int launch_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, con
   kp.geo = p.geo; kp.fld = p.fld; kp.cfg = p.cfg;
   kp.tcap = h->fit_chunk;
   kp.g = h->ft_g; kp.counters = h->ft_counters;
-  kp.mv_y = h->ft_y; kp.mv_D = (T*)h->ft_D; kp.mv_dep = (double*)h->ft_dep; kp.mv_from = h->ft_from; kp.mv_tgt = h->ft_tgt;
+  kp.mv_y = h->ft_y; kp.mv_D = (T*)h->ft_D; kp.mv_Dr = (T*)h->ft_Dr; kp.mv_dep = (double*)h->ft_dep; kp.mv_from = h->ft_from; kp.mv_tgt = h->ft_tgt;
   kp.mv_stop = h->ft_stop; kp.mv_order = h->ft_order;
   const int n_upper = o->n_tracks_upper > 0 ? std::min(o->n_tracks_upper, h->cfg.max_tracks) : h->cfg.max_tracks;
   const int ovm = others_in_flight(h, nullptr, st) ? 0 : h->chain_overlap;  // launch policy as in launch_find
@@ -337,10 +366,12 @@ int launch_fit(ckf_handle* h, const ckf_measurements* m, const ckf_seeds* s, con
       int32_t* g_next = h->ft_g + GBLK * ((level + 1) & 1);
       if (level > 0) {
         kp.g = g_this;
-        launch_chain(ckf_step<T, MinBlocks<T>::value>, h->step_grid, STEP_NT, 0, st, ovm & 2, kp, level);
+        if (h->grad) launch_chain(ckf_step<T, StepBlocks<T, true>::value, true>, h->step_grid, STEP_NT, 0, st, ovm & 2, kp, level);
+        else launch_chain(ckf_step<T, MinBlocks<T>::value>, h->step_grid, STEP_NT, 0, st, ovm & 2, kp, level);
       }
       kp.g = g_next;
-      launch_chain(ckf_fit_level<T>, grid, FIT_NT, 0, st, ovm & 64, kp, p, level, g_this);
+      if (h->grad) launch_chain(ckf_fit_level<T, true>, grid, FIT_NT, 0, st, ovm & 64, kp, p, level, g_this);
+      else launch_chain(ckf_fit_level<T>, grid, FIT_NT, 0, st, ovm & 64, kp, p, level, g_this);
     }
     ckf_fit_flush_work<<<1, 32, 0, st>>>(h->ft_counters, p.o_work);
     const bool f32 = sizeof(T) == 4 && o->smoother_precision == 32;
@@ -446,8 +477,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
   if (g->n_layers < 1 || g->n_modules < 1) return fail(h, CKF_E_ARG, "empty geometry");
   if (g->n_layers > 254) return fail(h, CKF_E_ARG, "at most 254 layers (the navigation cursors are 9-bit fields)");
   if (f->kind != 0 && f->kind != 1) return fail(h, CKF_E_ARG, "field kind must be 0 or 1");
-  if (c->field_gradient != 0)
-    return fail(h, CKF_E_ARG, "field_gradient = 1 (gradient terms in the transport Jacobian) is not built in the CUDA path");
+  if (c->field_gradient != 0 && c->field_gradient != 1) return fail(h, CKF_E_ARG, "field_gradient must be 0 or 1");
   if (f->kind == 1 && (!f->grid || f->n[0] < 2 || f->n[1] < 2 || f->n[2] < 2))
     return fail(h, CKF_E_ARG, "field grid needs >= 2 nodes per axis");
   for (int l = 0; l < g->n_layers; ++l)
@@ -510,6 +540,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
   // ---- a2 field store
   std::memset(&h->fld, 0, sizeof(h->fld));
   h->fld.kind = f->kind;
+  h->grad = c->field_gradient == 1 && f->kind == 1;
   for (int a = 0; a < 3; ++a) {
     h->fld.ub[a] = f->uniform_b[a];
     h->fld.n[a] = f->n[a];
@@ -544,27 +575,12 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
   h->kcfg.max_cands = c->max_candidates_per_seed; h->kcfg.max_holes = c->max_holes; h->kcfg.min_meas = c->min_measurements;
   h->kcfg.max_rk_steps = c->max_rk_steps_per_surface; h->kcfg.max_levels = c->max_levels;
   h->kcfg.energy_loss = c->energy_loss ? 1 : 0;
+  h->kcfg.field_gradient = h->grad ? 1 : 0;
   // ---- launch configuration: ckf_step is persistent (one wave of resident blocks), ckf_visit grid-strides
   {
-    int per_sm = 0, vper_sm = 0;
-    cudaFuncAttributes fa;
-    if (c->precision == 32) {
-      h->visit_smem = (int)((VISIT_NT / 32) * VSmem<float>::bytes(c->max_branches_per_surface));
-      CKB(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ckf_step<float, MinBlocks<float>::value>, STEP_NT, 0));
-      CKB(cudaFuncGetAttributes(&fa, ckf_step<float, MinBlocks<float>::value>));
-      CKB(cudaFuncSetAttribute(ckf_visit<float, VisitBlocks<float>::value>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->visit_smem));
-      CKB(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&vper_sm, ckf_visit<float, VisitBlocks<float>::value>, VISIT_NT, h->visit_smem));
-    } else {
-      h->visit_smem = (int)((VISIT_NT / 32) * VSmem<double>::bytes(c->max_branches_per_surface));
-      CKB(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, ckf_step<double, MinBlocks<double>::value>, STEP_NT, 0));
-      CKB(cudaFuncGetAttributes(&fa, ckf_step<double, MinBlocks<double>::value>));
-      CKB(cudaFuncSetAttribute(ckf_visit<double, VisitBlocks<double>::value>, cudaFuncAttributeMaxDynamicSharedMemorySize, h->visit_smem));
-      CKB(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&vper_sm, ckf_visit<double, VisitBlocks<double>::value>, VISIT_NT, h->visit_smem));
-    }
-    if (per_sm < 1 || vper_sm < 1) { fail(h, CKF_E_CUDA, "kernels do not fit on an SM (visit smem %d B)", h->visit_smem); return bail(CKF_E_CUDA); }
-    h->step_regs = fa.numRegs;
-    h->step_grid = per_sm * h->sm_count;
-    h->visit_grid = vper_sm * h->sm_count;
+    const int rc = h->grad ? (c->precision == 32 ? setup_launch<float, true>(h, c) : setup_launch<double, true>(h, c))
+                           : (c->precision == 32 ? setup_launch<float, false>(h, c) : setup_launch<double, false>(h, c));
+    if (rc != CKF_OK) return bail(rc);
   }
   if (h->cfg.max_tips_per_level <= 0)
     h->cfg.max_tips_per_level = (int32_t)std::min<long long>(std::max<long long>(8LL * c->max_seeds, 1024), 0x7ffffff0LL);
@@ -585,7 +601,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     const size_t TC = (size_t)h->tcap, KB = (size_t)c->max_branches_per_surface;
     CKB(dalloc(h, &w.tip_link, 2 * TC * 4)); CKB(dalloc(h, &w.tip_seed, 2 * TC * 4));
     CKB(dalloc(h, &w.mv_y, 8 * TC * sizeof(double))); CKB(dalloc(h, &w.pd_x, 6 * TC * sizeof(double)));
-    CKB(dalloc(h, (char**)&w.mv_D, (size_t)MVD * TC * ts)); CKB(dalloc(h, (char**)&w.mv_dep, (size_t)NDEP * TC * sizeof(double)));
+    CKB(dalloc(h, (char**)&w.mv_D, (size_t)MVD * TC * ts)); if (h->grad) CKB(dalloc(h, (char**)&w.mv_Dr, (size_t)12 * TC * ts)); CKB(dalloc(h, (char**)&w.mv_dep, (size_t)NDEP * TC * sizeof(double)));
     CKB(dalloc(h, (char**)&w.pd_C, 21 * TC * sizeof(double))); CKB(dalloc(h, (char**)&w.sel_chi2, KB * TC * ts));
     CKB(dalloc(h, &w.sel_idx, KB * TC * 4));
     CKB(dalloc(h, &w.mv_from, TC * 4)); CKB(dalloc(h, &w.mv_tgt, 2 * TC * 4)); CKB(dalloc(h, &w.mv_stop, TC * 4));
@@ -625,7 +641,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     CKB(dalloc(h, &h->fs_next, CHK * 4));
     CKB(dalloc(h, &h->ft_g, 2 * GBLK * 4)); CKB(dalloc(h, &h->ft_counters, CNT_N * 8));
     CKB(dalloc(h, &h->ft_y, 8 * CHK * sizeof(double)));
-    CKB(dalloc(h, (char**)&h->ft_D, (size_t)MVD * CHK * ts)); CKB(dalloc(h, (char**)&h->ft_dep, (size_t)NDEP * CHK * sizeof(double)));
+    CKB(dalloc(h, (char**)&h->ft_D, (size_t)MVD * CHK * ts)); if (h->grad) CKB(dalloc(h, (char**)&h->ft_Dr, (size_t)12 * CHK * ts)); CKB(dalloc(h, (char**)&h->ft_dep, (size_t)NDEP * CHK * sizeof(double)));
     CKB(dalloc(h, &h->ft_from, CHK * 4)); CKB(dalloc(h, &h->ft_tgt, 2 * CHK * 4)); CKB(dalloc(h, &h->ft_stop, CHK * 4));
     CKB(dalloc(h, &h->ft_order, (size_t)NBIN * CHK * 4));
     CKB(cudaEventCreateWithFlags(&h->fit_done, cudaEventDisableTiming));

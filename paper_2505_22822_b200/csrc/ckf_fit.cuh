@@ -66,7 +66,7 @@ constexpr int FIT_RUNNING = -1;
 // The step schedule is double-buffered by level parity (two blocks of globals, G_N ints apart): kp.g is the block
 // this level appends to for the next level's ckf_step; `g_done` is the block the ckf_step before this kernel
 // consumed, which thread 0 clears for the level after next.
-template <typename T>
+template <typename T, bool GRAD = false>
 __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, const FitParams<T> p, int level, int32_t* g_done) {
   chain_enter();
   if (blockIdx.x == 0 && threadIdx.x < G_N - G_STEP_CURSOR) g_done[G_STEP_CURSOR + threadIdx.x] = 0;
@@ -121,7 +121,13 @@ __global__ void __launch_bounds__(FIT_NT) ckf_fit_level(const KParams<T> kp, con
         double dep[NDEP];
 #pragma unroll
         for (int i = 0; i < NDEP; ++i) dep[i] = kp.mv_dep[i * CH + s];
-        status = move_arrive<T>(m, dep, p.geo, p.fld, p.cfg, xp, J);
+        if constexpr (GRAD) {
+          JacR<T> R;
+          load_jacr(kp.mv_Dr, (size_t)s, R);
+          status = move_arrive<T>(m, dep, p.geo, p.fld, p.cfg, xp, J, &R);
+        } else {
+          status = move_arrive<T>(m, dep, p.geo, p.fld, p.cfg, xp, J);
+        }
         if (status == STOP_NONE) {
           double C[21];
           const double* pt = p.fs_x + (size_t)(level - 1) * FS_X * CH + s;  // filtered covariance of the previous state

@@ -102,6 +102,7 @@ struct KParams {
   // departure / arrival state of the move (ckf_update -> ckf_step -> ckf_visit)
   double* mv_y;        // [tcap][8] r, d, t, q/p (move records, see below)
   T* mv_D;             // [tcap][MVD] transport Jacobian (ckf_step -> ckf_visit)
+  T* mv_Dr;            // [tcap][12] position columns of D (J2', config.field_gradient; null otherwise)
   double* mv_dep;      // [NDEP][tcap] direction on departure, Highland q_phi, q_theta, energy-loss factor g
   int32_t* mv_from;    // [tcap] module the tip stands on
   int32_t* mv_tgt;     // [2][tcap] module reached; overlap neighbour at departure (N2, by ckf_update), -1 none
@@ -200,6 +201,20 @@ __device__ __forceinline__ void load_jac(const double* mv_D, size_t t, Jac<doubl
     D.dq[i] = v[21 + i];
   }
   D.tq = v[24];
+}
+
+// position columns (J2'): Ru, Du, Rv, Dv, 12 T per tip
+template <typename T>
+__device__ __forceinline__ void store_jacr(T* mv_Dr, size_t t, const JacR<T>& R) {
+  T* q = mv_Dr + t * 12;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { q[i] = R.Ru[i]; q[3 + i] = R.Du[i]; q[6 + i] = R.Rv[i]; q[9 + i] = R.Dv[i]; }
+}
+template <typename T>
+__device__ __forceinline__ void load_jacr(const T* mv_Dr, size_t t, JacR<T>& R) {
+  const T* q = mv_Dr + t * 12;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { R.Ru[i] = q[i]; R.Du[i] = q[3 + i]; R.Rv[i] = q[6 + i]; R.Dv[i] = q[9 + i]; }
 }
 
 // ------------------------------------------------------------------------------------------ launch chain

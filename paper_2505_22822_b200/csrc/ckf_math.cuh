@@ -65,6 +65,7 @@ struct CfgDev {
   double rk_tol, surf_tol, h_max, mass;
   int32_t max_branches, max_cands, max_holes, min_meas, max_rk_steps, max_levels;
   int32_t energy_loss;   // rule E: mean energy loss in every crossed module (BASELINE configs: 0)
+  int32_t field_gradient;  // J2': field-gradient terms in the transport Jacobian (reading A13; BASELINE configs: 0)
 };
 
 // ------------------------------------------------------------------------------------------ small algebra
@@ -149,6 +150,55 @@ CKF_HD void field_at(const FieldDev& f, const double r[3], double B[3]) {
 #undef CKF_TRILERP
 }
 
+// J2' (config.field_gradient): G[i][j] = dB_i / dr_j, the exact derivative of the trilinear interpolant inside the cell
+// field_at picks for r (piecewise constant along the differentiated axis); zero for a uniform field.
+CKF_HD void field_gradient_at(const FieldDev& f, const double r[3], double G[3][3]) {
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) G[i][j] = 0.0;
+  if (f.kind == 0) return;
+  int idx[3];
+  double fr[3];
+#pragma unroll
+  for (int a = 0; a < 3; ++a) {
+    const double g = (r[a] - f.org[a]) * f.inv[a];
+    double ti = floor(g);
+    ti = ti < 0.0 ? 0.0 : ti;
+    ti = ti > f.nm2[a] ? f.nm2[a] : ti;
+    int i = (ti == ti) ? (int)ti : 0;
+    i = i < 0 ? 0 : i;
+    i = i > f.n[a] - 2 ? f.n[a] - 2 : i;
+    idx[a] = i;
+    fr[a] = g - ti;
+  }
+  const long long s1 = f.n[2], s0 = (long long)f.n[1] * f.n[2];
+  const double* p = f.grid + 4 * (idx[0] * s0 + idx[1] * s1 + idx[2]);
+  const D3 v000 = ld_node(p), v001 = ld_node(p + 4);
+  const D3 v010 = ld_node(p + 4 * s1), v011 = ld_node(p + 4 * s1 + 4);
+  const D3 v100 = ld_node(p + 4 * s0), v101 = ld_node(p + 4 * s0 + 4);
+  const D3 v110 = ld_node(p + 4 * (s0 + s1)), v111 = ld_node(p + 4 * (s0 + s1) + 4);
+#define CKF_TRIGRAD(C, ROW)                                                                         \
+  {                                                                                                 \
+    /* d/dx: differences along x, then lerp along y and z */                                        \
+    const double dx0 = (v100.C - v000.C) + fr[1] * ((v110.C - v010.C) - (v100.C - v000.C));         \
+    const double dx1 = (v101.C - v001.C) + fr[1] * ((v111.C - v011.C) - (v101.C - v001.C));         \
+    G[ROW][0] = (dx0 + fr[2] * (dx1 - dx0)) * f.inv[0];                                             \
+    /* d/dy: lerp along x, difference along y, lerp along z */                                      \
+    const double x00 = v000.C + fr[0] * (v100.C - v000.C), x10 = v010.C + fr[0] * (v110.C - v010.C); \
+    const double x01 = v001.C + fr[0] * (v101.C - v001.C), x11 = v011.C + fr[0] * (v111.C - v011.C); \
+    const double dy0 = x10 - x00, dy1 = x11 - x01;                                                  \
+    G[ROW][1] = (dy0 + fr[2] * (dy1 - dy0)) * f.inv[1];                                             \
+    /* d/dz: lerp along x and y, difference along z */                                              \
+    const double y0 = x00 + fr[1] * (x10 - x00), y1 = x01 + fr[1] * (x11 - x01);                    \
+    G[ROW][2] = (y1 - y0) * f.inv[2];                                                               \
+  }
+  CKF_TRIGRAD(x, 0)
+  CKF_TRIGRAD(y, 1)
+  CKF_TRIGRAD(z, 2)
+#undef CKF_TRIGRAD
+}
+
 // ------------------------------------------------------------------------------------------ trajectory state
 struct Traj {
   double r[3], d[3], t, qop;
@@ -176,6 +226,20 @@ CKF_HD void jac_identity(Jac<T>& J) {
   J.tq = T(0);
 }
 
+// J2': with the field-gradient terms the position columns of D are no longer trivial.  A move only needs them along
+// the two local axes of its departure module (r0 = c + l0 u + l1 v): two tangent vectors (dr, dd), started at
+// (u, 0) and (v, 0).  Without the gradient terms they stay there, which is what arrival_jacobian assumes by default.
+template <typename T>
+struct JacR {
+  T Ru[3], Du[3], Rv[3], Dv[3];
+};
+
+template <typename T>
+CKF_HD void jacr_begin(JacR<T>& R, const double u[3], const double v[3]) {
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { R.Ru[i] = (T)u[i]; R.Rv[i] = (T)v[i]; R.Du[i] = T(0); R.Dv[i] = T(0); }
+}
+
 CKF_HD double inv_beta(double qop, double mass) { return sqrt(1.0 + mass * mass * qop * qop); }
 CKF_HD double dinvbeta_dqop(double qop, double mass) { return mass * mass * qop / sqrt(1.0 + mass * mass * qop * qop); }
 
@@ -190,11 +254,12 @@ struct Trial {
   T q1[3], q2[3], q3[3], q4[3];
   double s1[3], s2[3];
   double eps;
+  double rm[3], re[3];  // stage points, kept only by rk_trial<T, true> (J2' reads the field gradient there)
 };
 
 // B1 = field at y.r, read by the caller (move_target): it is the same for every retry of a rejected trial, and after an
 // accepted step its loads are issued before the Jacobian columns are computed, which hides their latency.
-template <typename T>
+template <typename T, bool GRAD = false>
 CKF_HD void rk_trial(const FieldDev& fld, const Traj& y, const double B1[3], double lam, double h, Trial<T>& t) {
   // The stage loop is unrolled: three inlined copies of field_at.  In the monolithic level loop of r01b one rolled
   // copy was needed to stay inside the SM's instruction cache; in the per-phase ckf_step the three copies fit
@@ -213,6 +278,10 @@ CKF_HD void rk_trial(const FieldDev& fld, const Traj& y, const double B1[3], dou
     } else {
 #pragma unroll
       for (int i = 0; i < 3; ++i) p[i] = y.r[i] + h * y.d[i] + hh2 * (lam * cr3[i]);
+    }
+    if (GRAD && st != 0) {
+#pragma unroll
+      for (int i = 0; i < 3; ++i) (st == 1 ? t.rm : t.re)[i] = p[i];
     }
     if (st != 0) field_at(fld, p, B);
     if (st == 0) {
@@ -280,6 +349,110 @@ CKF_HD void jac_column_q(T lam, T h, T qf, const T B1[3], const T B2[3], const T
   }
 }
 
+// J2' applied to one column: jac_column_q plus the dependence of the field on the stage points,
+//   k1 = lam [dd x B1 + w1 x (G1 dr)] + qf q1,          drm = dr + h/2 dd + h^2/8 k1
+//   k2 = lam [(dd + h/2 k1) x B2 + w2 x (G2 drm)] + qf q2,   k3 likewise from k2 with w3
+//   dre = dr + h dd + h^2/2 k3,    k4 = lam [(dd + h k3) x B4 + w4 x (G4 dre)] + qf q4
+// w1 = d, w2 = d + h/2 k1, w3 = d + h/2 k2, w4 = d + h k3 of the trajectory itself (StepGrad).
+template <typename T>
+struct StepGrad {
+  T G1[3][3], G2[3][3], G4[3][3];
+  T w1[3], w2[3], w3[3], w4[3];
+};
+
+// Gradients at the three stage points and the stage directions of an accepted trial; y is the state BEFORE the step.
+template <typename T>
+CKF_HD void step_gradients(const FieldDev& fld, const Traj& y, double h, const Trial<T>& t, StepGrad<T>& sg) {
+  double G[3][3];
+  field_gradient_at(fld, y.r, G);
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) sg.G1[i][j] = (T)G[i][j];
+  field_gradient_at(fld, t.rm, G);
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) sg.G2[i][j] = (T)G[i][j];
+  field_gradient_at(fld, t.re, G);
+#pragma unroll
+  for (int i = 0; i < 3; ++i)
+#pragma unroll
+    for (int j = 0; j < 3; ++j) sg.G4[i][j] = (T)G[i][j];
+  // k_i = lam cr_i = q/p * (kappa cr_i) = q/p * q_i
+  const double h2 = 0.5 * h;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    sg.w1[i] = (T)y.d[i];
+    sg.w2[i] = (T)(y.d[i] + h2 * (y.qop * (double)t.q1[i]));
+    sg.w3[i] = (T)(y.d[i] + h2 * (y.qop * (double)t.q2[i]));
+    sg.w4[i] = (T)(y.d[i] + h * (y.qop * (double)t.q3[i]));
+  }
+}
+
+template <typename T>
+CKF_HD void jac_column_g(T lam, T h, T qf, const Trial<T>& t, const StepGrad<T>& sg, T dr[3], T dd[3]) {
+  T k1[3], k2[3], k3[3], k4[3], w[3], gb[3], b[3], drs[3];
+  const T h2 = T(0.5) * h, h8 = h * h * T(0.125), hh2 = h * h * T(0.5);
+  auto gmul = [](const T G[3][3], const T v[3], T o[3]) {
+#pragma unroll
+    for (int i = 0; i < 3; ++i) o[i] = G[i][0] * v[0] + G[i][1] * v[1] + G[i][2] * v[2];
+  };
+  cross3(dd, t.B1, k1);
+  gmul(sg.G1, dr, gb);
+  cross3(sg.w1, gb, b);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) k1[i] = lam * (k1[i] + b[i]) + qf * t.q1[i];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) drs[i] = dr[i] + h2 * dd[i] + h8 * k1[i];
+  gmul(sg.G2, drs, gb);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) w[i] = dd[i] + h2 * k1[i];
+  cross3(w, t.B2, k2);
+  cross3(sg.w2, gb, b);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) k2[i] = lam * (k2[i] + b[i]) + qf * t.q2[i];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) w[i] = dd[i] + h2 * k2[i];
+  cross3(w, t.B2, k3);
+  cross3(sg.w3, gb, b);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) k3[i] = lam * (k3[i] + b[i]) + qf * t.q3[i];
+#pragma unroll
+  for (int i = 0; i < 3; ++i) drs[i] = dr[i] + h * dd[i] + hh2 * k3[i];
+  gmul(sg.G4, drs, gb);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) w[i] = dd[i] + h * k3[i];
+  cross3(w, t.B4, k4);
+  cross3(sg.w4, gb, b);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) k4[i] = lam * (k4[i] + b[i]) + qf * t.q4[i];
+  const T h6 = h * T(1.0 / 6.0), hh6 = h * h * T(1.0 / 6.0);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+    dr[i] = dr[i] + h * dd[i] + hh6 * (k1[i] + k2[i] + k3[i]);
+    dd[i] = dd[i] + h6 * (k1[i] + T(2) * k2[i] + T(2) * k3[i] + k4[i]);
+  }
+}
+
+// D <- D_step D with the gradient terms: the three d-columns, the q-column and the two position columns.
+template <typename T>
+CKF_HD void rk_accept_jac_g(double qop, Jac<T>& J, JacR<T>& R, double h, const Trial<T>& t, const StepGrad<T>& sg, double dib) {
+  const T lamT = (T)(KAPPA * qop), hT = (T)h;
+#pragma unroll
+  for (int j = 0; j < 3; ++j) {
+    T dr[3] = {J.Rd[0][j], J.Rd[1][j], J.Rd[2][j]};
+    T dd[3] = {J.Dd[0][j], J.Dd[1][j], J.Dd[2][j]};
+    jac_column_g<T>(lamT, hT, T(0), t, sg, dr, dd);
+#pragma unroll
+    for (int i = 0; i < 3; ++i) { J.Rd[i][j] = dr[i]; J.Dd[i][j] = dd[i]; }
+  }
+  jac_column_g<T>(lamT, hT, T(1), t, sg, J.rq, J.dq);
+  jac_column_g<T>(lamT, hT, T(0), t, sg, R.Ru, R.Du);
+  jac_column_g<T>(lamT, hT, T(0), t, sg, R.Rv, R.Dv);
+  J.tq += (T)(h * dib);
+}
+
 // Accept a trial, in two halves so that the caller can put the next field read between them: the state (P2), and
 // D <- D_step D column by column (J2, J3).  The Jacobian half does not read the state's position or direction.
 template <typename T>
@@ -327,6 +500,13 @@ CKF_HD void straight_close(Traj& y, Jac<T>& J, double s, double ib, double dib) 
   }
   J.tq += (T)(s * dib);
   y.t += s * ib;
+}
+
+template <typename T>
+CKF_HD void straight_close_r(JacR<T>& R, double s) {
+  const T sT = (T)s;
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { R.Ru[i] += sT * R.Du[i]; R.Rv[i] += sT * R.Dv[i]; }
 }
 
 // ------------------------------------------------------------------------------------------ step control

@@ -107,7 +107,8 @@ CKF_HD double mean_dedx_silicon(double p, double M) {
 // transport Jacobian D was accumulated in (float32 in fp32 mode).
 template <typename T, typename TD>
 CKF_HD void arrival_jacobian(const Jac<TD>& D, const double dep_u[3], const double dep_v[3], const T dep_d[3],
-                             const ModuleRec& arr, const Traj& y, const double Bd[3], double mass, T J[5][5]) {
+                             const ModuleRec& arr, const Traj& y, const double Bd[3], double mass, T J[5][5],
+                             const JacR<TD>* R = nullptr) {
   const double lam = KAPPA * y.qop;
   double kd[3];
   cross3(y.d, Bd, kd);
@@ -116,8 +117,8 @@ CKF_HD void arrival_jacobian(const Jac<TD>& D, const double dep_u[3], const doub
   for (int i = 0; i < 3; ++i) {
     k[i] = (T)(lam * kd[i]);
     n[i] = (T)arr.n[i];
-    u0[i] = (T)dep_u[i];
-    v0[i] = (T)dep_v[i];
+    u0[i] = R ? (T)R->Ru[i] : (T)dep_u[i];   // dr/dl0, dr/dl1: the departure axes unless J2' transported them
+    v0[i] = R ? (T)R->Rv[i] : (T)dep_v[i];
     dT[i] = (T)y.d[i];
   }
   const T nd = dot3(n, dT);
@@ -167,6 +168,10 @@ CKF_HD void arrival_jacobian(const Jac<TD>& D, const double dep_u[3], const doub
     for (int j = 0; j < 3; ++j) row[j] = f[0] * D.Dd[0][j] + f[1] * D.Dd[1][j] + f[2] * D.Dd[2][j] - fk * nR[j];
     J[2 + a][0] = -fk * nu0;
     J[2 + a][1] = -fk * nv0;
+    if (R) {  // dd/dl0, dd/dl1 (zero without the gradient terms)
+      J[2 + a][0] += f[0] * (T)R->Du[0] + f[1] * (T)R->Du[1] + f[2] * (T)R->Du[2];
+      J[2 + a][1] += f[0] * (T)R->Dv[0] + f[1] * (T)R->Dv[1] + f[2] * (T)R->Dv[2];
+    }
     J[2 + a][2] = dot3(row, gphi);
     J[2 + a][3] = dot3(row, gth);
     J[2 + a][4] = (T)dot3(f, D.dq) - fk * nrq;
@@ -319,6 +324,15 @@ struct Move {
   bool targeted;        // the next trial's length m.h and B1 are set (P4 done for the current position)
 };
 
+// A move that also transports the two position columns of D (J2', config.field_gradient).
+template <typename T>
+struct MoveG : Move<T> {
+  JacR<T> Dr;
+};
+template <typename M> struct MoveTraits;
+template <typename T> struct MoveTraits<Move<T>> { typedef T Scalar; static constexpr bool kGrad = false; };
+template <typename T> struct MoveTraits<MoveG<T>> { typedef T Scalar; static constexpr bool kGrad = true; };
+
 // Departure state of a tip with bound parameters x on module `from` (J1, V5): global position and direction,
 // the direction again for the bound->free Jacobian, the Highland variances to add to C[phi][phi], C[theta][theta] on
 // leaving (dep[3], dep[4]) and, with rule E, q/p after the mean energy loss in the module (y.qop) with
@@ -371,6 +385,12 @@ CKF_HD void move_begin(Move<T>& m, const CfgDev& cfg, int from) {
   m.ib = inv_beta(m.y.qop, cfg.mass);
   m.dib = dinvbeta_dqop(m.y.qop, cfg.mass);
   m.phase = PH_START;
+}
+
+template <typename T>
+CKF_HD void move_begin(MoveG<T>& m, const GeoDev& g, const CfgDev& cfg, int from) {
+  move_begin(static_cast<Move<T>&>(m), cfg, from);
+  jacr_begin(m.Dr, g.mod[from].u, g.mod[from].v);
 }
 
 // The 3x3 neighbourhood a move in PH_START / PH_LANDED wants tested.  Returns false when no module can be
@@ -567,18 +587,20 @@ CKF_HD void set_trial(Move<T>& m, const FieldDev& fld, const CfgDev& cfg, double
 }
 
 // P5 / P6 once no further trial follows: stop, or close onto the surface with a field-free step.
-template <typename T>
-CKF_HD void land_or_stop(Move<T>& m, int st, double s) {
+template <typename M>
+CKF_HD void land_or_stop(M& m, int st, double s) {
   if (st != STOP_NONE) { m.stop = st; m.phase = PH_FIN; return; }
   straight_close(m.y, m.D, s, m.ib, m.dib);
+  if constexpr (MoveTraits<M>::kGrad) straight_close_r(m.Dr, s);
   m.phase = (m.phase == PH_PLANE) ? PH_FIN : PH_LANDED;
 }
 
 // One step of a move in PH_CYL / PH_PLANE: targeting + landing (P4, P5), else one RKN4 trial (P2, P3).  After an
 // accepted trial the next one is targeted at once and its stage-1 field read is issued BEFORE the Jacobian columns of
 // the accepted step are computed, so that the loads fly during that arithmetic.
-template <typename T>
-CKF_HD void move_step(Move<T>& m, const FieldDev& fld, const CfgDev& cfg, int& n_trials, int& n_accepted) {
+template <typename T, typename M>
+CKF_HD void move_step(M& m, const FieldDev& fld, const CfgDev& cfg, int& n_trials, int& n_accepted) {
+  constexpr bool GRAD = MoveTraits<M>::kGrad;
   if (!m.targeted) {   // a fresh position (start of a phase)
     double s = 0.0;
     const int st = target_distance(m, s);
@@ -587,7 +609,7 @@ CKF_HD void move_step(Move<T>& m, const FieldDev& fld, const CfgDev& cfg, int& n
   }
   if (++m.n_steps > cfg.max_rk_steps) { m.stop = STOP_STEP_LIMIT; m.phase = PH_FIN; return; }
   Trial<T> t;
-  rk_trial<T>(fld, m.y, m.B1, KAPPA * m.y.qop, m.h, t);
+  rk_trial<T, GRAD>(fld, m.y, m.B1, KAPPA * m.y.qop, m.h, t);
   ++n_trials;
   if (!isfinite(t.eps)) { m.stop = STOP_NUMERIC; m.phase = PH_FIN; return; }
   double f;
@@ -599,6 +621,8 @@ CKF_HD void move_step(Move<T>& m, const FieldDev& fld, const CfgDev& cfg, int& n
   }
   if (t.eps <= cfg.rk_tol) {
     const double h = m.h;
+    StepGrad<T> sg;
+    if constexpr (GRAD) step_gradients<T>(fld, m.y, h, t, sg);   // at the stage points of the step, from the state before it
     rk_accept_state<T>(m.y, h, t, m.ib);
     m.h_ctrl = fabs(h) * f;
     ++n_accepted;
@@ -607,7 +631,8 @@ CKF_HD void move_step(Move<T>& m, const FieldDev& fld, const CfgDev& cfg, int& n
     const int st = target_distance(m, s);
     const bool more = st == STOP_NONE && fabs(s) > cfg.surf_tol;
     if (more) set_trial(m, fld, cfg, s);            // the loads of the next trial's stage 1 start here ...
-    rk_accept_jac<T>(m.y, m.D, h, t, m.dib);        // ... and fly while D <- D_step D is computed
+    if constexpr (GRAD) rk_accept_jac_g<T>(m.y.qop, m.D, m.Dr, h, t, sg, m.dib);
+    else rk_accept_jac<T>(m.y, m.D, h, t, m.dib);   // ... and fly while D <- D_step D is computed
     if (!more) land_or_stop(m, st, s);              // the closing drift acts on the updated D
   } else {
     m.h = m.h * f;                                  // retry from the same position: same B1
@@ -618,12 +643,12 @@ CKF_HD void move_step(Move<T>& m, const FieldDev& fld, const CfgDev& cfg, int& n
 // block.  Returns the final stop reason (NUMERIC if a predicted parameter is not finite).
 template <typename T>
 CKF_HD int move_arrive(const Move<T>& m, const double dep[NDEP], const GeoDev& g, const FieldDev& fld, const CfgDev& cfg,
-                       double xp[6], double J[5][5]) {
+                       double xp[6], double J[5][5], const JacR<T>* R = nullptr) {
   const ModuleRec& k = g.mod[m.tgt];
   const ModuleRec& m0 = g.mod[m.from];
   double B[3];
   field_at(fld, m.y.r, B);
-  arrival_jacobian<double, T>(m.D, m0.u, m0.v, dep, k, m.y, B, cfg.mass, J);
+  arrival_jacobian<double, T>(m.D, m0.u, m0.v, dep, k, m.y, B, cfg.mass, J, R);
   const double rel[3] = {m.y.r[0] - k.c[0], m.y.r[1] - k.c[1], m.y.r[2] - k.c[2]};
   xp[0] = dot3(rel, k.u);
   xp[1] = dot3(rel, k.v);
@@ -638,15 +663,16 @@ CKF_HD int move_arrive(const Move<T>& m, const double dep[NDEP], const GeoDev& g
 }
 
 // One tip at a time (host test harness): the transitions above in their natural order.
-template <typename T>
-CKF_HD int move_to_next_module(const GeoDev& g, const FieldDev& fld, const CfgDev& cfg, int from, const double x[6],
-                               int& target, double xp[6], double J[5][5], double& q_phi, double& q_theta, double& g_e,
-                               StepCtl& sc) {
-  Move<T> m;
+template <typename T, typename M>
+CKF_HD int move_to_next_module_impl(const GeoDev& g, const FieldDev& fld, const CfgDev& cfg, int from, const double x[6],
+                                    int& target, double xp[6], double J[5][5], double& q_phi, double& q_theta, double& g_e,
+                                    StepCtl& sc) {
+  M m;
   double dep[NDEP];
   const int st0 = departure_state(g, cfg, from, x, m.y, dep);
   if (st0 != STOP_NONE) return st0;
-  move_begin(m, cfg, from);
+  if constexpr (MoveTraits<M>::kGrad) move_begin(m, g, cfg, from);
+  else move_begin(m, cfg, from);
   while (m.phase != PH_FIN) {
     if (m.phase == PH_START || m.phase == PH_LANDED) {
       PickRequest q;
@@ -654,16 +680,25 @@ CKF_HD int move_to_next_module(const GeoDev& g, const FieldDev& fld, const CfgDe
       const int tgt = what == PICK_TEST ? pick_in_neighbourhood(g, q.layer, q.iphi, q.iz, q.exclude, m.y.r, m.y.d, q.s_min) : -1;
       move_pick_apply(m, g, tgt);
     } else {
-      move_step(m, fld, cfg, sc.n_trials, sc.n_accepted);
+      move_step<T>(m, fld, cfg, sc.n_trials, sc.n_accepted);
     }
   }
   q_phi = dep[3];
   q_theta = dep[4];
   g_e = dep[5];
   if (m.stop != STOP_NONE) return m.stop;
-  const int st = move_arrive(m, dep, g, fld, cfg, xp, J);
+  int st;
+  if constexpr (MoveTraits<M>::kGrad) st = move_arrive<T>(m, dep, g, fld, cfg, xp, J, &m.Dr);
+  else st = move_arrive<T>(m, dep, g, fld, cfg, xp, J);
   if (st == STOP_NONE) target = m.tgt;
   return st;
+}
+template <typename T>
+CKF_HD int move_to_next_module(const GeoDev& g, const FieldDev& fld, const CfgDev& cfg, int from, const double x[6],
+                               int& target, double xp[6], double J[5][5], double& q_phi, double& q_theta, double& g_e,
+                               StepCtl& sc) {
+  if (cfg.field_gradient) return move_to_next_module_impl<T, MoveG<T>>(g, fld, cfg, from, x, target, xp, J, q_phi, q_theta, g_e, sc);
+  return move_to_next_module_impl<T, Move<T>>(g, fld, cfg, from, x, target, xp, J, q_phi, q_theta, g_e, sc);
 }
 
 }  // namespace ckf

@@ -7,6 +7,7 @@
 // module choice wait until FETCH_MIN / PICK_MIN of them have gathered (or no lane can step), then are served together.
 // The module choice spreads its nine straight-line tests per tip over all 32 lanes.
 #pragma once
+#include <type_traits>
 #include "ckf_kernels.cuh"
 
 namespace ckf {
@@ -93,7 +94,7 @@ __device__ __forceinline__ void pick_warp(const GeoDev& geo, const PickSmem& ps,
   __syncwarp();
 }
 
-template <typename T, int MINB>
+template <typename T, int MINB, bool GRAD = false>
 __global__ void __launch_bounds__(STEP_NT, MINB) ckf_step(const KParams<T> p, int level) {
   chain_enter();
   if (p.g[G_NTIPS0 + (level & 1)] == 0 || level == 0) return;  // level 0: the seed's own module, identity transport (N6)
@@ -111,7 +112,8 @@ __global__ void __launch_bounds__(STEP_NT, MINB) ckf_step(const KParams<T> p, in
   ps.carve(smem_raw + (size_t)wib * PickSmem::bytes());
   const size_t TC = (size_t)p.tcap;
 
-  Move<T> m;
+  typename std::conditional<GRAD, MoveG<T>, Move<T>>::type m;
+  if constexpr (GRAD) jacr_begin(m.Dr, p.geo.mod[0].u, p.geo.mod[0].v);
   m.phase = PH_IDLE; m.stop = STOP_NONE; m.from = 0; m.tgt = -1; m.lp = 0; m.lb = -1; m.ld = -1; m.n_steps = 0; m.targeted = false; m.inward = false;
   m.B1[0] = m.B1[1] = m.B1[2] = 0.0;
   m.h = 0.0; m.h_ctrl = 0.0; m.R = 0.0; m.y.qop = 0.0; m.ib = 0.0; m.dib = 0.0;
@@ -130,6 +132,7 @@ __global__ void __launch_bounds__(STEP_NT, MINB) ckf_step(const KParams<T> p, in
         if (m.stop == STOP_NONE) {
           store_traj(p.mv_y, (size_t)tip, m.y);
           store_jac(p.mv_D, (size_t)tip, m.D);
+          if constexpr (GRAD) store_jacr(p.mv_Dr, (size_t)tip, m.Dr);
           p.mv_tgt[tip] = m.tgt;
         }
         p.mv_stop[tip] = m.stop;
@@ -152,7 +155,8 @@ __global__ void __launch_bounds__(STEP_NT, MINB) ckf_step(const KParams<T> p, in
         if (t >= 0) {  // every tip of the schedule is live (ckf_update / ckf_fit_level only append live ones)
           tip = t;
           load_traj(p.mv_y, (size_t)t, m.y);
-          move_begin<T>(m, p.cfg, p.mv_from[t]);
+          if constexpr (GRAD) move_begin(m, p.geo, p.cfg, p.mv_from[t]);
+          else move_begin<T>(m, p.cfg, p.mv_from[t]);
           move_pick_apply<T>(m, p.geo, p.mv_tgt[TC + t]);  // N2 was decided by ckf_update
         }
       }

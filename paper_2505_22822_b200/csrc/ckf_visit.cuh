@@ -152,7 +152,7 @@ __device__ __forceinline__ int gate_chunk(const KParams<T>& p, const VSmem<T>& s
   return nsel;
 }
 
-template <typename T, int MINB>
+template <typename T, int MINB, bool GRAD = false>
 __global__ void __launch_bounds__(VISIT_NT, MINB) ckf_visit(const KParams<T> p, int level) {
   chain_enter();
   const int n = p.g[G_NTIPS0 + (level & 1)];
@@ -214,7 +214,13 @@ __global__ void __launch_bounds__(VISIT_NT, MINB) ckf_visit(const KParams<T> p, 
           for (int i = 0; i < NDEP; ++i) dep[i] = p.mv_dep[i * TC + t];
           double xp[6];
           double J[5][5];
-          stop = move_arrive<T>(m, dep, p.geo, p.fld, p.cfg, xp, J);
+          if constexpr (GRAD) {
+            JacR<T> R;
+            load_jacr(p.mv_Dr, (size_t)t, R);
+            stop = move_arrive<T>(m, dep, p.geo, p.fld, p.cfg, xp, J, &R);
+          } else {
+            stop = move_arrive<T>(m, dep, p.geo, p.fld, p.cfg, xp, J);
+          }
           if (stop == STOP_NONE) {
             target = m.tgt;
             double C[21], Co[21];

@@ -43,7 +43,7 @@ class CKFSettings:
     max_rk_steps_per_surface: int = 64
     max_levels: int = 32
     energy_loss: int = 0          # rule E (mean energy loss per module); BASELINE configs: off
-    field_gradient: int = 0       # transport Jacobian with field-gradient terms (oracle only); BASELINE configs: off
+    field_gradient: int = 0       # transport Jacobian with field-gradient terms (rule J2'); BASELINE configs: off
     bidirectional: int = 0        # navigate radially inward-moving tips too (row f3); BASELINE configs: off (reading A7)
 
 

@@ -35,6 +35,7 @@ def lib():
         L.hm_move.argtypes = [C.c_void_p, C.c_int, C.c_int, _dp, _dp, _ip, _dp, _dp, _ip]
         L.hm_update.argtypes = [C.c_int, _dp, _dp, _dp, _dp, _dp, _dp, _dp]
         L.hm_field.argtypes = [C.c_void_p, _dp, _dp]
+        L.hm_field_gradient.argtypes = [C.c_void_p, _dp, _dp]
         _lib = L
     return _lib
 
@@ -71,6 +72,12 @@ class HostMath:
         b = np.zeros(3)
         lib().hm_field(self.ctx, r.ctypes.data_as(_dp), b.ctypes.data_as(_dp))
         return b
+
+    def field_gradient(self, r):
+        r = np.ascontiguousarray(r, np.float64)
+        g = np.zeros(9)
+        lib().hm_field_gradient(self.ctx, r.ctypes.data_as(_dp), g.ctypes.data_as(_dp))
+        return g.reshape(3, 3)
 
     def __del__(self):
         try:

@@ -84,6 +84,7 @@ void* hm_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c) 
   x->cfg.max_cands = c->max_candidates_per_seed; x->cfg.max_holes = c->max_holes; x->cfg.min_meas = c->min_measurements;
   x->cfg.max_rk_steps = c->max_rk_steps_per_surface; x->cfg.max_levels = c->max_levels;
   x->cfg.energy_loss = c->energy_loss ? 1 : 0;
+  x->cfg.field_gradient = (c->field_gradient == 1 && f->kind == 1) ? 1 : 0;
   return x;
 }
 void hm_destroy(void* p) { delete (Ctx*)p; }
@@ -99,4 +100,10 @@ void hm_update(int precision, const double* x, const double* C36, const double* 
   else update_t<double>(x, C36, loc, var, xo, Co36, chi2);
 }
 void hm_field(void* p, const double* r, double* B) { field_at(((Ctx*)p)->fld, r, B); }
+void hm_field_gradient(void* p, const double* r, double* G9) {
+  double G[3][3];
+  field_gradient_at(((Ctx*)p)->fld, r, G);
+  for (int i = 0; i < 3; ++i)
+    for (int j = 0; j < 3; ++j) G9[3 * i + j] = G[i][j];
+}
 }

@@ -1021,3 +1021,50 @@ def test_launch_overlap_policy_same_result(monkeypatch):
             for k in ref:
                 assert got[k] == ref[k], (mask, rep, k)
         ckf.close()
+
+
+@pytest.mark.parametrize("precision", [64, 32])
+def test_field_gradient_parity(precision):
+    """Row f3, J2' (config.field_gradient = 1, reading A13): ckf_find and ckf_fit with the field-gradient terms of the
+    transport Jacobian, through the inhomogeneous grid field of configs[2], against the oracle with the same flag --
+    fp64 (the float32 arrays of the event widened: bit-exact lists, 1e-9) and fp32.  The terms matter: the oracle's
+    covariances with and without them differ by far more than the parity bar."""
+    import copy
+    import dataclasses
+    import torch
+    import oracle
+    det, fld, cfg = synth.config_bundle(2)
+    cfg = dataclasses.replace(cfg, precision=precision, ckf=copy.deepcopy(cfg.ckf))
+    cfg.ckf.field_gradient = 1
+    ev = synth.make_event(2, det=det, n_particles=3000)
+    ora = _run_oracle(det, fld, cfg, ev)
+    ckf, dev, out, gpu, cnt = _run_gpu(det, fld, cfg, ev)
+    assert gpu.status == 0 and gpu.n_tracks > 3000
+    if precision == 64:
+        parity.assert_bit_exact_lists(gpu, ora)
+        rel, chi2, cov = parity.max_param_diffs(gpu, ora)
+        assert rel < 1e-9 and chi2 < 1e-8 and cov < 1e-7, (rel, chi2, cov)
+        for k in ("visits", "rk_trials", "rk_accepted", "gate_tests", "updates", "tips"):
+            assert cnt[k] == ora.counters[k], k
+    else:
+        r = parity.assert_fp32_parity(gpu, ora, ev.n_seeds, cfg.ckf.chi2_max, "field gradient, configs[2]")
+        print("field gradient fp32", {k: v for k, v in r.items() if k != "bad_seeds"})
+    cfg0 = dataclasses.replace(cfg, ckf=copy.deepcopy(cfg.ckf))
+    cfg0.ckf.field_gradient = 0
+    ora0 = _run_oracle(det, fld, cfg0, ev)
+    if ora0.n_tracks == ora.n_tracks and np.array_equal(ora0.meas_idx, ora.meas_idx):
+        d = np.abs(ora.cov - ora0.cov).reshape(ora.n_tracks, 6, 6)
+        sc = np.sqrt(np.einsum("ti,tj->tij", ora.cov.reshape(-1, 6, 6)[:, range(6), range(6)],
+                               ora.cov.reshape(-1, 6, 6)[:, range(6), range(6)]))
+        assert float(np.max(d / sc)) > 1e-4        # parity bars: 1e-7 (fp64), a few 1e-6 (fp32)
+    fits = ckf.alloc_fits()
+    for smoother in (0, 1):
+        ckf.fit(dev, out, fits, smoother=smoother)
+        torch.cuda.synchronize()
+        g = ckf.download_fits(fits, gpu.n_tracks, int(gpu.meas_idx.size))
+        o = oracle.kf_fit(oracle.Setup(det, fld, cfg.ckf), ev, gpu.track_offsets, gpu.meas_idx, gpu.seed_id, n_threads=8,
+                          smoother=smoother)
+        rf = parity.compare_fits(g, o, gpu.track_offsets)
+        tol = 1e-9 if precision == 64 else 1e-5
+        assert rf["n_not_pd_gpu_only"] == 0 and rf["max_smoothed_rel"] < tol and rf["max_last_rel"] < tol, (smoother, rf)
+    ckf.close()

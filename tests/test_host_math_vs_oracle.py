@@ -150,3 +150,67 @@ def test_bidirectional_moves_match_oracle(endcap):
             n_inward += int(np.dot(d, nrm) < 0.0)
             x, Cm, m = xo, Co, tgo
     assert n_moves > 2000 and n_inward > 80 and n_exit > 250, (n_moves, n_inward, n_exit)
+
+
+def test_field_gradient_read_is_the_derivative_of_the_field_read():
+    """J2' on the CUDA side: field_gradient_at against central differences of ITS OWN field_at inside a cell (the
+    interpolant is trilinear: the difference quotient along one axis is exact up to rounding), at random points."""
+    det, fld, cfg = synth.config_bundle(2)
+    hm = HostMath(det, fld, cfg.ckf)
+    rng = np.random.default_rng(5)
+    sp = float(fld.spacing[0])
+    worst = 0.0
+    for _ in range(200):
+        cell = rng.integers(2, int(fld.n[0]) - 3, 3)
+        r = fld.origin + sp * (cell + rng.uniform(0.2, 0.8, 3))
+        G = hm.field_gradient(r)
+        for j in range(3):
+            e = np.zeros(3)
+            e[j] = 0.1 * sp
+            fd = (hm.field(r + e) - hm.field(r - e)) / (2 * e[j])
+            worst = max(worst, float(np.max(np.abs(G[:, j] - fd))))
+    scale = float(np.max(np.abs(hm.field_gradient(fld.origin + sp * 20.3))))
+    assert scale > 1e-7 and worst < 1e-9 * max(1.0, scale / 1e-6), (worst, scale)
+
+
+@pytest.mark.parametrize("precision,tol_x,tol_c", [(64, 1e-10, 1e-9), (32, 1e-9, 2e-6)])
+def test_moves_with_field_gradient_match_oracle(precision, tol_x, tol_c):
+    """Row f3, J2' (config.field_gradient = 1, reading A13): the CUDA path's transport with the field-gradient terms
+    (MoveG: the d-, q- and the two position columns pushed through the four stages, csrc/ckf_math.cuh) against the
+    oracle's 8 x 8 tangent form, move by move through the inhomogeneous grid field of config 2 -- and the terms must
+    matter: against the oracle WITHOUT them the same covariances differ by far more than the tolerance."""
+    import copy
+    det, fld, cfg = synth.config_bundle(2)
+    cfg = copy.deepcopy(cfg)
+    cfg.ckf.field_gradient = 1
+    off = copy.deepcopy(cfg)
+    off.ckf.field_gradient = 0
+    ev = synth.make_event(2, det=det, n_particles=60, n_fake_seeds=0)
+    st, st_off = oracle.Setup(det, fld, cfg.ckf), oracle.Setup(det, fld, off.ckf)
+    hm = HostMath(det, fld, cfg.ckf)
+    floor_x = np.array([1.0, 1.0, 1.0, 1.0, 0.0, 1.0])
+    n_moves, worst_c, effect = 0, 0.0, 0.0
+    for s in range(ev.n_seeds):
+        x = ev.seed_params[s].astype(np.float64)
+        Cm = ev.seed_cov[s].reshape(6, 6).astype(np.float64)
+        m = int(ev.seed_module[s])
+        for level in range(1, 14):
+            co, tgo, xo, Co, _ = oracle.move(st, m, x, Cm)
+            tro = oracle.last_move_trials()
+            ch, tgh, xh, Ch, trh = hm.move(precision, m, x, Cm)
+            assert co == ch
+            if co != 0:
+                break
+            assert tgo == tgh and tro == trh
+            fl = floor_x.copy()
+            fl[4] = abs(xo[4])
+            assert np.max(_rel(xo, xh, fl)) < tol_x
+            scale = np.sqrt(np.outer(np.diag(Co), np.diag(Co)))
+            worst_c = max(worst_c, float(np.max(np.abs(Co - Ch) / scale)))
+            _, _, x0, C0, _ = oracle.move(st_off, m, x, Cm)
+            assert np.array_equal(x0, xo)                        # the flag never touches the state
+            effect = max(effect, float(np.max(np.abs(Co - C0) / scale)))
+            n_moves += 1
+            x, Cm, m = xo, Co, tgo
+    assert n_moves > 400 and worst_c < tol_c, (n_moves, worst_c)
+    assert effect > 100 * tol_c, effect
