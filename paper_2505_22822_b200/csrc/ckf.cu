@@ -281,7 +281,7 @@ int launch_find(ckf_handle* h, Workspace& w, const ckf_measurements* m, const ck
   // seeds/s), so the launches stay plain.  Timing mode puts an event between the kernels, which serialises them anyway.
   const int ovm = (h->timing || others_in_flight(h, &w, st)) ? 0 : h->chain_overlap;
   ckf_init_event<T><<<nb, 256, 0, st>>>(p); mark(0);  // plain launch: whatever precedes the find in the stream is not ours
-  launch_chain(ckf_sort_slices<T>, h->sm_count * 8, SORT_NT, 0, st, ovm & 1, p); mark(1);
+  launch_chain(ckf_sort_slices<T>, h->sm_count * (1024 / SORT_NT), SORT_NT, 0, st, ovm & 1, p); mark(1);
   // level loop: tips of level l were made by level l - 1; a tip at max_levels only stops (LEVEL_LIMIT) and emits.
   // Kernels of an empty level return at once, so the loop needs no host read of the level's size.
   const int wide = h->sm_count * 4;

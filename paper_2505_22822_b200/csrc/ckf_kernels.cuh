@@ -24,7 +24,7 @@ constexpr int CAND = 16;          // per-tip passer buffer of the gate fast path
 constexpr int STEP_NT = 128;      // threads per block of ckf_step
 constexpr int VISIT_NT = 128;     // threads per block of ckf_visit (4 warps, 32 tips each)
 constexpr int SCAN_NT = 256;      // threads per block of ckf_scan / ckf_update; tile of the scan
-constexpr int SORT_NT = 128;      // threads per block of the slice sort
+constexpr int SORT_NT = 512;      // threads per block of the slice sort
 constexpr int SORT_CAP = 2048;    // largest module slice sorted in shared memory; larger ones stay unsorted
 #ifndef CKF_FETCH_MIN
 #define CKF_FETCH_MIN 32

@@ -12,7 +12,8 @@
 namespace ckf {
 
 // Slices of at most 32 measurements (most modules) are rank-sorted by ONE warp with shuffles, four modules per
-// block at a time; longer slices by the whole block with a bitonic sort in shared memory.  Slices longer than
+// block at a time; slices of up to SORT_WARP_MAX by one warp through shared memory; longer slices by the whole block
+// with a bitonic sort in shared memory.  Slices longer than
 // SORT_CAP, or holding a variance that is not a positive finite number, are copied through unsorted and flagged
 // (s_v0max < 0): their tips gate the whole slice.
 template <typename T>
@@ -55,6 +56,66 @@ __device__ __forceinline__ void sort_slice_warp(const KParams<T>& p, int m, int 
   if (lane == 0) p.s_v0max[m] = any_bad ? T(-1) : vmax;
 }
 
+// Slices of 33 .. SORT_WARP_MAX measurements: still one warp, keys staged in the warp's own shared-memory strip, every
+// lane ranks its (up to SORT_WARP_MAX / 32) keys against all of them (broadcast reads).  Same order as the other paths:
+// ascending (loc0, index), NaN last.
+constexpr int SORT_WARP_MAX = 128;
+template <typename T>
+__device__ __forceinline__ void sort_slice_warp_mid(const KParams<T>& p, int m, int beg, int n, int lane, T* wkey) {
+  constexpr int PER = SORT_WARP_MAX / 32;
+  typename Vec2<T>::type lc[PER], vr[PER];
+  T vmax = T(0);
+  bool bad = false;
+#pragma unroll
+  for (int k = 0; k < PER; ++k) {
+    const int i = lane + 32 * k;
+    if (i < n) {
+      lc[k] = p.loc[beg + i];
+      vr[k] = p.var[beg + i];
+      T key = lc[k].x;
+      if (!(key == key)) key = (T)INFINITY;
+      wkey[i] = key;
+      bad = bad || !(vr[k].x > T(0)) || !(vr[k].y > T(0)) || !isfinite(vr[k].x) || !isfinite(vr[k].y);
+      vmax = vr[k].x > vmax ? vr[k].x : vmax;
+    }
+  }
+  __syncwarp();
+  const bool any_bad = __any_sync(0xffffffffu, bad);
+#pragma unroll
+  for (int o = 16; o > 0; o >>= 1) {
+    const T ov = __shfl_xor_sync(0xffffffffu, vmax, o);
+    vmax = ov > vmax ? ov : vmax;
+  }
+  int rank[PER];
+#pragma unroll
+  for (int k = 0; k < PER; ++k) rank[k] = 0;
+  if (!any_bad) {
+    T key[PER];
+#pragma unroll
+    for (int k = 0; k < PER; ++k) key[k] = (lane + 32 * k < n) ? wkey[lane + 32 * k] : (T)INFINITY;
+    for (int j = 0; j < n; ++j) {
+      const T kj = wkey[j];
+#pragma unroll
+      for (int k = 0; k < PER; ++k) rank[k] += key_less<T>(kj, j, key[k], lane + 32 * k) ? 1 : 0;
+    }
+  }
+#pragma unroll
+  for (int k = 0; k < PER; ++k) {
+    const int i = lane + 32 * k;
+    if (i < n) {
+      const int r = any_bad ? i : rank[k];
+      p.s_loc[beg + r] = lc[k];
+      p.s_var[beg + r] = vr[k];
+      p.s_idx[beg + r] = beg + i;
+    }
+  }
+  if (lane == 0) p.s_v0max[m] = any_bad ? T(-1) : vmax;
+  __syncwarp();  // the strip is reused by the warp's next module
+}
+
+// Module m of (round r, block b, warp w) is r * G * MPB + w * G + b (G = gridDim.x): consecutive modules -- the crowded
+// inner-layer ones have consecutive ids -- land on different blocks.  A warp sorts its module if the slice holds at
+// most SORT_WARP_MAX measurements; the longer ones of a round are then sorted by the whole block, one after the other.
 template <typename T>
 __global__ void __launch_bounds__(SORT_NT) ckf_sort_slices(const KParams<T> p) {
   chain_enter();
@@ -62,10 +123,14 @@ __global__ void __launch_bounds__(SORT_NT) ckf_sort_slices(const KParams<T> p) {
   __shared__ int32_t s_id[SORT_CAP];
   __shared__ T s_red[SORT_NT / 32];
   __shared__ int s_bad;
+  constexpr int MPB = SORT_NT / 32;  // modules taken per block and round, one per warp
+  __shared__ T s_wkey[MPB][SORT_WARP_MAX];
+  __shared__ int s_long[MPB];
   const int tid = threadIdx.x, lane = tid & 31, warp = tid >> 5;
-  constexpr int MPB = SORT_NT / 32;  // small modules taken per block and round, one per warp
-  for (int m0 = blockIdx.x * MPB; m0 < p.n_vmod; m0 += gridDim.x * MPB) {
-    const int mw = m0 + warp;
+  const int G = gridDim.x;
+  for (int m0 = 0; m0 < p.n_vmod; m0 += G * MPB) {   // same trip count for every thread of the block
+    const int mw = m0 + warp * G + (int)blockIdx.x;
+    int is_long = -1;
     if (mw < p.n_vmod) {
       int begw, endw;
       slice_of<T>(p, mw, begw, endw);
@@ -75,16 +140,17 @@ __global__ void __launch_bounds__(SORT_NT) ckf_sort_slices(const KParams<T> p) {
         if (rb != begw || re != endw) atomicOr(p.g + G_BAD_INPUT, 1);
       }
       if (nw <= 32) sort_slice_warp<T>(p, mw, begw, nw, lane);
+      else if (nw <= SORT_WARP_MAX) sort_slice_warp_mid<T>(p, mw, begw, nw, lane, s_wkey[warp]);
+      else is_long = mw;
     }
-  }
-  // long slices: one block per module, consecutive modules on different blocks (the crowded inner-layer
-  // modules have consecutive ids)
-  {
-    for (int m = blockIdx.x; m < p.n_vmod; m += gridDim.x) {
+    if (lane == 0) s_long[warp] = is_long;
+    __syncthreads();
+    for (int q = 0; q < MPB; ++q) {
+      const int m = s_long[q];
+      if (m < 0) continue;
       int beg, end;
       slice_of<T>(p, m, beg, end);
       const int n = end - beg;
-      if (n <= 32) continue;
       __syncthreads();
       if (tid == 0) s_bad = 0;
       __syncthreads();
@@ -157,6 +223,7 @@ __global__ void __launch_bounds__(SORT_NT) ckf_sort_slices(const KParams<T> p) {
         p.s_v0max[m] = v;
       }
     }
+    __syncthreads();  // s_long is rewritten by the next round
   }
 }
 
