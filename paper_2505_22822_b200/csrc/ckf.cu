@@ -297,7 +297,7 @@ int launch_find(ckf_handle* h, Workspace& w, const ckf_measurements* m, const ck
     launch_chain(ckf_update<T>, wide, SCAN_NT, 0, st, ovm & 16, p, level); mark(6);
   }
   launch_chain(ckf_scan_seeds<T>, (s->n + SEED_TILE - 1) / SEED_TILE + 1, SEED_TILE, 0, st, ovm & 32, p); mark(7);
-  launch_chain(ckf_emit_tracks<T>, h->sm_count * 4, 256, 0, st, ovm & 32, p); mark(8);
+  launch_chain(ckf_emit_tracks<T>, h->sm_count * 8, EMIT_NT, 0, st, ovm & 32, p); mark(8);
   launch_chain(ckf_finalize<T>, 1, 1, 0, st, ovm & 32, p); mark(9);
   w.last_launches = 5 + 4 * (h->cfg.max_levels + 1) - 1;
   if (h->timing) {

@@ -88,57 +88,98 @@ __global__ void __launch_bounds__(SEED_TILE) ckf_scan_seeds(const KParams<T> p) 
   }
 }
 
-// Thread per candidate: backtrace the links into the index list, copy the state at the last measurement.
+// Thread per candidate: backtrace the links into the index list, copy the state at the last measurement.  The 6 + 36
+// numbers per candidate are transposed through a shared-memory tile of the warp, so that the 32 candidates of a warp
+// (consecutive in the output) are written as contiguous runs instead of 42 stores of stride 24 / 144 bytes per lane.
+constexpr int EMIT_NT = 128;
 template <typename T>
-__global__ void __launch_bounds__(256) ckf_emit_tracks(const KParams<T> p) {
+__global__ void __launch_bounds__(EMIT_NT) ckf_emit_tracks(const KParams<T> p) {
   chain_enter();
+  __shared__ T s_tile[EMIT_NT / 32][32 * 37];
+  const int lane = threadIdx.x & 31;
+  T* tile = s_tile[threadIdx.x >> 5];
   const int total = p.g[G_TOTAL_TRACKS];
   const int cap = p.cfg.max_cands;
   const int ntiles = p.n_seeds > 0 ? (p.n_seeds + SEED_TILE - 1) / SEED_TILE : 1;
   const int32_t* tile_trk = p.seed_tile;
   const int32_t* tile_ent = p.seed_tile + (p.seed_tiles_cap + 1);
-  for (int t = blockIdx.x * blockDim.x + threadIdx.x; t < total; t += gridDim.x * blockDim.x) {
-    // seed = last s with (tile offset + in-tile prefix) <= t: tile first, then inside the tile
-    int lo = 0, hi = ntiles;
-    while (hi - lo > 1) {
-      const int mid = (lo + hi) >> 1;
-      if (tile_trk[mid] <= t) lo = mid; else hi = mid;
+  const int stride = gridDim.x * blockDim.x;
+  for (int t0 = (blockIdx.x * blockDim.x + threadIdx.x) - lane; t0 < total; t0 += stride) {   // warp-uniform
+    const int t = t0 + lane;
+    bool ok = t < total;
+    int ls = 0;
+    if (ok) {
+      // seed = last s with (tile offset + in-tile prefix) <= t: tile first, then inside the tile
+      int lo = 0, hi = ntiles;
+      while (hi - lo > 1) {
+        const int mid = (lo + hi) >> 1;
+        if (tile_trk[mid] <= t) lo = mid; else hi = mid;
+      }
+      const int toff = tile_trk[lo], eoff = tile_ent[lo];
+      int a = lo * SEED_TILE, b = min(p.n_seeds, a + SEED_TILE);
+      while (b - a > 1) {
+        const int mid = (a + b) >> 1;
+        if (toff + p.sd_track_base[mid] <= t) a = mid; else b = mid;
+      }
+      const int seed = a, j = t - (toff + p.sd_track_base[seed]);
+      const size_t li = (size_t)seed * cap + j;
+      const int leaf = p.leaf_link[li], meta = p.leaf_meta[li];
+      const int off = eoff + p.sd_entry_base[seed] + p.leaf_entry[li];
+      const int nm = p.lk_counts[leaf] & 0xffff;
+      if (t >= p.max_tracks || off + nm > p.max_entries) {
+        atomicMin(p.g + G_FIRST_BAD, t);
+        atomicOr(p.o_status, t >= p.max_tracks ? 1 : 2);
+        ok = false;
+      } else {
+        p.o_offsets[t] = off;
+        p.o_offsets[t + 1] = off + nm;
+        int pos = off + nm - 1;
+        for (int l = leaf; l >= 0; l = p.lk_parent[l]) {
+          const int m = p.lk_meas[l];
+          if (m >= 0) { p.o_meas[pos] = m; p.o_entrychi2[pos] = p.lk_chi2[l]; --pos; }
+        }
+        ls = p.lk_lastmeas[leaf];
+        p.o_seed[t] = seed;
+        p.o_nholes[t] = meta >> 8;
+        p.o_stop[t] = meta & 0xff;
+        p.o_lastmod[t] = p.lk_module[ls];
+        p.o_chi2sum[t] = (T)p.lk_chi2sum[leaf];
+      }
     }
-    const int toff = tile_trk[lo], eoff = tile_ent[lo];
-    int a = lo * SEED_TILE, b = min(p.n_seeds, a + SEED_TILE);
-    while (b - a > 1) {
-      const int mid = (a + b) >> 1;
-      if (toff + p.sd_track_base[mid] <= t) a = mid; else b = mid;
-    }
-    const int seed = a, j = t - (toff + p.sd_track_base[seed]);
-    const size_t li = (size_t)seed * cap + j;
-    const int leaf = p.leaf_link[li], meta = p.leaf_meta[li];
-    const int off = eoff + p.sd_entry_base[seed] + p.leaf_entry[li];
-    const int nm = p.lk_counts[leaf] & 0xffff;
-    if (t >= p.max_tracks || off + nm > p.max_entries) {
-      atomicMin(p.g + G_FIRST_BAD, t);
-      atomicOr(p.o_status, t >= p.max_tracks ? 1 : 2);
-      continue;
-    }
-    p.o_offsets[t] = off;
-    p.o_offsets[t + 1] = off + nm;
-    int pos = off + nm - 1;
-    for (int l = leaf; l >= 0; l = p.lk_parent[l]) {
-      const int m = p.lk_meas[l];
-      if (m >= 0) { p.o_meas[pos] = m; p.o_entrychi2[pos] = p.lk_chi2[l]; --pos; }
-    }
-    const int ls = p.lk_lastmeas[leaf];
-    p.o_seed[t] = seed;
-    p.o_nholes[t] = meta >> 8;
-    p.o_stop[t] = meta & 0xff;
-    p.o_lastmod[t] = p.lk_module[ls];
-    p.o_chi2sum[t] = (T)p.lk_chi2sum[leaf];
+    const unsigned okm = __ballot_sync(0xffffffffu, ok);
+    if (okm == 0u) continue;
+    // covariance: lane's row of the tile (row stride 37: conflict-free), then the tile row-major to the output
+    if (ok) {
 #pragma unroll
-    for (int i = 0; i < 6; ++i) p.o_params[(size_t)t * 6 + i] = (T)p.lk_x[(size_t)i * p.max_links + ls];
+      for (int i = 0; i < 6; ++i)
 #pragma unroll
-    for (int i = 0; i < 6; ++i)
+        for (int k = 0; k < 6; ++k) tile[lane * 37 + i * 6 + k] = (T)p.lk_C[(size_t)tri(i, k) * p.max_links + ls];
+    }
+    __syncwarp();
+    {
+      int row = 0, col = lane;   // element lane + 32 * n of the 32 x 36 block
+      T* dst = p.o_cov + (size_t)t0 * 36;
+      for (int i = lane; i < 32 * 36; i += 32) {
+        if ((okm >> row) & 1u) dst[i] = tile[row * 37 + col];
+        col += 32;
+        if (col >= 36) { col -= 36; ++row; }
+      }
+    }
+    __syncwarp();
+    if (ok) {
 #pragma unroll
-      for (int k = 0; k < 6; ++k) p.o_cov[(size_t)t * 36 + i * 6 + k] = (T)p.lk_C[(size_t)tri(i, k) * p.max_links + ls];
+      for (int i = 0; i < 6; ++i) tile[lane * 7 + i] = (T)p.lk_x[(size_t)i * p.max_links + ls];
+    }
+    __syncwarp();
+    {
+      T* dst = p.o_params + (size_t)t0 * 6;
+#pragma unroll
+      for (int n = 0; n < 6; ++n) {
+        const int i = lane + 32 * n, row = i / 6, col = i - row * 6;
+        if ((okm >> row) & 1u) dst[i] = tile[row * 7 + col];
+      }
+    }
+    __syncwarp();
   }
 }
 
