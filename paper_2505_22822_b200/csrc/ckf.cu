@@ -86,7 +86,7 @@ struct ckf_handle {
   ModuleRec* d_mod = nullptr;
   LayerRec* d_layer = nullptr;
   GeoDev geo;   // device pointers + layer summary (barrel count, first discs)
-  double* d_grid = nullptr;
+  float* d_grid = nullptr;
   FieldDev fld;
   CfgDev kcfg;
   int step_grid = 0, step_regs = 0, visit_grid = 0, visit_smem = 0, tcap = 0, tsize = 4;
@@ -548,25 +548,24 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
     h->fld.inv[a] = f->kind == 1 ? 1.0 / f->spacing[a] : 0.0;
     h->fld.nm2[a] = (double)(f->n[a] - 2);
   }
-  if (f->kind == 1) {
-    const size_t np = (size_t)f->n[0] * f->n[1] * f->n[2];
-    std::vector<double> pad(4 * np);
-    for (size_t i = 0; i < np; ++i) {
-      pad[4 * i] = (double)f->grid[3 * i]; pad[4 * i + 1] = (double)f->grid[3 * i + 1];
-      pad[4 * i + 2] = (double)f->grid[3 * i + 2]; pad[4 * i + 3] = 0.0;
+  {
+    // device copy of the grid: entry (i, j, k) = node (i, j, k) and node (i, j, k + 1), 8 float32 (ld_pair); a uniform
+    // field still owns a 2 x 2 x 2 grid of its value: field_at never reads it (kind 0 returns first), but ld_pair is a
+    // plain asm load which the compiler may hoist above that test, so every address field_at can form must be
+    // readable -- with n = 2 the index clamps leave only cell 0
+    std::vector<float> pairs;
+    if (f->kind == 1) {
+      fill_field_pairs(f->grid, f->n, pairs);
+    } else {
+      const float ub[3] = {(float)f->uniform_b[0], (float)f->uniform_b[1], (float)f->uniform_b[2]};
+      float cube[8 * 3];
+      for (int i = 0; i < 8; ++i) for (int a = 0; a < 3; ++a) cube[3 * i + a] = ub[a];
+      const int32_t n2[3] = {2, 2, 2};
+      fill_field_pairs(cube, n2, pairs);
+      for (int a = 0; a < 3; ++a) { h->fld.n[a] = 2; h->fld.nm2[a] = 0.0; h->fld.org[a] = 0.0; h->fld.inv[a] = 0.0; }
     }
-    CKB(dalloc(h, &h->d_grid, 4 * np * sizeof(double)));
-    CKB(cudaMemcpy(h->d_grid, pad.data(), 4 * np * sizeof(double), cudaMemcpyHostToDevice));
-    h->fld.grid = h->d_grid;
-  } else {
-    // a uniform field still owns a 2 x 2 x 2 grid of its value: field_at never reads it (kind 0 returns first), but
-    // ld_node is a plain asm load which the compiler may hoist above that test, so every address field_at can form
-    // must be readable -- with n = 2 the index clamps leave only cell 0
-    std::vector<double> pad(4 * 8, 0.0);
-    for (int i = 0; i < 8; ++i) for (int a = 0; a < 3; ++a) pad[4 * i + a] = f->uniform_b[a];
-    for (int a = 0; a < 3; ++a) { h->fld.n[a] = 2; h->fld.nm2[a] = 0.0; h->fld.org[a] = 0.0; h->fld.inv[a] = 0.0; }
-    CKB(dalloc(h, &h->d_grid, pad.size() * sizeof(double)));
-    CKB(cudaMemcpy(h->d_grid, pad.data(), pad.size() * sizeof(double), cudaMemcpyHostToDevice));
+    CKB(dalloc(h, &h->d_grid, pairs.size() * sizeof(float)));
+    CKB(cudaMemcpy(h->d_grid, pairs.data(), pairs.size() * sizeof(float), cudaMemcpyHostToDevice));
     h->fld.grid = h->d_grid;
   }
   // ---- config

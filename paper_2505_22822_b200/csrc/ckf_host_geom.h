@@ -68,4 +68,17 @@ inline void fill_geo_summary(const std::vector<LayerRec>& layers, GeoDev& geo) {
   }
 }
 
+// Device layout of the field grid (ckf_math.cuh, ld_pair): entry (i, j, k) = node (i, j, k) then node (i, j, k + 1),
+// each (Bx, By, Bz, 0) as float32; the last entry along z repeats its own node (no cell starts there).
+inline void fill_field_pairs(const float* grid, const int32_t n[3], std::vector<float>& out) {
+  const size_t n0 = n[0], n1 = n[1], n2 = n[2];
+  out.assign(8 * n0 * n1 * n2, 0.0f);
+  for (size_t i = 0; i < n0; ++i)
+    for (size_t j = 0; j < n1; ++j)
+      for (size_t k = 0; k < n2; ++k) {
+        const size_t e = (i * n1 + j) * n2 + k, e1 = (i * n1 + j) * n2 + (k + 1 < n2 ? k + 1 : k);
+        for (int c = 0; c < 3; ++c) { out[8 * e + c] = grid[3 * e + c]; out[8 * e + 4 + c] = grid[3 * e1 + c]; }
+      }
+}
+
 }  // namespace ckf

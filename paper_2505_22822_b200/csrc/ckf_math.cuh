@@ -57,7 +57,7 @@ struct FieldDev {
   double org[3];
   double inv[3];  // 1 / spacing
   double nm2[3];  // (double)(n - 2): largest cell index
-  const double* grid;  // [n0 * n1 * n2][4]
+  const float* grid;   // [n0 * n1 * n2][8] float32: node (i, j, k) then node (i, j, k + 1), each (Bx, By, Bz, pad)
 };
 
 struct CfgDev {
@@ -81,19 +81,26 @@ CKF_HD auto dot3(const A a[3], const B b[3]) -> decltype(a[0] * b[0]) {
 }
 
 struct D3 { double x, y, z; };
-CKF_HD D3 ld_node(const double* p) {
+// One grid entry = the nodes (i, j, k) and (i, j, k + 1) as 8 float32 in a 32-byte sector: ONE 256-bit load
+// (sm_100a: LDG.E.256) brings the two z-neighbours of a cell corner, so a cell is 4 loads.  The interpolation itself is
+// float64 on the widened values -- the grid arrives as float32 (ckf_field.grid), widening is exact, so the result is
+// the same as from a float64 copy of the grid.  History (profiles/r02_step_visit_update.md): the field read is the
+// busiest user of the L1 data pipe in ckf_step, and what that pipe counts is load instructions x scattered lanes
+// (wavefronts), not bytes: 16 loads of 128 + 64 bit per cell, then 8 of 256 bit (one node each), now 4.
+// The asm is NOT volatile (that costs ckf_step 4 %): to the compiler it is a pure function of p, which it may hoist
+// above the field-kind test of field_at -- it did in ckf_seed.  Hence every address field_at can form is readable: the
+// index clamps keep it inside the grid, and a uniform field owns a 2 x 2 x 2 grid of its value (ckf_create).
+CKF_HD void ld_pair(const float* p, D3& lo, D3& hi) {
 #if defined(__CUDA_ARCH__)
-  // one 256-bit load per node (sm_100a: LDG.E.256): the node is a 32-byte-aligned sector of 4 doubles.  Against a
-  // 128-bit + a 64-bit load this halves the load instructions and the L1 wavefronts of the field read, the busiest
-  // unit of ckf_step (l1tex data-pipe wavefronts 62 % of peak, profiles/r02_step_visit_update.md)
-  // NOT volatile (that costs ckf_step 4 %): to the compiler this is a pure function of p, which it may hoist above the
-  // field-kind test of field_at -- it did in ckf_seed.  Hence every address field_at can form is readable: the index
-  // clamps keep it inside the grid, and a uniform field owns a 2 x 2 x 2 grid of its value (ckf_create).
-  double x, y, z, w;
-  asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(x), "=d"(y), "=d"(z), "=d"(w) : "l"(p));
-  return D3{x, y, z};
+  unsigned long long a, b, c, d;
+  asm("ld.global.nc.v4.b64 {%0,%1,%2,%3}, [%4];" : "=l"(a), "=l"(b), "=l"(c), "=l"(d) : "l"(p));
+  lo.x = (double)__uint_as_float((unsigned)a); lo.y = (double)__uint_as_float((unsigned)(a >> 32));
+  lo.z = (double)__uint_as_float((unsigned)b);
+  hi.x = (double)__uint_as_float((unsigned)c); hi.y = (double)__uint_as_float((unsigned)(c >> 32));
+  hi.z = (double)__uint_as_float((unsigned)d);
 #else
-  return D3{p[0], p[1], p[2]};
+  lo = D3{(double)p[0], (double)p[1], (double)p[2]};
+  hi = D3{(double)p[4], (double)p[5], (double)p[6]};
 #endif
 }
 
@@ -128,11 +135,12 @@ CKF_HD void field_at(const FieldDev& f, const double r[3], double B[3]) {
     fr[a] = g - ti;
   }
   const long long s1 = f.n[2], s0 = (long long)f.n[1] * f.n[2];
-  const double* p = f.grid + 4 * (idx[0] * s0 + idx[1] * s1 + idx[2]);
-  const D3 v000 = ld_node(p), v001 = ld_node(p + 4);
-  const D3 v010 = ld_node(p + 4 * s1), v011 = ld_node(p + 4 * s1 + 4);
-  const D3 v100 = ld_node(p + 4 * s0), v101 = ld_node(p + 4 * s0 + 4);
-  const D3 v110 = ld_node(p + 4 * (s0 + s1)), v111 = ld_node(p + 4 * (s0 + s1) + 4);
+  const float* p = f.grid + 8 * (idx[0] * s0 + idx[1] * s1 + idx[2]);
+  D3 v000, v001, v010, v011, v100, v101, v110, v111;
+  ld_pair(p, v000, v001);
+  ld_pair(p + 8 * s1, v010, v011);
+  ld_pair(p + 8 * s0, v100, v101);
+  ld_pair(p + 8 * (s0 + s1), v110, v111);
 #define CKF_TRILERP(C)                                              \
   {                                                                 \
     const double x00 = v000.C + fr[0] * (v100.C - v000.C);          \
@@ -173,11 +181,12 @@ CKF_HD void field_gradient_at(const FieldDev& f, const double r[3], double G[3][
     fr[a] = g - ti;
   }
   const long long s1 = f.n[2], s0 = (long long)f.n[1] * f.n[2];
-  const double* p = f.grid + 4 * (idx[0] * s0 + idx[1] * s1 + idx[2]);
-  const D3 v000 = ld_node(p), v001 = ld_node(p + 4);
-  const D3 v010 = ld_node(p + 4 * s1), v011 = ld_node(p + 4 * s1 + 4);
-  const D3 v100 = ld_node(p + 4 * s0), v101 = ld_node(p + 4 * s0 + 4);
-  const D3 v110 = ld_node(p + 4 * (s0 + s1)), v111 = ld_node(p + 4 * (s0 + s1) + 4);
+  const float* p = f.grid + 8 * (idx[0] * s0 + idx[1] * s1 + idx[2]);
+  D3 v000, v001, v010, v011, v100, v101, v110, v111;
+  ld_pair(p, v000, v001);
+  ld_pair(p + 8 * s1, v010, v011);
+  ld_pair(p + 8 * s0, v100, v101);
+  ld_pair(p + 8 * (s0 + s1), v110, v111);
 #define CKF_TRIGRAD(C, ROW)                                                                         \
   {                                                                                                 \
     /* d/dx: differences along x, then lerp along y and z */                                        \

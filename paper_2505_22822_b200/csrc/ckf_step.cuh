@@ -69,8 +69,9 @@ __device__ __forceinline__ void pick_warp(const GeoDev& geo, const PickSmem& ps,
         if (id != (rx >> 1) - 1) {
           const double r[3] = {ps.rd[0 * 32 + t], ps.rd[1 * 32 + t], ps.rd[2 * 32 + t]};
           const double d[3] = {ps.rd[3 * 32 + t], ps.rd[4 * 32 + t], ps.rd[5 * 32 + t]};
-          double sv;
-          if (line_hits_module(geo.mod[id], r, d, (rx & 1) ? 1e-3 : -1e-3, sv, geo.bidir)) sres = sv;
+          // no early exits: the four groups of fields of the module record are loaded at once instead of one L2 round
+          // trip per passed test (that chain was a quarter of this kernel's stall samples)
+          sres = line_test_module(geo.mod[id], r, d, (rx & 1) ? 1e-3 : -1e-3, geo.bidir);
         }
       }
       ps.hit[nb * 32 + t] = sres;

@@ -15,7 +15,7 @@ namespace {
 struct Ctx {
   std::vector<ModuleRec> mods;
   std::vector<LayerRec> layers;
-  std::vector<double> grid;
+  std::vector<float> grid;
   GeoDev geo;
   FieldDev fld;
   CfgDev cfg;
@@ -73,10 +73,7 @@ void* hm_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c) 
     x->fld.nm2[a] = (double)(f->n[a] - 2);
   }
   if (f->kind == 1) {
-    const size_t np = (size_t)f->n[0] * f->n[1] * f->n[2];
-    x->grid.resize(4 * np);
-    for (size_t i = 0; i < np; ++i)
-      for (int k = 0; k < 3; ++k) x->grid[4 * i + k] = (double)f->grid[3 * i + k];
+    fill_field_pairs(f->grid, f->n, x->grid);
     x->fld.grid = x->grid.data();
   }
   x->cfg.chi2_max = c->chi2_max; x->cfg.rk_tol = c->rk_tolerance_mm; x->cfg.surf_tol = c->surface_tolerance_mm;
