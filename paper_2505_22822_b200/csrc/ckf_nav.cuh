@@ -612,30 +612,31 @@ CKF_HD void move_step(M& m, const FieldDev& fld, const CfgDev& cfg, int& n_trial
   rk_trial<T, GRAD>(fld, m.y, m.B1, KAPPA * m.y.qop, m.h, t);
   ++n_trials;
   if (!isfinite(t.eps)) { m.stop = STOP_NUMERIC; m.phase = PH_FIN; return; }
-  double f;
-  if (t.eps == 0.0) f = 4.0;
-  else {
-    f = 0.9 * sqrt(sqrt(cfg.rk_tol / t.eps));
+  // P3 factor 0.9 (tol / eps)^(1/4) clamped to [0.25, 4]; eps = 0 gives +inf, which the upper clamp turns into the
+  // rule's 4 (no branch).  It is evaluated inside each arm of the accept test, after the work that does not need it, so
+  // that its division and two square roots overlap that work instead of preceding the branch.
+  auto step_factor = [&]() {
+    double f = 0.9 * sqrt(sqrt(cfg.rk_tol / t.eps));
     f = f < 0.25 ? 0.25 : f;
-    f = f > 4.0 ? 4.0 : f;
-  }
+    return f > 4.0 ? 4.0 : f;
+  };
   if (t.eps <= cfg.rk_tol) {
     const double h = m.h;
     StepGrad<T> sg;
     if constexpr (GRAD) step_gradients<T>(fld, m.y, h, t, sg);   // at the stage points of the step, from the state before it
     rk_accept_state<T>(m.y, h, t, m.ib);
-    m.h_ctrl = fabs(h) * f;
     ++n_accepted;
     m.targeted = false;
     double s = 0.0;
     const int st = target_distance(m, s);
+    m.h_ctrl = fabs(h) * step_factor();
     const bool more = st == STOP_NONE && fabs(s) > cfg.surf_tol;
     if (more) set_trial(m, fld, cfg, s);            // the loads of the next trial's stage 1 start here ...
     if constexpr (GRAD) rk_accept_jac_g<T>(m.y.qop, m.D, m.Dr, h, t, sg, m.dib);
     else rk_accept_jac<T>(m.y, m.D, h, t, m.dib);   // ... and fly while D <- D_step D is computed
     if (!more) land_or_stop(m, st, s);              // the closing drift acts on the updated D
   } else {
-    m.h = m.h * f;                                  // retry from the same position: same B1
+    m.h = m.h * step_factor();                      // retry from the same position: same B1
   }
 }
 
