@@ -239,9 +239,9 @@ bool others_in_flight(ckf_handle* h, const Workspace* self, cudaStream_t st) {
   for (auto& o : h->ws) {
     if (&o == self) continue;
     if (o.enqueuing.load()) return true;
-    if (o.done_valid.load() && o.done_stream.load() != (void*)st && cudaEventQuery(o.done) == cudaErrorNotReady) {
-      (void)cudaGetLastError();  // 'not ready' is an answer, not an error of this call
-      return true;
+    if (o.done_valid.load() && o.done_stream.load() != (void*)st && cudaEventQuery(o.done) != cudaSuccess) {
+      (void)cudaGetLastError();  // 'not ready' is an answer, not an error of this call; any other answer (an event of a
+      return true;               // capturing stream, say) is taken the careful way: plain launches
     }
   }
   return false;
