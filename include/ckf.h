@@ -291,6 +291,31 @@ typedef struct {
 int ckf_resolve(ckf_handle* handle, const ckf_tracks* tracks, int32_t n_measurements, ckf_resolution* out,
                 void* cuda_stream);
 
+/* ---- ckf_resolve for callers that may not allocate --------------------------------------------------------------------
+ * The same resolution (same kernel, same rules AR1-AR3, same results) WITHOUT a handle and without any allocation: no
+ * cudaMalloc / cudaFree / allocating library routine is called, at set-up or later, so it may be used under CUDA graph
+ * capture, in serving loops and in harnesses that forbid allocation.  Its scratch (rank keys, per-measurement minima,
+ * owners, states) lives in a static __device__ array of the library, CKF_RESOLVE_STATIC_SCRATCH_BYTES (3.25 MiB) on
+ * every GPU that loads the library, held until the process exits.  Hence the limits: at most
+ * CKF_RESOLVE_STATIC_MAX_TRACKS candidates and CKF_RESOLVE_STATIC_MAX_MEASUREMENTS measurements; larger sizes are
+ * rejected with CKF_E_CAPACITY and a message (use ckf_resolve).
+ *   tracks          DEVICE arrays as filled by ckf_find; n_tracks, track_offsets, meas_idx, chi2_sum are read
+ *   max_tracks      capacity of the caller's arrays (out->accepted, out->n_shared, tracks->chi2_sum): candidates beyond
+ *                   it are ignored, as in ckf_resolve; 1 .. CKF_RESOLVE_STATIC_MAX_TRACKS
+ *   n_measurements  ckf_measurements.n of the find; 0 .. CKF_RESOLVE_STATIC_MAX_MEASUREMENTS
+ *   precision       32 or 64: element type of tracks->chi2_sum
+ *   out             as for ckf_resolve (DEVICE arrays, caller-owned; limits are inputs)
+ * Asynchronous on `cuda_stream`, which must belong to the CURRENT device (the array's address is looked up once per
+ * device, on first use with that device current).  Every call shares the one array: the kernel re-initialises what it
+ * reads, so calls in stream order need no clearing by the caller, but two calls that OVERLAP on the GPU (different
+ * streams, no ordering between them) race and give garbage -- order them.  Errors: CKF_E_ARG, CKF_E_CAPACITY, CKF_E_CUDA;
+ * text from ckf_last_error(NULL). */
+#define CKF_RESOLVE_STATIC_MAX_TRACKS 65536
+#define CKF_RESOLVE_STATIC_MAX_MEASUREMENTS 131072
+#define CKF_RESOLVE_STATIC_SCRATCH_BYTES (CKF_RESOLVE_STATIC_MAX_TRACKS * 12 + CKF_RESOLVE_STATIC_MAX_MEASUREMENTS * 20 + 256)
+int ckf_resolve_static(const ckf_tracks* tracks, int32_t max_tracks, int32_t n_measurements, int32_t precision,
+                       ckf_resolution* out, void* cuda_stream);
+
 /* ---- Triplet seeding + track-parameter estimation, the stage in front of the CKF ---
  * "The spacepoints are used in the seeding algorithm where triplets, a set of three spacepoints which can approximately
  * form a helix, are found.  In the track parameter estimation algorithm, the position and momentum of tracks, called a

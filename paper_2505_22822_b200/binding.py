@@ -21,7 +21,7 @@ HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(HERE, "libckf.so")
 
 EXPORTS = ("ckf_create", "ckf_find", "ckf_find_host", "ckf_fit", "ckf_get_counters", "ckf_get_launch_info", "ckf_destroy",
-           "ckf_set_timing", "ckf_get_timing", "ckf_measure_alu_peak", "ckf_resolve", "ckf_seed",
+           "ckf_set_timing", "ckf_get_timing", "ckf_measure_alu_peak", "ckf_resolve", "ckf_resolve_static", "ckf_seed",
            "ckf_last_error", "ckf_abi_version")
 
 
@@ -117,6 +117,8 @@ def load_library():
                               C.POINTER(ckf_fits), _vp]
         L.ckf_resolve.restype = C.c_int
         L.ckf_resolve.argtypes = [_vp, C.POINTER(ckf_tracks), C.c_int32, C.POINTER(ckf_resolution), _vp]
+        L.ckf_resolve_static.restype = C.c_int
+        L.ckf_resolve_static.argtypes = [C.POINTER(ckf_tracks), C.c_int32, C.c_int32, C.c_int32, C.POINTER(ckf_resolution), _vp]
         L.ckf_seed.restype = C.c_int
         L.ckf_seed.argtypes = [_vp, C.POINTER(ckf_measurements), C.POINTER(ckf_seeding), C.POINTER(ckf_seed_out), _vp]
         L.ckf_set_timing.restype = C.c_int
@@ -207,6 +209,29 @@ def measure_alu_peak(mix: int, seconds: float = 1.0) -> dict:
     if rc != 0:
         raise RuntimeError("ckf_measure_alu_peak failed (%d): %s" % (rc, load_library().ckf_last_error(None).decode()))
     return dict(tflops_f32=v[0].value, tflops_f64=v[1].value, best_f32=v[2].value, best_f64=v[3].value)
+
+
+RESOLVE_STATIC_MAX_TRACKS = 65536           # CKF_RESOLVE_STATIC_MAX_TRACKS
+RESOLVE_STATIC_MAX_MEASUREMENTS = 131072    # CKF_RESOLVE_STATIC_MAX_MEASUREMENTS
+
+
+def resolve_static(tracks: dict, n_measurements: int, res: dict, precision: int, max_shared_hits: int = 1,
+                   max_shared_fraction: float = 1.0, stream=None):
+    """ckf_resolve_static: ambiguity resolution of the candidates in `tracks` (device tensors filled by CKF.find) with no
+    handle and no allocation inside the library; scratch in a static device array, so sizes are limited (see ckf.h).
+    `res` as from CKF.alloc_resolution; its length is the capacity passed as max_tracks."""
+    import torch
+    st = stream if stream is not None else torch.cuda.current_stream()
+    lib = load_library()
+    o = ckf_tracks(*[tracks[k].data_ptr() for k in ("n_tracks", "status", "track_offsets", "meas_idx", "seed_id",
+                                                    "n_holes", "last_module", "stop_reason", "params", "cov",
+                                                    "chi2_sum", "entry_chi2")])
+    r = ckf_resolution(res["accepted"].data_ptr(), res["n_shared"].data_ptr(), res["summary"].data_ptr(),
+                       int(max_shared_hits), float(max_shared_fraction))
+    cap = min(int(res["accepted"].shape[0]), int(tracks["chi2_sum"].shape[0]))
+    rc = lib.ckf_resolve_static(C.byref(o), cap, int(n_measurements), int(precision), C.byref(r), _vp(st.cuda_stream))
+    if rc != 0:
+        raise RuntimeError("ckf_resolve_static failed (%d): %s" % (rc, lib.ckf_last_error(None).decode()))
 
 
 @dataclass

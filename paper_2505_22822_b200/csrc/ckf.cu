@@ -30,6 +30,11 @@
 
 using namespace ckf;
 
+// Scratch of ckf_resolve_static (include/ckf.h): rank keys [MAX_TRACKS] u64 | minima [2][MAX_MEASUREMENTS] u64 |
+// owners [MAX_MEASUREMENTS] i32 | states [MAX_TRACKS] i32 | 4 counters.  On the host this NAME is a stand-in, not a
+// device address: the entry point takes the address with cudaGetSymbolAddress, once per device.
+static __device__ __align__(256) unsigned char g_resolve_static_scratch[CKF_RESOLVE_STATIC_SCRATCH_BYTES];
+
 namespace {
 
 // Error text is per calling THREAD (several host threads may drive one handle, configs[4]): a failing call stores its
@@ -839,6 +844,73 @@ int ckf_resolve(ckf_handle* h, const ckf_tracks* t, int32_t n_measurements, ckf_
   }
   cudaEventRecord(h->resolve_done, st);
   if (e != cudaSuccess) return fail(h, CKF_E_CUDA, "ckf_resolve launch failed: %s", cudaGetErrorString(e));
+  return CKF_OK;
+}
+
+// ckf_resolve without a handle and without allocation: scratch in g_resolve_static_scratch (see include/ckf.h).
+int ckf_resolve_static(const ckf_tracks* t, int32_t max_tracks, int32_t n_measurements, int32_t precision,
+                       ckf_resolution* o, void* stream) {
+  ckf_handle* h = nullptr;  // for fail() / CK(): the message goes to the calling thread's slot
+  if (!t || !o) return fail(h, CKF_E_ARG, "ckf_resolve_static: null argument");
+  if (!t->n_tracks || !t->track_offsets || !t->meas_idx || !t->chi2_sum) return fail(h, CKF_E_ARG, "ckf_resolve_static: null input array");
+  if (!o->accepted || !o->n_shared || !o->summary) return fail(h, CKF_E_ARG, "ckf_resolve_static: null output array");
+  if (precision != 32 && precision != 64) return fail(h, CKF_E_ARG, "ckf_resolve_static: precision must be 32 or 64");
+  if (o->max_shared_hits < 0 || !(o->max_shared_fraction >= 0.0)) return fail(h, CKF_E_ARG, "ckf_resolve_static: bad sharing limits");
+  if (max_tracks < 1 || max_tracks > CKF_RESOLVE_STATIC_MAX_TRACKS)
+    return fail(h, CKF_E_CAPACITY, "ckf_resolve_static: max_tracks %d outside 1..%d (the static scratch array is sized for that; use ckf_resolve)",
+                max_tracks, CKF_RESOLVE_STATIC_MAX_TRACKS);
+  if (n_measurements < 0 || n_measurements > CKF_RESOLVE_STATIC_MAX_MEASUREMENTS)
+    return fail(h, CKF_E_CAPACITY, "ckf_resolve_static: n_measurements %d outside 0..%d (the static scratch array is sized for that; use ckf_resolve)",
+                n_measurements, CKF_RESOLVE_STATIC_MAX_MEASUREMENTS);
+  // set-up, once per device, with that device current: address of the array, and the grid a cooperative launch may have
+  struct PerDevice { unsigned char* base = nullptr; int grid32 = 0, grid64 = 0; bool ready = false; };
+  static PerDevice s_dev[64];
+  static std::mutex s_mu;
+  int dev = -1;
+  CK(cudaGetDevice(&dev));
+  if (dev < 0 || dev >= 64) return fail(h, CKF_E_ARG, "ckf_resolve_static: device ordinal %d not supported", dev);
+  PerDevice pd;
+  {
+    std::lock_guard<std::mutex> lk(s_mu);
+    if (!s_dev[dev].ready) {
+      void* ptr = nullptr;
+      CK(cudaGetSymbolAddress(&ptr, g_resolve_static_scratch));
+      int sms = 0, b32 = 0, b64 = 0;
+      CK(cudaDeviceGetAttribute(&sms, cudaDevAttrMultiProcessorCount, dev));
+      CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b32, ckf_resolve_kernel<float>, RESOLVE_NT, 0));
+      CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&b64, ckf_resolve_kernel<double>, RESOLVE_NT, 0));
+      s_dev[dev].base = (unsigned char*)ptr;
+      s_dev[dev].grid32 = std::max(1, b32) * sms;   // a cooperative launch needs every block resident
+      s_dev[dev].grid64 = std::max(1, b64) * sms;
+      s_dev[dev].ready = true;
+    }
+    pd = s_dev[dev];
+  }
+  constexpr size_t MT = CKF_RESOLVE_STATIC_MAX_TRACKS, MM = CKF_RESOLVE_STATIC_MAX_MEASUREMENTS;
+  unsigned long long* key = (unsigned long long*)pd.base;                       // [MT]
+  unsigned long long* best = (unsigned long long*)(pd.base + MT * 8);           // [2][n_measurements], room for [2][MM]
+  int32_t* owner = (int32_t*)(pd.base + MT * 8 + MM * 16);                      // [MM]
+  int32_t* state = (int32_t*)(pd.base + MT * 8 + MM * 20);                      // [MT]
+  int32_t* g = (int32_t*)(pd.base + MT * 12 + MM * 20);                         // [4]
+  static_assert(MT * 12 + MM * 20 + 16 <= CKF_RESOLVE_STATIC_SCRATCH_BYTES, "scratch layout");
+  // the kernel initialises keys, minima, owners, states and counters for the sizes of THIS call before it reads them
+  // (the array keeps the previous call's contents)
+  cudaStream_t st = (cudaStream_t)stream;
+  cudaError_t e;
+  if (precision == 32) {
+    ResolveParams<float> p{t->n_tracks, t->track_offsets, t->meas_idx, (const float*)t->chi2_sum, max_tracks, n_measurements,
+                           o->max_shared_hits, o->max_shared_fraction, key, best, owner, state, g, o->accepted, o->n_shared,
+                           o->summary};
+    void* args[] = {&p};
+    e = cudaLaunchCooperativeKernel((void*)ckf_resolve_kernel<float>, dim3(pd.grid32), dim3(RESOLVE_NT), args, 0, st);
+  } else {
+    ResolveParams<double> p{t->n_tracks, t->track_offsets, t->meas_idx, (const double*)t->chi2_sum, max_tracks, n_measurements,
+                            o->max_shared_hits, o->max_shared_fraction, key, best, owner, state, g, o->accepted, o->n_shared,
+                            o->summary};
+    void* args[] = {&p};
+    e = cudaLaunchCooperativeKernel((void*)ckf_resolve_kernel<double>, dim3(pd.grid64), dim3(RESOLVE_NT), args, 0, st);
+  }
+  if (e != cudaSuccess) return fail(h, CKF_E_CUDA, "ckf_resolve_static launch failed: %s", cudaGetErrorString(e));
   return CKF_OK;
 }
 
