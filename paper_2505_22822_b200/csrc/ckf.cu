@@ -80,6 +80,10 @@ struct Workspace {
   bool used = false;
   float last_ms[10] = {0};  // per-kernel-kind times of the last timed ckf_find (ckf_set_timing)
   int last_launches = 0;
+  // CUDA graph of the last repeated find on this workspace (launch_find): its key = the kernel parameters + launch policy
+  cudaGraphExec_t graph_exec = nullptr;
+  cudaStream_t cap_stream = nullptr;
+  std::vector<unsigned char> graph_key, last_key;
 };
 
 }  // namespace
@@ -123,6 +127,7 @@ struct ckf_handle {
   // 32 emission, 64 ckf_fit_level.  Measured (profiles/r02_launch_overlap.md): step + visit + update is best; with ckf_scan in the chain as
   // well the whole level loop is one cascade of waiting blocks and a batched find gets 10 % slower.  CKF_CHAIN_OVERLAP=<mask>
   // overrides (0 = plain launches), for A/B measurements.
+  bool use_graph = true;  // CKF_GRAPH=0: never replay a repeated find from a CUDA graph
   bool grad = false;  // J2': config.field_gradient on an interpolated field (a uniform field has no gradient: the default kernels)
   int chain_overlap = 2 | 4 | 16 | 64;
   bool timing = false;  // ckf_set_timing / CKF_TIMING=1: per-kernel CUDA-event times of every ckf_find on stderr (debug aid; synchronises)
@@ -256,6 +261,7 @@ template <typename T>
 int launch_find(ckf_handle* h, Workspace& w, const ckf_measurements* m, const ckf_seeds* s, ckf_tracks* o,
                 cudaStream_t st, int32_t* summary = nullptr) {
   KParams<T> p;
+  std::memset(&p, 0, sizeof(p));   // padding too: the bytes of p are the key of the graph cache below
   fill_params<T>(h, w, p);
   p.o_summary = summary;
   p.n_meas = m->n; p.n_seeds = s->n;
@@ -285,25 +291,63 @@ int launch_find(ckf_handle* h, Workspace& w, const ckf_measurements* m, const ck
   // waiting for their predecessor take room from the other streams' kernels (2 batches in flight: 20.4 -> 19.2 M
   // seeds/s), so the launches stay plain.  Timing mode puts an event between the kernels, which serialises them anyway.
   const int ovm = (h->timing || others_in_flight(h, &w, st)) ? 0 : h->chain_overlap;
-  ckf_init_event<T><<<nb, 256, 0, st>>>(p); mark(0);  // plain launch: whatever precedes the find in the stream is not ours
-  launch_chain(ckf_sort_slices<T>, h->sm_count * (1024 / SORT_NT), SORT_NT, 0, st, ovm & 1, p); mark(1);
-  // level loop: tips of level l were made by level l - 1; a tip at max_levels only stops (LEVEL_LIMIT) and emits.
-  // Kernels of an empty level return at once, so the loop needs no host read of the level's size.
-  const int wide = h->sm_count * 4;
-  for (int level = 0; level <= h->cfg.max_levels; ++level) {
-    if (h->grad) {
-      if (level > 0) { launch_chain(ckf_step<T, StepBlocks<T, true>::value, true>, h->step_grid, STEP_NT, 0, st, ovm & 2, p, level); mark(2); }
-      launch_chain(ckf_visit<T, VisitBlocks<T>::value, true>, h->visit_grid, VISIT_NT, h->visit_smem, st, ovm & 4, p, level); mark(3);
-    } else {
-      if (level > 0) { launch_chain(ckf_step<T, MinBlocks<T>::value>, h->step_grid, STEP_NT, 0, st, ovm & 2, p, level); mark(2); }
-      launch_chain(ckf_visit<T, VisitBlocks<T>::value>, h->visit_grid, VISIT_NT, h->visit_smem, st, ovm & 4, p, level); mark(3);
+  auto enqueue = [&](cudaStream_t q) {
+    ckf_init_event<T><<<nb, 256, 0, q>>>(p); mark(0);  // plain launch: whatever precedes the find in the stream is not ours
+    launch_chain(ckf_sort_slices<T>, h->sm_count * (1024 / SORT_NT), SORT_NT, 0, q, ovm & 1, p); mark(1);
+    // level loop: tips of level l were made by level l - 1; a tip at max_levels only stops (LEVEL_LIMIT) and emits.
+    // Kernels of an empty level return at once, so the loop needs no host read of the level's size.
+    const int wide = h->sm_count * 4;
+    for (int level = 0; level <= h->cfg.max_levels; ++level) {
+      if (h->grad) {
+        if (level > 0) { launch_chain(ckf_step<T, StepBlocks<T, true>::value, true>, h->step_grid, STEP_NT, 0, q, ovm & 2, p, level); mark(2); }
+        launch_chain(ckf_visit<T, VisitBlocks<T>::value, true>, h->visit_grid, VISIT_NT, h->visit_smem, q, ovm & 4, p, level); mark(3);
+      } else {
+        if (level > 0) { launch_chain(ckf_step<T, MinBlocks<T>::value>, h->step_grid, STEP_NT, 0, q, ovm & 2, p, level); mark(2); }
+        launch_chain(ckf_visit<T, VisitBlocks<T>::value>, h->visit_grid, VISIT_NT, h->visit_smem, q, ovm & 4, p, level); mark(3);
+      }
+      launch_chain(ckf_scan<T>, wide, SCAN_NT, 0, q, ovm & 8, p, level); mark(5);
+      launch_chain(ckf_update<T>, wide, SCAN_NT, 0, q, ovm & 16, p, level); mark(6);
     }
-    launch_chain(ckf_scan<T>, wide, SCAN_NT, 0, st, ovm & 8, p, level); mark(5);
-    launch_chain(ckf_update<T>, wide, SCAN_NT, 0, st, ovm & 16, p, level); mark(6);
+    launch_chain(ckf_scan_seeds<T>, (s->n + SEED_TILE - 1) / SEED_TILE + 1, SEED_TILE, 0, q, ovm & 32, p); mark(7);
+    launch_chain(ckf_emit_tracks<T>, h->sm_count * 8, EMIT_NT, 0, q, ovm & 32, p); mark(8);
+    launch_chain(ckf_finalize<T>, 1, 1, 0, q, ovm & 32, p); mark(9);
+  };
+  // A find whose arguments repeat (same arrays, same sizes, same launch policy: the usual case of a pipeline that runs on
+  // preallocated buffers) is replayed from a CUDA graph of its ~136 launches: the second call in a row with the same
+  // arguments captures it, later ones launch it (configs[3] 3.29 -> 3.20 ms, configs[0] 0.92 -> 0.81 ms).  Anything else
+  // -- new arguments, timing mode, a caller who is capturing the stream himself -- is enqueued launch by launch as before.
+  bool done = false;
+  if (!h->timing && h->use_graph) {
+    std::vector<unsigned char> key(sizeof(p) + sizeof(int));
+    std::memcpy(key.data(), &p, sizeof(p));
+    std::memcpy(key.data() + sizeof(p), &ovm, sizeof(int));
+    cudaStreamCaptureStatus cs = cudaStreamCaptureStatusNone;
+    if (cudaStreamIsCapturing(st, &cs) != cudaSuccess) { (void)cudaGetLastError(); cs = cudaStreamCaptureStatusActive; }
+    if (cs == cudaStreamCaptureStatusNone) {
+      if (w.graph_exec && w.graph_key == key) {
+        done = cudaGraphLaunch(w.graph_exec, st) == cudaSuccess;
+      } else if (w.last_key == key) {
+        cudaGraph_t g = nullptr;
+        cudaGraphExec_t ge = nullptr;
+        // captured on a stream of the workspace's own (the caller's may be the legacy default stream, which cannot
+        // capture); the graph does not remember it
+        if (!w.cap_stream) cudaStreamCreateWithFlags(&w.cap_stream, cudaStreamNonBlocking);
+        if (w.cap_stream && cudaStreamBeginCapture(w.cap_stream, cudaStreamCaptureModeThreadLocal) == cudaSuccess) {
+          enqueue(w.cap_stream);
+          if (cudaStreamEndCapture(w.cap_stream, &g) == cudaSuccess && g && cudaGraphInstantiate(&ge, g, 0) == cudaSuccess) {
+            if (w.graph_exec) cudaGraphExecDestroy(w.graph_exec);
+            w.graph_exec = ge;
+            w.graph_key = key;
+            done = cudaGraphLaunch(w.graph_exec, st) == cudaSuccess;
+          }
+          if (g) cudaGraphDestroy(g);
+        }
+        if (!done) (void)cudaGetLastError();   // no graph then: the plain path below
+      }
+    }
+    if (!done) w.last_key.swap(key);
   }
-  launch_chain(ckf_scan_seeds<T>, (s->n + SEED_TILE - 1) / SEED_TILE + 1, SEED_TILE, 0, st, ovm & 32, p); mark(7);
-  launch_chain(ckf_emit_tracks<T>, h->sm_count * 8, EMIT_NT, 0, st, ovm & 32, p); mark(8);
-  launch_chain(ckf_finalize<T>, 1, 1, 0, st, ovm & 32, p); mark(9);
+  if (!done) enqueue(st);
   w.last_launches = 5 + 4 * (h->cfg.max_levels + 1) - 1;
   if (h->timing) {
     static const char* names[10] = {"init", "sort", "step", "visit", "cap", "scan", "update", "scan_seeds", "emit", "finalize"};
@@ -519,6 +563,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
   }
   h->sm_count = prop.multiProcessorCount;
   { const char* t = getenv("CKF_TIMING"); h->timing = h->timing_print = t && t[0] == '1'; }
+  { const char* t = getenv("CKF_GRAPH"); if (t && t[0] == '0') h->use_graph = false; }
   { const char* t = getenv("CKF_CHAIN_OVERLAP"); if (t && t[0]) h->chain_overlap = atoi(t); }
   h->n_modules = g->n_modules;
   h->n_layers = g->n_layers;
@@ -1022,6 +1067,8 @@ int ckf_destroy(ckf_handle* h) {
   if (!h) return CKF_E_ARG;
   cudaDeviceSynchronize();
   for (auto& w : h->ws) {
+    if (w.graph_exec) cudaGraphExecDestroy(w.graph_exec);
+    if (w.cap_stream) cudaStreamDestroy(w.cap_stream);
     if (w.done) cudaEventDestroy(w.done);
     if (w.pinned_nt) cudaFreeHost(w.pinned_nt);
   }

@@ -1068,3 +1068,53 @@ def test_field_gradient_parity(precision):
         tol = 1e-9 if precision == 64 else 1e-5
         assert rf["n_not_pd_gpu_only"] == 0 and rf["max_smoothed_rel"] < tol and rf["max_last_rel"] < tol, (smoother, rf)
     ckf.close()
+
+
+def test_graph_replay_of_a_repeated_find_same_result(monkeypatch):
+    """A find whose arguments repeat is replayed from a CUDA graph from the third call on (ckf.cu, launch_find).  Replays,
+    the capture call and plain calls give byte-identical outputs; new arguments fall back to plain launches and a later
+    return to the old arguments (captured again) is still right."""
+    import torch
+    from paper_2505_22822_b200 import CKF
+    det, fld, cfg = synth.config_bundle(2)
+    evs = [synth.make_event(2, event_index=i, det=det, n_particles=2500) for i in range(2)]
+    ms, mm = max(e.n_seeds for e in evs), max(e.n_measurements for e in evs)
+
+    def snapshot(out):
+        n = int(out["n_tracks"][0])
+        ne = int(out["track_offsets"][n])
+        d = {k: out[k][:n].cpu().numpy().tobytes() for k in ("seed_id", "n_holes", "last_module", "stop_reason", "params", "cov", "chi2_sum")}
+        d["offsets"] = out["track_offsets"][:n + 1].cpu().numpy().tobytes()
+        d["meas"] = out["meas_idx"][:ne].cpu().numpy().tobytes()
+        d["entry_chi2"] = out["entry_chi2"][:ne].cpu().numpy().tobytes()
+        return d
+
+    monkeypatch.setenv("CKF_GRAPH", "0")
+    plain = CKF(det, fld, cfg.ckf, cfg.precision, max_seeds=ms, max_measurements=mm, max_fit_tracks=0)
+    want = []
+    for ev in evs:
+        dev, out = plain.upload_event(ev), plain.alloc_tracks()
+        plain.find(dev, out)
+        torch.cuda.synchronize()
+        want.append(snapshot(out))
+    plain.close()
+    monkeypatch.delenv("CKF_GRAPH")
+    ckf = CKF(det, fld, cfg.ckf, cfg.precision, max_seeds=ms, max_measurements=mm, max_fit_tracks=0)
+    devs = [ckf.upload_event(ev) for ev in evs]
+    out = ckf.alloc_tracks()
+    s2 = torch.cuda.Stream()
+    for which, reps, stream in ((0, 4, None), (1, 3, None), (0, 3, None), (1, 1, None), (0, 4, s2)):
+        for r in range(reps):
+            for v in out.values():
+                v.zero_()
+            if stream is None:
+                ckf.find(devs[which], out)
+            else:
+                stream.wait_stream(torch.cuda.current_stream())
+                with torch.cuda.stream(stream):
+                    ckf.find(devs[which], out, stream)
+            torch.cuda.synchronize()
+            got = snapshot(out)
+            for k in want[which]:
+                assert got[k] == want[which][k], (which, r, k)
+    ckf.close()
