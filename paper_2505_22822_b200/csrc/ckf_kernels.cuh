@@ -149,50 +149,75 @@ __device__ __forceinline__ void slice_of(const KParams<T>& p, int m, int& beg, i
 //   mv_y[t * 8 ..)    r[3], d[3], t, q/p   float64 (one 64-byte record)
 //   mv_D[t * MVD ..)  Rd[9], Dd[9], rq[3], dq[3], tq, padding   T (one 128- / 256-byte record)
 constexpr int MVD = 32;
+// 256-bit accesses (sm_100a: LDG.E.256 / STG.E.256): a record is read or written by ONE lane, the lanes of a warp touch
+// unrelated records, and what the L1 data pipe then counts is instructions x lanes -- half as many with 32-byte pieces.
+__device__ __forceinline__ void ld256(const void* p, double& a, double& b, double& c, double& d) {
+  asm volatile("ld.global.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(a), "=d"(b), "=d"(c), "=d"(d) : "l"(p) : "memory");
+}
+__device__ __forceinline__ void st256(void* p, double a, double b, double c, double d) {
+  asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(p), "d"(a), "d"(b), "d"(c), "d"(d) : "memory");
+}
+__device__ __forceinline__ double pack2(float lo, float hi) {
+  return __longlong_as_double(((long long)__float_as_uint(hi) << 32) | (long long)__float_as_uint(lo));
+}
+__device__ __forceinline__ void unpack2(double v, float& lo, float& hi) {
+  const long long b = __double_as_longlong(v);
+  lo = __uint_as_float((unsigned)b);
+  hi = __uint_as_float((unsigned)(b >> 32));
+}
 __device__ __forceinline__ void store_traj(double* mv_y, size_t t, const Traj& y) {
-  double2* q = reinterpret_cast<double2*>(mv_y + t * 8);
-  q[0] = make_double2(y.r[0], y.r[1]); q[1] = make_double2(y.r[2], y.d[0]);
-  q[2] = make_double2(y.d[1], y.d[2]); q[3] = make_double2(y.t, y.qop);
+  double* q = mv_y + t * 8;
+  st256(q, y.r[0], y.r[1], y.r[2], y.d[0]);
+  st256(q + 4, y.d[1], y.d[2], y.t, y.qop);
 }
 __device__ __forceinline__ void load_traj(const double* mv_y, size_t t, Traj& y) {
-  const double2* q = reinterpret_cast<const double2*>(mv_y + t * 8);
-  const double2 a = q[0], b = q[1], c = q[2], d = q[3];
-  y.r[0] = a.x; y.r[1] = a.y; y.r[2] = b.x; y.d[0] = b.y; y.d[1] = c.x; y.d[2] = c.y; y.t = d.x; y.qop = d.y;
+  const double* q = mv_y + t * 8;
+  ld256(q, y.r[0], y.r[1], y.r[2], y.d[0]);
+  ld256(q + 4, y.d[1], y.d[2], y.t, y.qop);
 }
 __device__ __forceinline__ void store_jac(float* mv_D, size_t t, const Jac<float>& D) {
-  float4* q = reinterpret_cast<float4*>(mv_D + t * MVD);
-  q[0] = make_float4(D.Rd[0][0], D.Rd[0][1], D.Rd[0][2], D.Rd[1][0]);
-  q[1] = make_float4(D.Rd[1][1], D.Rd[1][2], D.Rd[2][0], D.Rd[2][1]);
-  q[2] = make_float4(D.Rd[2][2], D.Dd[0][0], D.Dd[0][1], D.Dd[0][2]);
-  q[3] = make_float4(D.Dd[1][0], D.Dd[1][1], D.Dd[1][2], D.Dd[2][0]);
-  q[4] = make_float4(D.Dd[2][1], D.Dd[2][2], D.rq[0], D.rq[1]);
-  q[5] = make_float4(D.rq[2], D.dq[0], D.dq[1], D.dq[2]);
-  q[6] = make_float4(D.tq, 0.f, 0.f, 0.f);
+  float* q = mv_D + t * MVD;
+  const float v[32] = {D.Rd[0][0], D.Rd[0][1], D.Rd[0][2], D.Rd[1][0], D.Rd[1][1], D.Rd[1][2], D.Rd[2][0], D.Rd[2][1],
+                       D.Rd[2][2], D.Dd[0][0], D.Dd[0][1], D.Dd[0][2], D.Dd[1][0], D.Dd[1][1], D.Dd[1][2], D.Dd[2][0],
+                       D.Dd[2][1], D.Dd[2][2], D.rq[0], D.rq[1], D.rq[2], D.dq[0], D.dq[1], D.dq[2], D.tq, 0.f, 0.f, 0.f,
+                       0.f, 0.f, 0.f, 0.f};
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+    st256(q + 8 * i, pack2(v[8 * i], v[8 * i + 1]), pack2(v[8 * i + 2], v[8 * i + 3]), pack2(v[8 * i + 4], v[8 * i + 5]),
+          pack2(v[8 * i + 6], v[8 * i + 7]));
 }
 __device__ __forceinline__ void load_jac(const float* mv_D, size_t t, Jac<float>& D) {
-  const float4* q = reinterpret_cast<const float4*>(mv_D + t * MVD);
-  const float4 a = q[0], b = q[1], c = q[2], d = q[3], e = q[4], f = q[5], g = q[6];
-  D.Rd[0][0] = a.x; D.Rd[0][1] = a.y; D.Rd[0][2] = a.z; D.Rd[1][0] = a.w;
-  D.Rd[1][1] = b.x; D.Rd[1][2] = b.y; D.Rd[2][0] = b.z; D.Rd[2][1] = b.w;
-  D.Rd[2][2] = c.x; D.Dd[0][0] = c.y; D.Dd[0][1] = c.z; D.Dd[0][2] = c.w;
-  D.Dd[1][0] = d.x; D.Dd[1][1] = d.y; D.Dd[1][2] = d.z; D.Dd[2][0] = d.w;
-  D.Dd[2][1] = e.x; D.Dd[2][2] = e.y; D.rq[0] = e.z; D.rq[1] = e.w;
-  D.rq[2] = f.x; D.dq[0] = f.y; D.dq[1] = f.z; D.dq[2] = f.w;
-  D.tq = g.x;
+  const float* q = mv_D + t * MVD;
+  float v[32];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    double a, b, c, d;
+    ld256(q + 8 * i, a, b, c, d);
+    unpack2(a, v[8 * i], v[8 * i + 1]); unpack2(b, v[8 * i + 2], v[8 * i + 3]);
+    unpack2(c, v[8 * i + 4], v[8 * i + 5]); unpack2(d, v[8 * i + 6], v[8 * i + 7]);
+  }
+#pragma unroll
+  for (int i = 0; i < 3; ++i) {
+#pragma unroll
+    for (int j = 0; j < 3; ++j) { D.Rd[i][j] = v[i * 3 + j]; D.Dd[i][j] = v[9 + i * 3 + j]; }
+    D.rq[i] = v[18 + i];
+    D.dq[i] = v[21 + i];
+  }
+  D.tq = v[24];
 }
 __device__ __forceinline__ void store_jac(double* mv_D, size_t t, const Jac<double>& D) {
-  double2* q = reinterpret_cast<double2*>(mv_D + t * MVD);
-  const double v[26] = {D.Rd[0][0], D.Rd[0][1], D.Rd[0][2], D.Rd[1][0], D.Rd[1][1], D.Rd[1][2], D.Rd[2][0], D.Rd[2][1],
+  double* q = mv_D + t * MVD;
+  const double v[28] = {D.Rd[0][0], D.Rd[0][1], D.Rd[0][2], D.Rd[1][0], D.Rd[1][1], D.Rd[1][2], D.Rd[2][0], D.Rd[2][1],
                         D.Rd[2][2], D.Dd[0][0], D.Dd[0][1], D.Dd[0][2], D.Dd[1][0], D.Dd[1][1], D.Dd[1][2], D.Dd[2][0],
-                        D.Dd[2][1], D.Dd[2][2], D.rq[0], D.rq[1], D.rq[2], D.dq[0], D.dq[1], D.dq[2], D.tq, 0.0};
+                        D.Dd[2][1], D.Dd[2][2], D.rq[0], D.rq[1], D.rq[2], D.dq[0], D.dq[1], D.dq[2], D.tq, 0.0, 0.0, 0.0};
 #pragma unroll
-  for (int i = 0; i < 13; ++i) q[i] = make_double2(v[2 * i], v[2 * i + 1]);
+  for (int i = 0; i < 7; ++i) st256(q + 4 * i, v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
 }
 __device__ __forceinline__ void load_jac(const double* mv_D, size_t t, Jac<double>& D) {
-  const double2* q = reinterpret_cast<const double2*>(mv_D + t * MVD);
-  double v[26];
+  const double* q = mv_D + t * MVD;
+  double v[28];
 #pragma unroll
-  for (int i = 0; i < 13; ++i) { const double2 a = q[i]; v[2 * i] = a.x; v[2 * i + 1] = a.y; }
+  for (int i = 0; i < 7; ++i) ld256(q + 4 * i, v[4 * i], v[4 * i + 1], v[4 * i + 2], v[4 * i + 3]);
 #pragma unroll
   for (int i = 0; i < 3; ++i) {
 #pragma unroll

@@ -46,10 +46,9 @@ struct LayerRec {
   int32_t n_phi, n_z, offset, kind, next_disc, pad;
 };
 
-// a2 field store: uniform, or the float32 grid [ix][iy][iz] widened ONCE to float64 and padded to 4 doubles
-// per node (one 32-byte sector).  The widening is exact, so the trilinear read returns the same float64 value
-// as widening at read time; it removes 24 float->double conversions per read from the RKN4 trial loop, whose
-// bottleneck on B200 is the conversion/special-function (XU) pipe (profiles/r01c).
+// a2 field store: uniform, or the float32 grid [ix][iy][iz] stored as (node, z-neighbour) pairs of 8 float32 (one
+// 32-byte sector, one 256-bit load: ld_pair below) and widened to float64 in registers; the widening is exact, so the
+// trilinear read returns the same float64 value as from a float64 copy of the grid.
 struct FieldDev {
   int32_t kind;
   int32_t n[3];

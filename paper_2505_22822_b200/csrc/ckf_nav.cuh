@@ -50,6 +50,46 @@ CKF_HD double line_test_module(const ModuleRec& k, const double r[3], const doub
 #endif
 }
 
+// The same test on a record held as 16 doubles in ModuleRec order (c, u, v, n, half_u, half_v, ..), and the loader that
+// fills it with four 256-bit loads on the device.
+CKF_HD void ld_module_rec(const ModuleRec* k, double rec[16]) {
+#if defined(__CUDA_ARCH__)
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+    asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];"
+        : "=d"(rec[4 * i]), "=d"(rec[4 * i + 1]), "=d"(rec[4 * i + 2]), "=d"(rec[4 * i + 3])
+        : "l"((const double*)k + 4 * i));
+#else
+  const double* q = (const double*)k;
+  for (int i = 0; i < 16; ++i) rec[i] = q[i];
+#endif
+}
+// A module record in registers: the fields the per-tip code uses, filled by four 256-bit loads.
+struct ModuleLite {
+  double c[3], u[3], v[3], n[3], half_u, half_v, xx0;
+};
+CKF_HD void load_module(const ModuleRec* k, ModuleLite& o) {
+  double rec[16];
+  ld_module_rec(k, rec);
+#pragma unroll
+  for (int i = 0; i < 3; ++i) { o.c[i] = rec[i]; o.u[i] = rec[3 + i]; o.v[i] = rec[6 + i]; o.n[i] = rec[9 + i]; }
+  o.half_u = rec[12]; o.half_v = rec[13]; o.xx0 = rec[14];
+}
+CKF_HD double line_test_rec(const double rec[16], const double r[3], const double d[3], double s_min, int bidir = 0) {
+  const double *c = rec, *u = rec + 3, *v = rec + 6, *n = rec + 9;
+  const double half_u = rec[12], half_v = rec[13];
+  const double dn = dot3(d, n);
+  const double rel[3] = {c[0] - r[0], c[1] - r[1], c[2] - r[2]};
+  const double s = dot3(rel, n) / dn;
+  const double q[3] = {r[0] + s * d[0] - c[0], r[1] + s * d[1] - c[1], r[2] + s * d[2] - c[2]};
+  const bool ok = (bidir ? fabs(dn) > 1e-6 : dn > 1e-6) && fabs(dot3(q, u)) <= half_u && fabs(dot3(q, v)) <= half_v && s > s_min;
+#if defined(__CUDA_ARCH__)
+  return ok ? s : __longlong_as_double(0x7ff8000000000000LL);
+#else
+  return ok ? s : NAN;
+#endif
+}
+
 // Nearest in-bounds module of the 3x3 neighbourhood (phi wraps, z clamps) of (iphi, iz) on `layer`, one tip per
 // thread.  ckf_step evaluates the same nine tests cooperatively over a warp, see pick_warp.
 CKF_HD int pick_in_neighbourhood(const GeoDev& g, int layer, int iphi, int iz, int exclude, const double r[3],
@@ -64,7 +104,9 @@ CKF_HD int pick_in_neighbourhood(const GeoDev& g, int layer, int iphi, int iz, i
     const int jj = iz + (nb % 3 - 1);
     const int id = L.offset + ii * L.n_z + jj;
     const bool test = jj >= 0 && jj < L.n_z && id != exclude;   // a predicate, not a branch around the loads
-    sv[nb] = test ? line_test_module(g.mod[id], r, d, s_min, g.bidir) : 0.0;
+    double rec[16];   // the record as four 256-bit loads (see pick_warp); an untested neighbour reads a valid record
+    ld_module_rec(g.mod + (test ? id : L.offset), rec);
+    sv[nb] = test ? line_test_rec(rec, r, d, s_min, g.bidir) : 0.0;
     idv[nb] = test ? id : -1;
   }
   int best = -1;
@@ -105,9 +147,9 @@ CKF_HD double mean_dedx_silicon(double p, double M) {
 //   arr          : arrival module;  y : state on its plane;  B : field there
 // T = arithmetic type of the bound->bound block (float64 in the product), TD = type the running
 // transport Jacobian D was accumulated in (float32 in fp32 mode).
-template <typename T, typename TD>
+template <typename T, typename TD, typename MOD>
 CKF_HD void arrival_jacobian(const Jac<TD>& D, const double dep_u[3], const double dep_v[3], const T dep_d[3],
-                             const ModuleRec& arr, const Traj& y, const double Bd[3], double mass, T J[5][5],
+                             const MOD& arr, const Traj& y, const double Bd[3], double mass, T J[5][5],
                              const JacR<TD>* R = nullptr) {
   const double lam = KAPPA * y.qop;
   double kd[3];
@@ -344,7 +386,8 @@ CKF_HD int departure_state(const GeoDev& g, const CfgDev& cfg, int from, const d
   for (int i = 0; i < 6; ++i) ok = ok && isfinite(x[i]);
   ok = ok && (x[3] > 0.0 && x[3] < PI_D);
   if (!ok) return STOP_NUMERIC;
-  const ModuleRec& k = g.mod[from];
+  ModuleLite k;
+  load_module(g.mod + from, k);
   double sp, cp, st, ct;
   sincos(x[2], &sp, &cp);
   sincos(x[3], &st, &ct);
@@ -645,8 +688,9 @@ CKF_HD void move_step(M& m, const FieldDev& fld, const CfgDev& cfg, int& n_trial
 template <typename T>
 CKF_HD int move_arrive(const Move<T>& m, const double dep[NDEP], const GeoDev& g, const FieldDev& fld, const CfgDev& cfg,
                        double xp[6], double J[5][5], const JacR<T>* R = nullptr) {
-  const ModuleRec& k = g.mod[m.tgt];
-  const ModuleRec& m0 = g.mod[m.from];
+  ModuleLite k, m0;
+  load_module(g.mod + m.tgt, k);
+  load_module(g.mod + m.from, m0);
   double B[3];
   field_at(fld, m.y.r, B);
   arrival_jacobian<double, T>(m.D, m0.u, m0.v, dep, k, m.y, B, cfg.mass, J, R);

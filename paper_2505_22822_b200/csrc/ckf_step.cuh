@@ -14,11 +14,12 @@ namespace ckf {
 
 // scratch of one warp for the module choice
 struct PickSmem {
-  double* hit;     // [9][32] path length of each (tip, neighbour) test; NaN = no hit
+  double* hit;     // [32][9] path length of each (requester rank, neighbour) test; NaN = no hit
   double* rd;      // [6][32] position and direction of the requesting tips
-  int32_t* hid;    // [9][32] module id of each test
+  int32_t* hid;    // [32][9] module id of each test
   int32_t *rl, *ri, *rj, *rx, *list;  // [32] request: layer, iphi, iz, exclude | s_min sign; compacted lanes
-  static constexpr size_t BYTES = 8 * 9 * 32 + 8 * 6 * 32 + 4 * 9 * 32 + 4 * 5 * 32;
+  int32_t *rnp, *rnz, *rof;           // [32] the layer's n_phi, n_z, module offset (read once by the requesting lane)
+  static constexpr size_t BYTES = 8 * 9 * 32 + 8 * 6 * 32 + 4 * 9 * 32 + 4 * 8 * 32;
   __host__ __device__ static constexpr size_t bytes() { return BYTES; }
   __device__ void carve(unsigned char* raw) {
     unsigned char* p = raw;
@@ -30,6 +31,9 @@ struct PickSmem {
     rj = (int32_t*)p; p += 4 * 32;
     rx = (int32_t*)p; p += 4 * 32;
     list = (int32_t*)p; p += 4 * 32;
+    rnp = (int32_t*)p; p += 4 * 32;
+    rnz = (int32_t*)p; p += 4 * 32;
+    rof = (int32_t*)p; p += 4 * 32;
   }
 };
 
@@ -46,6 +50,7 @@ __device__ __forceinline__ void pick_warp(const GeoDev& geo, const PickSmem& ps,
   const unsigned breq = __ballot_sync(0xffffffffu, ok);
   if (ok) {
     ps.rl[lane] = q.layer; ps.ri[lane] = q.iphi; ps.rj[lane] = q.iz;
+    { const LayerRec* LR = geo.layer + q.layer; ps.rnp[lane] = LR->n_phi; ps.rnz[lane] = LR->n_z; ps.rof[lane] = LR->offset; }
     ps.rx[lane] = (q.exclude < 0 ? 0 : q.exclude + 1) * 2 + (q.s_min > 0.0 ? 1 : 0);
 #pragma unroll
     for (int i = 0; i < 3; ++i) { ps.rd[i * 32 + lane] = m.y.r[i]; ps.rd[(3 + i) * 32 + lane] = m.y.d[i]; }
@@ -57,25 +62,29 @@ __device__ __forceinline__ void pick_warp(const GeoDev& geo, const PickSmem& ps,
     const int pr = q0 + lane;
     if (pr < total) {
       const int t = ps.list[pr / 9], nb = pr % 9;
-      const LayerRec L = geo.layer[ps.rl[t]];
+      const int Ln_phi = ps.rnp[t], Ln_z = ps.rnz[t], Loffset = ps.rof[t];
       int ii = ps.ri[t] + (nb / 3 - 1);
-      ii = ii < 0 ? ii + L.n_phi : (ii >= L.n_phi ? ii - L.n_phi : ii);
+      ii = ii < 0 ? ii + Ln_phi : (ii >= Ln_phi ? ii - Ln_phi : ii);
       const int jj = ps.rj[t] + (nb % 3 - 1);
       const int rx = ps.rx[t];
       double sres = __longlong_as_double(0x7ff8000000000000LL);
       int id = -1;
-      if (jj >= 0 && jj < L.n_z) {
-        id = L.offset + ii * L.n_z + jj;
+      if (jj >= 0 && jj < Ln_z) {
+        id = Loffset + ii * Ln_z + jj;
         if (id != (rx >> 1) - 1) {
           const double r[3] = {ps.rd[0 * 32 + t], ps.rd[1 * 32 + t], ps.rd[2 * 32 + t]};
           const double d[3] = {ps.rd[3 * 32 + t], ps.rd[4 * 32 + t], ps.rd[5 * 32 + t]};
           // no early exits: the four groups of fields of the module record are loaded at once instead of one L2 round
           // trip per passed test (that chain was a quarter of this kernel's stall samples)
-          sres = line_test_module(geo.mod[id], r, d, (rx & 1) ? 1e-3 : -1e-3, geo.bidir);
+          // the record as four 256-bit loads (c, u, v, n, half_u, half_v = its first 112 bytes): what the L1 data pipe of
+          // this kernel counts is load instructions x scattered lanes, and the module tests were half of them
+          double rec[16];
+          ld_module_rec(geo.mod + id, rec);
+          sres = line_test_rec(rec, r, d, (rx & 1) ? 1e-3 : -1e-3, geo.bidir);
         }
       }
-      ps.hit[nb * 32 + t] = sres;
-      ps.hid[nb * 32 + t] = id;
+      ps.hit[pr] = sres;   // [requester rank][neighbour]: consecutive lanes, consecutive words (no bank conflicts)
+      ps.hid[pr] = id;
     }
   }
   __syncwarp();
@@ -83,10 +92,11 @@ __device__ __forceinline__ void pick_warp(const GeoDev& geo, const PickSmem& ps,
     int best = -1;
     double best_s = 0.0;
     if (ok) {
+      const int rank9 = 9 * __popc(breq & ((1u << lane) - 1u));
 #pragma unroll 1
       for (int nb = 0; nb < 9; ++nb) {
-        const double sv = ps.hit[nb * 32 + lane];
-        const int id = ps.hid[nb * 32 + lane];
+        const double sv = ps.hit[rank9 + nb];
+        const int id = ps.hid[rank9 + nb];
         if (sv == sv && (best < 0 || sv < best_s || (sv == best_s && id < best))) { best = id; best_s = sv; }
       }
     }
