@@ -1118,3 +1118,13 @@ def test_graph_replay_of_a_repeated_find_same_result(monkeypatch):
             for k in want[which]:
                 assert got[k] == want[which][k], (which, r, k)
     ckf.close()
+
+
+def test_probe_module_reports_a_find():
+    """paper_2505_22822_b200.probe (the command the timing tables of profiles/ name): runs and reports consistent figures."""
+    from paper_2505_22822_b200 import probe
+    rep = probe.main(["--config", "1", "--particles", "300", "--fake-seeds", "50", "--calls", "3"])
+    assert rep["seeds"] == 350 and rep["candidates"] >= 300 and rep["launches_per_find"] > 100
+    assert 0.0 < rep["find_ms_min"] <= rep["find_ms_median"] < 50.0
+    assert rep["live_levels"] >= 10 and rep["rk_trials"] > rep["tips"] > rep["seeds"]
+    assert set(rep["per_kernel_ms_timing_mode"]) >= {"step_ms", "visit_ms", "scan_ms", "update_ms"}
