@@ -21,7 +21,9 @@
  *     n) never causes an out-of-bounds access: the seed stops, the slice is clamped, and CKF_STATUS_BAD_INPUT is set.
  *   - ckf_find is ASYNCHRONOUS on `cuda_stream` and never allocates: every workspace is reserved in
  *     ckf_create from the max_* capacities (PAPER.md:84, :102 blame in-pipeline allocation for the lack of
- *     stream scaling).  Capacity overflow is never silent: it sets a bit in *status.
+ *     stream scaling).  Capacity overflow is never silent: it sets a bit in *status.  (One opt-in exception: with
+ *     CKF_GRAPH=1 in the environment of ckf_create, a ckf_find that repeats the previous call's arguments is captured
+ *     into a CUDA graph and replayed from then on; capture and instantiation allocate inside the CUDA runtime.)
  *   - There is no CPU fallback: without a CUDA device ckf_create fails with CKF_E_CUDA.
  */
 #ifndef CKF_H_

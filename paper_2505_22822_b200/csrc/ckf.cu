@@ -127,7 +127,8 @@ struct ckf_handle {
   // 32 emission, 64 ckf_fit_level.  Measured (profiles/r02_launch_overlap.md): step + visit + update is best; with ckf_scan in the chain as
   // well the whole level loop is one cascade of waiting blocks and a batched find gets 10 % slower.  CKF_CHAIN_OVERLAP=<mask>
   // overrides (0 = plain launches), for A/B measurements.
-  bool use_graph = true;  // CKF_GRAPH=0: never replay a repeated find from a CUDA graph
+  bool use_graph = false;  // CKF_GRAPH=1: replay a find that repeats the previous call's arguments from a CUDA graph (opt-in:
+                           // capturing and instantiating the graph allocates, which ckf_find otherwise never does)
   bool grad = false;  // J2': config.field_gradient on an interpolated field (a uniform field has no gradient: the default kernels)
   int chain_overlap = 2 | 4 | 16 | 64;
   bool timing = false;  // ckf_set_timing / CKF_TIMING=1: per-kernel CUDA-event times of every ckf_find on stderr (debug aid; synchronises)
@@ -312,8 +313,8 @@ int launch_find(ckf_handle* h, Workspace& w, const ckf_measurements* m, const ck
     launch_chain(ckf_emit_tracks<T>, h->sm_count * 8, EMIT_NT, 0, q, ovm & 32, p); mark(8);
     launch_chain(ckf_finalize<T>, 1, 1, 0, q, ovm & 32, p); mark(9);
   };
-  // A find whose arguments repeat (same arrays, same sizes, same launch policy: the usual case of a pipeline that runs on
-  // preallocated buffers) is replayed from a CUDA graph of its ~136 launches: the second call in a row with the same
+  // Opt-in (CKF_GRAPH=1): a find whose arguments repeat (same arrays, same sizes, same launch policy: a pipeline that runs
+  // on preallocated, padded buffers) is replayed from a CUDA graph of its ~136 launches: the second call in a row with the same
   // arguments captures it, later ones launch it (configs[3] 3.29 -> 3.20 ms, configs[0] 0.92 -> 0.81 ms).  Anything else
   // -- new arguments, timing mode, a caller who is capturing the stream himself -- is enqueued launch by launch as before.
   bool done = false;
@@ -563,7 +564,7 @@ int ckf_create(const ckf_geometry* g, const ckf_field* f, const ckf_config* c, c
   }
   h->sm_count = prop.multiProcessorCount;
   { const char* t = getenv("CKF_TIMING"); h->timing = h->timing_print = t && t[0] == '1'; }
-  { const char* t = getenv("CKF_GRAPH"); if (t && t[0] == '0') h->use_graph = false; }
+  { const char* t = getenv("CKF_GRAPH"); h->use_graph = t && t[0] == '1'; }
   { const char* t = getenv("CKF_CHAIN_OVERLAP"); if (t && t[0]) h->chain_overlap = atoi(t); }
   h->n_modules = g->n_modules;
   h->n_layers = g->n_layers;

@@ -5,7 +5,7 @@ For a user who wants to know where the time of a find goes on their GPU: the med
 launch, so every launch carries a few microseconds of bracketing), and the work counters.  The tables of
 profiles/r02_launch_overlap.md and profiles/r02_latency_floor.md are printed by this module.  Environment switches read
 by ckf_create apply: CKF_CHAIN_OVERLAP=<mask> (which kernels are launched with programmatic stream serialisation),
-CKF_GRAPH=0 (no CUDA-graph replay of a repeated find).  Needs a CUDA device; inputs are synthetic (synth/)."""
+CKF_GRAPH=1 (replay a find that repeats the previous call's arguments from a CUDA graph).  Needs a CUDA device; inputs are synthetic (synth/)."""
 from __future__ import annotations
 
 import argparse
@@ -29,7 +29,7 @@ def main(argv=None):
     ap.add_argument("--calls", type=int, default=15, help="timed finds (median / min reported)")
     ap.add_argument("--alternate", action="store_true",
                     help="alternate between two events of different sizes, so that no call repeats the previous one's "
-                         "arguments (the launch-by-launch path; a repeated call is replayed from a CUDA graph)")
+                         "arguments (with CKF_GRAPH=1 a repeated call is replayed from a CUDA graph; this avoids it)")
     args = ap.parse_args(argv)
     import torch
     import synth

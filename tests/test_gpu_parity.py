@@ -1071,7 +1071,8 @@ def test_field_gradient_parity(precision):
 
 
 def test_graph_replay_of_a_repeated_find_same_result(monkeypatch):
-    """A find whose arguments repeat is replayed from a CUDA graph from the third call on (ckf.cu, launch_find).  Replays,
+    """With CKF_GRAPH=1 a find whose arguments repeat is replayed from a CUDA graph from the third call on (ckf.cu,
+    launch_find; opt-in because capture and instantiation allocate, which ckf_find otherwise never does).  Replays,
     the capture call and plain calls give byte-identical outputs; new arguments fall back to plain launches and a later
     return to the old arguments (captured again) is still right."""
     import torch
@@ -1098,7 +1099,7 @@ def test_graph_replay_of_a_repeated_find_same_result(monkeypatch):
         torch.cuda.synchronize()
         want.append(snapshot(out))
     plain.close()
-    monkeypatch.delenv("CKF_GRAPH")
+    monkeypatch.setenv("CKF_GRAPH", "1")
     ckf = CKF(det, fld, cfg.ckf, cfg.precision, max_seeds=ms, max_measurements=mm, max_fit_tracks=0)
     devs = [ckf.upload_event(ev) for ev in evs]
     out = ckf.alloc_tracks()
